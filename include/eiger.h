@@ -1,0 +1,155 @@
+/* eiger.h — C ABI of the B200-native adaptive GROUP BY library (libeiger.so).
+ *
+ * One hot path of Eiger (arxiv/paper_2607_04489): runtime-adaptive GROUP BY
+ * aggregation (SUM / COUNT / MIN / MAX over integer keys) whose kernel variant
+ * and hash-table size are chosen from statistics gathered on the key column at
+ * run time — an exact min/max range pass and a HyperLogLog NDV sketch
+ * (§1 "Runtime adaptive execution"; §4.1; PAPER.md:79
+ * §3.3; §4.3 for the range-first order).
+ *
+ * Conventions (all entry points):
+ *   - Columnar input, one contiguous region per column, 64-bit row counts
+ *     (§3.1).  No null masks (the paper never mentions any).
+ *   - Unless a parameter says HOST, data pointers are DEVICE pointers owned by
+ *     the caller and must be 16-byte aligned (any cudaMalloc / torch allocation
+ *     is).  The library never frees or keeps them.
+ *   - Work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream).  Host-visible outputs (eiger_stats, *n_groups,
+ *     *chosen) are valid when the call returns: the library synchronises the
+ *     stream where it has to read a statistic or a count back.
+ *   - Scratch memory comes from the caller's `workspace` (device memory, sized
+ *     by eiger_groupby_workspace_bytes).  The library itself holds one small
+ *     per-process device block (sketch registers, counters) and one pinned host
+ *     block, allocated on first use and released by eiger_shutdown().
+ *   - Every function returns 0 (EIGER_OK) or a negative eiger_status.  Nothing
+ *     throws, nothing aborts; there is no CPU fallback of any step.
+ */
+#ifndef EIGER_H_
+#define EIGER_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { EIGER_I8 = 0, EIGER_I32 = 1, EIGER_I64 = 2, EIGER_F64 = 3 } eiger_dtype;
+typedef enum { EIGER_SUM = 0, EIGER_COUNT = 1, EIGER_MIN = 2, EIGER_MAX = 3 } eiger_op;
+typedef enum {
+  EIGER_AUTO = 0,      /* profile, then pick one of the four below            */
+  EIGER_DIRECT = 1,    /* direct-index array, slot = key - min                */
+  EIGER_SMEM = 2,      /* per-CTA shared-memory open addressing, merged       */
+  EIGER_GLOBAL = 3,    /* one global open-addressing table (L2-resident)      */
+  EIGER_PARTITION = 4  /* radix partition by hash bits, then aggregate        */
+} eiger_variant;
+
+typedef enum {
+  EIGER_OK = 0,
+  EIGER_ERR_ARG = -1,          /* null pointer, bad dtype/op, n < 0, misaligned column      */
+  EIGER_ERR_WORKSPACE = -2,    /* workspace too small; see eiger_groupby_workspace_bytes     */
+  EIGER_ERR_OUT_CAPACITY = -3, /* more groups than out_capacity; *n_groups holds the count   */
+  EIGER_ERR_INFEASIBLE = -4,   /* the forced variant cannot run on this input                */
+  EIGER_ERR_CUDA = -5,         /* a CUDA runtime call failed; eiger_last_cuda_error() says   */
+  EIGER_ERR_TABLE_OVERFLOW = -6 /* NDV estimate too low and no room in workspace to retry   */
+} eiger_status;
+
+typedef struct { const void* data; int32_t dtype; int32_t reserved; } eiger_col; /* length n */
+typedef struct { int32_t op; int32_t val_col; } eiger_agg;   /* COUNT ignores val_col        */
+
+/* HOST struct.  n = 0 gives min = INT64_MAX, max = INT64_MIN, ndv_est = 0. */
+typedef struct { int64_t min, max; double ndv_est; int64_t n; } eiger_stats;
+
+/* eiger_profile — statistics of one integer key column in a single fused pass
+ * (steps A1-A3 of DESIGN.md): exact min and max, and the
+ * HyperLogLog estimate of the number of distinct values (p = 14, hash = splitmix64
+ * output function of the sign-extended key, table-free estimator; R1-R5),
+ * clamped to [0, min(n, max - min + 1)].
+ *   keys  DEVICE, n elements of `dtype` (EIGER_I8 / I32 / I64)
+ *   out   HOST
+ * Errors: EIGER_ERR_ARG, EIGER_ERR_CUDA. */
+int eiger_profile(const void* keys, int32_t dtype, int64_t n, eiger_stats* out, void* stream);
+
+/* eiger_hll_registers — test hook: the raw sketch registers of a key column.
+ *   regs_out  DEVICE, 16384 bytes, register j in byte j (values 0 .. 51).
+ * The register array is an exact function of the key set (R3). */
+int eiger_hll_registers(const void* keys, int32_t dtype, int64_t n, uint8_t* regs_out, void* stream);
+
+/* eiger_hll_estimate_host — step A3 alone: estimate from 16384 HOST registers. */
+double eiger_hll_estimate_host(const uint8_t* regs);
+
+/* eiger_groupby — GROUP BY keys, aggregating value columns (steps A0, A4-A7;
+ * PAPER.md:79 §3.3, §4.1, PAPER.md:184 retrieveAll).
+ *   keys[n_key_cols]   1 or 2 integer key columns (EIGER_I8 / I32 / I64).  Two columns are
+ *                      fused into one key by frame-of-reference + positional packing
+ *                      (§4.3) and un-fused on output.
+ *   vals[n_vals]       value columns, EIGER_I64 or EIGER_F64, n_vals <= 8
+ *   aggs[n_aggs]       n_aggs <= 8; result type: SUM/MIN/MAX of I64 -> int64 (SUM wraps modulo
+ *                      2^64), of F64 -> double; COUNT -> int64 row count
+ *   stats              HOST, n_key_cols entries from eiger_profile, or NULL: the library then
+ *                      profiles inside this call (that is what EIGER_AUTO timing includes)
+ *   out_keys[k]        DEVICE array of out_capacity elements of key column k's dtype
+ *   out_aggs[j]        DEVICE array of out_capacity 8-byte elements
+ *   n_groups           HOST; number of groups written (order of groups unspecified)
+ *   force              EIGER_AUTO or a variant to run regardless of the statistics
+ *   chosen             HOST, may be NULL; the variant that ran
+ *   workspace          DEVICE scratch of workspace_bytes
+ * Errors: EIGER_ERR_ARG; EIGER_ERR_WORKSPACE; EIGER_ERR_OUT_CAPACITY (a safe capacity is
+ * min(n, range)); EIGER_ERR_INFEASIBLE (e.g. EIGER_DIRECT on a 2^40 range);
+ * EIGER_ERR_TABLE_OVERFLOW (the sketch under-estimated and the workspace has no room for the
+ * larger table: call again with stats->ndv_est raised, e.g. to min(n, range)); EIGER_ERR_CUDA.
+ * fp64 MIN/MAX order -0.0 below +0.0; NaN inputs are not supported. */
+int eiger_groupby(const eiger_col* keys, int32_t n_key_cols, int64_t n,
+                  const eiger_col* vals, int32_t n_vals,
+                  const eiger_agg* aggs, int32_t n_aggs,
+                  const eiger_stats* stats,
+                  void* const* out_keys, void* const* out_aggs, int64_t out_capacity,
+                  int64_t* n_groups, int32_t force, int32_t* chosen,
+                  void* workspace, size_t workspace_bytes, void* stream);
+
+/* Workspace needed by eiger_groupby for the same arguments (data pointers inside keys / vals
+ * are ignored and may be NULL).  stats may be NULL: worst case over the variants `force`
+ * allows, with the group count bounded by n only.  Returns 0 on bad arguments. */
+size_t eiger_groupby_workspace_bytes(const eiger_col* keys, int32_t n_key_cols, int64_t n,
+                                     const eiger_col* vals, int32_t n_vals,
+                                     const eiger_agg* aggs, int32_t n_aggs,
+                                     const eiger_stats* stats, int32_t force);
+
+/* The variant EIGER_AUTO picks for these statistics (step A4), without running anything;
+ * negative eiger_status on bad arguments. */
+int32_t eiger_select_variant(const eiger_col* keys, int32_t n_key_cols, int64_t n,
+                             const eiger_col* vals, int32_t n_vals,
+                             const eiger_agg* aggs, int32_t n_aggs, const eiger_stats* stats);
+
+/* eiger_groupby_host — the same operation end to end from HOST buffers (pinned or pageable):
+ * copies the columns to the device, profiles, aggregates and copies the groups back.
+ * keys/vals/out_keys/out_aggs are HOST pointers here.  Device memory comes from a library
+ * arena that grows on demand and is kept between calls (eiger_shutdown releases it).
+ * h2d_bytes / d2h_bytes (HOST, may be NULL) receive the bytes copied in each direction. */
+int eiger_groupby_host(const eiger_col* keys, int32_t n_key_cols, int64_t n,
+                       const eiger_col* vals, int32_t n_vals,
+                       const eiger_agg* aggs, int32_t n_aggs,
+                       void* const* out_keys, void* const* out_aggs, int64_t out_capacity,
+                       int64_t* n_groups, int32_t force, int32_t* chosen,
+                       int64_t* h2d_bytes, int64_t* d2h_bytes, void* stream);
+
+/* Number of kernels this library has launched in this process (bench.py's gpu_launches). */
+int64_t eiger_launch_count(void);
+
+/* Per-kernel device time, measured with CUDA events on the caller's stream inside the calls
+ * above while enabled (eiger_set_kernel_timing(1)); off by default.  `which`: 0 = aggregation
+ * kernel (the dominant one), 1 = profile kernel, 2 = partition kernels, 3 = table init,
+ * 4 = compaction.  Returns the milliseconds accumulated since the last call with reset != 0;
+ * *launches (may be NULL) receives how many launches that covers. */
+void eiger_set_kernel_timing(int32_t enabled);
+double eiger_kernel_time_ms(int32_t which, int32_t reset, int64_t* launches);
+
+const char* eiger_strerror(int code);
+const char* eiger_last_cuda_error(void);
+const char* eiger_variant_name(int32_t variant);
+void eiger_shutdown(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EIGER_H_ */

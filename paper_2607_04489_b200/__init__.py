@@ -1,0 +1,341 @@
+"""paper_2607_04489_b200 — thin Python binding of libeiger.so (include/eiger.h).
+
+Argument marshalling only: every step of the path (profile, select, init, aggregate,
+partition, compact) runs inside the C-ABI library's CUDA kernels.  PyTorch is used for
+device memory and streams.  There is no CPU fallback: if the library is missing or
+was not built for this GPU the import of the first symbol raises.
+
+    import paper_2607_04489_b200 as eiger
+    st  = eiger.profile(keys)                                   # eiger_profile
+    res = eiger.groupby([keys], [vals], [(eiger.SUM, 0), (eiger.COUNT, 0)])
+    res.keys[0], res.aggs[0], res.n_groups, res.variant
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libeiger.so")
+
+I8, I32, I64, F64 = 0, 1, 2, 3
+SUM, COUNT, MIN, MAX = 0, 1, 2, 3
+AUTO, DIRECT, SMEM, GLOBAL, PARTITION = 0, 1, 2, 3, 4
+VARIANT_NAMES = {AUTO: "auto", DIRECT: "direct", SMEM: "smem", GLOBAL: "global", PARTITION: "partition"}
+OK, ERR_ARG, ERR_WORKSPACE, ERR_OUT_CAPACITY, ERR_INFEASIBLE, ERR_CUDA, ERR_TABLE_OVERFLOW = 0, -1, -2, -3, -4, -5, -6
+HLL_M = 1 << 14
+
+# every symbol include/eiger.h declares (tests check the library exports each of them)
+EXPORTS = [
+    "eiger_profile", "eiger_hll_registers", "eiger_hll_estimate_host", "eiger_groupby",
+    "eiger_groupby_workspace_bytes", "eiger_select_variant", "eiger_groupby_host",
+    "eiger_launch_count", "eiger_set_kernel_timing", "eiger_kernel_time_ms", "eiger_strerror",
+    "eiger_last_cuda_error", "eiger_variant_name", "eiger_shutdown",
+]
+
+_DTYPES = {torch.int8: I8, torch.int32: I32, torch.int64: I64, torch.float64: F64}
+
+
+class EigerError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"eiger error {code}: {msg}")
+        self.code = code
+
+
+class _Col(ctypes.Structure):
+    _fields_ = [("data", ctypes.c_void_p), ("dtype", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
+class _Agg(ctypes.Structure):
+    _fields_ = [("op", ctypes.c_int32), ("val_col", ctypes.c_int32)]
+
+
+class _Stats(ctypes.Structure):
+    _fields_ = [("min", ctypes.c_int64), ("max", ctypes.c_int64), ("ndv_est", ctypes.c_double), ("n", ctypes.c_int64)]
+
+
+@dataclass
+class Stats:
+    min: int
+    max: int
+    ndv_est: float
+    n: int
+
+
+@dataclass
+class GroupByResult:
+    keys: list          # one tensor per key column (key dtype), n_groups long, order unspecified
+    aggs: list          # one tensor per aggregate (int64 or float64)
+    n_groups: int
+    variant: int
+
+    def sorted(self) -> "GroupByResult":
+        """Groups ordered by key (for comparisons)."""
+        if self.n_groups == 0:
+            return self
+        order = torch.arange(self.n_groups, device=self.keys[0].device)
+        for k in reversed(self.keys):
+            order = order[torch.sort(k[order], stable=True).indices]
+        return GroupByResult([k[order] for k in self.keys], [a[order] for a in self.aggs], self.n_groups, self.variant)
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """The loaded C-ABI library; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError(f"{_LIB_PATH} is missing: run `python -m paper_2607_04489_b200.build` "
+                              "(or __graft_entry__.build()); there is no CPU fallback")
+        L = ctypes.CDLL(_LIB_PATH)
+        vp, i32, i64, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_size_t
+        L.eiger_profile.restype = ctypes.c_int
+        L.eiger_profile.argtypes = [vp, i32, i64, ctypes.POINTER(_Stats), vp]
+        L.eiger_hll_registers.restype = ctypes.c_int
+        L.eiger_hll_registers.argtypes = [vp, i32, i64, vp, vp]
+        L.eiger_hll_estimate_host.restype = ctypes.c_double
+        L.eiger_hll_estimate_host.argtypes = [vp]
+        L.eiger_groupby.restype = ctypes.c_int
+        L.eiger_groupby.argtypes = [vp, i32, i64, vp, i32, vp, i32, vp, vp, vp, i64,
+                                    ctypes.POINTER(i64), i32, ctypes.POINTER(i32), vp, sz, vp]
+        L.eiger_groupby_workspace_bytes.restype = sz
+        L.eiger_groupby_workspace_bytes.argtypes = [vp, i32, i64, vp, i32, vp, i32, vp, i32]
+        L.eiger_select_variant.restype = i32
+        L.eiger_select_variant.argtypes = [vp, i32, i64, vp, i32, vp, i32, vp]
+        L.eiger_groupby_host.restype = ctypes.c_int
+        L.eiger_groupby_host.argtypes = [vp, i32, i64, vp, i32, vp, i32, vp, vp, i64,
+                                         ctypes.POINTER(i64), i32, ctypes.POINTER(i32),
+                                         ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
+        L.eiger_launch_count.restype = i64
+        L.eiger_set_kernel_timing.argtypes = [i32]
+        L.eiger_kernel_time_ms.restype = ctypes.c_double
+        L.eiger_kernel_time_ms.argtypes = [i32, i32, ctypes.POINTER(i64)]
+        L.eiger_strerror.restype = ctypes.c_char_p
+        L.eiger_strerror.argtypes = [ctypes.c_int]
+        L.eiger_last_cuda_error.restype = ctypes.c_char_p
+        L.eiger_variant_name.restype = ctypes.c_char_p
+        L.eiger_variant_name.argtypes = [i32]
+        L.eiger_shutdown.restype = None
+        _lib = L
+    return _lib
+
+
+def _check(code: int):
+    if code != OK:
+        L = lib()
+        msg = L.eiger_strerror(code).decode()
+        if code == ERR_CUDA:
+            msg += " — " + L.eiger_last_cuda_error().decode()
+        raise EigerError(code, msg)
+
+
+def _stream(device) -> int:
+    return torch.cuda.current_stream(device).cuda_stream
+
+
+def _cols(tensors, allowed) -> ctypes.Array:
+    arr = (_Col * max(1, len(tensors)))()
+    for i, t in enumerate(tensors):
+        if t.dtype not in allowed:
+            raise TypeError(f"unsupported column dtype {t.dtype}")
+        if not t.is_contiguous():
+            raise ValueError("columns must be contiguous")
+        arr[i].data = t.data_ptr() if t.numel() else None
+        arr[i].dtype = _DTYPES[t.dtype]
+    return arr
+
+
+def _aggs(aggs) -> ctypes.Array:
+    arr = (_Agg * max(1, len(aggs)))()
+    for i, (op, col) in enumerate(aggs):
+        arr[i].op, arr[i].val_col = int(op), int(col)
+    return arr
+
+
+def _stats_arr(stats):
+    if stats is None:
+        return None
+    arr = (_Stats * len(stats))()
+    for i, s in enumerate(stats):
+        arr[i].min, arr[i].max, arr[i].ndv_est, arr[i].n = s.min, s.max, s.ndv_est, s.n
+    return arr
+
+
+_KEY_T = (torch.int8, torch.int32, torch.int64)
+_VAL_T = (torch.int64, torch.float64)
+
+
+def profile(keys: torch.Tensor) -> Stats:
+    """eiger_profile: exact min/max and the HyperLogLog NDV estimate of a device key column."""
+    if not keys.is_cuda:
+        raise ValueError("keys must be a CUDA tensor")
+    s = _Stats()
+    with torch.cuda.device(keys.device):
+        _check(lib().eiger_profile(_cols([keys], _KEY_T)[0].data, _DTYPES[keys.dtype], keys.numel(),
+                                   ctypes.byref(s), _stream(keys.device)))
+    return Stats(s.min, s.max, s.ndv_est, s.n)
+
+
+def hll_registers(keys: torch.Tensor) -> torch.Tensor:
+    """eiger_hll_registers: the 16384 sketch registers (uint8, device)."""
+    out = torch.empty(HLL_M, dtype=torch.uint8, device=keys.device)
+    with torch.cuda.device(keys.device):
+        _check(lib().eiger_hll_registers(_cols([keys], _KEY_T)[0].data, _DTYPES[keys.dtype], keys.numel(),
+                                         out.data_ptr(), _stream(keys.device)))
+    return out
+
+
+def hll_estimate(regs) -> float:
+    """eiger_hll_estimate_host on 16384 host registers."""
+    r = torch.as_tensor(regs, dtype=torch.uint8).cpu().contiguous()
+    assert r.numel() == HLL_M
+    return float(lib().eiger_hll_estimate_host(r.data_ptr()))
+
+
+def select_variant(keys, vals, aggs, stats) -> int:
+    n = keys[0].numel()
+    v = lib().eiger_select_variant(_cols(keys, _KEY_T), len(keys), n, _cols(vals, _VAL_T), len(vals),
+                                   _aggs(aggs), len(aggs), _stats_arr(stats))
+    if v < 0:
+        _check(v)
+    return v
+
+
+def workspace_bytes(keys, vals, aggs, stats=None, force: int = AUTO) -> int:
+    n = keys[0].numel()
+    return int(lib().eiger_groupby_workspace_bytes(_cols(keys, _KEY_T), len(keys), n, _cols(vals, _VAL_T), len(vals),
+                                                   _aggs(aggs), len(aggs), _stats_arr(stats), force))
+
+
+class Workspace:
+    """A reusable device scratch buffer (grown on demand) plus reusable output columns."""
+
+    def __init__(self, device):
+        self.device = device
+        self.buf = None
+        self.out = {}
+
+    def scratch(self, nbytes: int) -> torch.Tensor:
+        if self.buf is None or self.buf.numel() < nbytes:
+            self.buf = None
+            self.buf = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=self.device)
+        return self.buf
+
+    def column(self, name, n: int, dtype) -> torch.Tensor:
+        t = self.out.get(name)
+        if t is None or t.numel() < n or t.dtype != dtype:
+            t = torch.empty(max(n, 1), dtype=dtype, device=self.device)
+            self.out[name] = t
+        return t
+
+
+def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int | None = None,
+            workspace: Workspace | None = None) -> GroupByResult:
+    """eiger_groupby on device columns.
+
+    keys: 1-2 CUDA integer tensors; vals: CUDA int64/float64 tensors; aggs: [(op, val_col)].
+    With stats=None the key columns are profiled first (eiger_profile), which is what the
+    adaptive path's time includes; pass stats from profile() to skip that.
+    """
+    if isinstance(keys, torch.Tensor):
+        keys = [keys]
+    dev = keys[0].device
+    if not all(t.is_cuda for t in list(keys) + list(vals)):
+        raise ValueError("all columns must be CUDA tensors")
+    n = keys[0].numel()
+    if any(t.numel() != n for t in list(keys) + list(vals)):
+        raise ValueError("column length mismatch")
+    L = lib()
+    ws = workspace or Workspace(dev)
+    with torch.cuda.device(dev):
+        if stats is None and n > 0:
+            stats = [profile(k) for k in keys]
+        kc, vc, ac, sc = _cols(keys, _KEY_T), _cols(vals, _VAL_T), _aggs(aggs), _stats_arr(stats)
+        for attempt in range(3):
+            nbytes = int(L.eiger_groupby_workspace_bytes(kc, len(keys), n, vc, len(vals), ac, len(aggs), sc, force))
+            if nbytes == 0:
+                # bad arguments or an infeasible forced variant: let eiger_groupby say which
+                nbytes = 256
+            if out_capacity is None:
+                cap = n
+                if stats:
+                    rng = 1
+                    for s in stats:
+                        rng *= (s.max - s.min + 1)
+                    cap = max(0, min(n, rng))
+                    if force in (AUTO, SMEM, GLOBAL, PARTITION) and stats and len(stats) == 1:
+                        cap = min(cap, int(stats[0].ndv_est * 1.25) + 1024)
+            else:
+                cap = out_capacity
+            buf = ws.scratch(nbytes)
+            ok = [ws.column(("k", i), cap, k.dtype) for i, k in enumerate(keys)]
+            oa = [ws.column(("a", j), cap, torch.float64 if (op != COUNT and vals[c].dtype == torch.float64) else torch.int64)
+                  for j, (op, c) in enumerate(aggs)]
+            okp = (ctypes.c_void_p * 2)(*[t.data_ptr() for t in ok])
+            oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
+            ng, chosen = ctypes.c_int64(0), ctypes.c_int32(0)
+            rc = L.eiger_groupby(kc, len(keys), n, vc, len(vals), ac, len(aggs), sc, okp, oap, cap,
+                                 ctypes.byref(ng), force, ctypes.byref(chosen), buf.data_ptr(), buf.numel(), _stream(dev))
+            if rc == ERR_OUT_CAPACITY and out_capacity is None:
+                out_capacity = int(ng.value)
+                continue
+            if rc == ERR_TABLE_OVERFLOW and stats is not None and attempt < 2:
+                # the sketch under-estimated: size for the exact bound and run again
+                stats = [Stats(s.min, s.max, float(min(n, s.max - s.min + 1)), s.n) for s in stats]
+                sc = _stats_arr(stats)
+                out_capacity = None
+                continue
+            _check(rc)
+            g = int(ng.value)
+            return GroupByResult([t[:g] for t in ok], [t[:g] for t in oa], g, int(chosen.value))
+    raise EigerError(ERR_TABLE_OVERFLOW, "could not size the table")
+
+
+def groupby_host(keys, vals, aggs, force: int = AUTO, out_capacity: int | None = None, out=None):
+    """eiger_groupby_host: host tensors (ideally pinned) in, host tensors out; the H2D / D2H
+    copies happen inside the library call.  Returns (GroupByResult on host, h2d_bytes, d2h_bytes)."""
+    if isinstance(keys, torch.Tensor):
+        keys = [keys]
+    if any(t.is_cuda for t in list(keys) + list(vals)):
+        raise ValueError("groupby_host takes host tensors")
+    n = keys[0].numel()
+    L = lib()
+    cap = n if out_capacity is None else out_capacity
+    if out is None:
+        ok = [torch.empty(max(cap, 1), dtype=k.dtype).pin_memory() for k in keys]
+        oa = [torch.empty(max(cap, 1), dtype=torch.float64 if (op != COUNT and vals[c].dtype == torch.float64) else torch.int64).pin_memory()
+              for (op, c) in aggs]
+    else:
+        ok, oa = out
+    okp = (ctypes.c_void_p * 2)(*[t.data_ptr() for t in ok])
+    oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
+    ng, chosen, h2d, d2h = ctypes.c_int64(0), ctypes.c_int32(0), ctypes.c_int64(0), ctypes.c_int64(0)
+    rc = L.eiger_groupby_host(_cols(keys, _KEY_T), len(keys), n, _cols(vals, _VAL_T), len(vals), _aggs(aggs), len(aggs),
+                              okp, oap, cap, ctypes.byref(ng), force, ctypes.byref(chosen),
+                              ctypes.byref(h2d), ctypes.byref(d2h), _stream(torch.device("cuda", torch.cuda.current_device())))
+    _check(rc)
+    g = int(ng.value)
+    return GroupByResult([t[:g] for t in ok], [t[:g] for t in oa], g, int(chosen.value)), int(h2d.value), int(d2h.value)
+
+
+def launch_count() -> int:
+    return int(lib().eiger_launch_count())
+
+
+def set_kernel_timing(enabled: bool) -> None:
+    lib().eiger_set_kernel_timing(1 if enabled else 0)
+
+
+def kernel_time_ms(which: int = 0, reset: bool = True):
+    n = ctypes.c_int64(0)
+    ms = lib().eiger_kernel_time_ms(which, 1 if reset else 0, ctypes.byref(n))
+    return float(ms), int(n.value)
+
+
+def shutdown() -> None:
+    lib().eiger_shutdown()

@@ -1,0 +1,621 @@
+// The C ABI of libeiger (include/eiger.h): runtime state, step A4 (select + size) and the
+// host-side orchestration of profile -> init -> aggregate -> compact.
+#include <algorithm>
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <mutex>
+
+#include "internal.h"
+
+namespace eiger {
+
+namespace {
+std::mutex g_mu;
+Runtime g_rt;
+std::atomic<int64_t> g_launches{0};
+char g_cuda_err[512] = "";
+bool g_timing = false;
+constexpr int kTimeSlots = 5;
+double g_time_ms[kTimeSlots] = {0, 0, 0, 0, 0};
+int64_t g_time_n[kTimeSlots] = {0, 0, 0, 0, 0};
+
+// event pairs recorded during one call, resolved after the call's final synchronise
+struct Pending { cudaEvent_t a, b; int slot; };
+Pending g_pending[16];
+int g_n_pending = 0;
+cudaEvent_t g_pool[32];
+int g_pool_n = 0, g_pool_used = 0;
+
+cudaEvent_t take_event() {
+  if (g_pool_used == g_pool_n) {
+    if (g_pool_n == 32) return nullptr;
+    if (cudaEventCreate(&g_pool[g_pool_n]) != cudaSuccess) return nullptr;
+    ++g_pool_n;
+  }
+  return g_pool[g_pool_used++];
+}
+struct Timed {
+  cudaStream_t s; int slot; cudaEvent_t a = nullptr, b = nullptr;
+  Timed(cudaStream_t st, int sl) : s(st), slot(sl) {
+    if (g_timing && g_n_pending < 16) { a = take_event(); b = take_event(); if (a && b) cudaEventRecord(a, s); }
+  }
+  ~Timed() {
+    if (a && b) { cudaEventRecord(b, s); g_pending[g_n_pending++] = Pending{a, b, slot}; }
+  }
+};
+void resolve_timing() {
+  for (int i = 0; i < g_n_pending; ++i) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, g_pending[i].a, g_pending[i].b) == cudaSuccess) {
+      g_time_ms[g_pending[i].slot] += ms; g_time_n[g_pending[i].slot] += 1;
+    }
+  }
+  g_n_pending = 0; g_pool_used = 0;
+}
+
+constexpr double kSigma = 0.008125;             // 1.04 / sqrt(2^14)
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline bool is_key_dtype(int d) { return d == EIGER_I8 || d == EIGER_I32 || d == EIGER_I64; }
+inline int dtype_size(int d) { return d == EIGER_I8 ? 1 : d == EIGER_I32 ? 4 : 8; }
+
+// Tunables of step A4; EIGER_* environment variables override them
+// for the crossover sweeps.
+struct Tunables {
+  size_t priv_smem = 96 * 1024;       // FRONT_PRIV: private cells of one CTA
+  size_t sdirect_bytes = 160 * 1024;  // FRONT_SDIRECT: largest per-CTA direct array
+  size_t sdirect_replica_budget = 64 * 1024;
+  size_t shash_bytes = 96 * 1024;     // FRONT_SHASH table per CTA
+  size_t direct_l2_bytes = 48ull << 20;   // AUTO takes DIRECT/global-atomics up to this table size
+  size_t global_l2_bytes = 64ull << 20;   // AUTO takes GLOBAL up to this table size
+  size_t part_target_bytes = 24ull << 20; // PARTITION: table slice per partition
+  double load = 0.5;
+  int global_front = 1;               // hot-key cache in front of the global table
+  Tunables() {
+    auto env = [](const char* k, double dflt) { const char* v = std::getenv(k); return v ? std::atof(v) : dflt; };
+    direct_l2_bytes = (size_t)env("EIGER_DIRECT_L2_MB", 48) << 20;
+    global_l2_bytes = (size_t)env("EIGER_GLOBAL_L2_MB", 64) << 20;
+    part_target_bytes = (size_t)env("EIGER_PART_MB", 24) << 20;
+    global_front = (int)env("EIGER_GLOBAL_FRONT", 1);
+    load = env("EIGER_LOAD", 0.5);
+  }
+};
+const Tunables& tun() { static Tunables t; return t; }
+
+struct QueryPlan {
+  int variant = 0, key_kind = 0, sig = 0, front = 0, back = 0;
+  KeyDesc key{};
+  AggPlan plan{};
+  int n_user_aggs = 0;
+  int val_src[kMaxVals];        // plan value slot -> caller's value column
+  uint64_t R = 0;               // fused key range; 0 = 2^64 (or not representable)
+  double ndv = 0;
+  uint32_t front_slots = 0, front_limit = 0, front_replicas = 1;
+  size_t smem_bytes = 0;
+  uint64_t cap = 0, cap_bound = 0;
+  uint32_t stride = 0;
+  int part_bits = 0;
+  size_t table_bytes = 0, part_bytes = 0, total_bytes = 0;
+};
+
+uint64_t range_of(const eiger_stats& s) {   // max - min + 1, 0 when it is 2^64
+  return (uint64_t)s.max - (uint64_t)s.min + 1ull;
+}
+uint32_t floor_pow2(uint64_t x) { uint32_t p = 1; while ((uint64_t)p * 2 <= x && p < (1u << 30)) p *= 2; return p; }
+
+int detect_sig(const AggPlan& p, int n_user) {
+  auto is = [&](int j, int op, int col, int f) { return p.op[j] == op && (op == EIGER_COUNT || (p.col[j] == col && p.f64[j] == f)); };
+  if (p.n_acc != n_user) return SIG_GENERIC;
+  if (n_user == 2 && is(0, EIGER_SUM, 0, 0) && is(1, EIGER_COUNT, 0, 0)) return SIG_SC;
+  if (n_user == 4 && is(1, EIGER_COUNT, 0, 0)) {
+    if (is(0, EIGER_SUM, 0, 0) && is(2, EIGER_MIN, 0, 0) && is(3, EIGER_MAX, 0, 0)) return SIG_A4I;
+    if (is(0, EIGER_SUM, 0, 1) && is(2, EIGER_MIN, 0, 1) && is(3, EIGER_MAX, 0, 1)) return SIG_A4F;
+  }
+  if (n_user == 5 && p.n_vals == 4 && is(0, EIGER_SUM, 0, 0) && is(1, EIGER_SUM, 1, 0) && is(2, EIGER_SUM, 2, 0) &&
+      is(3, EIGER_SUM, 3, 0) && is(4, EIGER_COUNT, 0, 0)) return SIG_S4C;
+  return SIG_GENERIC;
+}
+
+// Step A4: choose the variant and size everything (readings R8-R10).
+int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eiger_col* vals, int nv,
+               const eiger_agg* aggs, int na, const eiger_stats* st, int force, QueryPlan* q) {
+  if (!keys || nk < 1 || nk > 2 || n < 0 || nv < 0 || nv > kMaxVals || na < 1 || na > kMaxAggs || !aggs) return EIGER_ERR_ARG;
+  if (nv > 0 && !vals) return EIGER_ERR_ARG;
+  if (force < EIGER_AUTO || force > EIGER_PARTITION) return EIGER_ERR_ARG;
+  for (int k = 0; k < nk; ++k) if (!is_key_dtype(keys[k].dtype)) return EIGER_ERR_ARG;
+  for (int c = 0; c < nv; ++c) if (vals[c].dtype != EIGER_I64 && vals[c].dtype != EIGER_F64) return EIGER_ERR_ARG;
+
+  // aggregates -> accumulator plan over the value columns that are actually used
+  AggPlan& p = q->plan;
+  std::memset(&p, 0, sizeof(p));
+  int slot_of[kMaxVals];
+  for (int c = 0; c < kMaxVals; ++c) slot_of[c] = -1;
+  bool has_count = false;
+  p.cnt_acc = -1;
+  for (int j = 0; j < na; ++j) {
+    const int op = aggs[j].op;
+    if (op < EIGER_SUM || op > EIGER_MAX) return EIGER_ERR_ARG;
+    p.op[j] = (uint8_t)op;
+    if (op == EIGER_COUNT) { if (!has_count) p.cnt_acc = j; has_count = true; continue; }
+    const int c = aggs[j].val_col;
+    if (c < 0 || c >= nv) return EIGER_ERR_ARG;
+    if (slot_of[c] < 0) { slot_of[c] = p.n_vals; q->val_src[p.n_vals] = c; p.vals[p.n_vals] = vals[c].data; ++p.n_vals; }
+    p.col[j] = (uint8_t)slot_of[c];
+    p.f64[j] = vals[c].dtype == EIGER_F64;
+  }
+  p.n_acc = na;
+  q->n_user_aggs = na;
+
+  // keys: ranges and fusion (A0)
+  KeyDesc& kd = q->key;
+  std::memset(&kd, 0, sizeof(kd));
+  kd.ncols = nk; kd.mul = 1;
+  bool have_stats = st != nullptr;
+  uint64_t Rk[2] = {0, 0};
+  for (int k = 0; k < nk; ++k) {
+    kd.ptr[k] = keys[k].data; kd.dtype[k] = keys[k].dtype;
+    if (have_stats) { kd.base[k] = (uint64_t)st[k].min; Rk[k] = n > 0 ? range_of(st[k]) : 1; }
+    else {  // bound by the type
+      const int bits = 8 * dtype_size(keys[k].dtype);
+      kd.base[k] = bits == 64 ? (uint64_t)INT64_MIN : (uint64_t)(-(1ll << (bits - 1)));
+      Rk[k] = bits == 64 ? 0 : (1ull << bits);
+    }
+  }
+  uint64_t R = Rk[0];
+  if (nk == 2) {
+    if (Rk[0] == 0 || Rk[1] == 0) return EIGER_ERR_INFEASIBLE;
+    const unsigned __int128 prod = (unsigned __int128)Rk[0] * Rk[1];
+    if (prod >> 64) return EIGER_ERR_INFEASIBLE;   // fused key must fit 64 bits
+    R = (uint64_t)prod; kd.mul = Rk[1];
+  }
+  q->R = R;
+  // group-count bound and estimate
+  double bound = (double)n;
+  if (R != 0) bound = std::min(bound, (double)R);
+  double ndv = bound;
+  if (have_stats) {
+    double e = st[0].ndv_est;
+    if (nk == 2) e *= st[1].ndv_est;
+    ndv = std::min(bound, std::max(e, 1.0));
+  }
+  q->ndv = ndv;
+  q->cap_bound = (uint64_t)std::max(1.0, std::ceil(bound / tun().load)) + 64;
+
+  const Tunables& T = tun();
+  const int n_acc_direct = na + (has_count ? 0 : 1);
+  const bool direct_ok = R != 0 && R <= (1ull << 33);
+  const unsigned __int128 direct_bytes = (unsigned __int128)R * 8 * n_acc_direct;
+
+  // FRONT_SHASH geometry
+  const int key_kind_hash = (nk == 1 && keys[0].dtype == EIGER_I32 && R != 0 && R <= 0xFFFFFFFFull) ? KK_I32
+                            : (nk == 1 && keys[0].dtype == EIGER_I64) ? KK_I64 : KK_GEN;
+  const size_t ubytes = key_kind_hash == KK_I32 ? 4 : 8;
+  const size_t shash_slot = 8 * (size_t)na + ubytes;
+  const uint32_t shash_slots = floor_pow2(T.shash_bytes / shash_slot);
+  const uint32_t hash_stride = [&] { uint32_t s = 16; while (s < 8u * (1 + na)) s *= 2; return s; }();
+  auto hash_cap = [&](double g) { return (uint64_t)std::max(1024.0, std::ceil(g * (1.0 + 4 * kSigma) * 1.02 / T.load)); };
+
+  int variant = force;
+  if (variant == EIGER_AUTO) {
+    if (direct_ok && (direct_bytes * 256 <= T.priv_smem || direct_bytes <= T.sdirect_bytes ||
+                      (direct_bytes <= T.direct_l2_bytes && (double)R <= 16.0 * (double)std::max<int64_t>(n, 1)))) variant = EIGER_DIRECT;
+    else if (ndv * (1.0 + 4 * kSigma) <= 0.5 * shash_slots) variant = EIGER_SMEM;
+    else if ((unsigned __int128)hash_cap(ndv) * hash_stride <= T.global_l2_bytes) variant = EIGER_GLOBAL;
+    else variant = EIGER_PARTITION;
+  }
+  q->variant = variant;
+
+  if (variant == EIGER_DIRECT) {
+    if (!direct_ok) return EIGER_ERR_INFEASIBLE;
+    if (!has_count) { p.op[na] = EIGER_COUNT; p.cnt_acc = na; p.n_acc = na + 1; }
+    q->back = BACK_DIRECT;
+    q->key_kind = (nk == 1 && keys[0].dtype == EIGER_I32 && R <= 0xFFFFFFFFull) ? KK_I32
+                  : (nk == 1 && keys[0].dtype == EIGER_I64) ? KK_I64
+                  : (nk == 2 && keys[0].dtype == EIGER_I8 && keys[1].dtype == EIGER_I8) ? KK_I8I8 : KK_GEN;
+    q->cap = R; q->stride = 8u * p.n_acc;
+    q->table_bytes = align_up((size_t)R * q->stride, 256);
+    if (direct_bytes * 256 <= T.priv_smem) {
+      q->front = FRONT_PRIV; q->front_slots = (uint32_t)R; q->smem_bytes = (size_t)direct_bytes * 256;
+    } else if (direct_bytes <= T.sdirect_bytes) {
+      q->front = FRONT_SDIRECT; q->front_slots = (uint32_t)R;
+      q->front_replicas = (uint32_t)std::max<size_t>(1, std::min<size_t>(8, T.sdirect_replica_budget / (size_t)direct_bytes));
+      q->smem_bytes = (size_t)direct_bytes * q->front_replicas;
+    } else {
+      q->front = FRONT_NONE;
+    }
+  } else {
+    q->back = BACK_HASH;
+    q->stride = hash_stride;
+    q->cap = std::min(hash_cap(ndv), q->cap_bound);
+    q->key_kind = key_kind_hash;
+    const bool want_front = variant == EIGER_SMEM || ((variant == EIGER_GLOBAL || variant == EIGER_PARTITION) && T.global_front);
+    if (variant == EIGER_PARTITION) {
+      q->key_kind = KK_U64PRE;
+      const double tb = (double)q->cap * q->stride;
+      int bits = 1;
+      while (bits < 12 && tb / (double)(1u << bits) > (double)T.part_target_bytes) ++bits;
+      q->part_bits = bits;
+      const size_t P = (size_t)1 << bits;
+      q->part_bytes = align_up(P * 4, 256) + align_up(P * 8, 256) + (size_t)(1 + p.n_vals) * align_up((size_t)n * 8, 256);
+    }
+    if (want_front) {
+      const size_t ub = q->key_kind == KK_I32 ? 4 : 8;
+      q->front = FRONT_SHASH;
+      q->front_slots = floor_pow2(T.shash_bytes / (8 * (size_t)na + ub));
+      q->front_limit = q->front_slots / 2;
+      q->smem_bytes = align_up((size_t)q->front_slots * (8 * (size_t)na + ub) + 16, 16);
+    } else {
+      q->front = FRONT_NONE;
+    }
+    q->table_bytes = align_up((size_t)(q->cap + 1) * q->stride, 256);
+  }
+  q->sig = detect_sig(p, na);
+  if (!aggregate_supported(q->key_kind, q->sig, q->front, q->back)) return EIGER_ERR_INFEASIBLE;
+  q->total_bytes = q->table_bytes + q->part_bytes + 256;
+  (void)rt;
+  return EIGER_OK;
+}
+
+int do_profile(Runtime* rt, const void* keys, int dtype, int64_t n, int with_hll, eiger_stats* out, cudaStream_t s) {
+  {
+    Timed t(s, 1);
+    int rc = launch_profile(rt, keys, dtype, n, 0, with_hll, true, s);
+    if (rc) return rc;
+  }
+  if (with_hll) { int rc = launch_hll_hist(rt, s); if (rc) return rc; }
+  struct Back { long long mn, mx; uint32_t hist[64]; };
+  Back* b = static_cast<Back*>(rt->pinned);
+  EIGER_CUDA(cudaMemcpyAsync(&b->mn, &rt->prof->min[0], 8, cudaMemcpyDeviceToHost, s));
+  EIGER_CUDA(cudaMemcpyAsync(&b->mx, &rt->prof->max[0], 8, cudaMemcpyDeviceToHost, s));
+  if (with_hll) EIGER_CUDA(cudaMemcpyAsync(b->hist, rt->prof->hist, sizeof(b->hist), cudaMemcpyDeviceToHost, s));
+  EIGER_CUDA(cudaStreamSynchronize(s));
+  resolve_timing();
+  out->min = b->mn; out->max = b->mx; out->n = n;
+  if (n == 0) { out->ndv_est = 0.0; return EIGER_OK; }
+  const double range = (double)((uint64_t)b->mx - (uint64_t)b->mn) + 1.0;
+  double est = with_hll ? hll_estimate_from_hist(b->hist) : range;   // range-first: R bounds NDV
+  est = std::min(est, std::min((double)n, range));
+  out->ndv_est = std::max(est, 0.0);
+  return EIGER_OK;
+}
+
+int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eiger_col* vals, int nv,
+                const eiger_agg* aggs, int na, const eiger_stats* stats_in,
+                void* const* out_keys, void* const* out_aggs, int64_t out_capacity,
+                int64_t* n_groups, int force, int32_t* chosen, void* workspace, size_t workspace_bytes,
+                cudaStream_t s) {
+  if (!n_groups || !out_keys || !out_aggs || out_capacity < 0) return EIGER_ERR_ARG;
+  *n_groups = 0;
+  if (!keys || nk < 1 || nk > 2 || n < 0) return EIGER_ERR_ARG;
+  for (int k = 0; k < nk; ++k) {
+    if (!is_key_dtype(keys[k].dtype)) return EIGER_ERR_ARG;
+    if (n > 0 && (!keys[k].data || ((uintptr_t)keys[k].data & 15))) return EIGER_ERR_ARG;
+    if (!out_keys[k] && out_capacity > 0) return EIGER_ERR_ARG;
+  }
+  for (int c = 0; c < nv; ++c) if (n > 0 && vals && (!vals[c].data || ((uintptr_t)vals[c].data & 15))) return EIGER_ERR_ARG;
+  eiger_stats local[2];
+  const eiger_stats* st = stats_in;
+  if (!st && n > 0) {
+    // profile inside the call: fused min/max + sketch for 4/8-byte keys; 1-byte keys take the
+    // range test only (HLL only when the range test fails; a 1-byte range never does)
+    for (int k = 0; k < nk; ++k) {
+      int rc = do_profile(rt, keys[k].data, keys[k].dtype, n, keys[k].dtype != EIGER_I8, &local[k], s);
+      if (rc) return rc;
+    }
+    st = local;
+  }
+  QueryPlan q;
+  int rc = plan_query(rt, keys, nk, n, vals, nv, aggs, na, st, force, &q);
+  if (rc) return rc;
+  if (chosen) *chosen = q.variant;
+  if (n == 0) return EIGER_OK;
+  if (q.total_bytes > workspace_bytes || !workspace) return EIGER_ERR_WORKSPACE;
+  if ((uintptr_t)workspace & 255) return EIGER_ERR_ARG;
+
+  char* ws = static_cast<char*>(workspace);
+  struct Back { unsigned long long n_groups; uint32_t overflow; uint32_t pad; };
+  Back* hb = reinterpret_cast<Back*>(static_cast<char*>(rt->pinned) + 1024);
+
+  for (int attempt = 0;; ++attempt) {
+    // workspace: [table][partition scratch]
+    void* table = ws;
+    char* pws = ws + q.table_bytes;
+    EIGER_CUDA(cudaMemsetAsync(rt->call, 0, sizeof(CallDev), s));
+    AggLaunch L{};
+    L.key = q.key; L.plan = q.plan; L.n = n;
+    L.key_kind = q.key_kind; L.sig = q.sig; L.front = q.front; L.back = q.back;
+    L.front_slots = q.front_slots; L.front_limit = q.front_limit; L.front_replicas = q.front_replicas;
+    L.table = table; L.cap = q.cap; L.stride = q.stride; L.call = rt->call;
+    L.threads = 256; L.smem_bytes = q.smem_bytes;
+    { Timed t(s, 3); rc = launch_table_init(L, s); if (rc) return rc; }
+
+    if (q.variant == EIGER_PARTITION) {
+      PartitionLaunch P{};
+      P.key = q.key; P.plan = q.plan; P.n = n; P.bits = q.part_bits;
+      P.key_kind = (nk == 1 && keys[0].dtype == EIGER_I32 && q.R != 0 && q.R <= 0xFFFFFFFFull) ? KK_I32
+                   : (nk == 1 && keys[0].dtype == EIGER_I64) ? KK_I64 : KK_GEN;
+      const size_t np = (size_t)1 << q.part_bits;
+      P.hist = reinterpret_cast<uint32_t*>(pws); pws += align_up(np * 4, 256);
+      P.cursor = reinterpret_cast<unsigned long long*>(pws); pws += align_up(np * 8, 256);
+      P.out_u = reinterpret_cast<uint64_t*>(pws); pws += align_up((size_t)n * 8, 256);
+      for (int c = 0; c < q.plan.n_vals; ++c) { P.out_vals[c] = reinterpret_cast<uint64_t*>(pws); pws += align_up((size_t)n * 8, 256); }
+      { Timed t(s, 2); rc = launch_partition(P, rt->sm_count, s); if (rc) return rc; }
+      // the aggregation pass reads the partitioned copy
+      L.key.ptr[0] = P.out_u; L.key.ncols = 1; L.key.base[0] = 0; L.key.mul = 1;
+      for (int c = 0; c < q.plan.n_vals; ++c) L.plan.vals[c] = P.out_vals[c];
+    }
+
+    // persistent grid: as many CTAs as fit, never more than there are tiles
+    int occ = 1;
+    {
+      const size_t per_cta = std::max<size_t>(q.smem_bytes, 1024);
+      occ = (int)std::min<size_t>(8, std::max<size_t>(1, (rt->smem_optin + 1024) / (per_cta + 1024)));
+      if (q.front == FRONT_NONE) occ = 8;
+    }
+    const int64_t tiles = std::max<int64_t>(1, (n + 1023) / 1024);
+    L.blocks = (int)std::min<int64_t>((int64_t)rt->sm_count * occ, tiles);
+    { Timed t(s, 0); rc = launch_aggregate(L, s); if (rc) return rc; }
+
+    CompactLaunch C{};
+    C.key = q.key; C.plan = q.plan; C.back = q.back; C.table = table; C.cap = q.cap; C.stride = q.stride;
+    C.out_keys[0] = out_keys[0]; C.out_keys[1] = nk == 2 ? out_keys[1] : nullptr;
+    for (int j = 0; j < na; ++j) { if (!out_aggs[j] && out_capacity > 0) return EIGER_ERR_ARG; C.out_aggs[j] = out_aggs[j]; }
+    C.n_out_aggs = na; C.out_capacity = out_capacity; C.call = rt->call;
+    { Timed t(s, 4); rc = launch_compact(C, rt->sm_count, s); if (rc) return rc; }
+
+    EIGER_CUDA(cudaMemcpyAsync(hb, rt->call, sizeof(Back), cudaMemcpyDeviceToHost, s));
+    EIGER_CUDA(cudaStreamSynchronize(s));
+    resolve_timing();
+    if (hb->overflow) {
+      // the sketch under-estimated (R10): grow towards the exact bound and run again
+      if (q.back != BACK_HASH || q.cap >= q.cap_bound || attempt >= 8) return EIGER_ERR_TABLE_OVERFLOW;
+      q.cap = std::min(q.cap_bound, q.cap * 4);
+      const size_t old_total = q.total_bytes;
+      q.table_bytes = align_up((size_t)(q.cap + 1) * q.stride, 256);
+      q.total_bytes = q.table_bytes + q.part_bytes + 256;
+      if (q.total_bytes > workspace_bytes) { (void)old_total; return EIGER_ERR_TABLE_OVERFLOW; }
+      continue;
+    }
+    *n_groups = (int64_t)hb->n_groups;
+    if ((int64_t)hb->n_groups > out_capacity) return EIGER_ERR_OUT_CAPACITY;
+    return EIGER_OK;
+  }
+}
+
+// ---- device arena for eiger_groupby_host ---------------------------------------------------
+struct Arena { char* base = nullptr; size_t size = 0; } g_arena;
+int arena_reserve(size_t bytes) {
+  if (bytes <= g_arena.size) return EIGER_OK;
+  if (g_arena.base) { cudaFree(g_arena.base); g_arena.base = nullptr; g_arena.size = 0; }
+  EIGER_CUDA(cudaMalloc(reinterpret_cast<void**>(&g_arena.base), bytes));
+  g_arena.size = bytes;
+  return EIGER_OK;
+}
+
+}  // namespace
+
+void count_launch(int k) { g_launches.fetch_add(k, std::memory_order_relaxed); }
+
+int cuda_fail(cudaError_t e, const char* what) {
+  std::snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
+  cudaGetLastError();
+  return EIGER_ERR_CUDA;
+}
+
+Runtime* runtime() {
+  if (g_rt.device >= 0) return &g_rt;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cuda_fail(cudaGetLastError(), "cudaGetDevice"); return nullptr; }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { cuda_fail(cudaGetLastError(), "cudaGetDeviceProperties"); return nullptr; }
+  g_rt.sm_count = prop.multiProcessorCount;
+  g_rt.smem_optin = prop.sharedMemPerBlockOptin;
+  g_rt.l2_bytes = (size_t)prop.l2CacheSize;
+  if (cudaMalloc(reinterpret_cast<void**>(&g_rt.prof), sizeof(ProfileDev)) != cudaSuccess ||
+      cudaMalloc(reinterpret_cast<void**>(&g_rt.call), sizeof(CallDev)) != cudaSuccess ||
+      cudaMallocHost(&g_rt.pinned, 64 * 1024) != cudaSuccess) {
+    cuda_fail(cudaGetLastError(), "runtime allocation");
+    return nullptr;
+  }
+  g_rt.device = dev;
+  return &g_rt;
+}
+
+}  // namespace eiger
+
+using namespace eiger;
+
+extern "C" {
+
+int eiger_profile(const void* keys, int32_t dtype, int64_t n, eiger_stats* out, void* stream) {
+  if (!out || n < 0 || !is_key_dtype(dtype) || (n > 0 && (!keys || ((uintptr_t)keys & 15)))) return EIGER_ERR_ARG;
+  std::lock_guard<std::mutex> lk(g_mu);
+  Runtime* rt = runtime();
+  if (!rt) return EIGER_ERR_CUDA;
+  return do_profile(rt, keys, dtype, n, 1, out, static_cast<cudaStream_t>(stream));
+}
+
+int eiger_hll_registers(const void* keys, int32_t dtype, int64_t n, uint8_t* regs_out, void* stream) {
+  if (!regs_out || n < 0 || !is_key_dtype(dtype) || (n > 0 && (!keys || ((uintptr_t)keys & 15)))) return EIGER_ERR_ARG;
+  std::lock_guard<std::mutex> lk(g_mu);
+  Runtime* rt = runtime();
+  if (!rt) return EIGER_ERR_CUDA;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  int rc = launch_profile(rt, keys, dtype, n, 0, 1, true, s);
+  if (rc) return rc;
+  rc = launch_regs_to_bytes(rt, regs_out, s);
+  if (rc) return rc;
+  EIGER_CUDA(cudaStreamSynchronize(s));
+  return EIGER_OK;
+}
+
+double eiger_hll_estimate_host(const uint8_t* regs) {
+  if (!regs) return -1.0;
+  uint32_t hist[64] = {0};
+  for (int i = 0; i < kHllM; ++i) hist[regs[i] & 63] += 1;
+  return hll_estimate_from_hist(hist);
+}
+
+int eiger_groupby(const eiger_col* keys, int32_t n_key_cols, int64_t n, const eiger_col* vals, int32_t n_vals,
+                  const eiger_agg* aggs, int32_t n_aggs, const eiger_stats* stats,
+                  void* const* out_keys, void* const* out_aggs, int64_t out_capacity,
+                  int64_t* n_groups, int32_t force, int32_t* chosen,
+                  void* workspace, size_t workspace_bytes, void* stream) {
+  std::lock_guard<std::mutex> lk(g_mu);
+  Runtime* rt = runtime();
+  if (!rt) return EIGER_ERR_CUDA;
+  return run_groupby(rt, keys, n_key_cols, n, vals, n_vals, aggs, n_aggs, stats, out_keys, out_aggs, out_capacity,
+                     n_groups, force, chosen, workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
+}
+
+size_t eiger_groupby_workspace_bytes(const eiger_col* keys, int32_t n_key_cols, int64_t n,
+                                     const eiger_col* vals, int32_t n_vals, const eiger_agg* aggs, int32_t n_aggs,
+                                     const eiger_stats* stats, int32_t force) {
+  size_t worst = 0;
+  const int lo = (force == EIGER_AUTO && !stats) ? EIGER_DIRECT : force;
+  const int hi = (force == EIGER_AUTO && !stats) ? EIGER_PARTITION : force;
+  bool any = false;
+  for (int v = lo; v <= hi; ++v) {
+    QueryPlan q;
+    const int rc = plan_query(nullptr, keys, n_key_cols, n, vals, n_vals, aggs, n_aggs, stats, v, &q);
+    if (rc == EIGER_OK) { worst = std::max(worst, q.total_bytes); any = true; }
+    else if (rc != EIGER_ERR_INFEASIBLE) return 0;
+  }
+  return any ? std::max<size_t>(worst, 256) : 0;
+}
+
+int32_t eiger_select_variant(const eiger_col* keys, int32_t n_key_cols, int64_t n, const eiger_col* vals, int32_t n_vals,
+                             const eiger_agg* aggs, int32_t n_aggs, const eiger_stats* stats) {
+  QueryPlan q;
+  const int rc = plan_query(nullptr, keys, n_key_cols, n, vals, n_vals, aggs, n_aggs, stats, EIGER_AUTO, &q);
+  return rc ? rc : q.variant;
+}
+
+int eiger_groupby_host(const eiger_col* keys, int32_t nk, int64_t n, const eiger_col* vals, int32_t nv,
+                       const eiger_agg* aggs, int32_t na, void* const* out_keys, void* const* out_aggs,
+                       int64_t out_capacity, int64_t* n_groups, int32_t force, int32_t* chosen,
+                       int64_t* h2d_bytes, int64_t* d2h_bytes, void* stream) {
+  if (!keys || nk < 1 || nk > 2 || n < 0 || nv < 0 || nv > kMaxVals || !aggs || na < 1 || na > kMaxAggs ||
+      !n_groups || !out_keys || !out_aggs || out_capacity < 0) return EIGER_ERR_ARG;
+  std::lock_guard<std::mutex> lk(g_mu);
+  Runtime* rt = runtime();
+  if (!rt) return EIGER_ERR_CUDA;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  for (int k = 0; k < nk; ++k) if (!is_key_dtype(keys[k].dtype) || (n > 0 && !keys[k].data)) return EIGER_ERR_ARG;
+  for (int c = 0; c < nv; ++c) if ((vals[c].dtype != EIGER_I64 && vals[c].dtype != EIGER_F64) || (n > 0 && !vals[c].data)) return EIGER_ERR_ARG;
+
+  // arena layout: input columns | output columns | workspace (sized after the profile)
+  size_t in_bytes = 0, out_bytes = 0;
+  for (int k = 0; k < nk; ++k) { in_bytes += align_up((size_t)n * dtype_size(keys[k].dtype), 256); out_bytes += align_up((size_t)out_capacity * dtype_size(keys[k].dtype), 256); }
+  in_bytes += (size_t)nv * align_up((size_t)n * 8, 256);
+  out_bytes += (size_t)na * align_up((size_t)out_capacity * 8, 256);
+  // first reservation covers the columns; the workspace is added once the statistics are known
+  int rc = arena_reserve(std::max<size_t>(g_arena.size, in_bytes + out_bytes + ((size_t)64 << 20)));
+  if (rc) return rc;
+  int64_t h2d = 0, d2h = 0;
+  auto stage = [&](char*& cur, eiger_col* dk, eiger_col* dv) -> int {
+    for (int k = 0; k < nk; ++k) {
+      const size_t b = (size_t)n * dtype_size(keys[k].dtype);
+      dk[k].data = cur; dk[k].dtype = keys[k].dtype; dk[k].reserved = 0;
+      if (b) EIGER_CUDA(cudaMemcpyAsync(cur, keys[k].data, b, cudaMemcpyHostToDevice, s));
+      h2d += (int64_t)b; cur += align_up(b, 256);
+    }
+    for (int c = 0; c < nv; ++c) {
+      const size_t b = (size_t)n * 8;
+      dv[c].data = cur; dv[c].dtype = vals[c].dtype; dv[c].reserved = 0;
+      if (b) EIGER_CUDA(cudaMemcpyAsync(cur, vals[c].data, b, cudaMemcpyHostToDevice, s));
+      h2d += (int64_t)b; cur += align_up(b, 256);
+    }
+    return EIGER_OK;
+  };
+  eiger_col dk[2], dv[kMaxVals];
+  char* cur = g_arena.base;
+  rc = stage(cur, dk, dv);
+  if (rc) return rc;
+  eiger_stats st[2];
+  for (int k = 0; k < nk; ++k) {
+    rc = do_profile(rt, dk[k].data, dk[k].dtype, n, dk[k].dtype != EIGER_I8, &st[k], s);
+    if (rc) return rc;
+  }
+  QueryPlan q;
+  rc = plan_query(rt, dk, nk, n, dv, nv, aggs, na, st, force, &q);
+  if (rc) return rc;
+  const size_t need = in_bytes + out_bytes + q.total_bytes + 512;
+  if (need > g_arena.size) {
+    // grow: the staged columns are lost with the old arena, copy them again
+    rc = arena_reserve(need + need / 8);
+    if (rc) return rc;
+    cur = g_arena.base; h2d = 0;
+    rc = stage(cur, dk, dv);
+    if (rc) return rc;
+  }
+  void* dok[2] = {nullptr, nullptr};
+  void* doa[kMaxAggs] = {nullptr};
+  for (int k = 0; k < nk; ++k) { dok[k] = cur; cur += align_up((size_t)out_capacity * dtype_size(keys[k].dtype), 256); }
+  for (int j = 0; j < na; ++j) { doa[j] = cur; cur += align_up((size_t)out_capacity * 8, 256); }
+  char* wsp = reinterpret_cast<char*>(align_up((uintptr_t)cur, 256));
+  const size_t ws_bytes = g_arena.size - (size_t)(wsp - g_arena.base);
+  rc = run_groupby(rt, dk, nk, n, dv, nv, aggs, na, st, dok, doa, out_capacity, n_groups, force, chosen, wsp, ws_bytes, s);
+  if (rc) return rc;
+  const int64_t g = *n_groups;
+  for (int k = 0; k < nk; ++k) {
+    const size_t b = (size_t)g * dtype_size(keys[k].dtype);
+    if (b) EIGER_CUDA(cudaMemcpyAsync(out_keys[k], dok[k], b, cudaMemcpyDeviceToHost, s));
+    d2h += (int64_t)b;
+  }
+  for (int j = 0; j < na; ++j) {
+    if (g) EIGER_CUDA(cudaMemcpyAsync(out_aggs[j], doa[j], (size_t)g * 8, cudaMemcpyDeviceToHost, s));
+    d2h += g * 8;
+  }
+  EIGER_CUDA(cudaStreamSynchronize(s));
+  if (h2d_bytes) *h2d_bytes = h2d;
+  if (d2h_bytes) *d2h_bytes = d2h;
+  return EIGER_OK;
+}
+
+int64_t eiger_launch_count(void) { return g_launches.load(); }
+
+void eiger_set_kernel_timing(int32_t enabled) { std::lock_guard<std::mutex> lk(g_mu); g_timing = enabled != 0; }
+
+double eiger_kernel_time_ms(int32_t which, int32_t reset, int64_t* launches) {
+  std::lock_guard<std::mutex> lk(g_mu);
+  if (which < 0 || which >= kTimeSlots) return -1.0;
+  const double ms = g_time_ms[which];
+  if (launches) *launches = g_time_n[which];
+  if (reset) { g_time_ms[which] = 0; g_time_n[which] = 0; }
+  return ms;
+}
+
+const char* eiger_strerror(int code) {
+  switch (code) {
+    case EIGER_OK: return "ok";
+    case EIGER_ERR_ARG: return "bad argument (null pointer, bad dtype/op, negative size or misaligned column)";
+    case EIGER_ERR_WORKSPACE: return "workspace too small (see eiger_groupby_workspace_bytes)";
+    case EIGER_ERR_OUT_CAPACITY: return "more groups than out_capacity";
+    case EIGER_ERR_INFEASIBLE: return "the forced variant cannot run on this input";
+    case EIGER_ERR_CUDA: return "CUDA runtime error (see eiger_last_cuda_error)";
+    case EIGER_ERR_TABLE_OVERFLOW: return "hash table overflow: NDV under-estimated and no workspace to retry";
+    default: return "unknown error";
+  }
+}
+const char* eiger_last_cuda_error(void) { return g_cuda_err; }
+const char* eiger_variant_name(int32_t v) {
+  switch (v) {
+    case EIGER_AUTO: return "auto"; case EIGER_DIRECT: return "direct"; case EIGER_SMEM: return "smem";
+    case EIGER_GLOBAL: return "global"; case EIGER_PARTITION: return "partition"; default: return "?";
+  }
+}
+void eiger_shutdown(void) {
+  std::lock_guard<std::mutex> lk(g_mu);
+  if (g_arena.base) { cudaFree(g_arena.base); g_arena = Arena{}; }
+  if (g_rt.device >= 0) {
+    cudaFree(g_rt.prof); cudaFree(g_rt.call); cudaFreeHost(g_rt.pinned);
+    for (int i = 0; i < g_pool_n; ++i) cudaEventDestroy(g_pool[i]);
+    g_pool_n = 0; g_pool_used = 0;
+    g_rt = Runtime{};
+  }
+}
+
+}  // extern "C"

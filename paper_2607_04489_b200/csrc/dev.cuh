@@ -1,0 +1,187 @@
+// Device-side building blocks shared by the kernels of libeiger (sm_100a).
+// Nothing here is shared with oracle/: the sketch hash and the estimator are
+// restated independently on each side.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "../../include/eiger.h"
+
+namespace eiger {
+
+constexpr int kMaxAggs = 8;            // user aggregates per call
+constexpr int kMaxAcc = 9;             // + one hidden COUNT for the direct table's presence test
+constexpr int kMaxVals = 8;
+constexpr int kHllP = 14;              // DESIGN.md R1
+constexpr int kHllM = 1 << kHllP;
+constexpr int kHllQ = 64 - kHllP;      // rho in [1, kHllQ + 1]
+constexpr uint64_t kEmpty64 = ~0ull;
+constexpr uint32_t kEmpty32 = ~0u;
+
+// How the key column(s) are read.  u = rebased, fused key (frame of reference +
+// positional packing): u = (k0 - min0) * mul + (k1 - min1).
+enum KeyKind : int { KK_I32 = 0, KK_I64 = 1, KK_I8I8 = 2, KK_GEN = 3, KK_U64PRE = 4 };
+
+struct KeyDesc {
+  const void* ptr[2];
+  int32_t dtype[2];
+  int32_t ncols;
+  int32_t pad;
+  uint64_t base[2];   // min of each column, sign-extended, as two's complement bits
+  uint64_t mul;       // range of column 1 (1 for a single column)
+};
+
+// Aggregate signatures with compile-time plans (the shapes of BASELINE.json's configs);
+// everything else runs the generic, plan-driven path.
+enum SigKind : int {
+  SIG_GENERIC = 0,
+  SIG_SC = 1,    // SUM(int64 c0), COUNT                        (C4, C5)
+  SIG_A4I = 2,   // SUM, COUNT, MIN, MAX of int64 c0            (C1)
+  SIG_A4F = 3,   // SUM, COUNT, MIN, MAX of fp64  c0            (C3)
+  SIG_S4C = 4    // SUM(int64 c0..c3), COUNT                    (C2)
+};
+
+struct AggPlan {
+  const void* vals[kMaxVals];
+  int32_t n_vals;
+  int32_t n_acc;            // accumulators per group (user aggregates [+ hidden COUNT])
+  uint8_t op[12];
+  uint8_t f64[12];
+  uint8_t col[12];
+  int32_t cnt_acc;          // index of an accumulator that counts rows (presence test)
+};
+
+template <int SIG> struct Sig;
+template <> struct Sig<SIG_GENERIC> {
+  static constexpr bool kStatic = false;
+  static constexpr int kAcc = kMaxAcc, kVals = kMaxVals;
+  __device__ static constexpr int op(int) { return 0; }
+  __device__ static constexpr int col(int) { return 0; }
+  __device__ static constexpr bool f64(int) { return false; }
+};
+template <> struct Sig<SIG_SC> {
+  static constexpr bool kStatic = true;
+  static constexpr int kAcc = 2, kVals = 1;
+  __device__ static constexpr int op(int j) { return j == 0 ? EIGER_SUM : EIGER_COUNT; }
+  __device__ static constexpr int col(int) { return 0; }
+  __device__ static constexpr bool f64(int) { return false; }
+};
+template <> struct Sig<SIG_A4I> {
+  static constexpr bool kStatic = true;
+  static constexpr int kAcc = 4, kVals = 1;
+  __device__ static constexpr int op(int j) { return j; }
+  __device__ static constexpr int col(int) { return 0; }
+  __device__ static constexpr bool f64(int) { return false; }
+};
+template <> struct Sig<SIG_A4F> {
+  static constexpr bool kStatic = true;
+  static constexpr int kAcc = 4, kVals = 1;
+  __device__ static constexpr int op(int j) { return j; }
+  __device__ static constexpr int col(int) { return 0; }
+  __device__ static constexpr bool f64(int j) { return j != 1; }
+};
+template <> struct Sig<SIG_S4C> {
+  static constexpr bool kStatic = true;
+  static constexpr int kAcc = 5, kVals = 4;
+  __device__ static constexpr int op(int j) { return j < 4 ? EIGER_SUM : EIGER_COUNT; }
+  __device__ static constexpr int col(int j) { return j < 4 ? j : 0; }
+  __device__ static constexpr bool f64(int) { return false; }
+};
+
+// ---- streamed loads: read once, keep out of L1, first to leave L2 ----------------
+__device__ __forceinline__ uint4 ldg_stream_16(const void* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ uint2 ldg_stream_8(const void* p) {
+  uint2 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];"
+               : "=r"(r.x), "=r"(r.y) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ uint32_t ldg_stream_4(const void* p) {
+  uint32_t r;
+  asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(r) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ uint32_t ldg_stream_2(const void* p) {
+  uint16_t r;
+  asm volatile("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=h"(r) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ uint32_t ldg_stream_1(const void* p) {
+  uint32_t r;
+  asm volatile("ld.global.nc.L1::no_allocate.u8 %0, [%1];" : "=r"(r) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ uint64_t ldg_stream_u64(const void* p) {
+  uint64_t r;
+  asm volatile("ld.global.nc.L1::no_allocate.u64 %0, [%1];" : "=l"(r) : "l"(p));
+  return r;
+}
+
+__device__ __forceinline__ uint64_t sext_load(const void* base, int dtype, int64_t i) {
+  switch (dtype) {
+    case EIGER_I8: return (uint64_t)(int64_t)(int8_t)ldg_stream_1((const int8_t*)base + i);
+    case EIGER_I32: return (uint64_t)(int64_t)(int32_t)ldg_stream_4((const int32_t*)base + i);
+    default: return ldg_stream_u64((const int64_t*)base + i);
+  }
+}
+
+// ---- hashes ------------------------------------------------------------------------
+// Sketch hash (R2): splitmix64 output function of the sign-extended key.
+__device__ __forceinline__ uint64_t hll_hash64(uint64_t x) {
+  uint64_t z = x + 0x9E3779B97F4A7C15ull;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+// Table hashes: free choice, results do not depend on them (R11).
+__device__ __forceinline__ uint64_t table_hash64(uint64_t u) {
+  uint64_t h = (u ^ (u >> 32)) * 0x9FB21C651E98DF25ull;
+  h = (h ^ (h >> 29)) * 0xD6E8FEB86659FD93ull;
+  return h ^ (h >> 32);
+}
+__device__ __forceinline__ uint32_t table_hash32(uint32_t u) {
+  uint32_t h = u * 0x9E3779B1u;
+  h = (h ^ (h >> 15)) * 0x85EBCA77u;
+  return h ^ (h >> 13);
+}
+
+// ---- accumulator algebra -------------------------------------------------------------
+// fp64 MIN/MAX run on an order-preserving int64 image of the double (an involution).
+__device__ __forceinline__ int64_t f64_order(uint64_t bits) {
+  const int64_t b = (int64_t)bits;
+  return b ^ ((b >> 63) & 0x7FFFFFFFFFFFFFFFll);
+}
+__device__ __forceinline__ uint64_t acc_identity(int op) {
+  return op == EIGER_MIN ? (uint64_t)INT64_MAX : op == EIGER_MAX ? (uint64_t)INT64_MIN : 0ull;
+}
+// What one row contributes to accumulator (op, f64): the "partial" form that merges with
+// add (SUM, COUNT) or min/max on int64 (MIN, MAX; doubles in f64_order space).
+__device__ __forceinline__ uint64_t row_partial(int op, bool f64, uint64_t raw) {
+  if (op == EIGER_COUNT) return 1ull;
+  if (f64 && op != EIGER_SUM) return (uint64_t)f64_order(raw);
+  return raw;
+}
+__device__ __forceinline__ uint64_t combine(int op, bool f64, uint64_t a, uint64_t b) {
+  if (op == EIGER_SUM && f64) return (uint64_t)__double_as_longlong(__longlong_as_double((int64_t)a) + __longlong_as_double((int64_t)b));
+  if (op == EIGER_SUM || op == EIGER_COUNT) return a + b;
+  if (op == EIGER_MIN) return (uint64_t)min((int64_t)a, (int64_t)b);
+  return (uint64_t)max((int64_t)a, (int64_t)b);
+}
+// Atomic merge of a partial into an accumulator cell (shared or global address).
+__device__ __forceinline__ void atomic_merge(uint64_t* cell, int op, bool f64, uint64_t part) {
+  if (op == EIGER_SUM && f64) atomicAdd(reinterpret_cast<double*>(cell), __longlong_as_double((int64_t)part));
+  else if (op == EIGER_SUM || op == EIGER_COUNT) atomicAdd(reinterpret_cast<unsigned long long*>(cell), (unsigned long long)part);
+  else if (op == EIGER_MIN) atomicMin(reinterpret_cast<long long*>(cell), (long long)part);
+  else atomicMax(reinterpret_cast<long long*>(cell), (long long)part);
+}
+__device__ __forceinline__ uint64_t acc_finalize(int op, bool f64, uint64_t acc) {
+  if (f64 && (op == EIGER_MIN || op == EIGER_MAX)) return (uint64_t)f64_order(acc);
+  return acc;
+}
+
+}  // namespace eiger

@@ -1,0 +1,99 @@
+// Host-side declarations shared by the translation units of libeiger.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "dev.cuh"
+
+namespace eiger {
+
+// Device block owned by the library (allocated once): profile outputs and call counters.
+struct ProfileDev {
+  long long min[2];
+  long long max[2];
+  uint32_t regs[kHllM];     // sketch registers, one per word (global atomicMax)
+  uint32_t hist[64];        // register-value histogram C[0 .. kHllQ + 1]
+};
+struct CallDev {
+  unsigned long long n_groups;   // compaction claim counter
+  uint32_t overflow;             // a hash table ran out of probes
+  uint32_t pad;
+};
+
+struct Runtime {
+  int device = -1;
+  int sm_count = 0;
+  size_t smem_optin = 0;
+  size_t l2_bytes = 0;
+  ProfileDev* prof = nullptr;    // device
+  CallDev* call = nullptr;       // device
+  void* pinned = nullptr;        // host staging for small read-backs (64 KB)
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+};
+Runtime* runtime();              // lazily initialised for the current device; nullptr on failure
+void count_launch(int k = 1);
+int cuda_fail(cudaError_t e, const char* what);   // records the message, returns EIGER_ERR_CUDA
+#define EIGER_CUDA(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) return ::eiger::cuda_fail(e__, #expr); } while (0)
+
+// ---- profile.cu ------------------------------------------------------------------------
+// Fused min/max (+ sketch registers) over one key column into rt->prof, slot `which` of
+// min/max.  with_hll = 0 skips the sketch (range-first order).
+int launch_profile(Runtime* rt, const void* keys, int dtype, int64_t n, int which, int with_hll,
+                   bool reset, cudaStream_t s);
+int launch_hll_hist(Runtime* rt, cudaStream_t s);
+int launch_regs_to_bytes(Runtime* rt, uint8_t* out, cudaStream_t s);
+double hll_estimate_from_hist(const uint32_t* hist);
+
+// ---- aggregate.cu ----------------------------------------------------------------------
+enum FrontKind : int { FRONT_NONE = 0, FRONT_PRIV = 1, FRONT_SDIRECT = 2, FRONT_SHASH = 3 };
+enum BackKind : int { BACK_DIRECT = 0, BACK_HASH = 1 };
+
+struct AggLaunch {
+  KeyDesc key;
+  AggPlan plan;
+  int64_t n;
+  int key_kind, sig, front, back;
+  // front
+  uint32_t front_slots;     // SDIRECT: R; SHASH: power-of-two slot count; PRIV: R
+  uint32_t front_limit;     // SHASH: stop inserting new keys beyond this many
+  uint32_t front_replicas;  // SDIRECT: table copies per CTA
+  // back
+  void* table;              // DIRECT: [cap][n_acc] cells; HASH: [cap] slots of `stride` bytes
+  uint64_t cap;
+  uint32_t stride;          // HASH: bytes per slot (power of two); DIRECT: 8 * n_acc
+  CallDev* call;
+  // launch shape
+  int threads, blocks;
+  size_t smem_bytes;
+};
+int launch_table_init(const AggLaunch& a, cudaStream_t s);
+int launch_aggregate(const AggLaunch& a, cudaStream_t s);
+bool aggregate_supported(int key_kind, int sig, int front, int back);
+
+struct CompactLaunch {
+  KeyDesc key;              // for un-fusing / un-rebasing
+  AggPlan plan;
+  int back;
+  const void* table; uint64_t cap; uint32_t stride;
+  void* out_keys[2]; void* out_aggs[kMaxAggs]; int n_out_aggs;
+  int64_t out_capacity;
+  CallDev* call;
+};
+int launch_compact(const CompactLaunch& c, int sm_count, cudaStream_t s);
+
+// ---- partition.cu ----------------------------------------------------------------------
+struct PartitionLaunch {
+  KeyDesc key;
+  AggPlan plan;             // value column pointers
+  int64_t n;
+  int key_kind;
+  int bits;                 // P = 2^bits partitions, taken from the top bits of table_hash64(u)
+  uint32_t* hist;           // [P]   device, zeroed by the launcher
+  unsigned long long* cursor;  // [P] device
+  uint64_t* out_u;          // [n] rebased fused keys in partition order
+  uint64_t* out_vals[kMaxVals];  // [n] per value column
+};
+int launch_partition(const PartitionLaunch& p, int sm_count, cudaStream_t s);
+
+}  // namespace eiger

@@ -1,0 +1,229 @@
+// Steps A1-A3: the fused single-pass profile kernel — exact min/max and HyperLogLog
+// registers of one key column — and the register-histogram / estimator that follow.
+// PAPER.md:30 §1, §4 ("close to the memory bandwidth"), §4.1
+// (HLL++ [14] before the group-by), §4.3 (range first).  Readings R1-R6.
+#include <cmath>
+
+#include "internal.h"
+
+namespace eiger {
+namespace {
+
+constexpr int kProfThreads = 512;
+constexpr int kProfUnroll = 4;     // 16-byte vectors in flight per thread
+
+__global__ void profile_reset_kernel(ProfileDev* out, int with_regs) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < 2) { out->min[t] = INT64_MAX; out->max[t] = INT64_MIN; }
+  if (t < 64) out->hist[t] = 0;
+  if (with_regs) for (int i = t; i < kHllM; i += gridDim.x * blockDim.x) out->regs[i] = 0;
+}
+
+// One sketch update against the CTA's byte registers in shared memory.  Registers only
+// grow and settle after the first few thousand keys, so the common case is one LDS.U8 and
+// a compare; the rare raise is a CAS on the containing word.
+__device__ __forceinline__ void hll_update(uint32_t* sregs, uint64_t x) {
+  const uint64_t z = hll_hash64(x);
+  const uint32_t idx = (uint32_t)(z >> (64 - kHllP));
+  const uint64_t w = z << kHllP;
+  const uint32_t rho = (uint32_t)min(__clzll((long long)w), kHllQ) + 1u;
+  const uint8_t cur = reinterpret_cast<const volatile uint8_t*>(sregs)[idx];
+  if (rho > cur) {
+    uint32_t* word = sregs + (idx >> 2);
+    const uint32_t sh = (idx & 3u) * 8u;
+    uint32_t old = *reinterpret_cast<volatile uint32_t*>(word);
+    while (((old >> sh) & 0xFFu) < rho) {
+      const uint32_t want = (old & ~(0xFFu << sh)) | (rho << sh);
+      const uint32_t seen = atomicCAS(word, old, want);
+      if (seen == old) break;
+      old = seen;
+    }
+  }
+}
+
+template <int DT> struct Elem;
+template <> struct Elem<EIGER_I8> { static constexpr int kPerVec = 16; };
+template <> struct Elem<EIGER_I32> { static constexpr int kPerVec = 4; };
+template <> struct Elem<EIGER_I64> { static constexpr int kPerVec = 2; };
+
+template <int DT, bool HLL>
+__device__ __forceinline__ void consume_vec(const uint4 v, long long& lo, long long& hi, uint32_t* sregs) {
+  if constexpr (DT == EIGER_I64) {
+    const long long a = (long long)(((uint64_t)v.y << 32) | v.x), b = (long long)(((uint64_t)v.w << 32) | v.z);
+    lo = min(lo, min(a, b)); hi = max(hi, max(a, b));
+    if constexpr (HLL) { hll_update(sregs, (uint64_t)a); hll_update(sregs, (uint64_t)b); }
+  } else if constexpr (DT == EIGER_I32) {
+    const int a = (int)v.x, b = (int)v.y, c = (int)v.z, d = (int)v.w;
+    const int l = min(min(a, b), min(c, d)), h = max(max(a, b), max(c, d));
+    lo = min(lo, (long long)l); hi = max(hi, (long long)h);
+    if constexpr (HLL) {
+      hll_update(sregs, (uint64_t)(long long)a); hll_update(sregs, (uint64_t)(long long)b);
+      hll_update(sregs, (uint64_t)(long long)c); hll_update(sregs, (uint64_t)(long long)d);
+    }
+  } else {
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+    uint32_t l4 = w[0], h4 = w[0];
+#pragma unroll
+    for (int k = 1; k < 4; ++k) { l4 = __vmins4(l4, w[k]); h4 = __vmaxs4(h4, w[k]); }
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      lo = min(lo, (long long)(int8_t)(l4 >> (8 * b)));
+      hi = max(hi, (long long)(int8_t)(h4 >> (8 * b)));
+    }
+    if constexpr (HLL) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) hll_update(sregs, (uint64_t)(long long)(int8_t)(w[k] >> (8 * b)));
+    }
+  }
+}
+
+template <int DT, bool HLL>
+__global__ void __launch_bounds__(kProfThreads)
+profile_kernel(const void* __restrict__ keys, int64_t n, ProfileDev* __restrict__ out, int which) {
+  __shared__ uint32_t sregs[HLL ? kHllM / 4 : 1];
+  __shared__ long long s_lo[kProfThreads / 32], s_hi[kProfThreads / 32];
+  const int tid = threadIdx.x;
+  if constexpr (HLL) {
+    for (int i = tid; i < kHllM / 4; i += kProfThreads) sregs[i] = 0;
+    __syncthreads();
+  }
+  long long lo = INT64_MAX, hi = INT64_MIN;
+  constexpr int EPV = Elem<DT>::kPerVec;
+  const int64_t nvec = n / EPV;
+  const uint4* vp = static_cast<const uint4*>(keys);
+  const int64_t stride = (int64_t)gridDim.x * kProfThreads;
+  int64_t v = (int64_t)blockIdx.x * kProfThreads + tid;
+  for (; v + (kProfUnroll - 1) * stride < nvec; v += kProfUnroll * stride) {
+    uint4 r[kProfUnroll];
+#pragma unroll
+    for (int k = 0; k < kProfUnroll; ++k) r[k] = ldg_stream_16(vp + v + k * stride);
+#pragma unroll
+    for (int k = 0; k < kProfUnroll; ++k) consume_vec<DT, HLL>(r[k], lo, hi, sregs);
+  }
+  for (; v < nvec; v += stride) consume_vec<DT, HLL>(ldg_stream_16(vp + v), lo, hi, sregs);
+  // ragged tail: fewer than EPV elements, taken by the first threads of CTA 0
+  if (blockIdx.x == 0 && tid < (int)(n - nvec * EPV)) {
+    const uint64_t x = sext_load(keys, DT, nvec * EPV + tid);
+    lo = min(lo, (long long)x); hi = max(hi, (long long)x);
+    if constexpr (HLL) hll_update(sregs, x);
+  }
+  // CTA-level merge: shuffles for the 64-bit min/max, one global atomic pair per CTA
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+    hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+  }
+  if ((tid & 31) == 0) { s_lo[tid >> 5] = lo; s_hi[tid >> 5] = hi; }
+  __syncthreads();
+  if (tid < 32) {
+    lo = tid < kProfThreads / 32 ? s_lo[tid] : INT64_MAX;
+    hi = tid < kProfThreads / 32 ? s_hi[tid] : INT64_MIN;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+      hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    if (tid == 0) {
+      if (lo != INT64_MAX) atomicMin(&out->min[which], lo);
+      if (hi != INT64_MIN) atomicMax(&out->max[which], hi);
+    }
+  }
+  if constexpr (HLL) {
+    // one CTA-level merge of the sketch: only non-zero registers touch global memory
+    for (int i = tid; i < kHllM / 4; i += kProfThreads) {
+      const uint32_t w = sregs[i];
+      if (w == 0) continue;
+#pragma unroll
+      for (int b = 0; b < 4; ++b) {
+        const uint32_t r = (w >> (8 * b)) & 0xFFu;
+        if (r) atomicMax(&out->regs[i * 4 + b], r);
+      }
+    }
+  }
+}
+
+__global__ void hll_hist_kernel(ProfileDev* out) {
+  __shared__ uint32_t h[64];
+  if (threadIdx.x < 64) h[threadIdx.x] = 0;
+  __syncthreads();
+  for (int i = threadIdx.x; i < kHllM; i += blockDim.x) atomicAdd(&h[out->regs[i] & 63u], 1u);
+  __syncthreads();
+  if (threadIdx.x < 64) out->hist[threadIdx.x] = h[threadIdx.x];
+}
+
+__global__ void regs_to_bytes_kernel(const ProfileDev* in, uint8_t* out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < kHllM) out[i] = (uint8_t)in->regs[i];
+}
+
+template <int DT>
+int launch_profile_dt(Runtime* rt, const void* keys, int64_t n, int which, int with_hll, cudaStream_t s) {
+  const int64_t nvec = n / Elem<DT>::kPerVec;
+  const int64_t want = (nvec + (int64_t)kProfThreads * kProfUnroll - 1) / ((int64_t)kProfThreads * kProfUnroll);
+  // persistent grid: two CTAs (32 warps) per SM, or fewer when the column is short
+  const int blocks = (int)std::max<int64_t>(1, std::min<int64_t>(want, 2LL * rt->sm_count));
+  if (with_hll) profile_kernel<DT, true><<<blocks, kProfThreads, 0, s>>>(keys, n, rt->prof, which);
+  else profile_kernel<DT, false><<<blocks, kProfThreads, 0, s>>>(keys, n, rt->prof, which);
+  count_launch();
+  EIGER_CUDA(cudaGetLastError());
+  return EIGER_OK;
+}
+
+}  // namespace
+
+int launch_profile(Runtime* rt, const void* keys, int dtype, int64_t n, int which, int with_hll,
+                   bool reset, cudaStream_t s) {
+  if (reset) {
+    profile_reset_kernel<<<16, 1024, 0, s>>>(rt->prof, 1);
+    count_launch();
+    EIGER_CUDA(cudaGetLastError());
+  }
+  if (n == 0) return EIGER_OK;
+  switch (dtype) {
+    case EIGER_I8: return launch_profile_dt<EIGER_I8>(rt, keys, n, which, with_hll, s);
+    case EIGER_I32: return launch_profile_dt<EIGER_I32>(rt, keys, n, which, with_hll, s);
+    case EIGER_I64: return launch_profile_dt<EIGER_I64>(rt, keys, n, which, with_hll, s);
+    default: return EIGER_ERR_ARG;
+  }
+}
+
+int launch_hll_hist(Runtime* rt, cudaStream_t s) {
+  hll_hist_kernel<<<1, 1024, 0, s>>>(rt->prof);
+  count_launch();
+  EIGER_CUDA(cudaGetLastError());
+  return EIGER_OK;
+}
+
+int launch_regs_to_bytes(Runtime* rt, uint8_t* out, cudaStream_t s) {
+  regs_to_bytes_kernel<<<kHllM / 256, 256, 0, s>>>(rt->prof, out);
+  count_launch();
+  EIGER_CUDA(cudaGetLastError());
+  return EIGER_OK;
+}
+
+// Step A3 (R5): table-free estimator from the register-value histogram.
+//   z = m tau(1 - C[q+1]/m); for k = q..1: z = (z + C[k]) / 2; z += m sigma(C[0]/m);
+//   est = m^2 / (2 ln 2 z)
+static double hll_sigma(double x) {
+  if (x == 1.0) return INFINITY;
+  double y = 1.0, z = x, prev;
+  do { x *= x; prev = z; z += x * y; y += y; } while (prev != z);
+  return z;
+}
+static double hll_tau(double x) {
+  if (x == 0.0 || x == 1.0) return 0.0;
+  double y = 1.0, z = 1.0 - x, prev;
+  do { x = std::sqrt(x); prev = z; y *= 0.5; const double d = 1.0 - x; z -= d * d * y; } while (prev != z);
+  return z / 3.0;
+}
+double hll_estimate_from_hist(const uint32_t* hist) {
+  const double m = (double)kHllM;
+  double z = m * hll_tau(1.0 - (double)hist[kHllQ + 1] / m);
+  for (int k = kHllQ; k >= 1; --k) z = 0.5 * (z + (double)hist[k]);
+  z += m * hll_sigma((double)hist[0] / m);
+  return m * m / (2.0 * std::log(2.0) * z);
+}
+
+}  // namespace eiger

@@ -1,0 +1,67 @@
+"""The C-ABI boundary without a GPU: the library builds, loads and exports every symbol
+include/eiger.h declares; host-only entry points behave (no compute calls here)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2607_04489_b200 as eiger
+from paper_2607_04489_b200.build import build_library
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build_library()
+    return eiger.lib()
+
+
+def test_header_symbols_are_exported(lib):
+    header = open(os.path.join(ROOT, "include", "eiger.h")).read()
+    declared = set(re.findall(r"\b(eiger_[a-z0-9_]+)\s*\(", header))
+    assert declared == set(eiger.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_strerror_and_names(lib):
+    assert lib.eiger_strerror(0) == b"ok"
+    assert b"workspace" in lib.eiger_strerror(eiger.ERR_WORKSPACE)
+    assert [lib.eiger_variant_name(v).decode() for v in range(5)] == ["auto", "direct", "smem", "global", "partition"]
+
+
+def test_host_estimator_matches_oracle(lib):
+    # step A3 is host arithmetic inside the library: compare with the oracle's estimator on
+    # registers produced by the oracle (independent implementations of the same reading R5)
+    for n in (0, 1, 100, 20_000, 3_000_000):
+        regs = oracle.hll_registers(np.arange(n, dtype=np.int64) * 2654435761)
+        got = eiger.hll_estimate(regs)
+        want = oracle.hll_estimate(regs)
+        assert got == pytest.approx(want, rel=1e-12, abs=1e-12)
+
+
+def test_selector_is_callable_without_a_gpu(lib):
+    import torch
+    keys = [torch.zeros(16, dtype=torch.int32)]
+    vals = [torch.zeros(16, dtype=torch.int64)]
+    aggs = [(eiger.SUM, 0), (eiger.COUNT, 0)]
+    n = 1 << 28
+
+    class Fake:   # only numel() / dtype / data_ptr are read by the marshalling code
+        def __init__(self, t, n): self.t, self.n = t, n
+        dtype = property(lambda s: s.t.dtype)
+        def numel(self): return self.n
+        def is_contiguous(self): return True
+        def data_ptr(self): return 0
+    fk, fv = [Fake(keys[0], n)], [Fake(vals[0], n)]
+    pick = lambda lo, hi, ndv: eiger.select_variant(fk, fv, aggs, [eiger.Stats(lo, hi, float(ndv), n)])
+    assert pick(0, 15, 16) == eiger.DIRECT
+    assert pick(0, (1 << 12) - 1, 1 << 12) == eiger.DIRECT
+    assert pick(-(1 << 31), (1 << 31) - 1, 256) == eiger.SMEM
+    assert pick(-(1 << 31), (1 << 31) - 1, 1 << 18) == eiger.GLOBAL
+    assert pick(-(1 << 31), (1 << 31) - 1, 1 << 26) == eiger.PARTITION
+    assert eiger.workspace_bytes(fk, fv, aggs, [eiger.Stats(0, 15, 16.0, n)]) >= 256

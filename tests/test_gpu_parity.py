@@ -1,0 +1,208 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Sizes span several tiles and a ragged tail."""
+import numpy as np
+import pytest
+import torch
+
+import datagen
+import oracle
+import paper_2607_04489_b200 as eiger
+from parity import assert_matches, oracle_result
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+ALL_VARIANTS = [eiger.AUTO, eiger.DIRECT, eiger.SMEM, eiger.GLOBAL, eiger.PARTITION]
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    assert torch.cuda.is_available(), "these tests need the B200"
+    eiger.lib()   # fails loudly if libeiger.so is missing: no fallback exists
+    yield
+
+
+def to_dev(ds):
+    return datagen.Dataset(ds.name, ds.n, [k.to(DEV) for k in ds.keys], [v.to(DEV) for v in ds.vals],
+                           ds.aggs, ds.ndv, ds.exact_f64_sum, ds.meta)
+
+
+def run_all_variants(ds, variants=ALL_VARIANTS, expect_infeasible=()):
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    ran = []
+    for v in variants:
+        try:
+            res = eiger.groupby(d.keys, d.vals, d.aggs, force=v)
+        except eiger.EigerError as e:
+            assert e.code == eiger.ERR_INFEASIBLE and v in expect_infeasible, (v, str(e))
+            continue
+        assert v == eiger.AUTO or res.variant == v
+        assert_matches(res, want, d.aggs, d.vals)
+        ran.append(res.variant)
+    return ran
+
+
+# ---- profile (A1-A3) ---------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", [torch.int8, torch.int32, torch.int64])
+@pytest.mark.parametrize("n", [0, 1, 15, 17, 4097, 1_000_003])
+def test_profile_parity(dtype, n):
+    g = torch.Generator().manual_seed(n + 1)
+    info = torch.iinfo(dtype)
+    keys = torch.randint(max(info.min, -(1 << 62)), min(info.max, (1 << 62)), (n,), generator=g, dtype=torch.int64).to(dtype)
+    if n > 4:
+        keys[3] = info.min; keys[n - 2] = info.max
+    want_regs = oracle.hll_registers(keys.numpy())
+    got_regs = eiger.hll_registers(keys.to(DEV)).cpu().numpy()
+    assert np.array_equal(got_regs, want_regs)                       # bit for bit
+    st = eiger.profile(keys.to(DEV))
+    ws = oracle.profile(keys.numpy())
+    assert (st.min, st.max, st.n) == (ws.min, ws.max, ws.n)
+    assert st.ndv_est == pytest.approx(ws.ndv_est, rel=1e-12, abs=1e-12)
+
+
+@pytest.mark.parametrize("lg,scattered", [(4, False), (12, True), (16, False), (20, True)])
+def test_profile_known_ndv(lg, scattered):
+    ds = datagen.config5(n=1 << 22, ndv=1 << lg, scattered=scattered)
+    st = eiger.profile(ds.keys[0].to(DEV))
+    ndv = min(1 << lg, 1 << 22)
+    assert abs(st.ndv_est - ndv) / ndv <= 4 * 1.04 / 128                 # 4 sigma, m = 2^14
+    assert np.array_equal(eiger.hll_registers(ds.keys[0].to(DEV)).cpu().numpy(), oracle.hll_registers(ds.keys[0].numpy()))
+
+
+def test_datagen_is_device_independent():
+    a = datagen.config3(n=300_000, D=5000)
+    b = datagen.config3(device=DEV, n=300_000, D=5000)
+    assert torch.equal(a.keys[0], b.keys[0].cpu()) and torch.equal(a.vals[0], b.vals[0].cpu())
+    a = datagen.config5(n=300_000, ndv=4096, scattered=True)
+    b = datagen.config5(device=DEV, n=300_000, ndv=4096, scattered=True)
+    assert torch.equal(a.keys[0], b.keys[0].cpu()) and torch.equal(a.vals[0], b.vals[0].cpu())
+
+
+# ---- the five configs, every variant -------------------------------------------------------
+def test_config1_all_variants():
+    ran = run_all_variants(datagen.config1())
+    assert ran[0] == eiger.DIRECT
+
+
+@pytest.mark.parametrize("skewed", [False, True])
+def test_config2_scaled(skewed):
+    ds = datagen.config2(n=3_000_017, skewed=skewed)
+    ran = run_all_variants(ds)
+    assert ran[0] == eiger.DIRECT
+
+
+@pytest.mark.parametrize("dense", [False, True])
+def test_config3_scaled(dense):
+    ds = datagen.config3(n=2_000_003, D=50_000, dense=dense)
+    run_all_variants(ds, expect_infeasible=() if dense else (eiger.DIRECT,))
+
+
+def test_config4_scaled():
+    ds = datagen.config4(n=3_000_001, D=600_000)
+    run_all_variants(ds, expect_infeasible=(eiger.DIRECT,))
+
+
+@pytest.mark.parametrize("lg", [4, 8, 12, 16, 20])
+@pytest.mark.parametrize("scattered", [False, True])
+def test_config5_scaled(lg, scattered):
+    ds = datagen.config5(n=(1 << 21) + 13, ndv=1 << lg, scattered=scattered)
+    run_all_variants(ds)
+
+
+# ---- edge cases ------------------------------------------------------------------------------
+def test_empty_input():
+    k = torch.zeros(0, dtype=torch.int64, device=DEV)
+    v = torch.zeros(0, dtype=torch.int64, device=DEV)
+    for f in ALL_VARIANTS:
+        res = eiger.groupby([k], [v], [(eiger.SUM, 0), (eiger.COUNT, 0)], force=f)
+        assert res.n_groups == 0
+    st = eiger.profile(k)
+    assert (st.min, st.max, st.ndv_est, st.n) == ((1 << 63) - 1, -(1 << 63), 0.0, 0)
+
+
+@pytest.mark.parametrize("n", [1, 2, 31, 33, 511, 513, 2047, 2049, 100_001])
+def test_ragged_sizes(n):
+    i = torch.arange(n, dtype=torch.int64)
+    ds = datagen.Dataset("rag", n, [(i % 7).to(torch.int32)], [i], [(eiger.COUNT, 0), (eiger.SUM, 0), (eiger.MIN, 0), (eiger.MAX, 0)])
+    run_all_variants(ds)
+
+
+def test_closed_form_without_oracle():
+    # key_i = i mod D, value_i = i (SURVEY.md 8(c) C.5 iii): checks 64-bit sums at a size the
+    # oracle is not needed for
+    n, D = (1 << 24) + 5, 1000
+    i = torch.arange(n, dtype=torch.int64, device=DEV)
+    res = eiger.groupby([(i % D).to(torch.int32)], [i], [(eiger.COUNT, 0), (eiger.SUM, 0), (eiger.MIN, 0), (eiger.MAX, 0)]).sorted()
+    k = torch.arange(D, dtype=torch.int64, device=DEV)
+    c = (n - k + D - 1) // D
+    assert torch.equal(res.keys[0].long(), k) and torch.equal(res.aggs[0], c)
+    assert torch.equal(res.aggs[1], c * k + D * c * (c - 1) // 2)
+    assert torch.equal(res.aggs[2], k) and torch.equal(res.aggs[3], k + D * (c - 1))
+
+
+def test_int64_extremes_and_sentinel_key():
+    k = torch.tensor([-(1 << 63), (1 << 63) - 1, -(1 << 63), 0, (1 << 63) - 1, 5, -1] * 300, dtype=torch.int64)
+    v = torch.arange(k.numel(), dtype=torch.int64) - 1000
+    ds = datagen.Dataset("ext", k.numel(), [k], [v], [(eiger.SUM, 0), (eiger.COUNT, 0), (eiger.MIN, 0), (eiger.MAX, 0)])
+    run_all_variants(ds, expect_infeasible=(eiger.DIRECT,))
+    k32 = torch.tensor([-(1 << 31), (1 << 31) - 1, 0, -1, (1 << 31) - 1] * 400, dtype=torch.int32)
+    v = torch.arange(k32.numel(), dtype=torch.int64)
+    ds = datagen.Dataset("ext32", k32.numel(), [k32], [v], [(eiger.SUM, 0), (eiger.COUNT, 0)])
+    run_all_variants(ds)
+
+
+def test_all_equal_and_all_distinct():
+    n = 70_001
+    v = torch.arange(n, dtype=torch.int64) * 3 - 7
+    run_all_variants(datagen.Dataset("eq", n, [torch.full((n,), -42, dtype=torch.int64)], [v],
+                                     [(eiger.SUM, 0), (eiger.COUNT, 0), (eiger.MIN, 0), (eiger.MAX, 0)]))
+    perm = torch.randperm(n, generator=torch.Generator().manual_seed(1)).to(torch.int32)
+    run_all_variants(datagen.Dataset("dist", n, [perm], [v], [(eiger.SUM, 0), (eiger.COUNT, 0)]))
+
+
+def test_generic_signatures():
+    g = torch.Generator().manual_seed(5)
+    n = 200_003
+    k0 = torch.randint(-3, 4, (n,), generator=g, dtype=torch.int64).to(torch.int8)
+    k1 = torch.randint(100, 140, (n,), generator=g, dtype=torch.int64).to(torch.int32)
+    vi = torch.randint(-10**9, 10**9, (n,), generator=g, dtype=torch.int64)
+    vf = torch.randint(0, 1 << 53, (n,), generator=g, dtype=torch.int64).to(torch.float64) * 2.0 ** -53
+    vneg = -vf - 1.0
+    aggs = [(eiger.MIN, 1), (eiger.MAX, 0), (eiger.SUM, 1), (eiger.MAX, 2), (eiger.MIN, 2), (eiger.SUM, 0)]   # no COUNT
+    ds = datagen.Dataset("gen", n, [k0, k1], [vi, vf, vneg], aggs, exact_f64_sum=False)
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    for f in ALL_VARIANTS:
+        res = eiger.groupby(d.keys, d.vals, d.aggs, force=f)
+        assert_matches(res, want, d.aggs, d.vals, rel=1e-9)          # sequential-sum oracle here
+    # single int8 key, COUNT only
+    ds = datagen.Dataset("cnt", n, [k0], [], [(eiger.COUNT, 0)])
+    run_all_variants(ds)
+
+
+def test_table_overflow_retry_and_errors():
+    ds = to_dev(datagen.config5(n=1 << 20, ndv=1 << 16, scattered=True))
+    want = oracle_result(ds)
+    st = eiger.profile(ds.keys[0])
+    low = [eiger.Stats(st.min, st.max, 64.0, st.n)]                   # injected under-estimate (R10)
+    for f in (eiger.SMEM, eiger.GLOBAL, eiger.PARTITION):
+        res = eiger.groupby(ds.keys, ds.vals, ds.aggs, force=f, stats=low)
+        assert_matches(res, want, ds.aggs, ds.vals)
+    with pytest.raises(eiger.EigerError) as e:
+        eiger.groupby(ds.keys, ds.vals, ds.aggs, out_capacity=10)
+    assert e.value.code == eiger.ERR_OUT_CAPACITY
+    with pytest.raises(eiger.EigerError) as e:                        # misaligned column
+        eiger.groupby([ds.keys[0][1:]], [ds.vals[0][1:]], ds.aggs)
+    assert e.value.code == eiger.ERR_ARG
+    wide = to_dev(datagen.config4(n=10_000, D=5_000))
+    with pytest.raises(eiger.EigerError) as e:
+        eiger.groupby(wide.keys, wide.vals, wide.aggs, force=eiger.DIRECT)
+    assert e.value.code == eiger.ERR_INFEASIBLE
+
+
+def test_host_entry_point():
+    ds = datagen.config1(n=300_007)
+    want = oracle_result(ds)
+    res, h2d, d2h = eiger.groupby_host([k.pin_memory() for k in ds.keys], [v.pin_memory() for v in ds.vals], ds.aggs)
+    assert h2d == ds.n * ds.row_bytes and d2h == res.n_groups * (4 + 8 * 4)
+    assert_matches(res, want, ds.aggs, ds.vals)
