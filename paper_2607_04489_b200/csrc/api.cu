@@ -295,9 +295,14 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     if (!out_keys[k] && out_capacity > 0) return EIGER_ERR_ARG;
   }
   for (int c = 0; c < nv; ++c) if (n > 0 && vals && (!vals[c].data || ((uintptr_t)vals[c].data & 15))) return EIGER_ERR_ARG;
+  if (n == 0) {   // legal: no groups; nothing is launched
+    if (force < EIGER_AUTO || force > EIGER_PARTITION) return EIGER_ERR_ARG;
+    if (chosen) *chosen = force;
+    return EIGER_OK;
+  }
   eiger_stats local[2];
   const eiger_stats* st = stats_in;
-  if (!st && n > 0) {
+  if (!st) {
     // profile inside the call: fused min/max + sketch for 4/8-byte keys; 1-byte keys take the
     // range test only (HLL only when the range test fails; a 1-byte range never does)
     for (int k = 0; k < nk; ++k) {
@@ -310,7 +315,6 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
   int rc = plan_query(rt, keys, nk, n, vals, nv, aggs, na, st, force, &q);
   if (rc) return rc;
   if (chosen) *chosen = q.variant;
-  if (n == 0) return EIGER_OK;
   if (q.total_bytes > workspace_bytes || !workspace) return EIGER_ERR_WORKSPACE;
   if ((uintptr_t)workspace & 255) return EIGER_ERR_ARG;
 
