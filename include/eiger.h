@@ -70,6 +70,13 @@ typedef struct { int64_t min, max; double ndv_est; int64_t n; } eiger_stats;
  * Errors: EIGER_ERR_ARG, EIGER_ERR_CUDA. */
 int eiger_profile(const void* keys, int32_t dtype, int64_t n, eiger_stats* out, void* stream);
 
+/* eiger_profile_keys — the statistics pass exactly as EIGER_AUTO runs it inside eiger_groupby
+ * when no statistics are supplied: one read-back for all key columns; min/max of each; the
+ * sketch only where the range test cannot decide ("range first"): 1-byte keys and
+ * two-column keys get ndv_est = min(n, max - min + 1) without a sketch.
+ *   keys[n_key_cols] DEVICE columns; out[n_key_cols] HOST. */
+int eiger_profile_keys(const eiger_col* keys, int32_t n_key_cols, int64_t n, eiger_stats* out, void* stream);
+
 /* eiger_hll_registers — test hook: the raw sketch registers of a key column.
  *   regs_out  DEVICE, 16384 bytes, register j in byte j (values 0 .. 51).
  * The register array is an exact function of the key set (R3). */

@@ -30,7 +30,7 @@ HLL_M = 1 << 14
 
 # every symbol include/eiger.h declares (tests check the library exports each of them)
 EXPORTS = [
-    "eiger_profile", "eiger_hll_registers", "eiger_hll_estimate_host", "eiger_groupby",
+    "eiger_profile", "eiger_profile_keys", "eiger_hll_registers", "eiger_hll_estimate_host", "eiger_groupby",
     "eiger_groupby_workspace_bytes", "eiger_select_variant", "eiger_groupby_host",
     "eiger_launch_count", "eiger_set_kernel_timing", "eiger_kernel_time_ms", "eiger_strerror",
     "eiger_last_cuda_error", "eiger_variant_name", "eiger_shutdown",
@@ -96,6 +96,8 @@ def lib() -> ctypes.CDLL:
         vp, i32, i64, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_size_t
         L.eiger_profile.restype = ctypes.c_int
         L.eiger_profile.argtypes = [vp, i32, i64, ctypes.POINTER(_Stats), vp]
+        L.eiger_profile_keys.restype = ctypes.c_int
+        L.eiger_profile_keys.argtypes = [vp, i32, i64, vp, vp]
         L.eiger_hll_registers.restype = ctypes.c_int
         L.eiger_hll_registers.argtypes = [vp, i32, i64, vp, vp]
         L.eiger_hll_estimate_host.restype = ctypes.c_double
@@ -181,6 +183,18 @@ def profile(keys: torch.Tensor) -> Stats:
     return Stats(s.min, s.max, s.ndv_est, s.n)
 
 
+def profile_keys(keys) -> list:
+    """eiger_profile_keys: the statistics pass of the adaptive path (range first, sketch only
+    where the range cannot decide), one read-back for all key columns."""
+    if isinstance(keys, torch.Tensor):
+        keys = [keys]
+    arr = (_Stats * len(keys))()
+    dev = keys[0].device
+    with torch.cuda.device(dev):
+        _check(lib().eiger_profile_keys(_cols(keys, _KEY_T), len(keys), keys[0].numel(), arr, _stream(dev)))
+    return [Stats(s.min, s.max, s.ndv_est, s.n) for s in arr]
+
+
 def hll_registers(keys: torch.Tensor) -> torch.Tensor:
     """eiger_hll_registers: the 16384 sketch registers (uint8, device)."""
     out = torch.empty(HLL_M, dtype=torch.uint8, device=keys.device)
@@ -254,7 +268,7 @@ def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int |
     ws = workspace or Workspace(dev)
     with torch.cuda.device(dev):
         if stats is None and n > 0:
-            stats = [profile(k) for k in keys]
+            stats = profile_keys(keys)
         kc, vc, ac, sc = _cols(keys, _KEY_T), _cols(vals, _VAL_T), _aggs(aggs), _stats_arr(stats)
         for attempt in range(3):
             nbytes = int(L.eiger_groupby_workspace_bytes(kc, len(keys), n, vc, len(vals), ac, len(aggs), sc, force))

@@ -258,26 +258,31 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   return EIGER_OK;
 }
 
-int do_profile(Runtime* rt, const void* keys, int dtype, int64_t n, int with_hll, eiger_stats* out, cudaStream_t s) {
+// Profiles nk key columns with one read-back: min/max of each, and (single column only) the
+// sketch.  with_hll = 0 is the range-first shortcut: ndv_est = min(n, range).
+int do_profile(Runtime* rt, const eiger_col* cols, int nk, int64_t n, int with_hll, eiger_stats* out, cudaStream_t s) {
+  if (nk > 1) with_hll = 0;
   {
     Timed t(s, 1);
-    int rc = launch_profile(rt, keys, dtype, n, 0, with_hll, true, s);
-    if (rc) return rc;
+    for (int k = 0; k < nk; ++k) {
+      int rc = launch_profile(rt, cols[k].data, cols[k].dtype, n, k, with_hll, k == 0, s);
+      if (rc) return rc;
+    }
+    if (with_hll) { int rc = launch_hll_hist(rt, s); if (rc) return rc; }
   }
-  if (with_hll) { int rc = launch_hll_hist(rt, s); if (rc) return rc; }
-  struct Back { long long mn, mx; uint32_t hist[64]; };
+  struct Back { long long mn[2], mx[2]; uint32_t hist[64]; };
   Back* b = static_cast<Back*>(rt->pinned);
-  EIGER_CUDA(cudaMemcpyAsync(&b->mn, &rt->prof->min[0], 8, cudaMemcpyDeviceToHost, s));
-  EIGER_CUDA(cudaMemcpyAsync(&b->mx, &rt->prof->max[0], 8, cudaMemcpyDeviceToHost, s));
-  if (with_hll) EIGER_CUDA(cudaMemcpyAsync(b->hist, rt->prof->hist, sizeof(b->hist), cudaMemcpyDeviceToHost, s));
+  EIGER_CUDA(cudaMemcpyAsync(b, rt->prof, sizeof(Back), cudaMemcpyDeviceToHost, s));
   EIGER_CUDA(cudaStreamSynchronize(s));
   resolve_timing();
-  out->min = b->mn; out->max = b->mx; out->n = n;
-  if (n == 0) { out->ndv_est = 0.0; return EIGER_OK; }
-  const double range = (double)((uint64_t)b->mx - (uint64_t)b->mn) + 1.0;
-  double est = with_hll ? hll_estimate_from_hist(b->hist) : range;   // range-first: R bounds NDV
-  est = std::min(est, std::min((double)n, range));
-  out->ndv_est = std::max(est, 0.0);
+  for (int k = 0; k < nk; ++k) {
+    out[k].min = b->mn[k]; out[k].max = b->mx[k]; out[k].n = n;
+    if (n == 0) { out[k].ndv_est = 0.0; continue; }
+    const double range = (double)((uint64_t)b->mx[k] - (uint64_t)b->mn[k]) + 1.0;
+    double est = with_hll ? hll_estimate_from_hist(b->hist) : range;
+    est = std::min(est, std::min((double)n, range));
+    out[k].ndv_est = std::max(est, 0.0);
+  }
   return EIGER_OK;
 }
 
@@ -305,10 +310,8 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
   if (!st) {
     // profile inside the call: fused min/max + sketch for 4/8-byte keys; 1-byte keys take the
     // range test only (HLL only when the range test fails; a 1-byte range never does)
-    for (int k = 0; k < nk; ++k) {
-      int rc = do_profile(rt, keys[k].data, keys[k].dtype, n, keys[k].dtype != EIGER_I8, &local[k], s);
-      if (rc) return rc;
-    }
+    int rc = do_profile(rt, keys, nk, n, keys[0].dtype != EIGER_I8, local, s);
+    if (rc) return rc;
     st = local;
   }
   QueryPlan q;
@@ -438,7 +441,18 @@ int eiger_profile(const void* keys, int32_t dtype, int64_t n, eiger_stats* out, 
   std::lock_guard<std::mutex> lk(g_mu);
   Runtime* rt = runtime();
   if (!rt) return EIGER_ERR_CUDA;
-  return do_profile(rt, keys, dtype, n, 1, out, static_cast<cudaStream_t>(stream));
+  eiger_col c{keys, dtype, 0};
+  return do_profile(rt, &c, 1, n, 1, out, static_cast<cudaStream_t>(stream));
+}
+
+int eiger_profile_keys(const eiger_col* keys, int32_t nk, int64_t n, eiger_stats* out, void* stream) {
+  if (!out || !keys || nk < 1 || nk > 2 || n < 0) return EIGER_ERR_ARG;
+  for (int k = 0; k < nk; ++k)
+    if (!is_key_dtype(keys[k].dtype) || (n > 0 && (!keys[k].data || ((uintptr_t)keys[k].data & 15)))) return EIGER_ERR_ARG;
+  std::lock_guard<std::mutex> lk(g_mu);
+  Runtime* rt = runtime();
+  if (!rt) return EIGER_ERR_CUDA;
+  return do_profile(rt, keys, nk, n, keys[0].dtype != EIGER_I8, out, static_cast<cudaStream_t>(stream));
 }
 
 int eiger_hll_registers(const void* keys, int32_t dtype, int64_t n, uint8_t* regs_out, void* stream) {
@@ -539,10 +553,8 @@ int eiger_groupby_host(const eiger_col* keys, int32_t nk, int64_t n, const eiger
   rc = stage(cur, dk, dv);
   if (rc) return rc;
   eiger_stats st[2];
-  for (int k = 0; k < nk; ++k) {
-    rc = do_profile(rt, dk[k].data, dk[k].dtype, n, dk[k].dtype != EIGER_I8, &st[k], s);
-    if (rc) return rc;
-  }
+  rc = do_profile(rt, dk, nk, n, dk[0].dtype != EIGER_I8, st, s);
+  if (rc) return rc;
   QueryPlan q;
   rc = plan_query(rt, dk, nk, n, dv, nv, aggs, na, st, force, &q);
   if (rc) return rc;

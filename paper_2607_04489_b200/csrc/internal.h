@@ -12,8 +12,8 @@ namespace eiger {
 struct ProfileDev {
   long long min[2];
   long long max[2];
-  uint32_t regs[kHllM];     // sketch registers, one per word (global atomicMax)
   uint32_t hist[64];        // register-value histogram C[0 .. kHllQ + 1]
+  uint32_t regs[kHllM];     // sketch registers, one per word (global atomicMax)
 };
 struct CallDev {
   unsigned long long n_groups;   // compaction claim counter

@@ -62,14 +62,16 @@ __device__ __forceinline__ void consume_vec(const uint4 v, long long& lo, long l
     }
   } else {
     const uint32_t w[4] = {v.x, v.y, v.z, v.w};
-    uint32_t l4 = w[0], h4 = w[0];
+    // per-byte sign extension + 32-bit min/max: ~3 ALU instructions per key, far below the
+    // issue budget of a 1-byte-per-key stream (the SIMD-in-word intrinsics are emulated)
+    int l = INT32_MAX, h = INT32_MIN;
 #pragma unroll
-    for (int k = 1; k < 4; ++k) { l4 = __vmins4(l4, w[k]); h4 = __vmaxs4(h4, w[k]); }
-#pragma unroll
-    for (int b = 0; b < 4; ++b) {
-      lo = min(lo, (long long)(int8_t)(l4 >> (8 * b)));
-      hi = max(hi, (long long)(int8_t)(h4 >> (8 * b)));
+    for (int k = 0; k < 4; ++k) {
+      const int b0 = (int)(int8_t)(w[k]), b1 = (int)(int8_t)(w[k] >> 8), b2 = (int)(int8_t)(w[k] >> 16), b3 = (int)w[k] >> 24;
+      l = min(min(l, b0), min(min(b1, b2), b3));
+      h = max(max(h, b0), max(max(b1, b2), b3));
     }
+    lo = min(lo, (long long)l); hi = max(hi, (long long)h);
     if constexpr (HLL) {
 #pragma unroll
       for (int k = 0; k < 4; ++k)
