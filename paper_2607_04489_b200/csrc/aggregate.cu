@@ -99,6 +99,49 @@ __device__ __forceinline__ uint64_t* back_hash_cells(void* table, uint64_t cap, 
   return nullptr;
 }
 
+// ---- shared-memory accumulators ------------------------------------------------------------
+// B200 shared memory has native 32-bit atomics (ATOMS.ADD / ATOMS.MAX, ~2 T/s chip-wide,
+// measured) but 64-bit ones are CAS loops (~0.1-0.3 T/s).  Integer SUM and COUNT cells are
+// therefore kept as two 32-bit planes, lo[S] then hi[S], and added with an explicit carry:
+// the final (hi:lo) equals the wrapping 64-bit sum whatever the interleaving, because every
+// wrap of lo is seen by exactly one atomicAdd's return value.  MIN / MAX and fp64 SUM keep
+// 64-bit cells; MIN / MAX look before they leap, so the CAS loop only runs on a new record.
+__device__ __forceinline__ bool add_type(int op, bool f64) { return op == EIGER_COUNT || (op == EIGER_SUM && !f64); }
+__device__ __forceinline__ void smem_add64(uint32_t* lo, uint32_t* hi, uint64_t v) {
+  const uint32_t vl = (uint32_t)v;
+  const uint32_t old = atomicAdd(lo, vl);
+  const uint32_t h = (uint32_t)(v >> 32) + ((uint32_t)(old + vl) < vl ? 1u : 0u);
+  if (h) atomicAdd(hi, h);
+}
+// accumulator j of a table of S slots that starts at base occupies 8 * S bytes
+__device__ __forceinline__ void smem_merge(unsigned char* base, uint32_t S, int j, uint32_t s, int op, bool f64, uint64_t part) {
+  unsigned char* plane = base + (size_t)j * 8 * S;
+  if (add_type(op, f64)) {
+    uint32_t* lo = reinterpret_cast<uint32_t*>(plane) + s;
+    smem_add64(lo, lo + S, part);
+  } else if (op == EIGER_SUM) {
+    atomicAdd(reinterpret_cast<double*>(plane) + s, __longlong_as_double((long long)part));
+  } else {
+    long long* cell = reinterpret_cast<long long*>(plane) + s;
+    const long long cur = *reinterpret_cast<volatile long long*>(cell);
+    if (op == EIGER_MIN) { if ((long long)part < cur) atomicMin(cell, (long long)part); }
+    else { if ((long long)part > cur) atomicMax(cell, (long long)part); }
+  }
+}
+__device__ __forceinline__ uint64_t smem_read(const unsigned char* base, uint32_t S, int j, uint32_t s, int op, bool f64) {
+  const unsigned char* plane = base + (size_t)j * 8 * S;
+  if (add_type(op, f64)) {
+    const uint32_t* lo = reinterpret_cast<const uint32_t*>(plane) + s;
+    return ((uint64_t)lo[S] << 32) | lo[0];
+  }
+  return reinterpret_cast<const uint64_t*>(plane)[s];
+}
+__device__ __forceinline__ void smem_init_plane(unsigned char* base, uint32_t S, int j, int op, bool f64, int tid, int T) {
+  uint64_t* plane = reinterpret_cast<uint64_t*>(base + (size_t)j * 8 * S);
+  const uint64_t v = add_type(op, f64) ? 0ull : acc_identity(op);
+  for (uint32_t c = tid; c < S; c += T) plane[c] = v;
+}
+
 struct AggArgs {
   KeyDesc key;
   AggPlan plan;
@@ -142,12 +185,13 @@ struct AggCtx {
       for (uint32_t c = 0; c < a.front_slots * (uint32_t)n_acc; ++c)
         acc[(size_t)c * T + tid] = acc_identity(sig_op<SIG>(a.plan, (int)(c % (uint32_t)n_acc)));
     } else if constexpr (FRONT == FRONT_SDIRECT) {
-      uint64_t* acc = reinterpret_cast<uint64_t*>(smem);
-      const uint32_t per = a.front_slots * (uint32_t)n_acc, tot = per * a.front_replicas;
-      for (uint32_t c = tid; c < tot; c += T) acc[c] = acc_identity(sig_op<SIG>(a.plan, (int)((c % per) / a.front_slots)));
+      for (uint32_t rep = 0; rep < a.front_replicas; ++rep)
+        for (int j = 0; j < n_acc; ++j)
+          smem_init_plane(smem + (size_t)rep * a.front_slots * 8 * (uint32_t)n_acc, a.front_slots, j, sig_op<SIG>(a.plan, j), sig_f64<SIG>(a.plan, j), tid, T);
     } else if constexpr (FRONT == FRONT_SHASH) {
       for (uint32_t c = tid; c < a.front_slots; c += T) skeys[c] = empty_of<U>();
-      for (uint32_t c = tid; c < a.front_slots * (uint32_t)n_acc; c += T) sacc[c] = acc_identity(sig_op<SIG>(a.plan, (int)(c / a.front_slots)));
+      for (int j = 0; j < n_acc; ++j)
+        smem_init_plane(reinterpret_cast<unsigned char*>(sacc), a.front_slots, j, sig_op<SIG>(a.plan, j), sig_f64<SIG>(a.plan, j), tid, T);
       if (tid == 0) *scount = 0;
     }
     if constexpr (FRONT != FRONT_NONE) __syncthreads();
@@ -198,13 +242,13 @@ struct AggCtx {
         *c = combine(op, f, *c, row_partial(op, f, raw[sig_col<SIG>(a.plan, j)]));
       }
     } else if constexpr (FRONT == FRONT_SDIRECT) {
-      const uint32_t rep = (threadIdx.x >> 5) % a.front_replicas;
-      uint64_t* acc = reinterpret_cast<uint64_t*>(smem) + (size_t)rep * a.front_slots * (uint32_t)n_acc + (uint32_t)u;
+      const uint32_t rep = a.front_replicas > 1 ? (threadIdx.x >> 5) % a.front_replicas : 0u;
+      unsigned char* base = smem + (size_t)rep * a.front_slots * 8 * (uint32_t)n_acc;
 #pragma unroll
       for (int j = 0; j < NA; ++j) {
         if (!S::kStatic && j >= n_acc) break;
         const int op = sig_op<SIG>(a.plan, j); const bool f = sig_f64<SIG>(a.plan, j);
-        atomic_merge(acc + (size_t)j * a.front_slots, op, f, row_partial(op, f, raw[sig_col<SIG>(a.plan, j)]));
+        smem_merge(base, a.front_slots, j, (uint32_t)u, op, f, row_partial(op, f, raw[sig_col<SIG>(a.plan, j)]));
       }
     } else if constexpr (FRONT == FRONT_SHASH) {
       const int h = shash_find(u);
@@ -213,7 +257,7 @@ struct AggCtx {
       for (int j = 0; j < NA; ++j) {
         if (!S::kStatic && j >= n_acc) break;
         const int op = sig_op<SIG>(a.plan, j); const bool f = sig_f64<SIG>(a.plan, j);
-        atomic_merge(sacc + (size_t)j * a.front_slots + h, op, f, row_partial(op, f, raw[sig_col<SIG>(a.plan, j)]));
+        smem_merge(reinterpret_cast<unsigned char*>(sacc), a.front_slots, j, (uint32_t)h, op, f, row_partial(op, f, raw[sig_col<SIG>(a.plan, j)]));
       }
     } else {
       back_row(u, raw);
@@ -245,11 +289,12 @@ struct AggCtx {
         if (lane == 0) back_merge(c / (uint32_t)n_acc, j, v, static_cast<uint64_t*>(a.table) + (uint64_t)(c / (uint32_t)n_acc) * (uint32_t)n_acc);
       }
     } else if constexpr (FRONT == FRONT_SDIRECT) {
-      const uint64_t* acc = reinterpret_cast<const uint64_t*>(smem);
       const uint32_t per = a.front_slots * (uint32_t)n_acc, tot = per * a.front_replicas;
       for (uint32_t c = tid; c < tot; c += T) {
-        const uint32_t w = c % per, j = w / a.front_slots, u = w % a.front_slots;
-        back_merge(u, (int)j, acc[c], static_cast<uint64_t*>(a.table) + (uint64_t)u * (uint32_t)n_acc);
+        const uint32_t rep = c / per, w = c % per, j = w / a.front_slots, u = w % a.front_slots;
+        const uint64_t v = smem_read(smem + (size_t)rep * a.front_slots * 8 * (uint32_t)n_acc, a.front_slots, (int)j, u,
+                                     sig_op<SIG>(a.plan, (int)j), sig_f64<SIG>(a.plan, (int)j));
+        back_merge(u, (int)j, v, static_cast<uint64_t*>(a.table) + (uint64_t)u * (uint32_t)n_acc);
       }
     } else if constexpr (FRONT == FRONT_SHASH) {
       for (uint32_t h = tid; h < a.front_slots; h += T) {
@@ -257,7 +302,8 @@ struct AggCtx {
         if (k == empty_of<U>()) continue;
         uint64_t* cells = back_hash_cells(a.table, a.cap, a.stride, (uint64_t)k, a.call);
         if (!cells) continue;
-        for (int j = 0; j < n_acc; ++j) back_merge((uint64_t)k, j, sacc[(size_t)j * a.front_slots + h], cells);
+        for (int j = 0; j < n_acc; ++j)
+          back_merge((uint64_t)k, j, smem_read(reinterpret_cast<const unsigned char*>(sacc), a.front_slots, j, h, sig_op<SIG>(a.plan, j), sig_f64<SIG>(a.plan, j)), cells);
       }
     }
   }

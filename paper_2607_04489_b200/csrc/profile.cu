@@ -19,26 +19,15 @@ __global__ void profile_reset_kernel(ProfileDev* out, int with_regs) {
   if (with_regs) for (int i = t; i < kHllM; i += gridDim.x * blockDim.x) out->regs[i] = 0;
 }
 
-// One sketch update against the CTA's byte registers in shared memory.  Registers only
-// grow and settle after the first few thousand keys, so the common case is one LDS.U8 and
-// a compare; the rare raise is a CAS on the containing word.
+// One sketch update against the CTA's registers in shared memory: one word per register and
+// one native ATOMS.MAX per key (B200 shared memory does ~2 T 32-bit atomics/s, measured, so
+// the unconditional atomic is cheaper than a look-before-you-leap branch plus a CAS loop).
 __device__ __forceinline__ void hll_update(uint32_t* sregs, uint64_t x) {
   const uint64_t z = hll_hash64(x);
   const uint32_t idx = (uint32_t)(z >> (64 - kHllP));
   const uint64_t w = z << kHllP;
   const uint32_t rho = (uint32_t)min(__clzll((long long)w), kHllQ) + 1u;
-  const uint8_t cur = reinterpret_cast<const volatile uint8_t*>(sregs)[idx];
-  if (rho > cur) {
-    uint32_t* word = sregs + (idx >> 2);
-    const uint32_t sh = (idx & 3u) * 8u;
-    uint32_t old = *reinterpret_cast<volatile uint32_t*>(word);
-    while (((old >> sh) & 0xFFu) < rho) {
-      const uint32_t want = (old & ~(0xFFu << sh)) | (rho << sh);
-      const uint32_t seen = atomicCAS(word, old, want);
-      if (seen == old) break;
-      old = seen;
-    }
-  }
+  atomicMax(sregs + idx, rho);
 }
 
 template <int DT> struct Elem;
@@ -84,11 +73,11 @@ __device__ __forceinline__ void consume_vec(const uint4 v, long long& lo, long l
 template <int DT, bool HLL>
 __global__ void __launch_bounds__(kProfThreads)
 profile_kernel(const void* __restrict__ keys, int64_t n, ProfileDev* __restrict__ out, int which) {
-  __shared__ uint32_t sregs[HLL ? kHllM / 4 : 1];
+  extern __shared__ uint32_t sregs[];   // kHllM words when HLL
   __shared__ long long s_lo[kProfThreads / 32], s_hi[kProfThreads / 32];
   const int tid = threadIdx.x;
   if constexpr (HLL) {
-    for (int i = tid; i < kHllM / 4; i += kProfThreads) sregs[i] = 0;
+    for (int i = tid; i < kHllM; i += kProfThreads) sregs[i] = 0;
     __syncthreads();
   }
   long long lo = INT64_MAX, hi = INT64_MIN;
@@ -134,14 +123,10 @@ profile_kernel(const void* __restrict__ keys, int64_t n, ProfileDev* __restrict_
   }
   if constexpr (HLL) {
     // one CTA-level merge of the sketch: only non-zero registers touch global memory
-    for (int i = tid; i < kHllM / 4; i += kProfThreads) {
-      const uint32_t w = sregs[i];
-      if (w == 0) continue;
-#pragma unroll
-      for (int b = 0; b < 4; ++b) {
-        const uint32_t r = (w >> (8 * b)) & 0xFFu;
-        if (r) atomicMax(&out->regs[i * 4 + b], r);
-      }
+    __syncthreads();
+    for (int i = tid; i < kHllM; i += kProfThreads) {
+      const uint32_t r = sregs[i];
+      if (r) atomicMax(&out->regs[i], r);
     }
   }
 }
@@ -166,8 +151,13 @@ int launch_profile_dt(Runtime* rt, const void* keys, int64_t n, int which, int w
   const int64_t want = (nvec + (int64_t)kProfThreads * kProfUnroll - 1) / ((int64_t)kProfThreads * kProfUnroll);
   // persistent grid: two CTAs (32 warps) per SM, or fewer when the column is short
   const int blocks = (int)std::max<int64_t>(1, std::min<int64_t>(want, 2LL * rt->sm_count));
-  if (with_hll) profile_kernel<DT, true><<<blocks, kProfThreads, 0, s>>>(keys, n, rt->prof, which);
-  else profile_kernel<DT, false><<<blocks, kProfThreads, 0, s>>>(keys, n, rt->prof, which);
+  if (with_hll) {
+    auto kern = profile_kernel<DT, true>;
+    EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kHllM * 4));
+    kern<<<blocks, kProfThreads, kHllM * 4, s>>>(keys, n, rt->prof, which);
+  } else {
+    profile_kernel<DT, false><<<blocks, kProfThreads, 0, s>>>(keys, n, rt->prof, which);
+  }
   count_launch();
   EIGER_CUDA(cudaGetLastError());
   return EIGER_OK;
