@@ -1,146 +1,23 @@
-// Steps A5-A7: table init, the aggregation kernels (all four variants are one kernel
-// template over a FRONT — what a CTA keeps in shared memory — and a BACK — the table in
-// global memory / L2), and compaction.
+// Steps A5, A6a and A7: table init, the direct-index aggregation kernel (slot = key - min;
+// one kernel template over what a CTA keeps in shared memory in FRONT of the global array)
+// and compaction of either table kind.
 //
-//   EIGER_DIRECT    BACK_DIRECT (slot = u) with FRONT_PRIV (per-thread private cells, no
-//                   atomics; tiny ranges), FRONT_SDIRECT (per-CTA shared-memory array) or
+//   EIGER_DIRECT    FRONT_PRIV (per-thread private cells, no atomics; tiny ranges),
+//                   FRONT_SDIRECT (per-CTA shared-memory array, replicated per warp group) or
 //                   FRONT_NONE (global atomics only; ranges beyond shared memory)
-//   EIGER_SMEM      FRONT_SHASH (per-CTA open addressing in shared memory) + BACK_HASH
-//   EIGER_GLOBAL    FRONT_NONE or a small FRONT_SHASH hot-key cache + BACK_HASH
-//   EIGER_PARTITION partition.cu reorders the rows, then BACK_HASH over KK_U64PRE keys
+//   The hash variants (EIGER_SMEM / EIGER_GLOBAL / EIGER_PARTITION) live in hashagg.cu.
 //
-// GROUP BY semantics: §3.3; hash group-by "perform well when the hash table is
-// cache-resident" PAPER.md:23; emit groups = HT.retrieveAll PAPER.md:184.
+// GROUP BY semantics: §3.3; range test PAPER.md:219 §4.3; emit groups =
+// HT.retrieveAll PAPER.md:184.
 #include <algorithm>
 
 #include "internal.h"
+#include "rows.cuh"
 
 namespace eiger {
 namespace {
 
 constexpr int kAggThreads = 256;
-constexpr int kFrontProbes = 8;
-constexpr int kBackProbes = 4096;
-
-template <int KK> struct KeyTraits;
-template <> struct KeyTraits<KK_I32> { using U = uint32_t; };
-template <> struct KeyTraits<KK_I8I8> { using U = uint32_t; };
-template <> struct KeyTraits<KK_I64> { using U = uint64_t; };
-template <> struct KeyTraits<KK_GEN> { using U = uint64_t; };
-template <> struct KeyTraits<KK_U64PRE> { using U = uint64_t; };
-
-template <class U> __device__ __forceinline__ U empty_of();
-template <> __device__ __forceinline__ uint32_t empty_of<uint32_t>() { return kEmpty32; }
-template <> __device__ __forceinline__ uint64_t empty_of<uint64_t>() { return kEmpty64; }
-
-// ---- key loading ---------------------------------------------------------------------
-template <int KK>
-__device__ __forceinline__ typename KeyTraits<KK>::U load_u(const KeyDesc& k, int64_t i) {
-  using U = typename KeyTraits<KK>::U;
-  if constexpr (KK == KK_I32) {
-    return (U)(ldg_stream_4((const int32_t*)k.ptr[0] + i) - (uint32_t)k.base[0]);
-  } else if constexpr (KK == KK_I64) {
-    return ldg_stream_u64((const int64_t*)k.ptr[0] + i) - k.base[0];
-  } else if constexpr (KK == KK_U64PRE) {
-    return ldg_stream_u64((const uint64_t*)k.ptr[0] + i);
-  } else if constexpr (KK == KK_I8I8) {
-    const uint32_t a = (uint32_t)(int32_t)(int8_t)ldg_stream_1((const int8_t*)k.ptr[0] + i) - (uint32_t)k.base[0];
-    const uint32_t b = (uint32_t)(int32_t)(int8_t)ldg_stream_1((const int8_t*)k.ptr[1] + i) - (uint32_t)k.base[1];
-    return a * (uint32_t)k.mul + b;
-  } else {
-    uint64_t u = sext_load(k.ptr[0], k.dtype[0], i) - k.base[0];
-    if (k.ncols == 2) u = u * k.mul + (sext_load(k.ptr[1], k.dtype[1], i) - k.base[1]);
-    return u;
-  }
-}
-// two consecutive rows starting at an even row index (vector loads)
-template <int KK>
-__device__ __forceinline__ void load_u2(const KeyDesc& k, int64_t i, typename KeyTraits<KK>::U (&u)[2]) {
-  if constexpr (KK == KK_I32) {
-    const uint2 v = ldg_stream_8((const int32_t*)k.ptr[0] + i);
-    u[0] = v.x - (uint32_t)k.base[0]; u[1] = v.y - (uint32_t)k.base[0];
-  } else if constexpr (KK == KK_I64 || KK == KK_U64PRE) {
-    const uint4 v = ldg_stream_16((const uint64_t*)k.ptr[0] + i);
-    const uint64_t b = KK == KK_I64 ? k.base[0] : 0ull;
-    u[0] = (((uint64_t)v.y << 32) | v.x) - b; u[1] = (((uint64_t)v.w << 32) | v.z) - b;
-  } else if constexpr (KK == KK_I8I8) {
-    const uint32_t a = ldg_stream_2((const int8_t*)k.ptr[0] + i), b = ldg_stream_2((const int8_t*)k.ptr[1] + i);
-    const uint32_t b0 = (uint32_t)k.base[0], b1 = (uint32_t)k.base[1], m = (uint32_t)k.mul;
-    u[0] = ((uint32_t)(int32_t)(int8_t)(a & 0xFF) - b0) * m + ((uint32_t)(int32_t)(int8_t)(b & 0xFF) - b1);
-    u[1] = ((uint32_t)(int32_t)(int8_t)(a >> 8) - b0) * m + ((uint32_t)(int32_t)(int8_t)(b >> 8) - b1);
-  } else {
-    u[0] = load_u<KK>(k, i); u[1] = load_u<KK>(k, i + 1);
-  }
-}
-
-// ---- the global hash table (BACK_HASH) -------------------------------------------------
-// Slot s lives at table + s * stride: [u64 key][acc 0]..[acc n-1][pad]; key = ~0 means empty.
-// Slot `cap` is the side slot of the one key whose rebased value equals the empty marker
-// (R18).  Returns the slot's accumulator cells, or nullptr when probing gave up.
-__device__ __forceinline__ uint64_t* back_hash_cells(void* table, uint64_t cap, uint32_t stride,
-                                                     uint64_t u, CallDev* call) {
-  if (u == kEmpty64) {
-    uint64_t* kp = reinterpret_cast<uint64_t*>(static_cast<char*>(table) + cap * stride);
-    if (__ldcg(kp) != 0ull) atomicExch(reinterpret_cast<unsigned long long*>(kp), 0ull);  // mark used
-    return kp + 1;
-  }
-  uint64_t slot = __umul64hi(table_hash64(u), cap);
-  for (int probe = 0; probe < kBackProbes; ++probe) {
-    uint64_t* kp = reinterpret_cast<uint64_t*>(static_cast<char*>(table) + slot * stride);
-    const uint64_t k = __ldcg(kp);
-    if (k == u) return kp + 1;
-    if (k == kEmpty64) {
-      const uint64_t old = atomicCAS(reinterpret_cast<unsigned long long*>(kp), kEmpty64, u);
-      if (old == kEmpty64 || old == u) return kp + 1;
-    }
-    slot = slot + 1 == cap ? 0 : slot + 1;
-  }
-  atomicOr(&call->overflow, 1u);
-  return nullptr;
-}
-
-// ---- shared-memory accumulators ------------------------------------------------------------
-// B200 shared memory has native 32-bit atomics (ATOMS.ADD / ATOMS.MAX, ~2 T/s chip-wide,
-// measured) but 64-bit ones are CAS loops (~0.1-0.3 T/s).  Integer SUM and COUNT cells are
-// therefore kept as two 32-bit planes, lo[S] then hi[S], and added with an explicit carry:
-// the final (hi:lo) equals the wrapping 64-bit sum whatever the interleaving, because every
-// wrap of lo is seen by exactly one atomicAdd's return value.  MIN / MAX and fp64 SUM keep
-// 64-bit cells; MIN / MAX look before they leap, so the CAS loop only runs on a new record.
-__device__ __forceinline__ bool add_type(int op, bool f64) { return op == EIGER_COUNT || (op == EIGER_SUM && !f64); }
-__device__ __forceinline__ void smem_add64(uint32_t* lo, uint32_t* hi, uint64_t v) {
-  const uint32_t vl = (uint32_t)v;
-  const uint32_t old = atomicAdd(lo, vl);
-  const uint32_t h = (uint32_t)(v >> 32) + ((uint32_t)(old + vl) < vl ? 1u : 0u);
-  if (h) atomicAdd(hi, h);
-}
-// accumulator j of a table of S slots that starts at base occupies 8 * S bytes
-__device__ __forceinline__ void smem_merge(unsigned char* base, uint32_t S, int j, uint32_t s, int op, bool f64, uint64_t part) {
-  unsigned char* plane = base + (size_t)j * 8 * S;
-  if (add_type(op, f64)) {
-    uint32_t* lo = reinterpret_cast<uint32_t*>(plane) + s;
-    smem_add64(lo, lo + S, part);
-  } else if (op == EIGER_SUM) {
-    atomicAdd(reinterpret_cast<double*>(plane) + s, __longlong_as_double((long long)part));
-  } else {
-    long long* cell = reinterpret_cast<long long*>(plane) + s;
-    const long long cur = *reinterpret_cast<volatile long long*>(cell);
-    if (op == EIGER_MIN) { if ((long long)part < cur) atomicMin(cell, (long long)part); }
-    else { if ((long long)part > cur) atomicMax(cell, (long long)part); }
-  }
-}
-__device__ __forceinline__ uint64_t smem_read(const unsigned char* base, uint32_t S, int j, uint32_t s, int op, bool f64) {
-  const unsigned char* plane = base + (size_t)j * 8 * S;
-  if (add_type(op, f64)) {
-    const uint32_t* lo = reinterpret_cast<const uint32_t*>(plane) + s;
-    return ((uint64_t)lo[S] << 32) | lo[0];
-  }
-  return reinterpret_cast<const uint64_t*>(plane)[s];
-}
-__device__ __forceinline__ void smem_init_plane(unsigned char* base, uint32_t S, int j, int op, bool f64, int tid, int T) {
-  uint64_t* plane = reinterpret_cast<uint64_t*>(base + (size_t)j * 8 * S);
-  const uint64_t v = add_type(op, f64) ? 0ull : acc_identity(op);
-  for (uint32_t c = tid; c < S; c += T) plane[c] = v;
-}
 
 struct AggArgs {
   KeyDesc key;
@@ -152,11 +29,7 @@ struct AggArgs {
   CallDev* call;
 };
 
-template <int SIG> __device__ __forceinline__ int sig_op(const AggPlan& p, int j) { if constexpr (Sig<SIG>::kStatic) return Sig<SIG>::op(j); else return p.op[j]; }
-template <int SIG> __device__ __forceinline__ int sig_col(const AggPlan& p, int j) { if constexpr (Sig<SIG>::kStatic) return Sig<SIG>::col(j); else return p.col[j]; }
-template <int SIG> __device__ __forceinline__ bool sig_f64(const AggPlan& p, int j) { if constexpr (Sig<SIG>::kStatic) return Sig<SIG>::f64(j); else return p.f64[j] != 0; }
-
-template <int KK, int SIG, int FRONT, int BACK>
+template <int KK, int SIG, int FRONT>
 struct AggCtx {
   using U = typename KeyTraits<KK>::U;
   using S = Sig<SIG>;
@@ -166,17 +39,9 @@ struct AggCtx {
   const AggArgs& a;
   const int n_acc;
   unsigned char* smem;
-  // FRONT_SHASH views
-  U* skeys; uint64_t* sacc; uint32_t* scount;
 
   __device__ AggCtx(const AggArgs& args, unsigned char* sm)
-      : a(args), n_acc(S::kStatic ? S::kAcc : args.plan.n_acc), smem(sm) {
-    if constexpr (FRONT == FRONT_SHASH) {
-      sacc = reinterpret_cast<uint64_t*>(smem);
-      skeys = reinterpret_cast<U*>(sacc + (size_t)n_acc * a.front_slots);
-      scount = reinterpret_cast<uint32_t*>(skeys + a.front_slots);
-    }
-  }
+      : a(args), n_acc(S::kStatic ? S::kAcc : args.plan.n_acc), smem(sm) {}
 
   __device__ void front_init() {
     const int tid = threadIdx.x, T = blockDim.x;
@@ -188,41 +53,12 @@ struct AggCtx {
       for (uint32_t rep = 0; rep < a.front_replicas; ++rep)
         for (int j = 0; j < n_acc; ++j)
           smem_init_plane(smem + (size_t)rep * a.front_slots * 8 * (uint32_t)n_acc, a.front_slots, j, sig_op<SIG>(a.plan, j), sig_f64<SIG>(a.plan, j), tid, T);
-    } else if constexpr (FRONT == FRONT_SHASH) {
-      for (uint32_t c = tid; c < a.front_slots; c += T) skeys[c] = empty_of<U>();
-      for (int j = 0; j < n_acc; ++j)
-        smem_init_plane(reinterpret_cast<unsigned char*>(sacc), a.front_slots, j, sig_op<SIG>(a.plan, j), sig_f64<SIG>(a.plan, j), tid, T);
-      if (tid == 0) *scount = 0;
     }
     if constexpr (FRONT != FRONT_NONE) __syncthreads();
   }
 
-  __device__ __forceinline__ int shash_find(U u) {
-    const uint32_t mask = a.front_slots - 1;
-    uint32_t h;
-    if constexpr (sizeof(U) == 4) h = table_hash32((uint32_t)u) & mask;
-    else { if (u == kEmpty64) return -1; h = (uint32_t)(table_hash64((uint64_t)u) >> 20) & mask; }
-#pragma unroll 1
-    for (int probe = 0; probe < kFrontProbes; ++probe) {
-      const U k = *reinterpret_cast<volatile U*>(skeys + h);
-      if (k == u) return (int)h;
-      if (k == empty_of<U>()) {
-        if (*reinterpret_cast<volatile uint32_t*>(scount) >= a.front_limit) return -1;
-        U old;
-        if constexpr (sizeof(U) == 4) old = atomicCAS(skeys + h, kEmpty32, u);
-        else old = (U)atomicCAS(reinterpret_cast<unsigned long long*>(skeys + h), (unsigned long long)kEmpty64, (unsigned long long)u);
-        if (old == empty_of<U>()) { atomicAdd(scount, 1u); return (int)h; }
-        if (old == u) return (int)h;
-      }
-      h = (h + 1) & mask;
-    }
-    return -1;
-  }
-
   __device__ __forceinline__ void back_row(U u, const uint64_t (&raw)[NV]) {
-    uint64_t* cells;
-    if constexpr (BACK == BACK_DIRECT) cells = static_cast<uint64_t*>(a.table) + (uint64_t)u * (uint32_t)n_acc;
-    else { cells = back_hash_cells(a.table, a.cap, a.stride, (uint64_t)u, a.call); if (!cells) return; }
+    uint64_t* cells = static_cast<uint64_t*>(a.table) + (uint64_t)u * (uint32_t)n_acc;
 #pragma unroll
     for (int j = 0; j < NA; ++j) {
       if (!S::kStatic && j >= n_acc) break;
@@ -249,15 +85,6 @@ struct AggCtx {
         if (!S::kStatic && j >= n_acc) break;
         const int op = sig_op<SIG>(a.plan, j); const bool f = sig_f64<SIG>(a.plan, j);
         smem_merge(base, a.front_slots, j, (uint32_t)u, op, f, row_partial(op, f, raw[sig_col<SIG>(a.plan, j)]));
-      }
-    } else if constexpr (FRONT == FRONT_SHASH) {
-      const int h = shash_find(u);
-      if (h < 0) { back_row(u, raw); return; }
-#pragma unroll
-      for (int j = 0; j < NA; ++j) {
-        if (!S::kStatic && j >= n_acc) break;
-        const int op = sig_op<SIG>(a.plan, j); const bool f = sig_f64<SIG>(a.plan, j);
-        smem_merge(reinterpret_cast<unsigned char*>(sacc), a.front_slots, j, (uint32_t)h, op, f, row_partial(op, f, raw[sig_col<SIG>(a.plan, j)]));
       }
     } else {
       back_row(u, raw);
@@ -296,24 +123,15 @@ struct AggCtx {
                                      sig_op<SIG>(a.plan, (int)j), sig_f64<SIG>(a.plan, (int)j));
         back_merge(u, (int)j, v, static_cast<uint64_t*>(a.table) + (uint64_t)u * (uint32_t)n_acc);
       }
-    } else if constexpr (FRONT == FRONT_SHASH) {
-      for (uint32_t h = tid; h < a.front_slots; h += T) {
-        const U k = skeys[h];
-        if (k == empty_of<U>()) continue;
-        uint64_t* cells = back_hash_cells(a.table, a.cap, a.stride, (uint64_t)k, a.call);
-        if (!cells) continue;
-        for (int j = 0; j < n_acc; ++j)
-          back_merge((uint64_t)k, j, smem_read(reinterpret_cast<const unsigned char*>(sacc), a.front_slots, j, h, sig_op<SIG>(a.plan, j), sig_f64<SIG>(a.plan, j)), cells);
-      }
     }
   }
 };
 
-template <int KK, int SIG, int FRONT, int BACK>
+template <int KK, int SIG, int FRONT>
 __global__ void __launch_bounds__(kAggThreads)
 aggregate_kernel(const __grid_constant__ AggArgs a) {
   extern __shared__ __align__(16) unsigned char smem[];
-  using Ctx = AggCtx<KK, SIG, FRONT, BACK>;
+  using Ctx = AggCtx<KK, SIG, FRONT>;
   using U = typename Ctx::U;
   constexpr int NV = Ctx::NV;
   constexpr int UNR = !Sig<SIG>::kStatic ? 1 : (NV >= 4 ? 2 : 4);
@@ -421,9 +239,9 @@ __global__ void __launch_bounds__(256) compact_kernel(const __grid_constant__ Co
 }
 
 // ---- dispatch --------------------------------------------------------------------------------
-template <int KK, int SIG, int FRONT, int BACK>
+template <int KK, int SIG, int FRONT>
 int launch_one(const AggLaunch& L, cudaStream_t s) {
-  auto kern = aggregate_kernel<KK, SIG, FRONT, BACK>;
+  auto kern = aggregate_kernel<KK, SIG, FRONT>;
   if (L.smem_bytes > 48 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
   AggArgs a;
   a.key = L.key; a.plan = L.plan; a.n = L.n;
@@ -437,21 +255,12 @@ int launch_one(const AggLaunch& L, cudaStream_t s) {
 
 template <int KK, int SIG>
 int launch_fb(const AggLaunch& L, cudaStream_t s) {
-  if (L.back == BACK_DIRECT) {
-    if constexpr (KK == KK_U64PRE) return EIGER_ERR_ARG;
-    else switch (L.front) {
-      case FRONT_NONE: return launch_one<KK, SIG, FRONT_NONE, BACK_DIRECT>(L, s);
-      case FRONT_PRIV: return launch_one<KK, SIG, FRONT_PRIV, BACK_DIRECT>(L, s);
-      case FRONT_SDIRECT: return launch_one<KK, SIG, FRONT_SDIRECT, BACK_DIRECT>(L, s);
-      default: return EIGER_ERR_ARG;
-    }
-  } else {
-    if constexpr (KK == KK_I8I8) return EIGER_ERR_ARG;
-    else switch (L.front) {
-      case FRONT_NONE: return launch_one<KK, SIG, FRONT_NONE, BACK_HASH>(L, s);
-      case FRONT_SHASH: return launch_one<KK, SIG, FRONT_SHASH, BACK_HASH>(L, s);
-      default: return EIGER_ERR_ARG;
-    }
+  if (L.back != BACK_DIRECT) return EIGER_ERR_ARG;
+  switch (L.front) {
+    case FRONT_NONE: return launch_one<KK, SIG, FRONT_NONE>(L, s);
+    case FRONT_PRIV: return launch_one<KK, SIG, FRONT_PRIV>(L, s);
+    case FRONT_SDIRECT: return launch_one<KK, SIG, FRONT_SDIRECT>(L, s);
+    default: return EIGER_ERR_ARG;
   }
 }
 
@@ -471,8 +280,8 @@ int launch_sig(const AggLaunch& L, cudaStream_t s) {
 
 bool aggregate_supported(int key_kind, int sig, int front, int back) {
   (void)sig;
-  if (back == BACK_DIRECT) return key_kind != KK_U64PRE && front != FRONT_SHASH;
-  return key_kind != KK_I8I8 && (front == FRONT_NONE || front == FRONT_SHASH);
+  return back == BACK_DIRECT && key_kind != KK_U64PRE && key_kind != KK_U32PRE &&
+         (front == FRONT_NONE || front == FRONT_PRIV || front == FRONT_SDIRECT);
 }
 
 int launch_aggregate(const AggLaunch& L, cudaStream_t s) {
@@ -482,7 +291,6 @@ int launch_aggregate(const AggLaunch& L, cudaStream_t s) {
     case KK_I64: return launch_sig<KK_I64>(L, s);
     case KK_I8I8: return launch_sig<KK_I8I8>(L, s);
     case KK_GEN: return launch_sig<KK_GEN>(L, s);
-    case KK_U64PRE: return launch_sig<KK_U64PRE>(L, s);
     default: return EIGER_ERR_ARG;
   }
 }

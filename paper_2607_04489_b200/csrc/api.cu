@@ -62,27 +62,36 @@ inline bool is_key_dtype(int d) { return d == EIGER_I8 || d == EIGER_I32 || d ==
 inline int dtype_size(int d) { return d == EIGER_I8 ? 1 : d == EIGER_I32 ? 4 : 8; }
 
 // Tunables of step A4; EIGER_* environment variables override them
-// for the crossover sweeps.
+// for the crossover sweeps.  Re-read on every call so that a sweep can change them in-process.
 struct Tunables {
   size_t priv_smem = 96 * 1024;       // FRONT_PRIV: private cells of one CTA
   size_t sdirect_bytes = 160 * 1024;  // FRONT_SDIRECT: largest per-CTA direct array
   size_t sdirect_replica_budget = 64 * 1024;
-  size_t shash_bytes = 96 * 1024;     // FRONT_SHASH table per CTA
-  size_t direct_l2_bytes = 48ull << 20;   // AUTO takes DIRECT/global-atomics up to this table size
-  size_t global_l2_bytes = 64ull << 20;   // AUTO takes GLOBAL up to this table size
-  size_t part_target_bytes = 24ull << 20; // PARTITION: table slice per partition
-  double load = 0.5;
-  int global_front = 1;               // hot-key cache in front of the global table
+  size_t smem_table_bytes;            // EIGER_SMEM / EIGER_GLOBAL: shared-memory table of one CTA (1 CTA per SM)
+  int smem_threads;
+  size_t part_table_bytes;            // EIGER_PARTITION: shared-memory table of one CTA
+  int part_threads;
+  int part_min_bits;                  // at least this many partitions (parallelism of the emit pass)
+  size_t direct_l2_bytes;             // AUTO takes DIRECT with global atomics up to this table size
+  size_t global_l2_bytes;             // AUTO takes GLOBAL up to this table size
+  double load;                        // target load factor of every hash table
+  double smem_fill;                   // AUTO takes EIGER_SMEM while ndv <= smem_fill * slots
+  int global_front;                   // hot-key shared-memory table in front of the global table
   Tunables() {
     auto env = [](const char* k, double dflt) { const char* v = std::getenv(k); return v ? std::atof(v) : dflt; };
+    smem_table_bytes = (size_t)env("EIGER_SMEM_KB", 200) << 10;
+    smem_threads = (int)env("EIGER_SMEM_THREADS", 1024);
+    part_table_bytes = (size_t)env("EIGER_PART_KB", 100) << 10;
+    part_threads = (int)env("EIGER_PART_THREADS", 512);
+    part_min_bits = (int)env("EIGER_PART_MIN_BITS", 9);
     direct_l2_bytes = (size_t)env("EIGER_DIRECT_L2_MB", 48) << 20;
     global_l2_bytes = (size_t)env("EIGER_GLOBAL_L2_MB", 64) << 20;
-    part_target_bytes = (size_t)env("EIGER_PART_MB", 24) << 20;
     global_front = (int)env("EIGER_GLOBAL_FRONT", 1);
     load = env("EIGER_LOAD", 0.5);
+    smem_fill = env("EIGER_SMEM_FILL", 0.6);
   }
 };
-const Tunables& tun() { static Tunables t; return t; }
+Tunables tun() { return Tunables(); }
 
 struct QueryPlan {
   int variant = 0, key_kind = 0, sig = 0, front = 0, back = 0;
@@ -92,18 +101,21 @@ struct QueryPlan {
   int val_src[kMaxVals];        // plan value slot -> caller's value column
   uint64_t R = 0;               // fused key range; 0 = 2^64 (or not representable)
   double ndv = 0;
+  // direct
   uint32_t front_slots = 0, front_limit = 0, front_replicas = 1;
+  // hash variants
+  uint32_t slots = 0, limit = 0;
+  int threads = 0;
+  int bits1 = 0, bits2 = 0;
   size_t smem_bytes = 0;
   uint64_t cap = 0, cap_bound = 0;
   uint32_t stride = 0;
-  int part_bits = 0;
   size_t table_bytes = 0, part_bytes = 0, total_bytes = 0;
 };
 
 uint64_t range_of(const eiger_stats& s) {   // max - min + 1, 0 when it is 2^64
   return (uint64_t)s.max - (uint64_t)s.min + 1ull;
 }
-uint32_t floor_pow2(uint64_t x) { uint32_t p = 1; while ((uint64_t)p * 2 <= x && p < (1u << 30)) p *= 2; return p; }
 
 int detect_sig(const AggPlan& p, int n_user) {
   auto is = [&](int j, int op, int col, int f) { return p.op[j] == op && (op == EIGER_COUNT || (p.col[j] == col && p.f64[j] == f)); };
@@ -183,17 +195,17 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   q->ndv = ndv;
   q->cap_bound = (uint64_t)std::max(1.0, std::ceil(bound / tun().load)) + 64;
 
-  const Tunables& T = tun();
+  const Tunables T = tun();
   const int n_acc_direct = na + (has_count ? 0 : 1);
   const bool direct_ok = R != 0 && R <= (1ull << 33);
   const unsigned __int128 direct_bytes = (unsigned __int128)R * 8 * n_acc_direct;
 
-  // FRONT_SHASH geometry
-  const int key_kind_hash = (nk == 1 && keys[0].dtype == EIGER_I32 && R != 0 && R <= 0xFFFFFFFFull) ? KK_I32
-                            : (nk == 1 && keys[0].dtype == EIGER_I64) ? KK_I64 : KK_GEN;
-  const size_t ubytes = key_kind_hash == KK_I32 ? 4 : 8;
-  const size_t shash_slot = 8 * (size_t)na + ubytes;
-  const uint32_t shash_slots = floor_pow2(T.shash_bytes / shash_slot);
+  // hash variants: key kind, shared-memory slot size, global slot stride
+  const int hk = (nk == 1 && keys[0].dtype == EIGER_I32 && R != 0 && R <= 0xFFFFFFFFull) ? KK_I32
+                 : (nk == 1 && keys[0].dtype == EIGER_I64) ? KK_I64 : KK_GEN;
+  const size_t slot_bytes = hash_agg_slot_bytes(p, hk);
+  const uint32_t smem_slots = (uint32_t)std::max<size_t>(64, (T.smem_table_bytes - 64) / slot_bytes) & ~7u;   // planes stay 8-byte aligned
+  const uint32_t part_slots = (uint32_t)std::max<size_t>(64, (T.part_table_bytes - 64) / slot_bytes) & ~7u;
   const uint32_t hash_stride = [&] { uint32_t s = 16; while (s < 8u * (1 + na)) s *= 2; return s; }();
   auto hash_cap = [&](double g) { return (uint64_t)std::max(1024.0, std::ceil(g * (1.0 + 4 * kSigma) * 1.02 / T.load)); };
 
@@ -201,7 +213,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   if (variant == EIGER_AUTO) {
     if (direct_ok && (direct_bytes * 256 <= T.priv_smem || direct_bytes <= T.sdirect_bytes ||
                       (direct_bytes <= T.direct_l2_bytes && (double)R <= 16.0 * (double)std::max<int64_t>(n, 1)))) variant = EIGER_DIRECT;
-    else if (ndv * (1.0 + 4 * kSigma) <= 0.5 * shash_slots) variant = EIGER_SMEM;
+    else if (ndv * (1.0 + 4 * kSigma) <= T.smem_fill * smem_slots) variant = EIGER_SMEM;
     else if ((unsigned __int128)hash_cap(ndv) * hash_stride <= T.global_l2_bytes) variant = EIGER_GLOBAL;
     else variant = EIGER_PARTITION;
   }
@@ -225,34 +237,40 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
     } else {
       q->front = FRONT_NONE;
     }
+    q->sig = detect_sig(p, na);
+    if (!aggregate_supported(q->key_kind, q->sig, q->front, q->back)) return EIGER_ERR_INFEASIBLE;
   } else {
     q->back = BACK_HASH;
     q->stride = hash_stride;
-    q->cap = std::min(hash_cap(ndv), q->cap_bound);
-    q->key_kind = key_kind_hash;
-    const bool want_front = variant == EIGER_SMEM || ((variant == EIGER_GLOBAL || variant == EIGER_PARTITION) && T.global_front);
+    q->key_kind = hk;
+    q->sig = detect_sig(p, na);
     if (variant == EIGER_PARTITION) {
-      q->key_kind = KK_U64PRE;
-      const double tb = (double)q->cap * q->stride;
-      int bits = 1;
-      while (bits < 12 && tb / (double)(1u << bits) > (double)T.part_target_bytes) ++bits;
-      q->part_bits = bits;
-      const size_t P = (size_t)1 << bits;
-      q->part_bytes = align_up(P * 4, 256) + align_up(P * 8, 256) + (size_t)(1 + p.n_vals) * align_up((size_t)n * 8, 256);
-    }
-    if (want_front) {
-      const size_t ub = q->key_kind == KK_I32 ? 4 : 8;
-      q->front = FRONT_SHASH;
-      q->front_slots = floor_pow2(T.shash_bytes / (8 * (size_t)na + ub));
-      q->front_limit = q->front_slots / 2;
-      q->smem_bytes = align_up((size_t)q->front_slots * (8 * (size_t)na + ub) + 16, 16);
+      if (n >= (1ll << 32)) return EIGER_ERR_INFEASIBLE;     // 32-bit per-partition counts
+      q->threads = T.part_threads; q->slots = part_slots; q->limit = (uint32_t)(0.85 * part_slots);
+      const double per = std::max(1.0, T.load * part_slots);
+      const double need = ndv * (1.0 + 4 * kSigma) / per;
+      int bits = T.part_min_bits;
+      while (bits < 20 && (double)(1u << bits) < need) ++bits;
+      const int mb = partition_max_bits_per_level();
+      if (bits <= mb) { q->bits1 = bits; q->bits2 = 0; } else { q->bits1 = (bits + 1) / 2; q->bits2 = bits - q->bits1; }
+      // the global table only takes what overflows a partition's shared-memory table
+      q->cap = std::min(q->cap_bound, (uint64_t)std::max(4096.0, ndv / 64.0));
+      const size_t P1 = (size_t)1 << q->bits1, P = (size_t)1 << (q->bits1 + q->bits2);
+      const size_t kb = hk == KK_I32 ? 4 : 8;
+      const size_t col = align_up((size_t)n * 8, 256), kcol = align_up((size_t)n * kb, 256);
+      q->part_bytes = align_up(P * 4, 256) + align_up((P1 + 1) * 8, 256) + align_up(P1 * 8, 256) +
+                      (kcol + (size_t)p.n_vals * col);
+      if (q->bits2 > 0) q->part_bytes += align_up((P + 1) * 8, 256) + align_up(P * 8, 256) + (kcol + (size_t)p.n_vals * col);
     } else {
-      q->front = FRONT_NONE;
+      q->threads = T.smem_threads;
+      const bool front = variant == EIGER_SMEM || T.global_front;
+      q->slots = front ? smem_slots : 64;
+      q->limit = front ? (uint32_t)(0.75 * smem_slots) : 0;
+      q->cap = std::min(hash_cap(ndv), q->cap_bound);
     }
+    q->smem_bytes = align_up((size_t)q->slots * slot_bytes + 64, 16);
     q->table_bytes = align_up((size_t)(q->cap + 1) * q->stride, 256);
   }
-  q->sig = detect_sig(p, na);
-  if (!aggregate_supported(q->key_kind, q->sig, q->front, q->back)) return EIGER_ERR_INFEASIBLE;
   q->total_bytes = q->table_bytes + q->part_bytes + 256;
   (void)rt;
   return EIGER_OK;
@@ -322,9 +340,11 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
   if ((uintptr_t)workspace & 255) return EIGER_ERR_ARG;
 
   char* ws = static_cast<char*>(workspace);
-  struct Back { unsigned long long n_groups; uint32_t overflow; uint32_t pad; };
+  struct Back { unsigned long long n_groups; uint32_t overflow; uint32_t abort; };
   Back* hb = reinterpret_cast<Back*>(static_cast<char*>(rt->pinned) + 1024);
 
+  for (int j = 0; j < na; ++j) if (!out_aggs[j] && out_capacity > 0) return EIGER_ERR_ARG;
+  const int src_kind = q.key_kind;
   for (int attempt = 0;; ++attempt) {
     // workspace: [table][partition scratch]
     void* table = ws;
@@ -338,37 +358,60 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     L.threads = 256; L.smem_bytes = q.smem_bytes;
     { Timed t(s, 3); rc = launch_table_init(L, s); if (rc) return rc; }
 
-    if (q.variant == EIGER_PARTITION) {
-      PartitionLaunch P{};
-      P.key = q.key; P.plan = q.plan; P.n = n; P.bits = q.part_bits;
-      P.key_kind = (nk == 1 && keys[0].dtype == EIGER_I32 && q.R != 0 && q.R <= 0xFFFFFFFFull) ? KK_I32
-                   : (nk == 1 && keys[0].dtype == EIGER_I64) ? KK_I64 : KK_GEN;
-      const size_t np = (size_t)1 << q.part_bits;
-      P.hist = reinterpret_cast<uint32_t*>(pws); pws += align_up(np * 4, 256);
-      P.cursor = reinterpret_cast<unsigned long long*>(pws); pws += align_up(np * 8, 256);
-      P.out_u = reinterpret_cast<uint64_t*>(pws); pws += align_up((size_t)n * 8, 256);
-      for (int c = 0; c < q.plan.n_vals; ++c) { P.out_vals[c] = reinterpret_cast<uint64_t*>(pws); pws += align_up((size_t)n * 8, 256); }
-      { Timed t(s, 2); rc = launch_partition(P, rt->sm_count, s); if (rc) return rc; }
-      // the aggregation pass reads the partitioned copy
-      L.key.ptr[0] = P.out_u; L.key.ncols = 1; L.key.base[0] = 0; L.key.mul = 1;
-      for (int c = 0; c < q.plan.n_vals; ++c) L.plan.vals[c] = P.out_vals[c];
-    }
-
-    // persistent grid: as many CTAs as fit, never more than there are tiles
-    int occ = 1;
-    {
+    if (q.variant == EIGER_DIRECT) {
+      // persistent grid: as many CTAs as fit, never more than there are tiles
       const size_t per_cta = std::max<size_t>(q.smem_bytes, 1024);
-      occ = (int)std::min<size_t>(8, std::max<size_t>(1, (rt->smem_optin + 1024) / (per_cta + 1024)));
+      int occ = (int)std::min<size_t>(8, std::max<size_t>(1, (rt->smem_optin + 1024) / (per_cta + 1024)));
       if (q.front == FRONT_NONE) occ = 8;
+      const int64_t tiles = std::max<int64_t>(1, (n + 1023) / 1024);
+      L.blocks = (int)std::min<int64_t>((int64_t)rt->sm_count * occ, tiles);
+      { Timed t(s, 0); rc = launch_aggregate(L, s); if (rc) return rc; }
+    } else {
+      HashAggLaunch H{};
+      H.key = q.key; H.plan = q.plan; H.n = n; H.key_kind = src_kind; H.sig = q.sig;
+      H.slots = q.slots; H.limit = q.limit; H.spec = 0;
+      H.table = table; H.cap = q.cap; H.stride = q.stride; H.call = rt->call;
+      H.out_keys[0] = out_keys[0]; H.out_keys[1] = nk == 2 ? out_keys[1] : nullptr;
+      for (int j = 0; j < na; ++j) H.out_aggs[j] = out_aggs[j];
+      H.n_out_aggs = na; H.out_capacity = out_capacity;
+      H.threads = q.threads; H.smem_bytes = q.smem_bytes;
+      if (q.variant == EIGER_PARTITION) {
+        PartitionLaunch P{};
+        P.key = q.key; P.plan = q.plan; P.n = n; P.key_kind = src_kind; P.bits1 = q.bits1; P.bits2 = q.bits2;
+        const size_t P1 = (size_t)1 << q.bits1, PP = (size_t)1 << (q.bits1 + q.bits2);
+        const size_t kb = src_kind == KK_I32 ? 4 : 8;
+        const size_t col = align_up((size_t)n * 8, 256), kcol = align_up((size_t)n * kb, 256);
+        auto take = [&](size_t bytes) { char* r = pws; pws += align_up(bytes, 256); return r; };
+        P.hist = reinterpret_cast<uint32_t*>(take(PP * 4));
+        P.off1 = reinterpret_cast<unsigned long long*>(take((P1 + 1) * 8));
+        P.cur1 = reinterpret_cast<unsigned long long*>(take(P1 * 8));
+        P.keysA = take(kcol);
+        for (int c = 0; c < q.plan.n_vals; ++c) P.valsA[c] = reinterpret_cast<uint64_t*>(take(col));
+        if (q.bits2 > 0) {
+          P.off2 = reinterpret_cast<unsigned long long*>(take((PP + 1) * 8));
+          P.cur2 = reinterpret_cast<unsigned long long*>(take(PP * 8));
+          P.keysB = take(kcol);
+          for (int c = 0; c < q.plan.n_vals; ++c) P.valsB[c] = reinterpret_cast<uint64_t*>(take(col));
+        }
+        { Timed t(s, 2); rc = launch_partition(P, rt->sm_count, s); if (rc) return rc; }
+        // the aggregation pass reads the partitioned copy, one CTA per partition at a time
+        H.key.ptr[0] = P.out_keys;
+        for (int c = 0; c < q.plan.n_vals; ++c) H.plan.vals[c] = P.out_vals[c];
+        H.key_kind = src_kind == KK_I32 ? KK_U32PRE : KK_U64PRE;
+        H.part_off = P.out_off; H.n_parts = P.n_parts;
+        const int occ = (int)std::max<size_t>(1, std::min<size_t>((size_t)(2048 / q.threads), (rt->smem_optin + 1024) / (q.smem_bytes + 1024)));
+        H.blocks = (int)std::min<int64_t>((int64_t)rt->sm_count * occ, P.n_parts);
+      } else {
+        const int64_t tiles = std::max<int64_t>(1, n / (4 * (int64_t)q.threads));
+        H.blocks = (int)std::min<int64_t>(rt->sm_count, tiles);
+      }
+      { Timed t(s, 0); rc = launch_hash_agg(H, s); if (rc) return rc; }
     }
-    const int64_t tiles = std::max<int64_t>(1, (n + 1023) / 1024);
-    L.blocks = (int)std::min<int64_t>((int64_t)rt->sm_count * occ, tiles);
-    { Timed t(s, 0); rc = launch_aggregate(L, s); if (rc) return rc; }
 
     CompactLaunch C{};
     C.key = q.key; C.plan = q.plan; C.back = q.back; C.table = table; C.cap = q.cap; C.stride = q.stride;
     C.out_keys[0] = out_keys[0]; C.out_keys[1] = nk == 2 ? out_keys[1] : nullptr;
-    for (int j = 0; j < na; ++j) { if (!out_aggs[j] && out_capacity > 0) return EIGER_ERR_ARG; C.out_aggs[j] = out_aggs[j]; }
+    for (int j = 0; j < na; ++j) C.out_aggs[j] = out_aggs[j];
     C.n_out_aggs = na; C.out_capacity = out_capacity; C.call = rt->call;
     { Timed t(s, 4); rc = launch_compact(C, rt->sm_count, s); if (rc) return rc; }
 
@@ -377,12 +420,23 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     resolve_timing();
     if (hb->overflow) {
       // the sketch under-estimated (R10): grow towards the exact bound and run again
-      if (q.back != BACK_HASH || q.cap >= q.cap_bound || attempt >= 8) return EIGER_ERR_TABLE_OVERFLOW;
+      if (q.back != BACK_HASH || attempt >= 8) return EIGER_ERR_TABLE_OVERFLOW;
+      if (q.cap >= q.cap_bound && q.variant != EIGER_PARTITION) return EIGER_ERR_TABLE_OVERFLOW;
       q.cap = std::min(q.cap_bound, q.cap * 4);
-      const size_t old_total = q.total_bytes;
       q.table_bytes = align_up((size_t)(q.cap + 1) * q.stride, 256);
+      if (q.variant == EIGER_PARTITION) {
+        // more partitions as well: re-plan the fan-out for four times the estimate
+        eiger_stats grown[2] = {st[0], st[nk == 2 ? 1 : 0]};
+        grown[0].ndv_est = std::min((double)n, std::max(q.ndv, 1.0) * 4.0); if (nk == 2) grown[1].ndv_est = 1.0;
+        QueryPlan q2;
+        rc = plan_query(rt, keys, nk, n, vals, nv, aggs, na, grown, EIGER_PARTITION, &q2);
+        if (rc) return rc;
+        q2.cap = std::max(q2.cap, q.cap); q2.table_bytes = align_up((size_t)(q2.cap + 1) * q2.stride, 256);
+        q2.total_bytes = q2.table_bytes + q2.part_bytes + 256;
+        q = q2;
+      }
       q.total_bytes = q.table_bytes + q.part_bytes + 256;
-      if (q.total_bytes > workspace_bytes) { (void)old_total; return EIGER_ERR_TABLE_OVERFLOW; }
+      if (q.total_bytes > workspace_bytes) return EIGER_ERR_TABLE_OVERFLOW;
       continue;
     }
     *n_groups = (int64_t)hb->n_groups;

@@ -20,7 +20,7 @@ constexpr uint32_t kEmpty32 = ~0u;
 
 // How the key column(s) are read.  u = rebased, fused key (frame of reference +
 // positional packing): u = (k0 - min0) * mul + (k1 - min1).
-enum KeyKind : int { KK_I32 = 0, KK_I64 = 1, KK_I8I8 = 2, KK_GEN = 3, KK_U64PRE = 4 };
+enum KeyKind : int { KK_I32 = 0, KK_I64 = 1, KK_I8I8 = 2, KK_GEN = 3, KK_U64PRE = 4, KK_U32PRE = 5 };
 
 struct KeyDesc {
   const void* ptr[2];
@@ -148,6 +148,13 @@ __device__ __forceinline__ uint32_t table_hash32(uint32_t u) {
   uint32_t h = u * 0x9E3779B1u;
   h = (h ^ (h >> 15)) * 0x85EBCA77u;
   return h ^ (h >> 13);
+}
+// a second, independent 32-bit hash: table_hash32's top bits choose the partition, this one
+// the slot inside the partition's shared-memory table
+__device__ __forceinline__ uint32_t table_hash32b(uint32_t u) {
+  uint32_t h = (u ^ (u >> 16)) * 0x7FEB352Du;
+  h = (h ^ (h >> 15)) * 0x846CA68Bu;
+  return h ^ (h >> 16);
 }
 
 // ---- accumulator algebra -------------------------------------------------------------

@@ -18,7 +18,7 @@ struct ProfileDev {
 struct CallDev {
   unsigned long long n_groups;   // compaction claim counter
   uint32_t overflow;             // a hash table ran out of probes
-  uint32_t pad;
+  uint32_t abort;                // speculative pass: some CTA's shared-memory table filled up
 };
 
 struct Runtime {
@@ -82,18 +82,44 @@ struct CompactLaunch {
 };
 int launch_compact(const CompactLaunch& c, int sm_count, cudaStream_t s);
 
+// ---- hashagg.cu -------------------------------------------------------------------------
+struct HashAggLaunch {
+  KeyDesc key;              // whole-input mode: the caller's columns; partition mode: ptr[0] = partitioned keys
+  AggPlan plan;             // value column pointers (partition mode: the partitioned copies)
+  int64_t n;
+  int key_kind, sig;
+  const unsigned long long* part_off;   // partition mode only: [n_parts + 1]
+  int n_parts;
+  uint32_t slots, limit;    // shared-memory table of each CTA
+  int spec;                 // speculative run (EIGER_AUTO without statistics)
+  void* table; uint64_t cap; uint32_t stride;   // global table (BACK_HASH layout)
+  CallDev* call;
+  void* out_keys[2]; void* out_aggs[kMaxAggs]; int n_out_aggs; int64_t out_capacity;   // partition mode emits
+  int threads, blocks;
+  size_t smem_bytes;
+};
+int launch_hash_agg(const HashAggLaunch& L, cudaStream_t s);
+size_t hash_agg_slot_bytes(const AggPlan& p, int key_kind);   // shared-memory bytes per slot
+
 // ---- partition.cu ----------------------------------------------------------------------
 struct PartitionLaunch {
   KeyDesc key;
   AggPlan plan;             // value column pointers
   int64_t n;
-  int key_kind;
-  int bits;                 // P = 2^bits partitions, taken from the top bits of table_hash64(u)
-  uint32_t* hist;           // [P]   device, zeroed by the launcher
-  unsigned long long* cursor;  // [P] device
-  uint64_t* out_u;          // [n] rebased fused keys in partition order
-  uint64_t* out_vals[kMaxVals];  // [n] per value column
+  int key_kind;             // KK_I32 (keys stay 32-bit), KK_I64 or KK_GEN
+  int bits1, bits2;         // fan-out 2^bits1 x 2^bits2 from the top bits of the table hash; bits2 = 0: one level
+  // workspace carved by the caller
+  uint32_t* hist;           // [2^(bits1 + bits2)]
+  unsigned long long* off1; // [2^bits1 + 1]
+  unsigned long long* cur1; // [2^bits1]
+  unsigned long long* off2; // [2^(bits1 + bits2) + 1]   (two levels)
+  unsigned long long* cur2; // [2^(bits1 + bits2)]
+  void* keysA; uint64_t* valsA[kMaxVals];   // level-1 output, n rows each
+  void* keysB; uint64_t* valsB[kMaxVals];   // level-2 output
+  // results
+  const void* out_keys; uint64_t* const* out_vals; const unsigned long long* out_off; int n_parts;
 };
-int launch_partition(const PartitionLaunch& p, int sm_count, cudaStream_t s);
+int launch_partition(PartitionLaunch& p, int sm_count, cudaStream_t s);
+int partition_max_bits_per_level();
 
 }  // namespace eiger

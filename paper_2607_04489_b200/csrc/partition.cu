@@ -1,153 +1,276 @@
 // Step A6d, first half: radix partition of the rows by the top bits of the table hash
 // ("applies a hash function to the keys before partitioning to ensure more even partition
 // sizes", §3.3; best for g > 2^20).  Keys leave this pass
-// already rebased and fused (KK_U64PRE); value columns travel with their keys (the paper's
-// GFTR).  Because the global table's slot is mulhi(hash, cap), rows of one
-// partition land in one contiguous slice of the table, which is what keeps the following
-// BACK_HASH pass inside L2.
+// already rebased and fused (KK_U32PRE / KK_U64PRE); value columns travel with their keys
+// (the paper's GFTR).
+//
+// One level = histogram (keys only) -> exclusive scan -> scatter.  The scatter stages every
+// tile in shared memory in partition order first, so that what leaves the SM are runs of
+// consecutive rows of one partition, not one 8-byte store per lane.  Two levels (fan-out
+// P1 x P2) are chained when the final partition count exceeds what one staged pass writes
+// efficiently; level 2 runs per level-1 partition (blockIdx.y) over the level-1 output.
 #include <algorithm>
 
 #include "internal.h"
+#include "rows.cuh"
 
 namespace eiger {
 namespace {
 
-constexpr int kPartThreads = 256;
-constexpr int kPartRows = 8;              // rows per thread per tile
-constexpr int kMaxPartBits = 12;
+constexpr int kPT = 512;                  // threads per CTA
+constexpr int kPR = 8;                    // rows per thread per tile
+constexpr int kTile = kPT * kPR;          // 4096 rows staged per tile
+constexpr int kMaxFan = 1024;             // partitions per level
 
-template <int KK> struct PK;
-template <> struct PK<KK_I32> { using U = uint32_t; };
-template <> struct PK<KK_I64> { using U = uint64_t; };
-template <> struct PK<KK_GEN> { using U = uint64_t; };
+template <int KK> struct SrcKey { using U = typename KeyTraits<KK>::U; };
 
-template <int KK>
-__device__ __forceinline__ uint64_t part_load_u(const KeyDesc& k, int64_t i) {
-  if constexpr (KK == KK_I32) return (uint64_t)(uint32_t)(ldg_stream_4((const int32_t*)k.ptr[0] + i) - (uint32_t)k.base[0]);
-  else if constexpr (KK == KK_I64) return ldg_stream_u64((const int64_t*)k.ptr[0] + i) - k.base[0];
-  else {
-    uint64_t u = sext_load(k.ptr[0], k.dtype[0], i) - k.base[0];
-    if (k.ncols == 2) u = u * k.mul + (sext_load(k.ptr[1], k.dtype[1], i) - k.base[1]);
-    return u;
-  }
+// partition hash: 32-bit keys hash in 32 bits, 64-bit keys in 64; ids come from the top bits
+template <class U> __device__ __forceinline__ uint32_t part_id(U u, int shift, uint32_t mask);
+template <> __device__ __forceinline__ uint32_t part_id<uint32_t>(uint32_t u, int shift, uint32_t mask) {
+  return (table_hash32(u) >> shift) & mask;
+}
+template <> __device__ __forceinline__ uint32_t part_id<uint64_t>(uint64_t u, int shift, uint32_t mask) {
+  return (uint32_t)(table_hash64(u) >> shift) & mask;
 }
 
-template <int KK>
-__global__ void __launch_bounds__(kPartThreads)
-partition_hist_kernel(const __grid_constant__ KeyDesc key, int64_t n, int bits, uint32_t* __restrict__ hist) {
-  __shared__ uint32_t s_hist[1 << kMaxPartBits];
-  const int P = 1 << bits;
-  for (int p = threadIdx.x; p < P; p += kPartThreads) s_hist[p] = 0;
-  __syncthreads();
-  const int64_t stride = (int64_t)gridDim.x * kPartThreads;
-  for (int64_t i = (int64_t)blockIdx.x * kPartThreads + threadIdx.x; i < n; i += stride) {
-    const uint64_t u = part_load_u<KK>(key, i);
-    atomicAdd(&s_hist[(uint32_t)(table_hash64(u) >> (64 - bits))], 1u);
-  }
-  __syncthreads();
-  for (int p = threadIdx.x; p < P; p += kPartThreads) if (s_hist[p]) atomicAdd(&hist[p], s_hist[p]);
-}
-
-// exclusive prefix sum of P <= 4096 counts -> 64-bit write cursors
-__global__ void partition_scan_kernel(const uint32_t* __restrict__ hist, unsigned long long* __restrict__ cursor, int P) {
-  __shared__ unsigned long long s_part[1024];
-  const int per = (P + 1023) / 1024;
-  unsigned long long local = 0;
-  for (int k = 0; k < per; ++k) { const int p = threadIdx.x * per + k; if (p < P) local += hist[p]; }
-  s_part[threadIdx.x] = local;
-  __syncthreads();
-  for (int o = 1; o < 1024; o <<= 1) {
-    const unsigned long long v = threadIdx.x >= o ? s_part[threadIdx.x - o] : 0ull;
-    __syncthreads();
-    s_part[threadIdx.x] += v;
-    __syncthreads();
-  }
-  unsigned long long run = s_part[threadIdx.x] - local;
-  for (int k = 0; k < per; ++k) { const int p = threadIdx.x * per + k; if (p < P) { cursor[p] = run; run += hist[p]; } }
-}
-
-struct ScatterArgs {
-  KeyDesc key;
+struct LevelArgs {
+  KeyDesc key;                              // source keys (original columns or a partitioned copy)
   const uint64_t* vals[kMaxVals];
   uint64_t* out_vals[kMaxVals];
-  uint64_t* out_u;
-  unsigned long long* cursor;
+  void* out_keys;                           // UO[n]
+  const unsigned long long* seg_off;        // nullptr: one segment [0, n); else [gridDim.y + 1]
+  uint32_t* hist;                           // [segments * fan]
+  unsigned long long* cursor;               // [segments * fan]
   int64_t n;
-  int n_vals, bits;
+  int32_t n_vals, fan, shift;
 };
 
 template <int KK>
-__global__ void __launch_bounds__(kPartThreads)
-partition_scatter_kernel(const __grid_constant__ ScatterArgs a) {
-  __shared__ uint32_t s_cnt[1 << kMaxPartBits];
-  __shared__ unsigned long long s_base[1 << kMaxPartBits];
-  const int P = 1 << a.bits, tid = threadIdx.x;
-  constexpr int64_t kTile = (int64_t)kPartThreads * kPartRows;
-  const int64_t n_tiles = (a.n + kTile - 1) / kTile;
-  for (int p = tid; p < P; p += kPartThreads) s_cnt[p] = 0;
+__global__ void __launch_bounds__(kPT)
+part_hist_kernel(const __grid_constant__ LevelArgs a) {
+  using U = typename SrcKey<KK>::U;
+  __shared__ uint32_t s_hist[kMaxFan];
+  const int tid = threadIdx.x, seg = blockIdx.y;
+  for (int p = tid; p < a.fan; p += kPT) s_hist[p] = 0;
   __syncthreads();
+  const int64_t r0 = a.seg_off ? (int64_t)a.seg_off[seg] : 0, r1 = a.seg_off ? (int64_t)a.seg_off[seg + 1] : a.n;
+  const uint32_t mask = (uint32_t)a.fan - 1u;
+  const int64_t stride = (int64_t)gridDim.x * kPT;
+  int64_t i = r0 + (int64_t)blockIdx.x * kPT + tid;
+  for (; i + 3 * stride < r1; i += 4 * stride) {
+    U u[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) u[k] = load_u<KK>(a.key, i + k * stride);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) atomicAdd(&s_hist[part_id<U>(u[k], a.shift, mask)], 1u);
+  }
+  for (; i < r1; i += stride) atomicAdd(&s_hist[part_id<U>(load_u<KK>(a.key, i), a.shift, mask)], 1u);
+  __syncthreads();
+  for (int p = tid; p < a.fan; p += kPT) if (s_hist[p]) atomicAdd(&a.hist[(size_t)seg * a.fan + p], s_hist[p]);
+}
+
+// exclusive prefix sum of `count` 32-bit counts -> 64-bit offsets [count + 1] and cursors [count]
+// (single CTA; count <= 2^20: a few microseconds)
+__global__ void __launch_bounds__(1024)
+part_scan_kernel(const uint32_t* __restrict__ hist, unsigned long long* __restrict__ off,
+                 unsigned long long* __restrict__ cursor, int count) {
+  __shared__ unsigned long long s_part[1024];
+  const int tid = threadIdx.x;
+  const int per = (count + 1023) / 1024;
+  const int b = tid * per, e = min(count, b + per);
+  unsigned long long local = 0;
+  for (int p = b; p < e; ++p) local += hist[p];
+  s_part[tid] = local;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {
+    const unsigned long long v = tid >= o ? s_part[tid - o] : 0ull;
+    __syncthreads();
+    s_part[tid] += v;
+    __syncthreads();
+  }
+  unsigned long long run = s_part[tid] - local;
+  for (int p = b; p < e; ++p) { off[p] = run; cursor[p] = run; run += hist[p]; }
+  if (tid == 1023) off[count] = s_part[1023];
+}
+
+template <int KK, class UO>
+__global__ void __launch_bounds__(kPT, 2)
+part_scatter_kernel(const __grid_constant__ LevelArgs a) {
+  using U = typename SrcKey<KK>::U;
+  // dynamic shared memory (above the 48 KB static limit): staging buffers, then the counters
+  extern __shared__ __align__(16) unsigned char dsm[];
+  uint64_t* s_val = reinterpret_cast<uint64_t*>(dsm);
+  UO* s_key = reinterpret_cast<UO*>(dsm + sizeof(uint64_t) * kTile);
+  long long* s_delta = reinterpret_cast<long long*>(dsm + (sizeof(uint64_t) + sizeof(UO)) * kTile);
+  uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_delta + kMaxFan);
+  uint32_t* s_loff = s_cnt + kMaxFan;
+  uint16_t* s_pid = reinterpret_cast<uint16_t*>(s_loff + kMaxFan);
+  __shared__ uint32_t s_warp[kPT / 32];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, seg = blockIdx.y;
+  const int fan = a.fan;
+  const uint32_t mask = (uint32_t)fan - 1u;
+  const int64_t r0 = a.seg_off ? (int64_t)a.seg_off[seg] : 0, r1 = a.seg_off ? (int64_t)a.seg_off[seg + 1] : a.n;
+  unsigned long long* cursor = a.cursor + (size_t)seg * fan;
+  UO* out_keys = static_cast<UO*>(a.out_keys);
+  for (int p = tid; p < fan; p += kPT) s_cnt[p] = 0;
+  __syncthreads();
+  const int64_t n_tiles = (r1 - r0 + kTile - 1) / kTile;
+  constexpr int kPer = kMaxFan / kPT;       // counters per thread in the scan (consecutive)
   for (int64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-    uint64_t u[kPartRows];
-    uint32_t part[kPartRows], rank[kPartRows];
+    const int64_t base = r0 + t * kTile;
+    const int m = (int)min((int64_t)kTile, r1 - base);
+    // A: keys -> partition ids and ranks inside the tile
+    U u[kPR];
+    uint32_t pos[kPR];
+    uint64_t v0[kPR];
 #pragma unroll
-    for (int r = 0; r < kPartRows; ++r) {
-      const int64_t i = t * kTile + (int64_t)r * kPartThreads + tid;
-      if (i < a.n) {
-        u[r] = part_load_u<KK>(a.key, i);
-        part[r] = (uint32_t)(table_hash64(u[r]) >> (64 - a.bits));
-        rank[r] = atomicAdd(&s_cnt[part[r]], 1u);
+    for (int r = 0; r < kPR; ++r) {
+      const int i = r * kPT + tid;
+      if (i < m) {
+        u[r] = load_u<KK>(a.key, base + i);
+        if (a.n_vals > 0) v0[r] = ldg_stream_u64(a.vals[0] + base + i);
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < kPR; ++r) {
+      const int i = r * kPT + tid;
+      if (i < m) {
+        const uint32_t q = part_id<U>(u[r], a.shift, mask);
+        pos[r] = (q << 16) | atomicAdd(&s_cnt[q], 1u);      // rank < 4096 fits 16 bits
       }
     }
     __syncthreads();
-    for (int p = tid; p < P; p += kPartThreads) {
-      const uint32_t c = s_cnt[p];
-      if (c) s_base[p] = atomicAdd(&a.cursor[p], (unsigned long long)c);
-    }
-    __syncthreads();
+    // B: exclusive scan of the per-partition counts; claim global space per partition
+    {
+      uint32_t c[kPer], sum = 0;
 #pragma unroll
-    for (int r = 0; r < kPartRows; ++r) {
-      const int64_t i = t * kTile + (int64_t)r * kPartThreads + tid;
-      if (i < a.n) {
-        const unsigned long long dst = s_base[part[r]] + rank[r];
-        a.out_u[dst] = u[r];
-        for (int c = 0; c < a.n_vals; ++c) a.out_vals[c][dst] = ldg_stream_u64(a.vals[c] + i);
+      for (int k = 0; k < kPer; ++k) { const int p = tid * kPer + k; c[k] = p < fan ? s_cnt[p] : 0u; sum += c[k]; }
+      uint32_t inc = sum;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += y; }
+      if (lane == 31) s_warp[warp] = inc;
+      __syncthreads();
+      if (warp == 0) {
+        uint32_t w = lane < kPT / 32 ? s_warp[lane] : 0u;
+        uint32_t winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += y; }
+        if (lane < kPT / 32) s_warp[lane] = winc - w;
+      }
+      __syncthreads();
+      uint32_t run = s_warp[warp] + inc - sum;
+#pragma unroll
+      for (int k = 0; k < kPer; ++k) {
+        const int p = tid * kPer + k;
+        if (p < fan) {
+          s_loff[p] = run;
+          if (c[k]) s_delta[p] = (long long)atomicAdd(&cursor[p], (unsigned long long)c[k]) - (long long)run;
+          s_cnt[p] = 0;
+          run += c[k];
+        }
       }
     }
     __syncthreads();
-    for (int p = tid; p < P; p += kPartThreads) s_cnt[p] = 0;
+    // C: stage keys (and the first value column) in partition order
+#pragma unroll
+    for (int r = 0; r < kPR; ++r) {
+      const int i = r * kPT + tid;
+      if (i < m) {
+        const uint32_t q = pos[r] >> 16;
+        pos[r] = s_loff[q] + (pos[r] & 0xFFFFu);
+        s_key[pos[r]] = (UO)u[r];
+        s_pid[pos[r]] = (uint16_t)q;
+        if (a.n_vals > 0) s_val[pos[r]] = v0[r];
+      }
+    }
+    __syncthreads();
+    // D: write runs
+#pragma unroll
+    for (int r = 0; r < kPR; ++r) {
+      const int j = r * kPT + tid;
+      if (j < m) {
+        const long long dst = s_delta[s_pid[j]] + j;
+        out_keys[dst] = s_key[j];
+        if (a.n_vals > 0) a.out_vals[0][dst] = s_val[j];
+      }
+    }
+    // remaining value columns, one staged at a time
+    for (int c = 1; c < a.n_vals; ++c) {
+      __syncthreads();
+#pragma unroll
+      for (int r = 0; r < kPR; ++r) {
+        const int i = r * kPT + tid;
+        if (i < m) s_val[pos[r]] = ldg_stream_u64(a.vals[c] + base + i);
+      }
+      __syncthreads();
+#pragma unroll
+      for (int r = 0; r < kPR; ++r) {
+        const int j = r * kPT + tid;
+        if (j < m) a.out_vals[c][s_delta[s_pid[j]] + j] = s_val[j];
+      }
+    }
     __syncthreads();
   }
 }
 
 template <int KK>
-int launch_kk(const PartitionLaunch& L, int sm_count, cudaStream_t s) {
-  const int P = 1 << L.bits;
-  EIGER_CUDA(cudaMemsetAsync(L.hist, 0, sizeof(uint32_t) * P, s));
-  const int64_t want = (L.n + kPartThreads * 16 - 1) / (kPartThreads * 16);
-  const int blocks = (int)std::max<int64_t>(1, std::min<int64_t>(want, (int64_t)sm_count * 6));
-  partition_hist_kernel<KK><<<blocks, kPartThreads, 0, s>>>(L.key, L.n, L.bits, L.hist);
+int run_level(LevelArgs a, int segments, unsigned long long* off, int sm_count, cudaStream_t s) {
+  using UO = typename SrcKey<KK>::U;
+  const int64_t avg_rows = a.n / segments + 1;
+  const int64_t tiles = std::max<int64_t>(1, (avg_rows + kTile - 1) / kTile);
+  const int64_t want = segments == 1 ? (int64_t)sm_count * 8 : std::max<int64_t>(1, ((int64_t)sm_count * 8 + segments - 1) / segments);
+  const int gx = (int)std::min<int64_t>(tiles, want);
+  EIGER_CUDA(cudaMemsetAsync(a.hist, 0, sizeof(uint32_t) * (size_t)segments * a.fan, s));
+  part_hist_kernel<KK><<<dim3(gx, segments), kPT, 0, s>>>(a);
   count_launch();
-  partition_scan_kernel<<<1, 1024, 0, s>>>(L.hist, L.cursor, P);
+  part_scan_kernel<<<1, 1024, 0, s>>>(a.hist, off, a.cursor, segments * a.fan);
   count_launch();
-  ScatterArgs a;
-  a.key = L.key; a.out_u = L.out_u; a.cursor = L.cursor; a.n = L.n; a.n_vals = L.plan.n_vals; a.bits = L.bits;
-  for (int c = 0; c < kMaxVals; ++c) { a.vals[c] = static_cast<const uint64_t*>(L.plan.vals[c]); a.out_vals[c] = L.out_vals[c]; }
-  const int64_t tiles = (L.n + kPartThreads * kPartRows - 1) / (kPartThreads * kPartRows);
-  const int sblocks = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)sm_count * 4));
-  partition_scatter_kernel<KK><<<sblocks, kPartThreads, 0, s>>>(a);
+  constexpr size_t smem = (sizeof(uint64_t) + sizeof(UO) + sizeof(uint16_t)) * kTile + (8 + 4 + 4) * kMaxFan;
+  auto kern = part_scatter_kernel<KK, UO>;
+  EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  kern<<<dim3(gx, segments), kPT, smem, s>>>(a);
   count_launch();
   EIGER_CUDA(cudaGetLastError());
   return EIGER_OK;
 }
 
+template <int KK, int KK2>
+int run_levels(PartitionLaunch& L, int sm_count, cudaStream_t s) {
+  using U = typename SrcKey<KK>::U;
+  const int W = 8 * (int)sizeof(U);
+  LevelArgs a{};
+  a.key = L.key; a.n = L.n; a.n_vals = L.plan.n_vals;
+  for (int c = 0; c < kMaxVals; ++c) { a.vals[c] = static_cast<const uint64_t*>(L.plan.vals[c]); a.out_vals[c] = L.valsA[c]; }
+  a.out_keys = L.keysA; a.seg_off = nullptr; a.hist = L.hist; a.cursor = L.cur1;
+  a.fan = 1 << L.bits1; a.shift = W - L.bits1;
+  int rc = run_level<KK>(a, 1, L.off1, sm_count, s);
+  if (rc) return rc;
+  L.out_keys = L.keysA; L.out_vals = L.valsA; L.out_off = L.off1; L.n_parts = 1 << L.bits1;
+  if (L.bits2 > 0) {
+    LevelArgs b{};
+    b.key = L.key; b.key.ptr[0] = L.keysA; b.key.ptr[1] = nullptr;
+    b.n = L.n; b.n_vals = L.plan.n_vals;
+    for (int c = 0; c < kMaxVals; ++c) { b.vals[c] = L.valsA[c]; b.out_vals[c] = L.valsB[c]; }
+    b.out_keys = L.keysB; b.seg_off = L.off1; b.hist = L.hist; b.cursor = L.cur2;
+    b.fan = 1 << L.bits2; b.shift = W - L.bits1 - L.bits2;
+    rc = run_level<KK2>(b, 1 << L.bits1, L.off2, sm_count, s);
+    if (rc) return rc;
+    L.out_keys = L.keysB; L.out_vals = L.valsB; L.out_off = L.off2; L.n_parts = 1 << (L.bits1 + L.bits2);
+  }
+  return EIGER_OK;
+}
+
 }  // namespace
 
-int launch_partition(const PartitionLaunch& L, int sm_count, cudaStream_t s) {
-  if (L.bits < 1 || L.bits > kMaxPartBits) return EIGER_ERR_ARG;
+int partition_max_bits_per_level() { int b = 0; while ((1 << (b + 1)) <= kMaxFan) ++b; return b; }
+
+int launch_partition(PartitionLaunch& L, int sm_count, cudaStream_t s) {
+  const int mb = partition_max_bits_per_level();
+  if (L.bits1 < 1 || L.bits1 > mb || L.bits2 < 0 || L.bits2 > mb) return EIGER_ERR_ARG;
   switch (L.key_kind) {
-    case KK_I32: return launch_kk<KK_I32>(L, sm_count, s);
-    case KK_I64: return launch_kk<KK_I64>(L, sm_count, s);
-    case KK_GEN: case KK_I8I8: return launch_kk<KK_GEN>(L, sm_count, s);
+    case KK_I32: return run_levels<KK_I32, KK_U32PRE>(L, sm_count, s);
+    case KK_I64: return run_levels<KK_I64, KK_U64PRE>(L, sm_count, s);
+    case KK_GEN: case KK_I8I8: return run_levels<KK_GEN, KK_U64PRE>(L, sm_count, s);
     default: return EIGER_ERR_ARG;
   }
 }

@@ -1,0 +1,158 @@
+// Row access shared by the aggregation and partition kernels: how the key column(s) become
+// the rebased, fused key u (step A0: frame of reference + positional packing,
+// PAPER.md:219-221 §4.3), the shared-memory accumulator planes, and the global hash table.
+#pragma once
+#include "dev.cuh"
+
+namespace eiger {
+
+template <int KK> struct KeyTraits;
+template <> struct KeyTraits<KK_I32> { using U = uint32_t; };
+template <> struct KeyTraits<KK_I8I8> { using U = uint32_t; };
+template <> struct KeyTraits<KK_I64> { using U = uint64_t; };
+template <> struct KeyTraits<KK_GEN> { using U = uint64_t; };
+template <> struct KeyTraits<KK_U64PRE> { using U = uint64_t; };
+template <> struct KeyTraits<KK_U32PRE> { using U = uint32_t; };
+
+template <class U> __device__ __forceinline__ U empty_of();
+template <> __device__ __forceinline__ uint32_t empty_of<uint32_t>() { return kEmpty32; }
+template <> __device__ __forceinline__ uint64_t empty_of<uint64_t>() { return kEmpty64; }
+
+// ---- key loading ---------------------------------------------------------------------
+template <int KK>
+__device__ __forceinline__ typename KeyTraits<KK>::U load_u(const KeyDesc& k, int64_t i) {
+  using U = typename KeyTraits<KK>::U;
+  if constexpr (KK == KK_I32) {
+    return (U)(ldg_stream_4((const int32_t*)k.ptr[0] + i) - (uint32_t)k.base[0]);
+  } else if constexpr (KK == KK_I64) {
+    return ldg_stream_u64((const int64_t*)k.ptr[0] + i) - k.base[0];
+  } else if constexpr (KK == KK_U64PRE) {
+    return ldg_stream_u64((const uint64_t*)k.ptr[0] + i);
+  } else if constexpr (KK == KK_U32PRE) {
+    return ldg_stream_4((const uint32_t*)k.ptr[0] + i);
+  } else if constexpr (KK == KK_I8I8) {
+    const uint32_t a = (uint32_t)(int32_t)(int8_t)ldg_stream_1((const int8_t*)k.ptr[0] + i) - (uint32_t)k.base[0];
+    const uint32_t b = (uint32_t)(int32_t)(int8_t)ldg_stream_1((const int8_t*)k.ptr[1] + i) - (uint32_t)k.base[1];
+    return a * (uint32_t)k.mul + b;
+  } else {
+    uint64_t u = sext_load(k.ptr[0], k.dtype[0], i) - k.base[0];
+    if (k.ncols == 2) u = u * k.mul + (sext_load(k.ptr[1], k.dtype[1], i) - k.base[1]);
+    return u;
+  }
+}
+// two consecutive rows starting at an even row index (vector loads)
+template <int KK>
+__device__ __forceinline__ void load_u2(const KeyDesc& k, int64_t i, typename KeyTraits<KK>::U (&u)[2]) {
+  if constexpr (KK == KK_I32 || KK == KK_U32PRE) {
+    const uint2 v = ldg_stream_8((const int32_t*)k.ptr[0] + i);
+    const uint32_t b = KK == KK_I32 ? (uint32_t)k.base[0] : 0u;
+    u[0] = v.x - b; u[1] = v.y - b;
+  } else if constexpr (KK == KK_I64 || KK == KK_U64PRE) {
+    const uint4 v = ldg_stream_16((const uint64_t*)k.ptr[0] + i);
+    const uint64_t b = KK == KK_I64 ? k.base[0] : 0ull;
+    u[0] = (((uint64_t)v.y << 32) | v.x) - b; u[1] = (((uint64_t)v.w << 32) | v.z) - b;
+  } else if constexpr (KK == KK_I8I8) {
+    const uint32_t a = ldg_stream_2((const int8_t*)k.ptr[0] + i), b = ldg_stream_2((const int8_t*)k.ptr[1] + i);
+    const uint32_t b0 = (uint32_t)k.base[0], b1 = (uint32_t)k.base[1], m = (uint32_t)k.mul;
+    u[0] = ((uint32_t)(int32_t)(int8_t)(a & 0xFF) - b0) * m + ((uint32_t)(int32_t)(int8_t)(b & 0xFF) - b1);
+    u[1] = ((uint32_t)(int32_t)(int8_t)(a >> 8) - b0) * m + ((uint32_t)(int32_t)(int8_t)(b >> 8) - b1);
+  } else {
+    u[0] = load_u<KK>(k, i); u[1] = load_u<KK>(k, i + 1);
+  }
+}
+
+// un-fuse and un-rebase group key u into the caller's key columns at row g
+__device__ __forceinline__ void store_group_key(const KeyDesc& key, void* const* out_keys, uint64_t u, uint64_t g) {
+  uint64_t part[2];
+  if (key.ncols == 2) { part[0] = u / key.mul; part[1] = u % key.mul; } else { part[0] = u; part[1] = 0; }
+  for (int k = 0; k < key.ncols; ++k) {
+    const uint64_t v = part[k] + key.base[k];
+    switch (key.dtype[k]) {
+      case EIGER_I8: static_cast<int8_t*>(out_keys[k])[g] = (int8_t)v; break;
+      case EIGER_I32: static_cast<int32_t*>(out_keys[k])[g] = (int32_t)v; break;
+      default: static_cast<int64_t*>(out_keys[k])[g] = (int64_t)v; break;
+    }
+  }
+}
+
+template <int SIG> __device__ __forceinline__ int sig_op(const AggPlan& p, int j) { if constexpr (Sig<SIG>::kStatic) return Sig<SIG>::op(j); else return p.op[j]; }
+template <int SIG> __device__ __forceinline__ int sig_col(const AggPlan& p, int j) { if constexpr (Sig<SIG>::kStatic) return Sig<SIG>::col(j); else return p.col[j]; }
+template <int SIG> __device__ __forceinline__ bool sig_f64(const AggPlan& p, int j) { if constexpr (Sig<SIG>::kStatic) return Sig<SIG>::f64(j); else return p.f64[j] != 0; }
+
+// ---- shared-memory accumulators ------------------------------------------------------------
+// B200 shared memory has native 32-bit atomics (ATOMS.ADD / ATOMS.MAX; 3 per row sustain
+// ~880 G rows/s chip-wide, measured) but 64-bit ones are CAS loops (~0.05-0.4 T/s).  Integer
+// SUM and COUNT cells are therefore kept as two 32-bit planes, lo[S] then hi[S], and added
+// with an explicit carry: the final (hi:lo) equals the wrapping 64-bit sum whatever the
+// interleaving, because every wrap of lo is seen by exactly one atomicAdd's return value.
+// MIN / MAX and fp64 SUM keep 64-bit cells; MIN / MAX look before they leap, so the CAS loop
+// only runs on a new record.
+__device__ __forceinline__ bool add_type(int op, bool f64) { return op == EIGER_COUNT || (op == EIGER_SUM && !f64); }
+__device__ __forceinline__ void smem_add64(uint32_t* lo, uint32_t* hi, uint64_t v) {
+  const uint32_t vl = (uint32_t)v;
+  const uint32_t old = atomicAdd(lo, vl);
+  const uint32_t h = (uint32_t)(v >> 32) + ((uint32_t)(old + vl) < vl ? 1u : 0u);
+  if (h) atomicAdd(hi, h);
+}
+// accumulator j of a table of S slots that starts at base occupies 8 * S bytes
+__device__ __forceinline__ void smem_merge(unsigned char* base, uint32_t S, int j, uint32_t s, int op, bool f64, uint64_t part) {
+  unsigned char* plane = base + (size_t)j * 8 * S;
+  if (add_type(op, f64)) {
+    uint32_t* lo = reinterpret_cast<uint32_t*>(plane) + s;
+    smem_add64(lo, lo + S, part);
+  } else if (op == EIGER_SUM) {
+    atomicAdd(reinterpret_cast<double*>(plane) + s, __longlong_as_double((long long)part));
+  } else {
+    long long* cell = reinterpret_cast<long long*>(plane) + s;
+    const long long cur = *reinterpret_cast<volatile long long*>(cell);
+    if (op == EIGER_MIN) { if ((long long)part < cur) atomicMin(cell, (long long)part); }
+    else { if ((long long)part > cur) atomicMax(cell, (long long)part); }
+  }
+}
+__device__ __forceinline__ uint64_t smem_read(const unsigned char* base, uint32_t S, int j, uint32_t s, int op, bool f64) {
+  const unsigned char* plane = base + (size_t)j * 8 * S;
+  if (add_type(op, f64)) {
+    const uint32_t* lo = reinterpret_cast<const uint32_t*>(plane) + s;
+    return ((uint64_t)lo[S] << 32) | lo[0];
+  }
+  return reinterpret_cast<const uint64_t*>(plane)[s];
+}
+__device__ __forceinline__ void smem_init_plane(unsigned char* base, uint32_t S, int j, int op, bool f64, int tid, int T) {
+  uint64_t* plane = reinterpret_cast<uint64_t*>(base + (size_t)j * 8 * S);
+  const uint64_t v = add_type(op, f64) ? 0ull : acc_identity(op);
+  for (uint32_t c = tid; c < S; c += T) plane[c] = v;
+}
+
+// ---- the global hash table -------------------------------------------------------------
+// Slot s lives at table + s * stride: [u64 key][acc 0]..[acc n-1][pad]; key = ~0 means empty.
+// Slot `cap` is the side slot of the one key whose rebased value equals the empty marker
+// (R18).  Find-or-insert with a single exit so that the lanes of a warp stay
+// converged (an early-return version ran 15x slower: every lane took its own copy of the
+// tail).  Returns the slot's accumulator cells, or nullptr when probing gave up.
+constexpr int kBackProbes = 4096;
+__device__ __forceinline__ uint64_t* back_find_or_insert(void* table, uint64_t cap, uint32_t stride,
+                                                         uint64_t u, CallDev* call) {
+  uint64_t* cells = nullptr;
+  uint64_t slot = __umul64hi(table_hash64(u), cap);
+  int probes = 0;
+  bool done = false;
+  if (u == kEmpty64) { slot = cap; }
+  while (!done) {
+    unsigned long long* kp = reinterpret_cast<unsigned long long*>(static_cast<char*>(table) + slot * stride);
+    if (slot == cap) {            // side slot: key word 0 = used
+      if (__ldcg(kp) != 0ull) atomicExch(kp, 0ull);
+      cells = reinterpret_cast<uint64_t*>(kp) + 1; done = true;
+    } else {
+      unsigned long long k = __ldcg(kp);
+      if (k == kEmpty64) { k = atomicCAS(kp, kEmpty64, (unsigned long long)u); if (k == kEmpty64) k = u; }
+      if (k == u) { cells = reinterpret_cast<uint64_t*>(kp) + 1; done = true; }
+      else {
+        slot = slot + 1 == cap ? 0 : slot + 1;
+        if (++probes >= kBackProbes) { atomicOr(&call->overflow, 1u); done = true; }
+      }
+    }
+  }
+  return cells;
+}
+
+}  // namespace eiger
