@@ -88,37 +88,67 @@ struct Front {
     for (uint32_t c = tid; c < Sn; c += T) skeys[c] = empty_of<U>();
   }
 
-  __device__ __forceinline__ uint32_t home(U u) const {
-    if constexpr (sizeof(U) == 4) return __umulhi(table_hash32b((uint32_t)u), Sn);
-    else return __umulhi((uint32_t)table_hash64((uint64_t)u), Sn);   // low word: the top bits chose the partition
+  // Buckets of 16 bytes (4 x 32-bit keys or 2 x 64-bit keys): one LDS.128 looks at a whole bucket,
+  // so that at the load factors used here almost every row resolves on its first probe and the
+  // lanes of a warp do not wait for each other's probe chains.
+  static constexpr uint32_t kB = 16 / sizeof(U);
+  __device__ __forceinline__ uint32_t home_bucket(U u) const {
+    if constexpr (sizeof(U) == 4) return __umulhi(table_hash32b((uint32_t)u), Sn / kB);
+    else return __umulhi((uint32_t)table_hash64((uint64_t)u), Sn / kB);   // low word: the top bits chose the partition
   }
-
-  // find-or-insert in the shared-memory table; single exit.  Returns the slot or -1.
-  __device__ __forceinline__ int find(U u, uint32_t* s_count) {
+  __device__ __forceinline__ uint4 load_bucket(uint32_t b) const {
+    uint4 r;
+    const uint32_t addr = (uint32_t)__cvta_generic_to_shared(reinterpret_cast<const unsigned char*>(skeys) + (size_t)b * 16);
+    asm volatile("ld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr) : "memory");
+    return r;
+  }
+  // position of u inside bucket q, or the first empty position + kB, or 2 * kB when full of others
+  __device__ __forceinline__ uint32_t scan_bucket(const uint4& q, U u) const {
+    if constexpr (sizeof(U) == 4) {
+      if (q.x == u) return 0; if (q.y == u) return 1; if (q.z == u) return 2; if (q.w == u) return 3;
+      if (q.x == kEmpty32) return 4; if (q.y == kEmpty32) return 5; if (q.z == kEmpty32) return 6; if (q.w == kEmpty32) return 7;
+      return 8;
+    } else {
+      const uint64_t k0 = ((uint64_t)q.y << 32) | q.x, k1 = ((uint64_t)q.w << 32) | q.z;
+      if (k0 == u) return 0; if (k1 == u) return 1;
+      if (k0 == kEmpty64) return 2; if (k1 == kEmpty64) return 3;
+      return 4;
+    }
+  }
+  // find-or-insert given the first bucket's contents; single exit.  Returns the slot or -1.
+  __device__ __forceinline__ int resolve(U u, uint32_t b, uint4 q, uint32_t* s_count) {
     int res = -1;
     bool done = false;
     if constexpr (sizeof(U) == 8) { if (u == kEmpty64) done = true; }
-    uint32_t h = home(u);
     int probes = 0;
     while (!done) {
-      U k = *reinterpret_cast<volatile U*>(skeys + h);
-      if (k == empty_of<U>()) {
+      const uint32_t r = scan_bucket(q, u);
+      if (r < kB) { res = (int)(b * kB + r); done = true; }
+      else if (r < 2 * kB) {
+        // not in the table (an empty position ends the chain): insert unless the table is closed
         if (*reinterpret_cast<volatile uint32_t*>(s_count) >= a.limit) { done = true; }
         else {
-          if constexpr (sizeof(U) == 4) k = atomicCAS(skeys + h, kEmpty32, u);
-          else k = (U)atomicCAS(reinterpret_cast<unsigned long long*>(skeys + h), (unsigned long long)kEmpty64, (unsigned long long)u);
-          if (k == empty_of<U>()) { atomicAdd(s_count, 1u); k = u; }
+          const uint32_t h = b * kB + (r - kB);
+          U old;
+          if constexpr (sizeof(U) == 4) old = atomicCAS(skeys + h, kEmpty32, u);
+          else old = (U)atomicCAS(reinterpret_cast<unsigned long long*>(skeys + h), (unsigned long long)kEmpty64, (unsigned long long)u);
+          if (old == empty_of<U>()) { atomicAdd(s_count, 1u); res = (int)h; done = true; }
+          else if (old == u) { res = (int)h; done = true; }
+          else q = load_bucket(b);          // somebody else took it: look at the bucket again
         }
-      }
-      if (!done) {
-        if (k == u) { res = (int)h; done = true; }
-        else { h = h + 1 == Sn ? 0 : h + 1; if (++probes >= 64) done = true; }
+      } else {
+        b = b + 1 == Sn / kB ? 0 : b + 1;
+        if (++probes >= 16) done = true; else q = load_bucket(b);
       }
     }
     return res;
   }
 
-  __device__ __forceinline__ void update(uint32_t h, const uint64_t (&raw)[NV]) {
+  // Accumulator updates in two steps so that the returning atomics of several rows are in flight
+  // together: issue() fires the 32-bit adds (SUM low word, COUNT) and reads MIN / MAX cells,
+  // finish() propagates carries and settles new minima / maxima.
+  struct Pending { uint32_t old[NA]; };
+  __device__ __forceinline__ void issue(uint32_t h, const uint64_t (&raw)[NV], Pending& pd) {
     uint32_t off = 0;
 #pragma unroll
     for (int j = 0; j < NA; ++j) {
@@ -127,18 +157,33 @@ struct Front {
       unsigned char* plane = smem + (size_t)off * a.slots;
       if (op == EIGER_COUNT) {
         atomicAdd(reinterpret_cast<uint32_t*>(plane) + h, 1u);
-      } else {
-        const uint64_t part = row_partial(op, f, raw[sig_col<SIG>(a.plan, j)]);
+      } else if (add_type(op, f)) {
+        pd.old[j] = atomicAdd(reinterpret_cast<uint32_t*>(plane) + h, (uint32_t)raw[sig_col<SIG>(a.plan, j)]);
+      } else if (op == EIGER_SUM) {
+        atomicAdd(reinterpret_cast<double*>(plane) + h, __longlong_as_double((long long)raw[sig_col<SIG>(a.plan, j)]));
+      }
+      off += plane_width(op);
+    }
+  }
+  __device__ __forceinline__ void finish(uint32_t h, const uint64_t (&raw)[NV], const Pending& pd) {
+    uint32_t off = 0;
+#pragma unroll
+    for (int j = 0; j < NA; ++j) {
+      if (!S::kStatic && j >= n_acc) break;
+      const int op = sig_op<SIG>(a.plan, j); const bool f = sig_f64<SIG>(a.plan, j);
+      unsigned char* plane = smem + (size_t)off * a.slots;
+      if (op != EIGER_COUNT) {
+        const uint64_t v = raw[sig_col<SIG>(a.plan, j)];
         if (add_type(op, f)) {
-          uint32_t* lo = reinterpret_cast<uint32_t*>(plane) + h;
-          smem_add64(lo, lo + a.slots, part);
-        } else if (op == EIGER_SUM) {
-          atomicAdd(reinterpret_cast<double*>(plane) + h, __longlong_as_double((long long)part));
-        } else {
+          const uint32_t vl = (uint32_t)v;
+          const uint32_t hi = (uint32_t)(v >> 32) + ((uint32_t)(pd.old[j] + vl) < vl ? 1u : 0u);
+          if (hi) atomicAdd(reinterpret_cast<uint32_t*>(plane) + a.slots + h, hi);
+        } else if (op != EIGER_SUM) {
+          const long long part = (long long)row_partial(op, f, v);
           long long* cell = reinterpret_cast<long long*>(plane) + h;
           const long long cur = *reinterpret_cast<volatile long long*>(cell);
-          if (op == EIGER_MIN) { if ((long long)part < cur) atomicMin(cell, (long long)part); }
-          else { if ((long long)part > cur) atomicMax(cell, (long long)part); }
+          if (op == EIGER_MIN) { if (part < cur) atomicMin(cell, part); }
+          else { if (part > cur) atomicMax(cell, part); }
         }
       }
       off += plane_width(op);
@@ -166,28 +211,48 @@ struct Front {
     }
   }
 
-  __device__ __forceinline__ void row(U u, const uint64_t (&raw)[NV], uint32_t* s_count, bool& missed) {
-    const int h = find(u, s_count);
-    if (h >= 0) update((uint32_t)h, raw);
-    else if (a.spec) missed = true;
-    else back_row(u, raw);
+  // two rows at a time: both first probes in flight, then both sets of atomics
+  __device__ __forceinline__ void pair(U u0, const uint64_t (&raw0)[NV], bool v0, U u1, const uint64_t (&raw1)[NV], bool v1,
+                                       uint32_t* s_count, bool& missed) {
+    const uint32_t b0 = home_bucket(u0), b1 = home_bucket(u1);
+    const uint4 q0 = load_bucket(b0), q1 = load_bucket(b1);
+    const int h0 = v0 ? resolve(u0, b0, q0, s_count) : -1;
+    __syncwarp();
+    const int h1 = v1 ? resolve(u1, b1, q1, s_count) : -1;
+    __syncwarp();
+    Pending p0, p1;
+    if (h0 >= 0) issue((uint32_t)h0, raw0, p0);
+    if (h1 >= 0) issue((uint32_t)h1, raw1, p1);
+    if (h0 >= 0) finish((uint32_t)h0, raw0, p0);
+    if (h1 >= 0) finish((uint32_t)h1, raw1, p1);
+    const bool m0 = v0 && h0 < 0, m1 = v1 && h1 < 0;
+    if (__any_sync(0xffffffffu, m0 || m1)) {        // rows the shared-memory table has no room for
+      if (a.spec) missed = missed || m0 || m1;
+      else { if (m0) back_row(u0, raw0); __syncwarp(); if (m1) back_row(u1, raw1); }
+    }
+    __syncwarp();
   }
 
   // merge every occupied slot into the global table
   __device__ void flush_merge(int tid, int T) {
-    for (uint32_t h = tid; h < Sn; h += T) {
-      const U k = skeys[h];
-      if (k == empty_of<U>()) continue;
-      uint64_t* cells = back_find_or_insert(a.table, a.cap, a.stride, (uint64_t)k, a.call);
-      if (!cells) continue;
-      uint32_t off = 0;
-      for (int j = 0; j < n_acc; ++j) {
-        const int op = sig_op<SIG>(a.plan, j); const bool f = sig_f64<SIG>(a.plan, j);
-        const uint64_t v = read(h, j, off);
-        off += plane_width(op);
-        if (v == acc_identity(op) && !(op == EIGER_SUM && f)) continue;
-        atomic_merge(cells + j, op, f, v);
+    const int lane = tid & 31;
+    for (uint32_t h0 = tid - lane; h0 < Sn; h0 += T) {       // warp-uniform trip count
+      const uint32_t h = h0 + lane;
+      const U k = h < Sn ? skeys[h] : empty_of<U>();
+      if (k != empty_of<U>()) {
+        uint64_t* cells = back_find_or_insert(a.table, a.cap, a.stride, (uint64_t)k, a.call);
+        if (cells) {
+          uint32_t off = 0;
+          for (int j = 0; j < n_acc; ++j) {
+            const int op = sig_op<SIG>(a.plan, j); const bool f = sig_f64<SIG>(a.plan, j);
+            const uint64_t v = read(h, j, off);
+            off += plane_width(op);
+            if (v == acc_identity(op) && !(op == EIGER_SUM && f)) continue;
+            atomic_merge(cells + j, op, f, v);
+          }
+        }
       }
+      __syncwarp();
     }
   }
 
@@ -233,8 +298,10 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
   const int n_vals = Sig<SIG>::kStatic ? NV : a.plan.n_vals;
 
   if constexpr (!IsPre<KK>::v) {
-    // ---- whole-input mode: tiles of 2 * T * UNR rows, grid-strided ----
-    constexpr int UNR = !Sig<SIG>::kStatic ? 1 : 2;
+    // ---- whole-input mode: tiles of 2 * T * UNR rows, grid-strided; the next tile's loads are
+    // in flight while the current one is processed (one CTA per SM: there is nobody else to
+    // hide HBM latency behind) ----
+    constexpr int UNR = !Sig<SIG>::kStatic ? 1 : (NV >= 4 ? 1 : (sizeof(U) == 8 ? 2 : 3));
     F f(a, smem, a.slots);
     if (tid == 0) { s_count = 0; s_abort = 0; }
     f.init(tid, T);
@@ -242,30 +309,50 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
     const int64_t step = 2 * (int64_t)T, tile = step * UNR;
     const int64_t n_tiles = a.n / tile;
     bool missed = false;
-    for (int64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-      if (a.spec) { if (missed || *reinterpret_cast<volatile uint32_t*>(&a.call->abort)) break; }
+    U u[2][UNR][2];
+    uint64_t raw[2][UNR][2][NV];
+    auto load_tile = [&](int b, int64_t t) {
       const int64_t r0 = t * tile + 2 * tid;
-      U u[UNR][2];
-      uint64_t raw[UNR][2][NV];
 #pragma unroll
       for (int s = 0; s < UNR; ++s) {
-        load_u2<KK>(a.key, r0 + s * step, u[s]);
+        load_u2<KK>(a.key, r0 + s * step, u[b][s]);
 #pragma unroll
         for (int c = 0; c < NV; ++c) {
-          if (!Sig<SIG>::kStatic && c >= n_vals) { raw[s][0][c] = 0; raw[s][1][c] = 0; continue; }
+          if (!Sig<SIG>::kStatic && c >= n_vals) { raw[b][s][0][c] = 0; raw[b][s][1][c] = 0; continue; }
           const uint4 v = ldg_stream_16(static_cast<const uint64_t*>(a.plan.vals[c]) + r0 + s * step);
-          raw[s][0][c] = ((uint64_t)v.y << 32) | v.x; raw[s][1][c] = ((uint64_t)v.w << 32) | v.z;
+          raw[b][s][0][c] = ((uint64_t)v.y << 32) | v.x; raw[b][s][1][c] = ((uint64_t)v.w << 32) | v.z;
         }
       }
+    };
+    auto process_tile = [&](int b) {
 #pragma unroll
-      for (int s = 0; s < UNR; ++s) { f.row(u[s][0], raw[s][0], &s_count, missed); f.row(u[s][1], raw[s][1], &s_count, missed); }
+      for (int s = 0; s < UNR; ++s) f.pair(u[b][s][0], raw[b][s][0], true, u[b][s][1], raw[b][s][1], true, &s_count, missed);
+    };
+    int64_t t = blockIdx.x;
+    if (t < n_tiles) load_tile(0, t);
+    while (t < n_tiles) {
+      if (a.spec) { if (__any_sync(0xffffffffu, missed || *reinterpret_cast<volatile uint32_t*>(&a.call->abort))) break; }
+      if (t + gridDim.x < n_tiles) load_tile(1, t + gridDim.x);
+      process_tile(0);
+      t += gridDim.x;
+      if (t >= n_tiles) break;
+      if (t + gridDim.x < n_tiles) load_tile(0, t + gridDim.x);
+      process_tile(1);
+      t += gridDim.x;
     }
-    if (!(a.spec && missed)) {
-      for (int64_t i = n_tiles * tile + (int64_t)blockIdx.x * T + tid; i < a.n; i += (int64_t)gridDim.x * T) {
-        uint64_t raw[NV];
+    if (!(a.spec && __any_sync(0xffffffffu, missed))) {
+      // ragged tail: row at a time, spread over the whole grid, warp-uniform trip count
+      const int lane = tid & 31;
+      for (int64_t i0 = n_tiles * tile + (int64_t)blockIdx.x * T + (tid - lane); i0 < a.n; i0 += (int64_t)gridDim.x * T) {
+        const int64_t i = i0 + lane;
+        uint64_t rawt[NV];
+        U ut = 0;
+        if (i < a.n) {
 #pragma unroll
-        for (int c = 0; c < NV; ++c) raw[c] = (Sig<SIG>::kStatic || c < n_vals) ? ldg_stream_u64(static_cast<const uint64_t*>(a.plan.vals[c]) + i) : 0ull;
-        f.row(load_u<KK>(a.key, i), raw, &s_count, missed);
+          for (int c = 0; c < NV; ++c) rawt[c] = (Sig<SIG>::kStatic || c < n_vals) ? ldg_stream_u64(static_cast<const uint64_t*>(a.plan.vals[c]) + i) : 0ull;
+          ut = load_u<KK>(a.key, i);
+        }
+        f.pair(ut, rawt, i < a.n, ut, rawt, false, &s_count, missed);
       }
     }
     if (a.spec) {
@@ -283,32 +370,46 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
       if (r1 <= r0) continue;
       // a table no larger than the partition needs: 2 slots per row is always enough
       const uint64_t want = 2ull * (uint64_t)(r1 - r0) + 64;
-      const uint32_t Sn = (uint32_t)(want < a.slots ? want : a.slots);
+      const uint32_t Sn = (uint32_t)(want < a.slots ? want : a.slots) & ~7u;   // whole buckets
       F f(a, smem, Sn);
       __syncthreads();                       // the previous partition's emit is over
       if (tid == 0) s_count = 0;
       f.init(tid, T);
       __syncthreads();
       bool missed = false;
-      constexpr int UNR = 4;
-      int64_t i = r0 + tid;
-      for (; i + (int64_t)(UNR - 1) * T < r1; i += (int64_t)UNR * T) {
-        U u[UNR];
-        uint64_t raw[UNR][NV];
+      // chunks of UNR * T rows, bounds-checked per row; the next chunk loads while this one is processed
+      constexpr int UNR = NV >= 4 ? 1 : 2;
+      U u[2][UNR];
+      uint64_t raw[2][UNR][NV];
+      const int64_t chunk = (int64_t)UNR * T;
+      auto load_chunk = [&](int b, int64_t c0) {
 #pragma unroll
         for (int s = 0; s < UNR; ++s) {
-          u[s] = load_u<KK>(a.key, i + (int64_t)s * T);
+          const int64_t i = c0 + (int64_t)s * T + tid;
+          if (i < r1) {
+            u[b][s] = load_u<KK>(a.key, i);
 #pragma unroll
-          for (int c = 0; c < NV; ++c) raw[s][c] = (Sig<SIG>::kStatic || c < n_vals) ? ldg_stream_u64(static_cast<const uint64_t*>(a.plan.vals[c]) + i + (int64_t)s * T) : 0ull;
+            for (int c = 0; c < NV; ++c) raw[b][s][c] = (Sig<SIG>::kStatic || c < n_vals) ? ldg_stream_u64(static_cast<const uint64_t*>(a.plan.vals[c]) + i) : 0ull;
+          }
         }
+      };
+      auto process_chunk = [&](int b, int64_t c0) {
 #pragma unroll
-        for (int s = 0; s < UNR; ++s) f.row(u[s], raw[s], &s_count, missed);
-      }
-      for (; i < r1; i += T) {
-        uint64_t raw[NV];
-#pragma unroll
-        for (int c = 0; c < NV; ++c) raw[c] = (Sig<SIG>::kStatic || c < n_vals) ? ldg_stream_u64(static_cast<const uint64_t*>(a.plan.vals[c]) + i) : 0ull;
-        f.row(load_u<KK>(a.key, i), raw, &s_count, missed);
+        for (int s = 0; s < UNR; s += 2) {
+          const bool v0 = c0 + (int64_t)s * T + tid < r1, v1 = (s + 1 < UNR) && (c0 + (int64_t)(s + 1) * T + tid < r1);
+          f.pair(v0 ? u[b][s] : (U)0, raw[b][s], v0, v1 ? u[b][s + 1 < UNR ? s + 1 : s] : (U)0, raw[b][s + 1 < UNR ? s + 1 : s], v1, &s_count, missed);
+        }
+      };
+      int64_t c0 = r0;
+      load_chunk(0, c0);
+      while (c0 < r1) {
+        if (c0 + chunk < r1) load_chunk(1, c0 + chunk);
+        process_chunk(0, c0);
+        c0 += chunk;
+        if (c0 >= r1) break;
+        if (c0 + chunk < r1) load_chunk(0, c0 + chunk);
+        process_chunk(1, c0);
+        c0 += chunk;
       }
       __syncthreads();
       f.flush_emit(tid, T, s_count, &s_base, &s_cursor);
