@@ -108,7 +108,7 @@ struct QueryPlan {
   int threads = 0;
   int bits1 = 0, bits2 = 0;
   size_t smem_bytes = 0;
-  uint64_t cap = 0, cap_bound = 0;
+  uint64_t cap = 0, cap_bound = 0, cap_hot = 0;
   uint32_t stride = 0;
   size_t table_bytes = 0, part_bytes = 0, total_bytes = 0;
 };
@@ -254,18 +254,22 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
       const int mb = partition_max_bits_per_level();
       if (bits <= mb) { q->bits1 = bits; q->bits2 = 0; } else { q->bits1 = (bits + 1) / 2; q->bits2 = bits - q->bits1; }
       // the global table only takes what overflows a partition's shared-memory table
+      // the global table only takes what overflows a partition's shared-memory table, and the keys
+      // of hot partitions that are cut into several work items (possible once n / P >= 32768)
       q->cap = std::min(q->cap_bound, (uint64_t)std::max(4096.0, ndv / 64.0));
+      q->cap_hot = std::min(q->cap_bound, hash_cap(ndv));
       const size_t P1 = (size_t)1 << q->bits1, P = (size_t)1 << (q->bits1 + q->bits2);
+      if (n / (int64_t)P >= 32768) q->cap = q->cap_hot;
       const size_t kb = hk == KK_I32 ? 4 : 8;
       const size_t col = align_up((size_t)n * 8, 256), kcol = align_up((size_t)n * kb, 256);
-      q->part_bytes = align_up(P * 4, 256) + align_up((P1 + 1) * 8, 256) + align_up(P1 * 8, 256) +
+      q->part_bytes = align_up(P * 4, 256) + align_up((P + 1) * 8, 256) + align_up((P1 + 1) * 8, 256) + align_up(P1 * 8, 256) +
                       (kcol + (size_t)p.n_vals * col);
       if (q->bits2 > 0) q->part_bytes += align_up((P + 1) * 8, 256) + align_up(P * 8, 256) + (kcol + (size_t)p.n_vals * col);
     } else {
       q->threads = T.smem_threads;
       const bool front = variant == EIGER_SMEM || T.global_front;
       q->slots = front ? smem_slots : 64;
-      q->limit = front ? (uint32_t)(0.75 * smem_slots) : 0;
+      q->limit = front ? (uint32_t)((variant == EIGER_SMEM ? 0.75 : 0.5) * smem_slots) : 0;
       q->cap = std::min(hash_cap(ndv), q->cap_bound);
     }
     q->smem_bytes = align_up((size_t)q->slots * slot_bytes + 64, 16);
@@ -383,6 +387,8 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         const size_t col = align_up((size_t)n * 8, 256), kcol = align_up((size_t)n * kb, 256);
         auto take = [&](size_t bytes) { char* r = pws; pws += align_up(bytes, 256); return r; };
         P.hist = reinterpret_cast<uint32_t*>(take(PP * 4));
+        P.item_off = reinterpret_cast<unsigned long long*>(take((PP + 1) * 8));
+        P.chunk_rows = std::max<int64_t>(32768, n / (int64_t)PP);
         P.off1 = reinterpret_cast<unsigned long long*>(take((P1 + 1) * 8));
         P.cur1 = reinterpret_cast<unsigned long long*>(take(P1 * 8));
         P.keysA = take(kcol);
@@ -398,9 +404,9 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         H.key.ptr[0] = P.out_keys;
         for (int c = 0; c < q.plan.n_vals; ++c) H.plan.vals[c] = P.out_vals[c];
         H.key_kind = src_kind == KK_I32 ? KK_U32PRE : KK_U64PRE;
-        H.part_off = P.out_off; H.n_parts = P.n_parts;
+        H.part_off = P.out_off; H.item_off = P.item_off; H.n_parts = P.n_parts;
         const int occ = (int)std::max<size_t>(1, std::min<size_t>((size_t)(2048 / q.threads), (rt->smem_optin + 1024) / (q.smem_bytes + 1024)));
-        H.blocks = (int)std::min<int64_t>((int64_t)rt->sm_count * occ, P.n_parts);
+        H.blocks = (int)std::min<int64_t>((int64_t)rt->sm_count * occ, (int64_t)P.n_parts + n / P.chunk_rows);
       } else {
         const int64_t tiles = std::max<int64_t>(1, n / (4 * (int64_t)q.threads));
         H.blocks = (int)std::min<int64_t>(rt->sm_count, tiles);

@@ -30,6 +30,7 @@ struct HashAggArgs {
   AggPlan plan;
   int64_t n;
   const unsigned long long* part_off;   // partition mode: [n_parts + 1] row offsets
+  const unsigned long long* item_off;   // partition mode: [n_parts + 1] work items (hot partitions are cut up)
   int32_t n_parts;
   uint32_t slots;        // shared-memory slots per CTA (any number >= 64)
   uint32_t limit;        // stop inserting new keys beyond this many
@@ -212,8 +213,9 @@ struct Front {
   }
 
   // two rows at a time: both first probes in flight, then both sets of atomics
-  __device__ __forceinline__ void pair(U u0, const uint64_t (&raw0)[NV], bool v0, U u1, const uint64_t (&raw1)[NV], bool v1,
-                                       uint32_t* s_count, bool& missed) {
+  // Returns bit 0 / 1 set for a row that found no room (the caller sends those to the global table).
+  __device__ __forceinline__ uint32_t pair(U u0, const uint64_t (&raw0)[NV], bool v0, U u1, const uint64_t (&raw1)[NV], bool v1,
+                                           uint32_t* s_count) {
     const uint32_t b0 = home_bucket(u0), b1 = home_bucket(u1);
     const uint4 q0 = load_bucket(b0), q1 = load_bucket(b1);
     const int h0 = v0 ? resolve(u0, b0, q0, s_count) : -1;
@@ -225,12 +227,33 @@ struct Front {
     if (h1 >= 0) issue((uint32_t)h1, raw1, p1);
     if (h0 >= 0) finish((uint32_t)h0, raw0, p0);
     if (h1 >= 0) finish((uint32_t)h1, raw1, p1);
-    const bool m0 = v0 && h0 < 0, m1 = v1 && h1 < 0;
-    if (__any_sync(0xffffffffu, m0 || m1)) {        // rows the shared-memory table has no room for
-      if (a.spec) missed = missed || m0 || m1;
-      else { if (m0) back_row(u0, raw0); __syncwarp(); if (m1) back_row(u1, raw1); }
-    }
     __syncwarp();
+    return (v0 && h0 < 0 ? 1u : 0u) | (v1 && h1 < 0 ? 2u : 0u);
+  }
+
+  // rows of one trip that found no room in shared memory: global table, one code copy per trip
+  template <int R>
+  __device__ __forceinline__ void spill(const U (&u)[R], const uint64_t (&raw)[R][NV], uint32_t miss, bool& missed) {
+    if (__any_sync(0xffffffffu, miss != 0)) {
+      if (a.spec) { missed = missed || miss != 0; }
+      else {
+#pragma unroll 1
+        for (int k = 0; k < R; ++k) {
+          U uu = u[0]; uint64_t rr[NV];
+#pragma unroll
+          for (int c = 0; c < NV; ++c) rr[c] = raw[0][c];
+#pragma unroll
+          for (int r = 1; r < R; ++r)
+            if (k == r) {
+              uu = u[r];
+#pragma unroll
+              for (int c = 0; c < NV; ++c) rr[c] = raw[r][c];
+            }
+          if ((miss >> k) & 1u) back_row(uu, rr);
+          __syncwarp();
+        }
+      }
+    }
   }
 
   // merge every occupied slot into the global table
@@ -309,24 +332,26 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
     const int64_t step = 2 * (int64_t)T, tile = step * UNR;
     const int64_t n_tiles = a.n / tile;
     bool missed = false;
-    U u[2][UNR][2];
-    uint64_t raw[2][UNR][2][NV];
+    U u[2][2 * UNR];
+    uint64_t raw[2][2 * UNR][NV];
     auto load_tile = [&](int b, int64_t t) {
       const int64_t r0 = t * tile + 2 * tid;
 #pragma unroll
       for (int s = 0; s < UNR; ++s) {
-        load_u2<KK>(a.key, r0 + s * step, u[b][s]);
+        { U uu[2]; load_u2<KK>(a.key, r0 + s * step, uu); u[b][2 * s] = uu[0]; u[b][2 * s + 1] = uu[1]; }
 #pragma unroll
         for (int c = 0; c < NV; ++c) {
-          if (!Sig<SIG>::kStatic && c >= n_vals) { raw[b][s][0][c] = 0; raw[b][s][1][c] = 0; continue; }
+          if (!Sig<SIG>::kStatic && c >= n_vals) { raw[b][2 * s][c] = 0; raw[b][2 * s + 1][c] = 0; continue; }
           const uint4 v = ldg_stream_16(static_cast<const uint64_t*>(a.plan.vals[c]) + r0 + s * step);
-          raw[b][s][0][c] = ((uint64_t)v.y << 32) | v.x; raw[b][s][1][c] = ((uint64_t)v.w << 32) | v.z;
+          raw[b][2 * s][c] = ((uint64_t)v.y << 32) | v.x; raw[b][2 * s + 1][c] = ((uint64_t)v.w << 32) | v.z;
         }
       }
     };
     auto process_tile = [&](int b) {
+      uint32_t miss = 0;
 #pragma unroll
-      for (int s = 0; s < UNR; ++s) f.pair(u[b][s][0], raw[b][s][0], true, u[b][s][1], raw[b][s][1], true, &s_count, missed);
+      for (int s = 0; s < UNR; ++s) miss |= f.pair(u[b][2 * s], raw[b][2 * s], true, u[b][2 * s + 1], raw[b][2 * s + 1], true, &s_count) << (2 * s);
+      f.spill(u[b], raw[b], miss, missed);
     };
     int64_t t = blockIdx.x;
     if (t < n_tiles) load_tile(0, t);
@@ -352,7 +377,9 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
           for (int c = 0; c < NV; ++c) rawt[c] = (Sig<SIG>::kStatic || c < n_vals) ? ldg_stream_u64(static_cast<const uint64_t*>(a.plan.vals[c]) + i) : 0ull;
           ut = load_u<KK>(a.key, i);
         }
-        f.pair(ut, rawt, i < a.n, ut, rawt, false, &s_count, missed);
+        const uint32_t miss = f.pair(ut, rawt, i < a.n, ut, rawt, false, &s_count);
+        if (__any_sync(0xffffffffu, miss != 0)) { if (a.spec) missed = missed || miss != 0; else if (miss) f.back_row(ut, rawt); }
+        __syncwarp();
       }
     }
     if (a.spec) {
@@ -364,10 +391,24 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
     }
     f.flush_merge(tid, T);
   } else {
-    // ---- partition mode: this CTA owns partitions blockIdx.x, + gridDim.x, ... ----
-    for (int p = blockIdx.x; p < a.n_parts; p += gridDim.x) {
-      const int64_t r0 = (int64_t)a.part_off[p], r1 = (int64_t)a.part_off[p + 1];
-      if (r1 <= r0) continue;
+    // ---- partition mode: work items blockIdx.x, + gridDim.x, ...; an item is a whole partition
+    // (this CTA then owns its keys and emits them) or a slice of a hot one (merged through the
+    // global table like the whole-input mode) ----
+    __shared__ int s_p;
+    const unsigned long long n_items = a.item_off[a.n_parts];
+    for (unsigned long long it = blockIdx.x; it < n_items; it += gridDim.x) {
+      if (tid == 0) {           // the partition of item `it`: the last p with item_off[p] <= it
+        int lo = 0, hi = a.n_parts;
+        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (a.item_off[mid] <= it) lo = mid; else hi = mid; }
+        s_p = lo;
+      }
+      __syncthreads();
+      const int p = s_p;
+      const unsigned long long n_chunks = a.item_off[p + 1] - a.item_off[p], ci = it - a.item_off[p];
+      const int64_t P0 = (int64_t)a.part_off[p], P1 = (int64_t)a.part_off[p + 1];
+      const int64_t per = (P1 - P0 + (int64_t)n_chunks - 1) / (int64_t)n_chunks;
+      const int64_t r0 = P0 + (int64_t)ci * per, r1 = r0 + per < P1 ? r0 + per : P1;
+      const bool exclusive = n_chunks == 1;
       // a table no larger than the partition needs: 2 slots per row is always enough
       const uint64_t want = 2ull * (uint64_t)(r1 - r0) + 64;
       const uint32_t Sn = (uint32_t)(want < a.slots ? want : a.slots) & ~7u;   // whole buckets
@@ -394,11 +435,13 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
         }
       };
       auto process_chunk = [&](int b, int64_t c0) {
+        uint32_t miss = 0;
 #pragma unroll
         for (int s = 0; s < UNR; s += 2) {
           const bool v0 = c0 + (int64_t)s * T + tid < r1, v1 = (s + 1 < UNR) && (c0 + (int64_t)(s + 1) * T + tid < r1);
-          f.pair(v0 ? u[b][s] : (U)0, raw[b][s], v0, v1 ? u[b][s + 1 < UNR ? s + 1 : s] : (U)0, raw[b][s + 1 < UNR ? s + 1 : s], v1, &s_count, missed);
+          miss |= f.pair(v0 ? u[b][s] : (U)0, raw[b][s], v0, v1 ? u[b][s + 1 < UNR ? s + 1 : s] : (U)0, raw[b][s + 1 < UNR ? s + 1 : s], v1, &s_count) << s;
         }
+        f.spill(u[b], raw[b], miss, missed);
       };
       int64_t c0 = r0;
       load_chunk(0, c0);
@@ -412,7 +455,8 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
         c0 += chunk;
       }
       __syncthreads();
-      f.flush_emit(tid, T, s_count, &s_base, &s_cursor);
+      if (exclusive) f.flush_emit(tid, T, s_count, &s_base, &s_cursor);
+      else f.flush_merge(tid, T);
     }
   }
 }
@@ -422,7 +466,7 @@ int launch_one(const HashAggLaunch& L, cudaStream_t s) {
   auto kern = hash_agg_kernel<KK, SIG>;
   if (L.smem_bytes > 48 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
   HashAggArgs a;
-  a.key = L.key; a.plan = L.plan; a.n = L.n; a.part_off = L.part_off; a.n_parts = L.n_parts;
+  a.key = L.key; a.plan = L.plan; a.n = L.n; a.part_off = L.part_off; a.item_off = L.item_off; a.n_parts = L.n_parts;
   a.slots = L.slots; a.limit = L.limit; a.spec = L.spec;
   a.table = L.table; a.cap = L.cap; a.stride = L.stride; a.call = L.call;
   a.out_keys[0] = L.out_keys[0]; a.out_keys[1] = L.out_keys[1];

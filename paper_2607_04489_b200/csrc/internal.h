@@ -89,6 +89,7 @@ struct HashAggLaunch {
   int64_t n;
   int key_kind, sig;
   const unsigned long long* part_off;   // partition mode only: [n_parts + 1]
+  const unsigned long long* item_off;   // partition mode only: [n_parts + 1] work items per partition
   int n_parts;
   uint32_t slots, limit;    // shared-memory table of each CTA
   int spec;                 // speculative run (EIGER_AUTO without statistics)
@@ -116,6 +117,8 @@ struct PartitionLaunch {
   unsigned long long* cur2; // [2^(bits1 + bits2)]
   void* keysA; uint64_t* valsA[kMaxVals];   // level-1 output, n rows each
   void* keysB; uint64_t* valsB[kMaxVals];   // level-2 output
+  unsigned long long* item_off;   // [2^(bits1 + bits2) + 1] work items of the aggregation pass
+  int64_t chunk_rows;       // partitions above 2 * chunk_rows rows are cut into items of chunk_rows
   // results
   const void* out_keys; uint64_t* const* out_vals; const unsigned long long* out_off; int n_parts;
 };

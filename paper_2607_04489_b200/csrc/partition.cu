@@ -93,6 +93,35 @@ part_scan_kernel(const uint32_t* __restrict__ hist, unsigned long long* __restri
   if (tid == 1023) off[count] = s_part[1023];
 }
 
+// Work items of the per-partition aggregation pass: a partition much larger than the average (a
+// hot key: C3's top key owns 12 % of the rows) is cut into several items so that one CTA is not
+// left with it; item_off[p] .. item_off[p + 1] are partition p's items (exclusive prefix sum).
+__global__ void __launch_bounds__(1024)
+part_items_kernel(const unsigned long long* __restrict__ off, unsigned long long* __restrict__ item_off,
+                  int count, unsigned long long chunk_rows) {
+  __shared__ unsigned long long s_part[1024];
+  const int tid = threadIdx.x;
+  const int per = (count + 1023) / 1024;
+  const int b = tid * per, e = min(count, b + per);
+  auto items = [&](int p) -> unsigned long long {
+    const unsigned long long rows = off[p + 1] - off[p];
+    return rows == 0 ? 0ull : (rows > 2 * chunk_rows ? (rows + chunk_rows - 1) / chunk_rows : 1ull);
+  };
+  unsigned long long local = 0;
+  for (int p = b; p < e; ++p) local += items(p);
+  s_part[tid] = local;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {
+    const unsigned long long v = tid >= o ? s_part[tid - o] : 0ull;
+    __syncthreads();
+    s_part[tid] += v;
+    __syncthreads();
+  }
+  unsigned long long run = s_part[tid] - local;
+  for (int p = b; p < e; ++p) { item_off[p] = run; run += items(p); }
+  if (tid == 1023) item_off[count] = s_part[1023];
+}
+
 template <int KK, class UO>
 __global__ void __launch_bounds__(kPT, 2)
 part_scatter_kernel(const __grid_constant__ LevelArgs a) {
@@ -257,6 +286,9 @@ int run_levels(PartitionLaunch& L, int sm_count, cudaStream_t s) {
     if (rc) return rc;
     L.out_keys = L.keysB; L.out_vals = L.valsB; L.out_off = L.off2; L.n_parts = 1 << (L.bits1 + L.bits2);
   }
+  part_items_kernel<<<1, 1024, 0, s>>>(L.out_off, L.item_off, L.n_parts, (unsigned long long)L.chunk_rows);
+  count_launch();
+  EIGER_CUDA(cudaGetLastError());
   return EIGER_OK;
 }
 
