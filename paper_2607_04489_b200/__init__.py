@@ -266,8 +266,32 @@ def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int |
         raise ValueError("column length mismatch")
     L = lib()
     ws = workspace or Workspace(dev)
+    def out_cols(cap):
+        ok = [ws.column(("k", i), cap, k.dtype) for i, k in enumerate(keys)]
+        oa = [ws.column(("a", j), cap, torch.float64 if (op != COUNT and vals[c].dtype == torch.float64) else torch.int64)
+              for j, (op, c) in enumerate(aggs)]
+        return ok, oa
+
     with torch.cuda.device(dev):
         if stats is None and n > 0:
+            # one library call, statistics gathered inside it (that is what EIGER_AUTO's time is):
+            # with whatever scratch this Workspace already holds; if the plan the library arrives
+            # at needs more room than that, profile here and size exactly (first call only)
+            kc, vc, ac = _cols(keys, _KEY_T), _cols(vals, _VAL_T), _aggs(aggs)
+            buf = ws.scratch(max(64 << 20, ws.buf.numel() if ws.buf is not None else 0))
+            have = min([t.numel() for t in ws.out.values()], default=0)
+            cap = out_capacity if out_capacity is not None else max(have, 1 << 20)
+            ok, oa = out_cols(cap)
+            okp = (ctypes.c_void_p * 2)(*[t.data_ptr() for t in ok])
+            oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
+            ng, chosen = ctypes.c_int64(0), ctypes.c_int32(0)
+            rc = L.eiger_groupby(kc, len(keys), n, vc, len(vals), ac, len(aggs), None, okp, oap, cap,
+                                 ctypes.byref(ng), force, ctypes.byref(chosen), buf.data_ptr(), buf.numel(), _stream(dev))
+            if rc == OK:
+                g = int(ng.value)
+                return GroupByResult([t[:g] for t in ok], [t[:g] for t in oa], g, int(chosen.value))
+            if rc not in (ERR_WORKSPACE, ERR_TABLE_OVERFLOW) and not (rc == ERR_OUT_CAPACITY and out_capacity is None):
+                _check(rc)
             stats = profile_keys(keys)
         kc, vc, ac, sc = _cols(keys, _KEY_T), _cols(vals, _VAL_T), _aggs(aggs), _stats_arr(stats)
         for attempt in range(3):

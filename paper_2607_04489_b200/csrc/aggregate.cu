@@ -24,6 +24,7 @@ struct AggArgs {
   AggPlan plan;
   int64_t n;
   uint32_t front_slots, front_limit, front_replicas, stride;
+  int32_t spec;
   void* table;
   uint64_t cap;
   CallDev* call;
@@ -68,6 +69,8 @@ struct AggCtx {
   }
 
   __device__ __forceinline__ void row(U u, const uint64_t (&raw)[NV]) {
+    // speculative run planned from a sample: the range is checked exactly here
+    if (a.spec && (uint64_t)u >= a.cap) { if (*reinterpret_cast<volatile uint32_t*>(&a.call->abort) == 0u) atomicOr(&a.call->abort, 1u); return; }
     if constexpr (FRONT == FRONT_PRIV) {
       uint64_t* acc = reinterpret_cast<uint64_t*>(smem) + (size_t)u * (uint32_t)n_acc * blockDim.x + threadIdx.x;
 #pragma unroll
@@ -245,7 +248,7 @@ int launch_one(const AggLaunch& L, cudaStream_t s) {
   if (L.smem_bytes > 48 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
   AggArgs a;
   a.key = L.key; a.plan = L.plan; a.n = L.n;
-  a.front_slots = L.front_slots; a.front_limit = L.front_limit; a.front_replicas = L.front_replicas;
+  a.front_slots = L.front_slots; a.front_limit = L.front_limit; a.front_replicas = L.front_replicas; a.spec = L.spec;
   a.stride = L.stride; a.table = L.table; a.cap = L.cap; a.call = L.call;
   kern<<<L.blocks, kAggThreads, L.smem_bytes, s>>>(a);
   count_launch();

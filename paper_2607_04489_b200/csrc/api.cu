@@ -77,6 +77,10 @@ struct Tunables {
   double load;                        // target load factor of every hash table
   double smem_fill;                   // AUTO takes EIGER_SMEM while ndv <= smem_fill * slots
   int global_front;                   // hot-key shared-memory table in front of the global table
+  int spec;                           // EIGER_AUTO without statistics tries one speculative pass first
+  int global_always;                  // take EIGER_GLOBAL whenever its table fits L2 (not only for skewed keys)
+  double skew_collision;              // sample collision rate above which the keys count as skewed
+  int64_t spec_samples, spec_min_rows;
   Tunables() {
     auto env = [](const char* k, double dflt) { const char* v = std::getenv(k); return v ? std::atof(v) : dflt; };
     smem_table_bytes = (size_t)env("EIGER_SMEM_KB", 200) << 10;
@@ -85,10 +89,15 @@ struct Tunables {
     part_threads = (int)env("EIGER_PART_THREADS", 512);
     part_min_bits = (int)env("EIGER_PART_MIN_BITS", 9);
     direct_l2_bytes = (size_t)env("EIGER_DIRECT_L2_MB", 48) << 20;
-    global_l2_bytes = (size_t)env("EIGER_GLOBAL_L2_MB", 64) << 20;
+    global_l2_bytes = (size_t)env("EIGER_GLOBAL_L2_MB", 192) << 20;
     global_front = (int)env("EIGER_GLOBAL_FRONT", 1);
     load = env("EIGER_LOAD", 0.5);
     smem_fill = env("EIGER_SMEM_FILL", 0.6);
+    spec = (int)env("EIGER_SPEC", 1);
+    global_always = (int)env("EIGER_GLOBAL_ALWAYS", 0);
+    skew_collision = env("EIGER_SKEW_COLLISION", 1e-3);
+    spec_samples = (int64_t)env("EIGER_SPEC_SAMPLES", 1 << 18);
+    spec_min_rows = (int64_t)env("EIGER_SPEC_MIN_ROWS", 1 << 22);
   }
 };
 Tunables tun() { return Tunables(); }
@@ -132,7 +141,7 @@ int detect_sig(const AggPlan& p, int n_user) {
 
 // Step A4: choose the variant and size everything (readings R8-R10).
 int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eiger_col* vals, int nv,
-               const eiger_agg* aggs, int na, const eiger_stats* st, int force, QueryPlan* q) {
+               const eiger_agg* aggs, int na, const eiger_stats* st, int force, QueryPlan* q, bool skewed = false) {
   if (!keys || nk < 1 || nk > 2 || n < 0 || nv < 0 || nv > kMaxVals || na < 1 || na > kMaxAggs || !aggs) return EIGER_ERR_ARG;
   if (nv > 0 && !vals) return EIGER_ERR_ARG;
   if (force < EIGER_AUTO || force > EIGER_PARTITION) return EIGER_ERR_ARG;
@@ -201,7 +210,9 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   const unsigned __int128 direct_bytes = (unsigned __int128)R * 8 * n_acc_direct;
 
   // hash variants: key kind, shared-memory slot size, global slot stride
-  const int hk = (nk == 1 && keys[0].dtype == EIGER_I32 && R != 0 && R <= 0xFFFFFFFFull) ? KK_I32
+  // a single int32 column is hashed as 32-bit keys whatever its range: u = key - min (mod 2^32) is a
+  // bijection, and the one key that may land on the empty marker is kept in the global table
+  const int hk = (nk == 1 && keys[0].dtype == EIGER_I32) ? KK_I32
                  : (nk == 1 && keys[0].dtype == EIGER_I64) ? KK_I64 : KK_GEN;
   const size_t slot_bytes = hash_agg_slot_bytes(p, hk);
   const uint32_t smem_slots = (uint32_t)std::max<size_t>(64, (T.smem_table_bytes - 64) / slot_bytes) & ~7u;   // planes stay 8-byte aligned
@@ -213,8 +224,11 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   if (variant == EIGER_AUTO) {
     if (direct_ok && (direct_bytes * 256 <= T.priv_smem || direct_bytes <= T.sdirect_bytes ||
                       (direct_bytes <= T.direct_l2_bytes && (double)R <= 16.0 * (double)std::max<int64_t>(n, 1)))) variant = EIGER_DIRECT;
-    else if (ndv * (1.0 + 4 * kSigma) <= T.smem_fill * smem_slots) variant = EIGER_SMEM;
-    else if ((unsigned __int128)hash_cap(ndv) * hash_stride <= T.global_l2_bytes) variant = EIGER_GLOBAL;
+    else if (ndv * (1.0 + 4 * kSigma) <= (hk == KK_I32 ? T.smem_fill : 0.6 * T.smem_fill) * smem_slots) variant = EIGER_SMEM;   // 2-key buckets fill up sooner
+    // uniform keys: partition + shared-memory aggregation beats L2 atomics at every size measured
+    // (C5 sweep); a few hot keys in front of a long tail (sample collision rate) is where the global
+    // table with its hot-key front wins (C3), while its table still fits L2
+    else if ((skewed || T.global_always) && (unsigned __int128)hash_cap(ndv) * hash_stride <= T.global_l2_bytes) variant = EIGER_GLOBAL;
     else variant = EIGER_PARTITION;
   }
   q->variant = variant;
@@ -282,27 +296,31 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
 
 // Profiles nk key columns with one read-back: min/max of each, and (single column only) the
 // sketch.  with_hll = 0 is the range-first shortcut: ndv_est = min(n, range).
-int do_profile(Runtime* rt, const eiger_col* cols, int nk, int64_t n, int with_hll, eiger_stats* out, cudaStream_t s) {
+// samples > 0: statistics of an evenly spaced sample of that many keys (plan of the speculative pass).
+int do_profile(Runtime* rt, const eiger_col* cols, int nk, int64_t n, int with_hll, eiger_stats* out, cudaStream_t s,
+               int64_t samples = 0, double* collision = nullptr) {
   if (nk > 1) with_hll = 0;
   {
     Timed t(s, 1);
     for (int k = 0; k < nk; ++k) {
-      int rc = launch_profile(rt, cols[k].data, cols[k].dtype, n, k, with_hll, k == 0, s);
+      int rc = samples > 0 ? launch_profile_sample(rt, cols[k].data, cols[k].dtype, n, samples, k, with_hll, k == 0, s)
+                           : launch_profile(rt, cols[k].data, cols[k].dtype, n, k, with_hll, k == 0, s);
       if (rc) return rc;
     }
     if (with_hll) { int rc = launch_hll_hist(rt, s); if (rc) return rc; }
   }
-  struct Back { long long mn[2], mx[2]; uint32_t hist[64]; };
+  struct Back { long long mn[2], mx[2]; uint32_t hist[64]; uint32_t pair_eq, pair_n; };
   Back* b = static_cast<Back*>(rt->pinned);
   EIGER_CUDA(cudaMemcpyAsync(b, rt->prof, sizeof(Back), cudaMemcpyDeviceToHost, s));
   EIGER_CUDA(cudaStreamSynchronize(s));
   resolve_timing();
+  if (collision) *collision = b->pair_n ? (double)b->pair_eq / (double)b->pair_n : 0.0;
   for (int k = 0; k < nk; ++k) {
     out[k].min = b->mn[k]; out[k].max = b->mx[k]; out[k].n = n;
     if (n == 0) { out[k].ndv_est = 0.0; continue; }
     const double range = (double)((uint64_t)b->mx[k] - (uint64_t)b->mn[k]) + 1.0;
     double est = with_hll ? hll_estimate_from_hist(b->hist) : range;
-    est = std::min(est, std::min((double)n, range));
+    est = std::min(est, std::min((double)(samples > 0 ? std::min(n, samples) : n), range));
     out[k].ndv_est = std::max(est, 0.0);
   }
   return EIGER_OK;
@@ -327,27 +345,16 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     if (chosen) *chosen = force;
     return EIGER_OK;
   }
-  eiger_stats local[2];
-  const eiger_stats* st = stats_in;
-  if (!st) {
-    // profile inside the call: fused min/max + sketch for 4/8-byte keys; 1-byte keys take the
-    // range test only (PAPER.md:219: HLL only when the range test fails; a 1-byte range never does)
-    int rc = do_profile(rt, keys, nk, n, keys[0].dtype != EIGER_I8, local, s);
-    if (rc) return rc;
-    st = local;
-  }
-  QueryPlan q;
-  int rc = plan_query(rt, keys, nk, n, vals, nv, aggs, na, st, force, &q);
-  if (rc) return rc;
-  if (chosen) *chosen = q.variant;
-  if (q.total_bytes > workspace_bytes || !workspace) return EIGER_ERR_WORKSPACE;
   if ((uintptr_t)workspace & 255) return EIGER_ERR_ARG;
-
+  for (int j = 0; j < na; ++j) if (!out_aggs[j] && out_capacity > 0) return EIGER_ERR_ARG;
   char* ws = static_cast<char*>(workspace);
   struct Back { unsigned long long n_groups; uint32_t overflow; uint32_t abort; };
   Back* hb = reinterpret_cast<Back*>(static_cast<char*>(rt->pinned) + 1024);
+  int rc = EIGER_OK;
 
-  for (int j = 0; j < na; ++j) if (!out_aggs[j] && out_capacity > 0) return EIGER_ERR_ARG;
+  // runs plan q; spec != 0: a speculative run that may give up (*aborted) and leaves no result then
+  auto execute = [&](QueryPlan& q, const eiger_stats* st, int spec, bool* aborted) -> int {
+  if (q.total_bytes > workspace_bytes || !workspace) return EIGER_ERR_WORKSPACE;
   const int src_kind = q.key_kind;
   for (int attempt = 0;; ++attempt) {
     // workspace: [table][partition scratch]
@@ -359,7 +366,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     L.key_kind = q.key_kind; L.sig = q.sig; L.front = q.front; L.back = q.back;
     L.front_slots = q.front_slots; L.front_limit = q.front_limit; L.front_replicas = q.front_replicas;
     L.table = table; L.cap = q.cap; L.stride = q.stride; L.call = rt->call;
-    L.threads = 256; L.smem_bytes = q.smem_bytes;
+    L.threads = 256; L.smem_bytes = q.smem_bytes; L.spec = spec;
     { Timed t(s, 3); rc = launch_table_init(L, s); if (rc) return rc; }
 
     if (q.variant == EIGER_DIRECT) {
@@ -373,7 +380,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     } else {
       HashAggLaunch H{};
       H.key = q.key; H.plan = q.plan; H.n = n; H.key_kind = src_kind; H.sig = q.sig;
-      H.slots = q.slots; H.limit = q.limit; H.spec = 0;
+      H.slots = q.slots; H.limit = q.limit; H.spec = spec;
       H.table = table; H.cap = q.cap; H.stride = q.stride; H.call = rt->call;
       H.out_keys[0] = out_keys[0]; H.out_keys[1] = nk == 2 ? out_keys[1] : nullptr;
       for (int j = 0; j < na; ++j) H.out_aggs[j] = out_aggs[j];
@@ -424,6 +431,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     EIGER_CUDA(cudaMemcpyAsync(hb, rt->call, sizeof(Back), cudaMemcpyDeviceToHost, s));
     EIGER_CUDA(cudaStreamSynchronize(s));
     resolve_timing();
+    if (spec && (hb->abort || hb->overflow)) { *aborted = true; return EIGER_OK; }
     if (hb->overflow) {
       // the sketch under-estimated (R10): grow towards the exact bound and run again
       if (q.back != BACK_HASH || attempt >= 8) return EIGER_ERR_TABLE_OVERFLOW;
@@ -449,6 +457,56 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     if ((int64_t)hb->n_groups > out_capacity) return EIGER_ERR_OUT_CAPACITY;
     return EIGER_OK;
   }
+  };
+
+  eiger_stats local[2];
+  const Tunables T = tun();
+  bool skewed = false;
+  if (!stats_in && force == EIGER_AUTO && n >= T.spec_min_rows) {
+    // EIGER_AUTO, no statistics: first the statistics of an evenly spaced sample (one tiny kernel).
+    // When the sample says "few groups" one speculative pass aggregates AND verifies (every key
+    // inside the sampled range / room in every CTA's table), so low-NDV inputs are read exactly
+    // once; otherwise, or if the verification fails, the full profile (A1-A3) and the selected
+    // variant run as usual.  The sample also tells hot-key inputs from uniform ones.
+    double collision = 0.0;
+    rc = do_profile(rt, keys, nk, n, keys[0].dtype != EIGER_I8, local, s, T.spec_samples, &collision);
+    if (rc) return rc;
+    skewed = collision > T.skew_collision;
+    const bool fusable = nk == 1 || (keys[0].dtype == EIGER_I8 && keys[1].dtype == EIGER_I8);
+    for (int k = 0; k < nk; ++k) {       // a little slack around the sampled range (clamped to the key type)
+      const int bits = 8 * dtype_size(keys[k].dtype);
+      const int64_t tmin = bits == 64 ? INT64_MIN : -(1ll << (bits - 1)), tmax = bits == 64 ? INT64_MAX : (1ll << (bits - 1)) - 1;
+      const uint64_t R = (uint64_t)local[k].max - (uint64_t)local[k].min + 1ull;
+      const int64_t margin = (R > 64 && R <= (1ull << 24)) ? (int64_t)(R / 32) : 0;   // only direct tables need the range
+      local[k].min = local[k].min - tmin >= margin ? local[k].min - margin : tmin;
+      local[k].max = tmax - local[k].max >= margin ? local[k].max + margin : tmax;
+      local[k].n = n;
+    }
+    QueryPlan qs;
+    if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] sample: min %lld max %lld ndv %.1f collision %.5f\n", (long long)local[0].min, (long long)local[0].max, local[0].ndv_est, collision);
+    if (T.spec && fusable && plan_query(rt, keys, nk, n, vals, nv, aggs, na, local, EIGER_AUTO, &qs) == EIGER_OK &&
+        ((qs.variant == EIGER_DIRECT && qs.front != FRONT_NONE) ||
+         (qs.variant == EIGER_SMEM && qs.ndv * 1.25 <= 0.6 * qs.slots)) && qs.total_bytes <= workspace_bytes) {
+      bool aborted = false;
+      if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] plan: variant %d kk %d sig %d slots %u limit %u cap %llu stride %u smem %zu front %d R %llu\n", qs.variant, qs.key_kind, qs.sig, qs.slots, qs.limit, (unsigned long long)qs.cap, qs.stride, qs.smem_bytes, qs.front, (unsigned long long)qs.R);
+      rc = execute(qs, local, 1, &aborted);
+      if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] speculative %s: rc %d aborted %d\n", eiger_variant_name(qs.variant), rc, (int)aborted);
+      if (rc != EIGER_OK || !aborted) { if (chosen) *chosen = qs.variant; return rc; }
+    }
+  }
+  const eiger_stats* st = stats_in;
+  if (!st) {
+    // profile inside the call: fused min/max + sketch for 4/8-byte keys; 1-byte keys take the
+    // range test only (PAPER.md:219: HLL only when the range test fails; a 1-byte range never does)
+    rc = do_profile(rt, keys, nk, n, keys[0].dtype != EIGER_I8, local, s);
+    if (rc) return rc;
+    st = local;
+  }
+  QueryPlan q;
+  rc = plan_query(rt, keys, nk, n, vals, nv, aggs, na, st, force, &q, skewed);
+  if (rc) return rc;
+  if (chosen) *chosen = q.variant;
+  return execute(q, st, 0, nullptr);
 }
 
 // ---- device arena for eiger_groupby_host ---------------------------------------------------

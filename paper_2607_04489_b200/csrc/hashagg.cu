@@ -218,9 +218,10 @@ struct Front {
                                            uint32_t* s_count) {
     const uint32_t b0 = home_bucket(u0), b1 = home_bucket(u1);
     const uint4 q0 = load_bucket(b0), q1 = load_bucket(b1);
-    const int h0 = v0 ? resolve(u0, b0, q0, s_count) : -1;
+    // a 32-bit key whose rebased value equals the empty marker lives in the global table only
+    const int h0 = v0 && !(sizeof(U) == 4 && u0 == empty_of<U>()) ? resolve(u0, b0, q0, s_count) : -1;
     __syncwarp();
-    const int h1 = v1 ? resolve(u1, b1, q1, s_count) : -1;
+    const int h1 = v1 && !(sizeof(U) == 4 && u1 == empty_of<U>()) ? resolve(u1, b1, q1, s_count) : -1;
     __syncwarp();
     Pending p0, p1;
     if (h0 >= 0) issue((uint32_t)h0, raw0, p0);
@@ -354,9 +355,11 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
       f.spill(u[b], raw[b], miss, missed);
     };
     int64_t t = blockIdx.x;
+    uint32_t trip = 0;
     if (t < n_tiles) load_tile(0, t);
     while (t < n_tiles) {
-      if (a.spec) { if (__any_sync(0xffffffffu, missed || *reinterpret_cast<volatile uint32_t*>(&a.call->abort))) break; }
+      // speculative run: look at the global give-up flag every 16th trip only (an L2 round trip each time)
+      if (a.spec) { if (__any_sync(0xffffffffu, missed || ((trip++ & 15u) == 0u && *reinterpret_cast<volatile uint32_t*>(&a.call->abort)))) break; }
       if (t + gridDim.x < n_tiles) load_tile(1, t + gridDim.x);
       process_tile(0);
       t += gridDim.x;

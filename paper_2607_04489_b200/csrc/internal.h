@@ -13,6 +13,7 @@ struct ProfileDev {
   long long min[2];
   long long max[2];
   uint32_t hist[64];        // register-value histogram C[0 .. kHllQ + 1]
+  uint32_t pair_eq, pair_n; // sample pass: adjacent sample keys that are equal / compared (skew test)
   uint32_t regs[kHllM];     // sketch registers, one per word (global atomicMax)
 };
 struct CallDev {
@@ -41,6 +42,8 @@ int cuda_fail(cudaError_t e, const char* what);   // records the message, return
 // min/max.  with_hll = 0 skips the sketch (range-first order).
 int launch_profile(Runtime* rt, const void* keys, int dtype, int64_t n, int which, int with_hll,
                    bool reset, cudaStream_t s);
+int launch_profile_sample(Runtime* rt, const void* keys, int dtype, int64_t n, int64_t samples, int which, int with_hll,
+                          bool reset, cudaStream_t s);
 int launch_hll_hist(Runtime* rt, cudaStream_t s);
 int launch_regs_to_bytes(Runtime* rt, uint8_t* out, cudaStream_t s);
 double hll_estimate_from_hist(const uint32_t* hist);
@@ -55,7 +58,8 @@ struct AggLaunch {
   int64_t n;
   int key_kind, sig, front, back;
   // front
-  uint32_t front_slots;     // SDIRECT: R; SHASH: power-of-two slot count; PRIV: R
+  int spec;                 // speculative: a key outside [0, cap) raises call->abort instead of being aggregated
+  uint32_t front_slots;     // SDIRECT: R; PRIV: R
   uint32_t front_limit;     // SHASH: stop inserting new keys beyond this many
   uint32_t front_replicas;  // SDIRECT: table copies per CTA
   // back

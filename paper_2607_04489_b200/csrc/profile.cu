@@ -16,6 +16,7 @@ __global__ void profile_reset_kernel(ProfileDev* out, int with_regs) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t < 2) { out->min[t] = INT64_MAX; out->max[t] = INT64_MIN; }
   if (t < 64) out->hist[t] = 0;
+  if (t == 0) { out->pair_eq = 0; out->pair_n = 0; }
   if (with_regs) for (int i = t; i < kHllM; i += gridDim.x * blockDim.x) out->regs[i] = 0;
 }
 
@@ -131,6 +132,40 @@ profile_kernel(const void* __restrict__ keys, int64_t n, ProfileDev* __restrict_
   }
 }
 
+// Statistics of an evenly spaced SAMPLE of the column (step A1/A2 on `samples` keys): what the
+// speculative single pass of EIGER_AUTO is planned from.  The sample can only under-estimate the
+// range and the NDV; the speculative kernels check both exactly and give up if it did.
+__global__ void __launch_bounds__(256)
+profile_sample_kernel(const void* __restrict__ keys, int dtype, int64_t n, int64_t samples, ProfileDev* __restrict__ out,
+                      int which, int with_hll) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  long long lo = INT64_MAX, hi = INT64_MIN;
+  uint64_t x = 0;
+  if (t < samples) {
+    const int64_t i = (int64_t)(((unsigned __int128)t * (unsigned __int128)n) / (unsigned __int128)samples);
+    x = sext_load(keys, dtype, i);
+    lo = hi = (long long)x;
+    if (with_hll) {
+      const uint64_t z = hll_hash64(x);
+      const uint32_t idx = (uint32_t)(z >> (64 - kHllP));
+      const uint32_t rho = (uint32_t)min(__clzll((long long)(z << kHllP)), kHllQ) + 1u;
+      if (out->regs[idx] < rho) atomicMax(&out->regs[idx], rho);
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+    hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+  }
+  if ((threadIdx.x & 31) == 0 && lo != INT64_MAX) { atomicMin(&out->min[which], lo); atomicMax(&out->max[which], hi); }
+  // skew test: how often two neighbouring sample keys are equal estimates sum p_i^2 (1 / NDV when
+  // uniform, ~0.02 for C3's Zipf); the selector keeps hot-key inputs away from the partitioner
+  const uint64_t nb = __shfl_down_sync(0xffffffffu, x, 1);
+  const bool cmp = (threadIdx.x & 31) < 31 && t + 1 < samples;
+  const uint32_t eq = __ballot_sync(0xffffffffu, cmp && nb == x), nn = __ballot_sync(0xffffffffu, cmp);
+  if ((threadIdx.x & 31) == 0 && which == 0 && nn) { atomicAdd(&out->pair_eq, (uint32_t)__popc(eq)); atomicAdd(&out->pair_n, (uint32_t)__popc(nn)); }
+}
+
 __global__ void hll_hist_kernel(ProfileDev* out) {
   __shared__ uint32_t h[64];
   if (threadIdx.x < 64) h[threadIdx.x] = 0;
@@ -179,6 +214,20 @@ int launch_profile(Runtime* rt, const void* keys, int dtype, int64_t n, int whic
     case EIGER_I64: return launch_profile_dt<EIGER_I64>(rt, keys, n, which, with_hll, s);
     default: return EIGER_ERR_ARG;
   }
+}
+
+int launch_profile_sample(Runtime* rt, const void* keys, int dtype, int64_t n, int64_t samples, int which, int with_hll,
+                          bool reset, cudaStream_t s) {
+  if (reset) {
+    profile_reset_kernel<<<16, 1024, 0, s>>>(rt->prof, 1);
+    count_launch();
+  }
+  if (n > 0 && samples > 0) {
+    profile_sample_kernel<<<(unsigned)((samples + 255) / 256), 256, 0, s>>>(keys, dtype, n, samples, rt->prof, which, with_hll);
+    count_launch();
+  }
+  EIGER_CUDA(cudaGetLastError());
+  return EIGER_OK;
 }
 
 int launch_hll_hist(Runtime* rt, cudaStream_t s) {

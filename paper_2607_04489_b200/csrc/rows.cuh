@@ -33,7 +33,7 @@ __device__ __forceinline__ typename KeyTraits<KK>::U load_u(const KeyDesc& k, in
   } else if constexpr (KK == KK_I8I8) {
     const uint32_t a = (uint32_t)(int32_t)(int8_t)ldg_stream_1((const int8_t*)k.ptr[0] + i) - (uint32_t)k.base[0];
     const uint32_t b = (uint32_t)(int32_t)(int8_t)ldg_stream_1((const int8_t*)k.ptr[1] + i) - (uint32_t)k.base[1];
-    return a * (uint32_t)k.mul + b;
+    return b < (uint32_t)k.mul ? a * (uint32_t)k.mul + b : ~0u;    // ~0: outside the planned range (speculative runs)
   } else {
     uint64_t u = sext_load(k.ptr[0], k.dtype[0], i) - k.base[0];
     if (k.ncols == 2) u = u * k.mul + (sext_load(k.ptr[1], k.dtype[1], i) - k.base[1]);
@@ -54,8 +54,9 @@ __device__ __forceinline__ void load_u2(const KeyDesc& k, int64_t i, typename Ke
   } else if constexpr (KK == KK_I8I8) {
     const uint32_t a = ldg_stream_2((const int8_t*)k.ptr[0] + i), b = ldg_stream_2((const int8_t*)k.ptr[1] + i);
     const uint32_t b0 = (uint32_t)k.base[0], b1 = (uint32_t)k.base[1], m = (uint32_t)k.mul;
-    u[0] = ((uint32_t)(int32_t)(int8_t)(a & 0xFF) - b0) * m + ((uint32_t)(int32_t)(int8_t)(b & 0xFF) - b1);
-    u[1] = ((uint32_t)(int32_t)(int8_t)(a >> 8) - b0) * m + ((uint32_t)(int32_t)(int8_t)(b >> 8) - b1);
+    const uint32_t lo0 = (uint32_t)(int32_t)(int8_t)(b & 0xFF) - b1, lo1 = (uint32_t)(int32_t)(int8_t)(b >> 8) - b1;
+    u[0] = lo0 < m ? ((uint32_t)(int32_t)(int8_t)(a & 0xFF) - b0) * m + lo0 : ~0u;   // ~0: outside the planned range
+    u[1] = lo1 < m ? ((uint32_t)(int32_t)(int8_t)(a >> 8) - b0) * m + lo1 : ~0u;
   } else {
     u[0] = load_u<KK>(k, i); u[1] = load_u<KK>(k, i + 1);
   }

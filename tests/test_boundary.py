@@ -62,6 +62,13 @@ def test_selector_is_callable_without_a_gpu(lib):
     assert pick(0, 15, 16) == eiger.DIRECT
     assert pick(0, (1 << 12) - 1, 1 << 12) == eiger.DIRECT
     assert pick(-(1 << 31), (1 << 31) - 1, 256) == eiger.SMEM
-    assert pick(-(1 << 31), (1 << 31) - 1, 1 << 18) == eiger.GLOBAL
+    # uniform mid-NDV keys go to the partitioner (measured crossover); the
+    # L2-resident global table is AUTO's pick for hot-key inputs only, or when asked for by tunable
+    assert pick(-(1 << 31), (1 << 31) - 1, 1 << 18) == eiger.PARTITION
+    os.environ["EIGER_GLOBAL_ALWAYS"] = "1"
+    try:
+        assert pick(-(1 << 31), (1 << 31) - 1, 1 << 18) == eiger.GLOBAL
+    finally:
+        del os.environ["EIGER_GLOBAL_ALWAYS"]
     assert pick(-(1 << 31), (1 << 31) - 1, 1 << 26) == eiger.PARTITION
     assert eiger.workspace_bytes(fk, fv, aggs, [eiger.Stats(0, 15, 16.0, n)]) >= 256
