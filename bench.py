@@ -166,6 +166,19 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def max_over_ranks(ms: float, dist, device="cuda") -> float:
+    """The slowest rank's time, on every rank (replicas only, no data-path collective)."""
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(rows_per_rank: int, world: int, steps: int, ms: float) -> float:
+    """rows/s of the whole job: all ranks' rows over the slowest rank's time."""
+    return rows_per_rank * world * steps / (ms * 1e-3)
+
+
 def time_steps(fn, steps, warmup, torch, dist=None):
     for _ in range(warmup):
         fn()
@@ -180,11 +193,18 @@ def time_steps(fn, steps, warmup, torch, dist=None):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1)
     if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = max_over_ranks(ms, dist)
         dist.barrier()
-        ms = float(t.item())
     return ms
+
+
+def traffic_from_profiles(workload: str, kernel: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu capture, if there is one."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r1_traffic.json")) as f:
+            return json.load(f).get(f"{workload.split(':')[0].upper()}:{kernel}")
+    except (OSError, ValueError):
+        return None
 
 
 def main(argv=None):
@@ -239,15 +259,18 @@ def main(argv=None):
         assert int(res.aggs[cnt_idx[0]].sum().item()) == ds.n      # sum COUNT = n
 
     rows_total = ds.n * world * args.steps
-    value = rows_total / (ms * 1e-3)
+    value = whole_job_value(ds.n, world, args.steps, ms)
     in_bytes = ds.n * ds.row_bytes
-    agg_ms, agg_n = kt["aggregate"]
     peak, peak_src = measured_hbm_peak()
-    # dominant kernel: the aggregation kernel reads every input byte once
+    # dominant kernel and its algorithmic bytes per launch
     dom = max(("aggregate", "partition", "profile"), key=lambda k: kt[k][0])
-    alg_bytes = {"aggregate": in_bytes if res.variant != eiger.PARTITION else ds.n * 8 * (1 + len(ds.vals)),
-                 "partition": ds.n * (sum(k.element_size() for k in ds.keys) + ds.row_bytes + 8 * (1 + len(ds.vals))),
-                 "profile": ds.n * sum(k.element_size() for k in ds.keys)}[dom]
+    key_bytes = sum(k.element_size() for k in ds.keys)
+    part_row = (4 if (len(ds.keys) == 1 and ds.keys[0].dtype == torch.int32) else 8) + 8 * len(ds.vals)   # B'
+    out_row = key_bytes + 8 * len(ds.aggs)
+    levels = eiger.last_partition_levels() if res.variant == eiger.PARTITION else 0
+    alg_bytes = {"aggregate": in_bytes if res.variant != eiger.PARTITION else ds.n * part_row + res.n_groups * out_row,
+                 "partition": ds.n * (key_bytes + ds.row_bytes + part_row) + max(0, levels - 1) * ds.n * (part_row - 8 * len(ds.vals) + 2 * part_row),
+                 "profile": ds.n * key_bytes}[dom]
     dom_ms, dom_n = kt[dom]
     achieved = (alg_bytes / ((dom_ms / max(dom_n, 1)) * 1e-3)) / 1e9 if dom_ms > 0 else 0.0
     line = {
@@ -262,7 +285,7 @@ def main(argv=None):
         "gpu_launches": launches,
         "kernel_ms_per_step": {k: v[0] / args.steps for k, v in kt.items()},
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak if peak else None, "traffic": None, "peak_source": peak_src,
+                     "frac": achieved / peak if peak else None, "traffic": traffic_from_profiles(args.workload, dom), "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg_bytes, "launches_timed": dom_n},
         "clocks": clocks.summary(),
     }

@@ -140,6 +140,10 @@ int eiger_groupby_host(const eiger_col* keys, int32_t n_key_cols, int64_t n,
                        int64_t* n_groups, int32_t force, int32_t* chosen,
                        int64_t* h2d_bytes, int64_t* d2h_bytes, void* stream);
 
+/* Partition levels (0, 1 or 2) of the last eiger_groupby call that ran EIGER_PARTITION in this
+ * process: bench.py needs it for the algorithmic bytes of the partition pass. */
+int32_t eiger_last_partition_levels(void);
+
 /* Number of kernels this library has launched in this process (bench.py's gpu_launches). */
 int64_t eiger_launch_count(void);
 

@@ -32,7 +32,7 @@ HLL_M = 1 << 14
 EXPORTS = [
     "eiger_profile", "eiger_profile_keys", "eiger_hll_registers", "eiger_hll_estimate_host", "eiger_groupby",
     "eiger_groupby_workspace_bytes", "eiger_select_variant", "eiger_groupby_host",
-    "eiger_launch_count", "eiger_set_kernel_timing", "eiger_kernel_time_ms", "eiger_strerror",
+    "eiger_launch_count", "eiger_last_partition_levels", "eiger_set_kernel_timing", "eiger_kernel_time_ms", "eiger_strerror",
     "eiger_last_cuda_error", "eiger_variant_name", "eiger_shutdown",
 ]
 
@@ -114,6 +114,7 @@ def lib() -> ctypes.CDLL:
                                          ctypes.POINTER(i64), i32, ctypes.POINTER(i32),
                                          ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
         L.eiger_launch_count.restype = i64
+        L.eiger_last_partition_levels.restype = i32
         L.eiger_set_kernel_timing.argtypes = [i32]
         L.eiger_kernel_time_ms.restype = ctypes.c_double
         L.eiger_kernel_time_ms.argtypes = [i32, i32, ctypes.POINTER(i64)]
@@ -363,6 +364,10 @@ def groupby_host(keys, vals, aggs, force: int = AUTO, out_capacity: int | None =
 
 def launch_count() -> int:
     return int(lib().eiger_launch_count())
+
+
+def last_partition_levels() -> int:
+    return int(lib().eiger_last_partition_levels())
 
 
 def set_kernel_timing(enabled: bool) -> None:

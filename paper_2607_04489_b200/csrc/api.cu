@@ -18,6 +18,7 @@ Runtime g_rt;
 std::atomic<int64_t> g_launches{0};
 char g_cuda_err[512] = "";
 bool g_timing = false;
+int g_last_levels = 0;
 constexpr int kTimeSlots = 5;
 double g_time_ms[kTimeSlots] = {0, 0, 0, 0, 0};
 int64_t g_time_n[kTimeSlots] = {0, 0, 0, 0, 0};
@@ -407,6 +408,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
           for (int c = 0; c < q.plan.n_vals; ++c) P.valsB[c] = reinterpret_cast<uint64_t*>(take(col));
         }
         { Timed t(s, 2); rc = launch_partition(P, rt->sm_count, s); if (rc) return rc; }
+        g_last_levels = q.bits2 > 0 ? 2 : 1;
         // the aggregation pass reads the partitioned copy, one CTA per partition at a time
         H.key.ptr[0] = P.out_keys;
         for (int c = 0; c < q.plan.n_vals; ++c) H.plan.vals[c] = P.out_vals[c];
@@ -710,6 +712,7 @@ int eiger_groupby_host(const eiger_col* keys, int32_t nk, int64_t n, const eiger
 }
 
 int64_t eiger_launch_count(void) { return g_launches.load(); }
+int32_t eiger_last_partition_levels(void) { return g_last_levels; }
 
 void eiger_set_kernel_timing(int32_t enabled) { std::lock_guard<std::mutex> lk(g_mu); g_timing = enabled != 0; }
 
