@@ -286,11 +286,31 @@ def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int |
             okp = (ctypes.c_void_p * 2)(*[t.data_ptr() for t in ok])
             oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
             ng, chosen = ctypes.c_int64(0), ctypes.c_int32(0)
-            rc = L.eiger_groupby(kc, len(keys), n, vc, len(vals), ac, len(aggs), None, okp, oap, cap,
-                                 ctypes.byref(ng), force, ctypes.byref(chosen), buf.data_ptr(), buf.numel(), _stream(dev))
-            if rc == OK:
-                g = int(ng.value)
-                return GroupByResult([t[:g] for t in ok], [t[:g] for t in oa], g, int(chosen.value))
+            stats_known = None
+            for attempt in range(3):
+                rc = L.eiger_groupby(kc, len(keys), n, vc, len(vals), ac, len(aggs), None, okp, oap, cap,
+                                     ctypes.byref(ng), force, ctypes.byref(chosen), buf.data_ptr(), buf.numel(), _stream(dev))
+                if rc == OK:
+                    g = int(ng.value)
+                    return GroupByResult([t[:g] for t in ok], [t[:g] for t in oa], g, int(chosen.value))
+                if rc == ERR_OUT_CAPACITY and out_capacity is None:
+                    cap = int(ng.value)                      # the library says how many groups there are
+                elif rc == ERR_WORKSPACE:
+                    # room for whichever variant the library may pick with these statistics
+                    stats_known = stats_known or profile_keys(keys)
+                    sk = _stats_arr(stats_known)
+                    need = max(int(L.eiger_groupby_workspace_bytes(kc, len(keys), n, vc, len(vals), ac, len(aggs), sk, v))
+                               for v in ((GLOBAL, PARTITION) if force == AUTO else (force,)))
+                    if need <= buf.numel():
+                        break
+                    buf = ws.scratch(need + (need >> 3))
+                    if out_capacity is None and len(stats_known) == 1:
+                        cap = max(cap, int(stats_known[0].ndv_est * 1.25) + 1024)
+                else:
+                    break
+                ok, oa = out_cols(cap)
+                okp = (ctypes.c_void_p * 2)(*[t.data_ptr() for t in ok])
+                oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
             if rc not in (ERR_WORKSPACE, ERR_TABLE_OVERFLOW) and not (rc == ERR_OUT_CAPACITY and out_capacity is None):
                 _check(rc)
             stats = profile_keys(keys)

@@ -122,6 +122,8 @@ __device__ __forceinline__ uint64_t ldg_stream_u64(const void* p) {
   return r;
 }
 
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
+
 __device__ __forceinline__ uint64_t sext_load(const void* base, int dtype, int64_t i) {
   switch (dtype) {
     case EIGER_I8: return (uint64_t)(int64_t)(int8_t)ldg_stream_1((const int8_t*)base + i);

@@ -21,6 +21,10 @@ constexpr int kPT = 512;                  // threads per CTA
 constexpr int kPR = 8;                    // rows per thread per tile
 constexpr int kTile = kPT * kPR;          // 4096 rows staged per tile
 constexpr int kMaxFan = 1024;             // partitions per level
+#ifndef EIGER_SCATTER_CTAS
+#define EIGER_SCATTER_CTAS 2
+#endif
+constexpr int kScatterCtas = EIGER_SCATTER_CTAS;
 
 template <int KK> struct SrcKey { using U = typename KeyTraits<KK>::U; };
 
@@ -123,7 +127,7 @@ part_items_kernel(const unsigned long long* __restrict__ off, unsigned long long
 }
 
 template <int KK, class UO>
-__global__ void __launch_bounds__(kPT, 2)
+__global__ void __launch_bounds__(kPT, kScatterCtas)
 part_scatter_kernel(const __grid_constant__ LevelArgs a) {
   using U = typename SrcKey<KK>::U;
   // dynamic shared memory (above the 48 KB static limit): staging buffers, then the counters
@@ -148,6 +152,21 @@ part_scatter_kernel(const __grid_constant__ LevelArgs a) {
   for (int64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
     const int64_t base = r0 + t * kTile;
     const int m = (int)min((int64_t)kTile, r1 - base);
+    // the CTA's next tile is pulled into L2 now: its loads are what this kernel waits for most
+    // (ncu: long_scoreboard 49 % of stall samples with one tile in flight per CTA)
+    {
+      const int64_t nb = base + (int64_t)gridDim.x * kTile;
+      if (nb < r1 && a.key.ncols == 1) {
+        const int64_t nm = min((int64_t)kTile, r1 - nb);
+        const int64_t kbytes = nm * (int64_t)sizeof(U), vbytes = nm * 8;
+        const char* kp = static_cast<const char*>(a.key.ptr[0]) + nb * (int64_t)sizeof(U);
+        for (int64_t o = (int64_t)tid * 128; o < kbytes; o += (int64_t)kPT * 128) prefetch_l2(kp + o);
+        for (int c = 0; c < a.n_vals; ++c) {
+          const char* vp = reinterpret_cast<const char*>(a.vals[c] + nb);
+          for (int64_t o = (int64_t)tid * 128; o < vbytes; o += (int64_t)kPT * 128) prefetch_l2(vp + o);
+        }
+      }
+    }
     // A: keys -> partition ids and ranks inside the tile
     U u[kPR];
     uint32_t pos[kPR];
@@ -170,6 +189,10 @@ part_scatter_kernel(const __grid_constant__ LevelArgs a) {
     }
     __syncthreads();
     // B: exclusive scan of the per-partition counts; claim global space per partition
+    long long gclaim[kPer];
+    uint32_t gcnt[kPer];
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) { gclaim[k] = 0; gcnt[k] = 0; }
     {
       uint32_t c[kPer], sum = 0;
 #pragma unroll
@@ -188,12 +211,14 @@ part_scatter_kernel(const __grid_constant__ LevelArgs a) {
       }
       __syncthreads();
       uint32_t run = s_warp[warp] + inc - sum;
+      // the claims' round trips to L2 overlap the staging below: their results are first needed in D
 #pragma unroll
       for (int k = 0; k < kPer; ++k) {
         const int p = tid * kPer + k;
         if (p < fan) {
           s_loff[p] = run;
-          if (c[k]) s_delta[p] = (long long)atomicAdd(&cursor[p], (unsigned long long)c[k]) - (long long)run;
+          gclaim[k] = c[k] ? (long long)atomicAdd(&cursor[p], (unsigned long long)c[k]) - (long long)run : 0ll;
+          gcnt[k] = c[k];
           s_cnt[p] = 0;
           run += c[k];
         }
@@ -212,6 +237,8 @@ part_scatter_kernel(const __grid_constant__ LevelArgs a) {
         if (a.n_vals > 0) s_val[pos[r]] = v0[r];
       }
     }
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) { const int p = tid * kPer + k; if (p < fan && gcnt[k]) s_delta[p] = gclaim[k]; }
     __syncthreads();
     // D: write runs
 #pragma unroll
