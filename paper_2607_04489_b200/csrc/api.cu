@@ -224,7 +224,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   int variant = force;
   if (variant == EIGER_AUTO) {
     if (direct_ok && (direct_bytes * 256 <= T.priv_smem || direct_bytes <= T.sdirect_bytes ||
-                      (direct_bytes <= T.direct_l2_bytes && (double)R <= 16.0 * (double)std::max<int64_t>(n, 1)))) variant = EIGER_DIRECT;
+                      (!skewed && direct_bytes <= T.direct_l2_bytes && (double)R <= 16.0 * (double)std::max<int64_t>(n, 1)))) variant = EIGER_DIRECT;   // hot keys serialise global atomics
     else if (ndv * (1.0 + 4 * kSigma) <= (hk == KK_I32 ? T.smem_fill : 0.6 * T.smem_fill) * smem_slots) variant = EIGER_SMEM;   // 2-key buckets fill up sooner
     // uniform keys: partition + shared-memory aggregation beats L2 atomics at every size measured
     // (C5 sweep); a few hot keys in front of a long tail (sample collision rate) is where the global
@@ -486,8 +486,8 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     }
     QueryPlan qs;
     if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] sample: min %lld max %lld ndv %.1f collision %.5f\n", (long long)local[0].min, (long long)local[0].max, local[0].ndv_est, collision);
-    if (T.spec && fusable && plan_query(rt, keys, nk, n, vals, nv, aggs, na, local, EIGER_AUTO, &qs) == EIGER_OK &&
-        ((qs.variant == EIGER_DIRECT && qs.front != FRONT_NONE) ||
+    if (T.spec && fusable && plan_query(rt, keys, nk, n, vals, nv, aggs, na, local, EIGER_AUTO, &qs, skewed) == EIGER_OK &&
+        ((qs.variant == EIGER_DIRECT && (qs.front != FRONT_NONE || qs.R <= (1ull << 24))) ||
          (qs.variant == EIGER_SMEM && qs.ndv * 1.25 <= 0.6 * qs.slots)) && qs.total_bytes <= workspace_bytes) {
       bool aborted = false;
       if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] plan: variant %d kk %d sig %d slots %u limit %u cap %llu stride %u smem %zu front %d R %llu\n", qs.variant, qs.key_kind, qs.sig, qs.slots, qs.limit, (unsigned long long)qs.cap, qs.stride, qs.smem_bytes, qs.front, (unsigned long long)qs.R);
