@@ -148,7 +148,18 @@ struct Front {
   // Accumulator updates in two steps so that the returning atomics of several rows are in flight
   // together: issue() fires the 32-bit adds (SUM low word, COUNT) and reads MIN / MAX cells,
   // finish() propagates carries and settles new minima / maxima.
-  struct Pending { uint32_t old[NA]; };
+  // scalars, not an array: ptxas kept `old[NA]` in local memory (STL / LDL between issue and finish)
+  struct Pending {
+    uint32_t o0, o1, o2, o3, o4, o5, o6, o7, o8;
+    __device__ __forceinline__ uint32_t& at(int j) {
+      switch (j) { case 0: return o0; case 1: return o1; case 2: return o2; case 3: return o3; case 4: return o4;
+                   case 5: return o5; case 6: return o6; case 7: return o7; default: return o8; }
+    }
+    __device__ __forceinline__ uint32_t get(int j) const {
+      switch (j) { case 0: return o0; case 1: return o1; case 2: return o2; case 3: return o3; case 4: return o4;
+                   case 5: return o5; case 6: return o6; case 7: return o7; default: return o8; }
+    }
+  };
   __device__ __forceinline__ void issue(uint32_t h, const uint64_t (&raw)[NV], Pending& pd) {
     uint32_t off = 0;
 #pragma unroll
@@ -159,7 +170,7 @@ struct Front {
       if (op == EIGER_COUNT) {
         atomicAdd(reinterpret_cast<uint32_t*>(plane) + h, 1u);
       } else if (add_type(op, f)) {
-        pd.old[j] = atomicAdd(reinterpret_cast<uint32_t*>(plane) + h, (uint32_t)raw[sig_col<SIG>(a.plan, j)]);
+        pd.at(j) = atomicAdd(reinterpret_cast<uint32_t*>(plane) + h, (uint32_t)raw[sig_col<SIG>(a.plan, j)]);
       } else if (op == EIGER_SUM) {
         atomicAdd(reinterpret_cast<double*>(plane) + h, __longlong_as_double((long long)raw[sig_col<SIG>(a.plan, j)]));
       }
@@ -177,7 +188,7 @@ struct Front {
         const uint64_t v = raw[sig_col<SIG>(a.plan, j)];
         if (add_type(op, f)) {
           const uint32_t vl = (uint32_t)v;
-          const uint32_t hi = (uint32_t)(v >> 32) + ((uint32_t)(pd.old[j] + vl) < vl ? 1u : 0u);
+          const uint32_t hi = (uint32_t)(v >> 32) + ((uint32_t)(pd.get(j) + vl) < vl ? 1u : 0u);
           if (hi) atomicAdd(reinterpret_cast<uint32_t*>(plane) + a.slots + h, hi);
         } else if (op != EIGER_SUM) {
           const long long part = (long long)row_partial(op, f, v);
@@ -325,7 +336,7 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
     // ---- whole-input mode: tiles of 2 * T * UNR rows, grid-strided; the next tile's loads are
     // in flight while the current one is processed (one CTA per SM: there is nobody else to
     // hide HBM latency behind) ----
-    constexpr int UNR = !Sig<SIG>::kStatic ? 1 : (NV >= 4 ? 1 : (sizeof(U) == 8 ? 2 : 3));
+    constexpr int UNR = !Sig<SIG>::kStatic ? 1 : (NV >= 4 ? 1 : 2);   // 3 spills at the 64-register cap
     F f(a, smem, a.slots);
     if (tid == 0) { s_count = 0; s_abort = 0; }
     f.init(tid, T);
