@@ -206,3 +206,78 @@ def test_host_entry_point():
     res, h2d, d2h = eiger.groupby_host([k.pin_memory() for k in ds.keys], [v.pin_memory() for v in ds.vals], ds.aggs)
     assert h2d == ds.n * ds.row_bytes and d2h == res.n_groups * (4 + 8 * 4)
     assert_matches(res, want, ds.aggs, ds.vals)
+
+
+# ---- EIGER_AUTO's sample + speculative pass ------------------------------
+SPEC_N = (1 << 22) + 4099          # >= the row count from which AUTO samples and speculates
+
+
+def _auto_matches(ds, expect_variant=None):
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    res = eiger.groupby(d.keys, d.vals, d.aggs)          # AUTO, statistics gathered inside the call
+    assert_matches(res, want, d.aggs, d.vals)
+    if expect_variant is not None:
+        assert res.variant == expect_variant, eiger.VARIANT_NAMES[res.variant]
+    return res
+
+
+@pytest.mark.parametrize("lg,scattered,variant", [(4, False, eiger.DIRECT), (10, False, eiger.DIRECT),
+                                                  (4, True, eiger.SMEM), (11, True, eiger.SMEM),
+                                                  (18, False, eiger.DIRECT), (18, True, eiger.PARTITION)])
+def test_auto_speculative_pass(lg, scattered, variant):
+    _auto_matches(datagen.config5(n=SPEC_N, ndv=1 << lg, scattered=scattered), variant)
+
+
+def test_auto_speculation_gives_up_on_an_outlier():
+    # 16 dense groups and ONE row far outside the range the sample sees: the speculative direct pass
+    # must notice, discard its result and fall back to the full profile; the answer stays exact
+    ds = datagen.config5(n=SPEC_N, ndv=16)
+    ds.keys[0][SPEC_N // 3 + 7] = 1_000_000_007
+    res = _auto_matches(ds)
+    assert res.n_groups == 17
+    ds = datagen.config2(n=SPEC_N)
+    ds.keys[1][12345] = 100                      # an int8 code outside the sampled 0..1
+    res = _auto_matches(ds)
+    assert res.n_groups == 7
+
+
+def test_auto_speculation_gives_up_when_tables_fill():
+    # the sample sees few distinct keys (clustered layout: every CTA's share of the rows is another
+    # set of keys), the per-CTA tables cannot all hold them -> give up, fall back, exact answer
+    n = SPEC_N
+    i = torch.arange(n, dtype=torch.int64)
+    keys = (datagen.fmix32(i // 64) & 0x7FFFFFFF).to(torch.int32)      # 65 K distinct keys in runs of 64
+    vals = datagen.uniform_int(9, 1, i, 0, 1000)
+    _auto_matches(datagen.Dataset("clustered", n, [keys], [vals], [(eiger.SUM, 0), (eiger.COUNT, 0)]))
+
+
+def test_auto_routes_hot_keys_to_the_global_table():
+    ds = datagen.config3(n=SPEC_N, D=200_000)
+    _auto_matches(ds, eiger.GLOBAL)
+
+
+def test_partition_cuts_hot_partitions_into_items():
+    # 2^24 rows over 2^9 partitions: the hot keys' partitions exceed twice the average and are cut
+    # into several work items that merge through the global table
+    ds = datagen.config3(n=1 << 24, D=300_000)
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.PARTITION)
+    assert_matches(res, want, d.aggs, d.vals)
+
+
+def test_two_level_partition():
+    # enough distinct keys for two partition levels (more than 2^10 partitions)
+    ds = datagen.config4(n=6_000_011, D=5_000_000)
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.PARTITION)
+    assert eiger.last_partition_levels() == 2
+    assert_matches(res, want, d.aggs, d.vals)
+    ds = datagen.config5(n=6_000_011, ndv=1 << 22, scattered=True)
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.PARTITION)
+    assert eiger.last_partition_levels() == 2
+    assert_matches(res, want, d.aggs, d.vals)
