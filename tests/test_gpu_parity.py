@@ -243,13 +243,18 @@ def test_auto_speculation_gives_up_on_an_outlier():
 
 
 def test_auto_speculation_gives_up_when_tables_fill():
-    # the sample sees few distinct keys (clustered layout: every CTA's share of the rows is another
-    # set of keys), the per-CTA tables cannot all hold them -> give up, fall back, exact answer
-    n = SPEC_N
+    # n = 2^22 makes the sample stride exactly 16: the sample only sees rows i = 0 mod 16, which
+    # carry 8 scattered keys, while the other rows carry millions of distinct keys.  The plan from the
+    # sample is a shared-memory hash pass; every CTA's table fills up -> give up, fall back, exact
+    n = 1 << 22
     i = torch.arange(n, dtype=torch.int64)
-    keys = (datagen.fmix32(i // 64) & 0x7FFFFFFF).to(torch.int32)      # 65 K distinct keys in runs of 64
+    few = datagen.fmix32((i // 16) % 8 + 1000)
+    many = datagen.fmix32(i + (1 << 24))
+    k = torch.where(i % 16 == 0, few, many)
+    keys = torch.where(k >= (1 << 31), k - (1 << 32), k).to(torch.int32)
     vals = datagen.uniform_int(9, 1, i, 0, 1000)
-    _auto_matches(datagen.Dataset("clustered", n, [keys], [vals], [(eiger.SUM, 0), (eiger.COUNT, 0)]))
+    res = _auto_matches(datagen.Dataset("adversarial", n, [keys], [vals], [(eiger.SUM, 0), (eiger.COUNT, 0)]))
+    assert res.n_groups > 1_000_000
 
 
 def test_auto_routes_hot_keys_to_the_global_table():
