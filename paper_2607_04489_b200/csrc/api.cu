@@ -78,6 +78,7 @@ struct Tunables {
   double load;                        // target load factor of every hash table
   double smem_fill;                   // AUTO takes EIGER_SMEM while ndv <= smem_fill * slots
   int global_front;                   // hot-key shared-memory table in front of the global table
+  int global_front_probes;            // buckets that table looks at per key (1: set-associative cache)
   int spec;                           // EIGER_AUTO without statistics tries one speculative pass first
   int global_always;                  // take EIGER_GLOBAL whenever its table fits L2 (not only for skewed keys)
   double skew_collision;              // sample collision rate above which the keys count as skewed
@@ -92,6 +93,7 @@ struct Tunables {
     direct_l2_bytes = (size_t)env("EIGER_DIRECT_L2_MB", 48) << 20;
     global_l2_bytes = (size_t)env("EIGER_GLOBAL_L2_MB", 192) << 20;
     global_front = (int)env("EIGER_GLOBAL_FRONT", 1);
+    global_front_probes = (int)env("EIGER_GLOBAL_FRONT_PROBES", 1);
     load = env("EIGER_LOAD", 0.5);
     smem_fill = env("EIGER_SMEM_FILL", 0.6);
     spec = (int)env("EIGER_SPEC", 1);
@@ -354,6 +356,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
   int rc = EIGER_OK;
 
   // runs plan q; spec != 0: a speculative run that may give up (*aborted) and leaves no result then
+  const int T_front_probes = tun().global_front_probes;
   auto execute = [&](QueryPlan& q, const eiger_stats* st, int spec, bool* aborted) -> int {
   if (q.total_bytes > workspace_bytes || !workspace) return EIGER_ERR_WORKSPACE;
   const int src_kind = q.key_kind;
@@ -382,6 +385,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       HashAggLaunch H{};
       H.key = q.key; H.plan = q.plan; H.n = n; H.key_kind = src_kind; H.sig = q.sig;
       H.slots = q.slots; H.limit = q.limit; H.spec = spec;
+      H.max_probes = q.variant == EIGER_GLOBAL ? T_front_probes : 0;
       H.table = table; H.cap = q.cap; H.stride = q.stride; H.call = rt->call;
       H.out_keys[0] = out_keys[0]; H.out_keys[1] = nk == 2 ? out_keys[1] : nullptr;
       for (int j = 0; j < na; ++j) H.out_aggs[j] = out_aggs[j];

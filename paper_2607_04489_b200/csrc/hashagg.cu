@@ -34,6 +34,7 @@ struct HashAggArgs {
   int32_t n_parts;
   uint32_t slots;        // shared-memory slots per CTA (any number >= 64)
   uint32_t limit;        // stop inserting new keys beyond this many
+  int32_t max_probes;    // buckets looked at per key (1 = set-associative cache: home bucket or global table)
   int32_t spec;          // speculative: a full table raises call->abort and everybody stops
   void* table; uint64_t cap; uint32_t stride;   // global table
   CallDev* call;
@@ -139,7 +140,7 @@ struct Front {
         }
       } else {
         b = b + 1 == Sn / kB ? 0 : b + 1;
-        if (++probes >= 16) done = true; else q = load_bucket(b);
+        if (++probes >= a.max_probes) done = true; else q = load_bucket(b);
       }
     }
     return res;
@@ -336,7 +337,7 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
     // ---- whole-input mode: tiles of 2 * T * UNR rows, grid-strided; the next tile's loads are
     // in flight while the current one is processed (one CTA per SM: there is nobody else to
     // hide HBM latency behind) ----
-    constexpr int UNR = !Sig<SIG>::kStatic ? 1 : (NV >= 4 ? 1 : 2);   // 3 spills at the 64-register cap
+    constexpr int UNR = !Sig<SIG>::kStatic ? 1 : (NV >= 4 ? 1 : (sizeof(U) == 8 ? 1 : 2));   // 3 spills at the 64-register cap
     F f(a, smem, a.slots);
     if (tid == 0) { s_count = 0; s_abort = 0; }
     f.init(tid, T);
@@ -481,7 +482,7 @@ int launch_one(const HashAggLaunch& L, cudaStream_t s) {
   if (L.smem_bytes > 48 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
   HashAggArgs a;
   a.key = L.key; a.plan = L.plan; a.n = L.n; a.part_off = L.part_off; a.item_off = L.item_off; a.n_parts = L.n_parts;
-  a.slots = L.slots; a.limit = L.limit; a.spec = L.spec;
+  a.slots = L.slots; a.limit = L.limit; a.spec = L.spec; a.max_probes = L.max_probes > 0 ? L.max_probes : 16;
   a.table = L.table; a.cap = L.cap; a.stride = L.stride; a.call = L.call;
   a.out_keys[0] = L.out_keys[0]; a.out_keys[1] = L.out_keys[1];
   for (int j = 0; j < kMaxAggs; ++j) a.out_aggs[j] = static_cast<uint64_t*>(L.out_aggs[j]);

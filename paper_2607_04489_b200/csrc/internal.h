@@ -96,6 +96,7 @@ struct HashAggLaunch {
   const unsigned long long* item_off;   // partition mode only: [n_parts + 1] work items per partition
   int n_parts;
   uint32_t slots, limit;    // shared-memory table of each CTA
+  int max_probes;           // 0 = default (16 buckets); 1 = home bucket only (hot-key cache in front of the global table)
   int spec;                 // speculative run (EIGER_AUTO without statistics)
   void* table; uint64_t cap; uint32_t stride;   // global table (BACK_HASH layout)
   CallDev* call;
