@@ -87,8 +87,8 @@ struct Tunables {
     auto env = [](const char* k, double dflt) { const char* v = std::getenv(k); return v ? std::atof(v) : dflt; };
     smem_table_bytes = (size_t)env("EIGER_SMEM_KB", 200) << 10;
     smem_threads = (int)env("EIGER_SMEM_THREADS", 1024);
-    part_table_bytes = (size_t)env("EIGER_PART_KB", 100) << 10;
-    part_threads = (int)env("EIGER_PART_THREADS", 512);
+    part_table_bytes = (size_t)env("EIGER_PART_KB", 200) << 10;
+    part_threads = (int)env("EIGER_PART_THREADS", 1024);
     part_min_bits = (int)env("EIGER_PART_MIN_BITS", 9);
     direct_l2_bytes = (size_t)env("EIGER_DIRECT_L2_MB", 48) << 20;
     global_l2_bytes = (size_t)env("EIGER_GLOBAL_L2_MB", 192) << 20;

@@ -272,7 +272,15 @@ def test_partition_cuts_hot_partitions_into_items():
     assert_matches(res, want, d.aggs, d.vals)
 
 
-def test_two_level_partition():
+@pytest.fixture
+def small_partition_tables(monkeypatch):
+    # 48 KB per-CTA tables (the tunables are re-read on every call): two partition levels are then
+    # needed at sizes the oracle still handles in seconds
+    monkeypatch.setenv("EIGER_PART_KB", "48")
+    monkeypatch.setenv("EIGER_PART_THREADS", "256")
+
+
+def test_two_level_partition(small_partition_tables):
     # enough distinct keys for two partition levels (more than 2^10 partitions)
     ds = datagen.config4(n=6_000_011, D=5_000_000)
     want = oracle_result(ds)
