@@ -144,6 +144,12 @@ int eiger_groupby_host(const eiger_col* keys, int32_t n_key_cols, int64_t n,
  * process: bench.py needs it for the algorithmic bytes of the partition pass. */
 int32_t eiger_last_partition_levels(void);
 
+/* NDV estimate the last eiger_groupby call in this process planned with (after clamping to
+ * min(n, range)): the full-column sketch, the caller's statistics, or - when EIGER_AUTO settled
+ * EIGER_PARTITION from the sample - the sketch of a hash-space slice of the keys scaled up
+ * (DESIGN.md section 6).  Test hook: the estimate is checked against generators of known NDV. */
+double eiger_last_ndv_estimate(void);
+
 /* Number of kernels this library has launched in this process (bench.py's gpu_launches). */
 int64_t eiger_launch_count(void);
 

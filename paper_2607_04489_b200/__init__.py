@@ -32,7 +32,7 @@ HLL_M = 1 << 14
 EXPORTS = [
     "eiger_profile", "eiger_profile_keys", "eiger_hll_registers", "eiger_hll_estimate_host", "eiger_groupby",
     "eiger_groupby_workspace_bytes", "eiger_select_variant", "eiger_groupby_host",
-    "eiger_launch_count", "eiger_last_partition_levels", "eiger_set_kernel_timing", "eiger_kernel_time_ms", "eiger_strerror",
+    "eiger_launch_count", "eiger_last_partition_levels", "eiger_last_ndv_estimate", "eiger_set_kernel_timing", "eiger_kernel_time_ms", "eiger_strerror",
     "eiger_last_cuda_error", "eiger_variant_name", "eiger_shutdown",
 ]
 
@@ -115,6 +115,7 @@ def lib() -> ctypes.CDLL:
                                          ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
         L.eiger_launch_count.restype = i64
         L.eiger_last_partition_levels.restype = i32
+        L.eiger_last_ndv_estimate.restype = ctypes.c_double
         L.eiger_set_kernel_timing.argtypes = [i32]
         L.eiger_kernel_time_ms.restype = ctypes.c_double
         L.eiger_kernel_time_ms.argtypes = [i32, i32, ctypes.POINTER(i64)]
@@ -388,6 +389,10 @@ def launch_count() -> int:
 
 def last_partition_levels() -> int:
     return int(lib().eiger_last_partition_levels())
+
+
+def last_ndv_estimate() -> float:
+    return float(lib().eiger_last_ndv_estimate())
 
 
 def set_kernel_timing(enabled: bool) -> None:

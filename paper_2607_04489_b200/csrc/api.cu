@@ -19,6 +19,7 @@ std::atomic<int64_t> g_launches{0};
 char g_cuda_err[512] = "";
 bool g_timing = false;
 int g_last_levels = 0;
+double g_last_ndv = 0;
 constexpr int kTimeSlots = 5;
 double g_time_ms[kTimeSlots] = {0, 0, 0, 0, 0};
 int64_t g_time_n[kTimeSlots] = {0, 0, 0, 0, 0};
@@ -83,6 +84,8 @@ struct Tunables {
   int global_always;                  // take EIGER_GLOBAL whenever its table fits L2 (not only for skewed keys)
   double skew_collision;              // sample collision rate above which the keys count as skewed
   int64_t spec_samples, spec_min_rows;
+  int slice;                          // EIGER_AUTO sizes PARTITION from a hash-space slice sketch instead of the full profile
+  double slice_min_keys;              // distinct keys wanted in the slice (relative error 1 / sqrt of it)
   Tunables() {
     auto env = [](const char* k, double dflt) { const char* v = std::getenv(k); return v ? std::atof(v) : dflt; };
     smem_table_bytes = (size_t)env("EIGER_SMEM_KB", 200) << 10;
@@ -101,6 +104,8 @@ struct Tunables {
     skew_collision = env("EIGER_SKEW_COLLISION", 1e-3);
     spec_samples = (int64_t)env("EIGER_SPEC_SAMPLES", 1 << 18);
     spec_min_rows = (int64_t)env("EIGER_SPEC_MIN_ROWS", 1 << 22);
+    slice = (int)env("EIGER_SLICE", 1);
+    slice_min_keys = env("EIGER_SLICE_MIN_KEYS", 2048);
   }
 };
 Tunables tun() { return Tunables(); }
@@ -123,6 +128,7 @@ struct QueryPlan {
   uint64_t cap = 0, cap_bound = 0, cap_hot = 0;
   uint32_t stride = 0;
   size_t table_bytes = 0, part_bytes = 0, total_bytes = 0;
+  const uint32_t* pre_hist = nullptr;   // PARTITION: level-1 histogram taken with key.base at fan-out kPreFan
 };
 
 uint64_t range_of(const eiger_stats& s) {   // max - min + 1, 0 when it is 2^64
@@ -401,6 +407,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         P.hist = reinterpret_cast<uint32_t*>(take(PP * 4));
         P.item_off = reinterpret_cast<unsigned long long*>(take((PP + 1) * 8));
         P.chunk_rows = std::max<int64_t>(32768, n / (int64_t)PP);
+        P.pre_hist = q.pre_hist;
         P.off1 = reinterpret_cast<unsigned long long*>(take((P1 + 1) * 8));
         P.cur1 = reinterpret_cast<unsigned long long*>(take(P1 * 8));
         P.keysA = take(kcol);
@@ -453,6 +460,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         if (rc) return rc;
         q2.cap = std::max(q2.cap, q.cap); q2.table_bytes = align_up((size_t)(q2.cap + 1) * q2.stride, 256);
         q2.total_bytes = q2.table_bytes + q2.part_bytes + 256;
+        q2.key = q.key; q2.pre_hist = q.pre_hist;      // same key base (any base gives the same groups)
         q = q2;
       }
       q.total_bytes = q.table_bytes + q.part_bytes + 256;
@@ -500,6 +508,45 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       if (rc != EIGER_OK || !aborted) { if (chosen) *chosen = qs.variant; return rc; }
     }
   }
+  if (!stats_in && force == EIGER_AUTO && n >= T.spec_min_rows && T.slice && !skewed && nk == 1 && n < (1ll << 32) &&
+      (keys[0].dtype == EIGER_I32 || keys[0].dtype == EIGER_I64)) {
+    // The sample's range and NDV are lower bounds of the column's, and every rule of the selector
+    // is monotone in both: when even the sample's statistics select PARTITION, the full statistics
+    // do too.  What is still missing is the NDV that sizes the fan-out.  Instead of a full-column
+    // sketch, ONE keys-only pass takes the level-1 histogram (which the partitioner needs anyway),
+    // the exact min/max, and the sketch of a hash-space slice of the keys (profile.cu).
+    QueryPlan qp;
+    if (plan_query(rt, keys, nk, n, vals, nv, aggs, na, local, EIGER_AUTO, &qp, skewed) == EIGER_OK && qp.variant == EIGER_PARTITION) {
+      const double ds = std::max(1.0, local[0].ndv_est);
+      uint32_t sel = kPreFan;
+      while (sel > 1 && ds * (double)(sel / 2) / (double)kPreFan >= T.slice_min_keys) sel /= 2;
+      const uint64_t base = (uint64_t)local[0].min;
+      { Timed t(s, 1);
+        rc = launch_part_hist_hll(rt, keys[0].data, keys[0].dtype, n, base, sel, s); if (rc) return rc;
+        rc = launch_hll_hist(rt, s); if (rc) return rc; }
+      struct PBack { long long mn[2], mx[2]; uint32_t hist[64]; uint32_t pair_eq, pair_n; };
+      PBack* b = static_cast<PBack*>(rt->pinned);
+      EIGER_CUDA(cudaMemcpyAsync(b, rt->prof, sizeof(PBack), cudaMemcpyDeviceToHost, s));
+      EIGER_CUDA(cudaStreamSynchronize(s));
+      resolve_timing();
+      eiger_stats st2;
+      st2.min = b->mn[0]; st2.max = b->mx[0]; st2.n = n;
+      const double range = (double)((uint64_t)st2.max - (uint64_t)st2.min) + 1.0;
+      const double slice = hll_estimate_from_hist(b->hist);
+      // 1 / sqrt(slice NDV) sampling error on top of the sketch's own: four of those as head room
+      const double est = slice * (double)kPreFan / (double)sel * (1.0 + 4.0 / std::sqrt(std::max(slice, 1.0)));
+      st2.ndv_est = std::max(1.0, std::min(est, std::min((double)n, range)));
+      if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] slice sketch: sel %u / %d, slice ndv %.1f -> ndv %.1f, min %lld max %lld\n", sel, kPreFan, slice, st2.ndv_est, (long long)st2.min, (long long)st2.max);
+      QueryPlan q;
+      rc = plan_query(rt, keys, nk, n, vals, nv, aggs, na, &st2, EIGER_PARTITION, &q, skewed);
+      if (rc) return rc;
+      q.key.base[0] = base;                 // the histogram was taken with this base
+      q.pre_hist = rt->prof->part_hist;
+      g_last_ndv = st2.ndv_est;
+      if (chosen) *chosen = q.variant;
+      return execute(q, &st2, 0, nullptr);
+    }
+  }
   const eiger_stats* st = stats_in;
   if (!st) {
     // profile inside the call: fused min/max + sketch for 4/8-byte keys; 1-byte keys take the
@@ -512,6 +559,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
   rc = plan_query(rt, keys, nk, n, vals, nv, aggs, na, st, force, &q, skewed);
   if (rc) return rc;
   if (chosen) *chosen = q.variant;
+  g_last_ndv = q.ndv;
   return execute(q, st, 0, nullptr);
 }
 
@@ -717,6 +765,7 @@ int eiger_groupby_host(const eiger_col* keys, int32_t nk, int64_t n, const eiger
 
 int64_t eiger_launch_count(void) { return g_launches.load(); }
 int32_t eiger_last_partition_levels(void) { return g_last_levels; }
+double eiger_last_ndv_estimate(void) { return g_last_ndv; }
 
 void eiger_set_kernel_timing(int32_t enabled) { std::lock_guard<std::mutex> lk(g_mu); g_timing = enabled != 0; }
 

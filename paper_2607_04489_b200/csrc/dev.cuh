@@ -159,6 +159,19 @@ __device__ __forceinline__ uint32_t table_hash32b(uint32_t u) {
   return h ^ (h >> 16);
 }
 
+// partition id of a rebased key: the top bits of the table hash (32-bit keys hash in 32 bits,
+// 64-bit keys in 64); shift = key bits - log2(fan-out), so that the ids of a smaller fan-out are
+// the ids of a larger one shifted right (histograms fold)
+template <class U> __device__ __forceinline__ uint32_t part_id(U u, int shift, uint32_t mask);
+template <> __device__ __forceinline__ uint32_t part_id<uint32_t>(uint32_t u, int shift, uint32_t mask) {
+  return (table_hash32(u) >> shift) & mask;
+}
+template <> __device__ __forceinline__ uint32_t part_id<uint64_t>(uint64_t u, int shift, uint32_t mask) {
+  return (uint32_t)(table_hash64(u) >> shift) & mask;
+}
+constexpr int kPreBits = 10;             // fan-out of the histogram taken together with the slice sketch
+constexpr int kPreFan = 1 << kPreBits;
+
 // ---- accumulator algebra -------------------------------------------------------------
 // fp64 MIN/MAX run on an order-preserving int64 image of the double (an involution).
 __device__ __forceinline__ int64_t f64_order(uint64_t bits) {

@@ -225,22 +225,62 @@ struct Front {
     }
   }
 
-  // two rows at a time: both first probes in flight, then both sets of atomics
+  // position of u in its home bucket b as a slot number, or -1: branch-free, so that the lanes of
+  // a warp take the common case (key already in its home bucket) in lock step.  ok = row is valid
+  // and u is not the empty marker (which would "match" a free position).
+  __device__ __forceinline__ int match_home(const uint4& q, U u, uint32_t b, bool ok) const {
+    int r = -1;
+    if constexpr (sizeof(U) == 4) {
+      r = q.w == u ? 3 : r; r = q.z == u ? 2 : r; r = q.y == u ? 1 : r; r = q.x == u ? 0 : r;
+    } else {
+      const uint64_t k0 = ((uint64_t)q.y << 32) | q.x, k1 = ((uint64_t)q.w << 32) | q.z;
+      r = k1 == u ? 1 : r; r = k0 == u ? 0 : r;
+    }
+    return ok && r >= 0 ? (int)(b * kB) + r : -1;
+  }
+
+  // two rows at a time: both first probes in flight, then both sets of atomics.  Rows whose key is
+  // not in its home bucket yet (new key, or a bucket that overflowed) take the probe loop, one
+  // code copy for both rows.
   // Returns bit 0 / 1 set for a row that found no room (the caller sends those to the global table).
   __device__ __forceinline__ uint32_t pair(U u0, const uint64_t (&raw0)[NV], bool v0, U u1, const uint64_t (&raw1)[NV], bool v1,
                                            uint32_t* s_count) {
     const uint32_t b0 = home_bucket(u0), b1 = home_bucket(u1);
     const uint4 q0 = load_bucket(b0), q1 = load_bucket(b1);
-    // a 32-bit key whose rebased value equals the empty marker lives in the global table only
-    const int h0 = v0 && !(sizeof(U) == 4 && u0 == empty_of<U>()) ? resolve(u0, b0, q0, s_count) : -1;
-    __syncwarp();
-    const int h1 = v1 && !(sizeof(U) == 4 && u1 == empty_of<U>()) ? resolve(u1, b1, q1, s_count) : -1;
-    __syncwarp();
+    // a key whose rebased value equals the empty marker lives in the global table only
+    const bool ok0 = v0 && u0 != empty_of<U>(), ok1 = v1 && u1 != empty_of<U>();
+    int h0, h1;
+    if constexpr (sizeof(U) == 8) {
+      // measured: the branch-free first look pays for 64-bit keys (C3 -3 %, C4 -3.5 %) and costs
+      // 4-8 % for 32-bit keys, whose kernel is bound by shared-memory wavefronts, not issue slots
+      h0 = match_home(q0, u0, b0, ok0); h1 = match_home(q1, u1, b1, ok1);
+      if ((ok0 && h0 < 0) || (ok1 && h1 < 0)) {
+#pragma unroll 1
+        for (int k = 0; k < 2; ++k) {
+          const bool need = k == 0 ? (ok0 && h0 < 0) : (ok1 && h1 < 0);
+          if (need) {
+            const int h = resolve(k == 0 ? u0 : u1, k == 0 ? b0 : b1, k == 0 ? q0 : q1, s_count);
+            if (k == 0) h0 = h; else h1 = h;
+          }
+        }
+      }
+      __syncwarp();
+    } else {
+      h0 = ok0 ? resolve(u0, b0, q0, s_count) : -1;
+      __syncwarp();
+      h1 = ok1 ? resolve(u1, b1, q1, s_count) : -1;
+      __syncwarp();
+    }
     Pending p0, p1;
-    if (h0 >= 0) issue((uint32_t)h0, raw0, p0);
-    if (h1 >= 0) issue((uint32_t)h1, raw1, p1);
-    if (h0 >= 0) finish((uint32_t)h0, raw0, p0);
-    if (h1 >= 0) finish((uint32_t)h1, raw1, p1);
+    if (h0 >= 0 && h1 >= 0) {
+      issue((uint32_t)h0, raw0, p0);
+      issue((uint32_t)h1, raw1, p1);
+      finish((uint32_t)h0, raw0, p0);
+      finish((uint32_t)h1, raw1, p1);
+    } else {
+      if (h0 >= 0) { issue((uint32_t)h0, raw0, p0); finish((uint32_t)h0, raw0, p0); }
+      if (h1 >= 0) { issue((uint32_t)h1, raw1, p1); finish((uint32_t)h1, raw1, p1); }
+    }
     __syncwarp();
     return (v0 && h0 < 0 ? 1u : 0u) | (v1 && h1 < 0 ? 2u : 0u);
   }

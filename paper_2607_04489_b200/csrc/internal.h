@@ -15,6 +15,7 @@ struct ProfileDev {
   uint32_t hist[64];        // register-value histogram C[0 .. kHllQ + 1]
   uint32_t pair_eq, pair_n; // sample pass: adjacent sample keys that are equal / compared (skew test)
   uint32_t regs[kHllM];     // sketch registers, one per word (global atomicMax)
+  uint32_t part_hist[kPreFan];   // rows per level-1 partition at fan-out kPreFan (slice-sketch pass)
 };
 struct CallDev {
   unsigned long long n_groups;   // compaction claim counter
@@ -44,6 +45,10 @@ int launch_profile(Runtime* rt, const void* keys, int dtype, int64_t n, int whic
                    bool reset, cudaStream_t s);
 int launch_profile_sample(Runtime* rt, const void* keys, int dtype, int64_t n, int64_t samples, int which, int with_hll,
                           bool reset, cudaStream_t s);
+// Keys-only pass of EIGER_AUTO when the sample already settles PARTITION: exact min/max, the
+// partition histogram at fan-out kPreFan of u = key - base, and the sketch of the keys whose
+// partition id is below `sel` (a slice of the hash space: NDV = slice NDV * kPreFan / sel).
+int launch_part_hist_hll(Runtime* rt, const void* keys, int dtype, int64_t n, uint64_t base, uint32_t sel, cudaStream_t s);
 int launch_hll_hist(Runtime* rt, cudaStream_t s);
 int launch_regs_to_bytes(Runtime* rt, uint8_t* out, cudaStream_t s);
 double hll_estimate_from_hist(const uint32_t* hist);
@@ -124,6 +129,7 @@ struct PartitionLaunch {
   void* keysB; uint64_t* valsB[kMaxVals];   // level-2 output
   unsigned long long* item_off;   // [2^(bits1 + bits2) + 1] work items of the aggregation pass
   int64_t chunk_rows;       // partitions above 2 * chunk_rows rows are cut into items of chunk_rows
+  const uint32_t* pre_hist; // level-1 histogram already taken at fan-out kPreFan with this key base (or nullptr)
   // results
   const void* out_keys; uint64_t* const* out_vals; const unsigned long long* out_off; int n_parts;
 };

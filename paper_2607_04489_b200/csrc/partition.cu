@@ -28,15 +28,6 @@ constexpr int kScatterCtas = EIGER_SCATTER_CTAS;
 
 template <int KK> struct SrcKey { using U = typename KeyTraits<KK>::U; };
 
-// partition hash: 32-bit keys hash in 32 bits, 64-bit keys in 64; ids come from the top bits
-template <class U> __device__ __forceinline__ uint32_t part_id(U u, int shift, uint32_t mask);
-template <> __device__ __forceinline__ uint32_t part_id<uint32_t>(uint32_t u, int shift, uint32_t mask) {
-  return (table_hash32(u) >> shift) & mask;
-}
-template <> __device__ __forceinline__ uint32_t part_id<uint64_t>(uint64_t u, int shift, uint32_t mask) {
-  return (uint32_t)(table_hash64(u) >> shift) & mask;
-}
-
 struct LevelArgs {
   KeyDesc key;                              // source keys (original columns or a partitioned copy)
   const uint64_t* vals[kMaxVals];
@@ -71,6 +62,17 @@ part_hist_kernel(const __grid_constant__ LevelArgs a) {
   for (; i < r1; i += stride) atomicAdd(&s_hist[part_id<U>(load_u<KK>(a.key, i), a.shift, mask)], 1u);
   __syncthreads();
   for (int p = tid; p < a.fan; p += kPT) if (s_hist[p]) atomicAdd(&a.hist[(size_t)seg * a.fan + p], s_hist[p]);
+}
+
+// level-1 histogram from one already taken at a larger fan-out: ids are top bits of the hash,
+// so partition p of `fan` is partitions [p * g, (p + 1) * g) of `pre_fan`, g = pre_fan / fan
+__global__ void part_fold_kernel(const uint32_t* __restrict__ pre, int pre_fan, uint32_t* __restrict__ hist, int fan) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= fan) return;
+  const int g = pre_fan / fan;
+  uint32_t c = 0;
+  for (int k = 0; k < g; ++k) c += pre[p * g + k];
+  hist[p] = c;
 }
 
 // exclusive prefix sum of `count` 32-bit counts -> 64-bit offsets [count + 1] and cursors [count]
@@ -270,14 +272,18 @@ part_scatter_kernel(const __grid_constant__ LevelArgs a) {
 }
 
 template <int KK>
-int run_level(LevelArgs a, int segments, unsigned long long* off, int sm_count, cudaStream_t s) {
+int run_level(LevelArgs a, int segments, unsigned long long* off, int sm_count, cudaStream_t s, const uint32_t* pre_hist = nullptr) {
   using UO = typename SrcKey<KK>::U;
   const int64_t avg_rows = a.n / segments + 1;
   const int64_t tiles = std::max<int64_t>(1, (avg_rows + kTile - 1) / kTile);
   const int64_t want = segments == 1 ? (int64_t)sm_count * 8 : std::max<int64_t>(1, ((int64_t)sm_count * 8 + segments - 1) / segments);
   const int gx = (int)std::min<int64_t>(tiles, want);
-  EIGER_CUDA(cudaMemsetAsync(a.hist, 0, sizeof(uint32_t) * (size_t)segments * a.fan, s));
-  part_hist_kernel<KK><<<dim3(gx, segments), kPT, 0, s>>>(a);
+  if (pre_hist && segments == 1 && a.fan <= kPreFan) {
+    part_fold_kernel<<<(a.fan + 255) / 256, 256, 0, s>>>(pre_hist, kPreFan, a.hist, a.fan);
+  } else {
+    EIGER_CUDA(cudaMemsetAsync(a.hist, 0, sizeof(uint32_t) * (size_t)segments * a.fan, s));
+    part_hist_kernel<KK><<<dim3(gx, segments), kPT, 0, s>>>(a);
+  }
   count_launch();
   part_scan_kernel<<<1, 1024, 0, s>>>(a.hist, off, a.cursor, segments * a.fan);
   count_launch();
@@ -299,7 +305,7 @@ int run_levels(PartitionLaunch& L, int sm_count, cudaStream_t s) {
   for (int c = 0; c < kMaxVals; ++c) { a.vals[c] = static_cast<const uint64_t*>(L.plan.vals[c]); a.out_vals[c] = L.valsA[c]; }
   a.out_keys = L.keysA; a.seg_off = nullptr; a.hist = L.hist; a.cursor = L.cur1;
   a.fan = 1 << L.bits1; a.shift = W - L.bits1;
-  int rc = run_level<KK>(a, 1, L.off1, sm_count, s);
+  int rc = run_level<KK>(a, 1, L.off1, sm_count, s, L.pre_hist);
   if (rc) return rc;
   L.out_keys = L.keysA; L.out_vals = L.valsA; L.out_off = L.off1; L.n_parts = 1 << L.bits1;
   if (L.bits2 > 0) {

@@ -2,7 +2,9 @@
 // registers of one key column — and the register-histogram / estimator that follow.
 // PAPER.md:30 §1, §4 ("close to the memory bandwidth"), §4.1
 // (HLL++ [14] before the group-by), §4.3 (range first).  Readings R1-R6.
+#include <algorithm>
 #include <cmath>
+#include <type_traits>
 
 #include "internal.h"
 
@@ -18,6 +20,7 @@ __global__ void profile_reset_kernel(ProfileDev* out, int with_regs) {
   if (t < 64) out->hist[t] = 0;
   if (t == 0) { out->pair_eq = 0; out->pair_n = 0; }
   if (with_regs) for (int i = t; i < kHllM; i += gridDim.x * blockDim.x) out->regs[i] = 0;
+  if (with_regs) for (int i = t; i < kPreFan; i += gridDim.x * blockDim.x) out->part_hist[i] = 0;
 }
 
 // One sketch update against the CTA's registers in shared memory: one word per register and
@@ -132,6 +135,95 @@ profile_kernel(const void* __restrict__ keys, int64_t n, ProfileDev* __restrict_
   }
 }
 
+// Keys-only pass that replaces the full profile when the sample has already settled the variant
+// (PARTITION): exact min/max, the level-1 partition histogram at fan-out kPreFan of
+// u = key - base, and the sketch of the keys of partitions [0, sel) only.  Partitions are cut by
+// a hash of the key, so the keys of `sel` of them are a uniform sample of the column's DISTINCT
+// keys whatever their frequencies (distinct sampling): NDV ~ slice NDV * kPreFan / sel with
+// relative error 1 / sqrt(slice NDV), and only sel / kPreFan of the keys pay the 64-bit sketch hash.
+template <int DT>
+__global__ void __launch_bounds__(kProfThreads)
+part_hist_hll_kernel(const void* __restrict__ keys, int64_t n, uint64_t base, uint32_t sel, ProfileDev* __restrict__ out) {
+  using U = typename std::conditional<DT == EIGER_I32, uint32_t, uint64_t>::type;
+  using S = typename std::conditional<DT == EIGER_I32, int, long long>::type;
+  extern __shared__ uint32_t sregs[];   // kHllM sketch words, kPreFan counters, one 64-key queue per warp
+  uint32_t* s_hist = sregs + kHllM;
+  __shared__ long long s_lo[kProfThreads / 32], s_hi[kProfThreads / 32];
+  const int tid = threadIdx.x, lane = tid & 31;
+  S* wq = reinterpret_cast<S*>(s_hist + kPreFan) + (tid >> 5) * 64;
+  for (int i = tid; i < kHllM + kPreFan; i += kProfThreads) sregs[i] = 0;
+  __syncthreads();
+  constexpr int EPV = Elem<DT>::kPerVec;
+  constexpr int kShift = 8 * (int)sizeof(U) - kPreBits;
+  S lo = DT == EIGER_I32 ? (S)INT32_MAX : (S)INT64_MAX, hi = DT == EIGER_I32 ? (S)INT32_MIN : (S)INT64_MIN;
+  int cnt = 0;        // keys waiting in this warp's queue (warp-uniform)
+  // The keys of the slice are a minority spread over all lanes: they are queued per warp and
+  // sketched 32 at a time by a full warp, so the 64-bit sketch hash costs sel / kPreFan of a key's
+  // issue slots instead of a divergent branch that almost every warp would take.
+  auto one = [&](S k) {                  // all 32 lanes of the warp are here
+    lo = min(lo, k); hi = max(hi, k);
+    const uint32_t q = part_id<U>((U)k - (U)base, kShift, kPreFan - 1);
+    atomicAdd(s_hist + q, 1u);
+    const bool in = q < sel;
+    const uint32_t m = __ballot_sync(0xffffffffu, in);
+    if (m) {
+      if (in) wq[cnt + __popc(m & ((1u << lane) - 1u))] = k;
+      cnt += __popc(m);
+      if (cnt >= 32) {
+        __syncwarp();
+        cnt -= 32;
+        hll_update(sregs, (uint64_t)(long long)wq[cnt + lane]);
+        __syncwarp();
+      }
+    }
+  };
+  auto one_tail = [&](S k) {             // any subset of lanes
+    lo = min(lo, k); hi = max(hi, k);
+    const uint32_t q = part_id<U>((U)k - (U)base, kShift, kPreFan - 1);
+    atomicAdd(s_hist + q, 1u);
+    if (q < sel) hll_update(sregs, (uint64_t)(long long)k);
+  };
+  const int64_t nvec = n / EPV;
+  const uint4* vp = static_cast<const uint4*>(keys);
+  const int64_t stride = (int64_t)gridDim.x * kProfThreads;
+  int64_t v = (int64_t)blockIdx.x * kProfThreads + tid;
+  // warp-uniform bound: the whole warp's last vector of the trip is inside the column
+  for (; v - lane + 31 + (kProfUnroll - 1) * stride < nvec; v += kProfUnroll * stride) {
+    uint4 r[kProfUnroll];
+#pragma unroll
+    for (int k = 0; k < kProfUnroll; ++k) r[k] = ldg_stream_16(vp + v + k * stride);
+#pragma unroll
+    for (int k = 0; k < kProfUnroll; ++k) {
+      if constexpr (DT == EIGER_I32) { one((int)r[k].x); one((int)r[k].y); one((int)r[k].z); one((int)r[k].w); }
+      else { one((long long)(((uint64_t)r[k].y << 32) | r[k].x)); one((long long)(((uint64_t)r[k].w << 32) | r[k].z)); }
+    }
+  }
+  for (; v < nvec; v += stride) {
+    const uint4 r = ldg_stream_16(vp + v);
+    if constexpr (DT == EIGER_I32) { one_tail((int)r.x); one_tail((int)r.y); one_tail((int)r.z); one_tail((int)r.w); }
+    else { one_tail((long long)(((uint64_t)r.y << 32) | r.x)); one_tail((long long)(((uint64_t)r.w << 32) | r.z)); }
+  }
+  if (blockIdx.x == 0 && tid < (int)(n - nvec * EPV)) one_tail((S)sext_load(keys, DT, nvec * EPV + tid));
+  __syncwarp();
+  if (lane < cnt) hll_update(sregs, (uint64_t)(long long)wq[lane]);
+  long long lo64 = (long long)lo, hi64 = (long long)hi;
+  if (DT == EIGER_I32) { if (lo > hi) { lo64 = INT64_MAX; hi64 = INT64_MIN; } }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    lo64 = min(lo64, __shfl_xor_sync(0xffffffffu, lo64, o));
+    hi64 = max(hi64, __shfl_xor_sync(0xffffffffu, hi64, o));
+  }
+  if (lane == 0) { s_lo[tid >> 5] = lo64; s_hi[tid >> 5] = hi64; }
+  __syncthreads();
+  if (tid == 0) {
+    for (int w = 1; w < kProfThreads / 32; ++w) { lo64 = min(lo64, s_lo[w]); hi64 = max(hi64, s_hi[w]); }
+    if (lo64 != INT64_MAX) atomicMin(&out->min[0], lo64);
+    if (hi64 != INT64_MIN) atomicMax(&out->max[0], hi64);
+  }
+  for (int i = tid; i < kHllM; i += kProfThreads) { const uint32_t r = sregs[i]; if (r) atomicMax(&out->regs[i], r); }
+  for (int i = tid; i < kPreFan; i += kProfThreads) { const uint32_t c = s_hist[i]; if (c) atomicAdd(&out->part_hist[i], c); }
+}
+
 // Statistics of an evenly spaced SAMPLE of the column (step A1/A2 on `samples` keys): what the
 // speculative single pass of EIGER_AUTO is planned from.  The sample can only under-estimate the
 // range and the NDV; the speculative kernels check both exactly and give up if it did.
@@ -214,6 +306,29 @@ int launch_profile(Runtime* rt, const void* keys, int dtype, int64_t n, int whic
     case EIGER_I64: return launch_profile_dt<EIGER_I64>(rt, keys, n, which, with_hll, s);
     default: return EIGER_ERR_ARG;
   }
+}
+
+int launch_part_hist_hll(Runtime* rt, const void* keys, int dtype, int64_t n, uint64_t base, uint32_t sel, cudaStream_t s) {
+  if (dtype != EIGER_I32 && dtype != EIGER_I64) return EIGER_ERR_ARG;
+  profile_reset_kernel<<<16, 1024, 0, s>>>(rt->prof, 1);
+  count_launch();
+  const int epv = dtype == EIGER_I32 ? 4 : 2;
+  const int64_t nvec = n / epv;
+  const int64_t want = (nvec + (int64_t)kProfThreads * kProfUnroll - 1) / ((int64_t)kProfThreads * kProfUnroll);
+  const int blocks = (int)std::max<int64_t>(1, std::min<int64_t>(want, 2LL * rt->sm_count));
+  const int smem = (kHllM + kPreFan) * 4 + (kProfThreads / 32) * 64 * 8;
+  if (dtype == EIGER_I32) {
+    auto kern = part_hist_hll_kernel<EIGER_I32>;
+    EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    kern<<<blocks, kProfThreads, smem, s>>>(keys, n, base, sel, rt->prof);
+  } else {
+    auto kern = part_hist_hll_kernel<EIGER_I64>;
+    EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    kern<<<blocks, kProfThreads, smem, s>>>(keys, n, base, sel, rt->prof);
+  }
+  count_launch();
+  EIGER_CUDA(cudaGetLastError());
+  return EIGER_OK;
 }
 
 int launch_profile_sample(Runtime* rt, const void* keys, int dtype, int64_t n, int64_t samples, int which, int with_hll,

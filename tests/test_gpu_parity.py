@@ -294,3 +294,31 @@ def test_two_level_partition(small_partition_tables):
     res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.PARTITION)
     assert eiger.last_partition_levels() == 2
     assert_matches(res, want, d.aggs, d.vals)
+
+
+# ---- EIGER_AUTO sizes PARTITION from a hash-space slice sketch ---------
+@pytest.mark.parametrize("cfg,lg", [("c5", 14), ("c5", 18), ("c5", 22), ("c4", 21)])
+def test_auto_slice_sketch(cfg, lg):
+    # the sample settles PARTITION; one keys-only pass gives the level-1 histogram, exact min/max
+    # and the NDV from the sketch of a slice of the partitions.  The estimate is checked against
+    # the generator's exact NDV (head room 4 / sqrt(slice NDV) <= 9 % is added on purpose).
+    D = 1 << lg
+    ds = datagen.config5(n=SPEC_N + 12345, ndv=D, scattered=True) if cfg == "c5" else datagen.config4(n=SPEC_N + 777, D=D)
+    res = _auto_matches(ds, eiger.PARTITION)
+    assert res.n_groups == D
+    est = eiger.last_ndv_estimate()
+    assert 0.93 * D <= est <= 1.20 * D, (est, D)
+
+
+def test_auto_slice_sketch_two_levels(small_partition_tables):
+    ds = datagen.config5(n=SPEC_N, ndv=1 << 22, scattered=True)
+    res = _auto_matches(ds, eiger.PARTITION)
+    assert eiger.last_partition_levels() == 2 and res.n_groups == 1 << 22
+
+
+def test_auto_slice_sketch_off_matches(monkeypatch):
+    # same input through the full-column profile: same groups, and an estimate within the sketch's error
+    monkeypatch.setenv("EIGER_SLICE", "0")
+    D = 1 << 18
+    res = _auto_matches(datagen.config5(n=SPEC_N + 12345, ndv=D, scattered=True), eiger.PARTITION)
+    assert res.n_groups == D and abs(eiger.last_ndv_estimate() - D) <= 4 * 0.008125 * D
