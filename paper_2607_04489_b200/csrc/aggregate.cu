@@ -41,8 +41,13 @@ struct AggCtx {
   const int n_acc;
   unsigned char* smem;
 
+  unsigned char* rep_base;       // FRONT_SDIRECT: this warp's replica of the table
+
   __device__ AggCtx(const AggArgs& args, unsigned char* sm)
-      : a(args), n_acc(S::kStatic ? S::kAcc : args.plan.n_acc), smem(sm) {}
+      : a(args), n_acc(S::kStatic ? S::kAcc : args.plan.n_acc), smem(sm) {
+    const uint32_t rep = args.front_replicas > 1 ? (threadIdx.x >> 5) % args.front_replicas : 0u;
+    rep_base = sm + (size_t)rep * args.front_slots * 8 * (uint32_t)n_acc;
+  }
 
   __device__ void front_init() {
     const int tid = threadIdx.x, T = blockDim.x;
@@ -81,8 +86,7 @@ struct AggCtx {
         *c = combine(op, f, *c, row_partial(op, f, raw[sig_col<SIG>(a.plan, j)]));
       }
     } else if constexpr (FRONT == FRONT_SDIRECT) {
-      const uint32_t rep = a.front_replicas > 1 ? (threadIdx.x >> 5) % a.front_replicas : 0u;
-      unsigned char* base = smem + (size_t)rep * a.front_slots * 8 * (uint32_t)n_acc;
+      unsigned char* base = rep_base;
 #pragma unroll
       for (int j = 0; j < NA; ++j) {
         if (!S::kStatic && j >= n_acc) break;
@@ -91,6 +95,35 @@ struct AggCtx {
       }
     } else {
       back_row(u, raw);
+    }
+  }
+
+  // SUM(int64) + COUNT into the shared-memory array, R rows at a time: all returning adds first,
+  // then the counts, then the carries, so that a row's carry does not wait alone for its atomic
+  // (ncu: short_scoreboard was 28 % of the stall samples with one row at a time)
+  template <int R>
+  __device__ __forceinline__ void rows_sc(const U (&u)[R], const uint64_t (&raw)[R][NV]) {
+    static_assert(SIG == SIG_SC && FRONT == FRONT_SDIRECT, "SUM + COUNT signature only");
+    uint32_t* lo = reinterpret_cast<uint32_t*>(rep_base);
+    uint32_t* cnt = reinterpret_cast<uint32_t*>(rep_base + (size_t)8 * a.front_slots);
+    uint32_t old[R];
+    bool ok[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      ok[r] = !(a.spec && (uint64_t)u[r] >= a.cap);
+      if (ok[r]) old[r] = atomicAdd(lo + (uint32_t)u[r], (uint32_t)raw[r][0]);
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) if (ok[r]) atomicAdd(cnt + (uint32_t)u[r], 1u);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      if (ok[r]) {
+        const uint32_t vl = (uint32_t)raw[r][0];
+        const uint32_t h = (uint32_t)(raw[r][0] >> 32) + ((uint32_t)(old[r] + vl) < vl ? 1u : 0u);
+        if (h) atomicAdd(lo + a.front_slots + (uint32_t)u[r], h);
+      } else if (*reinterpret_cast<volatile uint32_t*>(&a.call->abort) == 0u) {
+        atomicOr(&a.call->abort, 1u);
+      }
     }
   }
 
@@ -119,11 +152,15 @@ struct AggCtx {
         if (lane == 0) back_merge(c / (uint32_t)n_acc, j, v, static_cast<uint64_t*>(a.table) + (uint64_t)(c / (uint32_t)n_acc) * (uint32_t)n_acc);
       }
     } else if constexpr (FRONT == FRONT_SDIRECT) {
-      const uint32_t per = a.front_slots * (uint32_t)n_acc, tot = per * a.front_replicas;
-      for (uint32_t c = tid; c < tot; c += T) {
-        const uint32_t rep = c / per, w = c % per, j = w / a.front_slots, u = w % a.front_slots;
-        const uint64_t v = smem_read(smem + (size_t)rep * a.front_slots * 8 * (uint32_t)n_acc, a.front_slots, (int)j, u,
-                                     sig_op<SIG>(a.plan, (int)j), sig_f64<SIG>(a.plan, (int)j));
+      // the CTA's replicas are combined first: one global atomic per cell and CTA (with 8 replicas of
+      // a 256-slot table the flush of ~900 CTAs otherwise queues millions of atomics on 512 addresses)
+      const uint32_t per = a.front_slots * (uint32_t)n_acc;
+      for (uint32_t w = tid; w < per; w += T) {
+        const uint32_t j = w / a.front_slots, u = w % a.front_slots;
+        const int op = sig_op<SIG>(a.plan, (int)j); const bool f = sig_f64<SIG>(a.plan, (int)j);
+        uint64_t v = smem_read(smem, a.front_slots, (int)j, u, op, f);
+        for (uint32_t rep = 1; rep < a.front_replicas; ++rep)
+          v = combine(op, f, v, smem_read(smem + (size_t)rep * a.front_slots * 8 * (uint32_t)n_acc, a.front_slots, (int)j, u, op, f));
         back_merge(u, (int)j, v, static_cast<uint64_t*>(a.table) + (uint64_t)u * (uint32_t)n_acc);
       }
     }
@@ -166,8 +203,15 @@ aggregate_kernel(const __grid_constant__ AggArgs a) {
         raw[s][0][c] = ((uint64_t)v.y << 32) | v.x; raw[s][1][c] = ((uint64_t)v.w << 32) | v.z;
       }
     }
+    if constexpr (SIG == SIG_SC && FRONT == FRONT_SDIRECT) {
+      U uu[2 * UNR]; uint64_t rr[2 * UNR][NV];
 #pragma unroll
-    for (int s = 0; s < UNR; ++s) { ctx.row(u[s][0], raw[s][0]); ctx.row(u[s][1], raw[s][1]); }
+      for (int s = 0; s < UNR; ++s) { uu[2 * s] = u[s][0]; uu[2 * s + 1] = u[s][1]; rr[2 * s][0] = raw[s][0][0]; rr[2 * s + 1][0] = raw[s][1][0]; }
+      ctx.template rows_sc<2 * UNR>(uu, rr);
+    } else {
+#pragma unroll
+      for (int s = 0; s < UNR; ++s) { ctx.row(u[s][0], raw[s][0]); ctx.row(u[s][1], raw[s][1]); }
+    }
   }
   // ragged tail: row at a time, spread over the whole grid
   for (int64_t i = n_tiles * kTile + (int64_t)blockIdx.x * kAggThreads + tid; i < a.n; i += (int64_t)gridDim.x * kAggThreads) {

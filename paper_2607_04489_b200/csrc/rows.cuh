@@ -98,7 +98,11 @@ __device__ __forceinline__ void smem_add64(uint32_t* lo, uint32_t* hi, uint64_t 
 // accumulator j of a table of S slots that starts at base occupies 8 * S bytes
 __device__ __forceinline__ void smem_merge(unsigned char* base, uint32_t S, int j, uint32_t s, int op, bool f64, uint64_t part) {
   unsigned char* plane = base + (size_t)j * 8 * S;
-  if (add_type(op, f64)) {
+  if (op == EIGER_COUNT) {
+    // a CTA never sees 2^32 rows (that many rows per CTA do not fit the device's memory): no carry,
+    // hence no returning atomic
+    atomicAdd(reinterpret_cast<uint32_t*>(plane) + s, (uint32_t)part);
+  } else if (add_type(op, f64)) {
     uint32_t* lo = reinterpret_cast<uint32_t*>(plane) + s;
     smem_add64(lo, lo + S, part);
   } else if (op == EIGER_SUM) {
