@@ -106,24 +106,24 @@ struct AggCtx {
     static_assert(SIG == SIG_SC && FRONT == FRONT_SDIRECT, "SUM + COUNT signature only");
     uint32_t* lo = reinterpret_cast<uint32_t*>(rep_base);
     uint32_t* cnt = reinterpret_cast<uint32_t*>(rep_base + (size_t)8 * a.front_slots);
-    uint32_t old[R];
-    bool ok[R];
+    if (a.spec) {
+      // speculative run planned from a sample: one key outside the planned range discards the whole
+      // pass anyway, so the trip is skipped as a whole (one branch per R rows, not one per atomic)
+      bool bad = false;
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-      ok[r] = !(a.spec && (uint64_t)u[r] >= a.cap);
-      if (ok[r]) old[r] = atomicAdd(lo + (uint32_t)u[r], (uint32_t)raw[r][0]);
+      for (int r = 0; r < R; ++r) bad = bad || (uint64_t)u[r] >= a.cap;
+      if (bad) { if (*reinterpret_cast<volatile uint32_t*>(&a.call->abort) == 0u) atomicOr(&a.call->abort, 1u); return; }
     }
+    uint32_t old[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) if (ok[r]) atomicAdd(cnt + (uint32_t)u[r], 1u);
+    for (int r = 0; r < R; ++r) old[r] = atomicAdd(lo + (uint32_t)u[r], (uint32_t)raw[r][0]);
+#pragma unroll
+    for (int r = 0; r < R; ++r) atomicAdd(cnt + (uint32_t)u[r], 1u);
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-      if (ok[r]) {
-        const uint32_t vl = (uint32_t)raw[r][0];
-        const uint32_t h = (uint32_t)(raw[r][0] >> 32) + ((uint32_t)(old[r] + vl) < vl ? 1u : 0u);
-        if (h) atomicAdd(lo + a.front_slots + (uint32_t)u[r], h);
-      } else if (*reinterpret_cast<volatile uint32_t*>(&a.call->abort) == 0u) {
-        atomicOr(&a.call->abort, 1u);
-      }
+      const uint32_t vl = (uint32_t)raw[r][0];
+      const uint32_t h = (uint32_t)(raw[r][0] >> 32) + ((uint32_t)(old[r] + vl) < vl ? 1u : 0u);
+      if (h) atomicAdd(lo + a.front_slots + (uint32_t)u[r], h);
     }
   }
 

@@ -17,8 +17,14 @@
 namespace eiger {
 namespace {
 
-constexpr int kPT = 512;                  // threads per CTA
-constexpr int kPR = 8;                    // rows per thread per tile
+#ifndef EIGER_SCATTER_PT
+#define EIGER_SCATTER_PT 512
+#endif
+#ifndef EIGER_SCATTER_PR
+#define EIGER_SCATTER_PR 8
+#endif
+constexpr int kPT = EIGER_SCATTER_PT;     // threads per CTA
+constexpr int kPR = EIGER_SCATTER_PR;     // rows per thread per tile
 constexpr int kTile = kPT * kPR;          // 4096 rows staged per tile
 constexpr int kMaxFan = 1024;             // partitions per level
 #ifndef EIGER_SCATTER_CTAS
