@@ -68,7 +68,8 @@ inline int dtype_size(int d) { return d == EIGER_I8 ? 1 : d == EIGER_I32 ? 4 : 8
 struct Tunables {
   size_t priv_smem = 96 * 1024;       // FRONT_PRIV: private cells of one CTA
   size_t sdirect_bytes = 160 * 1024;  // FRONT_SDIRECT: largest per-CTA direct array
-  size_t sdirect_replica_budget = 64 * 1024;
+  size_t sdirect_replica_budget;
+  int sdirect_max_replicas, sdirect_wide;
   size_t smem_table_bytes;            // EIGER_SMEM / EIGER_GLOBAL: shared-memory table of one CTA (1 CTA per SM)
   int smem_threads;
   size_t part_table_bytes;            // EIGER_PARTITION: shared-memory table of one CTA
@@ -89,6 +90,9 @@ struct Tunables {
   Tunables() {
     auto env = [](const char* k, double dflt) { const char* v = std::getenv(k); return v ? std::atof(v) : dflt; };
     smem_table_bytes = (size_t)env("EIGER_SMEM_KB", 200) << 10;
+    sdirect_replica_budget = (size_t)env("EIGER_SDIRECT_REPLICA_KB", 64) << 10;
+    sdirect_max_replicas = (int)env("EIGER_SDIRECT_MAX_REPLICAS", 8);
+    sdirect_wide = (int)env("EIGER_SDIRECT_WIDE", 1);
     smem_threads = (int)env("EIGER_SMEM_THREADS", 1024);
     part_table_bytes = (size_t)env("EIGER_PART_KB", 200) << 10;
     part_threads = (int)env("EIGER_PART_THREADS", 1024);
@@ -255,7 +259,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
       q->front = FRONT_PRIV; q->front_slots = (uint32_t)R; q->smem_bytes = (size_t)direct_bytes * 256;
     } else if (direct_bytes <= T.sdirect_bytes) {
       q->front = FRONT_SDIRECT; q->front_slots = (uint32_t)R;
-      q->front_replicas = (uint32_t)std::max<size_t>(1, std::min<size_t>(8, T.sdirect_replica_budget / (size_t)direct_bytes));
+      q->front_replicas = (uint32_t)std::max<size_t>(1, std::min<size_t>((size_t)T.sdirect_max_replicas, T.sdirect_replica_budget / (size_t)direct_bytes));
       q->smem_bytes = (size_t)direct_bytes * q->front_replicas;
     } else {
       q->front = FRONT_NONE;
@@ -384,6 +388,11 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       const size_t per_cta = std::max<size_t>(q.smem_bytes, 1024);
       int occ = (int)std::min<size_t>(8, std::max<size_t>(1, (rt->smem_optin + 1024) / (per_cta + 1024)));
       if (q.front == FRONT_NONE) occ = 8;
+      // shared-memory arrays: one 1024-thread CTA per SM.  Measured per 2^28 rows (C5 dense): 256-thread
+      // CTAs reach 0.53 ms only while three of them fit the 196 KB carve-out (65.5 KB arrays), 0.61 ms
+      // at 69.6 KB and 0.93 ms at 128 KB (one CTA = 8 warps per SM); the wide CTA runs 0.51-0.53 ms
+      // at every size from 2^5 to 2^13 slots
+      if (q.front == FRONT_SDIRECT && (tun().sdirect_wide || 3 * (per_cta + 1024) > (196u << 10))) { L.threads = 1024; occ = 1; }
       const int64_t tiles = std::max<int64_t>(1, (n + 1023) / 1024);
       L.blocks = (int)std::min<int64_t>((int64_t)rt->sm_count * occ, tiles);
       { Timed t(s, 0); rc = launch_aggregate(L, s); if (rc) return rc; }
