@@ -341,7 +341,7 @@ def sweep(args, eiger, torch, dev):
                          (lambda: eiger.groupby(ds.keys, ds.vals, ds.aggs, force=v, stats=st, workspace=ws))
                     r = fn()
                     assert r.n_groups == ds.ndv
-                    ms = time_steps(fn, args.steps, 1, torch) / args.steps
+                    ms = time_steps(fn, args.steps, 3, torch) / args.steps
                     row[name] = {"ms": ms, "rows_per_s": n / ms * 1e3, "gb_per_s": n * 12 / ms / 1e6,
                                  "variant": eiger.VARIANT_NAMES[r.variant]}
                 except eiger.EigerError as e:

@@ -94,7 +94,16 @@ double eiger_hll_estimate_host(const uint8_t* regs);
  *   aggs[n_aggs]       n_aggs <= 8; result type: SUM/MIN/MAX of I64 -> int64 (SUM wraps modulo
  *                      2^64), of F64 -> double; COUNT -> int64 row count
  *   stats              HOST, n_key_cols entries from eiger_profile, or NULL: the library then
- *                      profiles inside this call (that is what EIGER_AUTO timing includes)
+ *                      gathers the statistics inside this call (that is what EIGER_AUTO timing
+ *                      includes).  A forced variant runs the full profile.  EIGER_AUTO on
+ *                      n >= 2^22 rows first profiles an evenly spaced sample of 2^18 keys; if
+ *                      that settles DIRECT or SMEM, one speculative pass aggregates and verifies
+ *                      the plan exactly (a key outside the sampled range or a full table discards
+ *                      it); if it settles PARTITION (single I32 / I64 key, no hot keys), one
+ *                      keys-only pass takes min/max, the level-1 partition histogram and the
+ *                      sketch of a hash-space slice of the keys (NDV = slice NDV * 1024 / slice
+ *                      partitions); otherwise, or when verification fails, the full profile
+ *                      (A1-A3) runs.  Results never depend on which of these ran.
  *   out_keys[k]        DEVICE array of out_capacity elements of key column k's dtype
  *   out_aggs[j]        DEVICE array of out_capacity 8-byte elements
  *   n_groups           HOST; number of groups written (order of groups unspecified)
