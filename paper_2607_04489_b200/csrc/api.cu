@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <cstddef>
 #include <cstring>
 #include <mutex>
 
@@ -85,6 +86,8 @@ struct Tunables {
   int global_always;                  // take EIGER_GLOBAL whenever its table fits L2 (not only for skewed keys)
   double skew_collision;              // sample collision rate above which the keys count as skewed
   int64_t spec_samples, spec_min_rows;
+  int hot;                            // skewed inputs: heavy hitters are reduced inside the warp (hashagg.cu)
+  double hot_min_share;               // a key is hot from this share of the sample
   int slice;                          // EIGER_AUTO sizes PARTITION from a hash-space slice sketch instead of the full profile
   double slice_min_keys;              // distinct keys wanted in the slice (relative error 1 / sqrt of it)
   Tunables() {
@@ -108,6 +111,8 @@ struct Tunables {
     skew_collision = env("EIGER_SKEW_COLLISION", 1e-3);
     spec_samples = (int64_t)env("EIGER_SPEC_SAMPLES", 1 << 18);
     spec_min_rows = (int64_t)env("EIGER_SPEC_MIN_ROWS", 1 << 22);
+    hot = (int)env("EIGER_HOT", 1);
+    hot_min_share = env("EIGER_HOT_MIN_SHARE", 0.02);
     slice = (int)env("EIGER_SLICE", 1);
     slice_min_keys = env("EIGER_SLICE_MIN_KEYS", 2048);
   }
@@ -367,6 +372,8 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
 
   // runs plan q; spec != 0: a speculative run that may give up (*aborted) and leaves no result then
   const int T_front_probes = tun().global_front_probes;
+  int hot_n = 0;                 // heavy hitters of the key sample (skewed inputs only)
+  long long hot_key[kMaxHot];
   auto execute = [&](QueryPlan& q, const eiger_stats* st, int spec, bool* aborted) -> int {
   if (q.total_bytes > workspace_bytes || !workspace) return EIGER_ERR_WORKSPACE;
   const int src_kind = q.key_kind;
@@ -401,6 +408,9 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       H.key = q.key; H.plan = q.plan; H.n = n; H.key_kind = src_kind; H.sig = q.sig;
       H.slots = q.slots; H.limit = q.limit; H.spec = spec;
       H.max_probes = q.variant == EIGER_GLOBAL ? T_front_probes : 0;
+      H.n_hot = (!spec && nk == 1 && q.variant != EIGER_PARTITION) ? hot_n : 0;
+      for (int i = 0; i < H.n_hot; ++i) H.hot[i] = (uint64_t)hot_key[i] - q.key.base[0];
+      if (H.n_hot && src_kind == KK_I32) for (int i = 0; i < H.n_hot; ++i) H.hot[i] &= 0xFFFFFFFFull;
       H.table = table; H.cap = q.cap; H.stride = q.stride; H.call = rt->call;
       H.out_keys[0] = out_keys[0]; H.out_keys[1] = nk == 2 ? out_keys[1] : nullptr;
       for (int j = 0; j < na; ++j) H.out_aggs[j] = out_aggs[j];
@@ -495,6 +505,18 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     rc = do_profile(rt, keys, nk, n, keys[0].dtype != EIGER_I8, local, s, T.spec_samples, &collision);
     if (rc) return rc;
     skewed = collision > T.skew_collision;
+    if (skewed && T.hot && nk == 1) {
+      // which keys are the hot ones: the whole-input hash kernel reduces their rows inside the warp
+      { Timed t(s, 1); rc = launch_hot_keys(rt, keys[0].data, keys[0].dtype, n, s); if (rc) return rc; }
+      struct HBack { long long key[kMaxHot]; uint32_t cnt[kMaxHot]; uint32_t n, samples; };
+      HBack* hbk = reinterpret_cast<HBack*>(static_cast<char*>(rt->pinned) + 2048);
+      EIGER_CUDA(cudaMemcpyAsync(hbk, reinterpret_cast<const char*>(rt->prof) + offsetof(ProfileDev, hot_key), sizeof(HBack), cudaMemcpyDeviceToHost, s));
+      EIGER_CUDA(cudaStreamSynchronize(s));
+      resolve_timing();
+      for (uint32_t i = 0; i < hbk->n && i < (uint32_t)kMaxHot; ++i)
+        if ((double)hbk->cnt[i] >= T.hot_min_share * (double)hbk->samples) hot_key[hot_n++] = hbk->key[i];
+      if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] heavy hitters: %d (top share %.3f)\n", hot_n, hbk->n ? (double)hbk->cnt[0] / hbk->samples : 0.0);
+    }
     const bool fusable = nk == 1 || (keys[0].dtype == EIGER_I8 && keys[1].dtype == EIGER_I8);
     for (int k = 0; k < nk; ++k) {       // a little slack around the sampled range (clamped to the key type)
       const int bits = 8 * dtype_size(keys[k].dtype);

@@ -12,6 +12,7 @@ namespace eiger {
 constexpr int kMaxAggs = 8;            // user aggregates per call
 constexpr int kMaxAcc = 9;             // + one hidden COUNT for the direct table's presence test
 constexpr int kMaxVals = 8;
+constexpr int kMaxHot = 8;              // heavy-hitter keys handled outside the hash table
 constexpr int kHllP = 14;              // DESIGN.md R1
 constexpr int kHllM = 1 << kHllP;
 constexpr int kHllQ = 64 - kHllP;      // rho in [1, kHllQ + 1]

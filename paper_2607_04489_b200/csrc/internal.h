@@ -16,6 +16,9 @@ struct ProfileDev {
   uint32_t pair_eq, pair_n; // sample pass: adjacent sample keys that are equal / compared (skew test)
   uint32_t regs[kHllM];     // sketch registers, one per word (global atomicMax)
   uint32_t part_hist[kPreFan];   // rows per level-1 partition at fan-out kPreFan (slice-sketch pass)
+  long long hot_key[kMaxHot];    // heavy hitters of a key sample (hot_keys pass), most frequent first
+  uint32_t hot_cnt[kMaxHot];     // their sample counts
+  uint32_t hot_n, hot_samples;
 };
 struct CallDev {
   unsigned long long n_groups;   // compaction claim counter
@@ -49,6 +52,11 @@ int launch_profile_sample(Runtime* rt, const void* keys, int dtype, int64_t n, i
 // partition histogram at fan-out kPreFan of u = key - base, and the sketch of the keys whose
 // partition id is below `sel` (a slice of the hash space: NDV = slice NDV * kPreFan / sel).
 int launch_part_hist_hll(Runtime* rt, const void* keys, int dtype, int64_t n, uint64_t base, uint32_t sel, cudaStream_t s);
+// Heavy hitters of an evenly spaced key sample (single CTA): keys that own more than ~0.5 % of
+// the sample, at most kMaxHot, into rt->prof->hot_*.  EIGER_AUTO runs it when the sample's
+// collision rate says the keys are skewed; the whole-input hash kernel then reduces those keys'
+// rows inside the warp instead of hammering one shared-memory slot with atomics.
+int launch_hot_keys(Runtime* rt, const void* keys, int dtype, int64_t n, cudaStream_t s);
 int launch_hll_hist(Runtime* rt, cudaStream_t s);
 int launch_regs_to_bytes(Runtime* rt, uint8_t* out, cudaStream_t s);
 double hll_estimate_from_hist(const uint32_t* hist);
@@ -103,6 +111,7 @@ struct HashAggLaunch {
   uint32_t slots, limit;    // shared-memory table of each CTA
   int max_probes;           // 0 = default (16 buckets); 1 = home bucket only (hot-key cache in front of the global table)
   int spec;                 // speculative run (EIGER_AUTO without statistics)
+  uint64_t hot[kMaxHot]; int n_hot;   // whole-input mode: rebased heavy-hitter keys reduced inside the warp
   void* table; uint64_t cap; uint32_t stride;   // global table (BACK_HASH layout)
   CallDev* call;
   void* out_keys[2]; void* out_aggs[kMaxAggs]; int n_out_aggs; int64_t out_capacity;   // partition mode emits

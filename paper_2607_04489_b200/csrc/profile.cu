@@ -301,6 +301,55 @@ profile_sample_kernel(const void* __restrict__ keys, int dtype, int64_t n, int64
   }
 }
 
+// Heavy hitters of 4096 evenly spaced keys: a shared-memory count table (8192 slots), then the
+// slots above 0.4 % of the sample are ranked by one thread.  A heuristic input of the selector:
+// results never depend on it.
+constexpr int kHotSamples = 4096, kHotSlots = 8192, kHotCand = 64;
+constexpr long long kHotEmpty = INT64_MIN + 1;     // a key with this value is simply never reported
+__global__ void __launch_bounds__(1024)
+hot_keys_kernel(const void* __restrict__ keys, int dtype, int64_t n, ProfileDev* __restrict__ out) {
+  extern __shared__ __align__(16) unsigned char hot_smem[];       // 96 KB: keys, then counts
+  unsigned long long* s_k = reinterpret_cast<unsigned long long*>(hot_smem);
+  uint32_t* s_c = reinterpret_cast<uint32_t*>(hot_smem + sizeof(unsigned long long) * kHotSlots);
+  __shared__ long long s_ck[kHotCand];
+  __shared__ uint32_t s_cc[kHotCand], s_n;
+  const int tid = threadIdx.x;
+  for (int i = tid; i < kHotSlots; i += 1024) { s_k[i] = (unsigned long long)kHotEmpty; s_c[i] = 0; }
+  if (tid == 0) s_n = 0;
+  __syncthreads();
+  const int64_t samples = n < kHotSamples ? n : kHotSamples;
+  for (int64_t t = tid; t < samples; t += 1024) {
+    const int64_t i = (int64_t)(((unsigned __int128)t * (unsigned __int128)n) / (unsigned __int128)samples);
+    const unsigned long long x = sext_load(keys, dtype, i);
+    if ((long long)x == kHotEmpty) continue;
+    uint32_t slot = (uint32_t)(table_hash64(x) >> 51);       // 13 bits
+    bool done = false;
+    while (!done) {
+      const unsigned long long prev = atomicCAS(&s_k[slot], (unsigned long long)kHotEmpty, x);
+      if (prev == (unsigned long long)kHotEmpty || prev == x) { atomicAdd(&s_c[slot], 1u); done = true; }
+      else slot = (slot + 1) & (kHotSlots - 1);
+    }
+  }
+  __syncthreads();
+  const uint32_t thr = (uint32_t)(samples / 256 > 4 ? samples / 256 : 4);      // 0.4 % of the sample
+  for (int i = tid; i < kHotSlots; i += 1024) {
+    if (s_c[i] >= thr) { const uint32_t pos = atomicAdd(&s_n, 1u); if (pos < kHotCand) { s_ck[pos] = (long long)s_k[i]; s_cc[pos] = s_c[i]; } }
+  }
+  __syncthreads();
+  if (tid == 0) {
+    const int nc = (int)(s_n < kHotCand ? s_n : kHotCand);
+    int taken = 0;
+    for (; taken < kMaxHot && taken < nc; ++taken) {          // selection of the kMaxHot largest counts
+      int best = taken;
+      for (int c = taken + 1; c < nc; ++c) if (s_cc[c] > s_cc[best]) best = c;
+      const long long k = s_ck[best]; const uint32_t c = s_cc[best];
+      s_ck[best] = s_ck[taken]; s_cc[best] = s_cc[taken]; s_ck[taken] = k; s_cc[taken] = c;
+      out->hot_key[taken] = k; out->hot_cnt[taken] = c;
+    }
+    out->hot_n = (uint32_t)taken; out->hot_samples = (uint32_t)samples;
+  }
+}
+
 __global__ void hll_hist_kernel(ProfileDev* out) {
   __shared__ uint32_t h[64];
   if (threadIdx.x < 64) h[threadIdx.x] = 0;
@@ -384,6 +433,16 @@ int launch_profile_sample(Runtime* rt, const void* keys, int dtype, int64_t n, i
     profile_sample_kernel<<<(unsigned)((samples + 256 * kSamplePer - 1) / (256 * kSamplePer)), 256, 0, s>>>(keys, dtype, n, samples, rt->prof, which, with_hll);
     count_launch();
   }
+  EIGER_CUDA(cudaGetLastError());
+  return EIGER_OK;
+}
+
+int launch_hot_keys(Runtime* rt, const void* keys, int dtype, int64_t n, cudaStream_t s) {
+  if (n <= 0) return EIGER_ERR_ARG;
+  constexpr int smem = kHotSlots * 12;
+  EIGER_CUDA(cudaFuncSetAttribute(hot_keys_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  hot_keys_kernel<<<1, 1024, smem, s>>>(keys, dtype, n, rt->prof);
+  count_launch();
   EIGER_CUDA(cudaGetLastError());
   return EIGER_OK;
 }

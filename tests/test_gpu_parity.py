@@ -322,3 +322,45 @@ def test_auto_slice_sketch_off_matches(monkeypatch):
     D = 1 << 18
     res = _auto_matches(datagen.config5(n=SPEC_N + 12345, ndv=D, scattered=True), eiger.PARTITION)
     assert res.n_groups == D and abs(eiger.last_ndv_estimate() - D) <= 4 * 0.008125 * D
+
+
+# ---- direct-index shared-memory array: the 1024-thread CTA at its size limits ---------------
+@pytest.mark.parametrize("R", [4097, 8192, 10240, 10241])
+def test_direct_wide_array_sizes(R):
+    # SUM + COUNT: 16 bytes per slot, so 10240 slots fill the 160 KB limit of the shared-memory
+    # array and 10241 fall to the global-atomics flavour; every key of the range is present
+    n = 300_007
+    i = torch.arange(n, dtype=torch.int64)
+    keys = ((i * 7919) % R - R // 2).to(torch.int32)
+    vals = (datagen.uniform_int(11, 1, i, 0, (1 << 31) - 2) - (1 << 30)) * 4099          # +-2^42: carries into the high word
+    ds = datagen.Dataset("direct-wide", n, [keys], [vals], [(eiger.SUM, 0), (eiger.COUNT, 0)], ndv=R)
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    for force in (eiger.DIRECT, eiger.AUTO):
+        res = eiger.groupby(d.keys, d.vals, d.aggs, force=force)
+        assert res.variant == eiger.DIRECT and res.n_groups == R
+        assert_matches(res, want, d.aggs, d.vals)
+
+
+def test_direct_wide_array_all_aggregates():
+    # SUM, COUNT, MIN, MAX of int64 and of fp64 on a 3000-slot array (the generic accumulate path
+    # of the 1024-thread CTA)
+    n = 200_003
+    i = torch.arange(n, dtype=torch.int64)
+    keys = ((i * 104729) % 3000).to(torch.int64)
+    for fp in (False, True):
+        vals = datagen.unit_f64(12, 1, i) if fp else datagen.uniform_int(12, 1, i, -1000, 1000)
+        ds = datagen.Dataset("direct-wide-4", n, [keys], [vals], [(eiger.SUM, 0), (eiger.COUNT, 0), (eiger.MIN, 0), (eiger.MAX, 0)],
+                             ndv=3000, exact_f64_sum=fp)
+        want = oracle_result(ds)
+        d = to_dev(ds)
+        res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.DIRECT)
+        assert_matches(res, want, d.aggs, d.vals)
+
+
+def test_heavy_hitters_int32_keys():
+    # Zipf keys as a dense int32 column: the sample flags them as skewed, the heavy hitters (top key
+    # 12 % of the rows) take the warp-private cells of the whole-input hash kernel (32-bit key path)
+    ds = datagen.config3(n=SPEC_N, D=200_000, dense=True)
+    ds = datagen.Dataset("C3-int32", ds.n, [ds.keys[0].to(torch.int32) - 77_000], ds.vals, ds.aggs, ds.ndv, ds.exact_f64_sum, ds.meta)
+    _auto_matches(ds, eiger.GLOBAL)
