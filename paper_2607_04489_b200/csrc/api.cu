@@ -294,7 +294,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
       if (n / (int64_t)P >= 32768) q->cap = q->cap_hot;
       const size_t kb = hk == KK_I32 ? 4 : 8;
       const size_t col = align_up((size_t)n * 8, 256), kcol = align_up((size_t)n * kb, 256);
-      q->part_bytes = align_up(P * 4, 256) + align_up((P + 1) * 8, 256) + align_up((P1 + 1) * 8, 256) + align_up(P1 * 8, 256) +
+      q->part_bytes = align_up(P * 4, 256) + align_up((P + 1) * 8, 256) + align_up((2 * P + 2) * 4, 256) + align_up((P1 + 1) * 8, 256) + align_up(P1 * 8, 256) +
                       (kcol + (size_t)p.n_vals * col);
       if (q->bits2 > 0) q->part_bytes += align_up((P + 1) * 8, 256) + align_up(P * 8, 256) + (kcol + (size_t)p.n_vals * col);
     } else {
@@ -425,6 +425,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         auto take = [&](size_t bytes) { char* r = pws; pws += align_up(bytes, 256); return r; };
         P.hist = reinterpret_cast<uint32_t*>(take(PP * 4));
         P.item_off = reinterpret_cast<unsigned long long*>(take((PP + 1) * 8));
+        P.item_part = reinterpret_cast<uint32_t*>(take((2 * PP + 2) * 4));
         P.chunk_rows = std::max<int64_t>(32768, n / (int64_t)PP);
         P.pre_hist = q.pre_hist;
         P.off1 = reinterpret_cast<unsigned long long*>(take((P1 + 1) * 8));
@@ -443,7 +444,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         H.key.ptr[0] = P.out_keys;
         for (int c = 0; c < q.plan.n_vals; ++c) H.plan.vals[c] = P.out_vals[c];
         H.key_kind = src_kind == KK_I32 ? KK_U32PRE : KK_U64PRE;
-        H.part_off = P.out_off; H.item_off = P.item_off; H.n_parts = P.n_parts;
+        H.part_off = P.out_off; H.item_off = P.item_off; H.item_part = P.item_part; H.n_parts = P.n_parts;
         const int occ = (int)std::max<size_t>(1, std::min<size_t>((size_t)(2048 / q.threads), (rt->smem_optin + 1024) / (q.smem_bytes + 1024)));
         H.blocks = (int)std::min<int64_t>((int64_t)rt->sm_count * occ, (int64_t)P.n_parts + n / P.chunk_rows);
       } else {

@@ -32,6 +32,7 @@ struct HashAggArgs {
   int64_t n;
   const unsigned long long* part_off;   // partition mode: [n_parts + 1] row offsets
   const unsigned long long* item_off;   // partition mode: [n_parts + 1] work items (hot partitions are cut up)
+  const uint32_t* item_part;            // partition mode: partition of each work item
   int32_t n_parts;
   uint32_t slots;        // shared-memory slots per CTA (any number >= 64)
   uint32_t limit;        // stop inserting new keys beyond this many
@@ -550,23 +551,10 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
     // ---- partition mode: work items blockIdx.x, + gridDim.x, ...; an item is a whole partition
     // (this CTA then owns its keys and emits them) or a slice of a hot one (merged through the
     // global table like the whole-input mode) ----
-    __shared__ int s_p;
     const unsigned long long n_items = a.item_off[a.n_parts];
     for (unsigned long long it = blockIdx.x; it < n_items; it += gridDim.x) {
-      // the partition of item `it` (item_off[p] <= it < item_off[p + 1]): a T-ary search, two
-      // dependent L2 round trips instead of log2(n_parts) serial ones by one thread (measured:
-      // the serial search was a third of a small item's time)
-      {
-        const int stride = (a.n_parts + T - 1) / T;
-        const int lo = min(tid * stride, a.n_parts), hi = min(lo + stride, a.n_parts);
-        if (lo < hi && a.item_off[lo] <= it && it < a.item_off[hi]) s_p = lo;
-        __syncthreads();
-        const int base = s_p;
-        __syncthreads();
-        if (tid < stride && base + tid < a.n_parts && a.item_off[base + tid] <= it && it < a.item_off[base + tid + 1]) s_p = base + tid;
-        __syncthreads();
-      }
-      const int p = s_p;
+      // the partition of item `it`: one broadcast load from the map written by part_items_kernel
+      const int p = (int)a.item_part[it];
       const unsigned long long n_chunks = a.item_off[p + 1] - a.item_off[p], ci = it - a.item_off[p];
       const int64_t P0 = (int64_t)a.part_off[p], P1 = (int64_t)a.part_off[p + 1];
       const int64_t per = (P1 - P0 + (int64_t)n_chunks - 1) / (int64_t)n_chunks;
@@ -629,7 +617,7 @@ int launch_one(const HashAggLaunch& L, cudaStream_t s) {
   auto kern = hash_agg_kernel<KK, SIG>;
   if (L.smem_bytes > 48 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
   HashAggArgs a;
-  a.key = L.key; a.plan = L.plan; a.n = L.n; a.part_off = L.part_off; a.item_off = L.item_off; a.n_parts = L.n_parts;
+  a.key = L.key; a.plan = L.plan; a.n = L.n; a.part_off = L.part_off; a.item_off = L.item_off; a.item_part = L.item_part; a.n_parts = L.n_parts;
   a.slots = L.slots; a.limit = L.limit; a.spec = L.spec; a.max_probes = L.max_probes > 0 ? L.max_probes : 16;
   a.n_hot = (L.spec || IsPre<KK>::v) ? 0 : std::min(L.n_hot, kMaxHot);
   for (int i = 0; i < kMaxHot; ++i) a.hot[i] = i < a.n_hot ? L.hot[i] : 0ull;

@@ -107,6 +107,7 @@ struct HashAggLaunch {
   int key_kind, sig;
   const unsigned long long* part_off;   // partition mode only: [n_parts + 1]
   const unsigned long long* item_off;   // partition mode only: [n_parts + 1] work items per partition
+  const uint32_t* item_part;            // partition mode only: [items] partition of each work item
   int n_parts;
   uint32_t slots, limit;    // shared-memory table of each CTA
   int max_probes;           // 0 = default (16 buckets); 1 = home bucket only (hot-key cache in front of the global table)
@@ -137,6 +138,7 @@ struct PartitionLaunch {
   void* keysA; uint64_t* valsA[kMaxVals];   // level-1 output, n rows each
   void* keysB; uint64_t* valsB[kMaxVals];   // level-2 output
   unsigned long long* item_off;   // [2^(bits1 + bits2) + 1] work items of the aggregation pass
+  uint32_t* item_part;            // [2 * 2^(bits1 + bits2) + 2] partition of each work item
   int64_t chunk_rows;       // partitions above 2 * chunk_rows rows are cut into items of chunk_rows
   const uint32_t* pre_hist; // level-1 histogram already taken at fan-out kPreFan with this key base (or nullptr)
   // results

@@ -110,7 +110,7 @@ part_scan_kernel(const uint32_t* __restrict__ hist, unsigned long long* __restri
 // left with it; item_off[p] .. item_off[p + 1] are partition p's items (exclusive prefix sum).
 __global__ void __launch_bounds__(1024)
 part_items_kernel(const unsigned long long* __restrict__ off, unsigned long long* __restrict__ item_off,
-                  int count, unsigned long long chunk_rows) {
+                  uint32_t* __restrict__ item_part, int count, unsigned long long chunk_rows) {
   __shared__ unsigned long long s_part[1024];
   const int tid = threadIdx.x;
   const int per = (count + 1023) / 1024;
@@ -130,7 +130,13 @@ part_items_kernel(const unsigned long long* __restrict__ off, unsigned long long
     __syncthreads();
   }
   unsigned long long run = s_part[tid] - local;
-  for (int p = b; p < e; ++p) { item_off[p] = run; run += items(p); }
+  // item -> partition map: the aggregation pass reads its partition with one broadcast load
+  for (int p = b; p < e; ++p) {
+    item_off[p] = run;
+    const unsigned long long k = items(p);
+    for (unsigned long long i = 0; i < k; ++i) item_part[run + i] = (uint32_t)p;
+    run += k;
+  }
   if (tid == 1023) item_off[count] = s_part[1023];
 }
 
@@ -325,7 +331,7 @@ int run_levels(PartitionLaunch& L, int sm_count, cudaStream_t s) {
     if (rc) return rc;
     L.out_keys = L.keysB; L.out_vals = L.valsB; L.out_off = L.off2; L.n_parts = 1 << (L.bits1 + L.bits2);
   }
-  part_items_kernel<<<1, 1024, 0, s>>>(L.out_off, L.item_off, L.n_parts, (unsigned long long)L.chunk_rows);
+  part_items_kernel<<<1, 1024, 0, s>>>(L.out_off, L.item_off, L.item_part, L.n_parts, (unsigned long long)L.chunk_rows);
   count_launch();
   EIGER_CUDA(cudaGetLastError());
   return EIGER_OK;
