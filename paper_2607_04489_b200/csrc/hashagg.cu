@@ -494,33 +494,40 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
         }
       }
     };
-    auto process_tile = [&](int b) {
-      uint32_t miss = 0;
-      bool ab[2 * UNR];
+    // the tile loop, compiled twice: with and without the heavy-hitter look (runtime row-valid flags
+    // and the hot-key scan cost the plain path 5-15 % at low NDV when they were merely branched over)
+    auto run_tiles = [&](auto hot_c) {
+      constexpr bool HOT = decltype(hot_c)::value;
+      auto process_tile = [&](int b) {
+        uint32_t miss = 0;
+        if constexpr (HOT) {
+          bool ab[2 * UNR];
 #pragma unroll
-      for (int r = 0; r < 2 * UNR; ++r) ab[r] = false;
-      if (a.n_hot) {
+          for (int r = 0; r < 2 * UNR; ++r) ab[r] = f.hot_absorb(u[b][r], raw[b][r], my_hot, my_hot_rows, tid & 31);
 #pragma unroll
-        for (int r = 0; r < 2 * UNR; ++r) ab[r] = f.hot_absorb(u[b][r], raw[b][r], my_hot, my_hot_rows, tid & 31);
+          for (int s = 0; s < UNR; ++s) miss |= f.pair(u[b][2 * s], raw[b][2 * s], !ab[2 * s], u[b][2 * s + 1], raw[b][2 * s + 1], !ab[2 * s + 1], &s_count) << (2 * s);
+        } else {
+#pragma unroll
+          for (int s = 0; s < UNR; ++s) miss |= f.pair(u[b][2 * s], raw[b][2 * s], true, u[b][2 * s + 1], raw[b][2 * s + 1], true, &s_count) << (2 * s);
+        }
+        f.spill(u[b], raw[b], miss, missed);
+      };
+      int64_t t = blockIdx.x;
+      uint32_t trip = 0;
+      if (t < n_tiles) load_tile(0, t);
+      while (t < n_tiles) {
+        // speculative run: look at the global give-up flag every 16th trip only (an L2 round trip each time)
+        if (a.spec) { if (__any_sync(0xffffffffu, missed || ((trip++ & 15u) == 0u && *reinterpret_cast<volatile uint32_t*>(&a.call->abort)))) break; }
+        if (t + gridDim.x < n_tiles) load_tile(1, t + gridDim.x);
+        process_tile(0);
+        t += gridDim.x;
+        if (t >= n_tiles) break;
+        if (t + gridDim.x < n_tiles) load_tile(0, t + gridDim.x);
+        process_tile(1);
+        t += gridDim.x;
       }
-#pragma unroll
-      for (int s = 0; s < UNR; ++s) miss |= f.pair(u[b][2 * s], raw[b][2 * s], !ab[2 * s], u[b][2 * s + 1], raw[b][2 * s + 1], !ab[2 * s + 1], &s_count) << (2 * s);
-      f.spill(u[b], raw[b], miss, missed);
     };
-    int64_t t = blockIdx.x;
-    uint32_t trip = 0;
-    if (t < n_tiles) load_tile(0, t);
-    while (t < n_tiles) {
-      // speculative run: look at the global give-up flag every 16th trip only (an L2 round trip each time)
-      if (a.spec) { if (__any_sync(0xffffffffu, missed || ((trip++ & 15u) == 0u && *reinterpret_cast<volatile uint32_t*>(&a.call->abort)))) break; }
-      if (t + gridDim.x < n_tiles) load_tile(1, t + gridDim.x);
-      process_tile(0);
-      t += gridDim.x;
-      if (t >= n_tiles) break;
-      if (t + gridDim.x < n_tiles) load_tile(0, t + gridDim.x);
-      process_tile(1);
-      t += gridDim.x;
-    }
+    if (a.n_hot) run_tiles(std::true_type{}); else run_tiles(std::false_type{});
     if (!(a.spec && __any_sync(0xffffffffu, missed))) {
       // ragged tail: row at a time, spread over the whole grid, warp-uniform trip count
       const int lane = tid & 31;

@@ -247,58 +247,35 @@ part_hist_hll_kernel(const void* __restrict__ keys, int64_t n, uint64_t base, ui
 // Statistics of an evenly spaced SAMPLE of the column (step A1/A2 on `samples` keys): what the
 // speculative single pass of EIGER_AUTO is planned from.  The sample can only under-estimate the
 // range and the NDV; the speculative kernels check both exactly and give up if it did.
-constexpr int kSamplePer = 4;      // consecutive samples per thread (independent loads in flight)
 __global__ void __launch_bounds__(256)
 profile_sample_kernel(const void* __restrict__ keys, int dtype, int64_t n, int64_t samples, ProfileDev* __restrict__ out,
                       int which, int with_hll) {
-  __shared__ long long s_lo[8], s_hi[8];
-  __shared__ uint32_t s_eq[8], s_nn[8];
-  const int64_t t0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * kSamplePer;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   long long lo = INT64_MAX, hi = INT64_MIN;
-  uint64_t x[kSamplePer];
-#pragma unroll
-  for (int k = 0; k < kSamplePer; ++k) {
-    const int64_t t = t0 + k;
-    x[k] = 0;
-    if (t < samples) {
-      const int64_t i = (int64_t)(((unsigned __int128)t * (unsigned __int128)n) / (unsigned __int128)samples);
-      x[k] = sext_load(keys, dtype, i);
+  uint64_t x = 0;
+  if (t < samples) {
+    const int64_t i = (int64_t)(((unsigned __int128)t * (unsigned __int128)n) / (unsigned __int128)samples);
+    x = sext_load(keys, dtype, i);
+    lo = hi = (long long)x;
+    if (with_hll) {
+      const uint64_t z = hll_hash64(x);
+      const uint32_t idx = (uint32_t)(z >> (64 - kHllP));
+      const uint32_t rho = (uint32_t)min(__clzll((long long)(z << kHllP)), kHllQ) + 1u;
+      if (out->regs[idx] < rho) atomicMax(&out->regs[idx], rho);
     }
   }
-#pragma unroll
-  for (int k = 0; k < kSamplePer; ++k) {
-    if (t0 + k < samples) {
-      lo = min(lo, (long long)x[k]); hi = max(hi, (long long)x[k]);
-      if (with_hll) {
-        const uint64_t z = hll_hash64(x[k]);
-        const uint32_t idx = (uint32_t)(z >> (64 - kHllP));
-        const uint32_t rho = (uint32_t)min(__clzll((long long)(z << kHllP)), kHllQ) + 1u;
-        if (out->regs[idx] < rho) atomicMax(&out->regs[idx], rho);
-      }
-    }
-  }
-  // skew test: how often two neighbouring sample keys are equal estimates sum p_i^2 (1 / NDV when
-  // uniform, ~0.02 for C3's Zipf); the selector keeps hot-key inputs away from the partitioner
-  uint32_t eq = 0, nn = 0;
-#pragma unroll
-  for (int k = 0; k + 1 < kSamplePer; ++k) if (t0 + k + 1 < samples) { ++nn; eq += x[k] == x[k + 1] ? 1u : 0u; }
-  const uint64_t nb = __shfl_down_sync(0xffffffffu, x[0], 1);
-  if (lane < 31 && t0 + kSamplePer < samples) { ++nn; eq += nb == x[kSamplePer - 1] ? 1u : 0u; }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
     lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
     hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
-    eq += __shfl_xor_sync(0xffffffffu, eq, o);
-    nn += __shfl_xor_sync(0xffffffffu, nn, o);
   }
-  if (lane == 0) { s_lo[warp] = lo; s_hi[warp] = hi; s_eq[warp] = eq; s_nn[warp] = nn; }
-  __syncthreads();
-  if (threadIdx.x == 0) {      // one set of global atomics per CTA
-    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) { lo = min(lo, s_lo[w]); hi = max(hi, s_hi[w]); eq += s_eq[w]; nn += s_nn[w]; }
-    if (lo != INT64_MAX) { atomicMin(&out->min[which], lo); atomicMax(&out->max[which], hi); }
-    if (which == 0 && nn) { atomicAdd(&out->pair_eq, eq); atomicAdd(&out->pair_n, nn); }
-  }
+  if ((threadIdx.x & 31) == 0 && lo != INT64_MAX) { atomicMin(&out->min[which], lo); atomicMax(&out->max[which], hi); }
+  // skew test: how often two neighbouring sample keys are equal estimates sum p_i^2 (1 / NDV when
+  // uniform, ~0.02 for C3's Zipf); the selector keeps hot-key inputs away from the partitioner
+  const uint64_t nb = __shfl_down_sync(0xffffffffu, x, 1);
+  const bool cmp = (threadIdx.x & 31) < 31 && t + 1 < samples;
+  const uint32_t eq = __ballot_sync(0xffffffffu, cmp && nb == x), nn = __ballot_sync(0xffffffffu, cmp);
+  if ((threadIdx.x & 31) == 0 && which == 0 && nn) { atomicAdd(&out->pair_eq, (uint32_t)__popc(eq)); atomicAdd(&out->pair_n, (uint32_t)__popc(nn)); }
 }
 
 // Heavy hitters of 4096 evenly spaced keys: a shared-memory count table (8192 slots), then the
@@ -430,7 +407,7 @@ int launch_profile_sample(Runtime* rt, const void* keys, int dtype, int64_t n, i
     count_launch();
   }
   if (n > 0 && samples > 0) {
-    profile_sample_kernel<<<(unsigned)((samples + 256 * kSamplePer - 1) / (256 * kSamplePer)), 256, 0, s>>>(keys, dtype, n, samples, rt->prof, which, with_hll);
+    profile_sample_kernel<<<(unsigned)((samples + 255) / 256), 256, 0, s>>>(keys, dtype, n, samples, rt->prof, which, with_hll);
     count_launch();
   }
   EIGER_CUDA(cudaGetLastError());
