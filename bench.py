@@ -272,8 +272,10 @@ def main(argv=None):
     part_row = (4 if (len(ds.keys) == 1 and ds.keys[0].dtype == torch.int32) else 8) + 8 * len(ds.vals)   # B'
     out_row = key_bytes + 8 * len(ds.aggs)
     levels = eiger.last_partition_levels() if res.variant == eiger.PARTITION else 0
+    # EIGER_AUTO's slice-sketch pass already took the level-1 histogram: no keys-only read in the partition pass
+    hist1_bytes = 0 if (res.variant == eiger.PARTITION and eiger.last_partition_prehist()) else ds.n * key_bytes
     alg_bytes = {"aggregate": in_bytes if res.variant != eiger.PARTITION else ds.n * part_row + res.n_groups * out_row,
-                 "partition": ds.n * (key_bytes + ds.row_bytes + part_row) + max(0, levels - 1) * ds.n * (part_row - 8 * len(ds.vals) + 2 * part_row),
+                 "partition": hist1_bytes + ds.n * (ds.row_bytes + part_row) + max(0, levels - 1) * ds.n * (part_row - 8 * len(ds.vals) + 2 * part_row),
                  "profile": ds.n * key_bytes}[dom]
     dom_ms, dom_n = kt[dom]
     achieved = (alg_bytes / ((dom_ms / max(dom_n, 1)) * 1e-3)) / 1e9 if dom_ms > 0 else 0.0
@@ -341,8 +343,12 @@ def sweep(args, eiger, torch, dev):
                          (lambda: eiger.groupby(ds.keys, ds.vals, ds.aggs, force=v, stats=st, workspace=ws))
                     r = fn()
                     assert r.n_groups == ds.ndv
-                    ms = time_steps(fn, args.steps, 3, torch) / args.steps
-                    row[name] = {"ms": ms, "rows_per_s": n / ms * 1e3, "gb_per_s": n * 12 / ms / 1e6,
+                    # sub-millisecond calls get more timed steps (>= ~30 ms in all): 5 steps of a 0.6 ms
+                    # call are 3 ms of timing and moved by +-7 % from run to run
+                    est = time_steps(fn, 2, 3, torch) / 2
+                    k = max(args.steps, min(50, int(30.0 / max(est, 1e-3))))
+                    ms = time_steps(fn, k, 0, torch) / k
+                    row[name] = {"ms": ms, "steps": k, "rows_per_s": n / ms * 1e3, "gb_per_s": n * 12 / ms / 1e6,
                                  "variant": eiger.VARIANT_NAMES[r.variant]}
                 except eiger.EigerError as e:
                     row[name] = {"error": e.code}

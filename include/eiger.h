@@ -96,7 +96,7 @@ double eiger_hll_estimate_host(const uint8_t* regs);
  *   stats              HOST, n_key_cols entries from eiger_profile, or NULL: the library then
  *                      gathers the statistics inside this call (that is what EIGER_AUTO timing
  *                      includes).  A forced variant runs the full profile.  EIGER_AUTO on
- *                      n >= 2^22 rows first profiles an evenly spaced sample of 2^18 keys; if
+ *                      n >= 2^22 rows first profiles an evenly spaced sample of 2^16 keys; if
  *                      that settles DIRECT or SMEM, one speculative pass aggregates and verifies
  *                      the plan exactly (a key outside the sampled range or a full table discards
  *                      it); if it settles PARTITION (single I32 / I64 key, no hot keys), one
@@ -158,6 +158,11 @@ int32_t eiger_last_partition_levels(void);
  * EIGER_PARTITION from the sample - the sketch of a hash-space slice of the keys scaled up
  * (DESIGN.md section 6).  Test hook: the estimate is checked against generators of known NDV. */
 double eiger_last_ndv_estimate(void);
+
+/* 1 when the last EIGER_PARTITION call took its level-1 histogram from the statistics pass
+ * (EIGER_AUTO's slice-sketch pass reads the keys once for both), 0 when the partitioner ran its own
+ * keys-only histogram pass: bench.py needs it for the algorithmic bytes of the partition pass. */
+int32_t eiger_last_partition_prehist(void);
 
 /* Number of kernels this library has launched in this process (bench.py's gpu_launches). */
 int64_t eiger_launch_count(void);

@@ -21,6 +21,7 @@ char g_cuda_err[512] = "";
 bool g_timing = false;
 int g_last_levels = 0;
 double g_last_ndv = 0;
+int g_last_prehist = 0;
 constexpr int kTimeSlots = 5;
 double g_time_ms[kTimeSlots] = {0, 0, 0, 0, 0};
 int64_t g_time_n[kTimeSlots] = {0, 0, 0, 0, 0};
@@ -109,7 +110,7 @@ struct Tunables {
     spec = (int)env("EIGER_SPEC", 1);
     global_always = (int)env("EIGER_GLOBAL_ALWAYS", 0);
     skew_collision = env("EIGER_SKEW_COLLISION", 1e-3);
-    spec_samples = (int64_t)env("EIGER_SPEC_SAMPLES", 1 << 18);
+    spec_samples = (int64_t)env("EIGER_SPEC_SAMPLES", 1 << 16);
     spec_min_rows = (int64_t)env("EIGER_SPEC_MIN_ROWS", 1 << 22);
     hot = (int)env("EIGER_HOT", 1);
     hot_min_share = env("EIGER_HOT_MIN_SHARE", 0.02);
@@ -440,6 +441,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         }
         { Timed t(s, 2); rc = launch_partition(P, rt->sm_count, s); if (rc) return rc; }
         g_last_levels = q.bits2 > 0 ? 2 : 1;
+        g_last_prehist = q.pre_hist ? 1 : 0;
         // the aggregation pass reads the partitioned copy, one CTA per partition at a time
         H.key.ptr[0] = P.out_keys;
         for (int c = 0; c < q.plan.n_vals; ++c) H.plan.vals[c] = P.out_vals[c];
@@ -505,7 +507,8 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     double collision = 0.0;
     rc = do_profile(rt, keys, nk, n, keys[0].dtype != EIGER_I8, local, s, T.spec_samples, &collision);
     if (rc) return rc;
-    skewed = collision > T.skew_collision;
+    // uniform keys collide at rate 1 / NDV: "skewed" means well above that (and above the floor)
+    skewed = collision > T.skew_collision && collision * std::max(local[0].ndv_est, 1.0) > 4.0;
     if (skewed && T.hot && nk == 1) {
       // which keys are the hot ones: the whole-input hash kernel reduces their rows inside the warp
       { Timed t(s, 1); rc = launch_hot_keys(rt, keys[0].data, keys[0].dtype, n, s); if (rc) return rc; }
@@ -798,6 +801,7 @@ int eiger_groupby_host(const eiger_col* keys, int32_t nk, int64_t n, const eiger
 int64_t eiger_launch_count(void) { return g_launches.load(); }
 int32_t eiger_last_partition_levels(void) { return g_last_levels; }
 double eiger_last_ndv_estimate(void) { return g_last_ndv; }
+int32_t eiger_last_partition_prehist(void) { return g_last_prehist; }
 
 void eiger_set_kernel_timing(int32_t enabled) { std::lock_guard<std::mutex> lk(g_mu); g_timing = enabled != 0; }
 
