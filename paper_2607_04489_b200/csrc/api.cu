@@ -87,6 +87,7 @@ struct Tunables {
   int global_always;                  // take EIGER_GLOBAL whenever its table fits L2 (not only for skewed keys)
   double skew_collision;              // sample collision rate above which the keys count as skewed
   int64_t spec_samples, spec_min_rows;
+  double narrow_load;                 // 32-bit keys: 8-byte buckets while keys per table <= narrow_load x slots
   int hot;                            // skewed inputs: heavy hitters are reduced inside the warp (hashagg.cu)
   double hot_min_share;               // a key is hot from this share of the sample
   int slice;                          // EIGER_AUTO sizes PARTITION from a hash-space slice sketch instead of the full profile
@@ -112,6 +113,7 @@ struct Tunables {
     skew_collision = env("EIGER_SKEW_COLLISION", 1e-3);
     spec_samples = (int64_t)env("EIGER_SPEC_SAMPLES", 1 << 16);
     spec_min_rows = (int64_t)env("EIGER_SPEC_MIN_ROWS", 1 << 22);
+    narrow_load = env("EIGER_NARROW_LOAD", 0.06);
     hot = (int)env("EIGER_HOT", 1);
     hot_min_share = env("EIGER_HOT_MIN_SHARE", 0.02);
     slice = (int)env("EIGER_SLICE", 1);
@@ -417,6 +419,10 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       for (int j = 0; j < na; ++j) H.out_aggs[j] = out_aggs[j];
       H.n_out_aggs = na; H.out_capacity = out_capacity;
       H.threads = q.threads; H.smem_bytes = q.smem_bytes;
+      {   // 32-bit keys in a nearly empty shared-memory table: 8-byte buckets (hashagg.cu: BK)
+        const double per_table = q.variant == EIGER_PARTITION ? q.ndv / (double)((size_t)1 << (q.bits1 + q.bits2)) : q.ndv;
+        H.bucket_keys = (src_kind == KK_I32 && q.variant != EIGER_GLOBAL && per_table <= tun().narrow_load * q.slots) ? 2 : 0;
+      }
       if (q.variant == EIGER_PARTITION) {
         PartitionLaunch P{};
         P.key = q.key; P.plan = q.plan; P.n = n; P.key_kind = src_kind; P.bits1 = q.bits1; P.bits2 = q.bits2;

@@ -111,6 +111,7 @@ struct HashAggLaunch {
   int n_parts;
   uint32_t slots, limit;    // shared-memory table of each CTA
   int max_probes;           // 0 = default (16 buckets); 1 = home bucket only (hot-key cache in front of the global table)
+  int bucket_keys;          // 0 = 16-byte buckets; 2 = 8-byte buckets of 32-bit keys (nearly empty tables)
   int spec;                 // speculative run (EIGER_AUTO without statistics)
   uint64_t hot[kMaxHot]; int n_hot;   // whole-input mode: rebased heavy-hitter keys reduced inside the warp
   void* table; uint64_t cap; uint32_t stride;   // global table (BACK_HASH layout)
