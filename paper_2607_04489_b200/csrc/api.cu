@@ -419,7 +419,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       for (int j = 0; j < na; ++j) H.out_aggs[j] = out_aggs[j];
       H.n_out_aggs = na; H.out_capacity = out_capacity;
       H.threads = q.threads; H.smem_bytes = q.smem_bytes;
-      {   // 32-bit keys in a nearly empty shared-memory table: 8-byte buckets (hashagg.cu: BK)
+      {   // 32-bit keys in a nearly empty shared-memory table: 8-byte buckets (hashagg.cuh: BK)
         const double per_table = q.variant == EIGER_PARTITION ? q.ndv / (double)((size_t)1 << (q.bits1 + q.bits2)) : q.ndv;
         H.bucket_keys = (src_kind == KK_I32 && q.variant != EIGER_GLOBAL && per_table <= tun().narrow_load * q.slots) ? 2 : 0;
       }
