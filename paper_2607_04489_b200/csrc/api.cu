@@ -113,7 +113,7 @@ struct Tunables {
     skew_collision = env("EIGER_SKEW_COLLISION", 1e-3);
     spec_samples = (int64_t)env("EIGER_SPEC_SAMPLES", 1 << 16);
     spec_min_rows = (int64_t)env("EIGER_SPEC_MIN_ROWS", 1 << 22);
-    narrow_load = env("EIGER_NARROW_LOAD", 0.06);
+    narrow_load = env("EIGER_NARROW_LOAD", 0.10);
     hot = (int)env("EIGER_HOT", 1);
     hot_min_share = env("EIGER_HOT_MIN_SHARE", 0.02);
     slice = (int)env("EIGER_SLICE", 1);

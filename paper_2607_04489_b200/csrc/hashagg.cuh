@@ -55,8 +55,8 @@ template <int KK> struct IsPre { static constexpr bool v = (KK == KK_U32PRE || K
 __device__ __forceinline__ uint32_t plane_width(int op) { return op == EIGER_COUNT ? 4u : 8u; }
 
 // BK = keys per bucket: 16 bytes' worth by default; 2 for 32-bit keys in nearly empty tables
-// (measured, 2^28 rows: an LDS.64 look-up beats the LDS.128 one by 7-17 % at loads below ~0.05 and
-// loses 5-50 % above ~0.15, where the narrower bucket overflows into probe chains)
+// (measured, 2^28 rows: an LDS.64 look-up beats the LDS.128 one by 5-17 % at loads up to 0.08 and
+// loses 5-50 % from 0.16, where the narrower bucket overflows into probe chains)
 template <int KK, int SIG, int BK>
 struct Front {
   using U = typename KeyTraits<KK>::U;
