@@ -101,7 +101,7 @@ struct Tunables {
     smem_threads = (int)env("EIGER_SMEM_THREADS", 1024);
     part_table_bytes = (size_t)env("EIGER_PART_KB", 200) << 10;
     part_threads = (int)env("EIGER_PART_THREADS", 1024);
-    part_min_bits = (int)env("EIGER_PART_MIN_BITS", 9);
+    part_min_bits = (int)env("EIGER_PART_MIN_BITS", 7);
     direct_l2_bytes = (size_t)env("EIGER_DIRECT_L2_MB", 48) << 20;
     global_l2_bytes = (size_t)env("EIGER_GLOBAL_L2_MB", 192) << 20;
     global_front = (int)env("EIGER_GLOBAL_FRONT", 1);

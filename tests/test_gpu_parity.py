@@ -263,7 +263,7 @@ def test_auto_routes_hot_keys_to_the_global_table():
 
 
 def test_partition_cuts_hot_partitions_into_items():
-    # 2^24 rows over 2^9 partitions: the hot keys' partitions exceed twice the average and are cut
+    # 2^24 rows over 2^7 partitions: the hot keys' partitions exceed twice the average and are cut
     # into several work items that merge through the global table
     ds = datagen.config3(n=1 << 24, D=300_000)
     want = oracle_result(ds)
