@@ -558,7 +558,18 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     // the exact min/max, and the sketch of a hash-space slice of the keys (profile.cu).
     QueryPlan qp;
     if (plan_query(rt, keys, nk, n, vals, nv, aggs, na, local, EIGER_AUTO, &qp, skewed) == EIGER_OK && qp.variant == EIGER_PARTITION) {
-      const double ds = std::max(1.0, local[0].ndv_est);
+      // Lower bound of the column's NDV from the sample: the sample's own NDV ds, or - when the
+      // sample is far from having seen every key - half of what ds distinct keys among s samples
+      // mean for UNIFORM keys, ds / s = (1 - exp(-x)) / x with x = s / D (any other distribution
+      // with the same D shows fewer distinct keys, so the inversion can only fall short of D).
+      const double smp = (double)std::min<int64_t>(n, T.spec_samples);
+      double ds = std::max(1.0, local[0].ndv_est);
+      {
+        const double r = std::min(ds / smp, 0.999);
+        double lo = 0.05, hi = 50.0;                       // x = s / D; D capped at 20 s (sketch noise as r -> 1)
+        for (int it = 0; it < 60; ++it) { const double x = 0.5 * (lo + hi); if ((1.0 - std::exp(-x)) / x > r) lo = x; else hi = x; }
+        ds = std::max(ds, 0.5 * smp / (0.5 * (lo + hi)));
+      }
       uint32_t sel = kPreFan;
       while (sel > 1 && ds * (double)(sel / 2) / (double)kPreFan >= T.slice_min_keys) sel /= 2;
       const uint64_t base = (uint64_t)local[0].min;
