@@ -68,7 +68,8 @@ inline int dtype_size(int d) { return d == EIGER_I8 ? 1 : d == EIGER_I32 ? 4 : 8
 // Tunables of step A4; EIGER_* environment variables override them
 // for the crossover sweeps.  Re-read on every call so that a sweep can change them in-process.
 struct Tunables {
-  size_t priv_smem = 96 * 1024;       // FRONT_PRIV: private cells of one CTA
+  size_t priv_smem;                   // FRONT_PRIV: private cells of one CTA
+  int priv_max_range;                 // ... and only for this many keys (measured: 4 keys 0.46 vs 0.59 ms for the shared array, 8 keys 0.55 vs 0.48, 16 keys 0.52 vs 0.46; C2's 6 x 5 cells 2.89 vs 2.94)
   size_t sdirect_bytes = 160 * 1024;  // FRONT_SDIRECT: largest per-CTA direct array
   size_t sdirect_replica_budget;
   int sdirect_max_replicas, sdirect_wide;
@@ -94,6 +95,8 @@ struct Tunables {
   double slice_min_keys;              // distinct keys wanted in the slice (relative error 1 / sqrt of it)
   Tunables() {
     auto env = [](const char* k, double dflt) { const char* v = std::getenv(k); return v ? std::atof(v) : dflt; };
+    priv_smem = (size_t)env("EIGER_PRIV_KB", 96) << 10;
+    priv_max_range = (int)env("EIGER_PRIV_MAX_RANGE", 6);
     smem_table_bytes = (size_t)env("EIGER_SMEM_KB", 200) << 10;
     sdirect_replica_budget = (size_t)env("EIGER_SDIRECT_REPLICA_KB", 64) << 10;
     sdirect_max_replicas = (int)env("EIGER_SDIRECT_MAX_REPLICAS", 8);
@@ -263,7 +266,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
                   : (nk == 2 && keys[0].dtype == EIGER_I8 && keys[1].dtype == EIGER_I8) ? KK_I8I8 : KK_GEN;
     q->cap = R; q->stride = 8u * p.n_acc;
     q->table_bytes = align_up((size_t)R * q->stride, 256);
-    if (direct_bytes * 256 <= T.priv_smem) {
+    if (direct_bytes * 256 <= T.priv_smem && R <= (uint64_t)T.priv_max_range) {
       q->front = FRONT_PRIV; q->front_slots = (uint32_t)R; q->smem_bytes = (size_t)direct_bytes * 256;
     } else if (direct_bytes <= T.sdirect_bytes) {
       q->front = FRONT_SDIRECT; q->front_slots = (uint32_t)R;
