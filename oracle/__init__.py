@@ -44,10 +44,10 @@ def _load():
         L = ctypes.CDLL(_LIB)
         L.oracle_groupby_run.restype = ctypes.c_void_p
         L.oracle_groupby_run.argtypes = [
-            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
+            ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64,
             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32,
             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32,
-            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64]
+            ctypes.c_void_p, ctypes.c_int64]
         L.oracle_groupby_n_groups.restype = ctypes.c_int64
         L.oracle_groupby_n_groups.argtypes = [ctypes.c_void_p]
         L.oracle_groupby_status.restype = ctypes.c_int32
@@ -55,11 +55,11 @@ def _load():
         L.oracle_groupby_seconds.restype = ctypes.c_double
         L.oracle_groupby_seconds.argtypes = [ctypes.c_void_p]
         L.oracle_groupby_fetch.restype = None
-        L.oracle_groupby_fetch.argtypes = [ctypes.c_void_p] * 4
+        L.oracle_groupby_fetch.argtypes = [ctypes.c_void_p] * 3
         L.oracle_groupby_free.restype = None
         L.oracle_groupby_free.argtypes = [ctypes.c_void_p]
         L.oracle_exact_ndv.restype = ctypes.c_int64
-        L.oracle_exact_ndv.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64]
+        L.oracle_exact_ndv.argtypes = [ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64]
         L.oracle_minmax.restype = None
         L.oracle_minmax.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
         L.oracle_hash64.restype = ctypes.c_uint64
@@ -83,6 +83,15 @@ def _ptr(a: np.ndarray | None):
     return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
 
 
+MAX_KEY_COLS = 4
+
+
+def _ptrs(arrs):
+    """array of pointers to the given numpy arrays, as a void*"""
+    a = (ctypes.c_void_p * max(1, len(arrs)))(*[x.ctypes.data for x in arrs])
+    return ctypes.cast(a, ctypes.c_void_p)
+
+
 @dataclass
 class GroupByResult:
     keys: list            # one int64 array per key column, sorted ascending
@@ -92,13 +101,13 @@ class GroupByResult:
 
 
 def groupby(keys, vals, aggs, exact_f64_sum: bool = False, only=None) -> GroupByResult:
-    """keys: one array or a list of 1-2 integer arrays; vals: list of int64/float64
+    """keys: one array or a list of 1-4 integer arrays; vals: list of int64/float64
     arrays; aggs: list of (op, val_col).  Result sorted by key."""
     L = _load()
     if isinstance(keys, np.ndarray):
         keys = [keys]
-    if not 1 <= len(keys) <= 2:
-        raise ValueError("1 or 2 key columns")
+    if not 1 <= len(keys) <= MAX_KEY_COLS:
+        raise ValueError("1 to 4 key columns")
     k = [_i64(x) for x in keys]
     n = int(k[0].shape[0])
     v, isf = [], []
@@ -121,11 +130,12 @@ def groupby(keys, vals, aggs, exact_f64_sum: bool = False, only=None) -> GroupBy
         if isinstance(only, np.ndarray):
             only = [only]
         o = [_i64(x) for x in only]
-    h = L.oracle_groupby_run(_ptr(k[0]), _ptr(k[1]) if len(k) == 2 else None, n,
+        if len(o) != len(k):
+            raise ValueError("`only` needs one array per key column")
+    h = L.oracle_groupby_run(_ptrs(k), len(k), n,
                              ctypes.cast(vp, ctypes.c_void_p), _ptr(isf_a), len(v),
                              _ptr(ops), _ptr(cols), len(aggs), 1 if exact_f64_sum else 0,
-                             _ptr(o[0]) if o else None,
-                             _ptr(o[1]) if o and len(o) == 2 else None,
+                             _ptrs(o) if o else None,
                              int(o[0].shape[0]) if o else 0)
     try:
         st = L.oracle_groupby_status(h)
@@ -135,8 +145,7 @@ def groupby(keys, vals, aggs, exact_f64_sum: bool = False, only=None) -> GroupBy
         ok = [np.empty(g, dtype=np.int64) for _ in k]
         oa = [np.empty(g, dtype=np.int64) for _ in aggs]
         ap = (ctypes.c_void_p * max(1, len(oa)))(*[x.ctypes.data for x in oa])
-        L.oracle_groupby_fetch(h, _ptr(ok[0]), _ptr(ok[1]) if len(k) == 2 else None,
-                               ctypes.cast(ap, ctypes.c_void_p))
+        L.oracle_groupby_fetch(h, _ptrs(ok), ctypes.cast(ap, ctypes.c_void_p))
         secs = L.oracle_groupby_seconds(h)
     finally:
         L.oracle_groupby_free(h)
@@ -151,7 +160,7 @@ def exact_ndv(keys) -> int:
     if isinstance(keys, np.ndarray):
         keys = [keys]
     k = [_i64(x) for x in keys]
-    return int(L.oracle_exact_ndv(_ptr(k[0]), _ptr(k[1]) if len(k) == 2 else None, k[0].shape[0]))
+    return int(L.oracle_exact_ndv(_ptrs(k), len(k), k[0].shape[0]))
 
 
 def minmax(keys) -> tuple[int, int]:

@@ -52,23 +52,39 @@ struct Acc {
   double fmax = -std::numeric_limits<double>::infinity();
 };
 
+// A group key is the tuple of its key columns (§4.3 "group-bys with multiple
+// keys"): up to kMaxKeyCols columns, unused ones held at 0.  Equality and order are the
+// tuple's (lexicographic, first column most significant).
+constexpr int kMaxKeyCols = 4;
 struct Key {
-  int64_t a, b;
-  bool operator==(const Key& o) const { return a == o.a && b == o.b; }
-  bool operator<(const Key& o) const { return a != o.a ? a < o.a : b < o.b; }
+  int64_t v[kMaxKeyCols];
+  bool operator==(const Key& o) const {
+    for (int c = 0; c < kMaxKeyCols; ++c) if (v[c] != o.v[c]) return false;
+    return true;
+  }
+  bool operator<(const Key& o) const {
+    for (int c = 0; c < kMaxKeyCols; ++c) if (v[c] != o.v[c]) return v[c] < o.v[c];
+    return false;
+  }
 };
 struct KeyHash {
   size_t operator()(const Key& k) const {
     // any hash works: the result of a group-by does not depend on it
-    uint64_t x = (uint64_t)k.a * 0x9FB21C651E98DF25ull ^ ((uint64_t)k.b + 0x632BE59BD9B4E019ull);
-    x ^= x >> 29;
+    uint64_t x = 0x632BE59BD9B4E019ull;
+    for (int c = 0; c < kMaxKeyCols; ++c) { x = (x ^ (uint64_t)k.v[c]) * 0x9FB21C651E98DF25ull; x ^= x >> 29; }
     return (size_t)(x * 0xD6E8FEB86659FD93ull);
   }
 };
+inline Key key_at(const int64_t* const* cols, int32_t nk, int64_t i) {
+  Key k;
+  for (int c = 0; c < kMaxKeyCols; ++c) k.v[c] = c < nk ? cols[c][i] : 0;
+  return k;
+}
 
 struct Result {
   int32_t n_aggs = 0;
-  std::vector<Key> keys;                       // sorted ascending (a, then b)
+  int32_t n_key_cols = 0;
+  std::vector<Key> keys;                       // sorted ascending (column 0 first)
   std::vector<std::vector<uint64_t>> aggs;     // [agg][group], 8-byte bit patterns
   double seconds = 0.0;
   int32_t status = 0;
@@ -83,12 +99,12 @@ extern "C" {
 // ---------------------------------------------------------------------------
 // GROUP BY, the plain relational definition (§3.3 "Group-by";
 // PAPER.md:302 "number of groups g", "number of aggregations").  For rows
-// i = 0..n-1 with key k_i = (key0[i], key1[i]) the output is the set of distinct
+// i = 0..n-1 with key k_i = (keys[0][i], .., keys[n_key_cols-1][i]) the output is the set of distinct
 // keys; per key SUM = sum of the value column over the rows of that key,
 // COUNT = number of those rows, MIN / MAX = min / max over them.
 //
-//   key0, key1 : int64 arrays (key1 may be NULL for a single key column; the
-//                Python wrapper widens int8/int32 keys, which is exact)
+//   keys       : n_key_cols (1..4) pointers to int64 arrays (the Python wrapper
+//                widens int8/int32 keys, which is exact)
 //   vals       : n_vals pointers to 8-byte columns; val_is_f64[c] says how to
 //                read column c (int64 or IEEE double)
 //   ops/cols   : n_aggs aggregates; COUNT ignores its column
@@ -97,19 +113,21 @@ extern "C" {
 //                generator's fp64 values, reading R14); the sum is carried in
 //                a 128-bit integer and rounded to double once.  A value that
 //                violates the precondition sets status = -2.
-//   only0/only1/n_only: optional restriction used for spot checks at sizes where
+//   only/n_only: (n_key_cols pointers, n_only keys) optional restriction used for spot checks at sizes where
 //                the full result does not fit the host: when n_only > 0, rows
 //                whose key is not one of the n_only listed keys are skipped, so
 //                the result is the plain definition for exactly those groups.
 // Returns an opaque handle (free with oracle_groupby_free).
 // ---------------------------------------------------------------------------
-void* oracle_groupby_run(const int64_t* key0, const int64_t* key1, int64_t n,
+void* oracle_groupby_run(const int64_t* const* keys, int32_t n_key_cols, int64_t n,
                          const void* const* vals, const int32_t* val_is_f64, int32_t n_vals,
                          const int32_t* ops, const int32_t* cols, int32_t n_aggs,
                          int32_t f64_sum_mode,
-                         const int64_t* only0, const int64_t* only1, int64_t n_only) {
+                         const int64_t* const* only_keys, int64_t n_only) {
   Result* res = new Result();
   res->n_aggs = n_aggs;
+  res->n_key_cols = n_key_cols;
+  if (n_key_cols < 1 || n_key_cols > kMaxKeyCols) { res->status = -1; return res; }
   for (int j = 0; j < n_aggs; ++j) {
     if (ops[j] < 0 || ops[j] > 3 || (ops[j] != OP_COUNT && (cols[j] < 0 || cols[j] >= n_vals))) {
       res->status = -1;
@@ -118,10 +136,10 @@ void* oracle_groupby_run(const int64_t* key0, const int64_t* key1, int64_t n,
   }
   std::unordered_map<Key, std::vector<Acc>, KeyHash> map;
   std::unordered_map<Key, char, KeyHash> only;
-  for (int64_t i = 0; i < n_only; ++i) only.emplace(Key{only0[i], only1 ? only1[i] : 0}, 1);
+  for (int64_t i = 0; i < n_only; ++i) only.emplace(key_at(only_keys, n_key_cols, i), 1);
   auto t0 = std::chrono::steady_clock::now();
   for (int64_t i = 0; i < n; ++i) {
-    Key k{key0[i], key1 ? key1[i] : 0};
+    const Key k = key_at(keys, n_key_cols, i);
     if (n_only > 0 && only.find(k) == only.end()) continue;
     auto it = map.find(k);
     if (it == map.end()) it = map.emplace(k, std::vector<Acc>((size_t)n_aggs)).first;
@@ -200,12 +218,13 @@ int64_t oracle_groupby_n_groups(const void* h) { return (int64_t)static_cast<con
 int32_t oracle_groupby_status(const void* h) { return static_cast<const Result*>(h)->status; }
 double oracle_groupby_seconds(const void* h) { return static_cast<const Result*>(h)->seconds; }
 
-// Copies the result out: key0/key1 (key1 may be NULL) of n_groups int64 each, aggs as
+// Copies the result out: keys = n_key_cols pointers to n_groups int64 each, aggs as
 // n_aggs pointers to n_groups 8-byte cells (int64 bits or double bits).
-void oracle_groupby_fetch(const void* h, int64_t* key0, int64_t* key1, void* const* aggs) {
+void oracle_groupby_fetch(const void* h, int64_t* const* keys, void* const* aggs) {
   const Result* r = static_cast<const Result*>(h);
   const size_t g = r->keys.size();
-  for (size_t i = 0; i < g; ++i) { key0[i] = r->keys[i].a; if (key1) key1[i] = r->keys[i].b; }
+  for (size_t i = 0; i < g; ++i)
+    for (int c = 0; c < r->n_key_cols; ++c) keys[c][i] = r->keys[i].v[c];
   for (int j = 0; j < r->n_aggs; ++j) std::memcpy(aggs[j], r->aggs[(size_t)j].data(), g * 8);
 }
 void oracle_groupby_free(void* h) { delete static_cast<Result*>(h); }
@@ -214,9 +233,10 @@ void oracle_groupby_free(void* h) { delete static_cast<Result*>(h); }
 // Exact NDV by an independent second method: sort + unique (BASELINE.json
 // north_star "an exact-NDV counter").  Must equal the group-by's n_groups.
 // ---------------------------------------------------------------------------
-int64_t oracle_exact_ndv(const int64_t* key0, const int64_t* key1, int64_t n) {
+int64_t oracle_exact_ndv(const int64_t* const* keys, int32_t n_key_cols, int64_t n) {
+  if (n_key_cols < 1 || n_key_cols > kMaxKeyCols) return -1;
   std::vector<Key> v((size_t)n);
-  for (int64_t i = 0; i < n; ++i) v[(size_t)i] = Key{key0[i], key1 ? key1[i] : 0};
+  for (int64_t i = 0; i < n; ++i) v[(size_t)i] = key_at(keys, n_key_cols, i);
   std::sort(v.begin(), v.end());
   return (int64_t)(std::unique(v.begin(), v.end()) - v.begin());
 }

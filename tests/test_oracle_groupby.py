@@ -206,3 +206,56 @@ def test_empty_and_extremes():
     r = oracle.groupby(k, [np.array([1, 2, 3, 4], dtype=np.int64)], [(SUM, 0), (COUNT, 0)])
     assert r.keys[0].tolist() == [-(1 << 63), 0, (1 << 63) - 1]
     assert r.aggs[0].tolist() == [4, 4, 2] and r.aggs[1].tolist() == [2, 1, 1]
+
+
+# ---- multi-key group-by (§4.3): 3 and 4 key columns ---------------------------
+
+@pytest.mark.parametrize("nk,seed", [(3, 0), (3, 1), (4, 2), (4, 3), (4, 4)])
+def test_brute_force_multi_key(nk, seed):
+    rng = np.random.default_rng(700 + seed)
+    n = int(rng.integers(1, 81))
+    dts = [np.int8, np.int32, np.int64, np.int32]
+    spans = [(-2, 2), (1 << 20, (1 << 20) + 3), (-(1 << 40), -(1 << 40) + 2), (-1, 2)]
+    keys = [rng.integers(lo, hi, size=n).astype(dt) for (lo, hi), dt in list(zip(spans, dts))[:nk]]
+    v = rng.integers(-(1 << 62), 1 << 62, size=n).astype(np.int64)
+    got = as_dict(oracle.groupby(keys, [v], ALL4))
+    assert got == brute_force(keys, [v], ALL4)
+    assert oracle.exact_ndv(keys) == len(got)
+
+
+def test_multi_key_closed_form_crt():
+    """keys (i mod 3, i mod 5, i mod 7, i mod 11), i < 2 * 1155: by the Chinese remainder
+    theorem every one of the 3*5*7*11 = 1155 residue tuples occurs exactly twice, as rows
+    i0 and i0 + 1155 (i0 = the tuple's CRT solution), so SUM(i) = 2 * i0 + 1155."""
+    M = [3, 5, 7, 11]
+    P = 1155
+    i = np.arange(2 * P, dtype=np.int64)
+    keys = [(i % m).astype(np.int32) for m in M]
+    res = oracle.groupby(keys, [i], [(COUNT, 0), (SUM, 0), (MIN, 0), (MAX, 0)])
+    assert res.n_groups == P and oracle.exact_ndv(keys) == P
+    # sorted lexicographically, first column most significant
+    tup = [tuple(int(k[g]) for k in res.keys) for g in range(P)]
+    assert tup == sorted(tup) and tup[0] == (0, 0, 0, 0) and tup[-1] == (2, 4, 6, 10)
+    for g in (0, 1, 17, 500, P - 1):
+        i0 = next(x for x in range(P) if all(x % m == r for m, r in zip(M, tup[g])))
+        assert [int(a[g]) for a in res.aggs] == [2, 2 * i0 + P, i0, i0 + P]
+
+
+def test_multi_key_column_order_matters_and_unused_columns_do_not():
+    rng = np.random.default_rng(9)
+    a = rng.integers(0, 4, size=500).astype(np.int64)
+    b = rng.integers(0, 4, size=500).astype(np.int64)
+    c = rng.integers(0, 4, size=500).astype(np.int64)
+    v = rng.integers(-100, 100, size=500).astype(np.int64)
+    r_abc = as_dict(oracle.groupby([a, b, c], [v], ALL4))
+    r_cab = as_dict(oracle.groupby([c, a, b], [v], ALL4))
+    assert {(k[1], k[2], k[0]): x for k, x in r_cab.items()} == r_abc
+    # a constant extra column changes nothing but the key tuple
+    z = np.full(500, 7, dtype=np.int64)
+    r_abcz = as_dict(oracle.groupby([a, b, c, z], [v], ALL4))
+    assert {k[:3]: x for k, x in r_abcz.items()} == r_abc and all(k[3] == 7 for k in r_abcz)
+    # the `only` restriction on tuples
+    some = sorted(r_abc)[::5]
+    only = [np.array([k[j] for k in some], dtype=np.int64) for j in range(3)]
+    r_only = as_dict(oracle.groupby([a, b, c], [v], ALL4, only=only))
+    assert r_only == {k: r_abc[k] for k in some}
