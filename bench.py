@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — the adaptive GROUP BY hot path on B200, one JSON line.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2|C3|C4|C5:<log2 ndv>:<dense|scattered>|C1]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2|C3|C4|C5:<log2 ndv>:<dense|scattered>|C1|MK:<key cols>:<bits per col>]
                     [--force auto|direct|smem|global|partition] [--impl reference] [--sweep]
 
 A step = one pass of the whole hot path (profile -> select -> init -> aggregate -> compact,
@@ -64,6 +64,12 @@ def build_workload(name: str, device, scale: int = 1, seed_offset: int = 0):
         n = (1 << 28) // scale
         return datagen.config5(device, n=n, seed=5 + seed_offset, ndv=min(1 << lg, n),
                                scattered=len(parts) > 2 and parts[2] == "scattered")
+    if base == "MK":
+        # MK[:<key columns>[:<bits per column>]]: multi-key group-by, 2^28 rows of nk int32 key columns
+        # (PAPER.md:215-221 smart key fusion; the 4xI32 tables of)
+        nk = int(parts[1]) if len(parts) > 1 else 4
+        bits = int(parts[2]) if len(parts) > 2 else 4
+        return datagen.config_mk(device, n=(1 << 28) // scale, seed=6 + seed_offset, nk=nk, digit_bits=bits)
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -133,7 +139,7 @@ def cpu_baseline(ds_cpu, budget_rows: int):
 def cpu_sample_rows(name: str) -> int:
     # about 10-30 s of single-thread oracle time (measured rates: ~8 ns/row at 6 groups ... ~250 ns at 10^8)
     base = name.split(":")[0].upper()
-    return {"C1": 1_000_000, "C2": 400_000_000, "C3": 100_000_000, "C4": 50_000_000, "C5": 1 << 27}.get(base, 1 << 26)
+    return {"C1": 1_000_000, "C2": 400_000_000, "C3": 100_000_000, "C4": 50_000_000, "C5": 1 << 27, "MK": 1 << 27}.get(base, 1 << 26)
 
 
 def run_reference(args):
@@ -142,7 +148,7 @@ def run_reference(args):
     if rank != 0:
         return
     import oracle
-    sample = {"C1": 1_000_000, "C2": 1 << 26, "C3": 1 << 24, "C4": 1 << 23, "C5": 1 << 25}[args.workload.split(":")[0].upper()]
+    sample = {"C1": 1_000_000, "C2": 1 << 26, "C3": 1 << 24, "C4": 1 << 23, "C5": 1 << 25, "MK": 1 << 25}[args.workload.split(":")[0].upper()]
     ds = build_workload(args.workload, "cpu", scale=max(args.scale, 1))
     m = min(ds.n, sample)
     keys = [k[:m].numpy() for k in ds.keys]

@@ -131,7 +131,7 @@ def zipf_thresholds(s: float, N: int) -> np.ndarray:
 class Dataset:
     name: str
     n: int
-    keys: list                 # 1 or 2 tensors (int8 / int32 / int64)
+    keys: list                 # 1 to 4 tensors (int8 / int32 / int64)
     vals: list                 # int64 or float64 tensors
     aggs: list                 # [(op, val_col)], op codes: 0 SUM, 1 COUNT, 2 MIN, 3 MAX
     ndv: int | None = None     # exact NDV by construction, when known
@@ -232,3 +232,27 @@ def config5(device="cpu", n: int = 1 << 28, seed: int = 5, ndv: int = 1 << 16,
     vals = _fill(n, torch.int64, device, lambda i: uniform_int(seed, 1, i, 0, (1 << 31) - 2))
     return Dataset("C5", n, [keys], [vals], [(SUM, 0), (COUNT, 0)], ndv=min(ndv, n),
                    meta={"seed": seed, "ndv": ndv, "scattered": scattered})
+
+
+MK_OFFSETS = (-7, 1000, 1 << 20, -(1 << 30))
+
+
+def config_mk(device="cpu", n: int = 1 << 28, seed: int = 6, nk: int = 4, digit_bits: int = 4,
+              dtypes=None) -> Dataset:
+    """Multi-key group-by shaped like the paper's 4xI32 key tables (PAPER.md:409-419, Table 4;
+    §4.3): ``nk`` key columns, column c = digit c (``digit_bits`` bits) of an id
+    with exactly min(n, 2^(nk * digit_bits)) distinct values, plus a per-column offset so that
+    every column needs its own frame of reference; int64 values in [0, 2^31); SUM, COUNT."""
+    D = 1 << (nk * digit_bits)
+    dtypes = list(dtypes) if dtypes is not None else [torch.int32] * nk
+    assert len(dtypes) == nk and 1 <= nk <= 4
+    mask = (1 << digit_bits) - 1
+    keys = []
+    for c in range(nk):
+        off = MK_OFFSETS[c] if dtypes[c] != torch.int8 else -3
+        assert dtypes[c] != torch.int8 or mask + off <= 127
+        keys.append(_fill(n, dtypes[c], device,
+                          lambda i, c=c, off=off: ((known_ndv_ids(seed, 0, i, n, D) >> (c * digit_bits)) & mask) + off))
+    vals = _fill(n, torch.int64, device, lambda i: uniform_int(seed, 1, i, 0, (1 << 31) - 2))
+    return Dataset("MK", n, keys, [vals], [(SUM, 0), (COUNT, 0)], ndv=min(D, n),
+                   meta={"seed": seed, "nk": nk, "digit_bits": digit_bits})

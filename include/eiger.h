@@ -73,7 +73,7 @@ int eiger_profile(const void* keys, int32_t dtype, int64_t n, eiger_stats* out, 
 /* eiger_profile_keys — the statistics pass exactly as EIGER_AUTO runs it inside eiger_groupby
  * when no statistics are supplied: one read-back for all key columns; min/max of each; the
  * sketch only where the range test cannot decide ("range first"): 1-byte keys and
- * two-column keys get ndv_est = min(n, max - min + 1) without a sketch.
+ * multi-column keys get ndv_est = min(n, max - min + 1) per column without a sketch.
  *   keys[n_key_cols] DEVICE columns; out[n_key_cols] HOST. */
 int eiger_profile_keys(const eiger_col* keys, int32_t n_key_cols, int64_t n, eiger_stats* out, void* stream);
 
@@ -87,9 +87,13 @@ double eiger_hll_estimate_host(const uint8_t* regs);
 
 /* eiger_groupby — GROUP BY keys, aggregating value columns (steps A0, A4-A7;
  * PAPER.md:79 §3.3, §4.1, PAPER.md:184 retrieveAll).
- *   keys[n_key_cols]   1 or 2 integer key columns (EIGER_I8 / I32 / I64).  Two columns are
- *                      fused into one key by frame-of-reference + positional packing
- *                      (§4.3) and un-fused on output.
+ *   keys[n_key_cols]   1 to 4 integer key columns (EIGER_I8 / I32 / I64, any mix).  Several
+ *                      columns are fused on the fly into one 64-bit key by frame of reference +
+ *                      positional packing (smart key fusion without the dictionary step,
+ *                      PAPER.md:215-221 §4.3): u = (..((k0 - min0) * r1 + (k1 - min1)) * r2 + ..),
+ *                      r_c = max_c - min_c + 1, and un-fused on output.  The product of the
+ *                      column ranges must fit 64 bits, else EIGER_ERR_INFEASIBLE (the paper
+ *                      dictionary-encodes such keys first; not built).
  *   vals[n_vals]       value columns, EIGER_I64 or EIGER_F64, n_vals <= 8
  *   aggs[n_aggs]       n_aggs <= 8; result type: SUM/MIN/MAX of I64 -> int64 (SUM wraps modulo
  *                      2^64), of F64 -> double; COUNT -> int64 row count

@@ -171,6 +171,7 @@ def _stats_arr(stats):
     return arr
 
 
+MAX_KEY_COLS = 4
 _KEY_T = (torch.int8, torch.int32, torch.int64)
 _VAL_T = (torch.int64, torch.float64)
 
@@ -255,12 +256,14 @@ def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int |
             workspace: Workspace | None = None) -> GroupByResult:
     """eiger_groupby on device columns.
 
-    keys: 1-2 CUDA integer tensors; vals: CUDA int64/float64 tensors; aggs: [(op, val_col)].
+    keys: 1-4 CUDA integer tensors; vals: CUDA int64/float64 tensors; aggs: [(op, val_col)].
     With stats=None the key columns are profiled first (eiger_profile), which is what the
     adaptive path's time includes; pass stats from profile() to skip that.
     """
     if isinstance(keys, torch.Tensor):
         keys = [keys]
+    if not 1 <= len(keys) <= MAX_KEY_COLS:
+        raise EigerError(ERR_ARG, f"1 to {MAX_KEY_COLS} key columns")
     dev = keys[0].device
     if not all(t.is_cuda for t in list(keys) + list(vals)):
         raise ValueError("all columns must be CUDA tensors")
@@ -285,7 +288,7 @@ def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int |
             have = min([t.numel() for t in ws.out.values()], default=0)
             cap = out_capacity if out_capacity is not None else max(have, 1 << 20)
             ok, oa = out_cols(cap)
-            okp = (ctypes.c_void_p * 2)(*[t.data_ptr() for t in ok])
+            okp = (ctypes.c_void_p * 4)(*[t.data_ptr() for t in ok])
             oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
             ng, chosen = ctypes.c_int64(0), ctypes.c_int32(0)
             stats_known = None
@@ -311,7 +314,7 @@ def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int |
                 else:
                     break
                 ok, oa = out_cols(cap)
-                okp = (ctypes.c_void_p * 2)(*[t.data_ptr() for t in ok])
+                okp = (ctypes.c_void_p * 4)(*[t.data_ptr() for t in ok])
                 oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
             if rc not in (ERR_WORKSPACE, ERR_TABLE_OVERFLOW) and not (rc == ERR_OUT_CAPACITY and out_capacity is None):
                 _check(rc)
@@ -337,7 +340,7 @@ def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int |
             ok = [ws.column(("k", i), cap, k.dtype) for i, k in enumerate(keys)]
             oa = [ws.column(("a", j), cap, torch.float64 if (op != COUNT and vals[c].dtype == torch.float64) else torch.int64)
                   for j, (op, c) in enumerate(aggs)]
-            okp = (ctypes.c_void_p * 2)(*[t.data_ptr() for t in ok])
+            okp = (ctypes.c_void_p * 4)(*[t.data_ptr() for t in ok])
             oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
             ng, chosen = ctypes.c_int64(0), ctypes.c_int32(0)
             rc = L.eiger_groupby(kc, len(keys), n, vc, len(vals), ac, len(aggs), sc, okp, oap, cap,
@@ -364,6 +367,8 @@ def groupby_host(keys, vals, aggs, force: int = AUTO, out_capacity: int | None =
         keys = [keys]
     if any(t.is_cuda for t in list(keys) + list(vals)):
         raise ValueError("groupby_host takes host tensors")
+    if not 1 <= len(keys) <= MAX_KEY_COLS:
+        raise EigerError(ERR_ARG, f"1 to {MAX_KEY_COLS} key columns")
     n = keys[0].numel()
     L = lib()
     cap = n if out_capacity is None else out_capacity
@@ -373,7 +378,7 @@ def groupby_host(keys, vals, aggs, force: int = AUTO, out_capacity: int | None =
               for (op, c) in aggs]
     else:
         ok, oa = out
-    okp = (ctypes.c_void_p * 2)(*[t.data_ptr() for t in ok])
+    okp = (ctypes.c_void_p * 4)(*[t.data_ptr() for t in ok])
     oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
     ng, chosen, h2d, d2h = ctypes.c_int64(0), ctypes.c_int32(0), ctypes.c_int64(0), ctypes.c_int64(0)
     rc = L.eiger_groupby_host(_cols(keys, _KEY_T), len(keys), n, _cols(vals, _VAL_T), len(vals), _aggs(aggs), len(aggs),

@@ -245,7 +245,7 @@ struct CompactArgs {
   AggPlan plan;
   const unsigned char* table;
   uint64_t cap; uint32_t stride; int back;
-  void* out_keys[2]; uint64_t* out_aggs[kMaxAggs]; int n_out;
+  void* out_keys[kMaxKeyCols]; uint64_t* out_aggs[kMaxAggs]; int n_out;
   int64_t out_capacity;
   CallDev* call;
 };
@@ -282,8 +282,8 @@ __global__ void __launch_bounds__(256) compact_kernel(const __grid_constant__ Co
     const uint64_t g = start + __popc(m & ((1u << lane) - 1u));
     if ((int64_t)g >= c.out_capacity) continue;
     // un-fuse and un-rebase (PAPER.md:219-221 in reverse)
-    uint64_t part[2];
-    if (c.key.ncols == 2) { part[0] = u / c.key.mul; part[1] = u % c.key.mul; } else { part[0] = u; part[1] = 0; }
+    uint64_t part[kMaxKeyCols];
+    unfuse_key(c.key, u, part);
     for (int k = 0; k < c.key.ncols; ++k) {
       const uint64_t v = part[k] + c.key.base[k];
       switch (c.key.dtype[k]) {
@@ -376,7 +376,7 @@ int launch_compact(const CompactLaunch& c, int sm_count, cudaStream_t s) {
   CompactArgs a;
   a.key = c.key; a.plan = c.plan; a.table = static_cast<const unsigned char*>(c.table);
   a.cap = c.cap; a.stride = c.stride; a.back = c.back;
-  a.out_keys[0] = c.out_keys[0]; a.out_keys[1] = c.out_keys[1];
+  for (int k = 0; k < kMaxKeyCols; ++k) a.out_keys[k] = c.out_keys[k];
   for (int j = 0; j < kMaxAggs; ++j) a.out_aggs[j] = static_cast<uint64_t*>(c.out_aggs[j]);
   a.n_out = c.n_out_aggs; a.out_capacity = c.out_capacity; a.call = c.call;
   const uint64_t n_slots = c.cap + 1;

@@ -166,7 +166,7 @@ int detect_sig(const AggPlan& p, int n_user) {
 // Step A4: choose the variant and size everything (readings R8-R10).
 int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eiger_col* vals, int nv,
                const eiger_agg* aggs, int na, const eiger_stats* st, int force, QueryPlan* q, bool skewed = false) {
-  if (!keys || nk < 1 || nk > 2 || n < 0 || nv < 0 || nv > kMaxVals || na < 1 || na > kMaxAggs || !aggs) return EIGER_ERR_ARG;
+  if (!keys || nk < 1 || nk > kMaxKeyCols || n < 0 || nv < 0 || nv > kMaxVals || na < 1 || na > kMaxAggs || !aggs) return EIGER_ERR_ARG;
   if (nv > 0 && !vals) return EIGER_ERR_ARG;
   if (force < EIGER_AUTO || force > EIGER_PARTITION) return EIGER_ERR_ARG;
   for (int k = 0; k < nk; ++k) if (!is_key_dtype(keys[k].dtype)) return EIGER_ERR_ARG;
@@ -198,7 +198,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   std::memset(&kd, 0, sizeof(kd));
   kd.ncols = nk; kd.mul = 1;
   bool have_stats = st != nullptr;
-  uint64_t Rk[2] = {0, 0};
+  uint64_t Rk[kMaxKeyCols] = {0, 0, 0, 0};
   for (int k = 0; k < nk; ++k) {
     kd.ptr[k] = keys[k].data; kd.dtype[k] = keys[k].dtype;
     if (have_stats) { kd.base[k] = (uint64_t)st[k].min; Rk[k] = n > 0 ? range_of(st[k]) : 1; }
@@ -209,10 +209,14 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
     }
   }
   uint64_t R = Rk[0];
-  if (nk == 2) {
-    if (Rk[0] == 0 || Rk[1] == 0) return EIGER_ERR_INFEASIBLE;
-    const unsigned __int128 prod = (unsigned __int128)Rk[0] * Rk[1];
-    if (prod >> 64) return EIGER_ERR_INFEASIBLE;   // fused key must fit 64 bits
+  if (nk >= 2) {
+    unsigned __int128 prod = 1;
+    for (int k = 0; k < nk; ++k) {
+      if (Rk[k] == 0) return EIGER_ERR_INFEASIBLE;
+      prod *= Rk[k];
+      if (prod >> 64) return EIGER_ERR_INFEASIBLE;   // fused key must fit 64 bits
+      kd.rng[k] = Rk[k];
+    }
     R = (uint64_t)prod; kd.mul = Rk[1];
   }
   q->R = R;
@@ -222,7 +226,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   double ndv = bound;
   if (have_stats) {
     double e = st[0].ndv_est;
-    if (nk == 2) e *= st[1].ndv_est;
+    for (int k = 1; k < nk; ++k) e *= st[k].ndv_est;
     ndv = std::min(bound, std::max(e, 1.0));
   }
   q->ndv = ndv;
@@ -333,7 +337,7 @@ int do_profile(Runtime* rt, const eiger_col* cols, int nk, int64_t n, int with_h
     }
     if (with_hll) { int rc = launch_hll_hist(rt, s); if (rc) return rc; }
   }
-  struct Back { long long mn[2], mx[2]; uint32_t hist[64]; uint32_t pair_eq, pair_n; };
+  struct Back { long long mn[kMaxKeyCols], mx[kMaxKeyCols]; uint32_t hist[64]; uint32_t pair_eq, pair_n; };
   Back* b = static_cast<Back*>(rt->pinned);
   EIGER_CUDA(cudaMemcpyAsync(b, rt->prof, sizeof(Back), cudaMemcpyDeviceToHost, s));
   EIGER_CUDA(cudaStreamSynchronize(s));
@@ -357,7 +361,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
                 cudaStream_t s) {
   if (!n_groups || !out_keys || !out_aggs || out_capacity < 0) return EIGER_ERR_ARG;
   *n_groups = 0;
-  if (!keys || nk < 1 || nk > 2 || n < 0) return EIGER_ERR_ARG;
+  if (!keys || nk < 1 || nk > kMaxKeyCols || n < 0) return EIGER_ERR_ARG;
   for (int k = 0; k < nk; ++k) {
     if (!is_key_dtype(keys[k].dtype)) return EIGER_ERR_ARG;
     if (n > 0 && (!keys[k].data || ((uintptr_t)keys[k].data & 15))) return EIGER_ERR_ARG;
@@ -418,7 +422,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       for (int i = 0; i < H.n_hot; ++i) H.hot[i] = (uint64_t)hot_key[i] - q.key.base[0];
       if (H.n_hot && src_kind == KK_I32) for (int i = 0; i < H.n_hot; ++i) H.hot[i] &= 0xFFFFFFFFull;
       H.table = table; H.cap = q.cap; H.stride = q.stride; H.call = rt->call;
-      H.out_keys[0] = out_keys[0]; H.out_keys[1] = nk == 2 ? out_keys[1] : nullptr;
+      for (int k = 0; k < kMaxKeyCols; ++k) H.out_keys[k] = k < nk ? out_keys[k] : nullptr;
       for (int j = 0; j < na; ++j) H.out_aggs[j] = out_aggs[j];
       H.n_out_aggs = na; H.out_capacity = out_capacity;
       H.threads = q.threads; H.smem_bytes = q.smem_bytes;
@@ -467,7 +471,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
 
     CompactLaunch C{};
     C.key = q.key; C.plan = q.plan; C.back = q.back; C.table = table; C.cap = q.cap; C.stride = q.stride;
-    C.out_keys[0] = out_keys[0]; C.out_keys[1] = nk == 2 ? out_keys[1] : nullptr;
+    for (int k = 0; k < kMaxKeyCols; ++k) C.out_keys[k] = k < nk ? out_keys[k] : nullptr;
     for (int j = 0; j < na; ++j) C.out_aggs[j] = out_aggs[j];
     C.n_out_aggs = na; C.out_capacity = out_capacity; C.call = rt->call;
     { Timed t(s, 4); rc = launch_compact(C, rt->sm_count, s); if (rc) return rc; }
@@ -484,8 +488,9 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       q.table_bytes = align_up((size_t)(q.cap + 1) * q.stride, 256);
       if (q.variant == EIGER_PARTITION) {
         // more partitions as well: re-plan the fan-out for four times the estimate
-        eiger_stats grown[2] = {st[0], st[nk == 2 ? 1 : 0]};
-        grown[0].ndv_est = std::min((double)n, std::max(q.ndv, 1.0) * 4.0); if (nk == 2) grown[1].ndv_est = 1.0;
+        eiger_stats grown[kMaxKeyCols];
+        for (int k = 0; k < kMaxKeyCols; ++k) { grown[k] = st[k < nk ? k : 0]; grown[k].ndv_est = 1.0; }
+        grown[0].ndv_est = std::min((double)n, std::max(q.ndv, 1.0) * 4.0);
         QueryPlan q2;
         rc = plan_query(rt, keys, nk, n, vals, nv, aggs, na, grown, EIGER_PARTITION, &q2);
         if (rc) return rc;
@@ -504,7 +509,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
   }
   };
 
-  eiger_stats local[2];
+  eiger_stats local[kMaxKeyCols];
   const Tunables T = tun();
   bool skewed = false;
   if (!stats_in && force == EIGER_AUTO && n >= T.spec_min_rows) {
@@ -579,7 +584,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       { Timed t(s, 1);
         rc = launch_part_hist_hll(rt, keys[0].data, keys[0].dtype, n, base, sel, s); if (rc) return rc;
         rc = launch_hll_hist(rt, s); if (rc) return rc; }
-      struct PBack { long long mn[2], mx[2]; uint32_t hist[64]; uint32_t pair_eq, pair_n; };
+      struct PBack { long long mn[kMaxKeyCols], mx[kMaxKeyCols]; uint32_t hist[64]; uint32_t pair_eq, pair_n; };
       PBack* b = static_cast<PBack*>(rt->pinned);
       EIGER_CUDA(cudaMemcpyAsync(b, rt->prof, sizeof(PBack), cudaMemcpyDeviceToHost, s));
       EIGER_CUDA(cudaStreamSynchronize(s));
@@ -673,7 +678,7 @@ int eiger_profile(const void* keys, int32_t dtype, int64_t n, eiger_stats* out, 
 }
 
 int eiger_profile_keys(const eiger_col* keys, int32_t nk, int64_t n, eiger_stats* out, void* stream) {
-  if (!out || !keys || nk < 1 || nk > 2 || n < 0) return EIGER_ERR_ARG;
+  if (!out || !keys || nk < 1 || nk > kMaxKeyCols || n < 0) return EIGER_ERR_ARG;
   for (int k = 0; k < nk; ++k)
     if (!is_key_dtype(keys[k].dtype) || (n > 0 && (!keys[k].data || ((uintptr_t)keys[k].data & 15)))) return EIGER_ERR_ARG;
   std::lock_guard<std::mutex> lk(g_mu);
@@ -742,7 +747,7 @@ int eiger_groupby_host(const eiger_col* keys, int32_t nk, int64_t n, const eiger
                        const eiger_agg* aggs, int32_t na, void* const* out_keys, void* const* out_aggs,
                        int64_t out_capacity, int64_t* n_groups, int32_t force, int32_t* chosen,
                        int64_t* h2d_bytes, int64_t* d2h_bytes, void* stream) {
-  if (!keys || nk < 1 || nk > 2 || n < 0 || nv < 0 || nv > kMaxVals || !aggs || na < 1 || na > kMaxAggs ||
+  if (!keys || nk < 1 || nk > kMaxKeyCols || n < 0 || nv < 0 || nv > kMaxVals || !aggs || na < 1 || na > kMaxAggs ||
       !n_groups || !out_keys || !out_aggs || out_capacity < 0) return EIGER_ERR_ARG;
   std::lock_guard<std::mutex> lk(g_mu);
   Runtime* rt = runtime();
@@ -775,11 +780,11 @@ int eiger_groupby_host(const eiger_col* keys, int32_t nk, int64_t n, const eiger
     }
     return EIGER_OK;
   };
-  eiger_col dk[2], dv[kMaxVals];
+  eiger_col dk[kMaxKeyCols], dv[kMaxVals];
   char* cur = g_arena.base;
   rc = stage(cur, dk, dv);
   if (rc) return rc;
-  eiger_stats st[2];
+  eiger_stats st[kMaxKeyCols];
   rc = do_profile(rt, dk, nk, n, dk[0].dtype != EIGER_I8, st, s);
   if (rc) return rc;
   QueryPlan q;
@@ -794,7 +799,7 @@ int eiger_groupby_host(const eiger_col* keys, int32_t nk, int64_t n, const eiger
     rc = stage(cur, dk, dv);
     if (rc) return rc;
   }
-  void* dok[2] = {nullptr, nullptr};
+  void* dok[kMaxKeyCols] = {nullptr, nullptr, nullptr, nullptr};
   void* doa[kMaxAggs] = {nullptr};
   for (int k = 0; k < nk; ++k) { dok[k] = cur; cur += align_up((size_t)out_capacity * dtype_size(keys[k].dtype), 256); }
   for (int j = 0; j < na; ++j) { doa[j] = cur; cur += align_up((size_t)out_capacity * 8, 256); }

@@ -12,6 +12,7 @@ namespace eiger {
 constexpr int kMaxAggs = 8;            // user aggregates per call
 constexpr int kMaxAcc = 9;             // + one hidden COUNT for the direct table's presence test
 constexpr int kMaxVals = 8;
+constexpr int kMaxKeyCols = 4;         // key columns fused into one 64-bit key
 constexpr int kMaxHot = 8;              // heavy-hitter keys handled outside the hash table
 constexpr int kHllP = 14;              // DESIGN.md R1
 constexpr int kHllM = 1 << kHllP;
@@ -20,16 +21,18 @@ constexpr uint64_t kEmpty64 = ~0ull;
 constexpr uint32_t kEmpty32 = ~0u;
 
 // How the key column(s) are read.  u = rebased, fused key (frame of reference +
-// positional packing): u = (k0 - min0) * mul + (k1 - min1).
+// positional packing): u = (..((k0 - min0) * rng1 + (k1 - min1)) * rng2 + ..),
+// rng_c = max_c - min_c + 1 (mixed radix: no bits lost to rounding ranges up to powers of two).
 enum KeyKind : int { KK_I32 = 0, KK_I64 = 1, KK_I8I8 = 2, KK_GEN = 3, KK_U64PRE = 4, KK_U32PRE = 5 };
 
 struct KeyDesc {
-  const void* ptr[2];
-  int32_t dtype[2];
+  const void* ptr[kMaxKeyCols];
+  int32_t dtype[kMaxKeyCols];
   int32_t ncols;
   int32_t pad;
-  uint64_t base[2];   // min of each column, sign-extended, as two's complement bits
-  uint64_t mul;       // range of column 1 (1 for a single column)
+  uint64_t base[kMaxKeyCols];   // min of each column, sign-extended, as two's complement bits
+  uint64_t rng[kMaxKeyCols];    // range of each column (rng[0] is not used by the packing)
+  uint64_t mul;       // range of column 1 (1 for a single column): the two-column fast paths
 };
 
 // Aggregate signatures with compile-time plans (the shapes of BASELINE.json's configs);

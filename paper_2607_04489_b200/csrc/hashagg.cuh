@@ -45,7 +45,7 @@ struct HashAggArgs {
   uint64_t hot[kMaxHot]; // their rebased values
   void* table; uint64_t cap; uint32_t stride;   // global table
   CallDev* call;
-  void* out_keys[2]; uint64_t* out_aggs[kMaxAggs]; int32_t n_out; int64_t out_capacity;
+  void* out_keys[kMaxKeyCols]; uint64_t* out_aggs[kMaxAggs]; int32_t n_out; int64_t out_capacity;
 };
 
 template <int KK> struct IsPre { static constexpr bool v = (KK == KK_U32PRE || KK == KK_U64PRE); };
@@ -465,7 +465,7 @@ struct Front {
         default: emit_rows<int64_t>(tid, T, base, wbase); break;
       }
     } else {
-      emit_rows<uint8_t>(tid, T, base, wbase);     // two key columns: un-fuse per group
+      emit_rows<uint8_t>(tid, T, base, wbase);     // several key columns: un-fuse per group
     }
   }
 };
@@ -650,7 +650,7 @@ int launch_one(const HashAggLaunch& L, cudaStream_t s) {
   a.n_hot = (L.spec || IsPre<KK>::v) ? 0 : std::min(L.n_hot, kMaxHot);
   for (int i = 0; i < kMaxHot; ++i) a.hot[i] = i < a.n_hot ? L.hot[i] : 0ull;
   a.table = L.table; a.cap = L.cap; a.stride = L.stride; a.call = L.call;
-  a.out_keys[0] = L.out_keys[0]; a.out_keys[1] = L.out_keys[1];
+  for (int k = 0; k < kMaxKeyCols; ++k) a.out_keys[k] = L.out_keys[k];
   for (int j = 0; j < kMaxAggs; ++j) a.out_aggs[j] = static_cast<uint64_t*>(L.out_aggs[j]);
   a.n_out = L.n_out_aggs; a.out_capacity = L.out_capacity;
   kern<<<L.blocks, L.threads, L.smem_bytes, s>>>(a);

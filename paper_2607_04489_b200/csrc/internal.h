@@ -10,8 +10,8 @@ namespace eiger {
 
 // Device block owned by the library (allocated once): profile outputs and call counters.
 struct ProfileDev {
-  long long min[2];
-  long long max[2];
+  long long min[kMaxKeyCols];
+  long long max[kMaxKeyCols];
   uint32_t hist[64];        // register-value histogram C[0 .. kHllQ + 1]
   uint32_t pair_eq, pair_n; // sample pass: adjacent sample keys that are equal / compared (skew test)
   uint32_t regs[kHllM];     // sketch registers, one per word (global atomicMax)
@@ -93,7 +93,7 @@ struct CompactLaunch {
   AggPlan plan;
   int back;
   const void* table; uint64_t cap; uint32_t stride;
-  void* out_keys[2]; void* out_aggs[kMaxAggs]; int n_out_aggs;
+  void* out_keys[kMaxKeyCols]; void* out_aggs[kMaxAggs]; int n_out_aggs;
   int64_t out_capacity;
   CallDev* call;
 };
@@ -116,7 +116,7 @@ struct HashAggLaunch {
   uint64_t hot[kMaxHot]; int n_hot;   // whole-input mode: rebased heavy-hitter keys reduced inside the warp
   void* table; uint64_t cap; uint32_t stride;   // global table (BACK_HASH layout)
   CallDev* call;
-  void* out_keys[2]; void* out_aggs[kMaxAggs]; int n_out_aggs; int64_t out_capacity;   // partition mode emits
+  void* out_keys[kMaxKeyCols]; void* out_aggs[kMaxAggs]; int n_out_aggs; int64_t out_capacity;   // partition mode emits
   int threads, blocks;
   size_t smem_bytes;
 };

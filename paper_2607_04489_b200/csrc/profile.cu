@@ -16,7 +16,7 @@ constexpr int kProfUnroll = 4;     // 16-byte vectors in flight per thread
 
 __global__ void profile_reset_kernel(ProfileDev* out, int with_regs) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t < 2) { out->min[t] = INT64_MAX; out->max[t] = INT64_MIN; }
+  if (t < kMaxKeyCols) { out->min[t] = INT64_MAX; out->max[t] = INT64_MIN; }
   if (t < 64) out->hist[t] = 0;
   if (t == 0) { out->pair_eq = 0; out->pair_n = 0; }
   if (with_regs) for (int i = t; i < kHllM; i += gridDim.x * blockDim.x) out->regs[i] = 0;

@@ -36,7 +36,7 @@ __device__ __forceinline__ typename KeyTraits<KK>::U load_u(const KeyDesc& k, in
     return b < (uint32_t)k.mul ? a * (uint32_t)k.mul + b : ~0u;    // ~0: outside the planned range (speculative runs)
   } else {
     uint64_t u = sext_load(k.ptr[0], k.dtype[0], i) - k.base[0];
-    if (k.ncols == 2) u = u * k.mul + (sext_load(k.ptr[1], k.dtype[1], i) - k.base[1]);
+    for (int c = 1; c < k.ncols; ++c) u = u * k.rng[c] + (sext_load(k.ptr[c], k.dtype[c], i) - k.base[c]);
     return u;
   }
 }
@@ -63,9 +63,13 @@ __device__ __forceinline__ void load_u2(const KeyDesc& k, int64_t i, typename Ke
 }
 
 // un-fuse and un-rebase group key u into the caller's key columns at row g
+__device__ __forceinline__ void unfuse_key(const KeyDesc& key, uint64_t u, uint64_t (&part)[kMaxKeyCols]) {
+  for (int k = key.ncols - 1; k > 0; --k) { part[k] = u % key.rng[k]; u /= key.rng[k]; }
+  part[0] = u;
+}
 __device__ __forceinline__ void store_group_key(const KeyDesc& key, void* const* out_keys, uint64_t u, uint64_t g) {
-  uint64_t part[2];
-  if (key.ncols == 2) { part[0] = u / key.mul; part[1] = u % key.mul; } else { part[0] = u; part[1] = 0; }
+  uint64_t part[kMaxKeyCols];
+  unfuse_key(key, u, part);
   for (int k = 0; k < key.ncols; ++k) {
     const uint64_t v = part[k] + key.base[k];
     switch (key.dtype[k]) {

@@ -66,3 +66,12 @@ def test_scatter_bijections():
     assert len(torch.unique(datagen.scatter64(3, ids))) == 1 << 18
     s = datagen.scatter32(ids)
     assert int(s.min()) >= -(1 << 31) and int(s.max()) < (1 << 31)
+
+
+def test_config_mk_has_exact_ndv_and_per_column_frames():
+    import oracle
+    ds = datagen.config_mk(n=50_000, nk=3, digit_bits=3)
+    assert len(ds.keys) == 3 and ds.ndv == 512
+    assert oracle.exact_ndv([k.numpy() for k in ds.keys]) == 512
+    for c, k in enumerate(ds.keys):
+        assert int(k.min()) == datagen.MK_OFFSETS[c] and int(k.max()) == datagen.MK_OFFSETS[c] + 7

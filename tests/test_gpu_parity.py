@@ -364,3 +364,60 @@ def test_heavy_hitters_int32_keys():
     ds = datagen.config3(n=SPEC_N, D=200_000, dense=True)
     ds = datagen.Dataset("C3-int32", ds.n, [ds.keys[0].to(torch.int32) - 77_000], ds.vals, ds.aggs, ds.ndv, ds.exact_f64_sum, ds.meta)
     _auto_matches(ds, eiger.GLOBAL)
+
+
+# ---- general multi-key group-by: smart key fusion without the dictionary step ----
+@pytest.mark.parametrize("nk,digit_bits,n", [(3, 3, 300_007), (4, 2, 300_007), (4, 4, 1_500_001), (3, 6, 1_500_001)])
+def test_multi_key_all_variants(nk, digit_bits, n):
+    # fused domains 2^9, 2^8, 2^16 and 2^18: every variant (direct included) on 3 and 4 int32 columns
+    ds = datagen.config_mk(n=n, nk=nk, digit_bits=digit_bits)
+    ran = run_all_variants(ds)
+    assert len(ran) == len(ALL_VARIANTS)
+
+
+def test_multi_key_mixed_widths_and_four_aggregates():
+    g = torch.Generator().manual_seed(11)
+    n = 400_003
+    k0 = torch.randint(-5, 6, (n,), generator=g, dtype=torch.int64).to(torch.int8)
+    k1 = torch.randint(-(1 << 40), -(1 << 40) + 9, (n,), generator=g, dtype=torch.int64)
+    k2 = torch.randint((1 << 31) - 20, (1 << 31), (n,), generator=g, dtype=torch.int64).to(torch.int32)   # up to INT32_MAX
+    k3 = torch.randint(-128, -120, (n,), generator=g, dtype=torch.int64).to(torch.int8)                   # down to INT8_MIN
+    vf = torch.randint(0, 1 << 53, (n,), generator=g, dtype=torch.int64).to(torch.float64) * 2.0 ** -53
+    vi = torch.randint(-(1 << 62), 1 << 62, (n,), generator=g, dtype=torch.int64)
+    aggs = [(eiger.SUM, 0), (eiger.COUNT, 0), (eiger.MIN, 0), (eiger.MAX, 0), (eiger.SUM, 1), (eiger.MIN, 1)]
+    ds = datagen.Dataset("mk-mixed", n, [k0, k1, k2, k3], [vf, vi], aggs, exact_f64_sum=True)
+    run_all_variants(ds)
+    # three columns, the middle one constant
+    ds = datagen.Dataset("mk-const", n, [k2, torch.full((n,), 77, dtype=torch.int64), k0], [vi], [(eiger.SUM, 0), (eiger.COUNT, 0)])
+    run_all_variants(ds)
+
+
+def test_multi_key_wide_ranges_and_infeasible():
+    # three columns whose ranges multiply to ~2^61: the fused key needs the 64-bit path; DIRECT cannot run
+    g = torch.Generator().manual_seed(12)
+    n = 250_001
+    ids = torch.randint(0, 5000, (n,), generator=g, dtype=torch.int64)          # 5000 distinct tuples
+    k0 = (datagen.fmix64(ids) >> 44).to(torch.int32)                             # ~2^20 range
+    k1 = datagen.fmix64(ids + 77) >> 34                                          # ~2^30 range, int64
+    k2 = (datagen.fmix64(ids + 999) >> 53).to(torch.int32)                       # ~2^11 range
+    v = torch.randint(0, 1 << 31, (n,), generator=g, dtype=torch.int64)
+    ds = datagen.Dataset("mk-wide", n, [k0, k1, k2], [v], [(eiger.SUM, 0), (eiger.COUNT, 0)])
+    ran = run_all_variants(ds, expect_infeasible=(eiger.DIRECT,))
+    assert eiger.DIRECT not in ran[1:]
+    # a fourth full-range int64 column: the product of the ranges no longer fits 64 bits
+    k3 = datagen.fmix64(ids + 5)
+    d = to_dev(datagen.Dataset("mk-over", n, [k0, k1, k2, k3], [v], [(eiger.SUM, 0), (eiger.COUNT, 0)]))
+    with pytest.raises(eiger.EigerError) as e:
+        eiger.groupby(d.keys, d.vals, d.aggs)
+    assert e.value.code == eiger.ERR_INFEASIBLE
+    with pytest.raises(eiger.EigerError) as e:                                   # five key columns
+        eiger.groupby(d.keys + [d.keys[0]], d.vals, d.aggs)
+    assert e.value.code == eiger.ERR_ARG
+
+
+def test_multi_key_host_entry_point():
+    ds = datagen.config_mk(n=200_003, nk=4, digit_bits=3)
+    want = oracle_result(ds)
+    res, h2d, d2h = eiger.groupby_host(ds.keys, ds.vals, ds.aggs)
+    assert_matches(res, want, ds.aggs, ds.vals)
+    assert h2d == ds.n * ds.row_bytes
