@@ -209,15 +209,20 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
     }
   }
   uint64_t R = Rk[0];
+  for (int k = 0; k < kMaxKeyCols; ++k) kd.rng[k] = k < nk ? Rk[k] : 1;     // rng[0] = 0 (full 64-bit range) only on the single-column paths
   if (nk >= 2) {
     unsigned __int128 prod = 1;
     for (int k = 0; k < nk; ++k) {
       if (Rk[k] == 0) return EIGER_ERR_INFEASIBLE;
       prod *= Rk[k];
       if (prod >> 64) return EIGER_ERR_INFEASIBLE;   // fused key must fit 64 bits
-      kd.rng[k] = Rk[k];
     }
     R = (uint64_t)prod; kd.mul = Rk[1];
+  }
+  {
+    bool all32 = true;
+    for (int k = 0; k < nk; ++k) all32 = all32 && keys[k].dtype == EIGER_I32;
+    kd.flags = (all32 ? kKeyAll32 : 0) | (R != 0 && R <= 0xFFFFFFFFull ? kKey32 : 0);
   }
   q->R = R;
   // group-count bound and estimate
@@ -535,7 +540,8 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         if ((double)hbk->cnt[i] >= T.hot_min_share * (double)hbk->samples) hot_key[hot_n++] = hbk->key[i];
       if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] heavy hitters: %d (top share %.3f)\n", hot_n, hbk->n ? (double)hbk->cnt[0] / hbk->samples : 0.0);
     }
-    const bool fusable = nk == 1 || (keys[0].dtype == EIGER_I8 && keys[1].dtype == EIGER_I8);
+    // every key kind notices a key outside the planned range of its column (rows.cuh: fuse_cols)
+    const bool fusable = true;
     for (int k = 0; k < nk; ++k) {       // a little slack around the sampled range (clamped to the key type)
       const int bits = 8 * dtype_size(keys[k].dtype);
       const int64_t tmin = bits == 64 ? INT64_MIN : -(1ll << (bits - 1)), tmax = bits == 64 ? INT64_MAX : (1ll << (bits - 1)) - 1;

@@ -25,13 +25,15 @@ constexpr uint32_t kEmpty32 = ~0u;
 // rng_c = max_c - min_c + 1 (mixed radix: no bits lost to rounding ranges up to powers of two).
 enum KeyKind : int { KK_I32 = 0, KK_I64 = 1, KK_I8I8 = 2, KK_GEN = 3, KK_U64PRE = 4, KK_U32PRE = 5 };
 
+constexpr int kKeyAll32 = 1;   // every key column is EIGER_I32: 8-byte vector loads, 32-bit rebasing
+constexpr int kKey32 = 2;      // the fused domain fits 32 bits: 32-bit multiplies
 struct KeyDesc {
   const void* ptr[kMaxKeyCols];
   int32_t dtype[kMaxKeyCols];
   int32_t ncols;
-  int32_t pad;
+  int32_t flags;      // kKeyAll32 | kKey32 (generic path only)
   uint64_t base[kMaxKeyCols];   // min of each column, sign-extended, as two's complement bits
-  uint64_t rng[kMaxKeyCols];    // range of each column (rng[0] is not used by the packing)
+  uint64_t rng[kMaxKeyCols];    // range of each column; 1 for unused columns
   uint64_t mul;       // range of column 1 (1 for a single column): the two-column fast paths
 };
 

@@ -19,6 +19,28 @@ template <> __device__ __forceinline__ uint32_t empty_of<uint32_t>() { return kE
 template <> __device__ __forceinline__ uint64_t empty_of<uint64_t>() { return kEmpty64; }
 
 // ---- key loading ---------------------------------------------------------------------
+// Generic fusion of up to kMaxKeyCols rebased column values d[c] (0 for unused columns, whose
+// range is 1).  All columns are loaded before the multiply chain starts (independent loads in
+// flight together); a value outside its column's planned range gives ~0, which no valid fused
+// key equals (the product of the ranges fits 64 bits): speculative runs plan from a sample and
+// must notice such rows instead of aliasing them onto another group.
+__device__ __forceinline__ uint64_t fuse_cols(const KeyDesc& k, const uint64_t (&d)[kMaxKeyCols]) {
+  bool ok = true;
+#pragma unroll
+  for (int c = 0; c < kMaxKeyCols; ++c) ok = ok && d[c] < k.rng[c];
+  uint64_t u;
+  if (k.flags & kKey32) {
+    uint32_t w = (uint32_t)d[0];
+#pragma unroll
+    for (int c = 1; c < kMaxKeyCols; ++c) w = w * (uint32_t)k.rng[c] + (uint32_t)d[c];
+    u = w;
+  } else {
+    u = d[0];
+#pragma unroll
+    for (int c = 1; c < kMaxKeyCols; ++c) u = u * k.rng[c] + d[c];
+  }
+  return ok ? u : ~0ull;
+}
 template <int KK>
 __device__ __forceinline__ typename KeyTraits<KK>::U load_u(const KeyDesc& k, int64_t i) {
   using U = typename KeyTraits<KK>::U;
@@ -35,9 +57,10 @@ __device__ __forceinline__ typename KeyTraits<KK>::U load_u(const KeyDesc& k, in
     const uint32_t b = (uint32_t)(int32_t)(int8_t)ldg_stream_1((const int8_t*)k.ptr[1] + i) - (uint32_t)k.base[1];
     return b < (uint32_t)k.mul ? a * (uint32_t)k.mul + b : ~0u;    // ~0: outside the planned range (speculative runs)
   } else {
-    uint64_t u = sext_load(k.ptr[0], k.dtype[0], i) - k.base[0];
-    for (int c = 1; c < k.ncols; ++c) u = u * k.rng[c] + (sext_load(k.ptr[c], k.dtype[c], i) - k.base[c]);
-    return u;
+    uint64_t d[kMaxKeyCols];
+#pragma unroll
+    for (int c = 0; c < kMaxKeyCols; ++c) d[c] = c < k.ncols ? sext_load(k.ptr[c], k.dtype[c], i) - k.base[c] : 0ull;
+    return fuse_cols(k, d);
   }
 }
 // two consecutive rows starting at an even row index (vector loads)
@@ -58,7 +81,23 @@ __device__ __forceinline__ void load_u2(const KeyDesc& k, int64_t i, typename Ke
     u[0] = lo0 < m ? ((uint32_t)(int32_t)(int8_t)(a & 0xFF) - b0) * m + lo0 : ~0u;   // ~0: outside the planned range
     u[1] = lo1 < m ? ((uint32_t)(int32_t)(int8_t)(a >> 8) - b0) * m + lo1 : ~0u;
   } else {
-    u[0] = load_u<KK>(k, i); u[1] = load_u<KK>(k, i + 1);
+    uint64_t d0[kMaxKeyCols], d1[kMaxKeyCols];
+    if (k.flags & kKeyAll32) {
+#pragma unroll
+      for (int c = 0; c < kMaxKeyCols; ++c) {
+        if (c < k.ncols) {
+          const uint2 v = ldg_stream_8((const int32_t*)k.ptr[c] + i);
+          d0[c] = (uint32_t)(v.x - (uint32_t)k.base[c]); d1[c] = (uint32_t)(v.y - (uint32_t)k.base[c]);
+        } else { d0[c] = 0ull; d1[c] = 0ull; }
+      }
+    } else {
+#pragma unroll
+      for (int c = 0; c < kMaxKeyCols; ++c) {
+        if (c < k.ncols) { d0[c] = sext_load(k.ptr[c], k.dtype[c], i) - k.base[c]; d1[c] = sext_load(k.ptr[c], k.dtype[c], i + 1) - k.base[c]; }
+        else { d0[c] = 0ull; d1[c] = 0ull; }
+      }
+    }
+    u[0] = fuse_cols(k, d0); u[1] = fuse_cols(k, d1);
   }
 }
 
