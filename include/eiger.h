@@ -73,7 +73,11 @@ int eiger_profile(const void* keys, int32_t dtype, int64_t n, eiger_stats* out, 
 /* eiger_profile_keys — the statistics pass exactly as EIGER_AUTO runs it inside eiger_groupby
  * when no statistics are supplied: one read-back for all key columns; min/max of each; the
  * sketch only where the range test cannot decide ("range first"): 1-byte keys and
- * multi-column keys get ndv_est = min(n, max - min + 1) per column without a sketch.
+ * multi-column keys get ndv_est = min(n, max - min + 1) per column without a sketch, unless
+ * those ranges multiply to more than 2^22 (beyond a direct-index array): then one more pass
+ * sketches the FUSED key (the HLL++ branch of smart key fusion), out[0].ndv_est
+ * holds the estimate for the whole key and out[k >= 1].ndv_est = 1 (eiger_groupby multiplies
+ * the columns' estimates).
  *   keys[n_key_cols] DEVICE columns; out[n_key_cols] HOST. */
 int eiger_profile_keys(const eiger_col* keys, int32_t n_key_cols, int64_t n, eiger_stats* out, void* stream);
 

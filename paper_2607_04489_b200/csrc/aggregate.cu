@@ -300,7 +300,7 @@ __global__ void __launch_bounds__(256) compact_kernel(const __grid_constant__ Co
 template <int KK, int SIG, int FRONT, int THREADS = kAggThreads>
 int launch_one(const AggLaunch& L, cudaStream_t s) {
   auto kern = aggregate_kernel<KK, SIG, FRONT, THREADS>;
-  if (L.smem_bytes > 48 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
+  if (L.smem_bytes > 32 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
   AggArgs a;
   a.key = L.key; a.plan = L.plan; a.n = L.n;
   a.front_slots = L.front_slots; a.front_limit = L.front_limit; a.front_replicas = L.front_replicas; a.spec = L.spec;

@@ -93,9 +93,11 @@ struct Tunables {
   double hot_min_share;               // a key is hot from this share of the sample
   int slice;                          // EIGER_AUTO sizes PARTITION from a hash-space slice sketch instead of the full profile
   double slice_min_keys;              // distinct keys wanted in the slice (relative error 1 / sqrt of it)
+  double fused_sketch_min_range;      // multi-column keys: sketch the fused key when the ranges multiply to more than this
   Tunables() {
     auto env = [](const char* k, double dflt) { const char* v = std::getenv(k); return v ? std::atof(v) : dflt; };
     priv_smem = (size_t)env("EIGER_PRIV_KB", 96) << 10;
+    fused_sketch_min_range = env("EIGER_FUSED_SKETCH_MIN_RANGE", 4194304.0);   // beyond any direct-index array AUTO would take
     priv_max_range = (int)env("EIGER_PRIV_MAX_RANGE", 6);
     smem_table_bytes = (size_t)env("EIGER_SMEM_KB", 200) << 10;
     sdirect_replica_budget = (size_t)env("EIGER_SDIRECT_REPLICA_KB", 64) << 10;
@@ -247,9 +249,11 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   // bijection, and the one key that may land on the empty marker is kept in the global table
   const int hk = (nk == 1 && keys[0].dtype == EIGER_I32) ? KK_I32
                  : (nk == 1 && keys[0].dtype == EIGER_I64) ? KK_I64 : KK_GEN;
-  const size_t slot_bytes = hash_agg_slot_bytes(p, hk);
+  // partition source kind: a fused key whose domain fits 32 bits is partitioned and aggregated as 32-bit keys
+  const int hkp = (hk == KK_GEN && (kd.flags & kKey32)) ? KK_GEN32 : hk;
+  const size_t slot_bytes = hash_agg_slot_bytes(p, hk), part_slot_bytes = hash_agg_slot_bytes(p, hkp);
   const uint32_t smem_slots = (uint32_t)std::max<size_t>(64, (T.smem_table_bytes - 64) / slot_bytes) & ~7u;   // planes stay 8-byte aligned
-  const uint32_t part_slots = (uint32_t)std::max<size_t>(64, (T.part_table_bytes - 64) / slot_bytes) & ~7u;
+  const uint32_t part_slots = (uint32_t)std::max<size_t>(64, (T.part_table_bytes - 64) / part_slot_bytes) & ~7u;
   const uint32_t hash_stride = [&] { uint32_t s = 16; while (s < 8u * (1 + na)) s *= 2; return s; }();
   auto hash_cap = [&](double g) { return (uint64_t)std::max(1024.0, std::ceil(g * (1.0 + 4 * kSigma) * 1.02 / T.load)); };
 
@@ -293,6 +297,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
     q->sig = detect_sig(p, na);
     if (variant == EIGER_PARTITION) {
       if (n >= (1ll << 32)) return EIGER_ERR_INFEASIBLE;     // 32-bit per-partition counts
+      q->key_kind = hkp;
       q->threads = T.part_threads; q->slots = part_slots; q->limit = (uint32_t)(0.85 * part_slots);
       const double per = std::max(1.0, T.load * part_slots);
       const double need = ndv * (1.0 + 4 * kSigma) / per;
@@ -307,7 +312,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
       q->cap_hot = std::min(q->cap_bound, hash_cap(ndv));
       const size_t P1 = (size_t)1 << q->bits1, P = (size_t)1 << (q->bits1 + q->bits2);
       if (n / (int64_t)P >= 32768) q->cap = q->cap_hot;
-      const size_t kb = hk == KK_I32 ? 4 : 8;
+      const size_t kb = (hkp == KK_I32 || hkp == KK_GEN32) ? 4 : 8;
       const size_t col = align_up((size_t)n * 8, 256), kcol = align_up((size_t)n * kb, 256);
       q->part_bytes = align_up(P * 4, 256) + align_up((P + 1) * 8, 256) + align_up((2 * P + 2) * 4, 256) + align_up((P1 + 1) * 8, 256) + align_up(P1 * 8, 256) +
                       (kcol + (size_t)p.n_vals * col);
@@ -319,7 +324,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
       q->limit = front ? (uint32_t)((variant == EIGER_SMEM ? 0.75 : 0.5) * smem_slots) : 0;
       q->cap = std::min(hash_cap(ndv), q->cap_bound);
     }
-    q->smem_bytes = align_up((size_t)q->slots * slot_bytes + 64, 16);
+    q->smem_bytes = align_up((size_t)q->slots * (variant == EIGER_PARTITION ? part_slot_bytes : slot_bytes) + 64, 16);
     q->table_bytes = align_up((size_t)(q->cap + 1) * q->stride, 256);
   }
   q->total_bytes = q->table_bytes + q->part_bytes + 256;
@@ -355,6 +360,38 @@ int do_profile(Runtime* rt, const eiger_col* cols, int nk, int64_t n, int with_h
     double est = with_hll ? hll_estimate_from_hist(b->hist) : range;
     est = std::min(est, std::min((double)(samples > 0 ? std::min(n, samples) : n), range));
     out[k].ndv_est = std::max(est, 0.0);
+  }
+  // several key columns whose ranges multiply to more than a direct-index array can hold: the
+  // product says little about the number of groups, so sketch the FUSED key (the
+  // "otherwise HLL++" branch of smart key fusion).  out[0].ndv_est then carries the estimate for
+  // the whole key and the other columns 1 (the planner multiplies the columns' estimates).
+  if (nk > 1 && samples == 0 && n > 0) {
+    KeyDesc kd;
+    std::memset(&kd, 0, sizeof(kd));
+    kd.ncols = nk; kd.mul = 1;
+    unsigned __int128 prod = 1;
+    bool fits = true, all32 = true;
+    for (int k = 0; k < kMaxKeyCols; ++k) {
+      kd.rng[k] = 1;
+      if (k >= nk) continue;
+      kd.ptr[k] = cols[k].data; kd.dtype[k] = cols[k].dtype; kd.base[k] = (uint64_t)out[k].min;
+      kd.rng[k] = range_of(out[k]);
+      all32 = all32 && cols[k].dtype == EIGER_I32;
+      if (kd.rng[k] == 0) fits = false;
+      if (fits) { prod *= kd.rng[k]; if (prod >> 64) fits = false; }
+    }
+    if (fits && prod > (unsigned __int128)tun().fused_sketch_min_range) {
+      kd.flags = (all32 ? kKeyAll32 : 0) | (prod <= 0xFFFFFFFFull ? kKey32 : 0);
+      { Timed t(s, 1);
+        int rc = launch_fused_hll(rt, kd, n, s); if (rc) return rc;
+        rc = launch_hll_hist(rt, s); if (rc) return rc; }
+      EIGER_CUDA(cudaMemcpyAsync(b, rt->prof, sizeof(Back), cudaMemcpyDeviceToHost, s));
+      EIGER_CUDA(cudaStreamSynchronize(s));
+      resolve_timing();
+      const double est = std::min(hll_estimate_from_hist(b->hist), std::min((double)n, (double)prod));
+      out[0].ndv_est = std::max(est, 1.0);
+      for (int k = 1; k < nk; ++k) out[k].ndv_est = 1.0;
+    }
   }
   return EIGER_OK;
 }
@@ -433,13 +470,13 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       H.threads = q.threads; H.smem_bytes = q.smem_bytes;
       {   // 32-bit keys in a nearly empty shared-memory table: 8-byte buckets (hashagg.cuh: BK)
         const double per_table = q.variant == EIGER_PARTITION ? q.ndv / (double)((size_t)1 << (q.bits1 + q.bits2)) : q.ndv;
-        H.bucket_keys = (src_kind == KK_I32 && q.variant != EIGER_GLOBAL && per_table <= tun().narrow_load * q.slots) ? 2 : 0;
+        H.bucket_keys = ((src_kind == KK_I32 || src_kind == KK_GEN32) && q.variant != EIGER_GLOBAL && per_table <= tun().narrow_load * q.slots) ? 2 : 0;
       }
       if (q.variant == EIGER_PARTITION) {
         PartitionLaunch P{};
         P.key = q.key; P.plan = q.plan; P.n = n; P.key_kind = src_kind; P.bits1 = q.bits1; P.bits2 = q.bits2;
         const size_t P1 = (size_t)1 << q.bits1, PP = (size_t)1 << (q.bits1 + q.bits2);
-        const size_t kb = src_kind == KK_I32 ? 4 : 8;
+        const size_t kb = (src_kind == KK_I32 || src_kind == KK_GEN32) ? 4 : 8;
         const size_t col = align_up((size_t)n * 8, 256), kcol = align_up((size_t)n * kb, 256);
         auto take = [&](size_t bytes) { char* r = pws; pws += align_up(bytes, 256); return r; };
         P.hist = reinterpret_cast<uint32_t*>(take(PP * 4));
@@ -463,7 +500,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         // the aggregation pass reads the partitioned copy, one CTA per partition at a time
         H.key.ptr[0] = P.out_keys;
         for (int c = 0; c < q.plan.n_vals; ++c) H.plan.vals[c] = P.out_vals[c];
-        H.key_kind = src_kind == KK_I32 ? KK_U32PRE : KK_U64PRE;
+        H.key_kind = (src_kind == KK_I32 || src_kind == KK_GEN32) ? KK_U32PRE : KK_U64PRE;
         H.part_off = P.out_off; H.item_off = P.item_off; H.item_part = P.item_part; H.n_parts = P.n_parts;
         const int occ = (int)std::max<size_t>(1, std::min<size_t>((size_t)(2048 / q.threads), (rt->smem_optin + 1024) / (q.smem_bytes + 1024)));
         H.blocks = (int)std::min<int64_t>((int64_t)rt->sm_count * occ, (int64_t)P.n_parts + n / P.chunk_rows);

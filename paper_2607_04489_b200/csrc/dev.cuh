@@ -23,7 +23,9 @@ constexpr uint32_t kEmpty32 = ~0u;
 // How the key column(s) are read.  u = rebased, fused key (frame of reference +
 // positional packing): u = (..((k0 - min0) * rng1 + (k1 - min1)) * rng2 + ..),
 // rng_c = max_c - min_c + 1 (mixed radix: no bits lost to rounding ranges up to powers of two).
-enum KeyKind : int { KK_I32 = 0, KK_I64 = 1, KK_I8I8 = 2, KK_GEN = 3, KK_U64PRE = 4, KK_U32PRE = 5 };
+// KK_GEN32: the generic fused key when its domain fits 32 bits, as a 32-bit value (source kind of
+// the partition pass: 4-byte partitioned keys, 4-byte table slots).
+enum KeyKind : int { KK_I32 = 0, KK_I64 = 1, KK_I8I8 = 2, KK_GEN = 3, KK_U64PRE = 4, KK_U32PRE = 5, KK_GEN32 = 6 };
 
 constexpr int kKeyAll32 = 1;   // every key column is EIGER_I32: 8-byte vector loads, 32-bit rebasing
 constexpr int kKey32 = 2;      // the fused domain fits 32 bits: 32-bit multiplies

@@ -5,7 +5,7 @@
 namespace eiger {
 
 size_t hash_agg_slot_bytes(const AggPlan& p, int key_kind) {
-  size_t w = (key_kind == KK_I32 || key_kind == KK_U32PRE) ? 4 : 8;
+  size_t w = (key_kind == KK_I32 || key_kind == KK_U32PRE || key_kind == KK_GEN32) ? 4 : 8;
   for (int j = 0; j < p.n_acc; ++j) w += p.op[j] == EIGER_COUNT ? 4 : 8;
   return w;
 }

@@ -643,7 +643,7 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
 template <int KK, int SIG, int BK>
 int launch_one(const HashAggLaunch& L, cudaStream_t s) {
   auto kern = hash_agg_kernel<KK, SIG, BK>;
-  if (L.smem_bytes > 48 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
+  if (L.smem_bytes > 32 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
   HashAggArgs a;
   a.key = L.key; a.plan = L.plan; a.n = L.n; a.part_off = L.part_off; a.item_off = L.item_off; a.item_part = L.item_part; a.n_parts = L.n_parts;
   a.slots = L.slots; a.limit = L.limit; a.spec = L.spec; a.max_probes = L.max_probes > 0 ? L.max_probes : 16;

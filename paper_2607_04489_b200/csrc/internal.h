@@ -57,6 +57,9 @@ int launch_part_hist_hll(Runtime* rt, const void* keys, int dtype, int64_t n, ui
 // collision rate says the keys are skewed; the whole-input hash kernel then reduces those keys'
 // rows inside the warp instead of hammering one shared-memory slot with atomics.
 int launch_hot_keys(Runtime* rt, const void* keys, int dtype, int64_t n, cudaStream_t s);
+// Sketch registers of the fused key of a multi-column key (key.base / rng / flags filled in) into
+// rt->prof->regs; launch_hll_hist then gives the histogram the estimator reads.
+int launch_fused_hll(Runtime* rt, const KeyDesc& key, int64_t n, cudaStream_t s);
 int launch_hll_hist(Runtime* rt, cudaStream_t s);
 int launch_regs_to_bytes(Runtime* rt, uint8_t* out, cudaStream_t s);
 double hll_estimate_from_hist(const uint32_t* hist);

@@ -170,7 +170,7 @@ part_scatter_kernel(const __grid_constant__ LevelArgs a) {
     // (ncu: long_scoreboard 49 % of stall samples with one tile in flight per CTA)
     {
       const int64_t nb = base + (int64_t)gridDim.x * kTile;
-      if (nb < r1 && a.key.ncols == 1) {
+      if (nb < r1 && KK != KK_GEN && KK != KK_GEN32) {
         const int64_t nm = min((int64_t)kTile, r1 - nb);
         const int64_t kbytes = nm * (int64_t)sizeof(U), vbytes = nm * 8;
         const char* kp = static_cast<const char*>(a.key.ptr[0]) + nb * (int64_t)sizeof(U);
@@ -178,6 +178,18 @@ part_scatter_kernel(const __grid_constant__ LevelArgs a) {
         for (int c = 0; c < a.n_vals; ++c) {
           const char* vp = reinterpret_cast<const char*>(a.vals[c] + nb);
           for (int64_t o = (int64_t)tid * 128; o < vbytes; o += (int64_t)kPT * 128) prefetch_l2(vp + o);
+        }
+      } else if (nb < r1) {
+        // several key columns (level 1 of a fused key): each column at its own width
+        const int64_t nm = min((int64_t)kTile, r1 - nb);
+        for (int kc = 0; kc < a.key.ncols; ++kc) {
+          const int64_t w = a.key.dtype[kc] == EIGER_I8 ? 1 : (a.key.dtype[kc] == EIGER_I32 ? 4 : 8);
+          const char* kp = static_cast<const char*>(a.key.ptr[kc]) + nb * w;
+          for (int64_t o = (int64_t)tid * 128; o < nm * w; o += (int64_t)kPT * 128) prefetch_l2(kp + o);
+        }
+        for (int c = 0; c < a.n_vals; ++c) {
+          const char* vp = reinterpret_cast<const char*>(a.vals[c] + nb);
+          for (int64_t o = (int64_t)tid * 128; o < nm * 8; o += (int64_t)kPT * 128) prefetch_l2(vp + o);
         }
       }
     }
@@ -322,7 +334,8 @@ int run_levels(PartitionLaunch& L, int sm_count, cudaStream_t s) {
   L.out_keys = L.keysA; L.out_vals = L.valsA; L.out_off = L.off1; L.n_parts = 1 << L.bits1;
   if (L.bits2 > 0) {
     LevelArgs b{};
-    b.key = L.key; b.key.ptr[0] = L.keysA; b.key.ptr[1] = nullptr;
+    b.key = L.key; b.key.ptr[0] = L.keysA; b.key.ncols = 1;      // one pre-fused column from here on
+    for (int k = 1; k < kMaxKeyCols; ++k) b.key.ptr[k] = nullptr;
     b.n = L.n; b.n_vals = L.plan.n_vals;
     for (int c = 0; c < kMaxVals; ++c) { b.vals[c] = L.valsA[c]; b.out_vals[c] = L.valsB[c]; }
     b.out_keys = L.keysB; b.seg_off = L.off1; b.hist = L.hist; b.cursor = L.cur2;
@@ -348,6 +361,7 @@ int launch_partition(PartitionLaunch& L, int sm_count, cudaStream_t s) {
     case KK_I32: return run_levels<KK_I32, KK_U32PRE>(L, sm_count, s);
     case KK_I64: return run_levels<KK_I64, KK_U64PRE>(L, sm_count, s);
     case KK_GEN: case KK_I8I8: return run_levels<KK_GEN, KK_U64PRE>(L, sm_count, s);
+    case KK_GEN32: return run_levels<KK_GEN32, KK_U32PRE>(L, sm_count, s);
     default: return EIGER_ERR_ARG;
   }
 }

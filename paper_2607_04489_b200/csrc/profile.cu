@@ -7,6 +7,7 @@
 #include <type_traits>
 
 #include "internal.h"
+#include "rows.cuh"
 
 namespace eiger {
 namespace {
@@ -341,6 +342,37 @@ __global__ void regs_to_bytes_kernel(const ProfileDev* in, uint8_t* out) {
   if (i < kHllM) out[i] = (uint8_t)in->regs[i];
 }
 
+// Sketch of the FUSED key of a multi-column key (smart key fusion: where the range
+// cannot settle it, "calculate the HLL++ sketch on the key and find the number of distinct
+// values"): the same registers as profile_kernel's, over u = the rebased, packed key (rows.cuh:
+// fuse_cols) taken as a 64-bit value.  The product of the column ranges bounds the group count
+// only loosely (5000 distinct triples can span a 2^61 domain); this estimate sizes the tables.
+__global__ void __launch_bounds__(kProfThreads)
+fused_hll_kernel(const __grid_constant__ KeyDesc k, int64_t n, ProfileDev* __restrict__ out) {
+  extern __shared__ uint32_t sregs[];   // kHllM words
+  const int tid = threadIdx.x;
+  for (int i = tid; i < kHllM; i += kProfThreads) sregs[i] = 0;
+  __syncthreads();
+  const int64_t pairs = n / 2, stride = (int64_t)gridDim.x * kProfThreads;
+  int64_t p = (int64_t)blockIdx.x * kProfThreads + tid;
+  for (; p + stride < pairs; p += 2 * stride) {
+    uint64_t a[2], b[2];
+    load_u2<KK_GEN>(k, 2 * p, a); load_u2<KK_GEN>(k, 2 * (p + stride), b);
+    hll_update(sregs, a[0]); hll_update(sregs, a[1]); hll_update(sregs, b[0]); hll_update(sregs, b[1]);
+  }
+  for (; p < pairs; p += stride) {
+    uint64_t a[2];
+    load_u2<KK_GEN>(k, 2 * p, a);
+    hll_update(sregs, a[0]); hll_update(sregs, a[1]);
+  }
+  if ((n & 1) && blockIdx.x == 0 && tid == 0) hll_update(sregs, load_u<KK_GEN>(k, n - 1));
+  __syncthreads();
+  for (int i = tid; i < kHllM; i += kProfThreads) {
+    const uint32_t r = sregs[i];
+    if (r) atomicMax(&out->regs[i], r);
+  }
+}
+
 template <int DT>
 int launch_profile_dt(Runtime* rt, const void* keys, int64_t n, int which, int with_hll, cudaStream_t s) {
   const int64_t nvec = n / Elem<DT>::kPerVec;
@@ -375,6 +407,19 @@ int launch_profile(Runtime* rt, const void* keys, int dtype, int64_t n, int whic
     case EIGER_I64: return launch_profile_dt<EIGER_I64>(rt, keys, n, which, with_hll, s);
     default: return EIGER_ERR_ARG;
   }
+}
+
+int launch_fused_hll(Runtime* rt, const KeyDesc& key, int64_t n, cudaStream_t s) {
+  EIGER_CUDA(cudaMemsetAsync(rt->prof->regs, 0, sizeof(uint32_t) * kHllM, s));
+  if (n == 0) return EIGER_OK;
+  const int64_t want = (n / 2 + (int64_t)kProfThreads * 2 - 1) / ((int64_t)kProfThreads * 2);
+  const int blocks = (int)std::max<int64_t>(1, std::min<int64_t>(want, 2LL * rt->sm_count));
+  auto kern = fused_hll_kernel;
+  EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kHllM * 4));
+  kern<<<blocks, kProfThreads, kHllM * 4, s>>>(key, n, rt->prof);
+  count_launch();
+  EIGER_CUDA(cudaGetLastError());
+  return EIGER_OK;
 }
 
 int launch_part_hist_hll(Runtime* rt, const void* keys, int dtype, int64_t n, uint64_t base, uint32_t sel, cudaStream_t s) {

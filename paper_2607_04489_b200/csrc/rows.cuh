@@ -13,6 +13,7 @@ template <> struct KeyTraits<KK_I64> { using U = uint64_t; };
 template <> struct KeyTraits<KK_GEN> { using U = uint64_t; };
 template <> struct KeyTraits<KK_U64PRE> { using U = uint64_t; };
 template <> struct KeyTraits<KK_U32PRE> { using U = uint32_t; };
+template <> struct KeyTraits<KK_GEN32> { using U = uint32_t; };
 
 template <class U> __device__ __forceinline__ U empty_of();
 template <> __device__ __forceinline__ uint32_t empty_of<uint32_t>() { return kEmpty32; }
@@ -52,6 +53,8 @@ __device__ __forceinline__ typename KeyTraits<KK>::U load_u(const KeyDesc& k, in
     return ldg_stream_u64((const uint64_t*)k.ptr[0] + i);
   } else if constexpr (KK == KK_U32PRE) {
     return ldg_stream_4((const uint32_t*)k.ptr[0] + i);
+  } else if constexpr (KK == KK_GEN32) {
+    return (uint32_t)load_u<KK_GEN>(k, i);      // ~0 (out of range) stays ~0
   } else if constexpr (KK == KK_I8I8) {
     const uint32_t a = (uint32_t)(int32_t)(int8_t)ldg_stream_1((const int8_t*)k.ptr[0] + i) - (uint32_t)k.base[0];
     const uint32_t b = (uint32_t)(int32_t)(int8_t)ldg_stream_1((const int8_t*)k.ptr[1] + i) - (uint32_t)k.base[1];
@@ -74,6 +77,10 @@ __device__ __forceinline__ void load_u2(const KeyDesc& k, int64_t i, typename Ke
     const uint4 v = ldg_stream_16((const uint64_t*)k.ptr[0] + i);
     const uint64_t b = KK == KK_I64 ? k.base[0] : 0ull;
     u[0] = (((uint64_t)v.y << 32) | v.x) - b; u[1] = (((uint64_t)v.w << 32) | v.z) - b;
+  } else if constexpr (KK == KK_GEN32) {
+    uint64_t w[2];
+    load_u2<KK_GEN>(k, i, w);
+    u[0] = (uint32_t)w[0]; u[1] = (uint32_t)w[1];
   } else if constexpr (KK == KK_I8I8) {
     const uint32_t a = ldg_stream_2((const int8_t*)k.ptr[0] + i), b = ldg_stream_2((const int8_t*)k.ptr[1] + i);
     const uint32_t b0 = (uint32_t)k.base[0], b1 = (uint32_t)k.base[1], m = (uint32_t)k.mul;
