@@ -211,6 +211,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
     }
   }
   uint64_t R = Rk[0];
+  for (int k = nk; k < kMaxKeyCols; ++k) { kd.ptr[k] = kd.ptr[0]; kd.dtype[k] = kd.dtype[0]; }   // loadable, masked out (rows.cuh)
   for (int k = 0; k < kMaxKeyCols; ++k) kd.rng[k] = k < nk ? Rk[k] : 1;     // rng[0] = 0 (full 64-bit range) only on the single-column paths
   if (nk >= 2) {
     unsigned __int128 prod = 1;
@@ -373,7 +374,7 @@ int do_profile(Runtime* rt, const eiger_col* cols, int nk, int64_t n, int with_h
     bool fits = true, all32 = true;
     for (int k = 0; k < kMaxKeyCols; ++k) {
       kd.rng[k] = 1;
-      if (k >= nk) continue;
+      if (k >= nk) { kd.ptr[k] = cols[0].data; kd.dtype[k] = cols[0].dtype; continue; }
       kd.ptr[k] = cols[k].data; kd.dtype[k] = cols[k].dtype; kd.base[k] = (uint64_t)out[k].min;
       kd.rng[k] = range_of(out[k]);
       all32 = all32 && cols[k].dtype == EIGER_I32;

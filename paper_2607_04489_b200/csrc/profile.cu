@@ -355,10 +355,12 @@ fused_hll_kernel(const __grid_constant__ KeyDesc k, int64_t n, ProfileDev* __res
   __syncthreads();
   const int64_t pairs = n / 2, stride = (int64_t)gridDim.x * kProfThreads;
   int64_t p = (int64_t)blockIdx.x * kProfThreads + tid;
-  for (; p + stride < pairs; p += 2 * stride) {
-    uint64_t a[2], b[2];
-    load_u2<KK_GEN>(k, 2 * p, a); load_u2<KK_GEN>(k, 2 * (p + stride), b);
-    hll_update(sregs, a[0]); hll_update(sregs, a[1]); hll_update(sregs, b[0]); hll_update(sregs, b[1]);
+  for (; p + 3 * stride < pairs; p += 4 * stride) {
+    uint64_t a[4][2];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) load_u2<KK_GEN>(k, 2 * (p + j * stride), a[j]);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { hll_update(sregs, a[j][0]); hll_update(sregs, a[j][1]); }
   }
   for (; p < pairs; p += stride) {
     uint64_t a[2];
@@ -412,7 +414,7 @@ int launch_profile(Runtime* rt, const void* keys, int dtype, int64_t n, int whic
 int launch_fused_hll(Runtime* rt, const KeyDesc& key, int64_t n, cudaStream_t s) {
   EIGER_CUDA(cudaMemsetAsync(rt->prof->regs, 0, sizeof(uint32_t) * kHllM, s));
   if (n == 0) return EIGER_OK;
-  const int64_t want = (n / 2 + (int64_t)kProfThreads * 2 - 1) / ((int64_t)kProfThreads * 2);
+  const int64_t want = (n / 2 + (int64_t)kProfThreads * 4 - 1) / ((int64_t)kProfThreads * 4);
   const int blocks = (int)std::max<int64_t>(1, std::min<int64_t>(want, 2LL * rt->sm_count));
   auto kern = fused_hll_kernel;
   EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kHllM * 4));

@@ -61,8 +61,18 @@ __device__ __forceinline__ typename KeyTraits<KK>::U load_u(const KeyDesc& k, in
     return b < (uint32_t)k.mul ? a * (uint32_t)k.mul + b : ~0u;    // ~0: outside the planned range (speculative runs)
   } else {
     uint64_t d[kMaxKeyCols];
+    if (k.flags & kKeyAll32) {
+      // branch-free: unused columns point at column 0 (host side) and are masked out, so that the
+      // (volatile) loads of all columns sit in one basic block and go out back to back
+      uint32_t v[kMaxKeyCols];
 #pragma unroll
-    for (int c = 0; c < kMaxKeyCols; ++c) d[c] = c < k.ncols ? sext_load(k.ptr[c], k.dtype[c], i) - k.base[c] : 0ull;
+      for (int c = 0; c < kMaxKeyCols; ++c) v[c] = ldg_stream_4((const int32_t*)k.ptr[c] + i);
+#pragma unroll
+      for (int c = 0; c < kMaxKeyCols; ++c) d[c] = c < k.ncols ? (uint64_t)(uint32_t)(v[c] - (uint32_t)k.base[c]) : 0ull;
+    } else {
+#pragma unroll
+      for (int c = 0; c < kMaxKeyCols; ++c) d[c] = c < k.ncols ? sext_load(k.ptr[c], k.dtype[c], i) - k.base[c] : 0ull;
+    }
     return fuse_cols(k, d);
   }
 }
@@ -90,12 +100,24 @@ __device__ __forceinline__ void load_u2(const KeyDesc& k, int64_t i, typename Ke
   } else {
     uint64_t d0[kMaxKeyCols], d1[kMaxKeyCols];
     if (k.flags & kKeyAll32) {
+      // branch-free per column (see load_u): one code copy per column count
+      uint2 v[kMaxKeyCols];
+      if (k.ncols <= 2) {
+#pragma unroll
+        for (int c = 0; c < 2; ++c) v[c] = ldg_stream_8((const int32_t*)k.ptr[c] + i);
+        v[2] = v[0]; v[3] = v[0];
+      } else if (k.ncols == 3) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) v[c] = ldg_stream_8((const int32_t*)k.ptr[c] + i);
+        v[3] = v[0];
+      } else {
+#pragma unroll
+        for (int c = 0; c < kMaxKeyCols; ++c) v[c] = ldg_stream_8((const int32_t*)k.ptr[c] + i);
+      }
 #pragma unroll
       for (int c = 0; c < kMaxKeyCols; ++c) {
-        if (c < k.ncols) {
-          const uint2 v = ldg_stream_8((const int32_t*)k.ptr[c] + i);
-          d0[c] = (uint32_t)(v.x - (uint32_t)k.base[c]); d1[c] = (uint32_t)(v.y - (uint32_t)k.base[c]);
-        } else { d0[c] = 0ull; d1[c] = 0ull; }
+        d0[c] = c < k.ncols ? (uint64_t)(uint32_t)(v[c].x - (uint32_t)k.base[c]) : 0ull;
+        d1[c] = c < k.ncols ? (uint64_t)(uint32_t)(v[c].y - (uint32_t)k.base[c]) : 0ull;
       }
     } else {
 #pragma unroll
