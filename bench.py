@@ -208,7 +208,10 @@ def traffic_from_profiles(workload: str, kernel: str):
     """dram bytes per launch of the dominant kernel from the committed ncu capture, if there is one."""
     try:
         with open(os.path.join(ROOT, "profiles", "r1_traffic.json")) as f:
-            return json.load(f).get(f"{workload.split(':')[0].upper()}:{kernel}")
+            d = json.load(f)
+        # a capture of exactly this workload, else (C1-C4: one workload per name) of the config
+        base = workload.split(":")[0].upper()
+        return d.get(f"{workload.upper()}:{kernel}", d.get(f"{base}:{kernel}") if base in ("C1", "C2", "C3", "C4") else None)
     except (OSError, ValueError):
         return None
 
@@ -275,7 +278,8 @@ def main(argv=None):
     # dominant kernel and its algorithmic bytes per launch
     dom = max(("aggregate", "partition", "profile"), key=lambda k: kt[k][0])
     key_bytes = sum(k.element_size() for k in ds.keys)
-    part_row = (4 if (len(ds.keys) == 1 and ds.keys[0].dtype == torch.int32) else 8) + 8 * len(ds.vals)   # B'
+    part_key = eiger.last_partition_key_bytes() if last["res"].variant == eiger.PARTITION else 8
+    part_row = part_key + 8 * len(ds.vals)   # B': one row of the partitioned copy
     out_row = key_bytes + 8 * len(ds.aggs)
     levels = eiger.last_partition_levels() if res.variant == eiger.PARTITION else 0
     # EIGER_AUTO's slice-sketch pass already took the level-1 histogram: no keys-only read in the partition pass

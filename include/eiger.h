@@ -172,6 +172,11 @@ double eiger_last_ndv_estimate(void);
  * keys-only histogram pass: bench.py needs it for the algorithmic bytes of the partition pass. */
 int32_t eiger_last_partition_prehist(void);
 
+/* Bytes per key (4 or 8) of the partitioned copy written by the last EIGER_PARTITION call: 4 for a
+ * single int32 column and for multi-column keys whose fused domain fits 32 bits, else 8.
+ * bench.py needs it for the algorithmic bytes of the partition pass. */
+int32_t eiger_last_partition_key_bytes(void);
+
 /* Number of kernels this library has launched in this process (bench.py's gpu_launches). */
 int64_t eiger_launch_count(void);
 

@@ -32,7 +32,7 @@ HLL_M = 1 << 14
 EXPORTS = [
     "eiger_profile", "eiger_profile_keys", "eiger_hll_registers", "eiger_hll_estimate_host", "eiger_groupby",
     "eiger_groupby_workspace_bytes", "eiger_select_variant", "eiger_groupby_host",
-    "eiger_launch_count", "eiger_last_partition_levels", "eiger_last_ndv_estimate", "eiger_last_partition_prehist", "eiger_set_kernel_timing", "eiger_kernel_time_ms", "eiger_strerror",
+    "eiger_launch_count", "eiger_last_partition_levels", "eiger_last_ndv_estimate", "eiger_last_partition_prehist", "eiger_last_partition_key_bytes", "eiger_set_kernel_timing", "eiger_kernel_time_ms", "eiger_strerror",
     "eiger_last_cuda_error", "eiger_variant_name", "eiger_shutdown",
 ]
 
@@ -117,6 +117,7 @@ def lib() -> ctypes.CDLL:
         L.eiger_last_partition_levels.restype = i32
         L.eiger_last_ndv_estimate.restype = ctypes.c_double
         L.eiger_last_partition_prehist.restype = i32
+        L.eiger_last_partition_key_bytes.restype = i32
         L.eiger_set_kernel_timing.argtypes = [i32]
         L.eiger_kernel_time_ms.restype = ctypes.c_double
         L.eiger_kernel_time_ms.argtypes = [i32, i32, ctypes.POINTER(i64)]
@@ -403,6 +404,10 @@ def last_ndv_estimate() -> float:
 
 def last_partition_prehist() -> bool:
     return bool(lib().eiger_last_partition_prehist())
+
+
+def last_partition_key_bytes() -> int:
+    return int(lib().eiger_last_partition_key_bytes())
 
 
 def set_kernel_timing(enabled: bool) -> None:

@@ -22,6 +22,7 @@ bool g_timing = false;
 int g_last_levels = 0;
 double g_last_ndv = 0;
 int g_last_prehist = 0;
+int g_last_part_key_bytes = 0;
 constexpr int kTimeSlots = 5;
 double g_time_ms[kTimeSlots] = {0, 0, 0, 0, 0};
 int64_t g_time_n[kTimeSlots] = {0, 0, 0, 0, 0};
@@ -498,6 +499,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         { Timed t(s, 2); rc = launch_partition(P, rt->sm_count, s); if (rc) return rc; }
         g_last_levels = q.bits2 > 0 ? 2 : 1;
         g_last_prehist = q.pre_hist ? 1 : 0;
+        g_last_part_key_bytes = (int)kb;
         // the aggregation pass reads the partitioned copy, one CTA per partition at a time
         H.key.ptr[0] = P.out_keys;
         for (int c = 0; c < q.plan.n_vals; ++c) H.plan.vals[c] = P.out_vals[c];
@@ -871,6 +873,7 @@ int64_t eiger_launch_count(void) { return g_launches.load(); }
 int32_t eiger_last_partition_levels(void) { return g_last_levels; }
 double eiger_last_ndv_estimate(void) { return g_last_ndv; }
 int32_t eiger_last_partition_prehist(void) { return g_last_prehist; }
+int32_t eiger_last_partition_key_bytes(void) { return g_last_part_key_bytes; }
 
 void eiger_set_kernel_timing(int32_t enabled) { std::lock_guard<std::mutex> lk(g_mu); g_timing = enabled != 0; }
 
