@@ -170,7 +170,8 @@ part_scatter_kernel(const __grid_constant__ LevelArgs a) {
     // (ncu: long_scoreboard 49 % of stall samples with one tile in flight per CTA)
     {
       const int64_t nb = base + (int64_t)gridDim.x * kTile;
-      if (nb < r1 && KK != KK_GEN && KK != KK_GEN32) {
+      if constexpr (KK != KK_GEN && KK != KK_GEN32) {
+       if (nb < r1 && a.key.ncols == 1) {
         const int64_t nm = min((int64_t)kTile, r1 - nb);
         const int64_t kbytes = nm * (int64_t)sizeof(U), vbytes = nm * 8;
         const char* kp = static_cast<const char*>(a.key.ptr[0]) + nb * (int64_t)sizeof(U);
@@ -179,6 +180,7 @@ part_scatter_kernel(const __grid_constant__ LevelArgs a) {
           const char* vp = reinterpret_cast<const char*>(a.vals[c] + nb);
           for (int64_t o = (int64_t)tid * 128; o < vbytes; o += (int64_t)kPT * 128) prefetch_l2(vp + o);
         }
+       }
       } else if (nb < r1) {
         // several key columns (level 1 of a fused key): each column at its own width
         const int64_t nm = min((int64_t)kTile, r1 - nb);
