@@ -114,6 +114,20 @@ __device__ __forceinline__ void load_u2(const KeyDesc& k, int64_t i, typename Ke
 #pragma unroll
         for (int c = 0; c < kMaxKeyCols; ++c) v[c] = ldg_stream_8((const int32_t*)k.ptr[c] + i);
       }
+      if (k.flags & kKey32) {
+        // fused domain below 2^32: rebasing, range checks and packing all in 32-bit arithmetic
+        uint32_t w0 = 0, w1 = 0;
+        bool ok0 = true, ok1 = true;
+#pragma unroll
+        for (int c = 0; c < kMaxKeyCols; ++c) {
+          const uint32_t b = (uint32_t)k.base[c], r = (uint32_t)k.rng[c];
+          const uint32_t e0 = c < k.ncols ? v[c].x - b : 0u, e1 = c < k.ncols ? v[c].y - b : 0u;
+          ok0 = ok0 && e0 < r; ok1 = ok1 && e1 < r;
+          w0 = w0 * r + e0; w1 = w1 * r + e1;         // c = 0: 0 * r + e
+        }
+        u[0] = ok0 ? (uint64_t)w0 : ~0ull; u[1] = ok1 ? (uint64_t)w1 : ~0ull;
+        return;
+      }
 #pragma unroll
       for (int c = 0; c < kMaxKeyCols; ++c) {
         d0[c] = c < k.ncols ? (uint64_t)(uint32_t)(v[c].x - (uint32_t)k.base[c]) : 0ull;
