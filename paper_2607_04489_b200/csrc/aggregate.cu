@@ -350,6 +350,7 @@ int launch_aggregate(const AggLaunch& L, cudaStream_t s) {
     case KK_I64: return launch_sig<KK_I64>(L, s);
     case KK_I8I8: return launch_sig<KK_I8I8>(L, s);
     case KK_GEN: return launch_sig<KK_GEN>(L, s);
+    case KK_GEN32: return launch_sig<KK_GEN32>(L, s);
     default: return EIGER_ERR_ARG;
   }
 }

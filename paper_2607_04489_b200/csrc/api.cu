@@ -278,7 +278,8 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
     q->back = BACK_DIRECT;
     q->key_kind = (nk == 1 && keys[0].dtype == EIGER_I32 && R <= 0xFFFFFFFFull) ? KK_I32
                   : (nk == 1 && keys[0].dtype == EIGER_I64) ? KK_I64
-                  : (nk == 2 && keys[0].dtype == EIGER_I8 && keys[1].dtype == EIGER_I8) ? KK_I8I8 : KK_GEN;
+                  : (nk == 2 && keys[0].dtype == EIGER_I8 && keys[1].dtype == EIGER_I8) ? KK_I8I8
+                  : (kd.flags & kKey32) ? KK_GEN32 : KK_GEN;      // fused domain below 2^32: 32-bit slots indices
     q->cap = R; q->stride = 8u * p.n_acc;
     q->table_bytes = align_up((size_t)R * q->stride, 256);
     if (direct_bytes * 256 <= T.priv_smem && R <= (uint64_t)T.priv_max_range) {

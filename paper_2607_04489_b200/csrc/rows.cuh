@@ -42,6 +42,35 @@ __device__ __forceinline__ uint64_t fuse_cols(const KeyDesc& k, const uint64_t (
   }
   return ok ? u : ~0ull;
 }
+// All-int32 key columns with a fused domain below 2^32, two consecutive rows: rebasing, range
+// checks and packing in 32-bit arithmetic, NC columns known at compile time (one code copy per
+// column count: no work for absent columns, every load in one basic block).  ~0u = some column
+// outside its planned range (no valid fused key: the domain is below 2^32).
+template <int NC>
+__device__ __forceinline__ void fuse32_pair(const KeyDesc& k, int64_t i, uint32_t (&w)[2]) {
+  uint2 v[NC];
+#pragma unroll
+  for (int c = 0; c < NC; ++c) v[c] = ldg_stream_8((const int32_t*)k.ptr[c] + i);
+  uint32_t w0 = 0, w1 = 0;
+  bool ok0 = true, ok1 = true;
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    const uint32_t b = (uint32_t)k.base[c], r = (uint32_t)k.rng[c];
+    const uint32_t e0 = v[c].x - b, e1 = v[c].y - b;
+    ok0 = ok0 && e0 < r; ok1 = ok1 && e1 < r;
+    w0 = w0 * r + e0; w1 = w1 * r + e1;         // c = 0: 0 * r + e
+  }
+  w[0] = ok0 ? w0 : ~0u; w[1] = ok1 ? w1 : ~0u;
+}
+__device__ __forceinline__ void fuse32_pair_any(const KeyDesc& k, int64_t i, uint32_t (&w)[2]) {
+  switch (k.ncols) {
+    case 1: fuse32_pair<1>(k, i, w); break;
+    case 2: fuse32_pair<2>(k, i, w); break;
+    case 3: fuse32_pair<3>(k, i, w); break;
+    default: fuse32_pair<4>(k, i, w); break;
+  }
+}
+
 template <int KK>
 __device__ __forceinline__ typename KeyTraits<KK>::U load_u(const KeyDesc& k, int64_t i) {
   using U = typename KeyTraits<KK>::U;
@@ -88,9 +117,12 @@ __device__ __forceinline__ void load_u2(const KeyDesc& k, int64_t i, typename Ke
     const uint64_t b = KK == KK_I64 ? k.base[0] : 0ull;
     u[0] = (((uint64_t)v.y << 32) | v.x) - b; u[1] = (((uint64_t)v.w << 32) | v.z) - b;
   } else if constexpr (KK == KK_GEN32) {
-    uint64_t w[2];
-    load_u2<KK_GEN>(k, i, w);
-    u[0] = (uint32_t)w[0]; u[1] = (uint32_t)w[1];
+    if (k.flags & kKeyAll32) { fuse32_pair_any(k, i, u); }
+    else {
+      uint64_t w[2];
+      load_u2<KK_GEN>(k, i, w);
+      u[0] = (uint32_t)w[0]; u[1] = (uint32_t)w[1];
+    }
   } else if constexpr (KK == KK_I8I8) {
     const uint32_t a = ldg_stream_2((const int8_t*)k.ptr[0] + i), b = ldg_stream_2((const int8_t*)k.ptr[1] + i);
     const uint32_t b0 = (uint32_t)k.base[0], b1 = (uint32_t)k.base[1], m = (uint32_t)k.mul;
@@ -99,6 +131,12 @@ __device__ __forceinline__ void load_u2(const KeyDesc& k, int64_t i, typename Ke
     u[1] = lo1 < m ? ((uint32_t)(int32_t)(int8_t)(a >> 8) - b0) * m + lo1 : ~0u;
   } else {
     uint64_t d0[kMaxKeyCols], d1[kMaxKeyCols];
+    if ((k.flags & (kKeyAll32 | kKey32)) == (kKeyAll32 | kKey32)) {
+      uint32_t w[2];
+      fuse32_pair_any(k, i, w);
+      u[0] = w[0] == ~0u ? ~0ull : (uint64_t)w[0]; u[1] = w[1] == ~0u ? ~0ull : (uint64_t)w[1];
+      return;
+    }
     if (k.flags & kKeyAll32) {
       // branch-free per column (see load_u): one code copy per column count
       uint2 v[kMaxKeyCols];
@@ -113,20 +151,6 @@ __device__ __forceinline__ void load_u2(const KeyDesc& k, int64_t i, typename Ke
       } else {
 #pragma unroll
         for (int c = 0; c < kMaxKeyCols; ++c) v[c] = ldg_stream_8((const int32_t*)k.ptr[c] + i);
-      }
-      if (k.flags & kKey32) {
-        // fused domain below 2^32: rebasing, range checks and packing all in 32-bit arithmetic
-        uint32_t w0 = 0, w1 = 0;
-        bool ok0 = true, ok1 = true;
-#pragma unroll
-        for (int c = 0; c < kMaxKeyCols; ++c) {
-          const uint32_t b = (uint32_t)k.base[c], r = (uint32_t)k.rng[c];
-          const uint32_t e0 = c < k.ncols ? v[c].x - b : 0u, e1 = c < k.ncols ? v[c].y - b : 0u;
-          ok0 = ok0 && e0 < r; ok1 = ok1 && e1 < r;
-          w0 = w0 * r + e0; w1 = w1 * r + e1;         // c = 0: 0 * r + e
-        }
-        u[0] = ok0 ? (uint64_t)w0 : ~0ull; u[1] = ok1 ? (uint64_t)w1 : ~0ull;
-        return;
       }
 #pragma unroll
       for (int c = 0; c < kMaxKeyCols; ++c) {
