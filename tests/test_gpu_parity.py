@@ -455,3 +455,18 @@ def test_multi_key_fused_sketch():
     small = datagen.config_mk(n=100_001, nk=3, digit_bits=3)
     st = eiger.profile_keys([c.to(DEV) for c in small.keys])
     assert [s.ndv_est for s in st] == [8.0, 8.0, 8.0]
+
+
+@pytest.mark.parametrize("n", [0, 1, 3, 1025, 4097])
+def test_multi_key_tiny_and_ragged(n):
+    g = torch.Generator().manual_seed(40 + n)
+    k0 = torch.randint(-3, 4, (n,), generator=g, dtype=torch.int64).to(torch.int32)
+    k1 = torch.randint(50, 53, (n,), generator=g, dtype=torch.int64).to(torch.int32)
+    k2 = torch.randint(-2, 1, (n,), generator=g, dtype=torch.int64).to(torch.int8)
+    v = torch.randint(-10**6, 10**6, (n,), generator=g, dtype=torch.int64)
+    aggs = [(eiger.SUM, 0), (eiger.COUNT, 0), (eiger.MIN, 0), (eiger.MAX, 0)]
+    run_all_variants(datagen.Dataset("mk-tiny", n, [k0, k1, k2], [v], aggs))          # mixed widths: generic loads
+    run_all_variants(datagen.Dataset("mk-tiny32", n, [k0, k1], [v], [(eiger.SUM, 0), (eiger.COUNT, 0)]))   # all int32: 32-bit fusion
+    if n:
+        st = eiger.profile_keys([k0.to(DEV), k1.to(DEV), k2.to(DEV)])
+        assert [(s.min, s.max) for s in st] == [(int(k.min()), int(k.max())) for k in (k0, k1, k2)]
