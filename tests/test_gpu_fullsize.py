@@ -40,7 +40,8 @@ def _check_sampled_groups(ds, res, n_samples):
             assert res.aggs[cnt_j[0]][pos].item() == idx.numel()
 
 
-@pytest.mark.parametrize("name,n_samples", [("C2", 2), ("C3", 6), ("C4", 8), ("C5:12", 4), ("C5:24:scattered", 8)])
+@pytest.mark.parametrize("name,n_samples", [("C2", 2), ("C3", 6), ("C4", 8), ("C5:12", 4), ("C5:24:scattered", 8),
+                                            ("MK:4:2", 4), ("MK:3:4", 4), ("MK:4:6", 6)])
 def test_full_size_sampled_groups(name, n_samples):
     torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
@@ -52,6 +53,9 @@ def test_full_size_sampled_groups(name, n_samples):
         ds = datagen.config3(DEV)
     elif name == "C4":
         ds = datagen.config4(DEV)
+    elif name.startswith("MK"):
+        parts = name.split(":")                      # multi-key, 2^28 rows
+        ds = datagen.config_mk(DEV, nk=int(parts[1]), digit_bits=int(parts[2]))
     else:
         parts = name.split(":")
         ds = datagen.config5(DEV, ndv=1 << int(parts[1]), scattered=len(parts) > 2)
