@@ -188,6 +188,24 @@ int64_t eiger_launch_count(void);
 void eiger_set_kernel_timing(int32_t enabled);
 double eiger_kernel_time_ms(int32_t which, int32_t reset, int64_t* launches);
 
+/* eiger_probe — machine probes: measures one building-block rate on the current device, the
+ * numbers the selector's thresholds rest on (the paper's crossovers are "platform-dependent",
+ * PAPER.md:304-306).  Not on the hot path.  `name`:
+ *   "read_ldg"  / "read_bulk"   streamed read of param MiB (default 4096) with 16-byte loads / with
+ *                               cp.async.bulk into a 4-stage shared-memory ring of param2-byte chunks -> GB/s
+ *   "dsmem_red" / "dsmem_atom" / "dsmem_cas" / "dsmem_st"
+ *                               rows/s of random updates of a table spread over the shared memory of a
+ *                               thread-block cluster of param CTAs (1 = plain shared memory), param2 slots
+ *                               per CTA: 2 non-returning adds / 1 returning add + 1 add + carry /
+ *                               look-up + compare-and-swap / one 8-byte store per row -> G rows/s
+ *   "dsmem_bulk"                cp.async.bulk shared -> remote shared, cluster of param CTAs, param2 bytes -> GB/s
+ *   "store_bulk" / "store_warp" param-byte chunks to random aligned places in param2 MiB: cp.async.bulk
+ *                               from shared memory / one warp-wide store -> GB/s
+ *   "l2_red"                    two 64-bit global reductions per row on 2^param 16-byte cells -> G rows/s
+ *   "release"                   frees the probe's scratch memory
+ * result HOST.  Errors: EIGER_ERR_ARG (unknown name), EIGER_ERR_CUDA. */
+int eiger_probe(const char* name, int64_t param, int64_t param2, double* result, void* stream);
+
 const char* eiger_strerror(int code);
 const char* eiger_last_cuda_error(void);
 const char* eiger_variant_name(int32_t variant);

@@ -33,7 +33,7 @@ EXPORTS = [
     "eiger_profile", "eiger_profile_keys", "eiger_hll_registers", "eiger_hll_estimate_host", "eiger_groupby",
     "eiger_groupby_workspace_bytes", "eiger_select_variant", "eiger_groupby_host",
     "eiger_launch_count", "eiger_last_partition_levels", "eiger_last_ndv_estimate", "eiger_last_partition_prehist", "eiger_last_partition_key_bytes", "eiger_set_kernel_timing", "eiger_kernel_time_ms", "eiger_strerror",
-    "eiger_last_cuda_error", "eiger_variant_name", "eiger_shutdown",
+    "eiger_last_cuda_error", "eiger_variant_name", "eiger_shutdown", "eiger_probe",
 ]
 
 _DTYPES = {torch.int8: I8, torch.int32: I32, torch.int64: I64, torch.float64: F64}
@@ -127,6 +127,8 @@ def lib() -> ctypes.CDLL:
         L.eiger_variant_name.restype = ctypes.c_char_p
         L.eiger_variant_name.argtypes = [i32]
         L.eiger_shutdown.restype = None
+        L.eiger_probe.restype = ctypes.c_int
+        L.eiger_probe.argtypes = [ctypes.c_char_p, i64, i64, ctypes.POINTER(ctypes.c_double), vp]
         _lib = L
     return _lib
 
@@ -418,6 +420,14 @@ def kernel_time_ms(which: int = 0, reset: bool = True):
     n = ctypes.c_int64(0)
     ms = lib().eiger_kernel_time_ms(which, 1 if reset else 0, ctypes.byref(n))
     return float(ms), int(n.value)
+
+
+def probe(name: str, param: int = 0, param2: int = 0) -> float:
+    """eiger_probe: one measured building-block rate of the current device (see include/eiger.h)."""
+    r = ctypes.c_double(0.0)
+    _check(lib().eiger_probe(name.encode(), int(param), int(param2), ctypes.byref(r),
+                             _stream(torch.device("cuda", torch.cuda.current_device()))))
+    return float(r.value)
 
 
 def shutdown() -> None:
