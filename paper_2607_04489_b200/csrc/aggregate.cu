@@ -104,7 +104,7 @@ struct AggCtx {
   // (ncu: short_scoreboard was 28 % of the stall samples with one row at a time)
   template <int R>
   __device__ __forceinline__ void rows_sc(const U (&u)[R], const uint64_t (&raw)[R][NV]) {
-    static_assert(SIG == SIG_SC && FRONT == FRONT_SDIRECT, "SUM + COUNT signature only");
+    static_assert((SIG == SIG_SC || SIG == SIG_SC32) && FRONT == FRONT_SDIRECT, "SUM + COUNT signature only");
     uint32_t* lo = reinterpret_cast<uint32_t*>(rep_base);
     uint32_t* cnt = reinterpret_cast<uint32_t*>(rep_base + (size_t)8 * a.front_slots);
     if (a.spec) {
@@ -203,11 +203,10 @@ aggregate_kernel(const __grid_constant__ AggArgs a) {
 #pragma unroll
       for (int c = 0; c < NV; ++c) {
         if (!Sig<SIG>::kStatic && c >= n_vals) { raw[s][0][c] = 0; raw[s][1][c] = 0; continue; }
-        const uint4 v = ldg_stream_16(static_cast<const uint64_t*>(a.plan.vals[c]) + r0 + s * kStep);
-        raw[s][0][c] = ((uint64_t)v.y << 32) | v.x; raw[s][1][c] = ((uint64_t)v.w << 32) | v.z;
+        global_val2(a.plan, c, sig_vw<SIG>(a.plan, c), r0 + s * kStep, raw[s][0][c], raw[s][1][c]);
       }
     }
-    if constexpr (SIG == SIG_SC && FRONT == FRONT_SDIRECT) {
+    if constexpr ((SIG == SIG_SC || SIG == SIG_SC32) && FRONT == FRONT_SDIRECT) {
       U uu[2 * UNR]; uint64_t rr[2 * UNR][NV];
 #pragma unroll
       for (int s = 0; s < UNR; ++s) { uu[2 * s] = u[s][0]; uu[2 * s + 1] = u[s][1]; rr[2 * s][0] = raw[s][0][0]; rr[2 * s + 1][0] = raw[s][1][0]; }
@@ -221,7 +220,7 @@ aggregate_kernel(const __grid_constant__ AggArgs a) {
   for (int64_t i = n_tiles * kTile + (int64_t)blockIdx.x * kAggThreads + tid; i < a.n; i += (int64_t)gridDim.x * kAggThreads) {
     uint64_t raw[NV];
 #pragma unroll
-    for (int c = 0; c < NV; ++c) raw[c] = (Sig<SIG>::kStatic || c < n_vals) ? ldg_stream_u64(static_cast<const uint64_t*>(a.plan.vals[c]) + i) : 0ull;
+    for (int c = 0; c < NV; ++c) raw[c] = (Sig<SIG>::kStatic || c < n_vals) ? global_val(a.plan, c, sig_vw<SIG>(a.plan, c), i) : 0ull;
     ctx.row(load_u<KK>(a.key, i), raw);
   }
   ctx.front_flush();
@@ -331,6 +330,7 @@ int launch_sig(const AggLaunch& L, cudaStream_t s) {
     case SIG_A4I: return launch_fb<KK, SIG_A4I>(L, s);
     case SIG_A4F: return launch_fb<KK, SIG_A4F>(L, s);
     case SIG_S4C: return launch_fb<KK, SIG_S4C>(L, s);
+    case SIG_SC32: return launch_fb<KK, SIG_SC32>(L, s);
     default: return EIGER_ERR_ARG;
   }
 }

@@ -74,9 +74,11 @@ struct Tunables {
   size_t sdirect_bytes = 160 * 1024;  // FRONT_SDIRECT: largest per-CTA direct array
   size_t sdirect_replica_budget;
   int sdirect_max_replicas, sdirect_wide;
-  size_t smem_table_bytes;            // EIGER_SMEM / EIGER_GLOBAL: shared-memory table of one CTA (1 CTA per SM)
+  size_t smem_total;                  // dynamic shared memory of one hash-aggregation CTA: ring + table (1 CTA per SM)
+  int stages;                         // stages of the shared-memory ring the rows stream through (ring.cuh)
+  size_t smem_table_bytes;            // EIGER_SMEM / EIGER_GLOBAL: shared-memory table of one CTA; 0 = what the ring leaves of smem_total
   int smem_threads;
-  size_t part_table_bytes;            // EIGER_PARTITION: shared-memory table of one CTA
+  size_t part_table_bytes;            // EIGER_PARTITION: the same for the per-partition tables
   int part_threads;
   int part_min_bits;                  // at least this many partitions (parallelism of the emit pass)
   size_t direct_l2_bytes;             // AUTO takes DIRECT with global atomics up to this table size
@@ -100,12 +102,14 @@ struct Tunables {
     priv_smem = (size_t)env("EIGER_PRIV_KB", 96) << 10;
     fused_sketch_min_range = env("EIGER_FUSED_SKETCH_MIN_RANGE", 4194304.0);   // beyond any direct-index array AUTO would take
     priv_max_range = (int)env("EIGER_PRIV_MAX_RANGE", 6);
-    smem_table_bytes = (size_t)env("EIGER_SMEM_KB", 200) << 10;
+    smem_total = (size_t)env("EIGER_SMEM_TOTAL_KB", 225) << 10;
+    stages = (int)env("EIGER_STAGES", kDefaultStages);
+    smem_table_bytes = (size_t)env("EIGER_SMEM_KB", 0) << 10;
     sdirect_replica_budget = (size_t)env("EIGER_SDIRECT_REPLICA_KB", 64) << 10;
     sdirect_max_replicas = (int)env("EIGER_SDIRECT_MAX_REPLICAS", 8);
     sdirect_wide = (int)env("EIGER_SDIRECT_WIDE", 1);
     smem_threads = (int)env("EIGER_SMEM_THREADS", 1024);
-    part_table_bytes = (size_t)env("EIGER_PART_KB", 200) << 10;
+    part_table_bytes = (size_t)env("EIGER_PART_KB", 0) << 10;
     part_threads = (int)env("EIGER_PART_THREADS", 1024);
     part_min_bits = (int)env("EIGER_PART_MIN_BITS", 7);
     direct_l2_bytes = (size_t)env("EIGER_DIRECT_L2_MB", 48) << 20;
@@ -142,7 +146,10 @@ struct QueryPlan {
   uint32_t slots = 0, limit = 0;
   int threads = 0;
   int bits1 = 0, bits2 = 0;
-  size_t smem_bytes = 0;
+  size_t smem_bytes = 0;        // direct variants: the CTA's array; hash variants: the CTA's table
+  size_t smem_dyn = 0;          // hash variants: ring + table
+  int stages = 0;
+  bool hot_reserved = false;
   uint64_t cap = 0, cap_bound = 0, cap_hot = 0;
   uint32_t stride = 0;
   size_t table_bytes = 0, part_bytes = 0, total_bytes = 0;
@@ -156,6 +163,9 @@ uint64_t range_of(const eiger_stats& s) {   // max - min + 1, 0 when it is 2^64
 int detect_sig(const AggPlan& p, int n_user) {
   auto is = [&](int j, int op, int col, int f) { return p.op[j] == op && (op == EIGER_COUNT || (p.col[j] == col && p.f64[j] == f)); };
   if (p.n_acc != n_user) return SIG_GENERIC;
+  bool any32 = false;
+  for (int c = 0; c < p.n_vals; ++c) any32 = any32 || p.vw[c] == 4;
+  if (any32) return (n_user == 2 && p.n_vals == 1 && is(0, EIGER_SUM, 0, 0) && is(1, EIGER_COUNT, 0, 0)) ? SIG_SC32 : SIG_GENERIC;
   if (n_user == 2 && is(0, EIGER_SUM, 0, 0) && is(1, EIGER_COUNT, 0, 0)) return SIG_SC;
   if (n_user == 4 && is(1, EIGER_COUNT, 0, 0)) {
     if (is(0, EIGER_SUM, 0, 0) && is(2, EIGER_MIN, 0, 0) && is(3, EIGER_MAX, 0, 0)) return SIG_A4I;
@@ -173,7 +183,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   if (nv > 0 && !vals) return EIGER_ERR_ARG;
   if (force < EIGER_AUTO || force > EIGER_PARTITION) return EIGER_ERR_ARG;
   for (int k = 0; k < nk; ++k) if (!is_key_dtype(keys[k].dtype)) return EIGER_ERR_ARG;
-  for (int c = 0; c < nv; ++c) if (vals[c].dtype != EIGER_I64 && vals[c].dtype != EIGER_F64) return EIGER_ERR_ARG;
+  for (int c = 0; c < nv; ++c) if (vals[c].dtype != EIGER_I64 && vals[c].dtype != EIGER_F64 && vals[c].dtype != EIGER_I32) return EIGER_ERR_ARG;
 
   // aggregates -> accumulator plan over the value columns that are actually used
   AggPlan& p = q->plan;
@@ -189,7 +199,11 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
     if (op == EIGER_COUNT) { if (!has_count) p.cnt_acc = j; has_count = true; continue; }
     const int c = aggs[j].val_col;
     if (c < 0 || c >= nv) return EIGER_ERR_ARG;
-    if (slot_of[c] < 0) { slot_of[c] = p.n_vals; q->val_src[p.n_vals] = c; p.vals[p.n_vals] = vals[c].data; ++p.n_vals; }
+    if (slot_of[c] < 0) {
+      slot_of[c] = p.n_vals; q->val_src[p.n_vals] = c; p.vals[p.n_vals] = vals[c].data;
+      p.vw[p.n_vals] = vals[c].dtype == EIGER_I32 ? 4 : 8;      // int32 payloads are widened on the fly
+      ++p.n_vals;
+    }
     p.col[j] = (uint8_t)slot_of[c];
     p.f64[j] = vals[c].dtype == EIGER_F64;
   }
@@ -254,8 +268,18 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   // partition source kind: a fused key whose domain fits 32 bits is partitioned and aggregated as 32-bit keys
   const int hkp = (hk == KK_GEN && (kd.flags & kKey32)) ? KK_GEN32 : hk;
   const size_t slot_bytes = hash_agg_slot_bytes(p, hk), part_slot_bytes = hash_agg_slot_bytes(p, hkp);
-  const uint32_t smem_slots = (uint32_t)std::max<size_t>(64, (T.smem_table_bytes - 64) / slot_bytes) & ~7u;   // planes stay 8-byte aligned
-  const uint32_t part_slots = (uint32_t)std::max<size_t>(64, (T.part_table_bytes - 64) / part_slot_bytes) & ~7u;
+  // the table gets what the ring (and, for EIGER_GLOBAL, the heavy-hitter cells) leaves of the CTA's shared memory
+  const int pre_kind = (hkp == KK_I32 || hkp == KK_GEN32) ? KK_U32PRE : KK_U64PRE;
+  auto table_bytes_for = [&](int kind, int threads, bool hot, size_t fixed) {
+    if (fixed) return fixed;
+    const HashAggSmem lay = hash_agg_smem_layout(kd, p, kind, threads, hot, T.stages);
+    return T.smem_total > lay.table_off + 4096 ? T.smem_total - lay.table_off : (size_t)4096;
+  };
+  const bool want_hot = force == EIGER_GLOBAL || (force == EIGER_AUTO && skewed);
+  const size_t smem_tab = table_bytes_for(hk, T.smem_threads, want_hot, T.smem_table_bytes);
+  const size_t part_tab = table_bytes_for(pre_kind, T.part_threads, false, T.part_table_bytes);
+  const uint32_t smem_slots = (uint32_t)std::max<size_t>(64, (smem_tab - 64) / slot_bytes) & ~7u;   // planes stay 8-byte aligned
+  const uint32_t part_slots = (uint32_t)std::max<size_t>(64, (part_tab - 64) / part_slot_bytes) & ~7u;
   const uint32_t hash_stride = [&] { uint32_t s = 16; while (s < 8u * (1 + na)) s *= 2; return s; }();
   auto hash_cap = [&](double g) { return (uint64_t)std::max(1024.0, std::ceil(g * (1.0 + 4 * kSigma) * 1.02 / T.load)); };
 
@@ -328,6 +352,8 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
       q->cap = std::min(hash_cap(ndv), q->cap_bound);
     }
     q->smem_bytes = align_up((size_t)q->slots * (variant == EIGER_PARTITION ? part_slot_bytes : slot_bytes) + 64, 16);
+    q->stages = T.stages; q->hot_reserved = variant != EIGER_PARTITION && want_hot;
+    q->smem_dyn = q->smem_bytes + hash_agg_smem_layout(kd, p, variant == EIGER_PARTITION ? pre_kind : hk, q->threads, q->hot_reserved, T.stages).table_off;
     q->table_bytes = align_up((size_t)(q->cap + 1) * q->stride, 256);
   }
   q->total_bytes = q->table_bytes + q->part_bytes + 256;
@@ -463,14 +489,14 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       H.key = q.key; H.plan = q.plan; H.n = n; H.key_kind = src_kind; H.sig = q.sig;
       H.slots = q.slots; H.limit = q.limit; H.spec = spec;
       H.max_probes = q.variant == EIGER_GLOBAL ? T_front_probes : 0;
-      H.n_hot = (!spec && nk == 1 && q.variant != EIGER_PARTITION) ? hot_n : 0;
+      H.n_hot = (!spec && nk == 1 && q.variant != EIGER_PARTITION && q.hot_reserved) ? hot_n : 0;
       for (int i = 0; i < H.n_hot; ++i) H.hot[i] = (uint64_t)hot_key[i] - q.key.base[0];
       if (H.n_hot && src_kind == KK_I32) for (int i = 0; i < H.n_hot; ++i) H.hot[i] &= 0xFFFFFFFFull;
       H.table = table; H.cap = q.cap; H.stride = q.stride; H.call = rt->call;
       for (int k = 0; k < kMaxKeyCols; ++k) H.out_keys[k] = k < nk ? out_keys[k] : nullptr;
       for (int j = 0; j < na; ++j) H.out_aggs[j] = out_aggs[j];
       H.n_out_aggs = na; H.out_capacity = out_capacity;
-      H.threads = q.threads; H.smem_bytes = q.smem_bytes;
+      H.threads = q.threads; H.table_smem_bytes = q.smem_bytes; H.stages = q.stages; H.hot_reserved = q.hot_reserved;
       {   // 32-bit keys in a nearly empty shared-memory table: 8-byte buckets (hashagg.cuh: BK)
         const double per_table = q.variant == EIGER_PARTITION ? q.ndv / (double)((size_t)1 << (q.bits1 + q.bits2)) : q.ndv;
         H.bucket_keys = ((src_kind == KK_I32 || src_kind == KK_GEN32) && q.variant != EIGER_GLOBAL && per_table <= tun().narrow_load * q.slots) ? 2 : 0;
@@ -490,14 +516,14 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         P.off1 = reinterpret_cast<unsigned long long*>(take((P1 + 1) * 8));
         P.cur1 = reinterpret_cast<unsigned long long*>(take(P1 * 8));
         P.keysA = take(kcol);
-        for (int c = 0; c < q.plan.n_vals; ++c) P.valsA[c] = reinterpret_cast<uint64_t*>(take(col));
+        for (int c = 0; c < q.plan.n_vals; ++c) P.valsA[c] = take(col);
         if (q.bits2 > 0) {
           P.off2 = reinterpret_cast<unsigned long long*>(take((PP + 1) * 8));
           P.cur2 = reinterpret_cast<unsigned long long*>(take(PP * 8));
           P.keysB = take(kcol);
-          for (int c = 0; c < q.plan.n_vals; ++c) P.valsB[c] = reinterpret_cast<uint64_t*>(take(col));
+          for (int c = 0; c < q.plan.n_vals; ++c) P.valsB[c] = take(col);
         }
-        { Timed t(s, 2); rc = launch_partition(P, rt->sm_count, s); if (rc) return rc; }
+        { Timed t(s, 2); rc = launch_partition(P, rt->sm_count, rt->smem_optin, s); if (rc) return rc; }
         g_last_levels = q.bits2 > 0 ? 2 : 1;
         g_last_prehist = q.pre_hist ? 1 : 0;
         g_last_part_key_bytes = (int)kb;
@@ -506,7 +532,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         for (int c = 0; c < q.plan.n_vals; ++c) H.plan.vals[c] = P.out_vals[c];
         H.key_kind = (src_kind == KK_I32 || src_kind == KK_GEN32) ? KK_U32PRE : KK_U64PRE;
         H.part_off = P.out_off; H.item_off = P.item_off; H.item_part = P.item_part; H.n_parts = P.n_parts;
-        const int occ = (int)std::max<size_t>(1, std::min<size_t>((size_t)(2048 / q.threads), (rt->smem_optin + 1024) / (q.smem_bytes + 1024)));
+        const int occ = (int)std::max<size_t>(1, std::min<size_t>((size_t)(2048 / q.threads), (rt->smem_optin + 1024) / (q.smem_dyn + 1024)));
         H.blocks = (int)std::min<int64_t>((int64_t)rt->sm_count * occ, (int64_t)P.n_parts + n / P.chunk_rows);
       } else {
         const int64_t tiles = std::max<int64_t>(1, n / (4 * (int64_t)q.threads));

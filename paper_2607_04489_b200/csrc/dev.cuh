@@ -46,7 +46,8 @@ enum SigKind : int {
   SIG_SC = 1,    // SUM(int64 c0), COUNT                        (C4, C5)
   SIG_A4I = 2,   // SUM, COUNT, MIN, MAX of int64 c0            (C1)
   SIG_A4F = 3,   // SUM, COUNT, MIN, MAX of fp64  c0            (C3)
-  SIG_S4C = 4    // SUM(int64 c0..c3), COUNT                    (C2)
+  SIG_S4C = 4,   // SUM(int64 c0..c3), COUNT                    (C2)
+  SIG_SC32 = 5   // SUM(int32 c0), COUNT: the paper's 4-byte payloads
 };
 
 struct AggPlan {
@@ -56,6 +57,7 @@ struct AggPlan {
   uint8_t op[12];
   uint8_t f64[12];
   uint8_t col[12];
+  uint8_t vw[kMaxVals];     // bytes per element of value column c: 8, or 4 for EIGER_I32 (sign-extended into the 64-bit accumulators)
   int32_t cnt_acc;          // index of an accumulator that counts rows (presence test)
 };
 
@@ -66,6 +68,7 @@ template <> struct Sig<SIG_GENERIC> {
   __device__ static constexpr int op(int) { return 0; }
   __device__ static constexpr int col(int) { return 0; }
   __device__ static constexpr bool f64(int) { return false; }
+  __device__ static constexpr int vwidth(int) { return 8; }
 };
 template <> struct Sig<SIG_SC> {
   static constexpr bool kStatic = true;
@@ -73,6 +76,7 @@ template <> struct Sig<SIG_SC> {
   __device__ static constexpr int op(int j) { return j == 0 ? EIGER_SUM : EIGER_COUNT; }
   __device__ static constexpr int col(int) { return 0; }
   __device__ static constexpr bool f64(int) { return false; }
+  __device__ static constexpr int vwidth(int) { return 8; }
 };
 template <> struct Sig<SIG_A4I> {
   static constexpr bool kStatic = true;
@@ -80,6 +84,7 @@ template <> struct Sig<SIG_A4I> {
   __device__ static constexpr int op(int j) { return j; }
   __device__ static constexpr int col(int) { return 0; }
   __device__ static constexpr bool f64(int) { return false; }
+  __device__ static constexpr int vwidth(int) { return 8; }
 };
 template <> struct Sig<SIG_A4F> {
   static constexpr bool kStatic = true;
@@ -87,6 +92,15 @@ template <> struct Sig<SIG_A4F> {
   __device__ static constexpr int op(int j) { return j; }
   __device__ static constexpr int col(int) { return 0; }
   __device__ static constexpr bool f64(int j) { return j != 1; }
+  __device__ static constexpr int vwidth(int) { return 8; }
+};
+template <> struct Sig<SIG_SC32> {
+  static constexpr bool kStatic = true;
+  static constexpr int kAcc = 2, kVals = 1;
+  __device__ static constexpr int op(int j) { return j == 0 ? EIGER_SUM : EIGER_COUNT; }
+  __device__ static constexpr int col(int) { return 0; }
+  __device__ static constexpr bool f64(int) { return false; }
+  __device__ static constexpr int vwidth(int) { return 4; }
 };
 template <> struct Sig<SIG_S4C> {
   static constexpr bool kStatic = true;
@@ -94,6 +108,7 @@ template <> struct Sig<SIG_S4C> {
   __device__ static constexpr int op(int j) { return j < 4 ? EIGER_SUM : EIGER_COUNT; }
   __device__ static constexpr int col(int j) { return j < 4 ? j : 0; }
   __device__ static constexpr bool f64(int) { return false; }
+  __device__ static constexpr int vwidth(int) { return 8; }
 };
 
 // ---- streamed loads: read once, keep out of L1, first to leave L2 ----------------

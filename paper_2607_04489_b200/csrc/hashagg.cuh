@@ -22,6 +22,7 @@
 #include <type_traits>
 
 #include "internal.h"
+#include "ring.cuh"
 #include "rows.cuh"
 
 namespace eiger {
@@ -46,6 +47,11 @@ struct HashAggArgs {
   void* table; uint64_t cap; uint32_t stride;   // global table
   CallDev* call;
   void* out_keys[kMaxKeyCols]; uint64_t* out_aggs[kMaxAggs]; int32_t n_out; int64_t out_capacity;
+  // shared-memory ring (ring.cuh) and the layout of dynamic shared memory
+  int32_t stages; uint32_t stage_bytes; int32_t n_src;
+  uint32_t koff[kMaxKeyCols], voff[kMaxVals];   // byte offset of each column inside a stage
+  uint8_t kw[kMaxKeyCols], vw[kMaxVals];        // bytes per element
+  uint32_t hot_off, table_off;
 };
 
 template <int KK> struct IsPre { static constexpr bool v = (KK == KK_U32PRE || KK == KK_U64PRE); };
@@ -69,6 +75,7 @@ struct Front {
   const int n_acc;
   const uint32_t Sn;      // slots in use (<= a.slots)
   U* skeys;
+  uint32_t* s_spill = nullptr;   // partition mode: set when a row of this work item went to the global table
 
   __device__ Front(const HashAggArgs& args, unsigned char* sm, uint32_t slots_used)
       : a(args), smem(sm), n_acc(S::kStatic ? S::kAcc : args.plan.n_acc), Sn(slots_used) {
@@ -367,6 +374,11 @@ struct Front {
     if (__any_sync(0xffffffffu, miss != 0)) {
       if (a.spec) { missed = missed || miss != 0; }
       else {
+        // A key may now live in BOTH tables: a lane that found the table closed sends its row to the
+        // global table while another lane, which passed the limit check a moment earlier, inserts the
+        // same key here.  The work item therefore no longer owns its keys exclusively and must merge
+        // (not emit) at the end.
+        if (s_spill && miss) *reinterpret_cast<volatile uint32_t*>(s_spill) = 1u;
 #pragma unroll 1
         for (int k = 0; k < R; ++k) {
           U uu = u[0]; uint64_t rr[NV];
@@ -470,95 +482,138 @@ struct Front {
   }
 };
 
+// ---- rows out of the shared-memory ring (ring.cuh) ---------------------------------------------
+// A stage holds `chunk` = 2 x blockDim rows column by column: key column c at koff[c] (kw[c] bytes per
+// element), value column c at voff[c] (vw[c] bytes per element: int32 values are sign-extended to the
+// 64-bit accumulators, "4-byte data types (I32)").
+__device__ __forceinline__ uint64_t ring_elem(const unsigned char* col, int w, int r) {
+  if (w == 8) return *reinterpret_cast<const uint64_t*>(col + 8 * (size_t)r);
+  if (w == 4) return (uint64_t)(int64_t)*reinterpret_cast<const int32_t*>(col + 4 * (size_t)r);
+  return (uint64_t)(int64_t)*reinterpret_cast<const int8_t*>(col + r);
+}
+template <int KK>
+__device__ __forceinline__ typename KeyTraits<KK>::U ring_key(const HashAggArgs& a, const unsigned char* st, int r) {
+  using U = typename KeyTraits<KK>::U;
+  if constexpr (KK == KK_I32) return *reinterpret_cast<const uint32_t*>(st + a.koff[0] + 4 * (size_t)r) - (uint32_t)a.key.base[0];
+  else if constexpr (KK == KK_U32PRE) return *reinterpret_cast<const uint32_t*>(st + a.koff[0] + 4 * (size_t)r);
+  else if constexpr (KK == KK_I64) return *reinterpret_cast<const uint64_t*>(st + a.koff[0] + 8 * (size_t)r) - a.key.base[0];
+  else if constexpr (KK == KK_U64PRE) return *reinterpret_cast<const uint64_t*>(st + a.koff[0] + 8 * (size_t)r);
+  else {
+    uint64_t d[kMaxKeyCols];
+#pragma unroll
+    for (int c = 0; c < kMaxKeyCols; ++c) d[c] = c < a.key.ncols ? ring_elem(st + a.koff[c], a.kw[c], r) - a.key.base[c] : 0ull;
+    return (U)fuse_cols(a.key, d);
+  }
+}
+template <int SIG, int NV>
+__device__ __forceinline__ void ring_vals(const HashAggArgs& a, const unsigned char* st, int r, int n_vals, uint64_t (&raw)[NV]) {
+#pragma unroll
+  for (int c = 0; c < NV; ++c) {
+    if constexpr (Sig<SIG>::kStatic) raw[c] = ring_elem(st + a.voff[c], Sig<SIG>::vwidth(c), r);
+    else raw[c] = c < n_vals ? ring_elem(st + a.voff[c], a.vw[c], r) : 0ull;
+  }
+}
+// One elected thread keeps the ring full: rows [row0, row0 + rows) of every column go into stage
+// g % stages with one bulk copy per column (row0 a multiple of 32, rows a multiple of 32: every
+// copy starts 16-byte aligned and is a multiple of 16 bytes long, whatever the column width).
+__device__ __forceinline__ void ring_issue(const HashAggArgs& a, unsigned char* ring, uint64_t* full, uint64_t* empty,
+                                           uint32_t g, int64_t row0, uint32_t rows, uint64_t policy) {
+  const uint32_t s = g % (uint32_t)a.stages;
+  if (g >= (uint32_t)a.stages) mbar_wait(&empty[s], ((g / (uint32_t)a.stages) - 1u) & 1u);
+  unsigned char* st = ring + (size_t)s * a.stage_bytes;
+  uint32_t bytes = 0;
+  for (int c = 0; c < a.n_src; ++c) bytes += rows * a.kw[c];
+  for (int c = 0; c < a.plan.n_vals; ++c) bytes += rows * a.vw[c];
+  mbar_expect_tx(&full[s], bytes);
+  for (int c = 0; c < a.n_src; ++c)
+    bulk_g2s_hint(st + a.koff[c], static_cast<const unsigned char*>(a.key.ptr[c]) + row0 * a.kw[c], rows * a.kw[c], &full[s], policy);
+  for (int c = 0; c < a.plan.n_vals; ++c)
+    bulk_g2s_hint(st + a.voff[c], static_cast<const unsigned char*>(a.plan.vals[c]) + row0 * a.vw[c], rows * a.vw[c], &full[s], policy);
+}
+
 template <int KK, int SIG, int BK>
 __global__ void __launch_bounds__(kMaxThreads, 1)
 hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
-  extern __shared__ __align__(16) unsigned char smem[];
-  __shared__ uint32_t s_count, s_abort;
+  extern __shared__ __align__(128) unsigned char dyn[];     // [ring stages][heavy-hitter cells][table]
+  __shared__ __align__(8) uint64_t s_full[kMaxStages], s_empty[kMaxStages];
+  __shared__ uint32_t s_count, s_abort, s_spilled;
   __shared__ uint32_t s_wtot[32];
   __shared__ unsigned long long s_base;
   using F = Front<KK, SIG, BK>;
   using U = typename F::U;
   constexpr int NV = F::NV;
-  const int tid = threadIdx.x, T = blockDim.x;
+  const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31;
   const int n_vals = Sig<SIG>::kStatic ? NV : a.plan.n_vals;
+  unsigned char* ring = dyn;
+  unsigned char* smem = dyn + a.table_off;
+  const uint32_t chunk = 2u * (uint32_t)T;                  // rows per stage: two per thread
+  if (tid == 0) {
+    for (int s = 0; s < a.stages; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], (uint32_t)(T >> 5)); }
+    mbar_fence_init();
+  }
+  uint32_t g_cons = 0, g_issued = 0;                        // chunks consumed (all threads) / issued (thread 0)
+  const uint64_t policy = policy_evict_first();             // the rows are read once: first out of L2
 
   if constexpr (!IsPre<KK>::v) {
-    // ---- whole-input mode: tiles of 2 * T * UNR rows, grid-strided; the next tile's loads are
-    // in flight while the current one is processed (one CTA per SM: there is nobody else to
-    // hide HBM latency behind) ----
-    constexpr int UNR = !Sig<SIG>::kStatic ? 1 : (NV >= 4 ? 1 : (sizeof(U) == 8 ? 1 : 2));   // 3 spills at the 64-register cap
+    // ---- whole-input mode: chunk c = blockIdx.x, + gridDim.x, ... of the input ----
     F f(a, smem, a.slots);
-    __shared__ uint64_t s_hot[(kMaxThreads / 32) * kMaxHot * F::NA];
-    __shared__ uint32_t s_hot_rows[(kMaxThreads / 32) * kMaxHot];
+    uint64_t* s_hot = reinterpret_cast<uint64_t*>(dyn + a.hot_off);
+    uint32_t* s_hot_rows = reinterpret_cast<uint32_t*>(s_hot + (kMaxThreads / 32) * kMaxHot * kMaxAcc);
     uint64_t* my_hot = s_hot + (tid >> 5) * kMaxHot * F::NA;
     uint32_t* my_hot_rows = s_hot_rows + (tid >> 5) * kMaxHot;
     if (tid == 0) { s_count = 0; s_abort = 0; }
+    const int64_t n_chunks = a.n / chunk;
+    const int64_t mine = n_chunks > blockIdx.x ? (n_chunks - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    __syncthreads();                                         // barriers initialised
+    if (tid == 0)
+      for (; g_issued < (uint32_t)a.stages && (int64_t)g_issued < mine; ++g_issued)
+        ring_issue(a, ring, s_full, s_empty, g_issued, ((int64_t)blockIdx.x + (int64_t)g_issued * gridDim.x) * chunk, chunk, policy);
     f.init(tid, T);
     if (a.n_hot) f.hot_init(s_hot, s_hot_rows, tid, T);
     __syncthreads();
-    const int64_t step = 2 * (int64_t)T, tile = step * UNR;
-    const int64_t n_tiles = a.n / tile;
     bool missed = false;
-    U u[2][2 * UNR];
-    uint64_t raw[2][2 * UNR][NV];
-    auto load_tile = [&](int b, int64_t t) {
-      const int64_t r0 = t * tile + 2 * tid;
-#pragma unroll
-      for (int s = 0; s < UNR; ++s) {
-        { U uu[2]; load_u2<KK>(a.key, r0 + s * step, uu); u[b][2 * s] = uu[0]; u[b][2 * s + 1] = uu[1]; }
-#pragma unroll
-        for (int c = 0; c < NV; ++c) {
-          if (!Sig<SIG>::kStatic && c >= n_vals) { raw[b][2 * s][c] = 0; raw[b][2 * s + 1][c] = 0; continue; }
-          const uint4 v = ldg_stream_16(static_cast<const uint64_t*>(a.plan.vals[c]) + r0 + s * step);
-          raw[b][2 * s][c] = ((uint64_t)v.y << 32) | v.x; raw[b][2 * s + 1][c] = ((uint64_t)v.w << 32) | v.z;
-        }
-      }
-    };
-    // the tile loop, compiled twice: with and without the heavy-hitter look (runtime row-valid flags
+    // the chunk loop, compiled twice: with and without the heavy-hitter look (runtime row-valid flags
     // and the hot-key scan cost the plain path 5-15 % at low NDV when they were merely branched over)
-    auto run_tiles = [&](auto hot_c) {
+    auto run_chunks = [&](auto hot_c) {
       constexpr bool HOT = decltype(hot_c)::value;
-      auto process_tile = [&](int b) {
-        uint32_t miss = 0;
-        if constexpr (HOT) {
-          bool ab[2 * UNR];
-#pragma unroll
-          for (int r = 0; r < 2 * UNR; ++r) ab[r] = f.hot_absorb(u[b][r], raw[b][r], my_hot, my_hot_rows, tid & 31);
-#pragma unroll
-          for (int s = 0; s < UNR; ++s) miss |= f.pair(u[b][2 * s], raw[b][2 * s], !ab[2 * s], u[b][2 * s + 1], raw[b][2 * s + 1], !ab[2 * s + 1], &s_count) << (2 * s);
-        } else {
-#pragma unroll
-          for (int s = 0; s < UNR; ++s) miss |= f.pair(u[b][2 * s], raw[b][2 * s], true, u[b][2 * s + 1], raw[b][2 * s + 1], true, &s_count) << (2 * s);
-        }
-        f.spill(u[b], raw[b], miss, missed);
-      };
-      int64_t t = blockIdx.x;
-      uint32_t trip = 0;
-      if (t < n_tiles) load_tile(0, t);
-      while (t < n_tiles) {
+      for (int64_t k = 0; k < mine; ++k, ++g_cons) {
         // speculative run: look at the global give-up flag every 16th trip only (an L2 round trip each time)
-        if (a.spec) { if (__any_sync(0xffffffffu, missed || ((trip++ & 15u) == 0u && *reinterpret_cast<volatile uint32_t*>(&a.call->abort)))) break; }
-        if (t + gridDim.x < n_tiles) load_tile(1, t + gridDim.x);
-        process_tile(0);
-        t += gridDim.x;
-        if (t >= n_tiles) break;
-        if (t + gridDim.x < n_tiles) load_tile(0, t + gridDim.x);
-        process_tile(1);
-        t += gridDim.x;
+        if (a.spec) { if (__any_sync(0xffffffffu, missed || ((g_cons & 15u) == 0u && *reinterpret_cast<volatile uint32_t*>(&a.call->abort)))) break; }
+        const uint32_t s = g_cons % (uint32_t)a.stages;
+        mbar_wait(&s_full[s], (g_cons / (uint32_t)a.stages) & 1u);
+        const unsigned char* st = ring + (size_t)s * a.stage_bytes;
+        U u[2]; uint64_t raw[2][NV];
+        u[0] = ring_key<KK>(a, st, tid); u[1] = ring_key<KK>(a, st, T + tid);
+        ring_vals<SIG, NV>(a, st, tid, n_vals, raw[0]); ring_vals<SIG, NV>(a, st, T + tid, n_vals, raw[1]);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&s_empty[s]);             // this warp's rows are in registers: the stage may be refilled
+        if (tid == 0 && (int64_t)g_issued < mine) {
+          ring_issue(a, ring, s_full, s_empty, g_issued, ((int64_t)blockIdx.x + (int64_t)g_issued * gridDim.x) * chunk, chunk, policy);
+          ++g_issued;
+        }
+        uint32_t miss;
+        if constexpr (HOT) {
+          const bool ab0 = f.hot_absorb(u[0], raw[0], my_hot, my_hot_rows, lane);
+          const bool ab1 = f.hot_absorb(u[1], raw[1], my_hot, my_hot_rows, lane);
+          miss = f.pair(u[0], raw[0], !ab0, u[1], raw[1], !ab1, &s_count);
+        } else {
+          miss = f.pair(u[0], raw[0], true, u[1], raw[1], true, &s_count);
+        }
+        f.spill(u, raw, miss, missed);
       }
     };
-    if (a.n_hot) run_tiles(std::true_type{}); else run_tiles(std::false_type{});
+    if (a.n_hot) run_chunks(std::true_type{}); else run_chunks(std::false_type{});
+    // a speculative run that gave up leaves bulk copies in flight: they must land before the CTA ends
+    if (tid == 0) for (uint32_t g = g_cons; g < g_issued; ++g) mbar_wait(&s_full[g % (uint32_t)a.stages], (g / (uint32_t)a.stages) & 1u);
     if (!(a.spec && __any_sync(0xffffffffu, missed))) {
-      // ragged tail: row at a time, spread over the whole grid, warp-uniform trip count
-      const int lane = tid & 31;
-      for (int64_t i0 = n_tiles * tile + (int64_t)blockIdx.x * T + (tid - lane); i0 < a.n; i0 += (int64_t)gridDim.x * T) {
+      // ragged tail (fewer than `chunk` rows): row at a time, spread over the whole grid, warp-uniform trip count
+      for (int64_t i0 = n_chunks * chunk + (int64_t)blockIdx.x * T + (tid - lane); i0 < a.n; i0 += (int64_t)gridDim.x * T) {
         const int64_t i = i0 + lane;
         uint64_t rawt[NV];
         U ut = 0;
         if (i < a.n) {
 #pragma unroll
-          for (int c = 0; c < NV; ++c) rawt[c] = (Sig<SIG>::kStatic || c < n_vals) ? ldg_stream_u64(static_cast<const uint64_t*>(a.plan.vals[c]) + i) : 0ull;
+          for (int c = 0; c < NV; ++c) rawt[c] = (Sig<SIG>::kStatic || c < n_vals) ? global_val(a.plan, c, sig_vw<SIG>(a.plan, c), i) : 0ull;
           ut = load_u<KK>(a.key, i);
         }
         const uint32_t miss = f.pair(ut, rawt, i < a.n, ut, rawt, false, &s_count);
@@ -578,63 +633,77 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
   } else {
     // ---- partition mode: work items blockIdx.x, + gridDim.x, ...; an item is a whole partition
     // (this CTA then owns its keys and emits them) or a slice of a hot one (merged through the
-    // global table like the whole-input mode) ----
+    // global table like the whole-input mode).  The ring runs ACROSS items: while one item's table
+    // is read out and the next one's initialised, the next item's first rows are already landing. ----
     const unsigned long long n_items = a.item_off[a.n_parts];
-    for (unsigned long long it = blockIdx.x; it < n_items; it += gridDim.x) {
-      // the partition of item `it`: one broadcast load from the map written by part_items_kernel
-      const int p = (int)a.item_part[it];
-      const unsigned long long n_chunks = a.item_off[p + 1] - a.item_off[p], ci = it - a.item_off[p];
+    // rows [r0, r1) of item `it`; A = r0 rounded down to 32 rows (bulk copies start 16-byte aligned in every column)
+    auto item_rows = [&](unsigned long long it, int64_t& r0, int64_t& r1, bool& exclusive) {
+      const int p = (int)a.item_part[it];                    // one broadcast load from the map written by part_items_kernel
+      const unsigned long long n_cuts = a.item_off[p + 1] - a.item_off[p], ci = it - a.item_off[p];
       const int64_t P0 = (int64_t)a.part_off[p], P1 = (int64_t)a.part_off[p + 1];
-      const int64_t per = (P1 - P0 + (int64_t)n_chunks - 1) / (int64_t)n_chunks;
-      const int64_t r0 = P0 + (int64_t)ci * per, r1 = r0 + per < P1 ? r0 + per : P1;
-      const bool exclusive = n_chunks == 1;
+      const int64_t per = (P1 - P0 + (int64_t)n_cuts - 1) / (int64_t)n_cuts;
+      r0 = P0 + (int64_t)ci * per; r1 = r0 + per < P1 ? r0 + per : P1;
+      exclusive = n_cuts == 1;
+    };
+    // producer state lives in shared memory (only thread 0 touches it): kept in registers it cost every
+    // thread of the 64-register kernel a dozen of them
+    __shared__ unsigned long long sp_it;
+    __shared__ long long sp_A, sp_r1;
+    __shared__ uint32_t sp_k, sp_chunks, sp_issued;
+    auto producer_load = [&]() {                             // thread 0: describe item sp_it
+      if (sp_it < n_items) {
+        int64_t r0, r1; bool ex;
+        item_rows(sp_it, r0, r1, ex);
+        sp_A = r0 & ~(int64_t)31; sp_r1 = r1;
+        sp_chunks = r1 > r0 ? (uint32_t)((r1 - sp_A + chunk - 1) / chunk) : 0u;
+      }
+      sp_k = 0;
+    };
+    auto top_up = [&](uint32_t upto) {                       // thread 0: keep `stages` chunks requested ahead of the consumers
+      while (sp_issued < upto && sp_it < n_items) {
+        if (sp_k >= sp_chunks) { sp_it += gridDim.x; producer_load(); continue; }
+        const int64_t row0 = sp_A + (int64_t)sp_k * chunk;
+        const int64_t left = ((sp_r1 - row0) + 31) & ~(int64_t)31;
+        ring_issue(a, ring, s_full, s_empty, sp_issued, row0, (uint32_t)(left < (int64_t)chunk ? left : (int64_t)chunk), policy);
+        ++sp_issued; ++sp_k;
+      }
+    };
+    __syncthreads();                                         // barriers initialised
+    if (tid == 0) { sp_it = blockIdx.x; sp_issued = 0; producer_load(); top_up((uint32_t)a.stages); }
+    for (unsigned long long it = blockIdx.x; it < n_items; it += gridDim.x) {
+      int64_t r0, r1; bool exclusive;
+      item_rows(it, r0, r1, exclusive);
+      const uint32_t lo = (uint32_t)(r0 & 31), hi = (uint32_t)(r1 - (r0 & ~(int64_t)31));   // valid rows of the item, relative to A
+      const uint32_t chunks = r1 > r0 ? (hi + chunk - 1) / chunk : 0u;
       // a table no larger than the partition needs: 2 slots per row is always enough
       const uint64_t want = 2ull * (uint64_t)(r1 - r0) + 64;
       const uint32_t Sn = (uint32_t)(want < a.slots ? want : a.slots) & ~7u;   // whole buckets
       F f(a, smem, Sn);
-      __syncthreads();                       // the previous partition's emit is over
-      if (tid == 0) s_count = 0;
+      f.s_spill = &s_spilled;
+      __syncthreads();                       // the previous item's emit is over
+      if (tid == 0) { s_count = 0; s_spilled = 0; }
       f.init(tid, T);
       __syncthreads();
       bool missed = false;
-      // chunks of UNR * T rows, bounds-checked per row; the next chunk loads while this one is processed
-      constexpr int UNR = NV >= 4 ? 1 : 2;
-      U u[2][UNR];
-      uint64_t raw[2][UNR][NV];
-      const int64_t chunk = (int64_t)UNR * T;
-      auto load_chunk = [&](int b, int64_t c0) {
-#pragma unroll
-        for (int s = 0; s < UNR; ++s) {
-          const int64_t i = c0 + (int64_t)s * T + tid;
-          if (i < r1) {
-            u[b][s] = load_u<KK>(a.key, i);
-#pragma unroll
-            for (int c = 0; c < NV; ++c) raw[b][s][c] = (Sig<SIG>::kStatic || c < n_vals) ? ldg_stream_u64(static_cast<const uint64_t*>(a.plan.vals[c]) + i) : 0ull;
-          }
-        }
-      };
-      auto process_chunk = [&](int b, int64_t c0) {
-        uint32_t miss = 0;
-#pragma unroll
-        for (int s = 0; s < UNR; s += 2) {
-          const bool v0 = c0 + (int64_t)s * T + tid < r1, v1 = (s + 1 < UNR) && (c0 + (int64_t)(s + 1) * T + tid < r1);
-          miss |= f.pair(v0 ? u[b][s] : (U)0, raw[b][s], v0, v1 ? u[b][s + 1 < UNR ? s + 1 : s] : (U)0, raw[b][s + 1 < UNR ? s + 1 : s], v1, &s_count) << s;
-        }
-        f.spill(u[b], raw[b], miss, missed);
-      };
-      int64_t c0 = r0;
-      load_chunk(0, c0);
-      while (c0 < r1) {
-        if (c0 + chunk < r1) load_chunk(1, c0 + chunk);
-        process_chunk(0, c0);
-        c0 += chunk;
-        if (c0 >= r1) break;
-        if (c0 + chunk < r1) load_chunk(0, c0 + chunk);
-        process_chunk(1, c0);
-        c0 += chunk;
+      for (uint32_t k = 0; k < chunks; ++k, ++g_cons) {
+        const uint32_t s = g_cons % (uint32_t)a.stages;
+        mbar_wait(&s_full[s], (g_cons / (uint32_t)a.stages) & 1u);
+        const unsigned char* st = ring + (size_t)s * a.stage_bytes;
+        const uint32_t i0 = k * chunk + (uint32_t)tid, i1 = i0 + (uint32_t)T;
+        const bool v0 = i0 >= lo && i0 < hi, v1 = i1 >= lo && i1 < hi;
+        U u[2]; uint64_t raw[2][NV];
+        u[0] = ring_key<KK>(a, st, tid); u[1] = ring_key<KK>(a, st, T + tid);
+        ring_vals<SIG, NV>(a, st, tid, n_vals, raw[0]); ring_vals<SIG, NV>(a, st, T + tid, n_vals, raw[1]);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&s_empty[s]);
+        if (tid == 0) top_up(g_cons + 1u + (uint32_t)a.stages);
+        const uint32_t miss = f.pair(v0 ? u[0] : (U)0, raw[0], v0, v1 ? u[1] : (U)0, raw[1], v1, &s_count);
+        f.spill(u, raw, miss, missed);
       }
       __syncthreads();
-      if (exclusive) f.flush_emit(tid, T, s_count, &s_base, s_wtot);
+      // emit only what this CTA owns exclusively: a whole partition none of whose rows was sent to
+      // the global table (otherwise a key could be emitted here AND by the compaction pass)
+      if (exclusive && s_spilled == 0u) f.flush_emit(tid, T, s_count, &s_base, s_wtot);
       else f.flush_merge(tid, T);
     }
   }
@@ -643,7 +712,6 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
 template <int KK, int SIG, int BK>
 int launch_one(const HashAggLaunch& L, cudaStream_t s) {
   auto kern = hash_agg_kernel<KK, SIG, BK>;
-  if (L.smem_bytes > 32 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
   HashAggArgs a;
   a.key = L.key; a.plan = L.plan; a.n = L.n; a.part_off = L.part_off; a.item_off = L.item_off; a.item_part = L.item_part; a.n_parts = L.n_parts;
   a.slots = L.slots; a.limit = L.limit; a.spec = L.spec; a.max_probes = L.max_probes > 0 ? L.max_probes : 16;
@@ -653,7 +721,14 @@ int launch_one(const HashAggLaunch& L, cudaStream_t s) {
   for (int k = 0; k < kMaxKeyCols; ++k) a.out_keys[k] = L.out_keys[k];
   for (int j = 0; j < kMaxAggs; ++j) a.out_aggs[j] = static_cast<uint64_t*>(L.out_aggs[j]);
   a.n_out = L.n_out_aggs; a.out_capacity = L.out_capacity;
-  kern<<<L.blocks, L.threads, L.smem_bytes, s>>>(a);
+  // dynamic shared memory: [ring: stages x stage_bytes][heavy-hitter cells][table]
+  const HashAggSmem lay = hash_agg_smem_layout(L.key, L.plan, L.key_kind, L.threads, L.hot_reserved && !IsPre<KK>::v, L.stages);
+  for (int k = 0; k < kMaxKeyCols; ++k) { a.koff[k] = lay.koff[k]; a.kw[k] = lay.kw[k]; }
+  for (int c = 0; c < kMaxVals; ++c) { a.voff[c] = lay.voff[c]; a.vw[c] = lay.vw[c]; }
+  a.stages = lay.stages; a.stage_bytes = lay.stage_bytes; a.n_src = lay.n_src; a.hot_off = lay.hot_off; a.table_off = lay.table_off;
+  const size_t smem = (size_t)lay.table_off + L.table_smem_bytes;
+  if (smem > 32 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  kern<<<L.blocks, L.threads, smem, s>>>(a);
   count_launch();
   EIGER_CUDA(cudaGetLastError());
   return EIGER_OK;
@@ -667,6 +742,7 @@ int launch_sig_bk(const HashAggLaunch& L, cudaStream_t s) {
     case SIG_A4I: return launch_one<KK, SIG_A4I, BK>(L, s);
     case SIG_A4F: return launch_one<KK, SIG_A4F, BK>(L, s);
     case SIG_S4C: return launch_one<KK, SIG_S4C, BK>(L, s);
+    case SIG_SC32: return launch_one<KK, SIG_SC32, BK>(L, s);
     default: return EIGER_ERR_ARG;
   }
 }
@@ -676,6 +752,7 @@ int launch_sig(const HashAggLaunch& L, cudaStream_t s) {
   if constexpr (sizeof(U) == 4) {
     // the narrow-bucket kernels exist for the SUM + COUNT and the generic signature only (compile time)
     if (L.bucket_keys == 2 && L.sig == SIG_SC) return launch_one<KK, SIG_SC, 2>(L, s);
+    if (L.bucket_keys == 2 && L.sig == SIG_SC32) return launch_one<KK, SIG_SC32, 2>(L, s);
     if (L.bucket_keys == 2 && L.sig == SIG_GENERIC) return launch_one<KK, SIG_GENERIC, 2>(L, s);
   }
   return launch_sig_bk<KK, 16 / (int)sizeof(U)>(L, s);

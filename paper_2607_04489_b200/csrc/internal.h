@@ -121,10 +121,22 @@ struct HashAggLaunch {
   CallDev* call;
   void* out_keys[kMaxKeyCols]; void* out_aggs[kMaxAggs]; int n_out_aggs; int64_t out_capacity;   // partition mode emits
   int threads, blocks;
-  size_t smem_bytes;
+  int stages;               // shared-memory ring stages (ring.cuh); 0 = default
+  bool hot_reserved;        // room for the heavy-hitter cells is part of the layout (EIGER_GLOBAL)
+  size_t table_smem_bytes;  // shared-memory table of one CTA
 };
 int launch_hash_agg(const HashAggLaunch& L, cudaStream_t s);
 size_t hash_agg_slot_bytes(const AggPlan& p, int key_kind);   // shared-memory bytes per slot
+// Dynamic shared memory of the hash aggregation kernel: [ring: stages x stage_bytes][heavy-hitter cells][table].
+// A stage holds 2 x threads rows column by column (each column 128-byte aligned).
+struct HashAggSmem {
+  uint32_t koff[kMaxKeyCols], voff[kMaxVals];
+  uint8_t kw[kMaxKeyCols], vw[kMaxVals];
+  int n_src;                // key columns in the ring (1 in partition mode: the pre-fused key)
+  int stages; uint32_t stage_bytes, hot_off, table_off;
+};
+HashAggSmem hash_agg_smem_layout(const KeyDesc& key, const AggPlan& plan, int key_kind, int threads, bool hot, int stages);
+constexpr int kDefaultStages = 3;
 
 // ---- partition.cu ----------------------------------------------------------------------
 struct PartitionLaunch {
@@ -139,16 +151,16 @@ struct PartitionLaunch {
   unsigned long long* cur1; // [2^bits1]
   unsigned long long* off2; // [2^(bits1 + bits2) + 1]   (two levels)
   unsigned long long* cur2; // [2^(bits1 + bits2)]
-  void* keysA; uint64_t* valsA[kMaxVals];   // level-1 output, n rows each
-  void* keysB; uint64_t* valsB[kMaxVals];   // level-2 output
+  void* keysA; void* valsA[kMaxVals];   // level-1 output, n rows each (value columns keep their width)
+  void* keysB; void* valsB[kMaxVals];   // level-2 output
   unsigned long long* item_off;   // [2^(bits1 + bits2) + 1] work items of the aggregation pass
   uint32_t* item_part;            // [2 * 2^(bits1 + bits2) + 2] partition of each work item
   int64_t chunk_rows;       // partitions above 2 * chunk_rows rows are cut into items of chunk_rows
   const uint32_t* pre_hist; // level-1 histogram already taken at fan-out kPreFan with this key base (or nullptr)
   // results
-  const void* out_keys; uint64_t* const* out_vals; const unsigned long long* out_off; int n_parts;
+  const void* out_keys; void* const* out_vals; const unsigned long long* out_off; int n_parts;
 };
-int launch_partition(PartitionLaunch& p, int sm_count, cudaStream_t s);
+int launch_partition(PartitionLaunch& p, int sm_count, size_t smem_optin, cudaStream_t s);
 int partition_max_bits_per_level();
 
 }  // namespace eiger

@@ -11,7 +11,10 @@
 // efficiently; level 2 runs per level-1 partition (blockIdx.y) over the level-1 output.
 #include <algorithm>
 
+#include <cstdlib>
+
 #include "internal.h"
+#include "ring.cuh"
 #include "rows.cuh"
 
 namespace eiger {
@@ -36,8 +39,8 @@ template <int KK> struct SrcKey { using U = typename KeyTraits<KK>::U; };
 
 struct LevelArgs {
   KeyDesc key;                              // source keys (original columns or a partitioned copy)
-  const uint64_t* vals[kMaxVals];
-  uint64_t* out_vals[kMaxVals];
+  const void* vals[kMaxVals];             // value columns, sm.vw[c] bytes per element
+  void* out_vals[kMaxVals];
   void* out_keys;                           // UO[n]
   const unsigned long long* seg_off;        // nullptr: one segment [0, n); else [gridDim.y + 1]
   uint32_t* hist;                           // [segments * fan]
@@ -140,198 +143,290 @@ part_items_kernel(const unsigned long long* __restrict__ off, unsigned long long
   if (tid == 1023) item_off[count] = s_part[1023];
 }
 
-template <int KK, class UO>
-__global__ void __launch_bounds__(kPT, kScatterCtas)
-part_scatter_kernel(const __grid_constant__ LevelArgs a) {
+// ---- scatter ---------------------------------------------------------------------------------
+// The rows of a tile arrive through a shared-memory ring filled by bulk copies (ring.cuh): the read
+// stream does not stop while the CTA ranks, stages and writes (the round-1 kernel, whose threads
+// loaded their own rows, moved 3.4-3.9 TB/s with half of its stall samples on those loads).  A tile
+// is RPT x blockDim rows; each column is staged in partition order in shared memory and leaves
+// the SM as runs of consecutive rows of one partition (measured, eiger_probe("store_warp"): random
+// 256-byte runs are written at 6.0 TB/s, 128-byte runs at 4.4 TB/s).
+struct ScatterSmem {
+  uint32_t koff[kMaxKeyCols], voff[kMaxVals];   // columns inside a ring stage
+  uint8_t kw[kMaxKeyCols], vw[kMaxVals];
+  int n_src;
+  uint32_t stage_bytes, out_off, pid_off, total;
+  int stages;
+};
+struct ScatterArgs {
+  LevelArgs lv;
+  ScatterSmem sm;
+  uint32_t tile;
+};
+
+__device__ __forceinline__ uint64_t stage_elem(const unsigned char* col, int w, uint32_t r) {
+  if (w == 8) return *reinterpret_cast<const uint64_t*>(col + 8 * (size_t)r);
+  if (w == 4) return (uint64_t)(int64_t)*reinterpret_cast<const int32_t*>(col + 4 * (size_t)r);
+  return (uint64_t)(int64_t)*reinterpret_cast<const int8_t*>(col + r);
+}
+template <int KK>
+__device__ __forceinline__ typename KeyTraits<KK>::U stage_key(const KeyDesc& key, const ScatterSmem& sm, const unsigned char* st, uint32_t r) {
+  using U = typename KeyTraits<KK>::U;
+  if constexpr (KK == KK_I32) return *reinterpret_cast<const uint32_t*>(st + sm.koff[0] + 4 * (size_t)r) - (uint32_t)key.base[0];
+  else if constexpr (KK == KK_U32PRE) return *reinterpret_cast<const uint32_t*>(st + sm.koff[0] + 4 * (size_t)r);
+  else if constexpr (KK == KK_I64) return *reinterpret_cast<const uint64_t*>(st + sm.koff[0] + 8 * (size_t)r) - key.base[0];
+  else if constexpr (KK == KK_U64PRE) return *reinterpret_cast<const uint64_t*>(st + sm.koff[0] + 8 * (size_t)r);
+  else {
+    uint64_t d[kMaxKeyCols];
+#pragma unroll
+    for (int c = 0; c < kMaxKeyCols; ++c) d[c] = c < key.ncols ? stage_elem(st + sm.koff[c], sm.kw[c], r) - key.base[c] : 0ull;
+    return (U)fuse_cols(key, d);
+  }
+}
+
+template <int KK, class UO, int RPT>
+__global__ void __launch_bounds__(1024, 1)
+part_scatter_kernel(const __grid_constant__ ScatterArgs A) {
   using U = typename SrcKey<KK>::U;
-  // dynamic shared memory (above the 48 KB static limit): staging buffers, then the counters
-  extern __shared__ __align__(16) unsigned char dsm[];
-  uint64_t* s_val = reinterpret_cast<uint64_t*>(dsm);
-  UO* s_key = reinterpret_cast<UO*>(dsm + sizeof(uint64_t) * kTile);
-  long long* s_delta = reinterpret_cast<long long*>(dsm + (sizeof(uint64_t) + sizeof(UO)) * kTile);
-  uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_delta + kMaxFan);
-  uint32_t* s_loff = s_cnt + kMaxFan;
-  uint16_t* s_pid = reinterpret_cast<uint16_t*>(s_loff + kMaxFan);
-  __shared__ uint32_t s_warp[kPT / 32];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, seg = blockIdx.y;
+  const LevelArgs& a = A.lv;
+  const ScatterSmem& sm = A.sm;
+  extern __shared__ __align__(128) unsigned char dsm[];      // [ring stages][s_out: tile x 8][s_pid: tile x 2]
+  __shared__ __align__(8) uint64_t s_full[kMaxStages], s_empty[kMaxStages];
+  __shared__ long long s_delta[kMaxFan];
+  __shared__ uint32_t s_cnt[kMaxFan], s_loff[kMaxFan];
+  __shared__ uint32_t s_warp[32];
+  unsigned char* s_out = dsm + sm.out_off;
+  uint16_t* s_pid = reinterpret_cast<uint16_t*>(dsm + sm.pid_off);
+  const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5, seg = blockIdx.y;
   const int fan = a.fan;
-  const uint32_t mask = (uint32_t)fan - 1u;
+  const uint32_t mask = (uint32_t)fan - 1u, tile = A.tile;
   const int64_t r0 = a.seg_off ? (int64_t)a.seg_off[seg] : 0, r1 = a.seg_off ? (int64_t)a.seg_off[seg + 1] : a.n;
   unsigned long long* cursor = a.cursor + (size_t)seg * fan;
   UO* out_keys = static_cast<UO*>(a.out_keys);
-  for (int p = tid; p < fan; p += kPT) s_cnt[p] = 0;
+  for (int p = tid; p < fan; p += T) s_cnt[p] = 0;
+  if (tid == 0) {
+    for (int s = 0; s < sm.stages; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], (uint32_t)(T >> 5)); }
+    mbar_fence_init();
+  }
   __syncthreads();
-  const int64_t n_tiles = (r1 - r0 + kTile - 1) / kTile;
-  constexpr int kPer = kMaxFan / kPT;       // counters per thread in the scan (consecutive)
-  for (int64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-    const int64_t base = r0 + t * kTile;
-    const int m = (int)min((int64_t)kTile, r1 - base);
-    // the CTA's next tile is pulled into L2 now: its loads are what this kernel waits for most
-    // (ncu: long_scoreboard 49 % of stall samples with one tile in flight per CTA)
-    {
-      const int64_t nb = base + (int64_t)gridDim.x * kTile;
-      if constexpr (KK != KK_GEN && KK != KK_GEN32) {
-       if (nb < r1 && a.key.ncols == 1) {
-        const int64_t nm = min((int64_t)kTile, r1 - nb);
-        const int64_t kbytes = nm * (int64_t)sizeof(U), vbytes = nm * 8;
-        const char* kp = static_cast<const char*>(a.key.ptr[0]) + nb * (int64_t)sizeof(U);
-        for (int64_t o = (int64_t)tid * 128; o < kbytes; o += (int64_t)kPT * 128) prefetch_l2(kp + o);
-        for (int c = 0; c < a.n_vals; ++c) {
-          const char* vp = reinterpret_cast<const char*>(a.vals[c] + nb);
-          for (int64_t o = (int64_t)tid * 128; o < vbytes; o += (int64_t)kPT * 128) prefetch_l2(vp + o);
-        }
-       }
-      } else if (nb < r1) {
-        // several key columns (level 1 of a fused key): each column at its own width
-        const int64_t nm = min((int64_t)kTile, r1 - nb);
-        for (int kc = 0; kc < a.key.ncols; ++kc) {
-          const int64_t w = a.key.dtype[kc] == EIGER_I8 ? 1 : (a.key.dtype[kc] == EIGER_I32 ? 4 : 8);
-          const char* kp = static_cast<const char*>(a.key.ptr[kc]) + nb * w;
-          for (int64_t o = (int64_t)tid * 128; o < nm * w; o += (int64_t)kPT * 128) prefetch_l2(kp + o);
-        }
-        for (int c = 0; c < a.n_vals; ++c) {
-          const char* vp = reinterpret_cast<const char*>(a.vals[c] + nb);
-          for (int64_t o = (int64_t)tid * 128; o < nm * 8; o += (int64_t)kPT * 128) prefetch_l2(vp + o);
-        }
-      }
-    }
+  // tiles of this segment: tile t covers rows [A0 + t * tile, + tile), A0 = r0 rounded down to 32 rows
+  // (every bulk copy then starts 16-byte aligned); rows outside [r0, r1) are masked.  Only tiles that
+  // end inside the column(s) travel by bulk copy: the last, ragged one of a caller's column is loaded
+  // by the threads (a bulk copy must be a multiple of 16 bytes and may not run past the allocation).
+  const int64_t A0 = r0 & ~(int64_t)31;
+  const int64_t n_tiles = r1 > r0 ? (r1 - A0 + tile - 1) / tile : 0;
+  const bool padded = a.seg_off != nullptr;                  // level 2 reads the library's own padded copy
+  const int64_t n_bulk = padded ? n_tiles : (r1 - A0) / tile;
+  const int64_t mine = n_bulk > blockIdx.x ? (n_bulk - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+  const uint64_t policy = policy_evict_first();
+  uint32_t g_issued = 0;
+  auto issue = [&](uint32_t g) {                             // thread 0
+    const int64_t row0 = A0 + ((int64_t)blockIdx.x + (int64_t)g * gridDim.x) * tile;
+    int64_t rows = ((r1 - row0) + 31) & ~(int64_t)31;
+    if (rows > (int64_t)tile) rows = tile;
+    const uint32_t s = g % (uint32_t)sm.stages;
+    if (g >= (uint32_t)sm.stages) mbar_wait(&s_empty[s], ((g / (uint32_t)sm.stages) - 1u) & 1u);
+    unsigned char* st = dsm + (size_t)s * sm.stage_bytes;
+    uint32_t bytes = 0;
+    for (int c = 0; c < sm.n_src; ++c) bytes += (uint32_t)rows * sm.kw[c];
+    for (int c = 0; c < a.n_vals; ++c) bytes += (uint32_t)rows * sm.vw[c];
+    mbar_expect_tx(&s_full[s], bytes);
+    for (int c = 0; c < sm.n_src; ++c)
+      bulk_g2s_hint(st + sm.koff[c], static_cast<const unsigned char*>(a.key.ptr[c]) + row0 * sm.kw[c], (uint32_t)rows * sm.kw[c], &s_full[s], policy);
+    for (int c = 0; c < a.n_vals; ++c)
+      bulk_g2s_hint(st + sm.voff[c], reinterpret_cast<const unsigned char*>(a.vals[c]) + row0 * sm.vw[c], (uint32_t)rows * sm.vw[c], &s_full[s], policy);
+  };
+  if (tid == 0) for (; g_issued < (uint32_t)sm.stages && (int64_t)g_issued < mine; ++g_issued) issue(g_issued);
+
+  // one tile whose rows sit in stage `st`: rows [row0, row0 + tile) of the segment, valid where in [r0, r1)
+  auto process = [&](const unsigned char* st, int64_t row0, int ring_stage) {
+    const uint32_t lo = (uint32_t)(r0 > row0 ? r0 - row0 : 0), hi = (uint32_t)(r1 - row0 < (int64_t)tile ? r1 - row0 : (int64_t)tile);
     // A: keys -> partition ids and ranks inside the tile
-    U u[kPR];
-    uint32_t pos[kPR];
-    uint64_t v0[kPR];
+    U u[RPT];
+    uint32_t pos[RPT];
 #pragma unroll
-    for (int r = 0; r < kPR; ++r) {
-      const int i = r * kPT + tid;
-      if (i < m) {
-        u[r] = load_u<KK>(a.key, base + i);
-        if (a.n_vals > 0) v0[r] = ldg_stream_u64(a.vals[0] + base + i);
-      }
-    }
-#pragma unroll
-    for (int r = 0; r < kPR; ++r) {
-      const int i = r * kPT + tid;
-      if (i < m) {
+    for (int r = 0; r < RPT; ++r) {
+      const uint32_t i = (uint32_t)(r * T + tid);
+      if (i >= lo && i < hi) {
+        u[r] = stage_key<KK>(a.key, sm, st, i);
         const uint32_t q = part_id<U>(u[r], a.shift, mask);
-        pos[r] = (q << 16) | atomicAdd(&s_cnt[q], 1u);      // rank < 4096 fits 16 bits
+        pos[r] = (q << 16) | atomicAdd(&s_cnt[q], 1u);       // rank < tile <= 8192 fits 16 bits
       }
     }
     __syncthreads();
-    // B: exclusive scan of the per-partition counts; claim global space per partition
-    long long gclaim[kPer];
-    uint32_t gcnt[kPer];
-#pragma unroll
-    for (int k = 0; k < kPer; ++k) { gclaim[k] = 0; gcnt[k] = 0; }
+    // B: exclusive scan of the per-partition counts (one counter per thread: fan <= blockDim); claim global space
     {
-      uint32_t c[kPer], sum = 0;
-#pragma unroll
-      for (int k = 0; k < kPer; ++k) { const int p = tid * kPer + k; c[k] = p < fan ? s_cnt[p] : 0u; sum += c[k]; }
-      uint32_t inc = sum;
+      const uint32_t c = tid < fan ? s_cnt[tid] : 0u;
+      uint32_t inc = c;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += y; }
       if (lane == 31) s_warp[warp] = inc;
       __syncthreads();
       if (warp == 0) {
-        uint32_t w = lane < kPT / 32 ? s_warp[lane] : 0u;
+        const uint32_t w = lane < (T >> 5) ? s_warp[lane] : 0u;
         uint32_t winc = w;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += y; }
-        if (lane < kPT / 32) s_warp[lane] = winc - w;
+        s_warp[lane] = winc - w;
       }
       __syncthreads();
-      uint32_t run = s_warp[warp] + inc - sum;
-      // the claims' round trips to L2 overlap the staging below: their results are first needed in D
-#pragma unroll
-      for (int k = 0; k < kPer; ++k) {
-        const int p = tid * kPer + k;
-        if (p < fan) {
-          s_loff[p] = run;
-          gclaim[k] = c[k] ? (long long)atomicAdd(&cursor[p], (unsigned long long)c[k]) - (long long)run : 0ll;
-          gcnt[k] = c[k];
-          s_cnt[p] = 0;
-          run += c[k];
-        }
+      if (tid < fan) {
+        const uint32_t run = s_warp[warp] + inc - c;
+        s_loff[tid] = run;
+        s_delta[tid] = c ? (long long)atomicAdd(&cursor[tid], (unsigned long long)c) - (long long)run : 0ll;
+        s_cnt[tid] = 0;
       }
     }
     __syncthreads();
-    // C: stage keys (and the first value column) in partition order
+    // C/D per column: stage in partition order, then write runs.  Keys first (they are in registers).
+    UO* ko = reinterpret_cast<UO*>(s_out);
 #pragma unroll
-    for (int r = 0; r < kPR; ++r) {
-      const int i = r * kPT + tid;
-      if (i < m) {
+    for (int r = 0; r < RPT; ++r) {
+      const uint32_t i = (uint32_t)(r * T + tid);
+      if (i >= lo && i < hi) {
         const uint32_t q = pos[r] >> 16;
         pos[r] = s_loff[q] + (pos[r] & 0xFFFFu);
-        s_key[pos[r]] = (UO)u[r];
+        ko[pos[r]] = (UO)u[r];
         s_pid[pos[r]] = (uint16_t)q;
-        if (a.n_vals > 0) s_val[pos[r]] = v0[r];
-      }
-    }
-#pragma unroll
-    for (int k = 0; k < kPer; ++k) { const int p = tid * kPer + k; if (p < fan && gcnt[k]) s_delta[p] = gclaim[k]; }
-    __syncthreads();
-    // D: write runs
-#pragma unroll
-    for (int r = 0; r < kPR; ++r) {
-      const int j = r * kPT + tid;
-      if (j < m) {
-        const long long dst = s_delta[s_pid[j]] + j;
-        out_keys[dst] = s_key[j];
-        if (a.n_vals > 0) a.out_vals[0][dst] = s_val[j];
-      }
-    }
-    // remaining value columns, one staged at a time
-    for (int c = 1; c < a.n_vals; ++c) {
-      __syncthreads();
-#pragma unroll
-      for (int r = 0; r < kPR; ++r) {
-        const int i = r * kPT + tid;
-        if (i < m) s_val[pos[r]] = ldg_stream_u64(a.vals[c] + base + i);
-      }
-      __syncthreads();
-#pragma unroll
-      for (int r = 0; r < kPR; ++r) {
-        const int j = r * kPT + tid;
-        if (j < m) a.out_vals[c][s_delta[s_pid[j]] + j] = s_val[j];
       }
     }
     __syncthreads();
+    const uint32_t m = hi - lo;                              // rows of this tile
+    for (uint32_t j = tid; j < m; j += T) out_keys[s_delta[s_pid[j]] + j] = ko[j];
+    for (int c = 0; c < a.n_vals; ++c) {
+      __syncthreads();                                       // s_out is read by the previous column's write-out
+      const unsigned char* col = st + sm.voff[c];
+      if (sm.vw[c] == 8) {
+        uint64_t* vo = reinterpret_cast<uint64_t*>(s_out);
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) { const uint32_t i = (uint32_t)(r * T + tid); if (i >= lo && i < hi) vo[pos[r]] = *reinterpret_cast<const uint64_t*>(col + 8 * (size_t)i); }
+        if (c == a.n_vals - 1 && ring_stage >= 0) { __syncwarp(); if (lane == 0) mbar_arrive(&s_empty[ring_stage]); }
+        __syncthreads();
+        uint64_t* dst = static_cast<uint64_t*>(a.out_vals[c]);
+        for (uint32_t j = tid; j < m; j += T) dst[s_delta[s_pid[j]] + j] = vo[j];
+      } else {
+        uint32_t* vo = reinterpret_cast<uint32_t*>(s_out);
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) { const uint32_t i = (uint32_t)(r * T + tid); if (i >= lo && i < hi) vo[pos[r]] = *reinterpret_cast<const uint32_t*>(col + 4 * (size_t)i); }
+        if (c == a.n_vals - 1 && ring_stage >= 0) { __syncwarp(); if (lane == 0) mbar_arrive(&s_empty[ring_stage]); }
+        __syncthreads();
+        uint32_t* dst = static_cast<uint32_t*>(a.out_vals[c]);
+        for (uint32_t j = tid; j < m; j += T) dst[s_delta[s_pid[j]] + j] = vo[j];
+      }
+    }
+    if (a.n_vals == 0 && ring_stage >= 0) { __syncwarp(); if (lane == 0) mbar_arrive(&s_empty[ring_stage]); }
+    __syncthreads();                                         // s_out / s_pid / s_delta are reused by the next tile
+  };
+
+  for (int64_t k = 0; k < mine; ++k) {
+    const uint32_t g = (uint32_t)k, s = g % (uint32_t)sm.stages;
+    mbar_wait(&s_full[s], (g / (uint32_t)sm.stages) & 1u);
+    process(dsm + (size_t)s * sm.stage_bytes, A0 + ((int64_t)blockIdx.x + k * gridDim.x) * tile, (int)s);
+    if (tid == 0 && (int64_t)g_issued < mine) { issue(g_issued); ++g_issued; }
+  }
+  // the ragged last tile of a caller's column: loaded by the threads into stage 0 (every bulk copy of
+  // this CTA has landed and been consumed by now)
+  if (!padded && n_tiles > n_bulk && (int)(n_bulk % gridDim.x) == (int)blockIdx.x) {
+    const int64_t row0 = A0 + n_bulk * tile;
+    const uint32_t rows = (uint32_t)(r1 - row0);
+    unsigned char* st = dsm;
+    for (int c = 0; c < sm.n_src; ++c) {
+      const unsigned char* src = static_cast<const unsigned char*>(a.key.ptr[c]) + row0 * sm.kw[c];
+      for (uint32_t o = tid; o < rows * sm.kw[c]; o += T) st[sm.koff[c] + o] = src[o];
+    }
+    for (int c = 0; c < a.n_vals; ++c) {
+      const uint32_t* src = reinterpret_cast<const uint32_t*>(reinterpret_cast<const unsigned char*>(a.vals[c]) + row0 * sm.vw[c]);
+      uint32_t* d = reinterpret_cast<uint32_t*>(st + sm.voff[c]);
+      for (uint32_t o = tid; o < rows * (sm.vw[c] / 4u); o += T) d[o] = src[o];
+    }
+    __syncthreads();
+    process(st, row0, -1);
   }
 }
 
-template <int KK>
-int run_level(LevelArgs a, int segments, unsigned long long* off, int sm_count, cudaStream_t s, const uint32_t* pre_hist = nullptr) {
-  using UO = typename SrcKey<KK>::U;
-  const int64_t avg_rows = a.n / segments + 1;
-  const int64_t tiles = std::max<int64_t>(1, (avg_rows + kTile - 1) / kTile);
-  const int64_t want = segments == 1 ? (int64_t)sm_count * 8 : std::max<int64_t>(1, ((int64_t)sm_count * 8 + segments - 1) / segments);
-  const int gx = (int)std::min<int64_t>(tiles, want);
-  if (pre_hist && segments == 1 && a.fan <= kPreFan) {
-    part_fold_kernel<<<(a.fan + 255) / 256, 256, 0, s>>>(pre_hist, kPreFan, a.hist, a.fan);
-  } else {
-    EIGER_CUDA(cudaMemsetAsync(a.hist, 0, sizeof(uint32_t) * (size_t)segments * a.fan, s));
-    part_hist_kernel<KK><<<dim3(gx, segments), kPT, 0, s>>>(a);
+// shared-memory layout of the scatter kernel for a tile of `tile` rows
+ScatterSmem scatter_smem_layout(const KeyDesc& key, int key_kind, const uint8_t* vw, int n_vals, uint32_t tile, int stages, size_t out_key_bytes) {
+  ScatterSmem m{};
+  auto up = [](uint32_t x) { return (x + 127u) & ~127u; };
+  uint32_t off = 0;
+  const bool pre = key_kind == KK_U32PRE || key_kind == KK_U64PRE;
+  m.n_src = pre ? 1 : key.ncols;
+  for (int c = 0; c < m.n_src; ++c) {
+    const int w = pre ? (key_kind == KK_U32PRE ? 4 : 8) : (key.dtype[c] == EIGER_I8 ? 1 : key.dtype[c] == EIGER_I32 ? 4 : 8);
+    m.kw[c] = (uint8_t)w; m.koff[c] = off; off += up(tile * (uint32_t)w);
   }
-  count_launch();
-  part_scan_kernel<<<1, 1024, 0, s>>>(a.hist, off, a.cursor, segments * a.fan);
-  count_launch();
-  constexpr size_t smem = (sizeof(uint64_t) + sizeof(UO) + sizeof(uint16_t)) * kTile + (8 + 4 + 4) * kMaxFan;
-  auto kern = part_scatter_kernel<KK, UO>;
-  EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  kern<<<dim3(gx, segments), kPT, smem, s>>>(a);
+  for (int c = 0; c < n_vals; ++c) { m.vw[c] = vw[c] ? vw[c] : (uint8_t)8; m.voff[c] = off; off += up(tile * (uint32_t)m.vw[c]); }
+  m.stage_bytes = off;
+  m.stages = stages;
+  m.out_off = (uint32_t)stages * m.stage_bytes;
+  m.pid_off = m.out_off + up(tile * (uint32_t)std::max<size_t>(8, out_key_bytes));
+  m.total = m.pid_off + up(tile * 2u);
+  return m;
+}
+
+template <int KK, class UO, int RPT>
+int launch_scatter(const LevelArgs& a, const uint8_t* vw, int threads, int stages, int gx, int segments, cudaStream_t s) {
+  ScatterArgs A{};
+  A.lv = a;
+  A.tile = (uint32_t)(RPT * threads);
+  A.sm = scatter_smem_layout(a.key, KK, vw, a.n_vals, A.tile, stages, sizeof(UO));
+  auto kern = part_scatter_kernel<KK, UO, RPT>;
+  EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)A.sm.total));
+  kern<<<dim3(gx, segments), threads, A.sm.total, s>>>(A);
   count_launch();
   EIGER_CUDA(cudaGetLastError());
   return EIGER_OK;
 }
 
+template <int KK>
+int run_level(LevelArgs a, const uint8_t* vw, int segments, unsigned long long* off, int sm_count, size_t smem_optin, cudaStream_t s, const uint32_t* pre_hist = nullptr) {
+  using UO = typename SrcKey<KK>::U;
+  // tile shape: the largest of (1024 x 6), (1024 x 4), (512 x 6), (512 x 4), (256 x 4) rows whose ring
+  // (two stages) + staging buffer fit one CTA's shared memory
+  static const int cand[][2] = {{1024, 6}, {1024, 4}, {512, 6}, {512, 4}, {256, 4}};
+  int threads = 256, rpt = 4;
+  const int stages = 2;
+  {
+    const char* et = std::getenv("EIGER_SCATTER_T"); const char* er = std::getenv("EIGER_SCATTER_RPT");
+    bool found = false;
+    for (auto& c : cand) {
+      if (et && std::atoi(et) != c[0]) continue;
+      if (er && std::atoi(er) != c[1]) continue;
+      if (c[0] < a.fan) continue;                            // one counter per thread in the scan
+      const ScatterSmem m = scatter_smem_layout(a.key, KK, vw, a.n_vals, (uint32_t)(c[0] * c[1]), stages, sizeof(UO));
+      if ((size_t)m.total + 20 * 1024 <= smem_optin) { threads = c[0]; rpt = c[1]; found = true; break; }
+    }
+    if (!found) { threads = std::max(256, a.fan); rpt = 4; }
+  }
+  const int64_t tile = (int64_t)threads * rpt;
+  const int64_t avg_rows = a.n / segments + 1;
+  const int64_t tiles = std::max<int64_t>(1, (avg_rows + tile - 1) / tile);
+  const int64_t want = segments == 1 ? (int64_t)sm_count : std::max<int64_t>(1, ((int64_t)sm_count * 2 + segments - 1) / segments);
+  const int gx = (int)std::min<int64_t>(tiles, want);
+  if (pre_hist && segments == 1 && a.fan <= kPreFan) {
+    part_fold_kernel<<<(a.fan + 255) / 256, 256, 0, s>>>(pre_hist, kPreFan, a.hist, a.fan);
+  } else {
+    EIGER_CUDA(cudaMemsetAsync(a.hist, 0, sizeof(uint32_t) * (size_t)segments * a.fan, s));
+    const int64_t htiles = std::max<int64_t>(1, (avg_rows + kTile - 1) / kTile);
+    const int64_t hwant = segments == 1 ? (int64_t)sm_count * 8 : std::max<int64_t>(1, ((int64_t)sm_count * 8 + segments - 1) / segments);
+    part_hist_kernel<KK><<<dim3((int)std::min<int64_t>(htiles, hwant), segments), kPT, 0, s>>>(a);
+  }
+  count_launch();
+  part_scan_kernel<<<1, 1024, 0, s>>>(a.hist, off, a.cursor, segments * a.fan);
+  count_launch();
+  if (rpt == 6) return launch_scatter<KK, UO, 6>(a, vw, threads, stages, gx, segments, s);
+  return launch_scatter<KK, UO, 4>(a, vw, threads, stages, gx, segments, s);
+}
+
 template <int KK, int KK2>
-int run_levels(PartitionLaunch& L, int sm_count, cudaStream_t s) {
+int run_levels(PartitionLaunch& L, int sm_count, size_t smem_optin, cudaStream_t s) {
   using U = typename SrcKey<KK>::U;
   const int W = 8 * (int)sizeof(U);
   LevelArgs a{};
   a.key = L.key; a.n = L.n; a.n_vals = L.plan.n_vals;
-  for (int c = 0; c < kMaxVals; ++c) { a.vals[c] = static_cast<const uint64_t*>(L.plan.vals[c]); a.out_vals[c] = L.valsA[c]; }
+  for (int c = 0; c < kMaxVals; ++c) { a.vals[c] = L.plan.vals[c]; a.out_vals[c] = L.valsA[c]; }
   a.out_keys = L.keysA; a.seg_off = nullptr; a.hist = L.hist; a.cursor = L.cur1;
   a.fan = 1 << L.bits1; a.shift = W - L.bits1;
-  int rc = run_level<KK>(a, 1, L.off1, sm_count, s, L.pre_hist);
+  int rc = run_level<KK>(a, L.plan.vw, 1, L.off1, sm_count, smem_optin, s, L.pre_hist);
   if (rc) return rc;
   L.out_keys = L.keysA; L.out_vals = L.valsA; L.out_off = L.off1; L.n_parts = 1 << L.bits1;
   if (L.bits2 > 0) {
@@ -342,7 +437,7 @@ int run_levels(PartitionLaunch& L, int sm_count, cudaStream_t s) {
     for (int c = 0; c < kMaxVals; ++c) { b.vals[c] = L.valsA[c]; b.out_vals[c] = L.valsB[c]; }
     b.out_keys = L.keysB; b.seg_off = L.off1; b.hist = L.hist; b.cursor = L.cur2;
     b.fan = 1 << L.bits2; b.shift = W - L.bits1 - L.bits2;
-    rc = run_level<KK2>(b, 1 << L.bits1, L.off2, sm_count, s);
+    rc = run_level<KK2>(b, L.plan.vw, 1 << L.bits1, L.off2, sm_count, smem_optin, s);
     if (rc) return rc;
     L.out_keys = L.keysB; L.out_vals = L.valsB; L.out_off = L.off2; L.n_parts = 1 << (L.bits1 + L.bits2);
   }
@@ -356,14 +451,14 @@ int run_levels(PartitionLaunch& L, int sm_count, cudaStream_t s) {
 
 int partition_max_bits_per_level() { int b = 0; while ((1 << (b + 1)) <= kMaxFan) ++b; return b; }
 
-int launch_partition(PartitionLaunch& L, int sm_count, cudaStream_t s) {
+int launch_partition(PartitionLaunch& L, int sm_count, size_t smem_optin, cudaStream_t s) {
   const int mb = partition_max_bits_per_level();
   if (L.bits1 < 1 || L.bits1 > mb || L.bits2 < 0 || L.bits2 > mb) return EIGER_ERR_ARG;
   switch (L.key_kind) {
-    case KK_I32: return run_levels<KK_I32, KK_U32PRE>(L, sm_count, s);
-    case KK_I64: return run_levels<KK_I64, KK_U64PRE>(L, sm_count, s);
-    case KK_GEN: case KK_I8I8: return run_levels<KK_GEN, KK_U64PRE>(L, sm_count, s);
-    case KK_GEN32: return run_levels<KK_GEN32, KK_U32PRE>(L, sm_count, s);
+    case KK_I32: return run_levels<KK_I32, KK_U32PRE>(L, sm_count, smem_optin, s);
+    case KK_I64: return run_levels<KK_I64, KK_U64PRE>(L, sm_count, smem_optin, s);
+    case KK_GEN: case KK_I8I8: return run_levels<KK_GEN, KK_U64PRE>(L, sm_count, smem_optin, s);
+    case KK_GEN32: return run_levels<KK_GEN32, KK_U32PRE>(L, sm_count, smem_optin, s);
     default: return EIGER_ERR_ARG;
   }
 }

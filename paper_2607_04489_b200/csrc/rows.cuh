@@ -186,6 +186,23 @@ __device__ __forceinline__ void store_group_key(const KeyDesc& key, void* const*
   }
 }
 
+// value column c straight from global memory: one row, or two consecutive rows starting at an
+// even row index.  w = bytes per element: 8, or 4 for int32 payloads (sign-extended)
+__device__ __forceinline__ uint64_t global_val(const AggPlan& p, int c, int w, int64_t i) {
+  if (w == 8) return ldg_stream_u64(static_cast<const uint64_t*>(p.vals[c]) + i);
+  return (uint64_t)(int64_t)(int32_t)ldg_stream_4(static_cast<const int32_t*>(p.vals[c]) + i);
+}
+__device__ __forceinline__ void global_val2(const AggPlan& p, int c, int w, int64_t i, uint64_t& a, uint64_t& b) {
+  if (w == 8) {
+    const uint4 v = ldg_stream_16(static_cast<const uint64_t*>(p.vals[c]) + i);
+    a = ((uint64_t)v.y << 32) | v.x; b = ((uint64_t)v.w << 32) | v.z;
+  } else {
+    const uint2 v = ldg_stream_8(static_cast<const int32_t*>(p.vals[c]) + i);
+    a = (uint64_t)(int64_t)(int32_t)v.x; b = (uint64_t)(int64_t)(int32_t)v.y;
+  }
+}
+template <int SIG> __device__ __forceinline__ int sig_vw(const AggPlan& p, int c) { if constexpr (Sig<SIG>::kStatic) return Sig<SIG>::vwidth(c); else return p.vw[c]; }
+
 template <int SIG> __device__ __forceinline__ int sig_op(const AggPlan& p, int j) { if constexpr (Sig<SIG>::kStatic) return Sig<SIG>::op(j); else return p.op[j]; }
 template <int SIG> __device__ __forceinline__ int sig_col(const AggPlan& p, int j) { if constexpr (Sig<SIG>::kStatic) return Sig<SIG>::col(j); else return p.col[j]; }
 template <int SIG> __device__ __forceinline__ bool sig_f64(const AggPlan& p, int j) { if constexpr (Sig<SIG>::kStatic) return Sig<SIG>::f64(j); else return p.f64[j] != 0; }

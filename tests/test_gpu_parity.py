@@ -272,6 +272,29 @@ def test_partition_cuts_hot_partitions_into_items():
     assert_matches(res, want, d.aggs, d.vals)
 
 
+@pytest.mark.parametrize("part_kb,est_log2", [(None, 20), (48, 20), (None, 14), (48, 14)])
+def test_partition_tables_close_without_duplicate_groups(monkeypatch, part_kb, est_log2):
+    # Forced PARTITION with the NDV under-estimated (R10): 2^22 scattered keys, 16 rows each.
+    # est = 2^20 sizes the fan-out so that every partition holds ~1.3x its table's slots in distinct keys:
+    # the shared-memory tables CLOSE (0.85 x slots) and later rows go to the global table, whose capacity
+    # (2 x est) still takes them - the configuration in which a key could end up in both tables and be
+    # emitted twice (hashagg.cuh: s_spilled).  est = 2^14 additionally walks the overflow -> 4x re-run path.
+    # Repeated, because the duplicate needs two lanes to race on one key.
+    if part_kb is not None:
+        monkeypatch.setenv("EIGER_PART_KB", str(part_kb))
+    ds = datagen.config5(n=1 << 26, ndv=1 << 22, scattered=True)
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    st = eiger.profile(d.keys[0])
+    low = [eiger.Stats(st.min, st.max, float(1 << est_log2), st.n)]
+    for rep in range(10 if est_log2 == 20 else 3):
+        res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.PARTITION, stats=low)
+        k = res.sorted().keys[0]
+        assert bool((k[1:] > k[:-1]).all()), f"duplicate group keys in repetition {rep}"
+        assert res.n_groups == 1 << 22
+        assert_matches(res, want, d.aggs, d.vals)
+
+
 @pytest.fixture
 def small_partition_tables(monkeypatch):
     # 48 KB per-CTA tables (the tunables are re-read on every call): two partition levels are then
