@@ -27,7 +27,7 @@ if ROOT not in sys.path:
 
 METRIC = "groupby_rows_per_s"
 UNIT = "rows/s"
-VARIANTS = {"auto": 0, "direct": 1, "smem": 2, "global": 3, "partition": 4}
+VARIANTS = {"auto": 0, "direct": 1, "smem": 2, "global": 3, "partition": 4, "sort": 5}
 
 
 def parse_args(argv=None):
@@ -41,6 +41,8 @@ def parse_args(argv=None):
     ap.add_argument("--scale", type=int, default=1, help="divide the row count (development only; prints scale in config)")
     ap.add_argument("--sweep", action="store_true", help="config-5 crossover sweep: every variant at every NDV point")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-curve", action="store_true", help="skip the ndv_curve key (the metric is rows/s vs NDV: C5 points, C3, C4)")
+    ap.add_argument("--curve-forced", action="store_true", help="ndv_curve: also time the forced variants (statistics supplied) at every point")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args(argv)
 
@@ -289,6 +291,13 @@ def main(argv=None):
                  "profile": ds.n * key_bytes}[dom]
     dom_ms, dom_n = kt[dom]
     achieved = (alg_bytes / ((dom_ms / max(dom_n, 1)) * 1e-3)) / 1e9 if dom_ms > 0 else 0.0
+    # the driver's peak is a copy (read + write at once); a pure read stream of this device, measured
+    # now by the library's own probe kernels (16-byte loads / bulk copies), is quoted beside it
+    try:
+        read_peak = max(eiger.probe("read_ldg", 2048), eiger.probe("read_bulk", 2048, 32768))
+        eiger.probe("release")
+    except eiger.EigerError:
+        read_peak = None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -303,7 +312,8 @@ def main(argv=None):
         "ms_per_step_with_kernel_events": ms_instrumented / args.steps,
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak if peak else None, "traffic": traffic_from_profiles(args.workload, dom), "peak_source": peak_src,
-                     "algorithmic_bytes_per_launch": alg_bytes, "launches_timed": dom_n},
+                     "algorithmic_bytes_per_launch": alg_bytes, "launches_timed": dom_n,
+                     "read_only_peak_gbs": read_peak, "frac_of_read_only_peak": (achieved / read_peak) if read_peak else None},
         "clocks": clocks.summary(),
     }
 
@@ -327,10 +337,80 @@ def main(argv=None):
         del hk, hv
     if not args.no_cpu and world == 1 and rank == 0:
         line["cpu_baseline"] = cpu_baseline(ds.cpu(), cpu_sample_rows(args.workload) // max(args.scale, 1))
+    if not args.no_curve and world == 1:
+        del ds, res, ws
+        last.clear()
+        torch.cuda.empty_cache()
+        line["ndv_curve"] = ndv_curve(args, eiger, torch, dev, peak)
     if rank == 0:
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
+
+
+CURVE_POINTS = [f"C5:{lg}:{lay}" for lay in ("dense", "scattered") for lg in (4, 8, 12, 13, 14, 15, 16, 20, 24, 28)] + ["C3", "C4"]
+
+
+def ndv_curve(args, eiger, torch, dev, peak):
+    """The metric is "rows/s and input GB/s vs NDV": EIGER_AUTO (statistics gathered inside the timed
+    call) at every C5 point (both layouts, 2^13..2^15 included), C3 and C4, each with the per-kernel
+    device times of a second, instrumented region.  --curve-forced adds the forced variants with the
+    statistics supplied (profile excluded), the reading of "within 10 % of the best single variant"."""
+    out = []
+    ws = eiger.Workspace(dev)
+    names = ["aggregate", "profile", "partition", "init", "compact"]
+    for name in CURVE_POINTS:
+        try:
+            ds = build_workload(name, dev, scale=args.scale)
+        except torch.OutOfMemoryError:
+            out.append({"workload": name, "error": "oom"})
+            continue
+        fn = lambda: eiger.groupby(ds.keys, ds.vals, ds.aggs, workspace=ws)
+        try:
+            r = fn()
+            assert ds.ndv is None or r.n_groups == ds.ndv, (name, r.n_groups, ds.ndv)
+            est = time_steps(fn, 2, 3, torch) / 2
+            k = max(3, min(30, int(40.0 / max(est, 1e-3))))
+            ms = time_steps(fn, k, 0, torch) / k
+            eiger.set_kernel_timing(True)
+            for w in range(5):
+                eiger.kernel_time_ms(w, True)
+            time_steps(fn, k, 0, torch)
+            eiger.set_kernel_timing(False)
+            kt = {nm: eiger.kernel_time_ms(w, True)[0] / k for w, nm in enumerate(names)}
+            gbs = ds.n * ds.row_bytes / ms / 1e6
+            row = {"workload": name, "n": ds.n, "ndv": ds.ndv, "variant": eiger.VARIANT_NAMES[r.variant], "ms": round(ms, 4), "steps": k,
+                   "rows_per_s": ds.n / ms * 1e3, "input_gb_per_s": round(gbs, 1), "frac_8tbs": round(gbs / 8000.0, 4),
+                   "frac_measured_peak": round(gbs / peak, 4), "kernel_ms": {a: round(b, 4) for a, b in kt.items()}}
+            if args.curve_forced:
+                st = eiger.profile_keys(ds.keys)
+                lg = (ds.ndv or 1).bit_length() - 1
+                dense = not ds.meta.get("scattered", False) and name.startswith("C5")
+                forced = {}
+                for vname, v in VARIANTS.items():
+                    if v == 0 or (v == 1 and not dense) or (v == 2 and lg > 16) or (v == 3 and lg > 20):
+                        continue      # variants that take tens of milliseconds here (round-1 sweep) are not re-timed
+                    try:
+                        f2 = lambda: eiger.groupby(ds.keys, ds.vals, ds.aggs, force=v, stats=st, workspace=ws)
+                        f2()
+                        e2 = time_steps(f2, 2, 2, torch) / 2
+                        k2 = max(3, min(30, int(40.0 / max(e2, 1e-3))))
+                        forced[vname] = round(time_steps(f2, k2, 0, torch) / k2, 4)
+                    except eiger.EigerError as e:
+                        forced[vname] = f"error {e.code}"
+                row["forced_ms"] = forced
+                best = min((x for x in forced.values() if isinstance(x, float)), default=None)
+                row["auto_over_best_forced"] = round(ms / best, 3) if best else None
+            out.append(row)
+        except (eiger.EigerError, AssertionError) as e:
+            out.append({"workload": name, "error": str(e)[:200]})
+        except torch.OutOfMemoryError:
+            out.append({"workload": name, "error": "oom"})
+            ws = eiger.Workspace(dev)
+        print(json.dumps(out[-1]), file=sys.stderr, flush=True)
+        del ds
+        torch.cuda.empty_cache()
+    return out
 
 
 def sweep(args, eiger, torch, dev):

@@ -41,7 +41,9 @@ typedef enum {
   EIGER_DIRECT = 1,    /* direct-index array, slot = key - min                */
   EIGER_SMEM = 2,      /* per-CTA shared-memory open addressing, merged       */
   EIGER_GLOBAL = 3,    /* one global open-addressing table (L2-resident)      */
-  EIGER_PARTITION = 4  /* radix partition by hash bits, then aggregate        */
+  EIGER_PARTITION = 4, /* radix partition by hash bits, then aggregate        */
+  EIGER_SORT = 5       /* radix sort on the key bits, then segmented reduce;  */
+                       /* groups come out in ascending key order              */
 } eiger_variant;
 
 typedef enum {
@@ -51,7 +53,8 @@ typedef enum {
   EIGER_ERR_OUT_CAPACITY = -3, /* more groups than out_capacity; *n_groups holds the count   */
   EIGER_ERR_INFEASIBLE = -4,   /* the forced variant cannot run on this input                */
   EIGER_ERR_CUDA = -5,         /* a CUDA runtime call failed; eiger_last_cuda_error() says   */
-  EIGER_ERR_TABLE_OVERFLOW = -6 /* NDV estimate too low and no room in workspace to retry   */
+  EIGER_ERR_TABLE_OVERFLOW = -6, /* NDV estimate too low and no room in workspace to retry  */
+  EIGER_ERR_STATS = -7         /* a key lies outside the caller's eiger_stats [min, max]     */
 } eiger_status;
 
 typedef struct { const void* data; int32_t dtype; int32_t reserved; } eiger_col; /* length n */
@@ -101,7 +104,11 @@ double eiger_hll_estimate_host(const uint8_t* regs);
  *   vals[n_vals]       value columns, EIGER_I64 or EIGER_F64, n_vals <= 8
  *   aggs[n_aggs]       n_aggs <= 8; result type: SUM/MIN/MAX of I64 -> int64 (SUM wraps modulo
  *                      2^64), of F64 -> double; COUNT -> int64 row count
- *   stats              HOST, n_key_cols entries from eiger_profile, or NULL: the library then
+ *   stats              HOST, n_key_cols entries from eiger_profile (min / max MUST bound every key of
+ *                      their column; ndv_est may be off, R10).  A key outside them is detected where
+ *                      it would matter - direct-index arrays and fused multi-column keys run with a
+ *                      range check - and fails the call with EIGER_ERR_STATS; single-column hash
+ *                      variants rebase modulo 2^32 / 2^64 and are indifferent to it.  Or NULL: the library then
  *                      gathers the statistics inside this call (that is what EIGER_AUTO timing
  *                      includes).  A forced variant runs the full profile.  EIGER_AUTO on
  *                      n >= 2^22 rows first profiles an evenly spaced sample of 2^16 keys; if
@@ -121,7 +128,8 @@ double eiger_hll_estimate_host(const uint8_t* regs);
  * Errors: EIGER_ERR_ARG; EIGER_ERR_WORKSPACE; EIGER_ERR_OUT_CAPACITY (a safe capacity is
  * min(n, range)); EIGER_ERR_INFEASIBLE (e.g. EIGER_DIRECT on a 2^40 range);
  * EIGER_ERR_TABLE_OVERFLOW (the sketch under-estimated and the workspace has no room for the
- * larger table: call again with stats->ndv_est raised, e.g. to min(n, range)); EIGER_ERR_CUDA.
+ * larger table: call again with stats->ndv_est raised, e.g. to min(n, range)); EIGER_ERR_STATS;
+ * EIGER_ERR_CUDA.
  * fp64 MIN/MAX order -0.0 below +0.0; NaN inputs are not supported. */
 int eiger_groupby(const eiger_col* keys, int32_t n_key_cols, int64_t n,
                   const eiger_col* vals, int32_t n_vals,

@@ -23,9 +23,9 @@ _LIB_PATH = os.path.join(_HERE, "libeiger.so")
 
 I8, I32, I64, F64 = 0, 1, 2, 3
 SUM, COUNT, MIN, MAX = 0, 1, 2, 3
-AUTO, DIRECT, SMEM, GLOBAL, PARTITION = 0, 1, 2, 3, 4
-VARIANT_NAMES = {AUTO: "auto", DIRECT: "direct", SMEM: "smem", GLOBAL: "global", PARTITION: "partition"}
-OK, ERR_ARG, ERR_WORKSPACE, ERR_OUT_CAPACITY, ERR_INFEASIBLE, ERR_CUDA, ERR_TABLE_OVERFLOW = 0, -1, -2, -3, -4, -5, -6
+AUTO, DIRECT, SMEM, GLOBAL, PARTITION, SORT = 0, 1, 2, 3, 4, 5
+VARIANT_NAMES = {AUTO: "auto", DIRECT: "direct", SMEM: "smem", GLOBAL: "global", PARTITION: "partition", SORT: "sort"}
+OK, ERR_ARG, ERR_WORKSPACE, ERR_OUT_CAPACITY, ERR_INFEASIBLE, ERR_CUDA, ERR_TABLE_OVERFLOW, ERR_STATS = 0, -1, -2, -3, -4, -5, -6, -7
 HLL_M = 1 << 14
 
 # every symbol include/eiger.h declares (tests check the library exports each of them)
@@ -176,7 +176,7 @@ def _stats_arr(stats):
 
 MAX_KEY_COLS = 4
 _KEY_T = (torch.int8, torch.int32, torch.int64)
-_VAL_T = (torch.int64, torch.float64)
+_VAL_T = (torch.int64, torch.float64, torch.int32)
 
 
 def profile(keys: torch.Tensor) -> Stats:
@@ -335,7 +335,7 @@ def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int |
                     for s in stats:
                         rng *= (s.max - s.min + 1)
                     cap = max(0, min(n, rng))
-                    if force in (AUTO, SMEM, GLOBAL, PARTITION) and stats and len(stats) == 1:
+                    if force in (AUTO, SMEM, GLOBAL, PARTITION, SORT) and stats and len(stats) == 1:
                         cap = min(cap, int(stats[0].ndv_est * 1.25) + 1024)
             else:
                 cap = out_capacity

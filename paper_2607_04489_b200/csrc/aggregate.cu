@@ -246,6 +246,7 @@ struct CompactArgs {
   uint64_t cap; uint32_t stride; int back;
   void* out_keys[kMaxKeyCols]; uint64_t* out_aggs[kMaxAggs]; int n_out;
   int64_t out_capacity;
+  uint64_t R;               // several key columns: fused keys are below R; anything else is a row outside the planned ranges
   CallDev* call;
 };
 
@@ -272,6 +273,10 @@ __global__ void __launch_bounds__(256) compact_kernel(const __grid_constant__ Co
         u = s;
       }
     }
+    // several key columns: a row with a column outside its planned range was fused to the marker
+    // (rows.cuh: fuse_cols) and sits in the side slot / beyond the fused domain: the caller's
+    // statistics do not bound the keys
+    if (occ && c.key.ncols > 1 && c.back == BACK_HASH && (s == c.cap || u >= c.R)) { atomicOr(&c.call->abort, 1u); occ = false; }
     const uint32_t m = __ballot_sync(0xffffffffu, occ);
     if (m == 0) continue;
     unsigned long long start = 0;
@@ -379,7 +384,7 @@ int launch_compact(const CompactLaunch& c, int sm_count, cudaStream_t s) {
   a.cap = c.cap; a.stride = c.stride; a.back = c.back;
   for (int k = 0; k < kMaxKeyCols; ++k) a.out_keys[k] = c.out_keys[k];
   for (int j = 0; j < kMaxAggs; ++j) a.out_aggs[j] = static_cast<uint64_t*>(c.out_aggs[j]);
-  a.n_out = c.n_out_aggs; a.out_capacity = c.out_capacity; a.call = c.call;
+  a.n_out = c.n_out_aggs; a.out_capacity = c.out_capacity; a.call = c.call; a.R = c.R;
   const uint64_t n_slots = c.cap + 1;
   const int blocks = (int)std::max<uint64_t>(1, std::min<uint64_t>((n_slots + 255) / 256, (uint64_t)sm_count * 8));
   compact_kernel<<<blocks, 256, 0, s>>>(a);

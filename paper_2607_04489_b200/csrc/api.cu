@@ -154,6 +154,7 @@ struct QueryPlan {
   uint32_t stride = 0;
   size_t table_bytes = 0, part_bytes = 0, total_bytes = 0;
   const uint32_t* pre_hist = nullptr;   // PARTITION: level-1 histogram taken with key.base at fan-out kPreFan
+  int sort_bits = 0, sort_passes = 0;   // SORT: significant bits of the rebased fused key, 8-bit passes
 };
 
 uint64_t range_of(const eiger_stats& s) {   // max - min + 1, 0 when it is 2^64
@@ -181,7 +182,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
                const eiger_agg* aggs, int na, const eiger_stats* st, int force, QueryPlan* q, bool skewed = false) {
   if (!keys || nk < 1 || nk > kMaxKeyCols || n < 0 || nv < 0 || nv > kMaxVals || na < 1 || na > kMaxAggs || !aggs) return EIGER_ERR_ARG;
   if (nv > 0 && !vals) return EIGER_ERR_ARG;
-  if (force < EIGER_AUTO || force > EIGER_PARTITION) return EIGER_ERR_ARG;
+  if (force < EIGER_AUTO || force > EIGER_SORT) return EIGER_ERR_ARG;
   for (int k = 0; k < nk; ++k) if (!is_key_dtype(keys[k].dtype)) return EIGER_ERR_ARG;
   for (int c = 0; c < nv; ++c) if (vals[c].dtype != EIGER_I64 && vals[c].dtype != EIGER_F64 && vals[c].dtype != EIGER_I32) return EIGER_ERR_ARG;
 
@@ -230,12 +231,16 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   for (int k = 0; k < kMaxKeyCols; ++k) kd.rng[k] = k < nk ? Rk[k] : 1;     // rng[0] = 0 (full 64-bit range) only on the single-column paths
   if (nk >= 2) {
     unsigned __int128 prod = 1;
-    for (int k = 0; k < nk; ++k) {
-      if (Rk[k] == 0) return EIGER_ERR_INFEASIBLE;
+    bool fits = true;
+    for (int k = 0; k < nk && fits; ++k) {
+      if (Rk[k] == 0) { fits = false; break; }
       prod *= Rk[k];
-      if (prod >> 64) return EIGER_ERR_INFEASIBLE;   // fused key must fit 64 bits
+      if (prod >> 64) fits = false;                  // fused key must fit 64 bits
     }
-    R = (uint64_t)prod; kd.mul = Rk[1];
+    // without statistics (workspace sizing before the profile) the type ranges of several int32 /
+    // int64 columns always multiply past 2^64: size for "range unknown", the group count bounded by n
+    if (!fits && have_stats) return EIGER_ERR_INFEASIBLE;
+    R = fits ? (uint64_t)prod : 0; kd.mul = Rk[1];
   }
   {
     bool all32 = true;
@@ -317,6 +322,21 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
     }
     q->sig = detect_sig(p, na);
     if (!aggregate_supported(q->key_kind, q->sig, q->front, q->back)) return EIGER_ERR_INFEASIBLE;
+  } else if (variant == EIGER_SORT) {
+    // sort-based group-by: LSD radix sort on the bits the key range needs, then
+    // a segmented reduce.  No table: the workspace holds one or two copies of the rows.
+    if (n >= (1ll << 32)) return EIGER_ERR_INFEASIBLE;       // 32-bit tile offsets
+    q->back = BACK_HASH; q->stride = hash_stride; q->cap = 0; q->table_bytes = 0;
+    q->key_kind = hkp;
+    q->sig = detect_sig(p, na);
+    int bits = 64;
+    if (R != 0) { bits = 0; while (bits < 64 && (R - 1) >> bits) ++bits; }
+    if (hkp == KK_I32 && bits > 32) bits = 32;
+    q->sort_bits = bits; q->sort_passes = std::max(1, (bits + 7) / 8);
+    const size_t kb = (bits <= 32) ? 4 : 8;
+    size_t copy = align_up((size_t)n * kb, 256);
+    for (int c = 0; c < p.n_vals; ++c) copy += align_up((size_t)n * 8, 256);
+    q->part_bytes = copy * (q->sort_passes >= 2 ? 2 : 1) + align_up(((size_t)n / 1024 + 2) * 256 * 4, 256) + align_up(512 * 8, 256);
   } else {
     q->back = BACK_HASH;
     q->stride = hash_stride;
@@ -440,7 +460,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
   }
   for (int c = 0; c < nv; ++c) if (n > 0 && vals && (!vals[c].data || ((uintptr_t)vals[c].data & 15))) return EIGER_ERR_ARG;
   if (n == 0) {   // legal: no groups; nothing is launched
-    if (force < EIGER_AUTO || force > EIGER_PARTITION) return EIGER_ERR_ARG;
+    if (force < EIGER_AUTO || force > EIGER_SORT) return EIGER_ERR_ARG;
     if (chosen) *chosen = force;
     return EIGER_OK;
   }
@@ -455,6 +475,10 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
   const int T_front_probes = tun().global_front_probes;
   int hot_n = 0;                 // heavy hitters of the key sample (skewed inputs only)
   long long hot_key[kMaxHot];
+  // checked != 0: the statistics are the caller's: a key outside them must not corrupt memory
+  // (direct arrays are indexed with key - min) or alias onto another group (fused keys); the kernels
+  // run with the range check of the speculative pass and the call fails with EIGER_ERR_STATS
+  const int checked = stats_in != nullptr;
   auto execute = [&](QueryPlan& q, const eiger_stats* st, int spec, bool* aborted) -> int {
   if (q.total_bytes > workspace_bytes || !workspace) return EIGER_ERR_WORKSPACE;
   const int src_kind = q.key_kind;
@@ -468,7 +492,29 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     L.key_kind = q.key_kind; L.sig = q.sig; L.front = q.front; L.back = q.back;
     L.front_slots = q.front_slots; L.front_limit = q.front_limit; L.front_replicas = q.front_replicas;
     L.table = table; L.cap = q.cap; L.stride = q.stride; L.call = rt->call;
-    L.threads = 256; L.smem_bytes = q.smem_bytes; L.spec = spec;
+    L.threads = 256; L.smem_bytes = q.smem_bytes; L.spec = spec | checked;
+    if (q.variant == EIGER_SORT) {
+      SortLaunch S{};
+      S.key = q.key; S.plan = q.plan; S.n = n; S.key_kind = q.key_kind; S.sig = q.sig; S.bits = q.sort_bits;
+      const size_t kb = (q.sort_bits <= 32) ? 4 : 8;
+      const size_t col = align_up((size_t)n * 8, 256), kcol = align_up((size_t)n * kb, 256);
+      auto take = [&](size_t bytes) { char* r = pws; pws += align_up(bytes, 256); return r; };
+      S.tile_hist = reinterpret_cast<uint32_t*>(take(((size_t)n / 1024 + 2) * 256 * 4));
+      S.digit_base = reinterpret_cast<unsigned long long*>(take(512 * 8));
+      S.keysA = take(kcol);
+      for (int c = 0; c < q.plan.n_vals; ++c) S.valsA[c] = take(col);
+      if (q.sort_passes >= 2) { S.keysB = take(kcol); for (int c = 0; c < q.plan.n_vals; ++c) S.valsB[c] = take(col); }
+      for (int k = 0; k < kMaxKeyCols; ++k) S.out_keys[k] = k < nk ? out_keys[k] : nullptr;
+      for (int j = 0; j < na; ++j) S.out_aggs[j] = out_aggs[j];
+      S.n_out_aggs = na; S.out_capacity = out_capacity; S.call = rt->call;
+      { Timed t(s, 0); rc = launch_sort_groupby(S, rt->sm_count, rt->smem_optin, s); if (rc) return rc; }
+      EIGER_CUDA(cudaMemcpyAsync(hb, rt->call, sizeof(Back), cudaMemcpyDeviceToHost, s));
+      EIGER_CUDA(cudaStreamSynchronize(s));
+      resolve_timing();
+      *n_groups = (int64_t)hb->n_groups;
+      if ((int64_t)hb->n_groups > out_capacity) return EIGER_ERR_OUT_CAPACITY;
+      return EIGER_OK;
+    }
     { Timed t(s, 3); rc = launch_table_init(L, s); if (rc) return rc; }
 
     if (q.variant == EIGER_DIRECT) {
@@ -545,13 +591,14 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     C.key = q.key; C.plan = q.plan; C.back = q.back; C.table = table; C.cap = q.cap; C.stride = q.stride;
     for (int k = 0; k < kMaxKeyCols; ++k) C.out_keys[k] = k < nk ? out_keys[k] : nullptr;
     for (int j = 0; j < na; ++j) C.out_aggs[j] = out_aggs[j];
-    C.n_out_aggs = na; C.out_capacity = out_capacity; C.call = rt->call;
+    C.n_out_aggs = na; C.out_capacity = out_capacity; C.call = rt->call; C.R = q.R;
     { Timed t(s, 4); rc = launch_compact(C, rt->sm_count, s); if (rc) return rc; }
 
     EIGER_CUDA(cudaMemcpyAsync(hb, rt->call, sizeof(Back), cudaMemcpyDeviceToHost, s));
     EIGER_CUDA(cudaStreamSynchronize(s));
     resolve_timing();
     if (spec && (hb->abort || hb->overflow)) { *aborted = true; return EIGER_OK; }
+    if (hb->abort) return EIGER_ERR_STATS;
     if (hb->overflow) {
       // the sketch under-estimated (R10): grow towards the exact bound and run again
       if (q.back != BACK_HASH || attempt >= 8) return EIGER_ERR_TABLE_OVERFLOW;
@@ -614,8 +661,10 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       const int64_t tmin = bits == 64 ? INT64_MIN : -(1ll << (bits - 1)), tmax = bits == 64 ? INT64_MAX : (1ll << (bits - 1)) - 1;
       const uint64_t R = (uint64_t)local[k].max - (uint64_t)local[k].min + 1ull;
       const int64_t margin = (R > 64 && R <= (1ull << 24)) ? (int64_t)(R / 32) : 0;   // only direct tables need the range
-      local[k].min = local[k].min - tmin >= margin ? local[k].min - margin : tmin;
-      local[k].max = tmax - local[k].max >= margin ? local[k].max + margin : tmax;
+      // room to the type's ends in unsigned arithmetic (min - INT64_MIN overflows int64 for any min >= 0)
+      const uint64_t room_lo = (uint64_t)local[k].min - (uint64_t)tmin, room_hi = (uint64_t)tmax - (uint64_t)local[k].max;
+      local[k].min = room_lo >= (uint64_t)margin ? local[k].min - margin : tmin;
+      local[k].max = room_hi >= (uint64_t)margin ? local[k].max + margin : tmax;
       local[k].n = n;
     }
     QueryPlan qs;
@@ -827,12 +876,12 @@ int eiger_groupby_host(const eiger_col* keys, int32_t nk, int64_t n, const eiger
   if (!rt) return EIGER_ERR_CUDA;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   for (int k = 0; k < nk; ++k) if (!is_key_dtype(keys[k].dtype) || (n > 0 && !keys[k].data)) return EIGER_ERR_ARG;
-  for (int c = 0; c < nv; ++c) if ((vals[c].dtype != EIGER_I64 && vals[c].dtype != EIGER_F64) || (n > 0 && !vals[c].data)) return EIGER_ERR_ARG;
+  for (int c = 0; c < nv; ++c) if ((vals[c].dtype != EIGER_I64 && vals[c].dtype != EIGER_F64 && vals[c].dtype != EIGER_I32) || (n > 0 && !vals[c].data)) return EIGER_ERR_ARG;
 
   // arena layout: input columns | output columns | workspace (sized after the profile)
   size_t in_bytes = 0, out_bytes = 0;
   for (int k = 0; k < nk; ++k) { in_bytes += align_up((size_t)n * dtype_size(keys[k].dtype), 256); out_bytes += align_up((size_t)out_capacity * dtype_size(keys[k].dtype), 256); }
-  in_bytes += (size_t)nv * align_up((size_t)n * 8, 256);
+  for (int c = 0; c < nv; ++c) in_bytes += align_up((size_t)n * (vals[c].dtype == EIGER_I32 ? 4 : 8), 256);
   out_bytes += (size_t)na * align_up((size_t)out_capacity * 8, 256);
   // first reservation covers the columns; the workspace is added once the statistics are known
   int rc = arena_reserve(std::max<size_t>(g_arena.size, in_bytes + out_bytes + ((size_t)64 << 20)));
@@ -846,7 +895,7 @@ int eiger_groupby_host(const eiger_col* keys, int32_t nk, int64_t n, const eiger
       h2d += (int64_t)b; cur += align_up(b, 256);
     }
     for (int c = 0; c < nv; ++c) {
-      const size_t b = (size_t)n * 8;
+      const size_t b = (size_t)n * (vals[c].dtype == EIGER_I32 ? 4 : 8);
       dv[c].data = cur; dv[c].dtype = vals[c].dtype; dv[c].reserved = 0;
       if (b) EIGER_CUDA(cudaMemcpyAsync(cur, vals[c].data, b, cudaMemcpyHostToDevice, s));
       h2d += (int64_t)b; cur += align_up(b, 256);
@@ -922,6 +971,7 @@ const char* eiger_strerror(int code) {
     case EIGER_ERR_INFEASIBLE: return "the forced variant cannot run on this input";
     case EIGER_ERR_CUDA: return "CUDA runtime error (see eiger_last_cuda_error)";
     case EIGER_ERR_TABLE_OVERFLOW: return "hash table overflow: NDV under-estimated and no workspace to retry";
+    case EIGER_ERR_STATS: return "a key lies outside the [min, max] of the statistics supplied by the caller";
     default: return "unknown error";
   }
 }
@@ -929,7 +979,7 @@ const char* eiger_last_cuda_error(void) { return g_cuda_err; }
 const char* eiger_variant_name(int32_t v) {
   switch (v) {
     case EIGER_AUTO: return "auto"; case EIGER_DIRECT: return "direct"; case EIGER_SMEM: return "smem";
-    case EIGER_GLOBAL: return "global"; case EIGER_PARTITION: return "partition"; default: return "?";
+    case EIGER_GLOBAL: return "global"; case EIGER_PARTITION: return "partition"; case EIGER_SORT: return "sort"; default: return "?";
   }
 }
 void eiger_shutdown(void) {

@@ -19,6 +19,7 @@
 // instantiate it for their key kinds so that the three compile in parallel.)
 #pragma once
 #include <algorithm>
+#include <cstdlib>
 #include <type_traits>
 
 #include "internal.h"
@@ -52,6 +53,7 @@ struct HashAggArgs {
   uint32_t koff[kMaxKeyCols], voff[kMaxVals];   // byte offset of each column inside a stage
   uint8_t kw[kMaxKeyCols], vw[kMaxVals];        // bytes per element
   uint32_t hot_off, table_off;
+  int32_t ring_hint;             // bulk copies carry an L2 evict_first policy
 };
 
 template <int KK> struct IsPre { static constexpr bool v = (KK == KK_U32PRE || KK == KK_U64PRE); };
@@ -516,19 +518,33 @@ __device__ __forceinline__ void ring_vals(const HashAggArgs& a, const unsigned c
 // One elected thread keeps the ring full: rows [row0, row0 + rows) of every column go into stage
 // g % stages with one bulk copy per column (row0 a multiple of 32, rows a multiple of 32: every
 // copy starts 16-byte aligned and is a multiple of 16 bytes long, whatever the column width).
-__device__ __forceinline__ void ring_issue(const HashAggArgs& a, unsigned char* ring, uint64_t* full, uint64_t* empty,
-                                           uint32_t g, int64_t row0, uint32_t rows, uint64_t policy) {
+// `quit` (may be null): a shared flag raised by a warp that leaves the chunk loop early (speculative
+// runs); the stage it would have released never becomes free, so the wait gives up.  Returns whether
+// the chunk was requested.
+__device__ __forceinline__ bool ring_issue(const HashAggArgs& a, unsigned char* ring, uint64_t* full, uint64_t* empty,
+                                           uint32_t g, int64_t row0, uint32_t rows, uint64_t policy, const uint32_t* quit = nullptr) {
   const uint32_t s = g % (uint32_t)a.stages;
-  if (g >= (uint32_t)a.stages) mbar_wait(&empty[s], ((g / (uint32_t)a.stages) - 1u) & 1u);
+  if (g >= (uint32_t)a.stages) {
+    const uint32_t par = ((g / (uint32_t)a.stages) - 1u) & 1u;
+    while (!mbar_try_wait(&empty[s], par)) { if (quit && *reinterpret_cast<const volatile uint32_t*>(quit)) return false; }
+  }
   unsigned char* st = ring + (size_t)s * a.stage_bytes;
   uint32_t bytes = 0;
   for (int c = 0; c < a.n_src; ++c) bytes += rows * a.kw[c];
   for (int c = 0; c < a.plan.n_vals; ++c) bytes += rows * a.vw[c];
   mbar_expect_tx(&full[s], bytes);
-  for (int c = 0; c < a.n_src; ++c)
-    bulk_g2s_hint(st + a.koff[c], static_cast<const unsigned char*>(a.key.ptr[c]) + row0 * a.kw[c], rows * a.kw[c], &full[s], policy);
-  for (int c = 0; c < a.plan.n_vals; ++c)
-    bulk_g2s_hint(st + a.voff[c], static_cast<const unsigned char*>(a.plan.vals[c]) + row0 * a.vw[c], rows * a.vw[c], &full[s], policy);
+  if (policy) {
+    for (int c = 0; c < a.n_src; ++c)
+      bulk_g2s_hint(st + a.koff[c], static_cast<const unsigned char*>(a.key.ptr[c]) + row0 * a.kw[c], rows * a.kw[c], &full[s], policy);
+    for (int c = 0; c < a.plan.n_vals; ++c)
+      bulk_g2s_hint(st + a.voff[c], static_cast<const unsigned char*>(a.plan.vals[c]) + row0 * a.vw[c], rows * a.vw[c], &full[s], policy);
+  } else {
+    for (int c = 0; c < a.n_src; ++c)
+      bulk_g2s(st + a.koff[c], static_cast<const unsigned char*>(a.key.ptr[c]) + row0 * a.kw[c], rows * a.kw[c], &full[s]);
+    for (int c = 0; c < a.plan.n_vals; ++c)
+      bulk_g2s(st + a.voff[c], static_cast<const unsigned char*>(a.plan.vals[c]) + row0 * a.vw[c], rows * a.vw[c], &full[s]);
+  }
+  return true;
 }
 
 template <int KK, int SIG, int BK>
@@ -536,7 +552,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
 hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
   extern __shared__ __align__(128) unsigned char dyn[];     // [ring stages][heavy-hitter cells][table]
   __shared__ __align__(8) uint64_t s_full[kMaxStages], s_empty[kMaxStages];
-  __shared__ uint32_t s_count, s_abort, s_spilled;
+  __shared__ uint32_t s_count, s_abort, s_spilled, s_quit;
   __shared__ uint32_t s_wtot[32];
   __shared__ unsigned long long s_base;
   using F = Front<KK, SIG, BK>;
@@ -552,7 +568,7 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
     mbar_fence_init();
   }
   uint32_t g_cons = 0, g_issued = 0;                        // chunks consumed (all threads) / issued (thread 0)
-  const uint64_t policy = policy_evict_first();             // the rows are read once: first out of L2
+  const uint64_t policy = a.ring_hint ? policy_evict_first() : 0ull;   // the rows are read once: first out of L2
 
   if constexpr (!IsPre<KK>::v) {
     // ---- whole-input mode: chunk c = blockIdx.x, + gridDim.x, ... of the input ----
@@ -561,7 +577,7 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
     uint32_t* s_hot_rows = reinterpret_cast<uint32_t*>(s_hot + (kMaxThreads / 32) * kMaxHot * kMaxAcc);
     uint64_t* my_hot = s_hot + (tid >> 5) * kMaxHot * F::NA;
     uint32_t* my_hot_rows = s_hot_rows + (tid >> 5) * kMaxHot;
-    if (tid == 0) { s_count = 0; s_abort = 0; }
+    if (tid == 0) { s_count = 0; s_abort = 0; s_quit = 0; }
     const int64_t n_chunks = a.n / chunk;
     const int64_t mine = n_chunks > blockIdx.x ? (n_chunks - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
     __syncthreads();                                         // barriers initialised
@@ -577,10 +593,22 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
     auto run_chunks = [&](auto hot_c) {
       constexpr bool HOT = decltype(hot_c)::value;
       for (int64_t k = 0; k < mine; ++k, ++g_cons) {
-        // speculative run: look at the global give-up flag every 16th trip only (an L2 round trip each time)
-        if (a.spec) { if (__any_sync(0xffffffffu, missed || ((g_cons & 15u) == 0u && *reinterpret_cast<volatile uint32_t*>(&a.call->abort)))) break; }
+        // speculative run: look at the global give-up flag every 16th trip only (an L2 round trip each
+        // time).  A warp that leaves raises s_quit first: the producer and the warps still waiting for a
+        // chunk that will now never be requested must not wait for it.
+        if (a.spec) {
+          if (__any_sync(0xffffffffu, missed || ((g_cons & 15u) == 0u && *reinterpret_cast<volatile uint32_t*>(&a.call->abort)))) {
+            if (lane == 0) *reinterpret_cast<volatile uint32_t*>(&s_quit) = 1u;
+            break;
+          }
+        }
         const uint32_t s = g_cons % (uint32_t)a.stages;
-        mbar_wait(&s_full[s], (g_cons / (uint32_t)a.stages) & 1u);
+        {
+          const uint32_t par = (g_cons / (uint32_t)a.stages) & 1u;
+          bool gone = false;
+          while (!mbar_try_wait(&s_full[s], par)) { if (a.spec && *reinterpret_cast<volatile uint32_t*>(&s_quit)) { gone = true; break; } }
+          if (a.spec && __any_sync(0xffffffffu, gone)) break;      // warp-uniform: the lanes left the wait one by one
+        }
         const unsigned char* st = ring + (size_t)s * a.stage_bytes;
         U u[2]; uint64_t raw[2][NV];
         u[0] = ring_key<KK>(a, st, tid); u[1] = ring_key<KK>(a, st, T + tid);
@@ -588,8 +616,8 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
         __syncwarp();
         if (lane == 0) mbar_arrive(&s_empty[s]);             // this warp's rows are in registers: the stage may be refilled
         if (tid == 0 && (int64_t)g_issued < mine) {
-          ring_issue(a, ring, s_full, s_empty, g_issued, ((int64_t)blockIdx.x + (int64_t)g_issued * gridDim.x) * chunk, chunk, policy);
-          ++g_issued;
+          if (ring_issue(a, ring, s_full, s_empty, g_issued, ((int64_t)blockIdx.x + (int64_t)g_issued * gridDim.x) * chunk, chunk, policy, a.spec ? &s_quit : nullptr))
+            ++g_issued;
         }
         uint32_t miss;
         if constexpr (HOT) {
@@ -604,6 +632,7 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
     };
     if (a.n_hot) run_chunks(std::true_type{}); else run_chunks(std::false_type{});
     // a speculative run that gave up leaves bulk copies in flight: they must land before the CTA ends
+    // (every requested chunk completes its `full` phase whether or not anybody consumes it)
     if (tid == 0) for (uint32_t g = g_cons; g < g_issued; ++g) mbar_wait(&s_full[g % (uint32_t)a.stages], (g / (uint32_t)a.stages) & 1u);
     if (!(a.spec && __any_sync(0xffffffffu, missed))) {
       // ragged tail (fewer than `chunk` rows): row at a time, spread over the whole grid, warp-uniform trip count
@@ -725,7 +754,8 @@ int launch_one(const HashAggLaunch& L, cudaStream_t s) {
   const HashAggSmem lay = hash_agg_smem_layout(L.key, L.plan, L.key_kind, L.threads, L.hot_reserved && !IsPre<KK>::v, L.stages);
   for (int k = 0; k < kMaxKeyCols; ++k) { a.koff[k] = lay.koff[k]; a.kw[k] = lay.kw[k]; }
   for (int c = 0; c < kMaxVals; ++c) { a.voff[c] = lay.voff[c]; a.vw[c] = lay.vw[c]; }
-  a.stages = lay.stages; a.stage_bytes = lay.stage_bytes; a.n_src = lay.n_src; a.hot_off = lay.hot_off; a.table_off = lay.table_off;
+  a.stages = lay.stages; a.stage_bytes = lay.stage_bytes; a.n_src = lay.n_src;
+  { const char* e = std::getenv("EIGER_RING_HINT"); a.ring_hint = e ? std::atoi(e) : 1; } a.hot_off = lay.hot_off; a.table_off = lay.table_off;
   const size_t smem = (size_t)lay.table_off + L.table_smem_bytes;
   if (smem > 32 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<L.blocks, L.threads, smem, s>>>(a);

@@ -98,6 +98,7 @@ struct CompactLaunch {
   const void* table; uint64_t cap; uint32_t stride;
   void* out_keys[kMaxKeyCols]; void* out_aggs[kMaxAggs]; int n_out_aggs;
   int64_t out_capacity;
+  uint64_t R;               // fused key range (several key columns)
   CallDev* call;
 };
 int launch_compact(const CompactLaunch& c, int sm_count, cudaStream_t s);
@@ -162,5 +163,22 @@ struct PartitionLaunch {
 };
 int launch_partition(PartitionLaunch& p, int sm_count, size_t smem_optin, cudaStream_t s);
 int partition_max_bits_per_level();
+
+// ---- sortagg.cu -------------------------------------------------------------------------
+// EIGER_SORT: LSD radix sort of the rows on the `bits` significant bits of the rebased fused key,
+// then a segmented reduce that emits the groups in key order.
+struct SortLaunch {
+  KeyDesc key;
+  AggPlan plan;
+  int64_t n;
+  int key_kind, sig, bits;
+  void* keysA; void* valsA[kMaxVals];      // ping
+  void* keysB; void* valsB[kMaxVals];      // pong (two or more passes)
+  uint32_t* tile_hist;                     // [n / 1024 + 2][256]
+  unsigned long long* digit_base;          // [512]
+  void* out_keys[kMaxKeyCols]; void* out_aggs[kMaxAggs]; int n_out_aggs; int64_t out_capacity;
+  CallDev* call;
+};
+int launch_sort_groupby(SortLaunch& L, int sm_count, size_t smem_optin, cudaStream_t s);
 
 }  // namespace eiger

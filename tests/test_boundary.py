@@ -42,6 +42,13 @@ def test_host_estimator_matches_oracle(lib):
         got = eiger.hll_estimate(regs)
         want = oracle.hll_estimate(regs)
         assert got == pytest.approx(want, rel=1e-12, abs=1e-12)
+    # register arrays with many saturated registers: the tau term (zero on every real key set of these
+    # sizes) is exercised; the oracle's value on the same arrays is pinned to an exact evaluation of
+    # reading R5's formula in tests/test_oracle_hll.py
+    from test_oracle_hll import synthetic_register_arrays
+    for regs in synthetic_register_arrays():
+        got, want = eiger.hll_estimate(regs), oracle.hll_estimate(regs)
+        assert (got == want) if np.isinf(want) else got == pytest.approx(want, rel=1e-12), (got, want)
 
 
 def test_selector_is_callable_without_a_gpu(lib):
@@ -72,3 +79,9 @@ def test_selector_is_callable_without_a_gpu(lib):
         del os.environ["EIGER_GLOBAL_ALWAYS"]
     assert pick(-(1 << 31), (1 << 31) - 1, 1 << 26) == eiger.PARTITION
     assert eiger.workspace_bytes(fk, fv, aggs, [eiger.Stats(0, 15, 16.0, n)]) >= 256
+    # no statistics, several int32 / int64 key columns: the type ranges multiply past 2^64; the sizing
+    # call then bounds the group count by n instead of reporting bad arguments
+    fk2 = [Fake(keys[0], n), Fake(torch.zeros(1, dtype=torch.int64), n)]
+    assert eiger.workspace_bytes(fk2, fv, aggs) >= n * 8
+    fv32 = [Fake(torch.zeros(1, dtype=torch.int32), n)]
+    assert eiger.workspace_bytes(fk, fv32, aggs, [eiger.Stats(0, (1 << 31) - 1, float(1 << 26), n)], eiger.PARTITION) > 0

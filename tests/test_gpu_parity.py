@@ -11,7 +11,7 @@ from parity import assert_matches, oracle_result
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda:0"
-ALL_VARIANTS = [eiger.AUTO, eiger.DIRECT, eiger.SMEM, eiger.GLOBAL, eiger.PARTITION]
+ALL_VARIANTS = [eiger.AUTO, eiger.DIRECT, eiger.SMEM, eiger.GLOBAL, eiger.PARTITION, eiger.SORT]
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -58,6 +58,26 @@ def test_profile_parity(dtype, n):
     ws = oracle.profile(keys.numpy())
     assert (st.min, st.max, st.n) == (ws.min, ws.max, ws.n)
     assert st.ndv_est == pytest.approx(ws.ndv_est, rel=1e-12, abs=1e-12)
+
+
+def test_sketch_registers_deep_zero_runs_and_rho_cap():
+    # keys constructed (by inverting the sketch hash, tests/test_oracle_hll.py) so that the remaining
+    # 50 hash bits start with 31, 32, 33, 48, 49 zeros or are all zero: reaches the kernel's `wh == 0`
+    # branch (profile.cu: hll_update), which random keys take once per 2^32
+    from test_oracle_hll import deep_zero_keys
+    cases = deep_zero_keys()
+    filler = torch.arange(5000, dtype=torch.int64) * 7919 - 123456
+    keys = torch.cat([torch.tensor([c[0] for c in cases], dtype=torch.int64), filler, torch.tensor([c[0] for c in cases], dtype=torch.int64)])
+    want = oracle.hll_registers(keys.numpy())
+    for _, idx, rho in cases:
+        assert int(want[idx]) >= rho
+    got = eiger.hll_registers(keys.to(DEV)).cpu().numpy()
+    assert np.array_equal(got, want) and int(got.max()) == 51
+    only = torch.tensor([c[0] for c in cases], dtype=torch.int64)
+    got = eiger.hll_registers(only.to(DEV)).cpu().numpy()
+    assert {int(i): int(got[i]) for i in np.flatnonzero(got)} == {idx: rho for _, idx, rho in cases}
+    st, ws = eiger.profile(keys.to(DEV)), oracle.profile(keys.numpy())
+    assert st.ndv_est == pytest.approx(ws.ndv_est, rel=1e-12)
 
 
 @pytest.mark.parametrize("lg,scattered", [(4, False), (12, True), (16, False), (20, True)])
@@ -169,12 +189,13 @@ def test_generic_signatures():
     vf = torch.randint(0, 1 << 53, (n,), generator=g, dtype=torch.int64).to(torch.float64) * 2.0 ** -53
     vneg = -vf - 1.0
     aggs = [(eiger.MIN, 1), (eiger.MAX, 0), (eiger.SUM, 1), (eiger.MAX, 2), (eiger.MIN, 2), (eiger.SUM, 0)]   # no COUNT
-    ds = datagen.Dataset("gen", n, [k0, k1], [vi, vf, vneg], aggs, exact_f64_sum=False)
+    # vf = k 2^-53: the oracle sums it exactly (128-bit integers, one rounding), tolerance 1e-12
+    ds = datagen.Dataset("gen", n, [k0, k1], [vi, vf, vneg], aggs, exact_f64_sum=True)
     want = oracle_result(ds)
     d = to_dev(ds)
     for f in ALL_VARIANTS:
         res = eiger.groupby(d.keys, d.vals, d.aggs, force=f)
-        assert_matches(res, want, d.aggs, d.vals, rel=1e-9)          # sequential-sum oracle here
+        assert_matches(res, want, d.aggs, d.vals)
     # single int8 key, COUNT only
     ds = datagen.Dataset("cnt", n, [k0], [], [(eiger.COUNT, 0)])
     run_all_variants(ds)
@@ -493,3 +514,78 @@ def test_multi_key_tiny_and_ragged(n):
     if n:
         st = eiger.profile_keys([k0.to(DEV), k1.to(DEV), k2.to(DEV)])
         assert [(s.min, s.max) for s in st] == [(int(k.min()), int(k.max())) for k in (k0, k1, k2)]
+
+
+# ---- statistics supplied by the caller, int64 margins, int32 payloads ---------------------------------
+def test_auto_takes_direct_on_dense_nonnegative_int64_keys():
+    # the slack added around the sampled range is clamped to the key type in unsigned arithmetic
+    # (min - INT64_MIN overflowed int64 for every min >= 0 and sent such columns to PARTITION)
+    ds = datagen.config5(n=SPEC_N, ndv=1 << 12)
+    ds = datagen.Dataset("dense-i64", ds.n, [ds.keys[0].to(torch.int64) + 5], ds.vals, ds.aggs, ds.ndv)
+    _auto_matches(ds, eiger.DIRECT)
+    ds = datagen.Dataset("dense-i64-neg", ds.n, [ds.keys[0] - (1 << 40)], ds.vals, ds.aggs, ds.ndv)
+    _auto_matches(ds, eiger.DIRECT)
+
+
+def test_stale_statistics_are_detected_not_trusted():
+    # statistics profiled on another batch: a direct-index array would be indexed out of bounds, a
+    # fused multi-column key would alias onto another group -> EIGER_ERR_STATS, nothing is written
+    n = 300_007
+    i = torch.arange(n, dtype=torch.int64)
+    keys = (i % 1000).to(torch.int32).to(DEV)
+    vals = i.to(DEV)
+    aggs = [(eiger.SUM, 0), (eiger.COUNT, 0)]
+    good = eiger.profile(keys)
+    stale = [eiger.Stats(0, 499, 500.0, n)]
+    for stats, sig in ((stale, aggs), (stale, aggs + [(eiger.MIN, 0)])):
+        with pytest.raises(eiger.EigerError) as e:
+            eiger.groupby([keys], [vals], sig, force=eiger.DIRECT, stats=stats)
+        assert e.value.code == eiger.ERR_STATS
+    big = [eiger.Stats(0, 99_999, 1000.0, n)]                      # global-atomics flavour of DIRECT
+    keys2 = keys.clone(); keys2[n // 2] = 100_000
+    with pytest.raises(eiger.EigerError) as e:
+        eiger.groupby([keys2], [vals], aggs, force=eiger.DIRECT, stats=big)
+    assert e.value.code == eiger.ERR_STATS
+    assert eiger.groupby([keys], [vals], aggs, force=eiger.DIRECT, stats=[good]).n_groups == 1000
+    # single-column hash variants rebase modulo 2^32: stale bounds are harmless there
+    for f in (eiger.SMEM, eiger.GLOBAL, eiger.PARTITION):
+        assert eiger.groupby([keys], [vals], aggs, force=f, stats=[eiger.Stats(0, 499, 1000.0, n)]).n_groups == 1000
+    # two key columns, the second one's statistics too narrow
+    k1 = ((i // 1000) % 7).to(torch.int32).to(DEV)
+    st2 = [eiger.Stats(0, 999, 1000.0, n), eiger.Stats(0, 3, 4.0, n)]
+    for f in (eiger.DIRECT, eiger.SMEM, eiger.GLOBAL, eiger.PARTITION):      # (EIGER_SORT maps such rows to the marker key: one extra group)
+        with pytest.raises(eiger.EigerError) as e:
+            eiger.groupby([keys, k1], [vals], aggs, force=f, stats=st2)
+        assert e.value.code == eiger.ERR_STATS, f
+    ok = eiger.groupby([keys, k1], [vals], aggs, stats=eiger.profile_keys([keys, k1]))
+    assert ok.n_groups == 7000
+
+
+@pytest.mark.parametrize("kdtype", [torch.int32, torch.int64])
+def test_int32_value_columns(kdtype):
+    # 4-byte payloads ("both 4-byte data types (I32) and 8-byte"): widened on the fly,
+    # results are int64 like the oracle's (which widens before it aggregates)
+    n = (1 << 21) + 77
+    for lg, scattered in ((6, False), (11, True), (17, True), (17, False)):
+        ds = datagen.config5(n=n, ndv=1 << lg, scattered=scattered)
+        v32 = (ds.vals[0] - (1 << 30)).to(torch.int32)                       # negative values too
+        ds = datagen.Dataset(f"i32-{lg}", n, [ds.keys[0].to(kdtype)], [v32], [(eiger.SUM, 0), (eiger.COUNT, 0)], ds.ndv)
+        run_all_variants(ds)
+    v2 = datagen.uniform_int(21, 2, torch.arange(n, dtype=torch.int64), -(1 << 30), (1 << 30) - 2).to(torch.int32) * 2 + 1
+    vf = datagen.unit_f64(21, 3, torch.arange(n, dtype=torch.int64))
+    ds = datagen.config5(n=n, ndv=3000, scattered=True)
+    ds = datagen.Dataset("i32-mixed", n, [ds.keys[0].to(kdtype)], [v2, ds.vals[0], vf],
+                         [(eiger.SUM, 0), (eiger.MIN, 0), (eiger.MAX, 0), (eiger.COUNT, 0), (eiger.SUM, 1), (eiger.SUM, 2), (eiger.MAX, 2)],
+                         exact_f64_sum=True)
+    run_all_variants(ds)
+
+
+def test_int32_values_host_entry_point_and_two_keys():
+    ds = datagen.config_mk(n=300_011, nk=2, digit_bits=5)
+    v32 = (ds.vals[0] % 100_003 - 50_000).to(torch.int32)
+    ds = datagen.Dataset("mk-i32", ds.n, ds.keys, [v32], [(eiger.SUM, 0), (eiger.COUNT, 0)], ds.ndv)
+    run_all_variants(ds)
+    want = oracle_result(ds)
+    res, h2d, d2h = eiger.groupby_host(ds.keys, ds.vals, ds.aggs)
+    assert_matches(res, want, ds.aggs, ds.vals)
+    assert h2d == ds.n * (4 + 4 + 4)

@@ -56,11 +56,66 @@ def test_registers_match_big_integer_rederivation():
     assert np.array_equal(oracle.hll_registers(keys), want)
 
 
-def test_rho_cap_when_remaining_bits_are_zero():
-    # invert the mixer's last step is not needed: search a hash with w == 0 is infeasible, so
-    # check the cap through p: with p = 4 the same code path caps at 64 - 4 + 1 = 61
-    regs = oracle.hll_registers(np.arange(100000, dtype=np.int64), p=4)
-    assert regs.max() <= 61 and regs.min() >= 1
+def _unxorshift(z: int, k: int) -> int:
+    """inverse of z ^= z >> k on 64 bits"""
+    x = z
+    for _ in range(64 // k + 1):
+        x = z ^ (x >> k)
+    return x
+
+
+INV1 = pow(0xBF58476D1CE4E5B9, -1, 1 << 64)
+INV2 = pow(0x94D049BB133111EB, -1, 1 << 64)
+
+
+def key_with_hash(h: int) -> int:
+    """The int64 key whose sketch hash is exactly h: the splitmix64 output function is a bijection
+    (two odd multipliers, three xor-shifts, one addition), inverted step by step."""
+    z = _unxorshift(h & MASK, 31)
+    z = (z * INV2) & MASK
+    z = _unxorshift(z, 27)
+    z = (z * INV1) & MASK
+    z = _unxorshift(z, 30)
+    x = (z - 0x9E3779B97F4A7C15) & MASK
+    return x - (1 << 64) if x >= (1 << 63) else x
+
+
+def deep_zero_keys():
+    """Keys whose hash has a chosen register index and a chosen number of leading zeros in the
+    remaining 50 bits: 0, 1, 17, 31, 32, 33, 48, 49 zeros, and all 50 zero (w = 0: rho = 51, the cap of
+    reading R3).  By chance such hashes turn up once per 2^32 .. 2^50 keys."""
+    rng = np.random.default_rng(7)
+    out = []
+    for j, lz in enumerate([0, 1, 17, 31, 32, 33, 48, 49, 50]):
+        idx = 1000 + 37 * j
+        if lz == 50:
+            rest = 0
+        else:
+            low_bits = 49 - lz
+            rest = (1 << low_bits) | (int(rng.integers(0, 1 << low_bits)) if low_bits else 0)
+        h = (idx << 50) | rest
+        out.append((key_with_hash(h), idx, lz + 1))
+    return out
+
+
+def test_rho_cap_and_deep_zero_runs():
+    # (SURVEY.md C.3 step 4 / DESIGN.md R3: rho = min(clz64(w), 50) + 1, so w = 0 gives 51)
+    cases = deep_zero_keys()
+    for key, idx, rho in cases:
+        assert oracle.hash64(key) >> 50 == idx
+        assert py_idx_rho(key) == (idx, rho)
+        regs = oracle.hll_registers(np.array([key], dtype=np.int64))
+        assert np.flatnonzero(regs).tolist() == [idx] and int(regs[idx]) == rho
+    keys = np.array([c[0] for c in cases], dtype=np.int64)
+    regs = oracle.hll_registers(keys)
+    want = np.zeros(M, dtype=np.uint8)
+    for _, idx, rho in cases:
+        want[idx] = rho
+    assert np.array_equal(regs, want) and int(regs.max()) == 64 - P + 1
+    # the cap again through another precision: p = 4 caps at 64 - 4 + 1 = 61
+    k0 = key_with_hash(0x3 << 60)                      # idx 3, remaining 60 bits all zero
+    r4 = oracle.hll_registers(np.array([k0], dtype=np.int64), p=4)
+    assert int(r4[3]) == 61 and int(r4.sum()) == 61
 
 
 def test_register_set_invariants():
@@ -158,3 +213,76 @@ def test_profile_clamps():
     assert (s.min, s.max, s.n) == (100, 163, 64) and 60 <= s.ndv_est <= 64
     e = oracle.profile(np.zeros(0, dtype=np.int64))
     assert e.ndv_est == 0.0 and e.n == 0
+
+
+# ---- estimator (reading R5) against an exact evaluation of the same formula --------------------
+def _exact_estimate(hist, p=P):
+    """z = m tau(1 - C[q+1]/m); for k = q..1: z = (z + C[k]) / 2; z += m sigma(C[0]/m);
+    est = m^2 / (2 ln2 z), evaluated with 60 significant digits (mpmath), series summed to 1e-50."""
+    import mpmath as mp
+    mp.mp.dps = 60
+    m, q = mp.mpf(1 << p), 64 - p
+
+    def sigma(x):
+        if x == 1:
+            return mp.inf
+        z, y = x, mp.mpf(1)
+        for _ in range(400):
+            x = x * x
+            t = x * y
+            z += t
+            y += y
+            if t < mp.mpf(10) ** -50:
+                break
+        return z
+
+    def tau(x):
+        if x == 0 or x == 1:
+            return mp.mpf(0)
+        z, y = 1 - x, mp.mpf(1)
+        for _ in range(400):
+            x = mp.sqrt(x)
+            y *= mp.mpf(1) / 2
+            t = (1 - x) ** 2 * y
+            z -= t
+            if t < mp.mpf(10) ** -50:
+                break
+        return z / 3
+
+    z = m * tau(1 - mp.mpf(int(hist[q + 1])) / m)
+    for k in range(q, 0, -1):
+        z = (z + int(hist[k])) / 2
+    z += m * sigma(mp.mpf(int(hist[0])) / m)
+    if z == 0:
+        return math.inf              # every register saturated
+    return float(m * m / (2 * mp.log(2) * z))
+
+
+def synthetic_register_arrays():
+    """Register arrays no real key set of this size produces: many saturated registers (51), so that
+    the tau term is far from its trivial value tau(1) = 0, next to zeros and mid values."""
+    rng = np.random.default_rng(11)
+    arrays = []
+    for frac51, frac0 in [(0.0, 0.0), (0.01, 0.0), (0.25, 0.1), (0.5, 0.0), (0.9, 0.05), (0.999, 0.0), (1.0, 0.0), (0.0, 0.999), (0.3, 0.69)]:
+        r = rng.integers(1, 51, size=M).astype(np.uint8)
+        sel = rng.random(M)
+        r[sel < frac51] = 51
+        r[(sel >= frac51) & (sel < frac51 + frac0)] = 0
+        if frac51 == 1.0:
+            r[:] = 51
+        arrays.append(r)
+    arrays.append(rng.integers(0, 52, size=M).astype(np.uint8))         # uniform over 0 .. 51
+    arrays.append(np.minimum(rng.geometric(0.5, size=M) + 40, 51).astype(np.uint8))   # piled up at the cap
+    return arrays
+
+
+def test_estimator_matches_exact_formula_including_tau():
+    for regs in synthetic_register_arrays():
+        hist = np.bincount(regs, minlength=64)
+        want = _exact_estimate(hist)
+        got = oracle.hll_estimate(regs)
+        assert (got == want) if math.isinf(want) else got == pytest.approx(want, rel=1e-12), (hist[0], hist[51], got, want)
+    # tau is really exercised: saturating registers moves the estimate
+    base = np.full(M, 30, dtype=np.uint8)
+    sat = base.copy(); sat[: M // 2] = 51
+    assert oracle.hll_estimate(sat) > 1.5 * oracle.hll_estimate(base)
