@@ -76,6 +76,7 @@ struct Tunables {
   int sdirect_max_replicas, sdirect_wide;
   size_t smem_total;                  // dynamic shared memory of one hash-aggregation CTA: ring + table (1 CTA per SM)
   int stages;                         // stages of the shared-memory ring the rows stream through (ring.cuh)
+  int ring;                           // bit 0: whole-input hash kernels, bit 1: per-partition aggregation take their rows from the ring
   size_t smem_table_bytes;            // EIGER_SMEM / EIGER_GLOBAL: shared-memory table of one CTA; 0 = what the ring leaves of smem_total
   int smem_threads;
   size_t part_table_bytes;            // EIGER_PARTITION: the same for the per-partition tables
@@ -104,6 +105,7 @@ struct Tunables {
     priv_max_range = (int)env("EIGER_PRIV_MAX_RANGE", 6);
     smem_total = (size_t)env("EIGER_SMEM_TOTAL_KB", 225) << 10;
     stages = (int)env("EIGER_STAGES", kDefaultStages);
+    ring = (int)env("EIGER_RING", 0);
     smem_table_bytes = (size_t)env("EIGER_SMEM_KB", 0) << 10;
     sdirect_replica_budget = (size_t)env("EIGER_SDIRECT_REPLICA_KB", 64) << 10;
     sdirect_max_replicas = (int)env("EIGER_SDIRECT_MAX_REPLICAS", 8);
@@ -149,6 +151,7 @@ struct QueryPlan {
   size_t smem_bytes = 0;        // direct variants: the CTA's array; hash variants: the CTA's table
   size_t smem_dyn = 0;          // hash variants: ring + table
   int stages = 0;
+  bool ring = false;
   bool hot_reserved = false;
   uint64_t cap = 0, cap_bound = 0, cap_hot = 0;
   uint32_t stride = 0;
@@ -277,6 +280,8 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   const int pre_kind = (hkp == KK_I32 || hkp == KK_GEN32) ? KK_U32PRE : KK_U64PRE;
   auto table_bytes_for = [&](int kind, int threads, bool hot, size_t fixed) {
     if (fixed) return fixed;
+    const bool pre = kind == KK_U32PRE || kind == KK_U64PRE;
+    if (!(T.ring & (pre ? 2 : 1))) return pre ? (size_t)200 << 10 : ((size_t)200 << 10);     // per-thread loads: the table is the whole allocation (heavy-hitter cells are static)
     const HashAggSmem lay = hash_agg_smem_layout(kd, p, kind, threads, hot, T.stages);
     return T.smem_total > lay.table_off + 4096 ? T.smem_total - lay.table_off : (size_t)4096;
   };
@@ -373,7 +378,8 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
     }
     q->smem_bytes = align_up((size_t)q->slots * (variant == EIGER_PARTITION ? part_slot_bytes : slot_bytes) + 64, 16);
     q->stages = T.stages; q->hot_reserved = variant != EIGER_PARTITION && want_hot;
-    q->smem_dyn = q->smem_bytes + hash_agg_smem_layout(kd, p, variant == EIGER_PARTITION ? pre_kind : hk, q->threads, q->hot_reserved, T.stages).table_off;
+    q->ring = (T.ring & (variant == EIGER_PARTITION ? 2 : 1)) != 0;
+    q->smem_dyn = q->smem_bytes + (q->ring ? hash_agg_smem_layout(kd, p, variant == EIGER_PARTITION ? pre_kind : hk, q->threads, q->hot_reserved, T.stages).table_off : 0);
     q->table_bytes = align_up((size_t)(q->cap + 1) * q->stride, 256);
   }
   q->total_bytes = q->table_bytes + q->part_bytes + 256;
@@ -535,14 +541,14 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       H.key = q.key; H.plan = q.plan; H.n = n; H.key_kind = src_kind; H.sig = q.sig;
       H.slots = q.slots; H.limit = q.limit; H.spec = spec;
       H.max_probes = q.variant == EIGER_GLOBAL ? T_front_probes : 0;
-      H.n_hot = (!spec && nk == 1 && q.variant != EIGER_PARTITION && q.hot_reserved) ? hot_n : 0;
+      H.n_hot = (!spec && nk == 1 && q.variant != EIGER_PARTITION && (q.hot_reserved || !q.ring)) ? hot_n : 0;
       for (int i = 0; i < H.n_hot; ++i) H.hot[i] = (uint64_t)hot_key[i] - q.key.base[0];
       if (H.n_hot && src_kind == KK_I32) for (int i = 0; i < H.n_hot; ++i) H.hot[i] &= 0xFFFFFFFFull;
       H.table = table; H.cap = q.cap; H.stride = q.stride; H.call = rt->call;
       for (int k = 0; k < kMaxKeyCols; ++k) H.out_keys[k] = k < nk ? out_keys[k] : nullptr;
       for (int j = 0; j < na; ++j) H.out_aggs[j] = out_aggs[j];
       H.n_out_aggs = na; H.out_capacity = out_capacity;
-      H.threads = q.threads; H.table_smem_bytes = q.smem_bytes; H.stages = q.stages; H.hot_reserved = q.hot_reserved;
+      H.threads = q.threads; H.table_smem_bytes = q.smem_bytes; H.stages = q.stages; H.hot_reserved = q.hot_reserved; H.ring = q.ring ? 1 : 0;
       {   // 32-bit keys in a nearly empty shared-memory table: 8-byte buckets (hashagg.cuh: BK)
         const double per_table = q.variant == EIGER_PARTITION ? q.ndv / (double)((size_t)1 << (q.bits1 + q.bits2)) : q.ndv;
         H.bucket_keys = ((src_kind == KK_I32 || src_kind == KK_GEN32) && q.variant != EIGER_GLOBAL && per_table <= tun().narrow_load * q.slots) ? 2 : 0;

@@ -738,9 +738,187 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
   }
 }
 
+// ---- the same kernel with the rows loaded by the threads themselves (16-byte streaming loads into
+// registers, the next tile's loads in flight while the current one is processed).  The kernel is bound
+// by the shared-memory pipe (bucket look-ups + atomics); rows that arrive through the shared-memory
+// ring cost it 6 more wavefronts per 32 rows (the bulk copy's write + the threads' reads), so the ring
+// version is the slower one wherever the table work dominates (measured; EIGER_RING selects). ----
+template <int KK, int SIG, int BK>
+__global__ void __launch_bounds__(kMaxThreads, 1)
+hash_agg_ldg_kernel(const __grid_constant__ HashAggArgs a) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ uint32_t s_count, s_abort, s_spilled;
+  __shared__ uint32_t s_wtot[32];
+  __shared__ unsigned long long s_base;
+  using F = Front<KK, SIG, BK>;
+  using U = typename F::U;
+  constexpr int NV = F::NV;
+  const int tid = threadIdx.x, T = blockDim.x;
+  const int n_vals = Sig<SIG>::kStatic ? NV : a.plan.n_vals;
+
+  if constexpr (!IsPre<KK>::v) {
+    // ---- whole-input mode: tiles of 2 * T * UNR rows, grid-strided; the next tile's loads are
+    // in flight while the current one is processed (one CTA per SM: there is nobody else to
+    // hide HBM latency behind) ----
+    constexpr int UNR = !Sig<SIG>::kStatic ? 1 : (NV >= 4 ? 1 : (sizeof(U) == 8 ? 1 : 2));   // 3 spills at the 64-register cap
+    F f(a, smem, a.slots);
+    __shared__ uint64_t s_hot[(kMaxThreads / 32) * kMaxHot * F::NA];
+    __shared__ uint32_t s_hot_rows[(kMaxThreads / 32) * kMaxHot];
+    uint64_t* my_hot = s_hot + (tid >> 5) * kMaxHot * F::NA;
+    uint32_t* my_hot_rows = s_hot_rows + (tid >> 5) * kMaxHot;
+    if (tid == 0) { s_count = 0; s_abort = 0; }
+    f.init(tid, T);
+    if (a.n_hot) f.hot_init(s_hot, s_hot_rows, tid, T);
+    __syncthreads();
+    const int64_t step = 2 * (int64_t)T, tile = step * UNR;
+    const int64_t n_tiles = a.n / tile;
+    bool missed = false;
+    U u[2][2 * UNR];
+    uint64_t raw[2][2 * UNR][NV];
+    auto load_tile = [&](int b, int64_t t) {
+      const int64_t r0 = t * tile + 2 * tid;
+#pragma unroll
+      for (int s = 0; s < UNR; ++s) {
+        { U uu[2]; load_u2<KK>(a.key, r0 + s * step, uu); u[b][2 * s] = uu[0]; u[b][2 * s + 1] = uu[1]; }
+#pragma unroll
+        for (int c = 0; c < NV; ++c) {
+          if (!Sig<SIG>::kStatic && c >= n_vals) { raw[b][2 * s][c] = 0; raw[b][2 * s + 1][c] = 0; continue; }
+          global_val2(a.plan, c, sig_vw<SIG>(a.plan, c), r0 + s * step, raw[b][2 * s][c], raw[b][2 * s + 1][c]);
+        }
+      }
+    };
+    // the tile loop, compiled twice: with and without the heavy-hitter look (runtime row-valid flags
+    // and the hot-key scan cost the plain path 5-15 % at low NDV when they were merely branched over)
+    auto run_tiles = [&](auto hot_c) {
+      constexpr bool HOT = decltype(hot_c)::value;
+      auto process_tile = [&](int b) {
+        uint32_t miss = 0;
+        if constexpr (HOT) {
+          bool ab[2 * UNR];
+#pragma unroll
+          for (int r = 0; r < 2 * UNR; ++r) ab[r] = f.hot_absorb(u[b][r], raw[b][r], my_hot, my_hot_rows, tid & 31);
+#pragma unroll
+          for (int s = 0; s < UNR; ++s) miss |= f.pair(u[b][2 * s], raw[b][2 * s], !ab[2 * s], u[b][2 * s + 1], raw[b][2 * s + 1], !ab[2 * s + 1], &s_count) << (2 * s);
+        } else {
+#pragma unroll
+          for (int s = 0; s < UNR; ++s) miss |= f.pair(u[b][2 * s], raw[b][2 * s], true, u[b][2 * s + 1], raw[b][2 * s + 1], true, &s_count) << (2 * s);
+        }
+        f.spill(u[b], raw[b], miss, missed);
+      };
+      int64_t t = blockIdx.x;
+      uint32_t trip = 0;
+      if (t < n_tiles) load_tile(0, t);
+      while (t < n_tiles) {
+        // speculative run: look at the global give-up flag every 16th trip only (an L2 round trip each time)
+        if (a.spec) { if (__any_sync(0xffffffffu, missed || ((trip++ & 15u) == 0u && *reinterpret_cast<volatile uint32_t*>(&a.call->abort)))) break; }
+        if (t + gridDim.x < n_tiles) load_tile(1, t + gridDim.x);
+        process_tile(0);
+        t += gridDim.x;
+        if (t >= n_tiles) break;
+        if (t + gridDim.x < n_tiles) load_tile(0, t + gridDim.x);
+        process_tile(1);
+        t += gridDim.x;
+      }
+    };
+    if (a.n_hot) run_tiles(std::true_type{}); else run_tiles(std::false_type{});
+    if (!(a.spec && __any_sync(0xffffffffu, missed))) {
+      // ragged tail: row at a time, spread over the whole grid, warp-uniform trip count
+      const int lane = tid & 31;
+      for (int64_t i0 = n_tiles * tile + (int64_t)blockIdx.x * T + (tid - lane); i0 < a.n; i0 += (int64_t)gridDim.x * T) {
+        const int64_t i = i0 + lane;
+        uint64_t rawt[NV];
+        U ut = 0;
+        if (i < a.n) {
+#pragma unroll
+          for (int c = 0; c < NV; ++c) rawt[c] = (Sig<SIG>::kStatic || c < n_vals) ? global_val(a.plan, c, sig_vw<SIG>(a.plan, c), i) : 0ull;
+          ut = load_u<KK>(a.key, i);
+        }
+        const uint32_t miss = f.pair(ut, rawt, i < a.n, ut, rawt, false, &s_count);
+        if (__any_sync(0xffffffffu, miss != 0)) { if (a.spec) missed = missed || miss != 0; else if (miss) f.back_row(ut, rawt); }
+        __syncwarp();
+      }
+    }
+    if (a.spec) {
+      if (missed) { atomicOr(&a.call->abort, 1u); atomicOr(&s_abort, 1u); }
+      __syncthreads();
+      if (s_abort || *reinterpret_cast<volatile uint32_t*>(&a.call->abort)) return;   // result is discarded
+    } else {
+      __syncthreads();
+    }
+    f.flush_merge(tid, T);
+    if (a.n_hot) f.hot_flush(s_hot, s_hot_rows, tid, T);
+  } else {
+    // ---- partition mode: work items blockIdx.x, + gridDim.x, ...; an item is a whole partition
+    // (this CTA then owns its keys and emits them) or a slice of a hot one (merged through the
+    // global table like the whole-input mode) ----
+    const unsigned long long n_items = a.item_off[a.n_parts];
+    for (unsigned long long it = blockIdx.x; it < n_items; it += gridDim.x) {
+      // the partition of item `it`: one broadcast load from the map written by part_items_kernel
+      const int p = (int)a.item_part[it];
+      const unsigned long long n_chunks = a.item_off[p + 1] - a.item_off[p], ci = it - a.item_off[p];
+      const int64_t P0 = (int64_t)a.part_off[p], P1 = (int64_t)a.part_off[p + 1];
+      const int64_t per = (P1 - P0 + (int64_t)n_chunks - 1) / (int64_t)n_chunks;
+      const int64_t r0 = P0 + (int64_t)ci * per, r1 = r0 + per < P1 ? r0 + per : P1;
+      const bool exclusive = n_chunks == 1;
+      // a table no larger than the partition needs: 2 slots per row is always enough
+      const uint64_t want = 2ull * (uint64_t)(r1 - r0) + 64;
+      const uint32_t Sn = (uint32_t)(want < a.slots ? want : a.slots) & ~7u;   // whole buckets
+      F f(a, smem, Sn);
+      f.s_spill = &s_spilled;
+      __syncthreads();                       // the previous partition's emit is over
+      if (tid == 0) { s_count = 0; s_spilled = 0; }
+      f.init(tid, T);
+      __syncthreads();
+      bool missed = false;
+      // chunks of UNR * T rows, bounds-checked per row; the next chunk loads while this one is processed
+      constexpr int UNR = NV >= 4 ? 1 : 2;
+      U u[2][UNR];
+      uint64_t raw[2][UNR][NV];
+      const int64_t chunk = (int64_t)UNR * T;
+      auto load_chunk = [&](int b, int64_t c0) {
+#pragma unroll
+        for (int s = 0; s < UNR; ++s) {
+          const int64_t i = c0 + (int64_t)s * T + tid;
+          if (i < r1) {
+            u[b][s] = load_u<KK>(a.key, i);
+#pragma unroll
+            for (int c = 0; c < NV; ++c) raw[b][s][c] = (Sig<SIG>::kStatic || c < n_vals) ? global_val(a.plan, c, sig_vw<SIG>(a.plan, c), i) : 0ull;
+          }
+        }
+      };
+      auto process_chunk = [&](int b, int64_t c0) {
+        uint32_t miss = 0;
+#pragma unroll
+        for (int s = 0; s < UNR; s += 2) {
+          const bool v0 = c0 + (int64_t)s * T + tid < r1, v1 = (s + 1 < UNR) && (c0 + (int64_t)(s + 1) * T + tid < r1);
+          miss |= f.pair(v0 ? u[b][s] : (U)0, raw[b][s], v0, v1 ? u[b][s + 1 < UNR ? s + 1 : s] : (U)0, raw[b][s + 1 < UNR ? s + 1 : s], v1, &s_count) << s;
+        }
+        f.spill(u[b], raw[b], miss, missed);
+      };
+      int64_t c0 = r0;
+      load_chunk(0, c0);
+      while (c0 < r1) {
+        if (c0 + chunk < r1) load_chunk(1, c0 + chunk);
+        process_chunk(0, c0);
+        c0 += chunk;
+        if (c0 >= r1) break;
+        if (c0 + chunk < r1) load_chunk(0, c0 + chunk);
+        process_chunk(1, c0);
+        c0 += chunk;
+      }
+      __syncthreads();
+      // emit only what this CTA owns exclusively: a whole partition none of whose rows was sent to
+      // the global table (otherwise a key could be emitted here AND by the compaction pass)
+      if (exclusive && s_spilled == 0u) f.flush_emit(tid, T, s_count, &s_base, s_wtot);
+      else f.flush_merge(tid, T);
+    }
+  }
+}
+
+
 template <int KK, int SIG, int BK>
 int launch_one(const HashAggLaunch& L, cudaStream_t s) {
-  auto kern = hash_agg_kernel<KK, SIG, BK>;
+  auto kern = L.ring ? hash_agg_kernel<KK, SIG, BK> : hash_agg_ldg_kernel<KK, SIG, BK>;
   HashAggArgs a;
   a.key = L.key; a.plan = L.plan; a.n = L.n; a.part_off = L.part_off; a.item_off = L.item_off; a.item_part = L.item_part; a.n_parts = L.n_parts;
   a.slots = L.slots; a.limit = L.limit; a.spec = L.spec; a.max_probes = L.max_probes > 0 ? L.max_probes : 16;
@@ -751,7 +929,8 @@ int launch_one(const HashAggLaunch& L, cudaStream_t s) {
   for (int j = 0; j < kMaxAggs; ++j) a.out_aggs[j] = static_cast<uint64_t*>(L.out_aggs[j]);
   a.n_out = L.n_out_aggs; a.out_capacity = L.out_capacity;
   // dynamic shared memory: [ring: stages x stage_bytes][heavy-hitter cells][table]
-  const HashAggSmem lay = hash_agg_smem_layout(L.key, L.plan, L.key_kind, L.threads, L.hot_reserved && !IsPre<KK>::v, L.stages);
+  HashAggSmem lay = hash_agg_smem_layout(L.key, L.plan, L.key_kind, L.threads, L.hot_reserved && !IsPre<KK>::v, L.stages);
+  if (!L.ring) { lay.table_off = 0; lay.hot_off = 0; }     // no ring: the table is all of the dynamic shared memory
   for (int k = 0; k < kMaxKeyCols; ++k) { a.koff[k] = lay.koff[k]; a.kw[k] = lay.kw[k]; }
   for (int c = 0; c < kMaxVals; ++c) { a.voff[c] = lay.voff[c]; a.vw[c] = lay.vw[c]; }
   a.stages = lay.stages; a.stage_bytes = lay.stage_bytes; a.n_src = lay.n_src;

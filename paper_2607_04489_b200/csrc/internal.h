@@ -122,7 +122,8 @@ struct HashAggLaunch {
   CallDev* call;
   void* out_keys[kMaxKeyCols]; void* out_aggs[kMaxAggs]; int n_out_aggs; int64_t out_capacity;   // partition mode emits
   int threads, blocks;
-  int stages;               // shared-memory ring stages (ring.cuh); 0 = default
+  int ring;                 // rows arrive through the shared-memory ring (ring.cuh) instead of per-thread loads
+  int stages;               // shared-memory ring stages; 0 = default
   bool hot_reserved;        // room for the heavy-hitter cells is part of the layout (EIGER_GLOBAL)
   size_t table_smem_bytes;  // shared-memory table of one CTA
 };

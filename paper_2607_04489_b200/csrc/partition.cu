@@ -317,6 +317,166 @@ part_scatter_kernel(const __grid_constant__ ScatterArgs A) {
   }
 }
 
+// ---- the round-1 scatter: the threads load their own rows (8 per thread, 4096-row tiles, two CTAs
+// per SM, the next tile prefetched into L2); 8-byte value columns only.  Kept selectable
+// (EIGER_SCATTER_RING=0) for same-box comparisons with the ring version above. ----
+template <int KK, class UO>
+__global__ void __launch_bounds__(kPT, kScatterCtas)
+part_scatter_ldg_kernel(const __grid_constant__ LevelArgs a) {
+  using U = typename SrcKey<KK>::U;
+  // dynamic shared memory (above the 48 KB static limit): staging buffers, then the counters
+  extern __shared__ __align__(16) unsigned char dsm[];
+  uint64_t* s_val = reinterpret_cast<uint64_t*>(dsm);
+  UO* s_key = reinterpret_cast<UO*>(dsm + sizeof(uint64_t) * kTile);
+  long long* s_delta = reinterpret_cast<long long*>(dsm + (sizeof(uint64_t) + sizeof(UO)) * kTile);
+  uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_delta + kMaxFan);
+  uint32_t* s_loff = s_cnt + kMaxFan;
+  uint16_t* s_pid = reinterpret_cast<uint16_t*>(s_loff + kMaxFan);
+  __shared__ uint32_t s_warp[kPT / 32];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, seg = blockIdx.y;
+  const int fan = a.fan;
+  const uint32_t mask = (uint32_t)fan - 1u;
+  const int64_t r0 = a.seg_off ? (int64_t)a.seg_off[seg] : 0, r1 = a.seg_off ? (int64_t)a.seg_off[seg + 1] : a.n;
+  unsigned long long* cursor = a.cursor + (size_t)seg * fan;
+  UO* out_keys = static_cast<UO*>(a.out_keys);
+  for (int p = tid; p < fan; p += kPT) s_cnt[p] = 0;
+  __syncthreads();
+  const int64_t n_tiles = (r1 - r0 + kTile - 1) / kTile;
+  constexpr int kPer = kMaxFan / kPT;       // counters per thread in the scan (consecutive)
+  for (int64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+    const int64_t base = r0 + t * kTile;
+    const int m = (int)min((int64_t)kTile, r1 - base);
+    // the CTA's next tile is pulled into L2 now: its loads are what this kernel waits for most
+    // (ncu: long_scoreboard 49 % of stall samples with one tile in flight per CTA)
+    {
+      const int64_t nb = base + (int64_t)gridDim.x * kTile;
+      if constexpr (KK != KK_GEN && KK != KK_GEN32) {
+       if (nb < r1 && a.key.ncols == 1) {
+        const int64_t nm = min((int64_t)kTile, r1 - nb);
+        const int64_t kbytes = nm * (int64_t)sizeof(U), vbytes = nm * 8;
+        const char* kp = static_cast<const char*>(a.key.ptr[0]) + nb * (int64_t)sizeof(U);
+        for (int64_t o = (int64_t)tid * 128; o < kbytes; o += (int64_t)kPT * 128) prefetch_l2(kp + o);
+        for (int c = 0; c < a.n_vals; ++c) {
+          const char* vp = reinterpret_cast<const char*>(static_cast<const uint64_t*>(a.vals[c]) + nb);
+          for (int64_t o = (int64_t)tid * 128; o < vbytes; o += (int64_t)kPT * 128) prefetch_l2(vp + o);
+        }
+       }
+      } else if (nb < r1) {
+        // several key columns (level 1 of a fused key): each column at its own width
+        const int64_t nm = min((int64_t)kTile, r1 - nb);
+        for (int kc = 0; kc < a.key.ncols; ++kc) {
+          const int64_t w = a.key.dtype[kc] == EIGER_I8 ? 1 : (a.key.dtype[kc] == EIGER_I32 ? 4 : 8);
+          const char* kp = static_cast<const char*>(a.key.ptr[kc]) + nb * w;
+          for (int64_t o = (int64_t)tid * 128; o < nm * w; o += (int64_t)kPT * 128) prefetch_l2(kp + o);
+        }
+        for (int c = 0; c < a.n_vals; ++c) {
+          const char* vp = reinterpret_cast<const char*>(static_cast<const uint64_t*>(a.vals[c]) + nb);
+          for (int64_t o = (int64_t)tid * 128; o < nm * 8; o += (int64_t)kPT * 128) prefetch_l2(vp + o);
+        }
+      }
+    }
+    // A: keys -> partition ids and ranks inside the tile
+    U u[kPR];
+    uint32_t pos[kPR];
+    uint64_t v0[kPR];
+#pragma unroll
+    for (int r = 0; r < kPR; ++r) {
+      const int i = r * kPT + tid;
+      if (i < m) {
+        u[r] = load_u<KK>(a.key, base + i);
+        if (a.n_vals > 0) v0[r] = ldg_stream_u64(static_cast<const uint64_t*>(a.vals[0]) + base + i);
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < kPR; ++r) {
+      const int i = r * kPT + tid;
+      if (i < m) {
+        const uint32_t q = part_id<U>(u[r], a.shift, mask);
+        pos[r] = (q << 16) | atomicAdd(&s_cnt[q], 1u);      // rank < 4096 fits 16 bits
+      }
+    }
+    __syncthreads();
+    // B: exclusive scan of the per-partition counts; claim global space per partition
+    long long gclaim[kPer];
+    uint32_t gcnt[kPer];
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) { gclaim[k] = 0; gcnt[k] = 0; }
+    {
+      uint32_t c[kPer], sum = 0;
+#pragma unroll
+      for (int k = 0; k < kPer; ++k) { const int p = tid * kPer + k; c[k] = p < fan ? s_cnt[p] : 0u; sum += c[k]; }
+      uint32_t inc = sum;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += y; }
+      if (lane == 31) s_warp[warp] = inc;
+      __syncthreads();
+      if (warp == 0) {
+        uint32_t w = lane < kPT / 32 ? s_warp[lane] : 0u;
+        uint32_t winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += y; }
+        if (lane < kPT / 32) s_warp[lane] = winc - w;
+      }
+      __syncthreads();
+      uint32_t run = s_warp[warp] + inc - sum;
+      // the claims' round trips to L2 overlap the staging below: their results are first needed in D
+#pragma unroll
+      for (int k = 0; k < kPer; ++k) {
+        const int p = tid * kPer + k;
+        if (p < fan) {
+          s_loff[p] = run;
+          gclaim[k] = c[k] ? (long long)atomicAdd(&cursor[p], (unsigned long long)c[k]) - (long long)run : 0ll;
+          gcnt[k] = c[k];
+          s_cnt[p] = 0;
+          run += c[k];
+        }
+      }
+    }
+    __syncthreads();
+    // C: stage keys (and the first value column) in partition order
+#pragma unroll
+    for (int r = 0; r < kPR; ++r) {
+      const int i = r * kPT + tid;
+      if (i < m) {
+        const uint32_t q = pos[r] >> 16;
+        pos[r] = s_loff[q] + (pos[r] & 0xFFFFu);
+        s_key[pos[r]] = (UO)u[r];
+        s_pid[pos[r]] = (uint16_t)q;
+        if (a.n_vals > 0) s_val[pos[r]] = v0[r];
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) { const int p = tid * kPer + k; if (p < fan && gcnt[k]) s_delta[p] = gclaim[k]; }
+    __syncthreads();
+    // D: write runs
+#pragma unroll
+    for (int r = 0; r < kPR; ++r) {
+      const int j = r * kPT + tid;
+      if (j < m) {
+        const long long dst = s_delta[s_pid[j]] + j;
+        out_keys[dst] = s_key[j];
+        if (a.n_vals > 0) static_cast<uint64_t*>(a.out_vals[0])[dst] = s_val[j];
+      }
+    }
+    // remaining value columns, one staged at a time
+    for (int c = 1; c < a.n_vals; ++c) {
+      __syncthreads();
+#pragma unroll
+      for (int r = 0; r < kPR; ++r) {
+        const int i = r * kPT + tid;
+        if (i < m) s_val[pos[r]] = ldg_stream_u64(static_cast<const uint64_t*>(a.vals[c]) + base + i);
+      }
+      __syncthreads();
+#pragma unroll
+      for (int r = 0; r < kPR; ++r) {
+        const int j = r * kPT + tid;
+        if (j < m) static_cast<uint64_t*>(a.out_vals[c])[s_delta[s_pid[j]] + j] = s_val[j];
+      }
+    }
+    __syncthreads();
+  }
+}
+
 template <int KK, class UO, int RPT>
 int launch_scatter(const LevelArgs& a, const uint8_t* vw, int threads, int stages, int gx, int segments, cudaStream_t s) {
   ScatterArgs A{};
@@ -367,6 +527,21 @@ int run_level(LevelArgs a, const uint8_t* vw, int segments, unsigned long long* 
   count_launch();
   part_scan_kernel<<<1, 1024, 0, s>>>(a.hist, off, a.cursor, segments * a.fan);
   count_launch();
+  bool all8 = true;
+  for (int c = 0; c < a.n_vals; ++c) all8 = all8 && (vw[c] == 0 || vw[c] == 8);
+  const char* er = std::getenv("EIGER_SCATTER_RING");
+  if (all8 && er && std::atoi(er) == 0) {
+    const int64_t otiles = std::max<int64_t>(1, (avg_rows + kTile - 1) / kTile);
+    const int64_t owant = segments == 1 ? (int64_t)sm_count * 8 : std::max<int64_t>(1, ((int64_t)sm_count * 8 + segments - 1) / segments);
+    const int ogx = (int)std::min<int64_t>(otiles, owant);
+    constexpr size_t osmem = (sizeof(uint64_t) + sizeof(UO) + sizeof(uint16_t)) * kTile + (8 + 4 + 4) * kMaxFan;
+    auto kern = part_scatter_ldg_kernel<KK, UO>;
+    EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)osmem));
+    kern<<<dim3(ogx, segments), kPT, osmem, s>>>(a);
+    count_launch();
+    EIGER_CUDA(cudaGetLastError());
+    return EIGER_OK;
+  }
   if (rpt == 6) return launch_scatter<KK, UO, 6>(a, vw, threads, stages, gx, segments, s);
   return launch_scatter<KK, UO, 4>(a, vw, threads, stages, gx, segments, s);
 }
