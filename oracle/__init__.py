@@ -68,6 +68,8 @@ def _load():
         L.oracle_hll_registers.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_void_p]
         L.oracle_hll_estimate.restype = ctypes.c_double
         L.oracle_hll_estimate.argtypes = [ctypes.c_void_p, ctypes.c_int32]
+        L.oracle_dict_encode.restype = ctypes.c_int64
+        L.oracle_dict_encode.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
         _lib = L
     return _lib
 
@@ -209,3 +211,15 @@ def profile(keys, p: int = HLL_P) -> Stats:
     est = hll_estimate(hll_registers(k, p), p)
     est = min(est, float(n), float(hi - lo + 1))
     return Stats(lo, hi, max(est, 0.0), n)
+
+
+def dict_encode(keys):
+    """Order-preserving dictionary encoding (Algorithm 1): returns (codes int64[n],
+    dictionary int64[ndv] ascending, ndv) with dictionary[codes[i]] == keys[i]."""
+    L = _load()
+    k = _i64(keys)
+    n = int(k.shape[0])
+    codes = np.empty(n, dtype=np.int64)
+    d = np.empty(max(n, 1), dtype=np.int64)
+    ndv = int(L.oracle_dict_encode(_ptr(k), n, _ptr(codes), _ptr(d)))
+    return codes, d[:ndv].copy(), ndv

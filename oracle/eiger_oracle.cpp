@@ -21,6 +21,9 @@
 //   * oracle_hll_estimate   pinned (linear-counting closed form when only small
 //                           registers are set, known-NDV error bound 4 sigma,
 //                           golden whole-sketch estimates)
+//   * oracle_dict_encode    pinned (brute-force "number of smaller distinct values" on small
+//                           inputs, order / round-trip invariants, worked example;
+//                           tests/test_oracle_dict.py)
 //   * parity with the PAPER'S OWN implementation: unpinned (the paper prints no
 //     group-by result and no sketch value; DESIGN.md says so).
 //
@@ -329,6 +332,41 @@ double oracle_hll_estimate(const uint8_t* regs, int32_t p) {
   z += md * sigma_fn(C[0] / md);
   const double alpha_inf = 0.5 / std::log(2.0);
   return alpha_inf * md * md / z;
+}
+
+
+// ---------------------------------------------------------------------------
+// Order-preserving dictionary encoding, PAPER.md:171-211 (Algorithm 1), followed step by step in
+// the paper's order and notation (one thread = one loop iteration here):
+//   (1) compute_group_id: HT.insert_and_find(key[i], i) -> the first tuple that carries a key is
+//       its group leader; groupIdLoc[i] = the leader's tuple id; ndv counts the successful inserts.
+//   (2) [uniqueKeys, groupIds] = HT.retrieveAll()          (ndv pairs, groupIds = leader tuple ids)
+//   (3) argsortIds = argsort(uniqueKeys)
+//   (4) scatter: sparseGroupIds[groupIds[argsortIds[i]]] = i
+//   (5) gather:  C_out[i] = sparseGroupIds[groupIdLoc[i]]
+// Output: codes[n] (C_out), dict[ndv] = the unique keys in ascending order (dict[code] = key; the
+// paper keeps it implicitly as uniqueKeys[argsortIds]).  Returns ndv.
+// ---------------------------------------------------------------------------
+int64_t oracle_dict_encode(const int64_t* keys, int64_t n, int64_t* codes, int64_t* dict) {
+  std::unordered_map<int64_t, int64_t> HT;                       // key -> leader tuple id
+  std::vector<int64_t> groupIdLoc((size_t)n);
+  int64_t ndv = 0;
+  for (int64_t i = 0; i < n; ++i) {                               // (1)
+    auto r = HT.emplace(keys[i], i);
+    groupIdLoc[(size_t)i] = r.first->second;
+    if (r.second) ++ndv;
+  }
+  std::vector<int64_t> uniqueKeys, groupIds;                      // (2)
+  uniqueKeys.reserve((size_t)ndv); groupIds.reserve((size_t)ndv);
+  for (const auto& kv : HT) { uniqueKeys.push_back(kv.first); groupIds.push_back(kv.second); }
+  std::vector<int64_t> argsortIds((size_t)ndv);                   // (3)
+  for (int64_t i = 0; i < ndv; ++i) argsortIds[(size_t)i] = i;
+  std::sort(argsortIds.begin(), argsortIds.end(), [&](int64_t a, int64_t b) { return uniqueKeys[(size_t)a] < uniqueKeys[(size_t)b]; });
+  std::vector<int64_t> sparseGroupIds((size_t)n, -1);             // (4)
+  for (int64_t i = 0; i < ndv; ++i) sparseGroupIds[(size_t)groupIds[(size_t)argsortIds[(size_t)i]]] = i;
+  for (int64_t i = 0; i < n; ++i) codes[i] = sparseGroupIds[(size_t)groupIdLoc[(size_t)i]];   // (5)
+  for (int64_t i = 0; i < ndv; ++i) dict[i] = uniqueKeys[(size_t)argsortIds[(size_t)i]];
+  return ndv;
 }
 
 }  // extern "C"

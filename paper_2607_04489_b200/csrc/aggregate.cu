@@ -29,7 +29,11 @@ struct AggArgs {
   void* table;
   uint64_t cap;
   CallDev* call;
+  // FRONT_DICT: key -> dense id dictionary built from the key sample (image in global memory)
+  const uint2* dict; uint32_t dict_slots, dict_shift;
 };
+
+constexpr uint32_t kDictMul = 0x9E3779B1u;
 
 template <int KK, int SIG, int FRONT>
 struct AggCtx {
@@ -42,12 +46,27 @@ struct AggCtx {
   const int n_acc;
   unsigned char* smem;
 
-  unsigned char* rep_base;       // FRONT_SDIRECT: this warp's replica of the table
+  unsigned char* rep_base;       // FRONT_SDIRECT / FRONT_DICT: this warp's replica of the table
+  const uint2* sdict;            // FRONT_DICT: the dictionary (key, id) in shared memory, after the replicas
 
   __device__ AggCtx(const AggArgs& args, unsigned char* sm)
       : a(args), n_acc(S::kStatic ? S::kAcc : args.plan.n_acc), smem(sm) {
     const uint32_t rep = args.front_replicas > 1 ? (threadIdx.x >> 5) % args.front_replicas : 0u;
     rep_base = sm + (size_t)rep * args.front_slots * 8 * (uint32_t)n_acc;
+    sdict = reinterpret_cast<const uint2*>(sm + (size_t)args.front_replicas * args.front_slots * 8 * (uint32_t)n_acc);
+  }
+
+  // dense id of rebased key u, ~0u when the dictionary does not hold it (empty entries carry id ~0u)
+  __device__ __forceinline__ uint32_t dict_id(uint32_t u) const {
+    uint32_t h = (u * kDictMul) >> a.dict_shift, id = ~0u;
+    bool done = false;
+    while (!done) {
+      const uint2 e = sdict[h];
+      if (e.x == u) { id = e.y; done = true; }
+      else if (e.x == kEmpty32) done = true;
+      else h = (h + 1u) & (a.dict_slots - 1u);
+    }
+    return id;
   }
 
   __device__ void front_init() {
@@ -56,10 +75,14 @@ struct AggCtx {
       uint64_t* acc = reinterpret_cast<uint64_t*>(smem);
       for (uint32_t c = 0; c < a.front_slots * (uint32_t)n_acc; ++c)
         acc[(size_t)c * T + tid] = acc_identity(sig_op<SIG>(a.plan, (int)(c % (uint32_t)n_acc)));
-    } else if constexpr (FRONT == FRONT_SDIRECT) {
+    } else if constexpr (FRONT == FRONT_SDIRECT || FRONT == FRONT_DICT) {
       for (uint32_t rep = 0; rep < a.front_replicas; ++rep)
         for (int j = 0; j < n_acc; ++j)
           smem_init_plane(smem + (size_t)rep * a.front_slots * 8 * (uint32_t)n_acc, a.front_slots, j, sig_op<SIG>(a.plan, j), sig_f64<SIG>(a.plan, j), tid, T);
+      if constexpr (FRONT == FRONT_DICT) {
+        uint2* d = const_cast<uint2*>(sdict);
+        for (uint32_t i = tid; i < a.dict_slots; i += T) d[i] = a.dict[i];
+      }
     }
     if constexpr (FRONT != FRONT_NONE) __syncthreads();
   }
@@ -75,8 +98,14 @@ struct AggCtx {
   }
 
   __device__ __forceinline__ void row(U u, const uint64_t (&raw)[NV]) {
+    if constexpr (FRONT == FRONT_DICT) {
+      // the dictionary names the keys of the sample: a key it does not hold discards the pass
+      const uint32_t id = dict_id((uint32_t)u);
+      if (id >= a.front_slots) { if (*reinterpret_cast<volatile uint32_t*>(&a.call->abort) == 0u) atomicOr(&a.call->abort, 1u); return; }
+      u = (U)id;
+    }
     // speculative run planned from a sample: the range is checked exactly here
-    if (a.spec && (uint64_t)u >= a.cap) { if (*reinterpret_cast<volatile uint32_t*>(&a.call->abort) == 0u) atomicOr(&a.call->abort, 1u); return; }
+    if (FRONT != FRONT_DICT && a.spec && (uint64_t)u >= a.cap) { if (*reinterpret_cast<volatile uint32_t*>(&a.call->abort) == 0u) atomicOr(&a.call->abort, 1u); return; }
     if constexpr (FRONT == FRONT_PRIV) {
       uint64_t* acc = reinterpret_cast<uint64_t*>(smem) + (size_t)u * (uint32_t)n_acc * blockDim.x + threadIdx.x;
 #pragma unroll
@@ -86,7 +115,7 @@ struct AggCtx {
         uint64_t* c = acc + (size_t)j * blockDim.x;
         *c = combine(op, f, *c, row_partial(op, f, raw[sig_col<SIG>(a.plan, j)]));
       }
-    } else if constexpr (FRONT == FRONT_SDIRECT) {
+    } else if constexpr (FRONT == FRONT_SDIRECT || FRONT == FRONT_DICT) {
       unsigned char* base = rep_base;
 #pragma unroll
       for (int j = 0; j < NA; ++j) {
@@ -103,11 +132,22 @@ struct AggCtx {
   // then the counts, then the carries, so that a row's carry does not wait alone for its atomic
   // (ncu: short_scoreboard was 28 % of the stall samples with one row at a time)
   template <int R>
-  __device__ __forceinline__ void rows_sc(const U (&u)[R], const uint64_t (&raw)[R][NV]) {
-    static_assert((SIG == SIG_SC || SIG == SIG_SC32) && FRONT == FRONT_SDIRECT, "SUM + COUNT signature only");
+  __device__ __forceinline__ void rows_sc(const U (&uk)[R], const uint64_t (&raw)[R][NV]) {
+    static_assert((SIG == SIG_SC || SIG == SIG_SC32) && (FRONT == FRONT_SDIRECT || FRONT == FRONT_DICT), "SUM + COUNT signature only");
     uint32_t* lo = reinterpret_cast<uint32_t*>(rep_base);
     uint32_t* cnt = reinterpret_cast<uint32_t*>(rep_base + (size_t)8 * a.front_slots);
-    if (a.spec) {
+    U u[R];
+    if constexpr (FRONT == FRONT_DICT) {
+      // all look-ups first (R independent shared-memory loads in flight), then the misses are settled
+      bool bad = false;
+#pragma unroll
+      for (int r = 0; r < R; ++r) { u[r] = (U)dict_id((uint32_t)uk[r]); bad = bad || (uint32_t)u[r] >= a.front_slots; }
+      if (bad) { if (*reinterpret_cast<volatile uint32_t*>(&a.call->abort) == 0u) atomicOr(&a.call->abort, 1u); return; }
+    } else {
+#pragma unroll
+      for (int r = 0; r < R; ++r) u[r] = uk[r];
+    }
+    if (FRONT != FRONT_DICT && a.spec) {
       // speculative run planned from a sample: one key outside the planned range discards the whole
       // pass anyway, so the trip is skipped as a whole (one branch per R rows, not one per atomic)
       bool bad = false;
@@ -152,7 +192,7 @@ struct AggCtx {
         for (int o = 16; o > 0; o >>= 1) v = combine(op, f, v, __shfl_xor_sync(0xffffffffu, v, o));
         if (lane == 0) back_merge(c / (uint32_t)n_acc, j, v, static_cast<uint64_t*>(a.table) + (uint64_t)(c / (uint32_t)n_acc) * (uint32_t)n_acc);
       }
-    } else if constexpr (FRONT == FRONT_SDIRECT) {
+    } else if constexpr (FRONT == FRONT_SDIRECT || FRONT == FRONT_DICT) {
       // the CTA's replicas are combined first: one global atomic per cell and CTA (with 8 replicas of
       // a 256-slot table the flush of ~900 CTAs otherwise queues millions of atomics on 512 addresses)
       const uint32_t per = a.front_slots * (uint32_t)n_acc;
@@ -206,7 +246,7 @@ aggregate_kernel(const __grid_constant__ AggArgs a) {
         global_val2(a.plan, c, sig_vw<SIG>(a.plan, c), r0 + s * kStep, raw[s][0][c], raw[s][1][c]);
       }
     }
-    if constexpr ((SIG == SIG_SC || SIG == SIG_SC32) && FRONT == FRONT_SDIRECT) {
+    if constexpr ((SIG == SIG_SC || SIG == SIG_SC32) && (FRONT == FRONT_SDIRECT || FRONT == FRONT_DICT)) {
       U uu[2 * UNR]; uint64_t rr[2 * UNR][NV];
 #pragma unroll
       for (int s = 0; s < UNR; ++s) { uu[2 * s] = u[s][0]; uu[2 * s + 1] = u[s][1]; rr[2 * s][0] = raw[s][0][0]; rr[2 * s + 1][0] = raw[s][1][0]; }
@@ -224,6 +264,38 @@ aggregate_kernel(const __grid_constant__ AggArgs a) {
     ctx.row(load_u<KK>(a.key, i), raw);
   }
   ctx.front_flush();
+}
+
+// ---- dictionary of the sampled keys (FRONT_DICT) ----------------------------------------------------
+// One thread per sampled row (the same evenly spaced rows the sample statistics were taken from):
+// the rebased fused key u is inserted into an open-addressing image (u, dense id) in global memory;
+// the first thread to claim a key draws its id.  This is the paper's dictionary encoding
+// (Algorithm 1, steps 1-2: insert-and-find, one leader per key) applied to the
+// sample: keys that are sparse in a wide range get dense codes, and the aggregation pass then
+// indexes a direct array with the code.  id >= cap (more keys than planned): the pass gives up.
+__global__ void __launch_bounds__(256)
+dict_build_kernel(const __grid_constant__ KeyDesc key, int64_t n, int64_t samples, uint2* __restrict__ img, uint32_t slots, uint32_t shift,
+                  uint32_t cap, uint32_t* __restrict__ dict_keys, uint32_t* __restrict__ dict_n, CallDev* call) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= samples) return;
+  const int64_t i = (int64_t)(((unsigned __int128)t * (unsigned __int128)n) / (unsigned __int128)samples);
+  const uint64_t u64 = load_u<KK_GEN>(key, i);
+  if (u64 >= 0xFFFFFFFFull) return;                           // outside the planned ranges: the aggregation pass will notice
+  const uint32_t u = (uint32_t)u64;
+  uint32_t h = (u * kDictMul) >> shift;
+  uint32_t* w = reinterpret_cast<uint32_t*>(img);
+  for (uint32_t probes = 0; probes < slots; ++probes) {
+    const uint32_t old = atomicCAS(w + 2 * (size_t)h, kEmpty32, u);
+    if (old == kEmpty32) {
+      const uint32_t id = atomicAdd(dict_n, 1u);
+      if (id < cap) { dict_keys[id] = u; __threadfence(); w[2 * (size_t)h + 1] = id; }
+      else atomicOr(&call->abort, 1u);
+      return;
+    }
+    if (old == u) return;
+    h = (h + 1u) & (slots - 1u);
+  }
+  atomicOr(&call->abort, 1u);
 }
 
 // ---- table init (step A5) ----------------------------------------------------------------
@@ -247,6 +319,7 @@ struct CompactArgs {
   void* out_keys[kMaxKeyCols]; uint64_t* out_aggs[kMaxAggs]; int n_out;
   int64_t out_capacity;
   uint64_t R;               // several key columns: fused keys are below R; anything else is a row outside the planned ranges
+  const uint32_t* dict_keys; // FRONT_DICT: slot = dense id, key = dict_keys[id]
   CallDev* call;
 };
 
@@ -270,7 +343,7 @@ __global__ void __launch_bounds__(256) compact_kernel(const __grid_constant__ Co
         slot += 1;
       } else {
         occ = slot[c.plan.cnt_acc] != 0ull;
-        u = s;
+        u = c.dict_keys ? (uint64_t)c.dict_keys[s] : s;
       }
     }
     // several key columns: a row with a column outside its planned range was fused to the marker
@@ -309,6 +382,7 @@ int launch_one(const AggLaunch& L, cudaStream_t s) {
   a.key = L.key; a.plan = L.plan; a.n = L.n;
   a.front_slots = L.front_slots; a.front_limit = L.front_limit; a.front_replicas = L.front_replicas; a.spec = L.spec;
   a.stride = L.stride; a.table = L.table; a.cap = L.cap; a.call = L.call;
+  a.dict = static_cast<const uint2*>(L.dict); a.dict_slots = L.dict_slots; a.dict_shift = L.dict_shift;
   kern<<<L.blocks, THREADS, L.smem_bytes, s>>>(a);
   count_launch();
   EIGER_CUDA(cudaGetLastError());
@@ -323,6 +397,9 @@ int launch_fb(const AggLaunch& L, cudaStream_t s) {
     case FRONT_PRIV: return launch_one<KK, SIG, FRONT_PRIV>(L, s);
     case FRONT_SDIRECT: return L.threads == kAggThreadsWide ? launch_one<KK, SIG, FRONT_SDIRECT, kAggThreadsWide>(L, s)
                                                             : launch_one<KK, SIG, FRONT_SDIRECT>(L, s);
+    case FRONT_DICT:
+      if constexpr (sizeof(typename KeyTraits<KK>::U) == 4) return launch_one<KK, SIG, FRONT_DICT, kAggThreadsWide>(L, s);
+      else return EIGER_ERR_ARG;
     default: return EIGER_ERR_ARG;
   }
 }
@@ -345,11 +422,11 @@ int launch_sig(const AggLaunch& L, cudaStream_t s) {
 bool aggregate_supported(int key_kind, int sig, int front, int back) {
   (void)sig;
   return back == BACK_DIRECT && key_kind != KK_U64PRE && key_kind != KK_U32PRE &&
-         (front == FRONT_NONE || front == FRONT_PRIV || front == FRONT_SDIRECT);
+         (front == FRONT_NONE || front == FRONT_PRIV || front == FRONT_SDIRECT || front == FRONT_DICT);
 }
 
 int launch_aggregate(const AggLaunch& L, cudaStream_t s) {
-  if (L.threads != kAggThreads && !(L.threads == kAggThreadsWide && L.front == FRONT_SDIRECT)) return EIGER_ERR_ARG;
+  if (L.threads != kAggThreads && !(L.threads == kAggThreadsWide && (L.front == FRONT_SDIRECT || L.front == FRONT_DICT))) return EIGER_ERR_ARG;
   switch (L.key_kind) {
     case KK_I32: return launch_sig<KK_I32>(L, s);
     case KK_I64: return launch_sig<KK_I64>(L, s);
@@ -358,6 +435,18 @@ int launch_aggregate(const AggLaunch& L, cudaStream_t s) {
     case KK_GEN32: return launch_sig<KK_GEN32>(L, s);
     default: return EIGER_ERR_ARG;
   }
+}
+
+int launch_dict_build(const AggLaunch& L, int64_t samples, uint32_t* dict_keys, uint32_t* dict_n, cudaStream_t s) {
+  EIGER_CUDA(cudaMemsetAsync(L.dict, 0xFF, (size_t)L.dict_slots * 8, s));
+  EIGER_CUDA(cudaMemsetAsync(dict_n, 0, 4, s));
+  KeyDesc k = L.key;
+  k.flags &= ~kKey32;      // 64-bit fusion here (one thread per sampled row: speed is irrelevant), the marker stays ~0ull
+  dict_build_kernel<<<(unsigned)((samples + 255) / 256), 256, 0, s>>>(k, L.n, samples, static_cast<uint2*>(L.dict), L.dict_slots, L.dict_shift,
+                                                                       L.front_slots, dict_keys, dict_n, L.call);
+  count_launch();
+  EIGER_CUDA(cudaGetLastError());
+  return EIGER_OK;
 }
 
 int launch_table_init(const AggLaunch& L, cudaStream_t s) {
@@ -384,7 +473,7 @@ int launch_compact(const CompactLaunch& c, int sm_count, cudaStream_t s) {
   a.cap = c.cap; a.stride = c.stride; a.back = c.back;
   for (int k = 0; k < kMaxKeyCols; ++k) a.out_keys[k] = c.out_keys[k];
   for (int j = 0; j < kMaxAggs; ++j) a.out_aggs[j] = static_cast<uint64_t*>(c.out_aggs[j]);
-  a.n_out = c.n_out_aggs; a.out_capacity = c.out_capacity; a.call = c.call; a.R = c.R;
+  a.n_out = c.n_out_aggs; a.out_capacity = c.out_capacity; a.call = c.call; a.R = c.R; a.dict_keys = c.dict_keys;
   const uint64_t n_slots = c.cap + 1;
   const int blocks = (int)std::max<uint64_t>(1, std::min<uint64_t>((n_slots + 255) / 256, (uint64_t)sm_count * 8));
   compact_kernel<<<blocks, 256, 0, s>>>(a);

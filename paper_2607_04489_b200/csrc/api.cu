@@ -98,6 +98,8 @@ struct Tunables {
   int slice;                          // EIGER_AUTO sizes PARTITION from a hash-space slice sketch instead of the full profile
   double slice_min_keys;              // distinct keys wanted in the slice (relative error 1 / sqrt of it)
   double fused_sketch_min_range;      // multi-column keys: sketch the fused key when the ranges multiply to more than this
+  int dict;                           // EIGER_AUTO: scattered keys the sample names completely get a dictionary + direct array (FRONT_DICT)
+  double dict_max_keys;               // ... while the sample holds at most this many distinct keys
   Tunables() {
     auto env = [](const char* k, double dflt) { const char* v = std::getenv(k); return v ? std::atof(v) : dflt; };
     priv_smem = (size_t)env("EIGER_PRIV_KB", 96) << 10;
@@ -130,6 +132,8 @@ struct Tunables {
     hot_min_share = env("EIGER_HOT_MIN_SHARE", 0.02);
     slice = (int)env("EIGER_SLICE", 1);
     slice_min_keys = env("EIGER_SLICE_MIN_KEYS", 2048);
+    dict = (int)env("EIGER_DICT", 1);
+    dict_max_keys = env("EIGER_DICT_MAX_KEYS", 1024);
   }
 };
 Tunables tun() { return Tunables(); }
@@ -158,6 +162,7 @@ struct QueryPlan {
   size_t table_bytes = 0, part_bytes = 0, total_bytes = 0;
   const uint32_t* pre_hist = nullptr;   // PARTITION: level-1 histogram taken with key.base at fan-out kPreFan
   int sort_bits = 0, sort_passes = 0;   // SORT: significant bits of the rebased fused key, 8-bit passes
+  uint32_t dict_slots = 0, dict_shift = 0;   // FRONT_DICT: dictionary image entries (power of two)
 };
 
 uint64_t range_of(const eiger_stats& s) {   // max - min + 1, 0 when it is 2^64
@@ -387,6 +392,40 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   return EIGER_OK;
 }
 
+// Turns the EIGER_SMEM plan of a key sample into the dictionary plan (FRONT_DICT): the sample's keys
+// get dense ids (dictionary encoding; "if NDV is below a certain
+// threshold, we will use dictionary encoding") and the aggregation indexes a per-CTA direct array with
+// the id - the batched accumulate of FRONT_SDIRECT instead of the hash table's find-or-insert.
+// Only for rebased keys of 32 bits; false when the shape does not fit.
+bool make_dict_plan(QueryPlan* q, const eiger_col* keys, int nk, int na, double sample_ndv, const Tunables& T) {
+  if (!T.dict || sample_ndv > T.dict_max_keys) return false;
+  int kk;
+  if (nk == 1 && keys[0].dtype == EIGER_I32) kk = KK_I32;
+  else if (q->key.flags & kKey32) kk = KK_GEN32;
+  else return false;
+  AggPlan& p = q->plan;
+  bool has_count = false;
+  for (int j = 0; j < na; ++j) has_count = has_count || p.op[j] == EIGER_COUNT;
+  if (!has_count) { if (na >= kMaxAcc) return false; p.op[na] = EIGER_COUNT; p.cnt_acc = na; p.n_acc = na + 1; }
+  uint32_t cap = 64;
+  while (cap < 2048 && (double)cap < 2.0 * sample_ndv + 16.0) cap *= 2;
+  const size_t cell = (size_t)cap * 8 * p.n_acc;
+  if (cell > (64u << 10)) return false;
+  uint32_t slots = 4096;
+  while (slots < 16384 && slots < 16 * cap) slots *= 2;
+  int shift = 32; for (uint32_t x = slots; x > 1; x >>= 1) --shift;
+  const uint32_t reps = (uint32_t)std::max<size_t>(1, std::min<size_t>(8, (64u << 10) / cell));
+  q->back = BACK_DIRECT; q->front = FRONT_DICT; q->key_kind = kk;
+  q->front_slots = cap; q->front_replicas = reps; q->cap = cap; q->stride = 8u * p.n_acc;
+  q->dict_slots = slots; q->dict_shift = (uint32_t)shift;
+  q->smem_bytes = cell * reps + (size_t)slots * 8;
+  q->sig = detect_sig(p, na);
+  q->table_bytes = align_up((size_t)cap * q->stride, 256);
+  q->part_bytes = align_up((size_t)slots * 8, 256) + align_up((size_t)cap * 4, 256) + 256;
+  q->total_bytes = q->table_bytes + q->part_bytes + 256;
+  return aggregate_supported(kk, q->sig, FRONT_DICT, BACK_DIRECT);
+}
+
 // Profiles nk key columns with one read-back: min/max of each, and (single column only) the
 // sketch.  with_hll = 0 is the range-first shortcut: ndv_est = min(n, range).
 // samples > 0: statistics of an evenly spaced sample of that many keys (plan of the speculative pass).
@@ -523,7 +562,16 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     }
     { Timed t(s, 3); rc = launch_table_init(L, s); if (rc) return rc; }
 
-    if (q.variant == EIGER_DIRECT) {
+    uint32_t* dict_keys = nullptr;
+    if (q.front == FRONT_DICT) {
+      // workspace after the table: dictionary image, id -> key, id counter
+      auto take = [&](size_t bytes) { char* r = pws; pws += align_up(bytes, 256); return r; };
+      L.dict = take((size_t)q.dict_slots * 8); L.dict_slots = q.dict_slots; L.dict_shift = q.dict_shift;
+      dict_keys = reinterpret_cast<uint32_t*>(take((size_t)q.cap * 4));
+      uint32_t* dict_n = reinterpret_cast<uint32_t*>(take(256));
+      { Timed t(s, 1); rc = launch_dict_build(L, std::min<int64_t>(n, tun().spec_samples), dict_keys, dict_n, s); if (rc) return rc; }
+    }
+    if (q.variant == EIGER_DIRECT || q.front == FRONT_DICT) {
       // persistent grid: as many CTAs as fit, never more than there are tiles
       const size_t per_cta = std::max<size_t>(q.smem_bytes, 1024);
       int occ = (int)std::min<size_t>(8, std::max<size_t>(1, (rt->smem_optin + 1024) / (per_cta + 1024)));
@@ -532,7 +580,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       // CTAs reach 0.53 ms only while three of them fit the 196 KB carve-out (65.5 KB arrays), 0.61 ms
       // at 69.6 KB and 0.93 ms at 128 KB (one CTA = 8 warps per SM); the wide CTA runs 0.51-0.53 ms
       // at every size from 2^5 to 2^13 slots
-      if (q.front == FRONT_SDIRECT && (tun().sdirect_wide || 3 * (per_cta + 1024) > (196u << 10))) { L.threads = 1024; occ = 1; }
+      if (q.front == FRONT_DICT || (q.front == FRONT_SDIRECT && (tun().sdirect_wide || 3 * (per_cta + 1024) > (196u << 10)))) { L.threads = 1024; occ = 1; }
       const int64_t tiles = std::max<int64_t>(1, (n + 1023) / 1024);
       L.blocks = (int)std::min<int64_t>((int64_t)rt->sm_count * occ, tiles);
       { Timed t(s, 0); rc = launch_aggregate(L, s); if (rc) return rc; }
@@ -597,7 +645,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     C.key = q.key; C.plan = q.plan; C.back = q.back; C.table = table; C.cap = q.cap; C.stride = q.stride;
     for (int k = 0; k < kMaxKeyCols; ++k) C.out_keys[k] = k < nk ? out_keys[k] : nullptr;
     for (int j = 0; j < na; ++j) C.out_aggs[j] = out_aggs[j];
-    C.n_out_aggs = na; C.out_capacity = out_capacity; C.call = rt->call; C.R = q.R;
+    C.n_out_aggs = na; C.out_capacity = out_capacity; C.call = rt->call; C.R = q.R; C.dict_keys = dict_keys;
     { Timed t(s, 4); rc = launch_compact(C, rt->sm_count, s); if (rc) return rc; }
 
     EIGER_CUDA(cudaMemcpyAsync(hb, rt->call, sizeof(Back), cudaMemcpyDeviceToHost, s));
@@ -672,6 +720,21 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       local[k].min = room_lo >= (uint64_t)margin ? local[k].min - margin : tmin;
       local[k].max = room_hi >= (uint64_t)margin ? local[k].max + margin : tmax;
       local[k].n = n;
+    }
+    {
+      // scattered keys that the sample names completely: dictionary + direct array, verified exactly
+      // (a key the dictionary does not hold discards the pass)
+      QueryPlan qd;
+      double sndv = local[0].ndv_est;
+      for (int k = 1; k < nk; ++k) sndv *= local[k].ndv_est;
+      sndv = std::min(sndv, (double)T.spec_samples);
+      if (T.spec && T.dict && !skewed && plan_query(rt, keys, nk, n, vals, nv, aggs, na, local, EIGER_AUTO, &qd, skewed) == EIGER_OK &&
+          qd.variant == EIGER_SMEM && make_dict_plan(&qd, keys, nk, na, sndv, T) && qd.total_bytes <= workspace_bytes) {
+        bool aborted = false;
+        rc = execute(qd, local, 1, &aborted);
+        if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] dictionary pass (%u ids, %u dictionary slots, %u replicas): rc %d aborted %d\n", qd.front_slots, qd.dict_slots, qd.front_replicas, rc, (int)aborted);
+        if (rc != EIGER_OK || !aborted) { if (chosen) *chosen = EIGER_SMEM; return rc; }
+      }
     }
     QueryPlan qs;
     if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] sample: min %lld max %lld ndv %.1f collision %.5f\n", (long long)local[0].min, (long long)local[0].max, local[0].ndv_est, collision);

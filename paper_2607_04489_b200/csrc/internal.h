@@ -65,7 +65,7 @@ int launch_regs_to_bytes(Runtime* rt, uint8_t* out, cudaStream_t s);
 double hll_estimate_from_hist(const uint32_t* hist);
 
 // ---- aggregate.cu ----------------------------------------------------------------------
-enum FrontKind : int { FRONT_NONE = 0, FRONT_PRIV = 1, FRONT_SDIRECT = 2, FRONT_SHASH = 3 };
+enum FrontKind : int { FRONT_NONE = 0, FRONT_PRIV = 1, FRONT_SDIRECT = 2, FRONT_SHASH = 3, FRONT_DICT = 4 };
 enum BackKind : int { BACK_DIRECT = 0, BACK_HASH = 1 };
 
 struct AggLaunch {
@@ -83,10 +83,13 @@ struct AggLaunch {
   uint64_t cap;
   uint32_t stride;          // HASH: bytes per slot (power of two); DIRECT: 8 * n_acc
   CallDev* call;
+  // FRONT_DICT: dictionary image (key, dense id) of dict_slots entries (a power of two), slot = (u * mul) >> dict_shift
+  void* dict; uint32_t dict_slots, dict_shift;
   // launch shape
   int threads, blocks;
   size_t smem_bytes;
 };
+int launch_dict_build(const AggLaunch& a, int64_t samples, uint32_t* dict_keys, uint32_t* dict_n, cudaStream_t s);
 int launch_table_init(const AggLaunch& a, cudaStream_t s);
 int launch_aggregate(const AggLaunch& a, cudaStream_t s);
 bool aggregate_supported(int key_kind, int sig, int front, int back);
@@ -99,6 +102,7 @@ struct CompactLaunch {
   void* out_keys[kMaxKeyCols]; void* out_aggs[kMaxAggs]; int n_out_aggs;
   int64_t out_capacity;
   uint64_t R;               // fused key range (several key columns)
+  const uint32_t* dict_keys; // FRONT_DICT: key of dense id
   CallDev* call;
 };
 int launch_compact(const CompactLaunch& c, int sm_count, cudaStream_t s);
