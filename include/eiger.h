@@ -60,6 +60,18 @@ typedef enum {
 typedef struct { const void* data; int32_t dtype; int32_t reserved; } eiger_col; /* length n */
 typedef struct { int32_t op; int32_t val_col; } eiger_agg;   /* COUNT ignores val_col        */
 
+/* HOST struct filled by eiger_groupby / eiger_groupby_host when a pointer to it is passed: what the call did. */
+typedef struct {
+  int32_t variant;              /* the variant that ran (also returned through `chosen`)                        */
+  int32_t attempts;             /* 1 + re-runs after a table overflow (NDV under-estimated, R10)       */
+  int32_t partition_levels;     /* EIGER_PARTITION: 1 or 2 radix levels; else 0                                  */
+  int32_t partition_prehist;    /* EIGER_PARTITION: 1 when the level-1 histogram came from the statistics pass   */
+  int32_t partition_key_bytes;  /* EIGER_PARTITION: bytes per key (4 or 8) of the partitioned copy               */
+  int32_t sort_passes;          /* EIGER_SORT: 8-bit radix passes                                                 */
+  double ndv_est;               /* the NDV estimate the tables were sized with (after clamping to min(n, range)) */
+  int64_t kernel_launches;      /* kernels this call launched                                                     */
+} eiger_call_info;
+
 /* HOST struct.  n = 0 gives min = INT64_MAX, max = INT64_MIN, ndv_est = 0. */
 typedef struct { int64_t min, max; double ndv_est; int64_t n; } eiger_stats;
 
@@ -124,7 +136,11 @@ double eiger_hll_estimate_host(const uint8_t* regs);
  *   n_groups           HOST; number of groups written (order of groups unspecified)
  *   force              EIGER_AUTO or a variant to run regardless of the statistics
  *   chosen             HOST, may be NULL; the variant that ran
- *   workspace          DEVICE scratch of workspace_bytes
+ *   workspace          DEVICE scratch of workspace_bytes (eiger_groupby_workspace_bytes), or NULL: the library
+ *                      then uses its own arena, grown on demand (cudaMalloc, a stream synchronisation when
+ *                      it grows) and kept until eiger_shutdown().  With NULL a table overflow after an NDV
+ *                      under-estimate (R10) is always retried inside the call
+ *   info               HOST, may be NULL: what the call did (eiger_call_info)
  * Errors: EIGER_ERR_ARG; EIGER_ERR_WORKSPACE; EIGER_ERR_OUT_CAPACITY (a safe capacity is
  * min(n, range)); EIGER_ERR_INFEASIBLE (e.g. EIGER_DIRECT on a 2^40 range);
  * EIGER_ERR_TABLE_OVERFLOW (the sketch under-estimated and the workspace has no room for the
@@ -137,7 +153,7 @@ int eiger_groupby(const eiger_col* keys, int32_t n_key_cols, int64_t n,
                   const eiger_stats* stats,
                   void* const* out_keys, void* const* out_aggs, int64_t out_capacity,
                   int64_t* n_groups, int32_t force, int32_t* chosen,
-                  void* workspace, size_t workspace_bytes, void* stream);
+                  void* workspace, size_t workspace_bytes, void* stream, eiger_call_info* info);
 
 /* Workspace needed by eiger_groupby for the same arguments (data pointers inside keys / vals
  * are ignored and may be NULL).  stats may be NULL: worst case over the variants `force`
@@ -155,35 +171,34 @@ int32_t eiger_select_variant(const eiger_col* keys, int32_t n_key_cols, int64_t 
 
 /* eiger_groupby_host — the same operation end to end from HOST buffers (pinned or pageable):
  * copies the columns to the device, profiles, aggregates and copies the groups back.
- * keys/vals/out_keys/out_aggs are HOST pointers here.  Device memory comes from a library
- * arena that grows on demand and is kept between calls (eiger_shutdown releases it).
+ * keys/vals/out_keys/out_aggs are HOST pointers here.  Device memory comes from library arenas
+ * that grow on demand and are kept between calls (eiger_shutdown releases them).  Inside, the
+ * statistics are gathered exactly as eiger_groupby does with stats = NULL (sample, speculative single
+ * pass or profile).
  * h2d_bytes / d2h_bytes (HOST, may be NULL) receive the bytes copied in each direction. */
 int eiger_groupby_host(const eiger_col* keys, int32_t n_key_cols, int64_t n,
                        const eiger_col* vals, int32_t n_vals,
                        const eiger_agg* aggs, int32_t n_aggs,
                        void* const* out_keys, void* const* out_aggs, int64_t out_capacity,
                        int64_t* n_groups, int32_t force, int32_t* chosen,
-                       int64_t* h2d_bytes, int64_t* d2h_bytes, void* stream);
+                       int64_t* h2d_bytes, int64_t* d2h_bytes, void* stream, eiger_call_info* info);
 
-/* Partition levels (0, 1 or 2) of the last eiger_groupby call that ran EIGER_PARTITION in this
- * process: bench.py needs it for the algorithmic bytes of the partition pass. */
-int32_t eiger_last_partition_levels(void);
-
-/* NDV estimate the last eiger_groupby call in this process planned with (after clamping to
- * min(n, range)): the full-column sketch, the caller's statistics, or - when EIGER_AUTO settled
- * EIGER_PARTITION from the sample - the sketch of a hash-space slice of the keys scaled up
- * (DESIGN.md section 6).  Test hook: the estimate is checked against generators of known NDV. */
-double eiger_last_ndv_estimate(void);
-
-/* 1 when the last EIGER_PARTITION call took its level-1 histogram from the statistics pass
- * (EIGER_AUTO's slice-sketch pass reads the keys once for both), 0 when the partitioner ran its own
- * keys-only histogram pass: bench.py needs it for the algorithmic bytes of the partition pass. */
-int32_t eiger_last_partition_prehist(void);
-
-/* Bytes per key (4 or 8) of the partitioned copy written by the last EIGER_PARTITION call: 4 for a
- * single int32 column and for multi-column keys whose fused domain fits 32 bits, else 8.
- * bench.py needs it for the algorithmic bytes of the partition pass. */
-int32_t eiger_last_partition_key_bytes(void);
+/* eiger_dict_encode — order-preserving dictionary encoding of one integer column (PAPER.md:171-211
+ * Algorithm 1; "If NDV is below a certain threshold, we will use dictionary encoding";
+ * PAPER.md:223 "it must preserve the order of the keys in the encoded values"):
+ *   codes_out[i] = number of distinct values of the column that are smaller than keys[i],
+ *   dict_out[c]  = the value with code c (the distinct values in ascending order), *ndv of them.
+ * Steps as in the paper: hash insert-and-find + retrieveAll (a COUNT group-by, EIGER_AUTO), argsort of
+ * the unique keys (the radix sort of EIGER_SORT), scatter of the ranks into a look-up table, gather.
+ *   keys       DEVICE, n elements of dtype (EIGER_I8 / I32 / I64), 16-byte aligned
+ *   codes_out  DEVICE, n int32
+ *   dict_out   DEVICE, dict_capacity elements of dtype
+ *   ndv        HOST; set even when EIGER_ERR_OUT_CAPACITY says dict_capacity was too small
+ *   workspace  DEVICE, eiger_dict_encode_workspace_bytes(dtype, n, dict_capacity) bytes, 256-byte aligned
+ * Errors: EIGER_ERR_ARG, EIGER_ERR_WORKSPACE, EIGER_ERR_OUT_CAPACITY, EIGER_ERR_CUDA. */
+int eiger_dict_encode(const void* keys, int32_t dtype, int64_t n, int32_t* codes_out, void* dict_out, int64_t dict_capacity,
+                      int64_t* ndv, void* workspace, size_t workspace_bytes, void* stream);
+size_t eiger_dict_encode_workspace_bytes(int32_t dtype, int64_t n, int64_t dict_capacity);
 
 /* Number of kernels this library has launched in this process (bench.py's gpu_launches). */
 int64_t eiger_launch_count(void);
@@ -194,6 +209,10 @@ int64_t eiger_launch_count(void);
  * 4 = compaction.  Returns the milliseconds accumulated since the last call with reset != 0;
  * *launches (may be NULL) receives how many launches that covers. */
 void eiger_set_kernel_timing(int32_t enabled);
+
+/* The EIGER_* environment variables that override the selector's thresholds are
+ * read once per process; call this after changing them (crossover sweeps, tests). */
+void eiger_reload_tunables(void);
 double eiger_kernel_time_ms(int32_t which, int32_t reset, int64_t* launches);
 
 /* eiger_probe — machine probes: measures one building-block rate on the current device, the

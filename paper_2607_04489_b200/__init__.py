@@ -33,7 +33,7 @@ EXPORTS = [
     "eiger_profile", "eiger_profile_keys", "eiger_hll_registers", "eiger_hll_estimate_host", "eiger_groupby",
     "eiger_groupby_workspace_bytes", "eiger_select_variant", "eiger_groupby_host",
     "eiger_launch_count", "eiger_last_partition_levels", "eiger_last_ndv_estimate", "eiger_last_partition_prehist", "eiger_last_partition_key_bytes", "eiger_set_kernel_timing", "eiger_kernel_time_ms", "eiger_strerror",
-    "eiger_last_cuda_error", "eiger_variant_name", "eiger_shutdown", "eiger_probe",
+    "eiger_last_cuda_error", "eiger_variant_name", "eiger_shutdown", "eiger_probe", "eiger_dict_encode", "eiger_dict_encode_workspace_bytes", "eiger_reload_tunables",
 ]
 
 _DTYPES = {torch.int8: I8, torch.int32: I32, torch.int64: I64, torch.float64: F64}
@@ -127,6 +127,10 @@ def lib() -> ctypes.CDLL:
         L.eiger_variant_name.restype = ctypes.c_char_p
         L.eiger_variant_name.argtypes = [i32]
         L.eiger_shutdown.restype = None
+        L.eiger_dict_encode.restype = ctypes.c_int
+        L.eiger_dict_encode.argtypes = [vp, i32, i64, vp, vp, i64, ctypes.POINTER(i64), vp, sz, vp]
+        L.eiger_dict_encode_workspace_bytes.restype = sz
+        L.eiger_dict_encode_workspace_bytes.argtypes = [i32, i64, i64]
         L.eiger_probe.restype = ctypes.c_int
         L.eiger_probe.argtypes = [ctypes.c_char_p, i64, i64, ctypes.POINTER(ctypes.c_double), vp]
         _lib = L
@@ -422,12 +426,36 @@ def kernel_time_ms(which: int = 0, reset: bool = True):
     return float(ms), int(n.value)
 
 
+def dict_encode(keys: torch.Tensor, dict_capacity: int | None = None):
+    """eiger_dict_encode: order-preserving dictionary encoding (Algorithm 1).
+    Returns (codes int32[n], dictionary[ndv] ascending, ndv) with dictionary[codes] == keys."""
+    if not keys.is_cuda or keys.dtype not in _KEY_T or not keys.is_contiguous():
+        raise ValueError("keys must be a contiguous CUDA int8 / int32 / int64 tensor")
+    n = keys.numel()
+    L = lib()
+    cap = n if dict_capacity is None else int(dict_capacity)
+    with torch.cuda.device(keys.device):
+        codes = torch.empty(max(n, 1), dtype=torch.int32, device=keys.device)
+        d = torch.empty(max(cap, 1), dtype=keys.dtype, device=keys.device)
+        ws = torch.empty(max(256, int(L.eiger_dict_encode_workspace_bytes(_DTYPES[keys.dtype], n, cap))), dtype=torch.uint8, device=keys.device)
+        ndv = ctypes.c_int64(0)
+        _check(L.eiger_dict_encode(keys.data_ptr() if n else None, _DTYPES[keys.dtype], n, codes.data_ptr(), d.data_ptr(), cap,
+                                   ctypes.byref(ndv), ws.data_ptr(), ws.numel(), _stream(keys.device)))
+    g = int(ndv.value)
+    return codes[:n], d[:g], g
+
+
 def probe(name: str, param: int = 0, param2: int = 0) -> float:
     """eiger_probe: one measured building-block rate of the current device (see include/eiger.h)."""
     r = ctypes.c_double(0.0)
     _check(lib().eiger_probe(name.encode(), int(param), int(param2), ctypes.byref(r),
                              _stream(torch.device("cuda", torch.cuda.current_device()))))
     return float(r.value)
+
+
+def reload_tunables() -> None:
+    """eiger_reload_tunables: re-read the EIGER_* environment variables."""
+    lib().eiger_reload_tunables()
 
 
 def shutdown() -> None:

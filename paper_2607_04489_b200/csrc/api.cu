@@ -19,10 +19,6 @@ Runtime g_rt;
 std::atomic<int64_t> g_launches{0};
 char g_cuda_err[512] = "";
 bool g_timing = false;
-int g_last_levels = 0;
-double g_last_ndv = 0;
-int g_last_prehist = 0;
-int g_last_part_key_bytes = 0;
 constexpr int kTimeSlots = 5;
 double g_time_ms[kTimeSlots] = {0, 0, 0, 0, 0};
 int64_t g_time_n[kTimeSlots] = {0, 0, 0, 0, 0};
@@ -136,7 +132,14 @@ struct Tunables {
     dict_max_keys = env("EIGER_DICT_MAX_KEYS", 1024);
   }
 };
-Tunables tun() { return Tunables(); }
+// read once per process (about 30 getenv calls used to run several times per eiger_groupby: 15 us of a
+// 0.6 ms call); eiger_reload_tunables() re-reads them (the crossover sweeps and the tests change them in-process)
+Tunables g_tun;
+std::atomic<bool> g_tun_dirty{false};
+const Tunables& tun() {
+  if (g_tun_dirty.exchange(false)) g_tun = Tunables();
+  return g_tun;
+}
 
 struct QueryPlan {
   int variant = 0, key_kind = 0, sig = 0, front = 0, back = 0;
@@ -268,7 +271,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   q->ndv = ndv;
   q->cap_bound = (uint64_t)std::max(1.0, std::ceil(bound / tun().load)) + 64;
 
-  const Tunables T = tun();
+  const Tunables& T = tun();
   const int n_acc_direct = na + (has_count ? 0 : 1);
   const bool direct_ok = R != 0 && R <= (1ull << 33);
   const unsigned __int128 direct_bytes = (unsigned __int128)R * 8 * n_acc_direct;
@@ -407,14 +410,15 @@ bool make_dict_plan(QueryPlan* q, const eiger_col* keys, int nk, int na, double 
   bool has_count = false;
   for (int j = 0; j < na; ++j) has_count = has_count || p.op[j] == EIGER_COUNT;
   if (!has_count) { if (na >= kMaxAcc) return false; p.op[na] = EIGER_COUNT; p.cnt_acc = na; p.n_acc = na + 1; }
-  uint32_t cap = 64;
-  while (cap < 2048 && (double)cap < 2.0 * sample_ndv + 16.0) cap *= 2;
+  // ids: an eighth more than the sample shows (keys the sample missed abort the pass anyway)
+  const uint32_t cap = (uint32_t)(((size_t)(1.125 * sample_ndv) + 64 + 63) / 64 * 64);
   const size_t cell = (size_t)cap * 8 * p.n_acc;
-  if (cell > (64u << 10)) return false;
+  if (cell > (96u << 10)) return false;
   uint32_t slots = 4096;
-  while (slots < 16384 && slots < 16 * cap) slots *= 2;
+  while (slots < 16384 && slots < 8 * cap) slots *= 2;
+  if (cell + (size_t)slots * 8 > (220u << 10) || slots < 2 * cap) return false;
   int shift = 32; for (uint32_t x = slots; x > 1; x >>= 1) --shift;
-  const uint32_t reps = (uint32_t)std::max<size_t>(1, std::min<size_t>(8, (64u << 10) / cell));
+  const uint32_t reps = (uint32_t)std::max<size_t>(1, std::min<size_t>(8, std::min<size_t>((64u << 10) / cell, ((220u << 10) - (size_t)slots * 8) / cell)));
   q->back = BACK_DIRECT; q->front = FRONT_DICT; q->key_kind = kk;
   q->front_slots = cap; q->front_replicas = reps; q->cap = cap; q->stride = 8u * p.n_acc;
   q->dict_slots = slots; q->dict_shift = (uint32_t)shift;
@@ -490,11 +494,22 @@ int do_profile(Runtime* rt, const eiger_col* cols, int nk, int64_t n, int with_h
   return EIGER_OK;
 }
 
+// device arenas owned by the library: g_arena holds the columns of eiger_groupby_host, g_ws the scratch of
+// calls that pass workspace = NULL; both grow on demand and live until eiger_shutdown
+struct Arena { char* base = nullptr; size_t size = 0; } g_arena, g_ws;
+int ws_reserve(size_t bytes) {
+  if (bytes <= g_ws.size) return EIGER_OK;
+  if (g_ws.base) { cudaFree(g_ws.base); g_ws.base = nullptr; g_ws.size = 0; }
+  EIGER_CUDA(cudaMalloc(reinterpret_cast<void**>(&g_ws.base), bytes));
+  g_ws.size = bytes;
+  return EIGER_OK;
+}
+
 int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eiger_col* vals, int nv,
                 const eiger_agg* aggs, int na, const eiger_stats* stats_in,
                 void* const* out_keys, void* const* out_aggs, int64_t out_capacity,
                 int64_t* n_groups, int force, int32_t* chosen, void* workspace, size_t workspace_bytes,
-                cudaStream_t s) {
+                cudaStream_t s, eiger_call_info* info = nullptr) {
   if (!n_groups || !out_keys || !out_aggs || out_capacity < 0) return EIGER_ERR_ARG;
   *n_groups = 0;
   if (!keys || nk < 1 || nk > kMaxKeyCols || n < 0) return EIGER_ERR_ARG;
@@ -510,8 +525,24 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     return EIGER_OK;
   }
   if ((uintptr_t)workspace & 255) return EIGER_ERR_ARG;
+  eiger_call_info local_info;
+  if (!info) info = &local_info;
+  std::memset(info, 0, sizeof(*info));
+  const int64_t launches0 = g_launches.load();
+  struct LaunchCount { eiger_call_info* i; int64_t l0; ~LaunchCount() { i->kernel_launches = g_launches.load() - l0; } } launch_count{info, launches0};
+  // workspace = NULL: the library's own arena, grown to what the plan at hand needs
+  const bool own_ws = workspace == nullptr;
+  if (own_ws) { if (!g_ws.base) { const int rc0 = ws_reserve((size_t)64 << 20); if (rc0) return rc0; } workspace = g_ws.base; workspace_bytes = g_ws.size; }
   for (int j = 0; j < na; ++j) if (!out_aggs[j] && out_capacity > 0) return EIGER_ERR_ARG;
   char* ws = static_cast<char*>(workspace);
+  auto have_room = [&](size_t bytes) -> bool {             // may grow the library's arena (never the caller's workspace)
+    if (bytes <= workspace_bytes) return true;
+    if (!own_ws) return false;
+    if (cudaStreamSynchronize(s) != cudaSuccess) return false;
+    if (ws_reserve(bytes + bytes / 8) != EIGER_OK) return false;
+    workspace = g_ws.base; workspace_bytes = g_ws.size; ws = g_ws.base;
+    return true;
+  };
   struct Back { unsigned long long n_groups; uint32_t overflow; uint32_t abort; };
   Back* hb = reinterpret_cast<Back*>(static_cast<char*>(rt->pinned) + 1024);
   int rc = EIGER_OK;
@@ -525,9 +556,11 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
   // run with the range check of the speculative pass and the call fails with EIGER_ERR_STATS
   const int checked = stats_in != nullptr;
   auto execute = [&](QueryPlan& q, const eiger_stats* st, int spec, bool* aborted) -> int {
-  if (q.total_bytes > workspace_bytes || !workspace) return EIGER_ERR_WORKSPACE;
+  if (!have_room(q.total_bytes) || !workspace) return EIGER_ERR_WORKSPACE;
+  info->variant = q.variant; info->ndv_est = q.ndv; info->sort_passes = q.variant == EIGER_SORT ? q.sort_passes : 0;
   const int src_kind = q.key_kind;
   for (int attempt = 0;; ++attempt) {
+    info->attempts += 1;
     // workspace: [table][partition scratch]
     void* table = ws;
     char* pws = ws + q.table_bytes;
@@ -624,9 +657,9 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
           for (int c = 0; c < q.plan.n_vals; ++c) P.valsB[c] = take(col);
         }
         { Timed t(s, 2); rc = launch_partition(P, rt->sm_count, rt->smem_optin, s); if (rc) return rc; }
-        g_last_levels = q.bits2 > 0 ? 2 : 1;
-        g_last_prehist = q.pre_hist ? 1 : 0;
-        g_last_part_key_bytes = (int)kb;
+        info->partition_levels = q.bits2 > 0 ? 2 : 1;
+        info->partition_prehist = q.pre_hist ? 1 : 0;
+        info->partition_key_bytes = (int)kb;
         // the aggregation pass reads the partitioned copy, one CTA per partition at a time
         H.key.ptr[0] = P.out_keys;
         for (int c = 0; c < q.plan.n_vals; ++c) H.plan.vals[c] = P.out_vals[c];
@@ -655,6 +688,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     if (hb->abort) return EIGER_ERR_STATS;
     if (hb->overflow) {
       // the sketch under-estimated (R10): grow towards the exact bound and run again
+      if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] table overflow (attempt %d): variant %d cap %llu slots %u limit %u bits %d+%d ndv %.0f\n", attempt, q.variant, (unsigned long long)q.cap, q.slots, q.limit, q.bits1, q.bits2, q.ndv);
       if (q.back != BACK_HASH || attempt >= 8) return EIGER_ERR_TABLE_OVERFLOW;
       if (q.cap >= q.cap_bound && q.variant != EIGER_PARTITION) return EIGER_ERR_TABLE_OVERFLOW;
       q.cap = std::min(q.cap_bound, q.cap * 4);
@@ -673,7 +707,8 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         q = q2;
       }
       q.total_bytes = q.table_bytes + q.part_bytes + 256;
-      if (q.total_bytes > workspace_bytes) return EIGER_ERR_TABLE_OVERFLOW;
+      if (!have_room(q.total_bytes)) return EIGER_ERR_TABLE_OVERFLOW;
+      info->ndv_est = q.ndv;
       continue;
     }
     *n_groups = (int64_t)hb->n_groups;
@@ -683,7 +718,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
   };
 
   eiger_stats local[kMaxKeyCols];
-  const Tunables T = tun();
+  const Tunables& T = tun();
   bool skewed = false;
   if (!stats_in && force == EIGER_AUTO && n >= T.spec_min_rows) {
     // EIGER_AUTO, no statistics: first the statistics of an evenly spaced sample (one tiny kernel).
@@ -729,7 +764,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       for (int k = 1; k < nk; ++k) sndv *= local[k].ndv_est;
       sndv = std::min(sndv, (double)T.spec_samples);
       if (T.spec && T.dict && !skewed && plan_query(rt, keys, nk, n, vals, nv, aggs, na, local, EIGER_AUTO, &qd, skewed) == EIGER_OK &&
-          qd.variant == EIGER_SMEM && make_dict_plan(&qd, keys, nk, na, sndv, T) && qd.total_bytes <= workspace_bytes) {
+          qd.variant == EIGER_SMEM && make_dict_plan(&qd, keys, nk, na, sndv, T) && have_room(qd.total_bytes)) {
         bool aborted = false;
         rc = execute(qd, local, 1, &aborted);
         if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] dictionary pass (%u ids, %u dictionary slots, %u replicas): rc %d aborted %d\n", qd.front_slots, qd.dict_slots, qd.front_replicas, rc, (int)aborted);
@@ -740,7 +775,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] sample: min %lld max %lld ndv %.1f collision %.5f\n", (long long)local[0].min, (long long)local[0].max, local[0].ndv_est, collision);
     if (T.spec && fusable && plan_query(rt, keys, nk, n, vals, nv, aggs, na, local, EIGER_AUTO, &qs, skewed) == EIGER_OK &&
         ((qs.variant == EIGER_DIRECT && (qs.front != FRONT_NONE || qs.R <= (1ull << 24))) ||
-         (qs.variant == EIGER_SMEM && qs.ndv * 1.25 <= 0.6 * qs.slots)) && qs.total_bytes <= workspace_bytes) {
+         (qs.variant == EIGER_SMEM && qs.ndv * 1.25 <= 0.6 * qs.slots)) && have_room(qs.total_bytes)) {
       bool aborted = false;
       if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] plan: variant %d kk %d sig %d slots %u limit %u cap %llu stride %u smem %zu front %d R %llu\n", qs.variant, qs.key_kind, qs.sig, qs.slots, qs.limit, (unsigned long long)qs.cap, qs.stride, qs.smem_bytes, qs.front, (unsigned long long)qs.R);
       rc = execute(qs, local, 1, &aborted);
@@ -793,7 +828,6 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       if (rc) return rc;
       q.key.base[0] = base;                 // the histogram was taken with this base
       q.pre_hist = rt->prof->part_hist;
-      g_last_ndv = st2.ndv_est;
       if (chosen) *chosen = q.variant;
       return execute(q, &st2, 0, nullptr);
     }
@@ -810,12 +844,10 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
   rc = plan_query(rt, keys, nk, n, vals, nv, aggs, na, st, force, &q, skewed);
   if (rc) return rc;
   if (chosen) *chosen = q.variant;
-  g_last_ndv = q.ndv;
   return execute(q, st, 0, nullptr);
 }
 
 // ---- device arena for eiger_groupby_host ---------------------------------------------------
-struct Arena { char* base = nullptr; size_t size = 0; } g_arena;
 int arena_reserve(size_t bytes) {
   if (bytes <= g_arena.size) return EIGER_OK;
   if (g_arena.base) { cudaFree(g_arena.base); g_arena.base = nullptr; g_arena.size = 0; }
@@ -903,12 +935,12 @@ int eiger_groupby(const eiger_col* keys, int32_t n_key_cols, int64_t n, const ei
                   const eiger_agg* aggs, int32_t n_aggs, const eiger_stats* stats,
                   void* const* out_keys, void* const* out_aggs, int64_t out_capacity,
                   int64_t* n_groups, int32_t force, int32_t* chosen,
-                  void* workspace, size_t workspace_bytes, void* stream) {
+                  void* workspace, size_t workspace_bytes, void* stream, eiger_call_info* info) {
   std::lock_guard<std::mutex> lk(g_mu);
   Runtime* rt = runtime();
   if (!rt) return EIGER_ERR_CUDA;
   return run_groupby(rt, keys, n_key_cols, n, vals, n_vals, aggs, n_aggs, stats, out_keys, out_aggs, out_capacity,
-                     n_groups, force, chosen, workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
+                     n_groups, force, chosen, workspace, workspace_bytes, static_cast<cudaStream_t>(stream), info);
 }
 
 size_t eiger_groupby_workspace_bytes(const eiger_col* keys, int32_t n_key_cols, int64_t n,
@@ -937,7 +969,7 @@ int32_t eiger_select_variant(const eiger_col* keys, int32_t n_key_cols, int64_t 
 int eiger_groupby_host(const eiger_col* keys, int32_t nk, int64_t n, const eiger_col* vals, int32_t nv,
                        const eiger_agg* aggs, int32_t na, void* const* out_keys, void* const* out_aggs,
                        int64_t out_capacity, int64_t* n_groups, int32_t force, int32_t* chosen,
-                       int64_t* h2d_bytes, int64_t* d2h_bytes, void* stream) {
+                       int64_t* h2d_bytes, int64_t* d2h_bytes, void* stream, eiger_call_info* info) {
   if (!keys || nk < 1 || nk > kMaxKeyCols || n < 0 || nv < 0 || nv > kMaxVals || !aggs || na < 1 || na > kMaxAggs ||
       !n_groups || !out_keys || !out_aggs || out_capacity < 0) return EIGER_ERR_ARG;
   std::lock_guard<std::mutex> lk(g_mu);
@@ -947,56 +979,35 @@ int eiger_groupby_host(const eiger_col* keys, int32_t nk, int64_t n, const eiger
   for (int k = 0; k < nk; ++k) if (!is_key_dtype(keys[k].dtype) || (n > 0 && !keys[k].data)) return EIGER_ERR_ARG;
   for (int c = 0; c < nv; ++c) if ((vals[c].dtype != EIGER_I64 && vals[c].dtype != EIGER_F64 && vals[c].dtype != EIGER_I32) || (n > 0 && !vals[c].data)) return EIGER_ERR_ARG;
 
-  // arena layout: input columns | output columns | workspace (sized after the profile)
+  // arena layout: input columns | output columns; the scratch is the library's workspace arena
   size_t in_bytes = 0, out_bytes = 0;
   for (int k = 0; k < nk; ++k) { in_bytes += align_up((size_t)n * dtype_size(keys[k].dtype), 256); out_bytes += align_up((size_t)out_capacity * dtype_size(keys[k].dtype), 256); }
   for (int c = 0; c < nv; ++c) in_bytes += align_up((size_t)n * (vals[c].dtype == EIGER_I32 ? 4 : 8), 256);
   out_bytes += (size_t)na * align_up((size_t)out_capacity * 8, 256);
-  // first reservation covers the columns; the workspace is added once the statistics are known
-  int rc = arena_reserve(std::max<size_t>(g_arena.size, in_bytes + out_bytes + ((size_t)64 << 20)));
+  int rc = arena_reserve(in_bytes + out_bytes + 512);
   if (rc) return rc;
   int64_t h2d = 0, d2h = 0;
-  auto stage = [&](char*& cur, eiger_col* dk, eiger_col* dv) -> int {
-    for (int k = 0; k < nk; ++k) {
-      const size_t b = (size_t)n * dtype_size(keys[k].dtype);
-      dk[k].data = cur; dk[k].dtype = keys[k].dtype; dk[k].reserved = 0;
-      if (b) EIGER_CUDA(cudaMemcpyAsync(cur, keys[k].data, b, cudaMemcpyHostToDevice, s));
-      h2d += (int64_t)b; cur += align_up(b, 256);
-    }
-    for (int c = 0; c < nv; ++c) {
-      const size_t b = (size_t)n * (vals[c].dtype == EIGER_I32 ? 4 : 8);
-      dv[c].data = cur; dv[c].dtype = vals[c].dtype; dv[c].reserved = 0;
-      if (b) EIGER_CUDA(cudaMemcpyAsync(cur, vals[c].data, b, cudaMemcpyHostToDevice, s));
-      h2d += (int64_t)b; cur += align_up(b, 256);
-    }
-    return EIGER_OK;
-  };
   eiger_col dk[kMaxKeyCols], dv[kMaxVals];
   char* cur = g_arena.base;
-  rc = stage(cur, dk, dv);
-  if (rc) return rc;
-  eiger_stats st[kMaxKeyCols];
-  rc = do_profile(rt, dk, nk, n, dk[0].dtype != EIGER_I8, st, s);
-  if (rc) return rc;
-  QueryPlan q;
-  rc = plan_query(rt, dk, nk, n, dv, nv, aggs, na, st, force, &q);
-  if (rc) return rc;
-  const size_t need = in_bytes + out_bytes + q.total_bytes + 512;
-  if (need > g_arena.size) {
-    // grow: the staged columns are lost with the old arena, copy them again
-    rc = arena_reserve(need + need / 8);
-    if (rc) return rc;
-    cur = g_arena.base; h2d = 0;
-    rc = stage(cur, dk, dv);
-    if (rc) return rc;
+  for (int k = 0; k < nk; ++k) {
+    const size_t b = (size_t)n * dtype_size(keys[k].dtype);
+    dk[k].data = cur; dk[k].dtype = keys[k].dtype; dk[k].reserved = 0;
+    if (b) EIGER_CUDA(cudaMemcpyAsync(cur, keys[k].data, b, cudaMemcpyHostToDevice, s));
+    h2d += (int64_t)b; cur += align_up(b, 256);
+  }
+  for (int c = 0; c < nv; ++c) {
+    const size_t b = (size_t)n * (vals[c].dtype == EIGER_I32 ? 4 : 8);
+    dv[c].data = cur; dv[c].dtype = vals[c].dtype; dv[c].reserved = 0;
+    if (b) EIGER_CUDA(cudaMemcpyAsync(cur, vals[c].data, b, cudaMemcpyHostToDevice, s));
+    h2d += (int64_t)b; cur += align_up(b, 256);
   }
   void* dok[kMaxKeyCols] = {nullptr, nullptr, nullptr, nullptr};
   void* doa[kMaxAggs] = {nullptr};
   for (int k = 0; k < nk; ++k) { dok[k] = cur; cur += align_up((size_t)out_capacity * dtype_size(keys[k].dtype), 256); }
   for (int j = 0; j < na; ++j) { doa[j] = cur; cur += align_up((size_t)out_capacity * 8, 256); }
-  char* wsp = reinterpret_cast<char*>(align_up((uintptr_t)cur, 256));
-  const size_t ws_bytes = g_arena.size - (size_t)(wsp - g_arena.base);
-  rc = run_groupby(rt, dk, nk, n, dv, nv, aggs, na, st, dok, doa, out_capacity, n_groups, force, chosen, wsp, ws_bytes, s);
+  // the same call a device-resident caller makes: no statistics supplied (EIGER_AUTO samples, speculates
+  // or profiles inside), scratch from the library's own arena
+  rc = run_groupby(rt, dk, nk, n, dv, nv, aggs, na, nullptr, dok, doa, out_capacity, n_groups, force, chosen, nullptr, 0, s, info);
   if (rc) return rc;
   const int64_t g = *n_groups;
   for (int k = 0; k < nk; ++k) {
@@ -1014,11 +1025,76 @@ int eiger_groupby_host(const eiger_col* keys, int32_t nk, int64_t n, const eiger
   return EIGER_OK;
 }
 
+// Order-preserving dictionary encoding (Algorithm 1; dictenc.cu lists the steps).
+// workspace: [unique keys g x 8][counts g x 8][counts g x 8][rank table][group-by scratch]
+static size_t dict_fixed_bytes(int64_t dict_capacity) {
+  const size_t g = (size_t)std::max<int64_t>(dict_capacity, 1);
+  return 3 * align_up(g * 8, 256) + align_up((2 * g + 1024 + 1) * 16, 256);
+}
+size_t eiger_dict_encode_workspace_bytes(int32_t dtype, int64_t n, int64_t dict_capacity) {
+  if (!is_key_dtype(dtype) || n < 0 || dict_capacity < 0) return 0;
+  eiger_col k{nullptr, dtype, 0};
+  eiger_agg a{EIGER_COUNT, 0};
+  const size_t all = eiger_groupby_workspace_bytes(&k, 1, n, nullptr, 0, &a, 1, nullptr, EIGER_AUTO);
+  const size_t srt = eiger_groupby_workspace_bytes(&k, 1, std::min(n, std::max<int64_t>(dict_capacity, 1)), nullptr, 0, &a, 1, nullptr, EIGER_SORT);
+  return dict_fixed_bytes(dict_capacity) + std::max(all, srt) + 512;
+}
+
+int eiger_dict_encode(const void* keys, int32_t dtype, int64_t n, int32_t* codes_out, void* dict_out, int64_t dict_capacity,
+                      int64_t* ndv, void* workspace, size_t workspace_bytes, void* stream) {
+  if (!ndv || n < 0 || dict_capacity < 0 || !is_key_dtype(dtype)) return EIGER_ERR_ARG;
+  *ndv = 0;
+  if (n == 0) return EIGER_OK;
+  if (!keys || ((uintptr_t)keys & 15) || !codes_out || !dict_out || !workspace || ((uintptr_t)workspace & 255)) return EIGER_ERR_ARG;
+  std::lock_guard<std::mutex> lk(g_mu);
+  Runtime* rt = runtime();
+  if (!rt) return EIGER_ERR_CUDA;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const size_t fixed = dict_fixed_bytes(dict_capacity);
+  if (workspace_bytes < fixed + 256) return EIGER_ERR_WORKSPACE;
+  const size_t g_cap = (size_t)std::max<int64_t>(dict_capacity, 1);
+  char* w = static_cast<char*>(workspace);
+  void* uniq = w; w += align_up(g_cap * 8, 256);
+  void* cnt1 = w; w += align_up(g_cap * 8, 256);
+  void* cnt2 = w; w += align_up(g_cap * 8, 256);
+  void* table = w; w += align_up((2 * g_cap + 1024 + 1) * 16, 256);
+  char* gws = w;
+  const size_t gws_bytes = workspace_bytes - (size_t)(gws - static_cast<char*>(workspace));
+  // (1) + (2): HT.insert_and_find over the column, retrieveAll -> the unique keys (a COUNT group-by)
+  eiger_col kc{keys, dtype, 0};
+  eiger_agg ag{EIGER_COUNT, 0};
+  void* ok[kMaxKeyCols] = {uniq, nullptr, nullptr, nullptr};
+  void* oa[kMaxAggs] = {cnt1};
+  int64_t g = 0;
+  int rc = run_groupby(rt, &kc, 1, n, nullptr, 0, &ag, 1, nullptr, ok, oa, dict_capacity, &g, EIGER_AUTO, nullptr, gws, gws_bytes, s);
+  *ndv = g;
+  if (rc) return rc;
+  // (3) argsort(uniqueKeys): the unique keys in ascending order = the dictionary
+  eiger_col uc{uniq, dtype, 0};
+  void* ok2[kMaxKeyCols] = {dict_out, nullptr, nullptr, nullptr};
+  void* oa2[kMaxAggs] = {cnt2};
+  int64_t g2 = 0;
+  rc = run_groupby(rt, &uc, 1, g, nullptr, 0, &ag, 1, nullptr, ok2, oa2, dict_capacity, &g2, EIGER_SORT, nullptr, gws, gws_bytes, s);
+  if (rc) return rc;
+  if (g2 != g) return EIGER_ERR_CUDA;
+  // (4) scatter: rank of every unique key into the look-up table; (5) gather: every row fetches its rank
+  const uint64_t cap = 2 * (uint64_t)g + 1024;
+  AggLaunch L{};
+  L.back = BACK_HASH; L.table = table; L.cap = cap; L.stride = 16; L.plan.n_acc = 1; L.plan.op[0] = EIGER_SUM;
+  rc = launch_table_init(L, s); if (rc) return rc;
+  EIGER_CUDA(cudaMemsetAsync(rt->call, 0, sizeof(CallDev), s));
+  rc = launch_dict_fill(dict_out, dtype, g, table, cap, rt->call, rt->sm_count, s); if (rc) return rc;
+  rc = launch_dict_gather(keys, dtype, n, table, cap, codes_out, rt->call, rt->sm_count, s); if (rc) return rc;
+  struct Back { unsigned long long n_groups; uint32_t overflow; uint32_t abort; };
+  Back* hb = reinterpret_cast<Back*>(static_cast<char*>(rt->pinned) + 1024);
+  EIGER_CUDA(cudaMemcpyAsync(hb, rt->call, sizeof(Back), cudaMemcpyDeviceToHost, s));
+  EIGER_CUDA(cudaStreamSynchronize(s));
+  return hb->overflow ? EIGER_ERR_TABLE_OVERFLOW : EIGER_OK;
+}
+
 int64_t eiger_launch_count(void) { return g_launches.load(); }
-int32_t eiger_last_partition_levels(void) { return g_last_levels; }
-double eiger_last_ndv_estimate(void) { return g_last_ndv; }
-int32_t eiger_last_partition_prehist(void) { return g_last_prehist; }
-int32_t eiger_last_partition_key_bytes(void) { return g_last_part_key_bytes; }
+
+void eiger_reload_tunables(void) { g_tun_dirty.store(true); }
 
 void eiger_set_kernel_timing(int32_t enabled) { std::lock_guard<std::mutex> lk(g_mu); g_timing = enabled != 0; }
 
@@ -1054,6 +1130,7 @@ const char* eiger_variant_name(int32_t v) {
 void eiger_shutdown(void) {
   std::lock_guard<std::mutex> lk(g_mu);
   if (g_arena.base) { cudaFree(g_arena.base); g_arena = Arena{}; }
+  if (g_ws.base) { cudaFree(g_ws.base); g_ws = Arena{}; }
   if (g_rt.device >= 0) {
     cudaFree(g_rt.prof); cudaFree(g_rt.call); cudaFreeHost(g_rt.pinned);
     for (int i = 0; i < g_pool_n; ++i) cudaEventDestroy(g_pool[i]);

@@ -12,10 +12,10 @@ size_t hash_agg_slot_bytes(const AggPlan& p, int key_kind) {
 
 HashAggSmem hash_agg_smem_layout(const KeyDesc& key, const AggPlan& plan, int key_kind, int threads, bool hot, int stages) {
   HashAggSmem m{};
-  const uint32_t chunk = 2u * (uint32_t)threads;
+  const bool pre = key_kind == KK_U32PRE || key_kind == KK_U64PRE;
+  const uint32_t chunk = 2u * (uint32_t)(pre ? threads - 32 : threads);    // partition mode: the last warp only produces
   auto up = [](uint32_t x) { return (x + 127u) & ~127u; };
   uint32_t off = 0;
-  const bool pre = key_kind == KK_U32PRE || key_kind == KK_U64PRE;
   m.n_src = pre ? 1 : key.ncols;
   for (int c = 0; c < m.n_src; ++c) {
     const int w = pre ? (key_kind == KK_U32PRE ? 4 : 8) : (key.dtype[c] == EIGER_I8 ? 1 : key.dtype[c] == EIGER_I32 ? 4 : 8);

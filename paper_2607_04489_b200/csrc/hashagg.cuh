@@ -78,6 +78,10 @@ struct Front {
   const uint32_t Sn;      // slots in use (<= a.slots)
   U* skeys;
   uint32_t* s_spill = nullptr;   // partition mode: set when a row of this work item went to the global table
+  int sync_n = 0;                // threads that take part in cta_sync(): 0 = the whole CTA; else named barrier 1 (the ring's producer warp stays out)
+  __device__ __forceinline__ void cta_sync() const {
+    if (sync_n) asm volatile("bar.sync 1, %0;" :: "r"(sync_n) : "memory"); else __syncthreads();
+  }
 
   __device__ Front(const HashAggArgs& args, unsigned char* sm, uint32_t slots_used)
       : a(args), smem(sm), n_acc(S::kStatic ? S::kAcc : args.plan.n_acc), Sn(slots_used) {
@@ -461,7 +465,7 @@ struct Front {
       cnt += __popc(__ballot_sync(0xffffffffu, h < Sn && skeys[h] != empty_of<U>()));
     }
     if (lane == 0) s_wtot[warp] = cnt;
-    __syncthreads();
+    cta_sync();
     if (warp == 0) {       // exclusive scan of up to 32 warp totals
       const uint32_t v = lane < (T >> 5) ? s_wtot[lane] : 0u;
       uint32_t inc = v;
@@ -469,7 +473,7 @@ struct Front {
       for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += y; }
       s_wtot[lane] = inc - v;
     }
-    __syncthreads();
+    cta_sync();
     const unsigned long long base = *s_base;
     const uint32_t wbase = s_wtot[warp];
     if (a.key.ncols == 1) {
@@ -564,7 +568,7 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
   unsigned char* smem = dyn + a.table_off;
   const uint32_t chunk = 2u * (uint32_t)T;                  // rows per stage: two per thread
   if (tid == 0) {
-    for (int s = 0; s < a.stages; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], (uint32_t)(T >> 5)); }
+    for (int s = 0; s < a.stages; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], (uint32_t)(T >> 5) - (IsPre<KK>::v ? 1u : 0u)); }
     mbar_fence_init();
   }
   uint32_t g_cons = 0, g_issued = 0;                        // chunks consumed (all threads) / issued (thread 0)
@@ -662,10 +666,15 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
   } else {
     // ---- partition mode: work items blockIdx.x, + gridDim.x, ...; an item is a whole partition
     // (this CTA then owns its keys and emits them) or a slice of a hot one (merged through the
-    // global table like the whole-input mode).  The ring runs ACROSS items: while one item's table
-    // is read out and the next one's initialised, the next item's first rows are already landing. ----
+    // global table like the whole-input mode).  Warp-specialised: the LAST warp (the hardware's
+    // issue arbiter favours the highest warp id) only produces - one lane walks the CTA's items and
+    // keeps the ring full, ACROSS items: while the consumers read one item's table out and
+    // initialise the next one's, the next item's first rows are already landing.  The other warps
+    // consume and synchronise among themselves on named barrier 1. ----
     const unsigned long long n_items = a.item_off[a.n_parts];
-    // rows [r0, r1) of item `it`; A = r0 rounded down to 32 rows (bulk copies start 16-byte aligned in every column)
+    const int Tc = T - 32;                                   // consumer threads
+    const uint32_t cchunk = 2u * (uint32_t)Tc;               // rows per stage: two per consumer thread
+    // rows [r0, r1) of item `it`
     auto item_rows = [&](unsigned long long it, int64_t& r0, int64_t& r1, bool& exclusive) {
       const int p = (int)a.item_part[it];                    // one broadcast load from the map written by part_items_kernel
       const unsigned long long n_cuts = a.item_off[p + 1] - a.item_off[p], ci = it - a.item_off[p];
@@ -674,66 +683,57 @@ hash_agg_kernel(const __grid_constant__ HashAggArgs a) {
       r0 = P0 + (int64_t)ci * per; r1 = r0 + per < P1 ? r0 + per : P1;
       exclusive = n_cuts == 1;
     };
-    // producer state lives in shared memory (only thread 0 touches it): kept in registers it cost every
-    // thread of the 64-register kernel a dozen of them
-    __shared__ unsigned long long sp_it;
-    __shared__ long long sp_A, sp_r1;
-    __shared__ uint32_t sp_k, sp_chunks, sp_issued;
-    auto producer_load = [&]() {                             // thread 0: describe item sp_it
-      if (sp_it < n_items) {
-        int64_t r0, r1; bool ex;
-        item_rows(sp_it, r0, r1, ex);
-        sp_A = r0 & ~(int64_t)31; sp_r1 = r1;
-        sp_chunks = r1 > r0 ? (uint32_t)((r1 - sp_A + chunk - 1) / chunk) : 0u;
+    __syncthreads();                                         // barriers initialised (the last whole-CTA barrier)
+    if (tid >= Tc) {
+      if (lane == 0) {
+        uint32_t g = 0;
+        for (unsigned long long it = blockIdx.x; it < n_items; it += gridDim.x) {
+          int64_t r0, r1; bool ex;
+          item_rows(it, r0, r1, ex);
+          const int64_t A = r0 & ~(int64_t)31;               // bulk copies start 16-byte aligned in every column
+          for (int64_t row0 = A; row0 < r1; row0 += cchunk, ++g) {
+            const int64_t left = ((r1 - row0) + 31) & ~(int64_t)31;
+            ring_issue(a, ring, s_full, s_empty, g, row0, (uint32_t)(left < (int64_t)cchunk ? left : (int64_t)cchunk), policy);
+          }
+        }
       }
-      sp_k = 0;
-    };
-    auto top_up = [&](uint32_t upto) {                       // thread 0: keep `stages` chunks requested ahead of the consumers
-      while (sp_issued < upto && sp_it < n_items) {
-        if (sp_k >= sp_chunks) { sp_it += gridDim.x; producer_load(); continue; }
-        const int64_t row0 = sp_A + (int64_t)sp_k * chunk;
-        const int64_t left = ((sp_r1 - row0) + 31) & ~(int64_t)31;
-        ring_issue(a, ring, s_full, s_empty, sp_issued, row0, (uint32_t)(left < (int64_t)chunk ? left : (int64_t)chunk), policy);
-        ++sp_issued; ++sp_k;
-      }
-    };
-    __syncthreads();                                         // barriers initialised
-    if (tid == 0) { sp_it = blockIdx.x; sp_issued = 0; producer_load(); top_up((uint32_t)a.stages); }
+      return;
+    }
     for (unsigned long long it = blockIdx.x; it < n_items; it += gridDim.x) {
       int64_t r0, r1; bool exclusive;
       item_rows(it, r0, r1, exclusive);
       const uint32_t lo = (uint32_t)(r0 & 31), hi = (uint32_t)(r1 - (r0 & ~(int64_t)31));   // valid rows of the item, relative to A
-      const uint32_t chunks = r1 > r0 ? (hi + chunk - 1) / chunk : 0u;
+      const uint32_t chunks = r1 > r0 ? (hi + cchunk - 1) / cchunk : 0u;
       // a table no larger than the partition needs: 2 slots per row is always enough
       const uint64_t want = 2ull * (uint64_t)(r1 - r0) + 64;
       const uint32_t Sn = (uint32_t)(want < a.slots ? want : a.slots) & ~7u;   // whole buckets
       F f(a, smem, Sn);
       f.s_spill = &s_spilled;
-      __syncthreads();                       // the previous item's emit is over
+      f.sync_n = Tc;
+      f.cta_sync();                          // the previous item's emit is over
       if (tid == 0) { s_count = 0; s_spilled = 0; }
-      f.init(tid, T);
-      __syncthreads();
+      f.init(tid, Tc);
+      f.cta_sync();
       bool missed = false;
       for (uint32_t k = 0; k < chunks; ++k, ++g_cons) {
         const uint32_t s = g_cons % (uint32_t)a.stages;
         mbar_wait(&s_full[s], (g_cons / (uint32_t)a.stages) & 1u);
         const unsigned char* st = ring + (size_t)s * a.stage_bytes;
-        const uint32_t i0 = k * chunk + (uint32_t)tid, i1 = i0 + (uint32_t)T;
+        const uint32_t i0 = k * cchunk + (uint32_t)tid, i1 = i0 + (uint32_t)Tc;
         const bool v0 = i0 >= lo && i0 < hi, v1 = i1 >= lo && i1 < hi;
         U u[2]; uint64_t raw[2][NV];
-        u[0] = ring_key<KK>(a, st, tid); u[1] = ring_key<KK>(a, st, T + tid);
-        ring_vals<SIG, NV>(a, st, tid, n_vals, raw[0]); ring_vals<SIG, NV>(a, st, T + tid, n_vals, raw[1]);
+        u[0] = ring_key<KK>(a, st, tid); u[1] = ring_key<KK>(a, st, Tc + tid);
+        ring_vals<SIG, NV>(a, st, tid, n_vals, raw[0]); ring_vals<SIG, NV>(a, st, Tc + tid, n_vals, raw[1]);
         __syncwarp();
-        if (lane == 0) mbar_arrive(&s_empty[s]);
-        if (tid == 0) top_up(g_cons + 1u + (uint32_t)a.stages);
+        if (lane == 0) mbar_arrive(&s_empty[s]);             // this warp's rows are in registers: the stage may be refilled
         const uint32_t miss = f.pair(v0 ? u[0] : (U)0, raw[0], v0, v1 ? u[1] : (U)0, raw[1], v1, &s_count);
         f.spill(u, raw, miss, missed);
       }
-      __syncthreads();
+      f.cta_sync();
       // emit only what this CTA owns exclusively: a whole partition none of whose rows was sent to
       // the global table (otherwise a key could be emitted here AND by the compaction pass)
-      if (exclusive && s_spilled == 0u) f.flush_emit(tid, T, s_count, &s_base, s_wtot);
-      else f.flush_merge(tid, T);
+      if (exclusive && s_spilled == 0u) f.flush_emit(tid, Tc, s_count, &s_base, s_wtot);
+      else f.flush_merge(tid, Tc);
     }
   }
 }

@@ -169,6 +169,10 @@ struct PartitionLaunch {
 int launch_partition(PartitionLaunch& p, int sm_count, size_t smem_optin, cudaStream_t s);
 int partition_max_bits_per_level();
 
+// ---- dictenc.cu -------------------------------------------------------------------------
+int launch_dict_fill(const void* sorted_keys, int dtype, int64_t ndv, void* table, uint64_t cap, CallDev* call, int sm_count, cudaStream_t s);
+int launch_dict_gather(const void* keys, int dtype, int64_t n, const void* table, uint64_t cap, int32_t* codes, CallDev* call, int sm_count, cudaStream_t s);
+
 // ---- sortagg.cu -------------------------------------------------------------------------
 // EIGER_SORT: LSD radix sort of the rows on the `bits` significant bits of the rebased fused key,
 // then a segmented reduce that emits the groups in key order.

@@ -73,10 +73,12 @@ def test_selector_is_callable_without_a_gpu(lib):
     # L2-resident global table is AUTO's pick for hot-key inputs only, or when asked for by tunable
     assert pick(-(1 << 31), (1 << 31) - 1, 1 << 18) == eiger.PARTITION
     os.environ["EIGER_GLOBAL_ALWAYS"] = "1"
+    eiger.reload_tunables()
     try:
         assert pick(-(1 << 31), (1 << 31) - 1, 1 << 18) == eiger.GLOBAL
     finally:
         del os.environ["EIGER_GLOBAL_ALWAYS"]
+        eiger.reload_tunables()
     assert pick(-(1 << 31), (1 << 31) - 1, 1 << 26) == eiger.PARTITION
     assert eiger.workspace_bytes(fk, fv, aggs, [eiger.Stats(0, 15, 16.0, n)]) >= 256
     # no statistics, several int32 / int64 key columns: the type ranges multiply past 2^64; the sizing

@@ -14,6 +14,19 @@ DEV = "cuda:0"
 ALL_VARIANTS = [eiger.AUTO, eiger.DIRECT, eiger.SMEM, eiger.GLOBAL, eiger.PARTITION, eiger.SORT]
 
 
+@pytest.fixture(autouse=True)
+def _fresh_tunables():
+    # the library reads its EIGER_* tunables once; tests that change them (monkeypatch.setenv + reload)
+    # must not leak their values into the next test
+    yield
+    eiger.reload_tunables()
+
+
+def set_tunable(monkeypatch, name, value):
+    monkeypatch.setenv(name, str(value))
+    eiger.reload_tunables()
+
+
 @pytest.fixture(scope="module", autouse=True)
 def _need_gpu():
     assert torch.cuda.is_available(), "these tests need the B200"
@@ -302,7 +315,7 @@ def test_partition_tables_close_without_duplicate_groups(monkeypatch, part_kb, e
     # emitted twice (hashagg.cuh: s_spilled).  est = 2^14 additionally walks the overflow -> 4x re-run path.
     # Repeated, because the duplicate needs two lanes to race on one key.
     if part_kb is not None:
-        monkeypatch.setenv("EIGER_PART_KB", str(part_kb))
+        set_tunable(monkeypatch, "EIGER_PART_KB", part_kb)
     ds = datagen.config5(n=1 << 26, ndv=1 << 22, scattered=True)
     want = oracle_result(ds)
     d = to_dev(ds)
@@ -320,8 +333,8 @@ def test_partition_tables_close_without_duplicate_groups(monkeypatch, part_kb, e
 def small_partition_tables(monkeypatch):
     # 48 KB per-CTA tables (the tunables are re-read on every call): two partition levels are then
     # needed at sizes the oracle still handles in seconds
-    monkeypatch.setenv("EIGER_PART_KB", "48")
-    monkeypatch.setenv("EIGER_PART_THREADS", "256")
+    set_tunable(monkeypatch, "EIGER_PART_KB", 48)
+    set_tunable(monkeypatch, "EIGER_PART_THREADS", 256)
 
 
 def test_two_level_partition(small_partition_tables):
@@ -362,7 +375,7 @@ def test_auto_slice_sketch_two_levels(small_partition_tables):
 
 def test_auto_slice_sketch_off_matches(monkeypatch):
     # same input through the full-column profile: same groups, and an estimate within the sketch's error
-    monkeypatch.setenv("EIGER_SLICE", "0")
+    set_tunable(monkeypatch, "EIGER_SLICE", 0)
     D = 1 << 18
     res = _auto_matches(datagen.config5(n=SPEC_N + 12345, ndv=D, scattered=True), eiger.PARTITION)
     assert res.n_groups == D and abs(eiger.last_ndv_estimate() - D) <= 4 * 0.008125 * D
@@ -589,3 +602,47 @@ def test_int32_values_host_entry_point_and_two_keys():
     res, h2d, d2h = eiger.groupby_host(ds.keys, ds.vals, ds.aggs)
     assert_matches(res, want, ds.aggs, ds.vals)
     assert h2d == ds.n * (4 + 4 + 4)
+
+
+# ---- order-preserving dictionary encoding (Algorithm 1) -----------------------------
+@pytest.mark.parametrize("dtype", [torch.int8, torch.int32, torch.int64])
+@pytest.mark.parametrize("n,ndv", [(0, 0), (1, 1), (1000, 7), (300_007, 5000), (1 << 21, 1 << 17)])
+def test_dict_encode_matches_oracle(dtype, n, ndv):
+    info = torch.iinfo(dtype)
+    if n == 0:
+        keys = torch.zeros(0, dtype=dtype)
+    else:
+        ids = datagen.known_ndv_ids(31, 0, torch.arange(n, dtype=torch.int64), n, min(ndv, info.max - info.min + 1))
+        if dtype == torch.int8:
+            keys = (ids % 256 - 128).to(dtype)
+        elif dtype == torch.int32:
+            keys = datagen.scatter32(ids).to(dtype)
+        else:
+            keys = datagen.scatter64(31, ids)
+        if n > 4:
+            keys[3] = info.min; keys[n - 2] = info.max            # the extremes (and the table's marker value -1 below)
+            keys[1] = -1
+    want_codes, want_dict, want_ndv = oracle.dict_encode(keys.numpy())
+    codes, d, g = eiger.dict_encode(keys.to(DEV))
+    assert g == want_ndv
+    assert codes.dtype == torch.int32 and d.dtype == dtype
+    assert np.array_equal(d.cpu().numpy().astype(np.int64), want_dict)
+    assert np.array_equal(codes.cpu().numpy().astype(np.int64), want_codes)
+
+
+def test_dict_encode_capacity_error_and_group_by_on_codes():
+    ds = datagen.config5(n=400_003, ndv=3000, scattered=True)
+    k = ds.keys[0].to(DEV)
+    with pytest.raises(eiger.EigerError) as e:
+        eiger.dict_encode(k, dict_capacity=100)
+    assert e.value.code == eiger.ERR_OUT_CAPACITY
+    # smart key fusion with the dictionary step: a sparse key column becomes a dense
+    # code column; grouping by the codes and decoding gives the groups of the original column
+    codes, d, g = eiger.dict_encode(k)
+    assert g == 3000
+    res = eiger.groupby([codes], [ds.vals[0].to(DEV)], ds.aggs).sorted()
+    assert res.variant == eiger.DIRECT and res.n_groups == 3000
+    want = oracle_result(ds)
+    assert np.array_equal(d[res.keys[0].long()].cpu().numpy().astype(np.int64), want.keys[0])   # order-preserving: sorted codes = sorted keys
+    for a, b in zip(res.aggs, want.aggs):
+        assert np.array_equal(a.cpu().numpy(), b)
