@@ -280,12 +280,12 @@ def main(argv=None):
     # dominant kernel and its algorithmic bytes per launch
     dom = max(("aggregate", "partition", "profile"), key=lambda k: kt[k][0])
     key_bytes = sum(k.element_size() for k in ds.keys)
-    part_key = eiger.last_partition_key_bytes() if last["res"].variant == eiger.PARTITION else 8
+    part_key = res.info["partition_key_bytes"] if res.variant == eiger.PARTITION else 8
     part_row = part_key + 8 * len(ds.vals)   # B': one row of the partitioned copy
     out_row = key_bytes + 8 * len(ds.aggs)
-    levels = eiger.last_partition_levels() if res.variant == eiger.PARTITION else 0
+    levels = res.info["partition_levels"] if res.variant == eiger.PARTITION else 0
     # EIGER_AUTO's slice-sketch pass already took the level-1 histogram: no keys-only read in the partition pass
-    hist1_bytes = 0 if (res.variant == eiger.PARTITION and eiger.last_partition_prehist()) else ds.n * key_bytes
+    hist1_bytes = 0 if (res.variant == eiger.PARTITION and res.info["partition_prehist"]) else ds.n * key_bytes
     alg_bytes = {"aggregate": in_bytes if res.variant != eiger.PARTITION else ds.n * part_row + res.n_groups * out_row,
                  "partition": hist1_bytes + ds.n * (ds.row_bytes + part_row) + max(0, levels - 1) * ds.n * (part_row - 8 * len(ds.vals) + 2 * part_row),
                  "profile": ds.n * key_bytes}[dom]

@@ -32,7 +32,7 @@ HLL_M = 1 << 14
 EXPORTS = [
     "eiger_profile", "eiger_profile_keys", "eiger_hll_registers", "eiger_hll_estimate_host", "eiger_groupby",
     "eiger_groupby_workspace_bytes", "eiger_select_variant", "eiger_groupby_host",
-    "eiger_launch_count", "eiger_last_partition_levels", "eiger_last_ndv_estimate", "eiger_last_partition_prehist", "eiger_last_partition_key_bytes", "eiger_set_kernel_timing", "eiger_kernel_time_ms", "eiger_strerror",
+    "eiger_launch_count", "eiger_set_kernel_timing", "eiger_kernel_time_ms", "eiger_strerror",
     "eiger_last_cuda_error", "eiger_variant_name", "eiger_shutdown", "eiger_probe", "eiger_dict_encode", "eiger_dict_encode_workspace_bytes", "eiger_reload_tunables",
 ]
 
@@ -57,6 +57,15 @@ class _Stats(ctypes.Structure):
     _fields_ = [("min", ctypes.c_int64), ("max", ctypes.c_int64), ("ndv_est", ctypes.c_double), ("n", ctypes.c_int64)]
 
 
+class _CallInfo(ctypes.Structure):
+    _fields_ = [("variant", ctypes.c_int32), ("attempts", ctypes.c_int32), ("partition_levels", ctypes.c_int32),
+                ("partition_prehist", ctypes.c_int32), ("partition_key_bytes", ctypes.c_int32), ("sort_passes", ctypes.c_int32),
+                ("ndv_est", ctypes.c_double), ("kernel_launches", ctypes.c_int64)]
+
+    def as_dict(self) -> dict:
+        return {name: getattr(self, name) for name, _ in self._fields_}
+
+
 @dataclass
 class Stats:
     min: int
@@ -71,6 +80,7 @@ class GroupByResult:
     aggs: list          # one tensor per aggregate (int64 or float64)
     n_groups: int
     variant: int
+    info: dict = None   # eiger_call_info of the call: attempts, partition_levels, ndv_est, kernel_launches, ...
 
     def sorted(self) -> "GroupByResult":
         """Groups ordered by key (for comparisons)."""
@@ -79,7 +89,7 @@ class GroupByResult:
         order = torch.arange(self.n_groups, device=self.keys[0].device)
         for k in reversed(self.keys):
             order = order[torch.sort(k[order], stable=True).indices]
-        return GroupByResult([k[order] for k in self.keys], [a[order] for a in self.aggs], self.n_groups, self.variant)
+        return GroupByResult([k[order] for k in self.keys], [a[order] for a in self.aggs], self.n_groups, self.variant, self.info)
 
 
 _lib = None
@@ -104,7 +114,7 @@ def lib() -> ctypes.CDLL:
         L.eiger_hll_estimate_host.argtypes = [vp]
         L.eiger_groupby.restype = ctypes.c_int
         L.eiger_groupby.argtypes = [vp, i32, i64, vp, i32, vp, i32, vp, vp, vp, i64,
-                                    ctypes.POINTER(i64), i32, ctypes.POINTER(i32), vp, sz, vp]
+                                    ctypes.POINTER(i64), i32, ctypes.POINTER(i32), vp, sz, vp, ctypes.POINTER(_CallInfo)]
         L.eiger_groupby_workspace_bytes.restype = sz
         L.eiger_groupby_workspace_bytes.argtypes = [vp, i32, i64, vp, i32, vp, i32, vp, i32]
         L.eiger_select_variant.restype = i32
@@ -112,12 +122,8 @@ def lib() -> ctypes.CDLL:
         L.eiger_groupby_host.restype = ctypes.c_int
         L.eiger_groupby_host.argtypes = [vp, i32, i64, vp, i32, vp, i32, vp, vp, i64,
                                          ctypes.POINTER(i64), i32, ctypes.POINTER(i32),
-                                         ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
+                                         ctypes.POINTER(i64), ctypes.POINTER(i64), vp, ctypes.POINTER(_CallInfo)]
         L.eiger_launch_count.restype = i64
-        L.eiger_last_partition_levels.restype = i32
-        L.eiger_last_ndv_estimate.restype = ctypes.c_double
-        L.eiger_last_partition_prehist.restype = i32
-        L.eiger_last_partition_key_bytes.restype = i32
         L.eiger_set_kernel_timing.argtypes = [i32]
         L.eiger_kernel_time_ms.restype = ctypes.c_double
         L.eiger_kernel_time_ms.argtypes = [i32, i32, ctypes.POINTER(i64)]
@@ -238,18 +244,11 @@ def workspace_bytes(keys, vals, aggs, stats=None, force: int = AUTO) -> int:
 
 
 class Workspace:
-    """A reusable device scratch buffer (grown on demand) plus reusable output columns."""
+    """Reusable output columns (the scratch memory is the library's own arena)."""
 
     def __init__(self, device):
         self.device = device
-        self.buf = None
         self.out = {}
-
-    def scratch(self, nbytes: int) -> torch.Tensor:
-        if self.buf is None or self.buf.numel() < nbytes:
-            self.buf = None
-            self.buf = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=self.device)
-        return self.buf
 
     def column(self, name, n: int, dtype) -> torch.Tensor:
         t = self.out.get(name)
@@ -263,9 +262,12 @@ def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int |
             workspace: Workspace | None = None) -> GroupByResult:
     """eiger_groupby on device columns.
 
-    keys: 1-4 CUDA integer tensors; vals: CUDA int64/float64 tensors; aggs: [(op, val_col)].
-    With stats=None the key columns are profiled first (eiger_profile), which is what the
-    adaptive path's time includes; pass stats from profile() to skip that.
+    keys: 1-4 CUDA integer tensors; vals: CUDA int64 / float64 / int32 tensors; aggs: [(op, val_col)].
+    With stats=None the statistics are gathered inside the call (that is what the adaptive path's
+    time includes); pass stats from profile() to skip that.  Scratch memory is the library's own arena
+    (workspace = NULL at the C ABI); `workspace` only keeps the output columns between calls.  The one
+    decision taken here: when the caller fixed no out_capacity and the library reports more groups than
+    the output columns hold (EIGER_ERR_OUT_CAPACITY carries the count), allocate that many and call again.
     """
     if isinstance(keys, torch.Tensor):
         keys = [keys]
@@ -279,92 +281,26 @@ def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int |
         raise ValueError("column length mismatch")
     L = lib()
     ws = workspace or Workspace(dev)
-    def out_cols(cap):
-        ok = [ws.column(("k", i), cap, k.dtype) for i, k in enumerate(keys)]
-        oa = [ws.column(("a", j), cap, torch.float64 if (op != COUNT and vals[c].dtype == torch.float64) else torch.int64)
-              for j, (op, c) in enumerate(aggs)]
-        return ok, oa
-
+    kc, vc, ac, sc = _cols(keys, _KEY_T), _cols(vals, _VAL_T), _aggs(aggs), _stats_arr(stats)
+    have = min([t.numel() for t in ws.out.values()], default=0)
+    cap = out_capacity if out_capacity is not None else min(max(have, 1 << 20), max(n, 1))
     with torch.cuda.device(dev):
-        if stats is None and n > 0:
-            # one library call, statistics gathered inside it (that is what EIGER_AUTO's time is):
-            # with whatever scratch this Workspace already holds; if the plan the library arrives
-            # at needs more room than that, profile here and size exactly (first call only)
-            kc, vc, ac = _cols(keys, _KEY_T), _cols(vals, _VAL_T), _aggs(aggs)
-            buf = ws.scratch(max(64 << 20, ws.buf.numel() if ws.buf is not None else 0))
-            have = min([t.numel() for t in ws.out.values()], default=0)
-            cap = out_capacity if out_capacity is not None else max(have, 1 << 20)
-            ok, oa = out_cols(cap)
-            okp = (ctypes.c_void_p * 4)(*[t.data_ptr() for t in ok])
-            oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
-            ng, chosen = ctypes.c_int64(0), ctypes.c_int32(0)
-            stats_known = None
-            for attempt in range(3):
-                rc = L.eiger_groupby(kc, len(keys), n, vc, len(vals), ac, len(aggs), None, okp, oap, cap,
-                                     ctypes.byref(ng), force, ctypes.byref(chosen), buf.data_ptr(), buf.numel(), _stream(dev))
-                if rc == OK:
-                    g = int(ng.value)
-                    return GroupByResult([t[:g] for t in ok], [t[:g] for t in oa], g, int(chosen.value))
-                if rc == ERR_OUT_CAPACITY and out_capacity is None:
-                    cap = int(ng.value)                      # the library says how many groups there are
-                elif rc == ERR_WORKSPACE:
-                    # room for whichever variant the library may pick with these statistics
-                    stats_known = stats_known or profile_keys(keys)
-                    sk = _stats_arr(stats_known)
-                    need = max(int(L.eiger_groupby_workspace_bytes(kc, len(keys), n, vc, len(vals), ac, len(aggs), sk, v))
-                               for v in ((GLOBAL, PARTITION) if force == AUTO else (force,)))
-                    if need <= buf.numel():
-                        break
-                    buf = ws.scratch(need + (need >> 3))
-                    if out_capacity is None and len(stats_known) == 1:
-                        cap = max(cap, int(stats_known[0].ndv_est * 1.25) + 1024)
-                else:
-                    break
-                ok, oa = out_cols(cap)
-                okp = (ctypes.c_void_p * 4)(*[t.data_ptr() for t in ok])
-                oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
-            if rc not in (ERR_WORKSPACE, ERR_TABLE_OVERFLOW) and not (rc == ERR_OUT_CAPACITY and out_capacity is None):
-                _check(rc)
-            stats = profile_keys(keys)
-        kc, vc, ac, sc = _cols(keys, _KEY_T), _cols(vals, _VAL_T), _aggs(aggs), _stats_arr(stats)
-        for attempt in range(3):
-            nbytes = int(L.eiger_groupby_workspace_bytes(kc, len(keys), n, vc, len(vals), ac, len(aggs), sc, force))
-            if nbytes == 0:
-                # bad arguments or an infeasible forced variant: let eiger_groupby say which
-                nbytes = 256
-            if out_capacity is None:
-                cap = n
-                if stats:
-                    rng = 1
-                    for s in stats:
-                        rng *= (s.max - s.min + 1)
-                    cap = max(0, min(n, rng))
-                    if force in (AUTO, SMEM, GLOBAL, PARTITION, SORT) and stats and len(stats) == 1:
-                        cap = min(cap, int(stats[0].ndv_est * 1.25) + 1024)
-            else:
-                cap = out_capacity
-            buf = ws.scratch(nbytes)
+        for attempt in range(2):
             ok = [ws.column(("k", i), cap, k.dtype) for i, k in enumerate(keys)]
             oa = [ws.column(("a", j), cap, torch.float64 if (op != COUNT and vals[c].dtype == torch.float64) else torch.int64)
                   for j, (op, c) in enumerate(aggs)]
             okp = (ctypes.c_void_p * 4)(*[t.data_ptr() for t in ok])
             oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
-            ng, chosen = ctypes.c_int64(0), ctypes.c_int32(0)
+            ng, chosen, info = ctypes.c_int64(0), ctypes.c_int32(0), _CallInfo()
             rc = L.eiger_groupby(kc, len(keys), n, vc, len(vals), ac, len(aggs), sc, okp, oap, cap,
-                                 ctypes.byref(ng), force, ctypes.byref(chosen), buf.data_ptr(), buf.numel(), _stream(dev))
-            if rc == ERR_OUT_CAPACITY and out_capacity is None:
-                out_capacity = int(ng.value)
-                continue
-            if rc == ERR_TABLE_OVERFLOW and stats is not None and attempt < 2:
-                # the sketch under-estimated: size for the exact bound and run again
-                stats = [Stats(s.min, s.max, float(min(n, s.max - s.min + 1)), s.n) for s in stats]
-                sc = _stats_arr(stats)
-                out_capacity = None
+                                 ctypes.byref(ng), force, ctypes.byref(chosen), None, 0, _stream(dev), ctypes.byref(info))
+            if rc == ERR_OUT_CAPACITY and out_capacity is None and attempt == 0:
+                cap = int(ng.value)
                 continue
             _check(rc)
             g = int(ng.value)
-            return GroupByResult([t[:g] for t in ok], [t[:g] for t in oa], g, int(chosen.value))
-    raise EigerError(ERR_TABLE_OVERFLOW, "could not size the table")
+            return GroupByResult([t[:g] for t in ok], [t[:g] for t in oa], g, int(chosen.value), info.as_dict())
+    raise EigerError(ERR_OUT_CAPACITY, "more groups than the output columns hold")
 
 
 def groupby_host(keys, vals, aggs, force: int = AUTO, out_capacity: int | None = None, out=None):
@@ -387,33 +323,17 @@ def groupby_host(keys, vals, aggs, force: int = AUTO, out_capacity: int | None =
         ok, oa = out
     okp = (ctypes.c_void_p * 4)(*[t.data_ptr() for t in ok])
     oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
-    ng, chosen, h2d, d2h = ctypes.c_int64(0), ctypes.c_int32(0), ctypes.c_int64(0), ctypes.c_int64(0)
+    ng, chosen, h2d, d2h, info = ctypes.c_int64(0), ctypes.c_int32(0), ctypes.c_int64(0), ctypes.c_int64(0), _CallInfo()
     rc = L.eiger_groupby_host(_cols(keys, _KEY_T), len(keys), n, _cols(vals, _VAL_T), len(vals), _aggs(aggs), len(aggs),
                               okp, oap, cap, ctypes.byref(ng), force, ctypes.byref(chosen),
-                              ctypes.byref(h2d), ctypes.byref(d2h), _stream(torch.device("cuda", torch.cuda.current_device())))
+                              ctypes.byref(h2d), ctypes.byref(d2h), _stream(torch.device("cuda", torch.cuda.current_device())), ctypes.byref(info))
     _check(rc)
     g = int(ng.value)
-    return GroupByResult([t[:g] for t in ok], [t[:g] for t in oa], g, int(chosen.value)), int(h2d.value), int(d2h.value)
+    return GroupByResult([t[:g] for t in ok], [t[:g] for t in oa], g, int(chosen.value), info.as_dict()), int(h2d.value), int(d2h.value)
 
 
 def launch_count() -> int:
     return int(lib().eiger_launch_count())
-
-
-def last_partition_levels() -> int:
-    return int(lib().eiger_last_partition_levels())
-
-
-def last_ndv_estimate() -> float:
-    return float(lib().eiger_last_ndv_estimate())
-
-
-def last_partition_prehist() -> bool:
-    return bool(lib().eiger_last_partition_prehist())
-
-
-def last_partition_key_bytes() -> int:
-    return int(lib().eiger_last_partition_key_bytes())
 
 
 def set_kernel_timing(enabled: bool) -> None:

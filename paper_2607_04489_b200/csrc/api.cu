@@ -94,6 +94,8 @@ struct Tunables {
   int slice;                          // EIGER_AUTO sizes PARTITION from a hash-space slice sketch instead of the full profile
   double slice_min_keys;              // distinct keys wanted in the slice (relative error 1 / sqrt of it)
   double fused_sketch_min_range;      // multi-column keys: sketch the fused key when the ranges multiply to more than this
+  int part_full_table;                // EIGER_PARTITION reserves the full-size global table when partitions may be cut (round-1 behaviour)
+  int pack_stride;                    // global hash table slots of 40 / 48 bytes are not padded to 64
   int dict;                           // EIGER_AUTO: scattered keys the sample names completely get a dictionary + direct array (FRONT_DICT)
   double dict_max_keys;               // ... while the sample holds at most this many distinct keys
   Tunables() {
@@ -129,7 +131,9 @@ struct Tunables {
     slice = (int)env("EIGER_SLICE", 1);
     slice_min_keys = env("EIGER_SLICE_MIN_KEYS", 2048);
     dict = (int)env("EIGER_DICT", 1);
-    dict_max_keys = env("EIGER_DICT_MAX_KEYS", 1024);
+    pack_stride = (int)env("EIGER_PACK_STRIDE", 1);
+    part_full_table = (int)env("EIGER_PART_FULL_TABLE", 0);
+    dict_max_keys = env("EIGER_DICT_MAX_KEYS", 4600);   // measured: scattered 2^12 keys 0.90 ms through the dictionary, 1.25 ms through the hash table
   }
 };
 // read once per process (about 30 getenv calls used to run several times per eiger_groupby: 15 us of a
@@ -298,7 +302,15 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   const size_t part_tab = table_bytes_for(pre_kind, T.part_threads, false, T.part_table_bytes);
   const uint32_t smem_slots = (uint32_t)std::max<size_t>(64, (smem_tab - 64) / slot_bytes) & ~7u;   // planes stay 8-byte aligned
   const uint32_t part_slots = (uint32_t)std::max<size_t>(64, (part_tab - 64) / part_slot_bytes) & ~7u;
-  const uint32_t hash_stride = [&] { uint32_t s = 16; while (s < 8u * (1 + na)) s *= 2; return s; }();
+  // slot = [key][accumulators]: rounded up to a power of two (a slot then never straddles a 32-byte
+  // sector more than its size requires), except where that wastes a quarter of the table or more:
+  // C3's four aggregates need 40 bytes; 64-byte slots make its table 132 MB (past the 126 MB L2), packed
+  // 40-byte slots 84 MB - and a 40-byte slot at a multiple of 8 covers two sectors either way
+  const uint32_t hash_stride = [&] {
+    uint32_t s = 16; while (s < 8u * (1 + na)) s *= 2;
+    const uint32_t packed = 8u * (1 + na);
+    return (T.pack_stride && packed > 32 && 4 * packed <= 3 * s) ? packed : s;
+  }();
   auto hash_cap = [&](double g) { return (uint64_t)std::max(1024.0, std::ceil(g * (1.0 + 4 * kSigma) * 1.02 / T.load)); };
 
   int variant = force;
@@ -371,7 +383,12 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
       q->cap = std::min(q->cap_bound, (uint64_t)std::max(4096.0, ndv / 64.0));
       q->cap_hot = std::min(q->cap_bound, hash_cap(ndv));
       const size_t P1 = (size_t)1 << q->bits1, P = (size_t)1 << (q->bits1 + q->bits2);
-      if (n / (int64_t)P >= 32768) q->cap = q->cap_hot;
+      // (round 1 reserved the full-size table whenever the average partition held >= 32768 rows, because a
+      // partition of more than twice the average is cut into items that merge through it: for uniform keys
+      // nothing is ever cut and the unused 1 GB table cost 0.45 ms of init + compaction per call at
+      // NDV 2^24.  A skewed input that does cut partitions now overflows the small table once and is
+      // re-run with 4x the capacity, R10; EIGER_AUTO keeps skewed inputs away from this variant anyway)
+      if (T.part_full_table && n / (int64_t)P >= 32768) q->cap = q->cap_hot;
       const size_t kb = (hkp == KK_I32 || hkp == KK_GEN32) ? 4 : 8;
       const size_t col = align_up((size_t)n * 8, 256), kcol = align_up((size_t)n * kb, 256);
       q->part_bytes = align_up(P * 4, 256) + align_up((P + 1) * 8, 256) + align_up((2 * P + 2) * 4, 256) + align_up((P1 + 1) * 8, 256) + align_up(P1 * 8, 256) +

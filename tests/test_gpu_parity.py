@@ -343,13 +343,13 @@ def test_two_level_partition(small_partition_tables):
     want = oracle_result(ds)
     d = to_dev(ds)
     res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.PARTITION)
-    assert eiger.last_partition_levels() == 2
+    assert res.info["partition_levels"] == 2
     assert_matches(res, want, d.aggs, d.vals)
     ds = datagen.config5(n=6_000_011, ndv=1 << 22, scattered=True)
     want = oracle_result(ds)
     d = to_dev(ds)
     res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.PARTITION)
-    assert eiger.last_partition_levels() == 2
+    assert res.info["partition_levels"] == 2
     assert_matches(res, want, d.aggs, d.vals)
 
 
@@ -363,14 +363,14 @@ def test_auto_slice_sketch(cfg, lg):
     ds = datagen.config5(n=SPEC_N + 12345, ndv=D, scattered=True) if cfg == "c5" else datagen.config4(n=SPEC_N + 777, D=D)
     res = _auto_matches(ds, eiger.PARTITION)
     assert res.n_groups == D
-    est = eiger.last_ndv_estimate()
+    est = res.info["ndv_est"]
     assert 0.93 * D <= est <= 1.20 * D, (est, D)
 
 
 def test_auto_slice_sketch_two_levels(small_partition_tables):
     ds = datagen.config5(n=SPEC_N, ndv=1 << 22, scattered=True)
     res = _auto_matches(ds, eiger.PARTITION)
-    assert eiger.last_partition_levels() == 2 and res.n_groups == 1 << 22
+    assert res.info["partition_levels"] == 2 and res.n_groups == 1 << 22
 
 
 def test_auto_slice_sketch_off_matches(monkeypatch):
@@ -378,7 +378,7 @@ def test_auto_slice_sketch_off_matches(monkeypatch):
     set_tunable(monkeypatch, "EIGER_SLICE", 0)
     D = 1 << 18
     res = _auto_matches(datagen.config5(n=SPEC_N + 12345, ndv=D, scattered=True), eiger.PARTITION)
-    assert res.n_groups == D and abs(eiger.last_ndv_estimate() - D) <= 4 * 0.008125 * D
+    assert res.n_groups == D and abs(res.info["ndv_est"] - D) <= 4 * 0.008125 * D
 
 
 # ---- direct-index shared-memory array: the 1024-thread CTA at its size limits ---------------
@@ -506,7 +506,7 @@ def test_multi_key_fused_sketch():
     d = to_dev(ds)
     res = eiger.groupby(d.keys, d.vals, d.aggs)
     assert_matches(res, oracle_result(ds), d.aggs, d.vals)
-    assert eiger.last_ndv_estimate() == pytest.approx(want, rel=1e-9)    # AUTO planned with it
+    assert res.info["ndv_est"] == pytest.approx(want, rel=1e-9)    # AUTO planned with it
     assert res.variant != eiger.DIRECT
     # small domains keep the range product: no sketch pass
     small = datagen.config_mk(n=100_001, nk=3, digit_bits=3)
