@@ -95,6 +95,8 @@ struct Tunables {
   double slice_min_keys;              // distinct keys wanted in the slice (relative error 1 / sqrt of it)
   double fused_sketch_min_range;      // multi-column keys: sketch the fused key when the ranges multiply to more than this
   int part_full_table;                // EIGER_PARTITION reserves the full-size global table when partitions may be cut (round-1 behaviour)
+  int split_max;                      // direct-index array split over up to this many CTAs (splitagg.cu); 0 = off
+  size_t split_bytes;                 // ... each holding at most this much of it in shared memory
   int pack_stride;                    // global hash table slots of 40 / 48 bytes are not padded to 64
   int dict;                           // EIGER_AUTO: scattered keys the sample names completely get a dictionary + direct array (FRONT_DICT)
   double dict_max_keys;               // ... while the sample holds at most this many distinct keys
@@ -132,6 +134,8 @@ struct Tunables {
     slice_min_keys = env("EIGER_SLICE_MIN_KEYS", 2048);
     dict = (int)env("EIGER_DICT", 1);
     pack_stride = (int)env("EIGER_PACK_STRIDE", 1);
+    split_max = (int)env("EIGER_SPLIT_MAX", 16);
+    split_bytes = (size_t)env("EIGER_SPLIT_KB", 192) << 10;
     part_full_table = (int)env("EIGER_PART_FULL_TABLE", 0);
     dict_max_keys = env("EIGER_DICT_MAX_KEYS", 4600);   // measured: scattered 2^12 keys 0.90 ms through the dictionary, 1.25 ms through the hash table
   }
@@ -170,6 +174,7 @@ struct QueryPlan {
   const uint32_t* pre_hist = nullptr;   // PARTITION: level-1 histogram taken with key.base at fan-out kPreFan
   int sort_bits = 0, sort_passes = 0;   // SORT: significant bits of the rebased fused key, 8-bit passes
   uint32_t dict_slots = 0, dict_shift = 0;   // FRONT_DICT: dictionary image entries (power of two)
+  int split_lg = 0;                          // FRONT_SPLIT: log2 of the CTAs that share the array
 };
 
 uint64_t range_of(const eiger_stats& s) {   // max - min + 1, 0 when it is 2^64
@@ -344,9 +349,21 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
       q->smem_bytes = (size_t)direct_bytes * q->front_replicas;
     } else {
       q->front = FRONT_NONE;
+      // between one CTA's shared memory and the L2-atomics regime: the array split over 2 .. 16 CTAs that
+      // walk the same tiles (splitagg.cu); the smallest group whose share fits
+      if (q->key_kind != KK_I8I8 && !skewed) {
+        for (int lg = 1; (1 << lg) <= T.split_max; ++lg) {
+          const uint64_t local = (R + (1ull << lg) - 1) >> lg;
+          if ((unsigned __int128)local * 8 * p.n_acc <= T.split_bytes) {
+            q->front = FRONT_SPLIT; q->split_lg = lg; q->front_slots = (uint32_t)local;
+            q->smem_bytes = split_direct_smem(p.n_acc, (uint32_t)local);
+            break;
+          }
+        }
+      }
     }
     q->sig = detect_sig(p, na);
-    if (!aggregate_supported(q->key_kind, q->sig, q->front, q->back)) return EIGER_ERR_INFEASIBLE;
+    if (q->front != FRONT_SPLIT && !aggregate_supported(q->key_kind, q->sig, q->front, q->back)) return EIGER_ERR_INFEASIBLE;
   } else if (variant == EIGER_SORT) {
     // sort-based group-by: LSD radix sort on the bits the key range needs, then
     // a segmented reduce.  No table: the workspace holds one or two copies of the rows.
@@ -633,6 +650,15 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       if (q.front == FRONT_DICT || (q.front == FRONT_SDIRECT && (tun().sdirect_wide || 3 * (per_cta + 1024) > (196u << 10)))) { L.threads = 1024; occ = 1; }
       const int64_t tiles = std::max<int64_t>(1, (n + 1023) / 1024);
       L.blocks = (int)std::min<int64_t>((int64_t)rt->sm_count * occ, tiles);
+      if (q.front == FRONT_SPLIT) {
+        SplitLaunch SL{};
+        SL.key = q.key; SL.plan = q.plan; SL.n = n; SL.key_kind = q.key_kind; SL.sig = q.sig; SL.lgC = q.split_lg; SL.spec = spec | checked;
+        SL.cap = q.cap; SL.local_slots = q.front_slots; SL.table = table; SL.call = rt->call;
+        const int C = 1 << q.split_lg;
+        const int64_t want = std::min<int64_t>(rt->sm_count / C, (n + 4095) / 4096);
+        SL.blocks = (int)std::max<int64_t>(1, want) * C;
+        { Timed t(s, 0); rc = launch_split_direct(SL, s); if (rc) return rc; }
+      } else
       { Timed t(s, 0); rc = launch_aggregate(L, s); if (rc) return rc; }
     } else {
       HashAggLaunch H{};

@@ -65,7 +65,7 @@ int launch_regs_to_bytes(Runtime* rt, uint8_t* out, cudaStream_t s);
 double hll_estimate_from_hist(const uint32_t* hist);
 
 // ---- aggregate.cu ----------------------------------------------------------------------
-enum FrontKind : int { FRONT_NONE = 0, FRONT_PRIV = 1, FRONT_SDIRECT = 2, FRONT_SHASH = 3, FRONT_DICT = 4 };
+enum FrontKind : int { FRONT_NONE = 0, FRONT_PRIV = 1, FRONT_SDIRECT = 2, FRONT_SHASH = 3, FRONT_DICT = 4, FRONT_SPLIT = 5 };
 enum BackKind : int { BACK_DIRECT = 0, BACK_HASH = 1 };
 
 struct AggLaunch {
@@ -168,6 +168,18 @@ struct PartitionLaunch {
 };
 int launch_partition(PartitionLaunch& p, int sm_count, size_t smem_optin, cudaStream_t s);
 int partition_max_bits_per_level();
+
+// ---- splitagg.cu ------------------------------------------------------------------------
+// Direct-index array split over 2^lgC co-operating CTAs (slot u belongs to CTA u mod 2^lgC of its group).
+struct SplitLaunch {
+  KeyDesc key; AggPlan plan; int64_t n;
+  int key_kind, sig, lgC, spec;
+  uint64_t cap; uint32_t local_slots;
+  void* table; CallDev* call;
+  int blocks;
+};
+int launch_split_direct(const SplitLaunch& L, cudaStream_t s);
+size_t split_direct_smem(int n_acc, uint32_t local_slots);
 
 // ---- dictenc.cu -------------------------------------------------------------------------
 int launch_dict_fill(const void* sorted_keys, int dtype, int64_t ndv, void* table, uint64_t cap, CallDev* call, int sm_count, cudaStream_t s);

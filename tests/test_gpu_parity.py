@@ -646,3 +646,41 @@ def test_dict_encode_capacity_error_and_group_by_on_codes():
     assert np.array_equal(d[res.keys[0].long()].cpu().numpy().astype(np.int64), want.keys[0])   # order-preserving: sorted codes = sorted keys
     for a, b in zip(res.aggs, want.aggs):
         assert np.array_equal(a.cpu().numpy(), b)
+
+
+# ---- direct-index array split over co-operating CTAs (splitagg.cu) -------------------------------------
+@pytest.mark.parametrize("R", [12_000, 1 << 16, (1 << 17) + 3, 180_000])
+def test_split_direct_array(R):
+    # ranges between one CTA's shared memory (10240 SUM + COUNT slots) and 16 CTAs' worth: every slot of
+    # the range is present; ragged row count; values that carry into the high word
+    n = (1 << 21) + 4099
+    i = torch.arange(n, dtype=torch.int64)
+    keys = ((i * 7919) % R - R // 3).to(torch.int32)
+    vals = (datagen.uniform_int(13, 1, i, 0, (1 << 31) - 2) - (1 << 30)) * 4099
+    ds = datagen.Dataset("split", n, [keys], [vals], [(eiger.SUM, 0), (eiger.COUNT, 0)], ndv=R)
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    for force in (eiger.DIRECT, eiger.AUTO):
+        res = eiger.groupby(d.keys, d.vals, d.aggs, force=force)
+        assert res.variant == eiger.DIRECT and res.n_groups == R
+        assert_matches(res, want, d.aggs, d.vals)
+    # four aggregates of fp64 and an int64 key column (generic signature, 64-bit rebased keys)
+    vf = datagen.unit_f64(13, 2, i)
+    ds = datagen.Dataset("split-f", n, [keys.to(torch.int64) * 1 + (1 << 40)], [vf], [(eiger.SUM, 0), (eiger.COUNT, 0), (eiger.MIN, 0), (eiger.MAX, 0)],
+                         ndv=R, exact_f64_sum=True)
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.DIRECT)
+    assert_matches(res, want, d.aggs, d.vals)
+
+
+def test_split_direct_speculation_and_stale_statistics():
+    ds = datagen.config5(n=SPEC_N, ndv=1 << 15)
+    _auto_matches(ds, eiger.DIRECT)
+    ds.keys[0][SPEC_N // 2 + 11] = 77_000_000                 # one row outside the sampled range: the pass is discarded
+    res = _auto_matches(ds)
+    assert res.n_groups == (1 << 15) + 1
+    d = to_dev(datagen.config5(n=1 << 20, ndv=1 << 15))
+    with pytest.raises(eiger.EigerError) as e:
+        eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.DIRECT, stats=[eiger.Stats(0, (1 << 14) - 1, 1 << 14, d.n)])
+    assert e.value.code == eiger.ERR_STATS
