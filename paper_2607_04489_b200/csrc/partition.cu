@@ -265,7 +265,22 @@ part_scatter_kernel(const __grid_constant__ ScatterArgs A) {
     }
     __syncthreads();
     const uint32_t m = hi - lo;                              // rows of this tile
-    for (uint32_t j = tid; j < m; j += T) out_keys[s_delta[s_pid[j]] + j] = ko[j];
+    // write-out, unrolled: the destination of staged position j = r * T + tid is the same for every
+    // column, so it is computed once (all partition-id loads, then all offset loads: independent
+    // shared-memory loads in flight together instead of one dependent chain per position)
+    long long dstp[RPT];
+    {
+      uint32_t pid[RPT];
+#pragma unroll
+      for (int r = 0; r < RPT; ++r) { const uint32_t j = (uint32_t)(r * T + tid); pid[r] = j < m ? s_pid[j] : 0u; }
+#pragma unroll
+      for (int r = 0; r < RPT; ++r) { const uint32_t j = (uint32_t)(r * T + tid); dstp[r] = j < m ? s_delta[pid[r]] + (long long)j : -1ll; }
+      UO kv[RPT];
+#pragma unroll
+      for (int r = 0; r < RPT; ++r) { const uint32_t j = (uint32_t)(r * T + tid); if (j < m) kv[r] = ko[j]; }
+#pragma unroll
+      for (int r = 0; r < RPT; ++r) if (dstp[r] >= 0) out_keys[dstp[r]] = kv[r];
+    }
     for (int c = 0; c < a.n_vals; ++c) {
       __syncthreads();                                       // s_out is read by the previous column's write-out
       const unsigned char* col = st + sm.voff[c];
@@ -276,7 +291,11 @@ part_scatter_kernel(const __grid_constant__ ScatterArgs A) {
         if (c == a.n_vals - 1 && ring_stage >= 0) { __syncwarp(); if (lane == 0) mbar_arrive(&s_empty[ring_stage]); }
         __syncthreads();
         uint64_t* dst = static_cast<uint64_t*>(a.out_vals[c]);
-        for (uint32_t j = tid; j < m; j += T) dst[s_delta[s_pid[j]] + j] = vo[j];
+        uint64_t vv[RPT];
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) { const uint32_t j = (uint32_t)(r * T + tid); if (j < m) vv[r] = vo[j]; }
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) if (dstp[r] >= 0) dst[dstp[r]] = vv[r];
       } else {
         uint32_t* vo = reinterpret_cast<uint32_t*>(s_out);
 #pragma unroll
@@ -284,7 +303,11 @@ part_scatter_kernel(const __grid_constant__ ScatterArgs A) {
         if (c == a.n_vals - 1 && ring_stage >= 0) { __syncwarp(); if (lane == 0) mbar_arrive(&s_empty[ring_stage]); }
         __syncthreads();
         uint32_t* dst = static_cast<uint32_t*>(a.out_vals[c]);
-        for (uint32_t j = tid; j < m; j += T) dst[s_delta[s_pid[j]] + j] = vo[j];
+        uint32_t vv[RPT];
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) { const uint32_t j = (uint32_t)(r * T + tid); if (j < m) vv[r] = vo[j]; }
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) if (dstp[r] >= 0) dst[dstp[r]] = vv[r];
       }
     }
     if (a.n_vals == 0 && ring_stage >= 0) { __syncwarp(); if (lane == 0) mbar_arrive(&s_empty[ring_stage]); }
