@@ -318,11 +318,23 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   }();
   auto hash_cap = [&](double g) { return (uint64_t)std::max(1024.0, std::ceil(g * (1.0 + 4 * kSigma) * 1.02 / T.load)); };
 
+  // EIGER_SMEM split over 2^lg CTAs: the smallest group whose tables hold the keys at the target load; 0 = one CTA
+  // holds them all (or no group is large enough: the plain variant then overflows into the global table)
+  const uint32_t split_slots = (uint32_t)std::max<size_t>(64, (((size_t)200 << 10) - split_hash_queue_bytes(hk) - 64) / slot_bytes) & ~7u;
+  auto split_lg_for = [&](double g) -> int {
+    const double fill = hk == KK_I32 ? T.smem_fill : 0.6 * T.smem_fill;
+    if (g * (1.0 + 4 * kSigma) <= fill * smem_slots) return 0;
+    for (int lg = 1; (1 << lg) <= T.split_max; ++lg)
+      if (g * (1.0 + 4 * kSigma) <= 0.9 * fill * (double)split_slots * (double)(1 << lg)) return lg;
+    return 0;
+  };
   int variant = force;
   if (variant == EIGER_AUTO) {
     if (direct_ok && (direct_bytes * 256 <= T.priv_smem || direct_bytes <= T.sdirect_bytes ||
                       (!skewed && direct_bytes <= T.direct_l2_bytes && (double)R <= 16.0 * (double)std::max<int64_t>(n, 1)))) variant = EIGER_DIRECT;   // hot keys serialise global atomics
     else if (ndv * (1.0 + 4 * kSigma) <= (hk == KK_I32 ? T.smem_fill : 0.6 * T.smem_fill) * smem_slots) variant = EIGER_SMEM;   // 2-key buckets fill up sooner
+    // ... or the tables of up to 16 co-operating CTAs, each owning a hash slice of the keys (splitagg.cu)
+    else if (!skewed && split_lg_for(ndv) > 0) variant = EIGER_SMEM;
     // uniform keys: partition + shared-memory aggregation beats L2 atomics at every size measured
     // (C5 sweep); a few hot keys in front of a long tail (sample collision rate) is where the global
     // table with its hot-key front wins (C3), while its table still fits L2
@@ -417,6 +429,9 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
       q->slots = front ? smem_slots : 64;
       q->limit = front ? (uint32_t)((variant == EIGER_SMEM ? 0.75 : 0.5) * smem_slots) : 0;
       q->cap = std::min(hash_cap(ndv), q->cap_bound);
+      if (variant == EIGER_SMEM && !skewed && (q->split_lg = split_lg_for(ndv)) > 0) {
+        q->slots = split_slots; q->limit = (uint32_t)(0.75 * split_slots); q->threads = 1024;
+      }
     }
     q->smem_bytes = align_up((size_t)q->slots * (variant == EIGER_PARTITION ? part_slot_bytes : slot_bytes) + 64, 16);
     q->stages = T.stages; q->hot_reserved = variant != EIGER_PARTITION && want_hot;
@@ -714,6 +729,12 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         const int64_t tiles = std::max<int64_t>(1, n / (4 * (int64_t)q.threads));
         H.blocks = (int)std::min<int64_t>(rt->sm_count, tiles);
       }
+      if (q.variant == EIGER_SMEM && q.split_lg > 0) {
+        const int C = 1 << q.split_lg;
+        H.blocks = (int)std::max<int64_t>(1, std::min<int64_t>(rt->sm_count / C, (n + 4095) / 4096)) * C;
+        H.bucket_keys = 0;
+        { Timed t(s, 0); rc = launch_split_hash(H, q.split_lg, s); if (rc) return rc; }
+      } else
       { Timed t(s, 0); rc = launch_hash_agg(H, s); if (rc) return rc; }
     }
 
@@ -814,11 +835,26 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         if (rc != EIGER_OK || !aborted) { if (chosen) *chosen = EIGER_SMEM; return rc; }
       }
     }
+    // The sample's NDV is a lower bound; when the sample is far from having seen every key twice, plan the
+    // speculative pass for what that many distinct keys among s samples mean for UNIFORM keys
+    // (ds / s = (1 - exp(-x)) / x, x = s / D); a wrong guess only costs the discarded pass
+    eiger_stats plan_stats[kMaxKeyCols];
+    for (int k = 0; k < nk; ++k) plan_stats[k] = local[k];
+    if (nk == 1 && !skewed) {
+      const double smp = (double)std::min<int64_t>(n, T.spec_samples), ds = std::max(1.0, local[0].ndv_est);
+      const double r = std::min(ds / smp, 0.98);
+      if (r > 0.05) {
+        double lo = 0.02, hi = 50.0;
+        for (int it = 0; it < 60; ++it) { const double x = 0.5 * (lo + hi); if ((1.0 - std::exp(-x)) / x > r) lo = x; else hi = x; }
+        const double range = (double)((uint64_t)local[0].max - (uint64_t)local[0].min) + 1.0;
+        plan_stats[0].ndv_est = std::min(std::max(ds, smp / (0.5 * (lo + hi))), std::min((double)n, range));
+      }
+    }
     QueryPlan qs;
     if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] sample: min %lld max %lld ndv %.1f collision %.5f\n", (long long)local[0].min, (long long)local[0].max, local[0].ndv_est, collision);
-    if (T.spec && fusable && plan_query(rt, keys, nk, n, vals, nv, aggs, na, local, EIGER_AUTO, &qs, skewed) == EIGER_OK &&
+    if (T.spec && fusable && plan_query(rt, keys, nk, n, vals, nv, aggs, na, plan_stats, EIGER_AUTO, &qs, skewed) == EIGER_OK &&
         ((qs.variant == EIGER_DIRECT && (qs.front != FRONT_NONE || qs.R <= (1ull << 24))) ||
-         (qs.variant == EIGER_SMEM && qs.ndv * 1.25 <= 0.6 * qs.slots)) && have_room(qs.total_bytes)) {
+         (qs.variant == EIGER_SMEM && qs.ndv * 1.25 <= 0.6 * qs.slots * (double)(1 << qs.split_lg))) && have_room(qs.total_bytes)) {
       bool aborted = false;
       if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] plan: variant %d kk %d sig %d slots %u limit %u cap %llu stride %u smem %zu front %d R %llu\n", qs.variant, qs.key_kind, qs.sig, qs.slots, qs.limit, (unsigned long long)qs.cap, qs.stride, qs.smem_bytes, qs.front, (unsigned long long)qs.R);
       rc = execute(qs, local, 1, &aborted);

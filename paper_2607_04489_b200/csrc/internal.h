@@ -180,6 +180,9 @@ struct SplitLaunch {
 };
 int launch_split_direct(const SplitLaunch& L, cudaStream_t s);
 size_t split_direct_smem(int n_acc, uint32_t local_slots);
+// The same split with per-CTA hash tables (scattered keys): key owner = hash bits; L.table_smem_bytes = the table
+int launch_split_hash(const HashAggLaunch& L, int lgC, cudaStream_t s);
+size_t split_hash_queue_bytes(int key_kind);
 
 // ---- dictenc.cu -------------------------------------------------------------------------
 int launch_dict_fill(const void* sorted_keys, int dtype, int64_t ndv, void* table, uint64_t cap, CallDev* call, int sm_count, cudaStream_t s);

@@ -18,14 +18,40 @@
 // region between the small-table and the partitioned regime).
 #include <algorithm>
 
-#include "internal.h"
-#include "rows.cuh"
+#include "hashagg.cuh"
 
 namespace eiger {
 namespace {
 
 constexpr int kSplitThreads = 1024;
 constexpr int kQueue = 64;                       // queue entries per warp (flushed 32 at a time)
+
+
+// Keys of one tile, kVec vector loads per thread, all issued before the first use: a CTA scans C times
+// its share of the input, so the scan must keep many bytes in flight (the first version, two 8-byte
+// loads per thread and no prefetch, scanned at 16 GB/s per SM: 0.65 ms per 2^28 keys and group size).
+// Element e of vector v of thread t is row v * (E * 1024) + E * t + e of the tile.
+template <int KK> struct TileKeys {
+  using U = typename KeyTraits<KK>::U;
+  static constexpr int E = (KK == KK_I32) ? 4 : 2;             // keys per vector load
+  static constexpr int kVec = 4;
+  static constexpr int KR = E * kVec;                          // keys per thread and tile
+  static constexpr int64_t kTileRows = (int64_t)KR * kSplitThreads;
+  __device__ static __forceinline__ uint32_t row_of(int r, int tid) { return (uint32_t)((r / E) * (E * kSplitThreads) + E * tid + (r % E)); }
+  __device__ static __forceinline__ void load(const KeyDesc& key, int64_t base, int tid, U (&u)[KR]) {
+#pragma unroll
+    for (int v = 0; v < kVec; ++v) {
+      const int64_t i = base + (int64_t)v * (E * kSplitThreads) + E * tid;
+      if constexpr (KK == KK_I32) {
+        const uint4 x = ldg_stream_16(static_cast<const int32_t*>(key.ptr[0]) + i);
+        const uint32_t b = (uint32_t)key.base[0];
+        u[4 * v] = x.x - b; u[4 * v + 1] = x.y - b; u[4 * v + 2] = x.z - b; u[4 * v + 3] = x.w - b;
+      } else {
+        load_u2<KK>(key, i, *reinterpret_cast<U(*)[2]>(&u[2 * v]));
+      }
+    }
+  }
+};
 
 struct SplitArgs {
   KeyDesc key;
@@ -68,58 +94,68 @@ split_direct_kernel(const __grid_constant__ SplitArgs a) {
     }
   };
 
-  // tiles of 4 x 1024 rows; group g = blockIdx.x >> lgC of gridDim.x >> lgC groups walks tiles g, g + groups, ..
-  constexpr int kRows = 4;
-  const int64_t tile = (int64_t)kRows * kSplitThreads;
+  // group g = blockIdx.x >> lgC of gridDim.x >> lgC groups walks tiles g, g + groups, ..; the next tile's
+  // keys are requested before the current tile is processed
+  using TK = TileKeys<KK>;
+  constexpr int KR = TK::KR;
+  const int64_t tile = TK::kTileRows;
   const int64_t groups = gridDim.x >> a.lgC;
-  const int64_t n_tiles = (a.n + tile - 1) / tile;
+  const int64_t n_full = a.n / tile;
   int cnt = 0;                                   // entries waiting in this warp's queue (warp-uniform)
   bool bad = false;
-  for (int64_t t = blockIdx.x >> a.lgC; t < n_tiles; t += groups) {
-    const int64_t base = t * tile;
-    U u[kRows];
-    bool ok[kRows];
-    if (base + tile <= a.n) {
-      // rows base + 2 * tid, + 1 and base + 2048 + 2 * tid, + 1: two 8- or 16-byte key loads per thread
-      load_u2<KK>(a.key, base + 2 * tid, *reinterpret_cast<U(*)[2]>(&u[0]));
-      load_u2<KK>(a.key, base + 2 * kSplitThreads + 2 * tid, *reinterpret_cast<U(*)[2]>(&u[2]));
-#pragma unroll
-      for (int r = 0; r < kRows; ++r) ok[r] = true;
-    } else {
-#pragma unroll
-      for (int r = 0; r < kRows; ++r) {
-        const int64_t i = base + (r >> 1) * 2 * kSplitThreads + 2 * tid + (r & 1);
-        ok[r] = i < a.n;
-        u[r] = ok[r] ? load_u<KK>(a.key, i) : (U)0;
+  auto scan_row = [&](U ur, bool okr, uint32_t off, int64_t base) {
+    const uint64_t uu = (uint64_t)ur;
+    if (okr && uu >= a.cap) { bad = true; okr = false; }                  // outside the planned range (speculative / caller's statistics)
+    const bool mine = okr && ((uint32_t)uu & (C - 1)) == me;
+    const uint32_t m = __ballot_sync(0xffffffffu, mine);
+    if (m) {
+      if (mine) {
+        const int p = cnt + __popc(m & ((1u << lane) - 1u));
+        q_slot[p] = (uint32_t)(uu >> a.lgC);
+        q_row[p] = off;
+      }
+      cnt += __popc(m);
+      if (cnt >= 32) {
+        __syncwarp();
+        cnt -= 32;
+        consume(q_slot[cnt + lane], base + q_row[cnt + lane]);
+        __syncwarp();
       }
     }
-#pragma unroll
-    for (int r = 0; r < kRows; ++r) {
-      const uint64_t uu = (uint64_t)u[r];
-      if (ok[r] && uu >= a.cap) { bad = true; ok[r] = false; }            // outside the planned range (speculative / caller's statistics)
-      const bool mine = ok[r] && ((uint32_t)uu & (C - 1)) == me;
-      const uint32_t m = __ballot_sync(0xffffffffu, mine);
-      if (m) {
-        if (mine) {
-          const int p = cnt + __popc(m & ((1u << lane) - 1u));
-          q_slot[p] = (uint32_t)(uu >> a.lgC);
-          q_row[p] = (uint32_t)((r >> 1) * 2 * kSplitThreads + 2 * tid + (r & 1));
-        }
-        cnt += __popc(m);
-        if (cnt >= 32) {
-          __syncwarp();
-          cnt -= 32;
-          consume(q_slot[cnt + lane], base + q_row[cnt + lane]);
-          __syncwarp();
-        }
-      }
-    }
-    // the queue is drained at the end of every tile (row offsets are relative to the tile)
+  };
+  auto drain = [&](int64_t base) {               // the queue is drained at the end of every tile (row offsets are relative to it)
     __syncwarp();
     if (lane < cnt) consume(q_slot[lane], base + q_row[lane]);
     cnt = 0;
     __syncwarp();
-    if (a.spec && __any_sync(0xffffffffu, bad)) break;
+  };
+  {
+    U cur[KR], nxt[KR];
+    int64_t t = blockIdx.x >> a.lgC;
+    if (t < n_full) TK::load(a.key, t * tile, tid, cur);
+    for (; t < n_full; t += groups) {
+      const bool more = t + groups < n_full;
+      if (more) TK::load(a.key, (t + groups) * tile, tid, nxt);
+      const int64_t base = t * tile;
+#pragma unroll
+      for (int r = 0; r < KR; ++r) scan_row(cur[r], true, TK::row_of(r, tid), base);
+      drain(base);
+      if (a.spec && __any_sync(0xffffffffu, bad)) break;
+      if (more) {
+#pragma unroll
+        for (int r = 0; r < KR; ++r) cur[r] = nxt[r];
+      }
+    }
+  }
+  // the ragged last tile, by the group that would have taken it: row at a time
+  if (n_full * tile < a.n && (n_full % groups) == (blockIdx.x >> a.lgC)) {
+    const int64_t base = n_full * tile;
+    for (int64_t o = tid - lane; base + o < a.n; o += kSplitThreads) {          // warp-uniform trip count
+      const int64_t i = base + o + lane;
+      const bool okr = i < a.n;
+      scan_row(okr ? load_u<KK>(a.key, i) : (U)0, okr, (uint32_t)(o + lane), base);
+    }
+    drain(base);
   }
   if (bad) atomicOr(&a.call->abort, 1u);
   __syncthreads();
@@ -158,6 +194,134 @@ int launch_sig(const SplitLaunch& L, cudaStream_t s) {
   }
 }
 
+// ---- the same split for keys that are not dense: per-CTA hash tables ----------------------------
+// Owner of key u = top lgC bits of a multiplicative hash of u (independent of the table's bucket
+// hash); every CTA of a group scans all keys of the group's tiles, queues the rows it owns and runs
+// them through its own shared-memory hash table (hashagg.cuh: Front) with full warps.  At the end the
+// tables are merged into the global table like EIGER_SMEM's; a key lives in one CTA per group.
+template <class U> __device__ __forceinline__ uint32_t split_owner(U u, int lgC) {
+  return (uint32_t)(((uint32_t)u ^ (uint32_t)((uint64_t)u >> 32)) * 0x85EBCA77u) >> (32 - lgC);
+}
+
+template <int KK, int SIG>
+__global__ void __launch_bounds__(kSplitThreads, 1)
+split_hash_kernel(const __grid_constant__ HashAggArgs a, int lgC) {
+  using F = Front<KK, SIG, 16 / (int)sizeof(typename KeyTraits<KK>::U)>;
+  using U = typename F::U;
+  constexpr int NV = F::NV;
+  extern __shared__ __align__(16) unsigned char smem[];     // [table][queues: keys, row offsets]
+  __shared__ uint32_t s_count, s_abort;
+  const int n_vals = Sig<SIG>::kStatic ? NV : a.plan.n_vals;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t me = blockIdx.x & ((1u << lgC) - 1u);
+  F f(a, smem, a.slots);
+  U* q_key = reinterpret_cast<U*>(smem + a.table_off) + warp * kQueue;
+  uint32_t* q_row = reinterpret_cast<uint32_t*>(smem + a.table_off + (size_t)(kSplitThreads / 32) * kQueue * sizeof(U)) + warp * kQueue;
+  if (tid == 0) { s_count = 0; s_abort = 0; }
+  f.init(tid, kSplitThreads);
+  __syncthreads();
+  bool missed = false;
+  auto consume = [&](U u, int64_t row, bool valid) {       // all 32 lanes of the warp are here
+    uint64_t raw[NV];
+#pragma unroll
+    for (int c = 0; c < NV; ++c) raw[c] = (valid && (Sig<SIG>::kStatic || c < n_vals)) ? global_val(a.plan, c, sig_vw<SIG>(a.plan, c), row) : 0ull;
+    const uint32_t miss = f.pair(u, raw, valid, u, raw, false, &s_count);
+    if (__any_sync(0xffffffffu, miss != 0)) { if (a.spec) missed = missed || miss != 0; else if (miss) f.back_row(u, raw); }
+    __syncwarp();
+  };
+  using TK = TileKeys<KK>;
+  constexpr int KR = TK::KR;
+  const int64_t tile = TK::kTileRows;
+  const int64_t groups = gridDim.x >> lgC;
+  const int64_t n_full = a.n / tile;
+  int cnt = 0;
+  uint32_t trip = 0;
+  auto scan_row = [&](U ur, bool okr, uint32_t off, int64_t base) {
+    const bool mine = okr && split_owner<U>(ur, lgC) == me;
+    const uint32_t m = __ballot_sync(0xffffffffu, mine);
+    if (m) {
+      if (mine) {
+        const int p = cnt + __popc(m & ((1u << lane) - 1u));
+        q_key[p] = ur;
+        q_row[p] = off;
+      }
+      cnt += __popc(m);
+      if (cnt >= 32) {
+        __syncwarp();
+        cnt -= 32;
+        consume(q_key[cnt + lane], base + q_row[cnt + lane], true);
+        __syncwarp();
+      }
+    }
+  };
+  auto drain = [&](int64_t base) {
+    __syncwarp();
+    if (cnt > 0) consume(lane < cnt ? q_key[lane] : (U)0, base + (lane < cnt ? q_row[lane] : 0u), lane < cnt);
+    cnt = 0;
+    __syncwarp();
+  };
+  {
+    U cur[KR], nxt[KR];
+    int64_t t = blockIdx.x >> lgC;
+    if (t < n_full) TK::load(a.key, t * tile, tid, cur);
+    for (; t < n_full; t += groups) {
+      if (a.spec) { if (__any_sync(0xffffffffu, missed || ((trip++ & 15u) == 0u && *reinterpret_cast<volatile uint32_t*>(&a.call->abort)))) break; }
+      const bool more = t + groups < n_full;
+      if (more) TK::load(a.key, (t + groups) * tile, tid, nxt);
+      const int64_t base = t * tile;
+#pragma unroll
+      for (int r = 0; r < KR; ++r) scan_row(cur[r], true, TK::row_of(r, tid), base);
+      drain(base);
+      if (more) {
+#pragma unroll
+        for (int r = 0; r < KR; ++r) cur[r] = nxt[r];
+      }
+    }
+  }
+  if (n_full * tile < a.n && (n_full % groups) == (blockIdx.x >> lgC) && !(a.spec && __any_sync(0xffffffffu, missed))) {
+    const int64_t base = n_full * tile;
+    for (int64_t o = tid - lane; base + o < a.n; o += kSplitThreads) {
+      const int64_t i = base + o + lane;
+      const bool okr = i < a.n;
+      scan_row(okr ? load_u<KK>(a.key, i) : (U)0, okr, (uint32_t)(o + lane), base);
+    }
+    drain(base);
+  }
+  if (a.spec) {
+    if (missed) { atomicOr(&a.call->abort, 1u); atomicOr(&s_abort, 1u); }
+    __syncthreads();
+    if (s_abort || *reinterpret_cast<volatile uint32_t*>(&a.call->abort)) return;
+  } else {
+    __syncthreads();
+  }
+  f.flush_merge(tid, kSplitThreads);
+}
+
+template <int KK, int SIG>
+int launch_hash_one(const HashAggLaunch& L, int lgC, cudaStream_t s) {
+  using U = typename KeyTraits<KK>::U;
+  HashAggArgs a{};
+  a.key = L.key; a.plan = L.plan; a.n = L.n;
+  a.slots = L.slots; a.limit = L.limit; a.spec = L.spec; a.max_probes = 16; a.n_hot = 0;
+  a.table = L.table; a.cap = L.cap; a.stride = L.stride; a.call = L.call;
+  a.table_off = (uint32_t)((L.table_smem_bytes + 127) & ~(size_t)127);       // the queues follow the table
+  const size_t smem = (size_t)a.table_off + (size_t)(kSplitThreads / 32) * kQueue * (sizeof(U) + 4);
+  auto kern = split_hash_kernel<KK, SIG>;
+  EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  kern<<<L.blocks, kSplitThreads, smem, s>>>(a, lgC);
+  count_launch();
+  EIGER_CUDA(cudaGetLastError());
+  return EIGER_OK;
+}
+template <int KK>
+int launch_hash_sig(const HashAggLaunch& L, int lgC, cudaStream_t s) {
+  switch (L.sig) {
+    case SIG_SC: return launch_hash_one<KK, SIG_SC>(L, lgC, s);
+    case SIG_SC32: return launch_hash_one<KK, SIG_SC32>(L, lgC, s);
+    default: return launch_hash_one<KK, SIG_GENERIC>(L, lgC, s);
+  }
+}
+
 }  // namespace
 
 size_t split_direct_smem(int n_acc, uint32_t local_slots) { return (size_t)n_acc * 8 * local_slots + (size_t)(kSplitThreads / 32) * 2 * kQueue * 4; }
@@ -168,6 +332,18 @@ int launch_split_direct(const SplitLaunch& L, cudaStream_t s) {
     case KK_I64: return launch_sig<KK_I64>(L, s);
     case KK_GEN32: return launch_sig<KK_GEN32>(L, s);
     case KK_GEN: return launch_sig<KK_GEN>(L, s);
+    default: return EIGER_ERR_ARG;
+  }
+}
+
+// queue bytes that follow the per-CTA table of the split hash kernel
+size_t split_hash_queue_bytes(int key_kind) { return (size_t)(kSplitThreads / 32) * kQueue * ((key_kind == KK_I32 ? 4 : 8) + 4) + 128; }
+
+int launch_split_hash(const HashAggLaunch& L, int lgC, cudaStream_t s) {
+  switch (L.key_kind) {
+    case KK_I32: return launch_hash_sig<KK_I32>(L, lgC, s);
+    case KK_I64: return launch_hash_sig<KK_I64>(L, lgC, s);
+    case KK_GEN: return launch_hash_sig<KK_GEN>(L, lgC, s);
     default: return EIGER_ERR_ARG;
   }
 }

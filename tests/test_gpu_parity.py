@@ -684,3 +684,26 @@ def test_split_direct_speculation_and_stale_statistics():
     with pytest.raises(eiger.EigerError) as e:
         eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.DIRECT, stats=[eiger.Stats(0, (1 << 14) - 1, 1 << 14, d.n)])
     assert e.value.code == eiger.ERR_STATS
+
+
+@pytest.mark.parametrize("lg", [13, 15, 16])
+@pytest.mark.parametrize("kdtype", [torch.int32, torch.int64])
+def test_split_hash_tables(lg, kdtype):
+    # scattered keys, more of them than one CTA's shared-memory table holds: EIGER_SMEM splits them over
+    # 2 .. 16 co-operating CTAs (hash slices of the key space); AUTO speculates on it from the sample
+    n = SPEC_N + 777
+    ds = datagen.config5(n=n, ndv=1 << lg, scattered=True)
+    ds = datagen.Dataset(ds.name, n, [ds.keys[0].to(kdtype)], ds.vals, ds.aggs, ds.ndv)
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    st = eiger.profile_keys(d.keys)
+    res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.SMEM, stats=st)
+    assert_matches(res, want, d.aggs, d.vals)
+    res = eiger.groupby(d.keys, d.vals, d.aggs)
+    assert_matches(res, want, d.aggs, d.vals)
+    # generic signature (no static plan), forced
+    vf = datagen.unit_f64(17, 2, torch.arange(n, dtype=torch.int64))
+    ds2 = datagen.Dataset("split-hash-gen", n, ds.keys, [ds.vals[0], vf], [(eiger.MAX, 0), (eiger.SUM, 1), (eiger.MIN, 1), (eiger.COUNT, 0)], ds.ndv, exact_f64_sum=True)
+    d2 = to_dev(ds2)
+    res = eiger.groupby(d2.keys, d2.vals, d2.aggs, force=eiger.SMEM, stats=st)
+    assert_matches(res, oracle_result(ds2), d2.aggs, d2.vals)
