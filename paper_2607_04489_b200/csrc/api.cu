@@ -96,6 +96,7 @@ struct Tunables {
   double fused_sketch_min_range;      // multi-column keys: sketch the fused key when the ranges multiply to more than this
   int part_full_table;                // EIGER_PARTITION reserves the full-size global table when partitions may be cut (round-1 behaviour)
   int split_max;                      // direct-index array split over up to this many CTAs (splitagg.cu); 0 = off
+  int split_hash;                     // EIGER_SMEM may split its hash tables over up to 16 CTAs (experiment, off)
   size_t split_bytes;                 // ... each holding at most this much of it in shared memory
   int pack_stride;                    // global hash table slots of 40 / 48 bytes are not padded to 64
   int dict;                           // EIGER_AUTO: scattered keys the sample names completely get a dictionary + direct array (FRONT_DICT)
@@ -121,7 +122,7 @@ struct Tunables {
     global_front = (int)env("EIGER_GLOBAL_FRONT", 1);
     global_front_probes = (int)env("EIGER_GLOBAL_FRONT_PROBES", 1);
     load = env("EIGER_LOAD", 0.5);
-    smem_fill = env("EIGER_SMEM_FILL", 0.6);
+    smem_fill = env("EIGER_SMEM_FILL", 0.67);          // scattered 2^13 keys (load 0.66): 2.7 ms in one CTA's table, 3.6 ms partitioned
     spec = (int)env("EIGER_SPEC", 1);
     global_always = (int)env("EIGER_GLOBAL_ALWAYS", 0);
     skew_collision = env("EIGER_SKEW_COLLISION", 1e-3);
@@ -134,7 +135,8 @@ struct Tunables {
     slice_min_keys = env("EIGER_SLICE_MIN_KEYS", 2048);
     dict = (int)env("EIGER_DICT", 1);
     pack_stride = (int)env("EIGER_PACK_STRIDE", 1);
-    split_max = (int)env("EIGER_SPLIT_MAX", 16);
+    split_max = (int)env("EIGER_SPLIT_MAX", 4);        // measured (C5 dense, ms): C = 2 / 4 / 8 / 16 -> 1.26 / 1.86 / 3.11 / 5.15 against 2.8-3.3 for global RED
+    split_hash = (int)env("EIGER_SPLIT_HASH", 0);      // the hash flavour loses everywhere (scattered 2^13 / 2^14: 3.1 / 6.4 ms against 2.7 / 3.4)
     split_bytes = (size_t)env("EIGER_SPLIT_KB", 192) << 10;
     part_full_table = (int)env("EIGER_PART_FULL_TABLE", 0);
     dict_max_keys = env("EIGER_DICT_MAX_KEYS", 4600);   // measured: scattered 2^12 keys 0.90 ms through the dictionary, 1.25 ms through the hash table
@@ -323,8 +325,8 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
   const uint32_t split_slots = (uint32_t)std::max<size_t>(64, (((size_t)200 << 10) - split_hash_queue_bytes(hk) - 64) / slot_bytes) & ~7u;
   auto split_lg_for = [&](double g) -> int {
     const double fill = hk == KK_I32 ? T.smem_fill : 0.6 * T.smem_fill;
-    if (g * (1.0 + 4 * kSigma) <= fill * smem_slots) return 0;
-    for (int lg = 1; (1 << lg) <= T.split_max; ++lg)
+    if (g * (1.0 + 4 * kSigma) <= fill * smem_slots || !T.split_hash) return 0;
+    for (int lg = 1; (1 << lg) <= 16; ++lg)
       if (g * (1.0 + 4 * kSigma) <= 0.9 * fill * (double)split_slots * (double)(1 << lg)) return lg;
     return 0;
   };

@@ -650,7 +650,8 @@ def test_dict_encode_capacity_error_and_group_by_on_codes():
 
 # ---- direct-index array split over co-operating CTAs (splitagg.cu) -------------------------------------
 @pytest.mark.parametrize("R", [12_000, 1 << 16, (1 << 17) + 3, 180_000])
-def test_split_direct_array(R):
+def test_split_direct_array(monkeypatch, R):
+    set_tunable(monkeypatch, "EIGER_SPLIT_MAX", 16)          # groups of up to 16 CTAs (AUTO stops at 4: measured crossover)
     # ranges between one CTA's shared memory (10240 SUM + COUNT slots) and 16 CTAs' worth: every slot of
     # the range is present; ragged row count; values that carry into the high word
     n = (1 << 21) + 4099
@@ -688,7 +689,8 @@ def test_split_direct_speculation_and_stale_statistics():
 
 @pytest.mark.parametrize("lg", [13, 15, 16])
 @pytest.mark.parametrize("kdtype", [torch.int32, torch.int64])
-def test_split_hash_tables(lg, kdtype):
+def test_split_hash_tables(monkeypatch, lg, kdtype):
+    set_tunable(monkeypatch, "EIGER_SPLIT_HASH", 1)         # an experiment that lost: off by default, kept correct
     # scattered keys, more of them than one CTA's shared-memory table holds: EIGER_SMEM splits them over
     # 2 .. 16 co-operating CTAs (hash slices of the key space); AUTO speculates on it from the sample
     n = SPEC_N + 777
