@@ -96,6 +96,7 @@ struct Tunables {
   double fused_sketch_min_range;      // multi-column keys: sketch the fused key when the ranges multiply to more than this
   int part_full_table;                // EIGER_PARTITION reserves the full-size global table when partitions may be cut (round-1 behaviour)
   int split_max;                      // direct-index array split over up to this many CTAs (splitagg.cu); 0 = off
+  int miss_queue;                     // EIGER_GLOBAL queues the front's misses per warp (hashagg.cuh)
   int split_hash;                     // EIGER_SMEM may split its hash tables over up to 16 CTAs (experiment, off)
   size_t split_bytes;                 // ... each holding at most this much of it in shared memory
   int pack_stride;                    // global hash table slots of 40 / 48 bytes are not padded to 64
@@ -136,6 +137,7 @@ struct Tunables {
     dict = (int)env("EIGER_DICT", 1);
     pack_stride = (int)env("EIGER_PACK_STRIDE", 1);
     split_max = (int)env("EIGER_SPLIT_MAX", 4);        // measured (C5 dense, ms): C = 2 / 4 / 8 / 16 -> 1.26 / 1.86 / 3.11 / 5.15 against 2.8-3.3 for global RED
+    miss_queue = (int)env("EIGER_MISS_QUEUE", 1);
     split_hash = (int)env("EIGER_SPLIT_HASH", 0);      // the hash flavour loses everywhere (scattered 2^13 / 2^14: 3.1 / 6.4 ms against 2.7 / 3.4)
     split_bytes = (size_t)env("EIGER_SPLIT_KB", 192) << 10;
     part_full_table = (int)env("EIGER_PART_FULL_TABLE", 0);
@@ -168,6 +170,7 @@ struct QueryPlan {
   size_t smem_bytes = 0;        // direct variants: the CTA's array; hash variants: the CTA's table
   size_t smem_dyn = 0;          // hash variants: ring + table
   int stages = 0;
+  size_t queue_bytes = 0;
   bool ring = false;
   bool hot_reserved = false;
   uint64_t cap = 0, cap_bound = 0, cap_hot = 0;
@@ -182,6 +185,10 @@ struct QueryPlan {
 uint64_t range_of(const eiger_stats& s) {   // max - min + 1, 0 when it is 2^64
   return (uint64_t)s.max - (uint64_t)s.min + 1ull;
 }
+
+int detect_sig(const AggPlan& p, int n_user);
+// the per-warp miss queue exists in the kernels with a compile-time plan of at most two value columns
+inline bool Sig_static_or_small(const AggPlan& p, int na) { const int sg = detect_sig(p, na); return sg == SIG_SC || sg == SIG_A4I || sg == SIG_A4F || sg == SIG_SC32; }
 
 int detect_sig(const AggPlan& p, int n_user) {
   auto is = [&](int j, int op, int col, int f) { return p.op[j] == op && (op == EIGER_COUNT || (p.col[j] == col && p.f64[j] == f)); };
@@ -305,7 +312,10 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
     return T.smem_total > lay.table_off + 4096 ? T.smem_total - lay.table_off : (size_t)4096;
   };
   const bool want_hot = force == EIGER_GLOBAL || (force == EIGER_AUTO && skewed);
-  const size_t smem_tab = table_bytes_for(hk, T.smem_threads, want_hot, T.smem_table_bytes);
+  // EIGER_GLOBAL: the rows the front cannot hold are queued per warp (64 entries of key + values) and sent to
+  // the global table 32 at a time; the queues take their room from the front table
+  const size_t miss_queue = (want_hot && T.miss_queue && !(T.ring & 1) && Sig_static_or_small(p, na)) ? (size_t)(T.smem_threads / 32) * 64 * 8 * (1 + p.n_vals) + 128 : 0;
+  const size_t smem_tab = table_bytes_for(hk, T.smem_threads, want_hot, T.smem_table_bytes) - (T.smem_table_bytes ? 0 : miss_queue);
   const size_t part_tab = table_bytes_for(pre_kind, T.part_threads, false, T.part_table_bytes);
   const uint32_t smem_slots = (uint32_t)std::max<size_t>(64, (smem_tab - 64) / slot_bytes) & ~7u;   // planes stay 8-byte aligned
   const uint32_t part_slots = (uint32_t)std::max<size_t>(64, (part_tab - 64) / part_slot_bytes) & ~7u;
@@ -437,6 +447,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
     }
     q->smem_bytes = align_up((size_t)q->slots * (variant == EIGER_PARTITION ? part_slot_bytes : slot_bytes) + 64, 16);
     q->stages = T.stages; q->hot_reserved = variant != EIGER_PARTITION && want_hot;
+    q->queue_bytes = variant == EIGER_GLOBAL ? miss_queue : 0;
     q->ring = (T.ring & (variant == EIGER_PARTITION ? 2 : 1)) != 0;
     q->smem_dyn = q->smem_bytes + (q->ring ? hash_agg_smem_layout(kd, p, variant == EIGER_PARTITION ? pre_kind : hk, q->threads, q->hot_reserved, T.stages).table_off : 0);
     q->table_bytes = align_up((size_t)(q->cap + 1) * q->stride, 256);
@@ -689,7 +700,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       for (int k = 0; k < kMaxKeyCols; ++k) H.out_keys[k] = k < nk ? out_keys[k] : nullptr;
       for (int j = 0; j < na; ++j) H.out_aggs[j] = out_aggs[j];
       H.n_out_aggs = na; H.out_capacity = out_capacity;
-      H.threads = q.threads; H.table_smem_bytes = q.smem_bytes; H.stages = q.stages; H.hot_reserved = q.hot_reserved; H.ring = q.ring ? 1 : 0;
+      H.threads = q.threads; H.table_smem_bytes = q.smem_bytes; H.stages = q.stages; H.hot_reserved = q.hot_reserved; H.ring = q.ring ? 1 : 0; H.queue_bytes = spec ? 0 : q.queue_bytes;
       {   // 32-bit keys in a nearly empty shared-memory table: 8-byte buckets (hashagg.cuh: BK)
         const double per_table = q.variant == EIGER_PARTITION ? q.ndv / (double)((size_t)1 << (q.bits1 + q.bits2)) : q.ndv;
         H.bucket_keys = ((src_kind == KK_I32 || src_kind == KK_GEN32) && q.variant != EIGER_GLOBAL && per_table <= tun().narrow_load * q.slots) ? 2 : 0;

@@ -54,6 +54,7 @@ struct HashAggArgs {
   uint8_t kw[kMaxKeyCols], vw[kMaxVals];        // bytes per element
   uint32_t hot_off, table_off;
   int32_t ring_hint;             // bulk copies carry an L2 evict_first policy
+  uint32_t queue_off;            // whole-input mode, per-thread loads: per-warp miss queues start here in dynamic shared memory (0 = none)
 };
 
 template <int KK> struct IsPre { static constexpr bool v = (KK == KK_U32PRE || KK == KK_U64PRE); };
@@ -78,6 +79,10 @@ struct Front {
   const uint32_t Sn;      // slots in use (<= a.slots)
   U* skeys;
   uint32_t* s_spill = nullptr;   // partition mode: set when a row of this work item went to the global table
+  // rows that found no room wait in a per-warp queue (64 entries: keys, then each value column) and go to
+  // the global table 32 at a time with full warps (EIGER_GLOBAL: a quarter of C3's rows take this path)
+  unsigned char* q_base = nullptr;
+  int q_n = 0;
   int sync_n = 0;                // threads that take part in cta_sync(): 0 = the whole CTA; else named barrier 1 (the ring's producer warp stays out)
   __device__ __forceinline__ void cta_sync() const {
     if (sync_n) asm volatile("bar.sync 1, %0;" :: "r"(sync_n) : "memory"); else __syncthreads();
@@ -385,6 +390,34 @@ struct Front {
         // same key here.  The work item therefore no longer owns its keys exclusively and must merge
         // (not emit) at the end.
         if (s_spill && miss) *reinterpret_cast<volatile uint32_t*>(s_spill) = 1u;
+        if constexpr (NV <= 2) if (q_base) {
+          const int lane = threadIdx.x & 31;
+          uint64_t* qk = reinterpret_cast<uint64_t*>(q_base);
+#pragma unroll
+          for (int k = 0; k < R; ++k) {
+            const bool mk = (miss >> k) & 1u;
+            const uint32_t m = __ballot_sync(0xffffffffu, mk);
+            if (m) {
+              if (mk) {
+                const int p = q_n + __popc(m & ((1u << lane) - 1u));
+                qk[p] = (uint64_t)u[k];
+#pragma unroll
+                for (int c = 0; c < NV; ++c) qk[64 * (1 + c) + p] = raw[k][c];
+              }
+              q_n += __popc(m);
+              if (q_n >= 32) {
+                __syncwarp();
+                q_n -= 32;
+                uint64_t rr[NV];
+#pragma unroll
+                for (int c = 0; c < NV; ++c) rr[c] = qk[64 * (1 + c) + q_n + lane];
+                back_row((U)qk[q_n + lane], rr);
+                __syncwarp();
+              }
+            }
+          }
+          return;
+        }
 #pragma unroll 1
         for (int k = 0; k < R; ++k) {
           U uu = u[0]; uint64_t rr[NV];
@@ -402,6 +435,22 @@ struct Front {
         }
       }
     }
+  }
+
+  // the rows still waiting in this warp's queue
+  __device__ __forceinline__ void drain_queue() {
+    if (!q_base) return;
+    const int lane = threadIdx.x & 31;
+    __syncwarp();
+    if (lane < q_n) {
+      const uint64_t* qk = reinterpret_cast<const uint64_t*>(q_base);
+      uint64_t rr[NV];
+#pragma unroll
+      for (int c = 0; c < NV; ++c) rr[c] = qk[64 * (1 + c) + lane];
+      back_row((U)qk[lane], rr);
+    }
+    q_n = 0;
+    __syncwarp();
   }
 
   // merge every occupied slot into the global table
@@ -762,6 +811,7 @@ hash_agg_ldg_kernel(const __grid_constant__ HashAggArgs a) {
     // hide HBM latency behind) ----
     constexpr int UNR = !Sig<SIG>::kStatic ? 1 : (NV >= 4 ? 1 : (sizeof(U) == 8 ? 1 : 2));   // 3 spills at the 64-register cap
     F f(a, smem, a.slots);
+    if (a.queue_off && !a.spec) f.q_base = smem + a.queue_off + (size_t)(tid >> 5) * 64 * 8 * (1 + NV);
     __shared__ uint64_t s_hot[(kMaxThreads / 32) * kMaxHot * F::NA];
     __shared__ uint32_t s_hot_rows[(kMaxThreads / 32) * kMaxHot];
     uint64_t* my_hot = s_hot + (tid >> 5) * kMaxHot * F::NA;
@@ -838,6 +888,7 @@ hash_agg_ldg_kernel(const __grid_constant__ HashAggArgs a) {
         __syncwarp();
       }
     }
+    f.drain_queue();
     if (a.spec) {
       if (missed) { atomicOr(&a.call->abort, 1u); atomicOr(&s_abort, 1u); }
       __syncthreads();
@@ -935,7 +986,9 @@ int launch_one(const HashAggLaunch& L, cudaStream_t s) {
   for (int c = 0; c < kMaxVals; ++c) { a.voff[c] = lay.voff[c]; a.vw[c] = lay.vw[c]; }
   a.stages = lay.stages; a.stage_bytes = lay.stage_bytes; a.n_src = lay.n_src;
   { const char* e = std::getenv("EIGER_RING_HINT"); a.ring_hint = e ? std::atoi(e) : 1; } a.hot_off = lay.hot_off; a.table_off = lay.table_off;
-  const size_t smem = (size_t)lay.table_off + L.table_smem_bytes;
+  a.queue_off = 0;
+  size_t smem = (size_t)lay.table_off + L.table_smem_bytes;
+  if (!L.ring && !IsPre<KK>::v && L.queue_bytes) { a.queue_off = (uint32_t)((smem + 127) & ~(size_t)127); smem = a.queue_off + L.queue_bytes; }
   if (smem > 32 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<L.blocks, L.threads, smem, s>>>(a);
   count_launch();

@@ -130,6 +130,7 @@ struct HashAggLaunch {
   int stages;               // shared-memory ring stages; 0 = default
   bool hot_reserved;        // room for the heavy-hitter cells is part of the layout (EIGER_GLOBAL)
   size_t table_smem_bytes;  // shared-memory table of one CTA
+  size_t queue_bytes;       // whole-input mode: per-warp miss queues behind the table (0 = misses go to the global table lane by lane)
 };
 int launch_hash_agg(const HashAggLaunch& L, cudaStream_t s);
 size_t hash_agg_slot_bytes(const AggPlan& p, int key_kind);   // shared-memory bytes per slot
