@@ -137,7 +137,7 @@ struct Tunables {
     dict = (int)env("EIGER_DICT", 1);
     pack_stride = (int)env("EIGER_PACK_STRIDE", 1);
     split_max = (int)env("EIGER_SPLIT_MAX", 4);        // measured (C5 dense, ms): C = 2 / 4 / 8 / 16 -> 1.26 / 1.86 / 3.11 / 5.15 against 2.8-3.3 for global RED
-    miss_queue = (int)env("EIGER_MISS_QUEUE", 1);
+    miss_queue = (int)env("EIGER_MISS_QUEUE", 0);     // measured on C3: 5.25 ms with the queues (and a 32 KB smaller front) against 4.84 ms without
     split_hash = (int)env("EIGER_SPLIT_HASH", 0);      // the hash flavour loses everywhere (scattered 2^13 / 2^14: 3.1 / 6.4 ms against 2.7 / 3.4)
     split_bytes = (size_t)env("EIGER_SPLIT_KB", 192) << 10;
     part_full_table = (int)env("EIGER_PART_FULL_TABLE", 0);
