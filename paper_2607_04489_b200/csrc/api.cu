@@ -867,7 +867,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] sample: min %lld max %lld ndv %.1f collision %.5f\n", (long long)local[0].min, (long long)local[0].max, local[0].ndv_est, collision);
     if (T.spec && fusable && plan_query(rt, keys, nk, n, vals, nv, aggs, na, plan_stats, EIGER_AUTO, &qs, skewed) == EIGER_OK &&
         ((qs.variant == EIGER_DIRECT && (qs.front != FRONT_NONE || qs.R <= (1ull << 24))) ||
-         (qs.variant == EIGER_SMEM && qs.ndv * 1.25 <= 0.6 * qs.slots * (double)(1 << qs.split_lg))) && have_room(qs.total_bytes)) {
+         (qs.variant == EIGER_SMEM && qs.ndv * (1.0 + 4 * kSigma) <= 0.70 * qs.slots * (double)(1 << qs.split_lg))) && have_room(qs.total_bytes)) {   // tables close at 0.75 x slots: a fuller table than planned discards the pass
       bool aborted = false;
       if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] plan: variant %d kk %d sig %d slots %u limit %u cap %llu stride %u smem %zu front %d R %llu\n", qs.variant, qs.key_kind, qs.sig, qs.slots, qs.limit, (unsigned long long)qs.cap, qs.stride, qs.smem_bytes, qs.front, (unsigned long long)qs.R);
       rc = execute(qs, local, 1, &aborted);
