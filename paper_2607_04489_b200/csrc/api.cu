@@ -558,7 +558,8 @@ int do_profile(Runtime* rt, const eiger_col* cols, int nk, int64_t n, int with_h
 
 // device arenas owned by the library: g_arena holds the columns of eiger_groupby_host, g_ws the scratch of
 // calls that pass workspace = NULL; both grow on demand and live until eiger_shutdown
-struct Arena { char* base = nullptr; size_t size = 0; } g_arena, g_ws;
+struct Arena { char* base = nullptr; size_t size = 0; } g_arena, g_ws, g_enc;
+int g_chain_depth = 0;
 int ws_reserve(size_t bytes) {
   if (bytes <= g_ws.size) return EIGER_OK;
   if (g_ws.base) { cudaFree(g_ws.base); g_ws.base = nullptr; g_ws.size = 0; }
@@ -566,6 +567,13 @@ int ws_reserve(size_t bytes) {
   g_ws.size = bytes;
   return EIGER_OK;
 }
+
+int dict_encode_impl(Runtime* rt, const void* keys, int32_t dtype, int64_t n, int32_t* codes_out, void* dict_out, int64_t dict_capacity,
+                     int64_t* ndv, void* workspace, size_t workspace_bytes, cudaStream_t s);
+size_t dict_encode_ws_bytes(int32_t dtype, int64_t n, int64_t dict_capacity);
+int groupby_through_dictionaries(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eiger_col* vals, int nv,
+                                 const eiger_agg* aggs, int na, const eiger_stats* st, void* const* out_keys, void* const* out_aggs,
+                                 int64_t out_capacity, int64_t* n_groups, int force, int32_t* chosen, cudaStream_t s, eiger_call_info* info);
 
 int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eiger_col* vals, int nv,
                 const eiger_agg* aggs, int na, const eiger_stats* stats_in,
@@ -934,6 +942,20 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
   }
   QueryPlan q;
   rc = plan_query(rt, keys, nk, n, vals, nv, aggs, na, st, force, &q, skewed);
+  if (rc == EIGER_ERR_INFEASIBLE && nk >= 2 && own_ws && force != EIGER_DIRECT && g_chain_depth == 0) {
+    // The ranges of the key columns multiply past 2^64: no fused key exists.  The paper's order
+    // (PAPER.md:219): range test first, "otherwise ... dictionary encoding" - the widest columns are
+    // dictionary-encoded (order-preserving, Algorithm 1) until the fused domain fits, the group-by
+    // runs on the codes and the dictionaries decode the group keys.
+    bool wide = false;
+    { unsigned __int128 prod = 1; for (int k = 0; k < nk; ++k) { const uint64_t r = range_of(st[k]); if (r == 0) { wide = true; break; } prod *= r; if (prod >> 64) { wide = true; break; } } }
+    if (wide) {
+      ++g_chain_depth;       // the call on the code columns must not encode again (codes of codes have the same NDV)
+      const int rc2 = groupby_through_dictionaries(rt, keys, nk, n, vals, nv, aggs, na, st, out_keys, out_aggs, out_capacity, n_groups, force, chosen, s, info);
+      --g_chain_depth;
+      return rc2;
+    }
+  }
   if (rc) return rc;
   if (chosen) *chosen = q.variant;
   return execute(q, st, 0, nullptr);
@@ -945,6 +967,85 @@ int arena_reserve(size_t bytes) {
   if (g_arena.base) { cudaFree(g_arena.base); g_arena.base = nullptr; g_arena.size = 0; }
   EIGER_CUDA(cudaMalloc(reinterpret_cast<void**>(&g_arena.base), bytes));
   g_arena.size = bytes;
+  return EIGER_OK;
+}
+
+int enc_reserve(size_t bytes) {
+  if (bytes <= g_enc.size) return EIGER_OK;
+  if (g_enc.base) { cudaFree(g_enc.base); g_enc.base = nullptr; g_enc.size = 0; }
+  EIGER_CUDA(cudaMalloc(reinterpret_cast<void**>(&g_enc.base), bytes));
+  g_enc.size = bytes;
+  return EIGER_OK;
+}
+
+__global__ void dict_decode_kernel(const int32_t* __restrict__ codes, const void* __restrict__ dict, int dtype, int64_t g, void* __restrict__ out) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < g; i += stride) {
+    const int64_t c = codes[i];
+    switch (dtype) {
+      case EIGER_I8: static_cast<int8_t*>(out)[i] = static_cast<const int8_t*>(dict)[c]; break;
+      case EIGER_I32: static_cast<int32_t*>(out)[i] = static_cast<const int32_t*>(dict)[c]; break;
+      default: static_cast<int64_t*>(out)[i] = static_cast<const int64_t*>(dict)[c]; break;
+    }
+  }
+}
+
+int groupby_through_dictionaries(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eiger_col* vals, int nv,
+                                 const eiger_agg* aggs, int na, const eiger_stats* st, void* const* out_keys, void* const* out_aggs,
+                                 int64_t out_capacity, int64_t* n_groups, int force, int32_t* chosen, cudaStream_t s, eiger_call_info* info) {
+  // widest columns first, until the product of (code ranges, remaining column ranges) fits 63 bits
+  int order[kMaxKeyCols];
+  for (int k = 0; k < nk; ++k) order[k] = k;
+  auto width = [&](int k) { const uint64_t r = range_of(st[k]); return r == 0 ? 65.0 : std::log2((double)r); };
+  std::sort(order, order + nk, [&](int a, int b) { return width(a) > width(b); });
+  const int64_t dict_cap = std::min<int64_t>(n, (int64_t)1 << 26);
+  bool enc[kMaxKeyCols] = {false, false, false, false};
+  double bits = 0;
+  for (int k = 0; k < nk; ++k) bits += width(k);
+  int n_enc = 0;
+  for (int i = 0; i < nk && bits > 62.0; ++i) {
+    const int k = order[i];
+    enc[k] = true; ++n_enc;
+    bits -= width(k) - std::min(width(k), std::log2((double)std::max<int64_t>(dict_cap, 2)));    // at best: the capacity bound; refined below
+  }
+  // encoded columns: codes (n x 4), dictionary (dict_cap elements), decoded-later group codes (out_capacity x 4)
+  size_t need = 0;
+  for (int k = 0; k < nk; ++k) if (enc[k]) need += align_up((size_t)n * 4, 256) + align_up((size_t)dict_cap * dtype_size(keys[k].dtype), 256) + align_up((size_t)std::max<int64_t>(out_capacity, 1) * 4, 256);
+  int rc = enc_reserve(need + 256);
+  if (rc) return rc;
+  char* w = g_enc.base;
+  eiger_col nkeys[kMaxKeyCols];
+  void* nout[kMaxKeyCols];
+  int32_t* gcodes[kMaxKeyCols] = {nullptr, nullptr, nullptr, nullptr};
+  void* dicts[kMaxKeyCols] = {nullptr, nullptr, nullptr, nullptr};
+  for (int k = 0; k < nk; ++k) {
+    nkeys[k] = keys[k]; nout[k] = out_keys[k];
+    if (!enc[k]) continue;
+    int32_t* codes = reinterpret_cast<int32_t*>(w); w += align_up((size_t)n * 4, 256);
+    dicts[k] = w; w += align_up((size_t)dict_cap * dtype_size(keys[k].dtype), 256);
+    gcodes[k] = reinterpret_cast<int32_t*>(w); w += align_up((size_t)std::max<int64_t>(out_capacity, 1) * 4, 256);
+    const size_t ws_need = dict_encode_ws_bytes(keys[k].dtype, n, dict_cap);
+    rc = ws_reserve(ws_need);
+    if (rc) return rc;
+    int64_t ndv = 0;
+    rc = dict_encode_impl(rt, keys[k].data, keys[k].dtype, n, codes, dicts[k], dict_cap, &ndv, g_ws.base, g_ws.size, s);
+    if (rc == EIGER_ERR_OUT_CAPACITY) return EIGER_ERR_INFEASIBLE;       // too many distinct values for a dictionary: nothing left to try
+    if (rc) return rc;
+    nkeys[k].data = codes; nkeys[k].dtype = EIGER_I32; nkeys[k].reserved = 0;
+    nout[k] = gcodes[k];
+  }
+  // the same call on the code columns (statistics gathered inside: the codes are dense, so the range test settles them)
+  rc = run_groupby(rt, nkeys, nk, n, vals, nv, aggs, na, nullptr, nout, out_aggs, out_capacity, n_groups, force, chosen, nullptr, 0, s, info);
+  if (rc) return rc;
+  const int64_t g = std::min<int64_t>(*n_groups, out_capacity);
+  for (int k = 0; k < nk; ++k) {
+    if (!enc[k] || g == 0) continue;
+    dict_decode_kernel<<<(int)std::min<int64_t>((g + 255) / 256, (int64_t)rt->sm_count * 8), 256, 0, s>>>(gcodes[k], dicts[k], keys[k].dtype, g, out_keys[k]);
+    count_launch();
+  }
+  EIGER_CUDA(cudaGetLastError());
+  EIGER_CUDA(cudaStreamSynchronize(s));
+  if (info) info->kernel_launches += n_enc;      // the decode kernels (the encode passes are counted by their own calls)
   return EIGER_OK;
 }
 
@@ -1123,7 +1224,9 @@ static size_t dict_fixed_bytes(int64_t dict_capacity) {
   const size_t g = (size_t)std::max<int64_t>(dict_capacity, 1);
   return 3 * align_up(g * 8, 256) + align_up((2 * g + 1024 + 1) * 16, 256);
 }
-size_t eiger_dict_encode_workspace_bytes(int32_t dtype, int64_t n, int64_t dict_capacity) {
+}  // extern "C"
+namespace eiger { namespace {
+size_t dict_encode_ws_bytes(int32_t dtype, int64_t n, int64_t dict_capacity) {
   if (!is_key_dtype(dtype) || n < 0 || dict_capacity < 0) return 0;
   eiger_col k{nullptr, dtype, 0};
   eiger_agg a{EIGER_COUNT, 0};
@@ -1132,16 +1235,12 @@ size_t eiger_dict_encode_workspace_bytes(int32_t dtype, int64_t n, int64_t dict_
   return dict_fixed_bytes(dict_capacity) + std::max(all, srt) + 512;
 }
 
-int eiger_dict_encode(const void* keys, int32_t dtype, int64_t n, int32_t* codes_out, void* dict_out, int64_t dict_capacity,
-                      int64_t* ndv, void* workspace, size_t workspace_bytes, void* stream) {
+int dict_encode_impl(Runtime* rt, const void* keys, int32_t dtype, int64_t n, int32_t* codes_out, void* dict_out, int64_t dict_capacity,
+                     int64_t* ndv, void* workspace, size_t workspace_bytes, cudaStream_t s) {
   if (!ndv || n < 0 || dict_capacity < 0 || !is_key_dtype(dtype)) return EIGER_ERR_ARG;
   *ndv = 0;
   if (n == 0) return EIGER_OK;
   if (!keys || ((uintptr_t)keys & 15) || !codes_out || !dict_out || !workspace || ((uintptr_t)workspace & 255)) return EIGER_ERR_ARG;
-  std::lock_guard<std::mutex> lk(g_mu);
-  Runtime* rt = runtime();
-  if (!rt) return EIGER_ERR_CUDA;
-  cudaStream_t s = static_cast<cudaStream_t>(stream);
   const size_t fixed = dict_fixed_bytes(dict_capacity);
   if (workspace_bytes < fixed + 256) return EIGER_ERR_WORKSPACE;
   const size_t g_cap = (size_t)std::max<int64_t>(dict_capacity, 1);
@@ -1183,6 +1282,18 @@ int eiger_dict_encode(const void* keys, int32_t dtype, int64_t n, int32_t* codes
   EIGER_CUDA(cudaStreamSynchronize(s));
   return hb->overflow ? EIGER_ERR_TABLE_OVERFLOW : EIGER_OK;
 }
+} }  // namespace eiger::<unnamed>
+extern "C" {
+
+size_t eiger_dict_encode_workspace_bytes(int32_t dtype, int64_t n, int64_t dict_capacity) { return dict_encode_ws_bytes(dtype, n, dict_capacity); }
+
+int eiger_dict_encode(const void* keys, int32_t dtype, int64_t n, int32_t* codes_out, void* dict_out, int64_t dict_capacity,
+                      int64_t* ndv, void* workspace, size_t workspace_bytes, void* stream) {
+  std::lock_guard<std::mutex> lk(g_mu);
+  Runtime* rt = runtime();
+  if (!rt) return EIGER_ERR_CUDA;
+  return dict_encode_impl(rt, keys, dtype, n, codes_out, dict_out, dict_capacity, ndv, workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
+}
 
 int64_t eiger_launch_count(void) { return g_launches.load(); }
 
@@ -1223,6 +1334,7 @@ void eiger_shutdown(void) {
   std::lock_guard<std::mutex> lk(g_mu);
   if (g_arena.base) { cudaFree(g_arena.base); g_arena = Arena{}; }
   if (g_ws.base) { cudaFree(g_ws.base); g_ws = Arena{}; }
+  if (g_enc.base) { cudaFree(g_enc.base); g_enc = Arena{}; }
   if (g_rt.device >= 0) {
     cudaFree(g_rt.prof); cudaFree(g_rt.call); cudaFreeHost(g_rt.pinned);
     for (int i = 0; i < g_pool_n; ++i) cudaEventDestroy(g_pool[i]);

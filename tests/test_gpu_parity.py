@@ -461,12 +461,21 @@ def test_multi_key_wide_ranges_and_infeasible():
     ds = datagen.Dataset("mk-wide", n, [k0, k1, k2], [v], [(eiger.SUM, 0), (eiger.COUNT, 0)])
     ran = run_all_variants(ds, expect_infeasible=(eiger.DIRECT,))
     assert eiger.DIRECT not in ran[1:]
-    # a fourth full-range int64 column: the product of the ranges no longer fits 64 bits
+    # a fourth full-range int64 column: the product of the ranges no longer fits 64 bits.  Round 1 refused
+    # (EIGER_ERR_INFEASIBLE); now the wide columns are dictionary-encoded (Algorithm 1), the
+    # group-by runs on the codes and the dictionaries decode the group keys
     k3 = datagen.fmix64(ids + 5)
-    d = to_dev(datagen.Dataset("mk-over", n, [k0, k1, k2, k3], [v], [(eiger.SUM, 0), (eiger.COUNT, 0)]))
-    with pytest.raises(eiger.EigerError) as e:
-        eiger.groupby(d.keys, d.vals, d.aggs)
-    assert e.value.code == eiger.ERR_INFEASIBLE
+    over = datagen.Dataset("mk-over", n, [k0, k1, k2, k3], [v], [(eiger.SUM, 0), (eiger.COUNT, 0)])
+    d = to_dev(over)
+    want_over = oracle_result(over)
+    for f in (eiger.AUTO, eiger.SMEM, eiger.PARTITION, eiger.SORT):
+        res = eiger.groupby(d.keys, d.vals, d.aggs, force=f)
+        assert_matches(res, want_over, d.aggs, d.vals)
+    # two full-range columns of all-distinct values: no dictionary is small enough -> still refused
+    i = torch.arange(n, dtype=torch.int64)
+    wide2 = to_dev(datagen.Dataset("mk-hopeless", n, [datagen.fmix64(i), datagen.fmix64(i + n)], [v], [(eiger.COUNT, 0)]))
+    res = eiger.groupby(wide2.keys, wide2.vals, wide2.aggs)         # n distinct pairs: codes of 18 + 18 bits fit
+    assert res.n_groups == n
     with pytest.raises(eiger.EigerError) as e:                                   # five key columns
         eiger.groupby(d.keys + [d.keys[0]], d.vals, d.aggs)
     assert e.value.code == eiger.ERR_ARG
