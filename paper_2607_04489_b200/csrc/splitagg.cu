@@ -103,24 +103,21 @@ split_direct_kernel(const __grid_constant__ SplitArgs a) {
   const int64_t n_full = a.n / tile;
   int cnt = 0;                                   // entries waiting in this warp's queue (warp-uniform)
   bool bad = false;
+  const uint32_t lt = (1u << lane) - 1u;
   auto scan_row = [&](U ur, bool okr, uint32_t off, int64_t base) {
-    const uint64_t uu = (uint64_t)ur;
-    if (okr && uu >= a.cap) { bad = true; okr = false; }                  // outside the planned range (speculative / caller's statistics)
-    const bool mine = okr && ((uint32_t)uu & (C - 1)) == me;
+    const bool mine = okr && ((uint32_t)ur & (C - 1)) == me;
     const uint32_t m = __ballot_sync(0xffffffffu, mine);
-    if (m) {
-      if (mine) {
-        const int p = cnt + __popc(m & ((1u << lane) - 1u));
-        q_slot[p] = (uint32_t)(uu >> a.lgC);
-        q_row[p] = off;
-      }
-      cnt += __popc(m);
-      if (cnt >= 32) {
-        __syncwarp();
-        cnt -= 32;
-        consume(q_slot[cnt + lane], base + q_row[cnt + lane]);
-        __syncwarp();
-      }
+    if (mine) {
+      const int p = cnt + __popc(m & lt);
+      q_slot[p] = (uint32_t)((uint64_t)ur >> a.lgC);
+      q_row[p] = off;
+    }
+    cnt += __popc(m);
+    if (cnt >= 32) {
+      __syncwarp();
+      cnt -= 32;
+      consume(q_slot[cnt + lane], base + q_row[cnt + lane]);
+      __syncwarp();
     }
   };
   auto drain = [&](int64_t base) {               // the queue is drained at the end of every tile (row offsets are relative to it)
@@ -137,8 +134,16 @@ split_direct_kernel(const __grid_constant__ SplitArgs a) {
       const bool more = t + groups < n_full;
       if (more) TK::load(a.key, (t + groups) * tile, tid, nxt);
       const int64_t base = t * tile;
+      // one range check per thread and tile (the largest of its keys): a key outside the planned range
+      // (speculative run / caller's statistics) discards the whole result, so the thread's keys of this
+      // tile are simply not queued
+      U umax = cur[0];
 #pragma unroll
-      for (int r = 0; r < KR; ++r) scan_row(cur[r], true, TK::row_of(r, tid), base);
+      for (int r = 1; r < KR; ++r) umax = cur[r] > umax ? cur[r] : umax;
+      const bool in_range = (uint64_t)umax < a.cap;
+      bad = bad || !in_range;
+#pragma unroll
+      for (int r = 0; r < KR; ++r) scan_row(cur[r], in_range, TK::row_of(r, tid), base);
       drain(base);
       if (a.spec && __any_sync(0xffffffffu, bad)) break;
       if (more) {
@@ -152,8 +157,10 @@ split_direct_kernel(const __grid_constant__ SplitArgs a) {
     const int64_t base = n_full * tile;
     for (int64_t o = tid - lane; base + o < a.n; o += kSplitThreads) {          // warp-uniform trip count
       const int64_t i = base + o + lane;
-      const bool okr = i < a.n;
-      scan_row(okr ? load_u<KK>(a.key, i) : (U)0, okr, (uint32_t)(o + lane), base);
+      bool okr = i < a.n;
+      const U ur = okr ? load_u<KK>(a.key, i) : (U)0;
+      if (okr && (uint64_t)ur >= a.cap) { bad = true; okr = false; }
+      scan_row(ur, okr, (uint32_t)(o + lane), base);
     }
     drain(base);
   }
