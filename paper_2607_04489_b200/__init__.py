@@ -259,7 +259,7 @@ class Workspace:
 
 
 def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int | None = None,
-            workspace: Workspace | None = None) -> GroupByResult:
+            workspace: Workspace | None = None, scratch: torch.Tensor | None = None) -> GroupByResult:
     """eiger_groupby on device columns.
 
     keys: 1-4 CUDA integer tensors; vals: CUDA int64 / float64 / int32 tensors; aggs: [(op, val_col)].
@@ -268,6 +268,8 @@ def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int |
     (workspace = NULL at the C ABI); `workspace` only keeps the output columns between calls.  The one
     decision taken here: when the caller fixed no out_capacity and the library reports more groups than
     the output columns hold (EIGER_ERR_OUT_CAPACITY carries the count), allocate that many and call again.
+    `scratch`: a caller-owned uint8 CUDA tensor passed as the C ABI's workspace instead of the library arena
+    (size it with workspace_bytes(); too small -> EIGER_ERR_WORKSPACE).
     """
     if isinstance(keys, torch.Tensor):
         keys = [keys]
@@ -293,7 +295,9 @@ def groupby(keys, vals, aggs, force: int = AUTO, stats=None, out_capacity: int |
             oap = (ctypes.c_void_p * 8)(*[t.data_ptr() for t in oa])
             ng, chosen, info = ctypes.c_int64(0), ctypes.c_int32(0), _CallInfo()
             rc = L.eiger_groupby(kc, len(keys), n, vc, len(vals), ac, len(aggs), sc, okp, oap, cap,
-                                 ctypes.byref(ng), force, ctypes.byref(chosen), None, 0, _stream(dev), ctypes.byref(info))
+                                 ctypes.byref(ng), force, ctypes.byref(chosen),
+                                 scratch.data_ptr() if scratch is not None else None, scratch.numel() if scratch is not None else 0,
+                                 _stream(dev), ctypes.byref(info))
             if rc == ERR_OUT_CAPACITY and out_capacity is None and attempt == 0:
                 cap = int(ng.value)
                 continue

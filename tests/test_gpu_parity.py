@@ -718,3 +718,27 @@ def test_split_hash_tables(monkeypatch, lg, kdtype):
     d2 = to_dev(ds2)
     res = eiger.groupby(d2.keys, d2.vals, d2.aggs, force=eiger.SMEM, stats=st)
     assert_matches(res, oracle_result(ds2), d2.aggs, d2.vals)
+
+
+def test_caller_owned_workspace():
+    # the C ABI with the caller's scratch (sized by eiger_groupby_workspace_bytes) instead of the library arena
+    ds = datagen.config5(n=(1 << 21) + 5, ndv=1 << 17, scattered=True)
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    st = eiger.profile_keys(d.keys)
+    for f in (eiger.SMEM, eiger.GLOBAL, eiger.PARTITION, eiger.SORT):
+        need = eiger.workspace_bytes(d.keys, d.vals, d.aggs, st, f)
+        assert need > 0
+        buf = torch.empty(need + 256, dtype=torch.uint8, device=DEV)
+        off = (-buf.data_ptr()) % 256
+        res = eiger.groupby(d.keys, d.vals, d.aggs, force=f, stats=st, scratch=buf[off:off + need])
+        assert_matches(res, want, d.aggs, d.vals)
+        with pytest.raises(eiger.EigerError) as e:
+            eiger.groupby(d.keys, d.vals, d.aggs, force=f, stats=st, scratch=buf[off:off + 4096])
+        assert e.value.code == eiger.ERR_WORKSPACE
+    # no statistics: the worst case over the variants
+    need = eiger.workspace_bytes(d.keys, d.vals, d.aggs)
+    buf = torch.empty(need + 256, dtype=torch.uint8, device=DEV)
+    off = (-buf.data_ptr()) % 256
+    res = eiger.groupby(d.keys, d.vals, d.aggs, scratch=buf[off:off + need])
+    assert_matches(res, want, d.aggs, d.vals)
