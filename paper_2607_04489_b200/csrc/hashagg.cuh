@@ -83,7 +83,6 @@ struct Front {
   // the global table 32 at a time with full warps (EIGER_GLOBAL: a quarter of C3's rows take this path)
   unsigned char* q_base = nullptr;
   int q_n = 0;
-  uint32_t ins = 0;              // keys this lane inserted since the warp last added its count to the CTA's
   int sync_n = 0;                // threads that take part in cta_sync(): 0 = the whole CTA; else named barrier 1 (the ring's producer warp stays out)
   __device__ __forceinline__ void cta_sync() const {
     if (sync_n) asm volatile("bar.sync 1, %0;" :: "r"(sync_n) : "memory"); else __syncthreads();
@@ -178,7 +177,7 @@ struct Front {
           U old;
           if constexpr (sizeof(U) == 4) old = atomicCAS(skeys + h, kEmpty32, u);
           else old = (U)atomicCAS(reinterpret_cast<unsigned long long*>(skeys + h), (unsigned long long)kEmpty64, (unsigned long long)u);
-          if (old == empty_of<U>()) { ins += 1u; res = (int)h; done = true; }      // counted per warp in pair()
+          if (old == empty_of<U>()) { atomicAdd(s_count, 1u); res = (int)h; done = true; }
           else if (old == u) { res = (int)h; done = true; }
           else q = load_bucket(b);          // somebody else took it: look at the bucket again
         }
@@ -325,14 +324,6 @@ struct Front {
       if (h1 >= 0) { issue((uint32_t)h1, raw1, p1); finish((uint32_t)h1, raw1, p1); }
     }
     __syncwarp();
-    // new keys of this trip: one shared-memory add per warp instead of one per inserting lane (a work item
-    // of all-distinct keys queued 4096 same-address atomics on the counter: a quarter of its time).  The
-    // count that closes the table is therefore stale by at most one trip of every warp - a soft bound: a
-    // table that fills up beyond it sends the rows it cannot place to the global table as before.
-    {
-      const uint32_t tot = __reduce_add_sync(0xffffffffu, ins);
-      if (tot) { if ((threadIdx.x & 31) == 0) atomicAdd(s_count, tot); ins = 0; }
-    }
     return (v0 && h0 < 0 ? 1u : 0u) | (v1 && h1 < 0 ? 2u : 0u);
   }
 
@@ -490,18 +481,16 @@ struct Front {
   // totals, then every warp writes its groups in slot order (consecutive lanes -> consecutive
   // rows of the output columns).  KT = the single key column's C type (0 bytes: generic path).
   template <class KT>
-  __device__ __forceinline__ void emit_rows(int tid, int T, unsigned long long base, uint32_t* s_cursor) {
+  __device__ __forceinline__ void emit_rows(int tid, int T, unsigned long long base, uint32_t wbase) {
     const int lane = tid & 31;
+    uint32_t run = wbase;
     for (uint32_t h0 = tid - lane; h0 < Sn; h0 += T) {      // warp-uniform trip count
       const uint32_t h = h0 + lane;
       const U k = h < Sn ? skeys[h] : empty_of<U>();
       const bool occ = k != empty_of<U>();
       const uint32_t m = __ballot_sync(0xffffffffu, occ);
-      if (m == 0) continue;
-      uint32_t start = 0;
-      if (lane == 0) start = atomicAdd(s_cursor, (uint32_t)__popc(m));
-      start = __shfl_sync(0xffffffffu, start, 0);
-      const uint64_t g = base + start + __popc(m & ((1u << lane) - 1u));
+      const uint64_t g = base + run + __popc(m & ((1u << lane) - 1u));
+      run += __popc(m);
       if (occ && (int64_t)g < a.out_capacity) {
         if constexpr (sizeof(KT) == 1 && !std::is_same<KT, int8_t>::value) store_group_key(a.key, a.out_keys, (uint64_t)k, g);
         else static_cast<KT*>(a.out_keys[0])[g] = (KT)((uint64_t)k + a.key.base[0]);
@@ -517,24 +506,34 @@ struct Front {
     }
   }
   __device__ void flush_emit(int tid, int T, uint32_t n_keys, unsigned long long* s_base, uint32_t* s_wtot) {
-    // one pass: every warp claims room for the groups of its 32 slots from a cursor in shared memory
-    // (the order of the groups inside the partition is free); the CTA's block of the output was claimed
-    // with one global atomic.  (Round 1 counted per warp in a first pass over the slots, scanned, and
-    // wrote in a second pass: two more barriers and the keys read twice per work item.)
-    const int lane = tid & 31;
-    if (tid == 0) { *s_base = n_keys ? atomicAdd(&a.call->n_groups, (unsigned long long)n_keys) : 0ull; s_wtot[0] = 0u; }
+    const int lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) *s_base = n_keys ? atomicAdd(&a.call->n_groups, (unsigned long long)n_keys) : 0ull;
+    uint32_t cnt = 0;
+    for (uint32_t h0 = tid - lane; h0 < Sn; h0 += T) {
+      const uint32_t h = h0 + lane;
+      cnt += __popc(__ballot_sync(0xffffffffu, h < Sn && skeys[h] != empty_of<U>()));
+    }
+    if (lane == 0) s_wtot[warp] = cnt;
+    cta_sync();
+    if (warp == 0) {       // exclusive scan of up to 32 warp totals
+      const uint32_t v = lane < (T >> 5) ? s_wtot[lane] : 0u;
+      uint32_t inc = v;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += y; }
+      s_wtot[lane] = inc - v;
+    }
     cta_sync();
     const unsigned long long base = *s_base;
+    const uint32_t wbase = s_wtot[warp];
     if (a.key.ncols == 1) {
       switch (a.key.dtype[0]) {
-        case EIGER_I8: emit_rows<int8_t>(tid, T, base, s_wtot); break;
-        case EIGER_I32: emit_rows<int32_t>(tid, T, base, s_wtot); break;
-        default: emit_rows<int64_t>(tid, T, base, s_wtot); break;
+        case EIGER_I8: emit_rows<int8_t>(tid, T, base, wbase); break;
+        case EIGER_I32: emit_rows<int32_t>(tid, T, base, wbase); break;
+        default: emit_rows<int64_t>(tid, T, base, wbase); break;
       }
     } else {
-      emit_rows<uint8_t>(tid, T, base, s_wtot);     // several key columns: un-fuse per group
+      emit_rows<uint8_t>(tid, T, base, wbase);     // several key columns: un-fuse per group
     }
-    (void)lane;
   }
 };
 
