@@ -54,7 +54,8 @@ typedef enum {
   EIGER_ERR_INFEASIBLE = -4,   /* the forced variant cannot run on this input                */
   EIGER_ERR_CUDA = -5,         /* a CUDA runtime call failed; eiger_last_cuda_error() says   */
   EIGER_ERR_TABLE_OVERFLOW = -6, /* NDV estimate too low and no room in workspace to retry  */
-  EIGER_ERR_STATS = -7         /* a key lies outside the caller's eiger_stats [min, max]     */
+  EIGER_ERR_STATS = -7,        /* a key lies outside the caller's eiger_stats [min, max]     */
+  EIGER_ERR_STATIC_LIMIT = -8  /* eiger_groupby_direct_static: key range > EIGER_STATIC_MAX_SLOTS */
 } eiger_status;
 
 typedef struct { const void* data; int32_t dtype; int32_t reserved; } eiger_col; /* length n */
@@ -199,6 +200,34 @@ int eiger_groupby_host(const eiger_col* keys, int32_t n_key_cols, int64_t n,
 int eiger_dict_encode(const void* keys, int32_t dtype, int64_t n, int32_t* codes_out, void* dict_out, int64_t dict_capacity,
                       int64_t* ndv, void* workspace, size_t workspace_bytes, void* stream);
 size_t eiger_dict_encode_workspace_bytes(int32_t dtype, int64_t n, int64_t dict_capacity);
+
+/* eiger_groupby_direct_static — SUM + COUNT of one int64 value column per key, direct-index variant
+ * (the array-based group-by for a small key range), for callers that cannot
+ * allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.
+ * This entry point calls no cudaMalloc / cudaFree and no allocating library routine, and does not
+ * touch the library's arena or runtime state.  Its accumulator array is a file-scope __device__ array
+ * of EIGER_STATIC_MAX_SLOTS slots (1 MiB + 256 bytes on every GPU that loads the library, held until
+ * the process exits).
+ *   keys        DEVICE, n elements of key_dtype (EIGER_I8 / I32 / I64)
+ *   key_min, key_max   bounds of the keys, inclusive; key_max - key_min + 1 <= EIGER_STATIC_MAX_SLOTS,
+ *               else EIGER_ERR_STATIC_LIMIT (nothing is launched).  A key outside the bounds is not
+ *               aggregated and fails the call with EIGER_ERR_STATS.
+ *   vals        DEVICE, n int64; SUM wraps modulo 2^64 like eiger_groupby's
+ *   out_keys    DEVICE, out_capacity elements of key_dtype; out_sum, out_count DEVICE, out_capacity
+ *               int64 each; group order unspecified (as eiger_groupby).  Owned by the caller.
+ *   n_groups    HOST; set to the group count even when EIGER_ERR_OUT_CAPACITY says out_capacity was
+ *               too small (the first out_capacity positions are then filled)
+ *   stream      cudaStream_t (NULL = the default stream); the call returns after the stream has drained
+ * The array is shared by every call on a device and keeps the last call's contents; each call clears
+ * the part it uses on `stream` first.  Calls that overlap on the GPU (two streams, two host threads)
+ * RACE on it: serialise them.  Not usable from several processes' worth of concurrency either way -
+ * each process has its own copy.
+ * Errors: EIGER_ERR_ARG, EIGER_ERR_STATIC_LIMIT, EIGER_ERR_STATS, EIGER_ERR_OUT_CAPACITY, EIGER_ERR_CUDA. */
+#define EIGER_STATIC_MAX_SLOTS 65536
+int eiger_groupby_direct_static(const void* keys, int32_t key_dtype, int64_t n, int64_t key_min, int64_t key_max,
+                                const int64_t* vals, void* out_keys, int64_t* out_sum, int64_t* out_count,
+                                int64_t out_capacity, int64_t* n_groups, void* stream);
+int64_t eiger_static_max_slots(void);
 
 /* Number of kernels this library has launched in this process (bench.py's gpu_launches). */
 int64_t eiger_launch_count(void);

@@ -25,7 +25,7 @@ I8, I32, I64, F64 = 0, 1, 2, 3
 SUM, COUNT, MIN, MAX = 0, 1, 2, 3
 AUTO, DIRECT, SMEM, GLOBAL, PARTITION, SORT = 0, 1, 2, 3, 4, 5
 VARIANT_NAMES = {AUTO: "auto", DIRECT: "direct", SMEM: "smem", GLOBAL: "global", PARTITION: "partition", SORT: "sort"}
-OK, ERR_ARG, ERR_WORKSPACE, ERR_OUT_CAPACITY, ERR_INFEASIBLE, ERR_CUDA, ERR_TABLE_OVERFLOW, ERR_STATS = 0, -1, -2, -3, -4, -5, -6, -7
+OK, ERR_ARG, ERR_WORKSPACE, ERR_OUT_CAPACITY, ERR_INFEASIBLE, ERR_CUDA, ERR_TABLE_OVERFLOW, ERR_STATS, ERR_STATIC_LIMIT = 0, -1, -2, -3, -4, -5, -6, -7, -8
 HLL_M = 1 << 14
 
 # every symbol include/eiger.h declares (tests check the library exports each of them)
@@ -34,6 +34,7 @@ EXPORTS = [
     "eiger_groupby_workspace_bytes", "eiger_select_variant", "eiger_groupby_host",
     "eiger_launch_count", "eiger_set_kernel_timing", "eiger_kernel_time_ms", "eiger_strerror",
     "eiger_last_cuda_error", "eiger_variant_name", "eiger_shutdown", "eiger_probe", "eiger_dict_encode", "eiger_dict_encode_workspace_bytes", "eiger_reload_tunables",
+    "eiger_groupby_direct_static", "eiger_static_max_slots",
 ]
 
 _DTYPES = {torch.int8: I8, torch.int32: I32, torch.int64: I64, torch.float64: F64}
@@ -137,6 +138,9 @@ def lib() -> ctypes.CDLL:
         L.eiger_dict_encode.argtypes = [vp, i32, i64, vp, vp, i64, ctypes.POINTER(i64), vp, sz, vp]
         L.eiger_dict_encode_workspace_bytes.restype = sz
         L.eiger_dict_encode_workspace_bytes.argtypes = [i32, i64, i64]
+        L.eiger_groupby_direct_static.restype = ctypes.c_int
+        L.eiger_groupby_direct_static.argtypes = [vp, i32, i64, i64, i64, vp, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
+        L.eiger_static_max_slots.restype = i64
         L.eiger_probe.restype = ctypes.c_int
         L.eiger_probe.argtypes = [ctypes.c_char_p, i64, i64, ctypes.POINTER(ctypes.c_double), vp]
         _lib = L
@@ -367,6 +371,35 @@ def dict_encode(keys: torch.Tensor, dict_capacity: int | None = None):
                                    ctypes.byref(ndv), ws.data_ptr(), ws.numel(), _stream(keys.device)))
     g = int(ndv.value)
     return codes[:n], d[:g], g
+
+
+def groupby_direct_static(keys: torch.Tensor, vals: torch.Tensor, key_min: int, key_max: int,
+                          out_keys: torch.Tensor, out_sum: torch.Tensor, out_count: torch.Tensor) -> int:
+    """eiger_groupby_direct_static: SUM + COUNT per key with the accumulator array in the library's static
+    device scratch (no allocation anywhere in the call; key_max - key_min + 1 <= static_max_slots()).
+    The caller owns the three output tensors (capacity = the shortest); returns the group count.
+    Calls that overlap on the GPU race on the shared array (include/eiger.h)."""
+    if not keys.is_cuda or keys.dtype not in _KEY_T or not keys.is_contiguous():
+        raise ValueError("keys must be a contiguous CUDA int8 / int32 / int64 tensor")
+    if vals.dtype != torch.int64 or vals.device != keys.device or not vals.is_contiguous() or vals.numel() != keys.numel():
+        raise ValueError("vals must be a contiguous int64 tensor of the keys' length on the keys' device")
+    for o, dt in ((out_keys, keys.dtype), (out_sum, torch.int64), (out_count, torch.int64)):
+        if o.dtype != dt or o.device != keys.device or not o.is_contiguous():
+            raise ValueError("outputs: contiguous tensors on the keys' device, out_keys of the keys' dtype, the others int64")
+    cap = min(out_keys.numel(), out_sum.numel(), out_count.numel())
+    n = keys.numel()
+    g = ctypes.c_int64(0)
+    with torch.cuda.device(keys.device):
+        _check(lib().eiger_groupby_direct_static(keys.data_ptr() if n else None, _DTYPES[keys.dtype], n, int(key_min), int(key_max),
+                                                 vals.data_ptr() if n else None, out_keys.data_ptr() if cap else None,
+                                                 out_sum.data_ptr() if cap else None, out_count.data_ptr() if cap else None,
+                                                 cap, ctypes.byref(g), _stream(keys.device)))
+    return int(g.value)
+
+
+def static_max_slots() -> int:
+    """eiger_static_max_slots: the largest key range eiger_groupby_direct_static takes."""
+    return int(lib().eiger_static_max_slots())
 
 
 def probe(name: str, param: int = 0, param2: int = 0) -> float:

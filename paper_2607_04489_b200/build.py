@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libeiger.so")
-SOURCES = ["api.cu", "profile.cu", "aggregate.cu", "hashagg.cu", "hashagg_i32.cu", "hashagg_i64.cu", "hashagg_pre.cu", "partition.cu", "sortagg.cu", "dictenc.cu", "splitagg.cu", "probe.cu"]
+SOURCES = ["api.cu", "profile.cu", "aggregate.cu", "hashagg.cu", "hashagg_i32.cu", "hashagg_i64.cu", "hashagg_pre.cu", "partition.cu", "sortagg.cu", "dictenc.cu", "splitagg.cu", "probe.cu", "noalloc.cu"]
 HEADERS = ["dev.cuh", "rows.cuh", "ring.cuh", "scatter.cuh", "hashagg.cuh", "internal.h", os.path.join("..", "..", "include", "eiger.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr", "-Xptxas", "-warn-spills"]

@@ -1322,6 +1322,7 @@ const char* eiger_strerror(int code) {
     case EIGER_ERR_CUDA: return "CUDA runtime error (see eiger_last_cuda_error)";
     case EIGER_ERR_TABLE_OVERFLOW: return "hash table overflow: NDV under-estimated and no workspace to retry";
     case EIGER_ERR_STATS: return "a key lies outside the [min, max] of the statistics supplied by the caller";
+    case EIGER_ERR_STATIC_LIMIT: return "key range exceeds EIGER_STATIC_MAX_SLOTS, the size of the static scratch array of eiger_groupby_direct_static";
     default: return "unknown error";
   }
 }
