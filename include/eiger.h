@@ -71,6 +71,7 @@ typedef struct {
   int32_t sort_passes;          /* EIGER_SORT: 8-bit radix passes                                                 */
   double ndv_est;               /* the NDV estimate the tables were sized with (after clamping to min(n, range)) */
   int64_t kernel_launches;      /* kernels this call launched                                                     */
+  int64_t spill_rows;           /* EIGER_GLOBAL: rows (padding included) that went through the spill buffer; else 0 */
 } eiger_call_info;
 
 /* HOST struct.  n = 0 gives min = INT64_MAX, max = INT64_MIN, ndv_est = 0. */
@@ -235,7 +236,7 @@ int64_t eiger_launch_count(void);
 /* Per-kernel device time, measured with CUDA events on the caller's stream inside the calls
  * above while enabled (eiger_set_kernel_timing(1)); off by default.  `which`: 0 = aggregation
  * kernel (the dominant one), 1 = profile kernel, 2 = partition kernels, 3 = table init,
- * 4 = compaction.  Returns the milliseconds accumulated since the last call with reset != 0;
+ * 4 = compaction, 5 = aggregation of the spill buffer's partitions (EIGER_GLOBAL).  Returns the milliseconds accumulated since the last call with reset != 0;
  * *launches (may be NULL) receives how many launches that covers. */
 void eiger_set_kernel_timing(int32_t enabled);
 

@@ -1,6 +1,6 @@
 """Builds libeiger.so in-tree with nvcc for sm_100a (no torch involved).
 
-    python -m paper_2607_04489_b200.build [--force] [--verbose]
+    python -m paper_2607_04489_b200.build [--force] [--verbose] [--define NAME=VALUE ...] [--out FILE]
 """
 from __future__ import annotations
 
@@ -32,16 +32,22 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build_library(force: bool = False, verbose: bool = False) -> str:
+def build_library(force: bool = False, verbose: bool = False, defines: tuple = (), out: str | None = None) -> str:
+    """defines / out: an experiment build (e.g. defines=("EIGER_STREAM_L2_HINT=0",)) into another file; always rebuilt."""
+    if out or defines:
+        return _build(verbose, tuple(defines), out or LIB, os.path.join(HERE, "build", "x_" + "_".join(d.replace("=", "") for d in defines)))
     if not force and not _stale():
         return LIB
+    return _build(verbose, (), LIB, os.path.join(HERE, "build"))
+
+
+def _build(verbose: bool, defines: tuple, lib: str, objdir: str) -> str:
     nvcc = _nvcc()
-    objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     procs = []
     for src in SOURCES:
         obj = os.path.join(objdir, src.replace(".cu", ".o"))
-        cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-c",
+        cmd = [nvcc, *NVCC_FLAGS, *[f"-D{d}" for d in defines], *(["-Xptxas", "-v"] if verbose else []), "-c",
                os.path.join(CSRC, src), "-o", obj]
         procs.append((src, obj, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     objs = []
@@ -52,9 +58,12 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
         if verbose or "warning" in out.lower():
             sys.stderr.write(out)
         objs.append(obj)
-    subprocess.check_call([nvcc, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
-    return LIB
+    subprocess.check_call([nvcc, "-shared", "-o", lib, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
+    return lib
 
 
 if __name__ == "__main__":
-    print(build_library(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    # --define NAME=VALUE (repeatable) and --out FILE: an experiment build next to the ordinary one
+    defs = tuple(sys.argv[i + 1] for i, a in enumerate(sys.argv[:-1]) if a == "--define")
+    outs = [sys.argv[i + 1] for i, a in enumerate(sys.argv[:-1]) if a == "--out"]
+    print(build_library(force="--force" in sys.argv, verbose="--verbose" in sys.argv, defines=defs, out=outs[0] if outs else None))

@@ -19,9 +19,9 @@ Runtime g_rt;
 std::atomic<int64_t> g_launches{0};
 char g_cuda_err[512] = "";
 bool g_timing = false;
-constexpr int kTimeSlots = 5;
-double g_time_ms[kTimeSlots] = {0, 0, 0, 0, 0};
-int64_t g_time_n[kTimeSlots] = {0, 0, 0, 0, 0};
+constexpr int kTimeSlots = 6;
+double g_time_ms[kTimeSlots] = {0, 0, 0, 0, 0, 0};
+int64_t g_time_n[kTimeSlots] = {0, 0, 0, 0, 0, 0};
 
 // event pairs recorded during one call, resolved after the call's final synchronise
 struct Pending { cudaEvent_t a, b; int slot; };
@@ -97,6 +97,10 @@ struct Tunables {
   int part_full_table;                // EIGER_PARTITION reserves the full-size global table when partitions may be cut (round-1 behaviour)
   int split_max;                      // direct-index array split over up to this many CTAs (splitagg.cu); 0 = off
   int miss_queue;                     // EIGER_GLOBAL queues the front's misses per warp (hashagg.cuh)
+  int global_spill;                   // EIGER_GLOBAL: the front's misses go to a spill buffer that is partitioned and aggregated afterwards
+  double spill_frac;                  // ... with room for this share of the rows (what does not fit takes the global table)
+  double spill_min_rows;              // ... for inputs of at least this many rows
+  double spill_lg;                    // ... reserved by the CTAs in chunks of at least 2^spill_lg rows
   int split_hash;                     // EIGER_SMEM may split its hash tables over up to 16 CTAs (experiment, off)
   size_t split_bytes;                 // ... each holding at most this much of it in shared memory
   int pack_stride;                    // global hash table slots of 40 / 48 bytes are not padded to 64
@@ -138,6 +142,10 @@ struct Tunables {
     pack_stride = (int)env("EIGER_PACK_STRIDE", 1);
     split_max = (int)env("EIGER_SPLIT_MAX", 4);        // measured (C5 dense, ms): C = 2 / 4 / 8 / 16 -> 1.26 / 1.86 / 3.11 / 5.15 against 2.8-3.3 for global RED
     miss_queue = (int)env("EIGER_MISS_QUEUE", 0);     // measured on C3: 5.25 ms with the queues (and a 32 KB smaller front) against 4.84 ms without
+    global_spill = (int)env("EIGER_GLOBAL_SPILL", 0);  // measured on C3: 7.8 ms with the spill buffer against 5.5 ms without
+    spill_frac = env("EIGER_SPILL_FRAC", 0.5);
+    spill_min_rows = env("EIGER_SPILL_MIN_ROWS", 4194304);
+    spill_lg = env("EIGER_SPILL_LG", 9);
     split_hash = (int)env("EIGER_SPLIT_HASH", 0);      // the hash flavour loses everywhere (scattered 2^13 / 2^14: 3.1 / 6.4 ms against 2.7 / 3.4)
     split_bytes = (size_t)env("EIGER_SPLIT_KB", 192) << 10;
     part_full_table = (int)env("EIGER_PART_FULL_TABLE", 0);
@@ -180,6 +188,12 @@ struct QueryPlan {
   int sort_bits = 0, sort_passes = 0;   // SORT: significant bits of the rebased fused key, 8-bit passes
   uint32_t dict_slots = 0, dict_shift = 0;   // FRONT_DICT: dictionary image entries (power of two)
   int split_lg = 0;                          // FRONT_SPLIT: log2 of the CTAs that share the array
+  // GLOBAL with a spill buffer: capacity in rows (0 = none; a multiple of the chunk), chunk = 2^spill_lg rows, and
+  // the plan of the partition + per-partition aggregation that follows
+  uint64_t spill_rows = 0; int spill_lg = 0;
+  int sp_bits1 = 0, sp_bits2 = 0, sp_threads = 0;
+  uint32_t sp_slots = 0, sp_limit = 0;
+  size_t sp_smem_bytes = 0, sp_smem_dyn = 0;
 };
 
 uint64_t range_of(const eiger_stats& s) {   // max - min + 1, 0 when it is 2^64
@@ -444,6 +458,39 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
       if (variant == EIGER_SMEM && !skewed && (q->split_lg = split_lg_for(ndv)) > 0) {
         q->slots = split_slots; q->limit = (uint32_t)(0.75 * split_slots); q->threads = 1024;
       }
+      // EIGER_GLOBAL: the rows the front cannot hold (C3: 28 % of them) cost a look-up and one L2 reduction per
+      // accumulator each.  They are appended to a spill buffer instead, partitioned by hash and aggregated per
+      // partition in shared memory like EIGER_PARTITION's rows; the partitions merge into the global table.
+      // 64-bit rebased keys below the empty marker only (the marker pads the buffer), 8-byte value columns.
+      bool all8 = true;
+      for (int c = 0; c < p.n_vals; ++c) all8 = all8 && p.vw[c] != 4;
+      if (variant == EIGER_GLOBAL && T.global_spill && T.global_front && hk != KK_I32 && R != 0 && all8 && !(T.ring & 1) &&
+          (double)n >= T.spill_min_rows && n < (1ll << 32)) {
+        const int sms = rt ? std::max(1, rt->sm_count) : 148;
+        int lg = (int)T.spill_lg;
+        while (((uint64_t)n / (uint64_t)sms) >> lg >= 1000) ++lg;        // a CTA reserves at most 1024 chunks (hashagg.cuh)
+        const uint64_t chunk = 1ull << lg;
+        q->spill_lg = lg;
+        q->spill_rows = std::max<uint64_t>(chunk, ((uint64_t)((double)n * std::min(1.0, T.spill_frac)) + chunk - 1) / chunk * chunk);
+        const size_t sp_slot_bytes = hash_agg_slot_bytes(p, KK_U64PRE);
+        const size_t sp_tab = table_bytes_for(KK_U64PRE, T.part_threads, false, T.part_table_bytes);
+        q->sp_slots = (uint32_t)std::max<size_t>(64, (sp_tab - 64) / sp_slot_bytes) & ~7u;
+        q->sp_limit = (uint32_t)(0.85 * q->sp_slots); q->sp_threads = T.part_threads;
+        const double per = std::max(1.0, T.load * q->sp_slots);
+        const double need = ndv * (1.0 + 4 * kSigma) / per;
+        int bits = T.part_min_bits;
+        while (bits < 20 && (double)(1u << bits) < need) ++bits;
+        const int mb = partition_max_bits_per_level();
+        if (bits <= mb) { q->sp_bits1 = bits; q->sp_bits2 = 0; } else { q->sp_bits1 = (bits + 1) / 2; q->sp_bits2 = bits - q->sp_bits1; }
+        q->sp_smem_bytes = align_up((size_t)q->sp_slots * sp_slot_bytes + 64, 16);
+        q->sp_smem_dyn = q->sp_smem_bytes;                                  // this pass always loads its rows per thread
+        const size_t P1 = (size_t)1 << q->sp_bits1, P = (size_t)1 << (q->sp_bits1 + q->sp_bits2);
+        const size_t col = align_up((size_t)q->spill_rows * 8, 256);
+        const size_t copy = (1 + (size_t)p.n_vals) * col;
+        q->part_bytes = copy + align_up(P * 4, 256) + align_up((P + 1) * 8, 256) + align_up((2 * P + 2) * 4, 256) + align_up((P1 + 1) * 8, 256) +
+                        align_up(P1 * 8, 256) + copy;
+        if (q->sp_bits2 > 0) q->part_bytes += align_up((P + 1) * 8, 256) + align_up(P * 8, 256) + copy;
+      }
     }
     q->smem_bytes = align_up((size_t)q->slots * (variant == EIGER_PARTITION ? part_slot_bytes : slot_bytes) + 64, 16);
     q->stages = T.stages; q->hot_reserved = variant != EIGER_PARTITION && want_hot;
@@ -453,7 +500,6 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
     q->table_bytes = align_up((size_t)(q->cap + 1) * q->stride, 256);
   }
   q->total_bytes = q->table_bytes + q->part_bytes + 256;
-  (void)rt;
   return EIGER_OK;
 }
 
@@ -752,6 +798,14 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         const int64_t tiles = std::max<int64_t>(1, n / (4 * (int64_t)q.threads));
         H.blocks = (int)std::min<int64_t>(rt->sm_count, tiles);
       }
+      // EIGER_GLOBAL with a spill buffer: [keys][value columns] of q.spill_rows rows each, then the partition scratch
+      const bool spilling = q.variant == EIGER_GLOBAL && q.spill_rows > 0 && !spec && !q.ring;
+      const size_t sp_col = align_up((size_t)q.spill_rows * 8, 256);
+      if (spilling) {
+        H.spill_keys = reinterpret_cast<uint64_t*>(pws); pws += sp_col;
+        for (int c = 0; c < q.plan.n_vals; ++c) { H.spill_vals[c] = reinterpret_cast<uint64_t*>(pws); pws += sp_col; }
+        H.spill_lg = q.spill_lg; H.spill_cap_chunks = q.spill_rows >> q.spill_lg;
+      }
       if (q.variant == EIGER_SMEM && q.split_lg > 0) {
         const int C = 1 << q.split_lg;
         H.blocks = (int)std::max<int64_t>(1, std::min<int64_t>(rt->sm_count / C, (n + 4095) / 4096)) * C;
@@ -759,6 +813,52 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         { Timed t(s, 0); rc = launch_split_hash(H, q.split_lg, s); if (rc) return rc; }
       } else
       { Timed t(s, 0); rc = launch_hash_agg(H, s); if (rc) return rc; }
+      if (spilling) {
+        // how much was spilled (whole chunks; the tail of every CTA's last chunk is padding)
+        unsigned long long* chunks = reinterpret_cast<unsigned long long*>(static_cast<char*>(rt->pinned) + 1536);
+        EIGER_CUDA(cudaMemcpyAsync(chunks, reinterpret_cast<const char*>(rt->call) + offsetof(CallDev, spill_chunks), sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
+        EIGER_CUDA(cudaStreamSynchronize(s));
+        const int64_t n_sp = (int64_t)(std::min<unsigned long long>(*chunks, H.spill_cap_chunks) << q.spill_lg);
+        info->spill_rows = n_sp;
+        if (n_sp > 0) {
+          PartitionLaunch P{};
+          P.key = q.key; P.key.ptr[0] = H.spill_keys; P.key.ncols = 1;
+          for (int k = 1; k < kMaxKeyCols; ++k) P.key.ptr[k] = nullptr;
+          P.plan = q.plan;
+          for (int c = 0; c < q.plan.n_vals; ++c) { P.plan.vals[c] = H.spill_vals[c]; P.plan.vw[c] = 8; }
+          P.n = n_sp; P.key_kind = KK_U64PRE; P.bits1 = q.sp_bits1; P.bits2 = q.sp_bits2;
+          const size_t P1 = (size_t)1 << q.sp_bits1, PP = (size_t)1 << (q.sp_bits1 + q.sp_bits2);
+          auto take = [&](size_t bytes) { char* r = pws; pws += align_up(bytes, 256); return r; };
+          P.hist = reinterpret_cast<uint32_t*>(take(PP * 4));
+          P.item_off = reinterpret_cast<unsigned long long*>(take((PP + 1) * 8));
+          P.item_part = reinterpret_cast<uint32_t*>(take((2 * PP + 2) * 4));
+          P.chunk_rows = std::max<int64_t>(32768, n_sp / (int64_t)PP);
+          P.off1 = reinterpret_cast<unsigned long long*>(take((P1 + 1) * 8));
+          P.cur1 = reinterpret_cast<unsigned long long*>(take(P1 * 8));
+          P.keysA = take(sp_col);
+          for (int c = 0; c < q.plan.n_vals; ++c) P.valsA[c] = take(sp_col);
+          if (q.sp_bits2 > 0) {
+            P.off2 = reinterpret_cast<unsigned long long*>(take((PP + 1) * 8));
+            P.cur2 = reinterpret_cast<unsigned long long*>(take(PP * 8));
+            P.keysB = take(sp_col);
+            for (int c = 0; c < q.plan.n_vals; ++c) P.valsB[c] = take(sp_col);
+          }
+          { Timed t(s, 2); rc = launch_partition(P, rt->sm_count, rt->smem_optin, s); if (rc) return rc; }
+          info->partition_levels = q.sp_bits2 > 0 ? 2 : 1;
+          info->partition_key_bytes = 8;
+          HashAggLaunch H2 = H;
+          H2.key = P.key; H2.key.ptr[0] = P.out_keys; H2.plan = P.plan;
+          for (int c = 0; c < q.plan.n_vals; ++c) H2.plan.vals[c] = P.out_vals[c];
+          H2.n = n_sp; H2.key_kind = KK_U64PRE;
+          H2.part_off = P.out_off; H2.item_off = P.item_off; H2.item_part = P.item_part; H2.n_parts = P.n_parts;
+          H2.slots = q.sp_slots; H2.limit = q.sp_limit; H2.max_probes = 0; H2.bucket_keys = 0; H2.n_hot = 0;
+          H2.threads = q.sp_threads; H2.table_smem_bytes = q.sp_smem_bytes; H2.hot_reserved = false; H2.ring = 0; H2.queue_bytes = 0;
+          H2.spill_keys = nullptr; H2.skip_empty = 1; H2.force_merge = 1;
+          const int occ = (int)std::max<size_t>(1, std::min<size_t>((size_t)(2048 / q.sp_threads), (rt->smem_optin + 1024) / (q.sp_smem_dyn + 1024)));
+          H2.blocks = (int)std::min<int64_t>((int64_t)rt->sm_count * occ, (int64_t)P.n_parts + n_sp / P.chunk_rows);
+          { Timed t(s, 5); rc = launch_hash_agg(H2, s); if (rc) return rc; }
+        }
+      }
     }
 
     CompactLaunch C{};

@@ -112,36 +112,57 @@ template <> struct Sig<SIG_S4C> {
 };
 
 // ---- streamed loads: read once, keep out of L1, first to leave L2 ----------------
+// EIGER_STREAM_L2_HINT (default 1): the loads carry an L2 evict_first policy, so that what the kernels
+// keep L2-resident next to the stream (the global hash table, the global direct array) is not pushed
+// out by rows that are read exactly once (hash tables "perform well when ... cache-resident").
+#ifndef EIGER_STREAM_L2_HINT
+#define EIGER_STREAM_L2_HINT 1
+#endif
+#if EIGER_STREAM_L2_HINT
+// not volatile: a pure value, computed once per thread wherever the compiler hoists it
+__device__ __forceinline__ uint64_t stream_policy() {
+  uint64_t p;
+  asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+#define EIGER_LDG_HINT ".L2::cache_hint"
+#define EIGER_LDG_POL(n) ", %" #n
+#define EIGER_LDG_POL_ARG , "l"(stream_policy())
+#else
+#define EIGER_LDG_HINT ""
+#define EIGER_LDG_POL(n) ""
+#define EIGER_LDG_POL_ARG
+#endif
 __device__ __forceinline__ uint4 ldg_stream_16(const void* p) {
   uint4 r;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  asm volatile("ld.global.nc.L1::no_allocate" EIGER_LDG_HINT ".v4.u32 {%0,%1,%2,%3}, [%4]" EIGER_LDG_POL(5) ";"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p) EIGER_LDG_POL_ARG);
   return r;
 }
 __device__ __forceinline__ uint2 ldg_stream_8(const void* p) {
   uint2 r;
-  asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];"
-               : "=r"(r.x), "=r"(r.y) : "l"(p));
+  asm volatile("ld.global.nc.L1::no_allocate" EIGER_LDG_HINT ".v2.u32 {%0,%1}, [%2]" EIGER_LDG_POL(3) ";"
+               : "=r"(r.x), "=r"(r.y) : "l"(p) EIGER_LDG_POL_ARG);
   return r;
 }
 __device__ __forceinline__ uint32_t ldg_stream_4(const void* p) {
   uint32_t r;
-  asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(r) : "l"(p));
+  asm volatile("ld.global.nc.L1::no_allocate" EIGER_LDG_HINT ".u32 %0, [%1]" EIGER_LDG_POL(2) ";" : "=r"(r) : "l"(p) EIGER_LDG_POL_ARG);
   return r;
 }
 __device__ __forceinline__ uint32_t ldg_stream_2(const void* p) {
   uint16_t r;
-  asm volatile("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=h"(r) : "l"(p));
+  asm volatile("ld.global.nc.L1::no_allocate" EIGER_LDG_HINT ".u16 %0, [%1]" EIGER_LDG_POL(2) ";" : "=h"(r) : "l"(p) EIGER_LDG_POL_ARG);
   return r;
 }
 __device__ __forceinline__ uint32_t ldg_stream_1(const void* p) {
   uint32_t r;
-  asm volatile("ld.global.nc.L1::no_allocate.u8 %0, [%1];" : "=r"(r) : "l"(p));
+  asm volatile("ld.global.nc.L1::no_allocate" EIGER_LDG_HINT ".u8 %0, [%1]" EIGER_LDG_POL(2) ";" : "=r"(r) : "l"(p) EIGER_LDG_POL_ARG);
   return r;
 }
 __device__ __forceinline__ uint64_t ldg_stream_u64(const void* p) {
   uint64_t r;
-  asm volatile("ld.global.nc.L1::no_allocate.u64 %0, [%1];" : "=l"(r) : "l"(p));
+  asm volatile("ld.global.nc.L1::no_allocate" EIGER_LDG_HINT ".u64 %0, [%1]" EIGER_LDG_POL(2) ";" : "=l"(r) : "l"(p) EIGER_LDG_POL_ARG);
   return r;
 }
 

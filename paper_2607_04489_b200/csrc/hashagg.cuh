@@ -55,7 +55,12 @@ struct HashAggArgs {
   uint32_t hot_off, table_off;
   int32_t ring_hint;             // bulk copies carry an L2 evict_first policy
   uint32_t queue_off;            // whole-input mode, per-thread loads: per-warp miss queues start here in dynamic shared memory (0 = none)
+  // whole-input mode: spill buffer for the rows the front cannot hold (internal.h: HashAggLaunch); partition mode: flags
+  uint64_t* sp_keys; uint64_t* sp_vals[kMaxVals]; uint64_t sp_cap_chunks; int32_t sp_lg;
+  int32_t skip_empty, force_merge;
 };
+
+constexpr uint32_t kSpillChunks = 1024;    // chunks one CTA can reserve in the spill buffer
 
 template <int KK> struct IsPre { static constexpr bool v = (KK == KK_U32PRE || KK == KK_U64PRE); };
 
@@ -83,6 +88,10 @@ struct Front {
   // the global table 32 at a time with full warps (EIGER_GLOBAL: a quarter of C3's rows take this path)
   unsigned char* q_base = nullptr;
   int q_n = 0;
+  // spill buffer (EIGER_GLOBAL): rows appended by this CTA so far, and 1 + the global index of the CTA's k-th chunk
+  // (0 = nobody has reserved it yet, ~0 = the buffer is full: such rows take the global table)
+  uint32_t* sp_cursor = nullptr;
+  uint32_t* sp_base = nullptr;
   int sync_n = 0;                // threads that take part in cta_sync(): 0 = the whole CTA; else named barrier 1 (the ring's producer warp stays out)
   __device__ __forceinline__ void cta_sync() const {
     if (sync_n) asm volatile("bar.sync 1, %0;" :: "r"(sync_n) : "memory"); else __syncthreads();
@@ -382,6 +391,7 @@ struct Front {
   // rows of one trip that found no room in shared memory: global table, one code copy per trip
   template <int R>
   __device__ __forceinline__ void spill(const U (&u)[R], const uint64_t (&raw)[R][NV], uint32_t miss, bool& missed) {
+    // (miss is a copy: the spill-buffer path narrows it to the rows it could not place)
     if (__any_sync(0xffffffffu, miss != 0)) {
       if (a.spec) { missed = missed || miss != 0; }
       else {
@@ -390,6 +400,42 @@ struct Front {
         // same key here.  The work item therefore no longer owns its keys exclusively and must merge
         // (not emit) at the end.
         if (s_spill && miss) *reinterpret_cast<volatile uint32_t*>(s_spill) = 1u;
+        if constexpr (sizeof(U) == 8) if (sp_cursor) {
+          // Append to the spill buffer: the warp's rows get consecutive places in the CTA's numbering (one
+          // shared-memory atomic per warp and row position); the lane whose row opens a chunk reserves that chunk
+          // in the buffer (one global atomic per 2^sp_lg rows) and publishes it, the others wait for it.
+          const int lane = threadIdx.x & 31;
+          const uint32_t cmask = (1u << a.sp_lg) - 1u;
+          uint32_t fb = 0;           // rows that found the buffer full
+#pragma unroll
+          for (int k = 0; k < R; ++k) {
+            const bool mk = (miss >> k) & 1u;
+            const uint32_t m = __ballot_sync(0xffffffffu, mk);
+            if (m == 0u) continue;
+            uint32_t pos0 = 0;
+            if (lane == 0) pos0 = atomicAdd(sp_cursor, (uint32_t)__popc(m));
+            pos0 = __shfl_sync(0xffffffffu, pos0, 0);
+            const uint32_t li = pos0 + __popc(m & ((1u << lane) - 1u));
+            const uint32_t c = li >> a.sp_lg;
+            if (mk && (li & cmask) == 0u && c < kSpillChunks) {
+              const unsigned long long g = atomicAdd(&a.call->spill_chunks, 1ull);
+              *reinterpret_cast<volatile uint32_t*>(sp_base + c) = g < a.sp_cap_chunks ? (uint32_t)g + 1u : ~0u;
+            }
+            __syncwarp();
+            if (mk) {
+              uint32_t g = ~0u;
+              if (c < kSpillChunks) while ((g = *reinterpret_cast<volatile uint32_t*>(sp_base + c)) == 0u) {}
+              if (g != ~0u) {
+                const uint64_t at = ((uint64_t)(g - 1u) << a.sp_lg) | (li & cmask);
+                a.sp_keys[at] = (uint64_t)u[k];
+#pragma unroll
+                for (int cc = 0; cc < NV; ++cc) if (S::kStatic || cc < a.plan.n_vals) a.sp_vals[cc][at] = raw[k][cc];
+              } else fb |= 1u << k;
+            }
+          }
+          miss = fb;
+          if (!__any_sync(0xffffffffu, miss != 0)) return;
+        }
         if constexpr (NV <= 2) if (q_base) {
           const int lane = threadIdx.x & 31;
           uint64_t* qk = reinterpret_cast<uint64_t*>(q_base);
@@ -434,6 +480,20 @@ struct Front {
           __syncwarp();
         }
       }
+    }
+  }
+
+  // spill buffer: the unused tail of this CTA's last chunk is filled with the empty marker (a key no row of a
+  // spill buffer can have: api.cu takes the buffer only when the rebased keys stay below it), so that the
+  // buffer is one gapless run of whole chunks for the partition pass.  Called by all threads after a barrier.
+  __device__ void spill_pad(int tid, int T) {
+    if constexpr (sizeof(U) == 8) {
+      if (!sp_cursor) return;
+      const uint32_t total = *sp_cursor, cmask = (1u << a.sp_lg) - 1u, c = total >> a.sp_lg;
+      if ((total & cmask) == 0u || c >= kSpillChunks) return;
+      const uint32_t g = sp_base[c];
+      if (g == 0u || g == ~0u) return;
+      for (uint32_t li = (total & cmask) + tid; li <= cmask; li += T) a.sp_keys[((uint64_t)(g - 1u) << a.sp_lg) | li] = kEmpty64;
     }
   }
 
@@ -816,7 +876,13 @@ hash_agg_ldg_kernel(const __grid_constant__ HashAggArgs a) {
     __shared__ uint32_t s_hot_rows[(kMaxThreads / 32) * kMaxHot];
     uint64_t* my_hot = s_hot + (tid >> 5) * kMaxHot * F::NA;
     uint32_t* my_hot_rows = s_hot_rows + (tid >> 5) * kMaxHot;
-    if (tid == 0) { s_count = 0; s_abort = 0; }
+    __shared__ uint32_t s_sp_cursor;
+    __shared__ uint32_t s_sp_base[sizeof(U) == 8 ? kSpillChunks : 1];
+    if (tid == 0) { s_count = 0; s_abort = 0; s_sp_cursor = 0; }
+    if constexpr (sizeof(U) == 8) if (a.sp_keys && !a.spec) {
+      for (uint32_t c = tid; c < kSpillChunks; c += T) s_sp_base[c] = 0u;
+      f.sp_cursor = &s_sp_cursor; f.sp_base = s_sp_base;
+    }
     f.init(tid, T);
     if (a.n_hot) f.hot_init(s_hot, s_hot_rows, tid, T);
     __syncthreads();
@@ -896,6 +962,7 @@ hash_agg_ldg_kernel(const __grid_constant__ HashAggArgs a) {
     } else {
       __syncthreads();
     }
+    f.spill_pad(tid, T);
     f.flush_merge(tid, T);
     if (a.n_hot) f.hot_flush(s_hot, s_hot_rows, tid, T);
   } else {
@@ -941,7 +1008,11 @@ hash_agg_ldg_kernel(const __grid_constant__ HashAggArgs a) {
         uint32_t miss = 0;
 #pragma unroll
         for (int s = 0; s < UNR; s += 2) {
-          const bool v0 = c0 + (int64_t)s * T + tid < r1, v1 = (s + 1 < UNR) && (c0 + (int64_t)(s + 1) * T + tid < r1);
+          bool v0 = c0 + (int64_t)s * T + tid < r1, v1 = (s + 1 < UNR) && (c0 + (int64_t)(s + 1) * T + tid < r1);
+          if constexpr (sizeof(U) == 8) if (a.skip_empty) {      // padding rows of a spill buffer
+            v0 = v0 && u[b][s] != kEmpty64;
+            v1 = v1 && u[b][s + 1 < UNR ? s + 1 : s] != kEmpty64;
+          }
           miss |= f.pair(v0 ? u[b][s] : (U)0, raw[b][s], v0, v1 ? u[b][s + 1 < UNR ? s + 1 : s] : (U)0, raw[b][s + 1 < UNR ? s + 1 : s], v1, &s_count) << s;
         }
         f.spill(u[b], raw[b], miss, missed);
@@ -960,7 +1031,7 @@ hash_agg_ldg_kernel(const __grid_constant__ HashAggArgs a) {
       __syncthreads();
       // emit only what this CTA owns exclusively: a whole partition none of whose rows was sent to
       // the global table (otherwise a key could be emitted here AND by the compaction pass)
-      if (exclusive && s_spilled == 0u) f.flush_emit(tid, T, s_count, &s_base, s_wtot);
+      if (exclusive && s_spilled == 0u && !a.force_merge) f.flush_emit(tid, T, s_count, &s_base, s_wtot);
       else f.flush_merge(tid, T);
     }
   }
@@ -987,6 +1058,9 @@ int launch_one(const HashAggLaunch& L, cudaStream_t s) {
   a.stages = lay.stages; a.stage_bytes = lay.stage_bytes; a.n_src = lay.n_src;
   { const char* e = std::getenv("EIGER_RING_HINT"); a.ring_hint = e ? std::atoi(e) : 1; } a.hot_off = lay.hot_off; a.table_off = lay.table_off;
   a.queue_off = 0;
+  a.sp_keys = (L.ring || IsPre<KK>::v) ? nullptr : L.spill_keys; a.sp_cap_chunks = L.spill_cap_chunks; a.sp_lg = L.spill_lg;
+  for (int c = 0; c < kMaxVals; ++c) a.sp_vals[c] = L.spill_vals[c];
+  a.skip_empty = L.skip_empty; a.force_merge = L.force_merge;
   size_t smem = (size_t)lay.table_off + L.table_smem_bytes;
   if (!L.ring && !IsPre<KK>::v && L.queue_bytes) { a.queue_off = (uint32_t)((smem + 127) & ~(size_t)127); smem = a.queue_off + L.queue_bytes; }
   if (smem > 32 * 1024) EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -24,6 +24,7 @@ struct CallDev {
   unsigned long long n_groups;   // compaction claim counter
   uint32_t overflow;             // a hash table ran out of probes
   uint32_t abort;                // speculative pass: some CTA's shared-memory table filled up
+  unsigned long long spill_chunks;   // EIGER_GLOBAL with a spill buffer: chunks reserved so far (may exceed the buffer)
 };
 
 struct Runtime {
@@ -131,6 +132,14 @@ struct HashAggLaunch {
   bool hot_reserved;        // room for the heavy-hitter cells is part of the layout (EIGER_GLOBAL)
   size_t table_smem_bytes;  // shared-memory table of one CTA
   size_t queue_bytes;       // whole-input mode: per-warp miss queues behind the table (0 = misses go to the global table lane by lane)
+  // whole-input mode, EIGER_GLOBAL: the rows the front cannot hold are appended to a spill buffer (rebased 64-bit
+  // keys + raw 64-bit values, chunks of 2^spill_lg rows reserved per CTA; the tail of a CTA's last chunk is padded
+  // with the empty marker) instead of going to the global table row by row; they are partitioned and aggregated
+  // per partition afterwards.  spill_keys = nullptr: off.
+  uint64_t* spill_keys; uint64_t* spill_vals[kMaxVals]; uint64_t spill_cap_chunks; int spill_lg;
+  // partition mode over a spill buffer: rows whose key is the empty marker are padding; every item merges into the
+  // global table (its keys may also sit there, put by the fronts of the first pass)
+  int skip_empty, force_merge;
 };
 int launch_hash_agg(const HashAggLaunch& L, cudaStream_t s);
 size_t hash_agg_slot_bytes(const AggPlan& p, int key_kind);   // shared-memory bytes per slot

@@ -613,6 +613,7 @@ int launch_partition(PartitionLaunch& L, int sm_count, size_t smem_optin, cudaSt
     case KK_I64: return run_levels<KK_I64, KK_U64PRE>(L, sm_count, smem_optin, s);
     case KK_GEN: case KK_I8I8: return run_levels<KK_GEN, KK_U64PRE>(L, sm_count, smem_optin, s);
     case KK_GEN32: return run_levels<KK_GEN32, KK_U32PRE>(L, sm_count, smem_optin, s);
+    case KK_U64PRE: return run_levels<KK_U64PRE, KK_U64PRE>(L, sm_count, smem_optin, s);   // a spill buffer: keys already rebased and fused
     default: return EIGER_ERR_ARG;
   }
 }

@@ -296,6 +296,61 @@ def test_auto_routes_hot_keys_to_the_global_table():
     _auto_matches(ds, eiger.GLOBAL)
 
 
+@pytest.mark.parametrize("frac", [0.5, 0.001])
+def test_global_spill_buffer_partition_and_merge(monkeypatch, frac):
+    # EIGER_GLOBAL: the rows the front cannot hold go through the spill buffer, are partitioned and merged into
+    # the global table (frac 0.001: the buffer fills up and the rest of the misses take the global table)
+    set_tunable(monkeypatch, "EIGER_GLOBAL_SPILL", 1)             # off by default (measured slower on C3)
+    set_tunable(monkeypatch, "EIGER_SPILL_MIN_ROWS", 0)
+    set_tunable(monkeypatch, "EIGER_SPILL_FRAC", frac)
+    ds = datagen.config3(n=3_000_017, D=200_000)                 # fp64 SUM, COUNT, MIN, MAX; int64 keys
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.GLOBAL)
+    assert res.info["spill_rows"] > 0 and res.info["partition_levels"] == 1
+    if frac < 0.01:
+        assert res.info["spill_rows"] <= 0.001 * ds.n + 2048
+    assert_matches(res, want, d.aggs, d.vals)
+    res = _auto_matches(datagen.config3(n=SPEC_N, D=200_000), eiger.GLOBAL)      # EIGER_AUTO takes the same path
+    assert res.info["spill_rows"] > 0
+    # SUM + COUNT on int64 values, keys uniform (almost every row misses the front), ragged size
+    ds = datagen.config4(n=1_234_567, D=400_000)
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.GLOBAL)
+    assert res.info["spill_rows"] > 0
+    assert_matches(res, want, d.aggs, d.vals)
+    # the spill buffer is off for 32-bit keys and gives the same groups when switched off
+    set_tunable(monkeypatch, "EIGER_GLOBAL_SPILL", 0)
+    res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.GLOBAL)
+    assert res.info["spill_rows"] == 0
+    assert_matches(res, want, d.aggs, d.vals)
+
+
+def test_global_spill_two_partition_levels_and_generic_signature(small_partition_tables, monkeypatch):
+    set_tunable(monkeypatch, "EIGER_GLOBAL_SPILL", 1)
+    set_tunable(monkeypatch, "EIGER_SPILL_MIN_ROWS", 0)
+    ds = datagen.config4(n=6_000_011, D=5_000_000)
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.GLOBAL)
+    assert res.info["spill_rows"] > 0 and res.info["partition_levels"] == 2
+    assert_matches(res, want, d.aggs, d.vals)
+    # two int64 key columns (fused 64-bit key), three aggregates over two value columns (generic signature)
+    n = 2_000_003
+    i = torch.arange(n, dtype=torch.int64)
+    k0 = datagen.uniform_int(71, 0, i, -500, 499) * 1_000_003
+    k1 = datagen.uniform_int(71, 1, i, 0, 299)
+    v0 = datagen.uniform_int(71, 2, i, -1000, 1000)
+    v1 = datagen.unit_f64(71, 3, i)
+    ds = datagen.Dataset("two-key", n, [k0, k1], [v0, v1], [(eiger.MAX, 0), (eiger.SUM, 1), (eiger.MIN, 1)], exact_f64_sum=True)
+    want = oracle_result(ds)
+    d = to_dev(ds)
+    res = eiger.groupby(d.keys, d.vals, d.aggs, force=eiger.GLOBAL)
+    assert res.info["spill_rows"] > 0
+    assert_matches(res, want, d.aggs, d.vals)
+
+
 def test_partition_cuts_hot_partitions_into_items():
     # 2^24 rows over 2^7 partitions: the hot keys' partitions exceed twice the average and are cut
     # into several work items that merge through the global table
