@@ -96,6 +96,7 @@ struct Tunables {
   double fused_sketch_min_range;      // multi-column keys: sketch the fused key when the ranges multiply to more than this
   int part_full_table;                // EIGER_PARTITION reserves the full-size global table when partitions may be cut (round-1 behaviour)
   int split_max;                      // direct-index array split over up to this many CTAs (splitagg.cu); 0 = off
+  int slice_fused;                    // the slice-sketch pass also for several key columns (fused key)
   int miss_queue;                     // EIGER_GLOBAL queues the front's misses per warp (hashagg.cuh)
   int global_spill;                   // EIGER_GLOBAL: the front's misses go to a spill buffer that is partitioned and aggregated afterwards
   double spill_frac;                  // ... with room for this share of the rows (what does not fit takes the global table)
@@ -141,6 +142,7 @@ struct Tunables {
     dict = (int)env("EIGER_DICT", 1);
     pack_stride = (int)env("EIGER_PACK_STRIDE", 1);
     split_max = (int)env("EIGER_SPLIT_MAX", 4);        // measured (C5 dense, ms): C = 2 / 4 / 8 / 16 -> 1.26 / 1.86 / 3.11 / 5.15 against 2.8-3.3 for global RED
+    slice_fused = (int)env("EIGER_SLICE_FUSED", 1);
     miss_queue = (int)env("EIGER_MISS_QUEUE", 0);     // measured on C3: 5.25 ms with the queues (and a 32 KB smaller front) against 4.84 ms without
     global_spill = (int)env("EIGER_GLOBAL_SPILL", 0);  // measured on C3: 7.8 ms with the spill buffer against 5.5 ms without
     spill_frac = env("EIGER_SPILL_FRAC", 0.5);
@@ -547,7 +549,7 @@ int do_profile(Runtime* rt, const eiger_col* cols, int nk, int64_t n, int with_h
   {
     Timed t(s, 1);
     for (int k = 0; k < nk; ++k) {
-      int rc = samples > 0 ? launch_profile_sample(rt, cols[k].data, cols[k].dtype, n, samples, k, with_hll, k == 0, s)
+      int rc = samples > 0 ? launch_profile_sample(rt, cols[k].data, cols[k].dtype, n, samples, k, with_hll, k == 0, s, k == nk - 1)
                            : launch_profile(rt, cols[k].data, cols[k].dtype, n, k, with_hll, k == 0, s);
       if (rc) return rc;
     }
@@ -917,7 +919,11 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     rc = do_profile(rt, keys, nk, n, keys[0].dtype != EIGER_I8, local, s, T.spec_samples, &collision);
     if (rc) return rc;
     // uniform keys collide at rate 1 / NDV: "skewed" means well above that (and above the floor)
-    skewed = collision > T.skew_collision && collision * std::max(local[0].ndv_est, 1.0) > 4.0;
+    // (several key columns: `collision` compares whole sample rows, and the NDV beside it is the product of the
+    // columns' sample estimates, capped by the sample size)
+    double sample_ndv = 1.0;
+    for (int k = 0; k < nk; ++k) sample_ndv = std::min((double)T.spec_samples, sample_ndv * std::max(local[k].ndv_est, 1.0));
+    skewed = collision > T.skew_collision && collision * sample_ndv > 4.0;
     if (skewed && T.hot && nk == 1) {
       // which keys are the hot ones: the whole-input hash kernel reduces their rows inside the warp
       { Timed t(s, 1); rc = launch_hot_keys(rt, keys[0].data, keys[0].dtype, n, s); if (rc) return rc; }
@@ -1032,6 +1038,43 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       q.pre_hist = rt->prof->part_hist;
       if (chosen) *chosen = q.variant;
       return execute(q, &st2, 0, nullptr);
+    }
+  }
+  if (!stats_in && force == EIGER_AUTO && n >= T.spec_min_rows && T.slice && T.slice_fused && !skewed && nk >= 2 && n < (1ll << 32)) {
+    // Several key columns: the full profile costs one pass per column (min/max), one over all of them (sketch of
+    // the fused key) and the partitioner a third (level-1 histogram).  When the sample's ranges already send the
+    // query to PARTITION, ONE pass does all of it: the columns are fused with the sample's ranges - a value
+    // outside its column's range flags the pass, and the full profile below runs after all - the fused key's
+    // level-1 histogram is taken, and the fused keys of a sixteenth of the hash space are sketched (distinct
+    // sampling, as for one column).  The product of the per-column NDVs says little about the number of groups
+    // (5000 triples can span 2^61), so the selector runs again on the verified ranges and the slice estimate and
+    // may still pick another variant; the histogram is used when it stays with PARTITION.
+    QueryPlan qp;
+    if (plan_query(rt, keys, nk, n, vals, nv, aggs, na, local, EIGER_AUTO, &qp, skewed) == EIGER_OK && qp.variant == EIGER_PARTITION &&
+        (qp.key_kind == KK_GEN || qp.key_kind == KK_GEN32)) {
+      const uint32_t sel = kPreFan / 16;
+      { Timed t(s, 1);
+        rc = launch_fused_part_hist_hll(rt, qp.key, qp.key_kind, n, sel, s); if (rc) return rc;
+        rc = launch_hll_hist(rt, s); if (rc) return rc; }
+      struct PBack { long long mn[kMaxKeyCols], mx[kMaxKeyCols]; uint32_t hist[64]; uint32_t pair_eq, pair_n, oor, oor_pad; };
+      PBack* b = static_cast<PBack*>(rt->pinned);
+      EIGER_CUDA(cudaMemcpyAsync(b, rt->prof, sizeof(PBack), cudaMemcpyDeviceToHost, s));
+      EIGER_CUDA(cudaStreamSynchronize(s));
+      resolve_timing();
+      if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] fused slice sketch: out of range %u, slice ndv %.1f\n", b->oor, hll_estimate_from_hist(b->hist));
+      if (b->oor == 0u) {
+        eiger_stats st2[kMaxKeyCols];
+        for (int k = 0; k < nk; ++k) { st2[k] = local[k]; st2[k].ndv_est = 1.0; }
+        const double slice = hll_estimate_from_hist(b->hist);
+        const double est = slice * (double)kPreFan / (double)sel * (1.0 + 4.0 / std::sqrt(std::max(slice, 1.0)));
+        st2[0].ndv_est = std::max(256.0, std::min(est, (double)n));       // (an empty slice says "few", not "none")
+        QueryPlan q;
+        rc = plan_query(rt, keys, nk, n, vals, nv, aggs, na, st2, EIGER_AUTO, &q, skewed);
+        if (rc) return rc;
+        if (q.variant == EIGER_PARTITION && q.key_kind == qp.key_kind) q.pre_hist = rt->prof->part_hist;   // same ranges, same fusion, same hash
+        if (chosen) *chosen = q.variant;
+        return execute(q, st2, 0, nullptr);
+      }
     }
   }
   const eiger_stats* st = stats_in;

@@ -8,17 +8,20 @@
 
 namespace eiger {
 
+constexpr int kPairWords = 8192;     // 2^18 samples
 // Device block owned by the library (allocated once): profile outputs and call counters.
 struct ProfileDev {
   long long min[kMaxKeyCols];
   long long max[kMaxKeyCols];
   uint32_t hist[64];        // register-value histogram C[0 .. kHllQ + 1]
   uint32_t pair_eq, pair_n; // sample pass: adjacent sample keys that are equal / compared (skew test)
+  uint32_t oor, oor_pad;    // fused slice-sketch pass: some row had a key column outside the planned range
   uint32_t regs[kHllM];     // sketch registers, one per word (global atomicMax)
   uint32_t part_hist[kPreFan];   // rows per level-1 partition at fan-out kPreFan (slice-sketch pass)
   long long hot_key[kMaxHot];    // heavy hitters of a key sample (hot_keys pass), most frequent first
   uint32_t hot_cnt[kMaxHot];     // their sample counts
   uint32_t hot_n, hot_samples;
+  uint32_t pair_mask[kPairWords];   // sample pass over several key columns: neighbouring sample rows equal in every column so far
 };
 struct CallDev {
   unsigned long long n_groups;   // compaction claim counter
@@ -48,11 +51,14 @@ int cuda_fail(cudaError_t e, const char* what);   // records the message, return
 int launch_profile(Runtime* rt, const void* keys, int dtype, int64_t n, int which, int with_hll,
                    bool reset, cudaStream_t s);
 int launch_profile_sample(Runtime* rt, const void* keys, int dtype, int64_t n, int64_t samples, int which, int with_hll,
-                          bool reset, cudaStream_t s);
+                          bool reset, cudaStream_t s, bool last = true);   // last: the final column of a multi-column key (counts the equal neighbour rows)
 // Keys-only pass of EIGER_AUTO when the sample already settles PARTITION: exact min/max, the
 // partition histogram at fan-out kPreFan of u = key - base, and the sketch of the keys whose
 // partition id is below `sel` (a slice of the hash space: NDV = slice NDV * kPreFan / sel).
 int launch_part_hist_hll(Runtime* rt, const void* keys, int dtype, int64_t n, uint64_t base, uint32_t sel, cudaStream_t s);
+// The same for several key columns: histogram and slice sketch of the FUSED key (key.base / rng / mul / flags from
+// the sample's ranges; key_kind KK_GEN or KK_GEN32); rt->prof->oor != 0 afterwards: a row lay outside those ranges.
+int launch_fused_part_hist_hll(Runtime* rt, const KeyDesc& key, int key_kind, int64_t n, uint32_t sel, cudaStream_t s);
 // Heavy hitters of an evenly spaced key sample (single CTA): keys that own more than ~0.5 % of
 // the sample, at most kMaxHot, into rt->prof->hot_*.  EIGER_AUTO runs it when the sample's
 // collision rate says the keys are skewed; the whole-input hash kernel then reduces those keys'

@@ -19,7 +19,7 @@ __global__ void profile_reset_kernel(ProfileDev* out, int with_regs) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t < kMaxKeyCols) { out->min[t] = INT64_MAX; out->max[t] = INT64_MIN; }
   if (t < 64) out->hist[t] = 0;
-  if (t == 0) { out->pair_eq = 0; out->pair_n = 0; }
+  if (t == 0) { out->pair_eq = 0; out->pair_n = 0; out->oor = 0; }
   if (with_regs) for (int i = t; i < kHllM; i += gridDim.x * blockDim.x) out->regs[i] = 0;
   if (with_regs) for (int i = t; i < kPreFan; i += gridDim.x * blockDim.x) out->part_hist[i] = 0;
 }
@@ -250,7 +250,7 @@ part_hist_hll_kernel(const void* __restrict__ keys, int64_t n, uint64_t base, ui
 // range and the NDV; the speculative kernels check both exactly and give up if it did.
 __global__ void __launch_bounds__(256)
 profile_sample_kernel(const void* __restrict__ keys, int dtype, int64_t n, int64_t samples, ProfileDev* __restrict__ out,
-                      int which, int with_hll) {
+                      int which, int with_hll, int last) {
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   long long lo = INT64_MAX, hi = INT64_MIN;
   uint64_t x = 0;
@@ -276,7 +276,17 @@ profile_sample_kernel(const void* __restrict__ keys, int dtype, int64_t n, int64
   const uint64_t nb = __shfl_down_sync(0xffffffffu, x, 1);
   const bool cmp = (threadIdx.x & 31) < 31 && t + 1 < samples;
   const uint32_t eq = __ballot_sync(0xffffffffu, cmp && nb == x), nn = __ballot_sync(0xffffffffu, cmp);
-  if ((threadIdx.x & 31) == 0 && which == 0 && nn) { atomicAdd(&out->pair_eq, (uint32_t)__popc(eq)); atomicAdd(&out->pair_n, (uint32_t)__popc(nn)); }
+  // several key columns (one launch per column, in stream order): two neighbouring sample ROWS are equal when
+  // they agree in every column - each launch ANDs its column's verdicts into a bit mask, the last one counts
+  if ((threadIdx.x & 31) == 0 && nn) {
+    const int64_t w = t >> 5;
+    uint32_t all = eq;
+    if (w < kPairWords) {
+      if (which > 0) all &= out->pair_mask[w];
+      if (!last) out->pair_mask[w] = all;
+    } else if (which > 0 || !last) all = 0u;             // beyond the mask (more than 2^18 samples): a single column's pairs only
+    if (last && (w < kPairWords || which == 0)) { atomicAdd(&out->pair_eq, (uint32_t)__popc(all)); atomicAdd(&out->pair_n, (uint32_t)__popc(nn)); }
+  }
 }
 
 // Heavy hitters of 4096 evenly spaced keys: a shared-memory count table (8192 slots), then the
@@ -375,6 +385,70 @@ fused_hll_kernel(const __grid_constant__ KeyDesc k, int64_t n, ProfileDev* __res
   }
 }
 
+// The slice-sketch pass for SEVERAL key columns: one pass over the key columns fuses
+// them with the sample's ranges (rows.cuh; a value outside its column's range makes the fused key ~0, which
+// raises out->oor: the caller then falls back to the full profile), takes the level-1 partition histogram of
+// the fused key at fan-out kPreFan and sketches the fused keys of partitions [0, sel).
+template <int KK>
+__global__ void __launch_bounds__(kProfThreads)
+fused_part_hist_hll_kernel(const __grid_constant__ KeyDesc k, int64_t n, uint32_t sel, ProfileDev* __restrict__ out) {
+  using U = typename KeyTraits<KK>::U;
+  extern __shared__ uint32_t sregs[];   // kHllM sketch words, kPreFan counters, one 64-key queue per warp
+  uint32_t* s_hist = sregs + kHllM;
+  const int tid = threadIdx.x, lane = tid & 31;
+  uint64_t* wq = reinterpret_cast<uint64_t*>(s_hist + kPreFan) + (tid >> 5) * 64;
+  for (int i = tid; i < kHllM + kPreFan; i += kProfThreads) sregs[i] = 0;
+  __syncthreads();
+  constexpr int kShift = 8 * (int)sizeof(U) - kPreBits;
+  int cnt = 0;
+  bool bad = false;
+  auto one = [&](U u) {                  // all 32 lanes of the warp are here
+    bad = bad || u == empty_of<U>();
+    const uint32_t q = part_id<U>(u, kShift, kPreFan - 1);
+    atomicAdd(s_hist + q, 1u);
+    const bool in = q < sel;
+    const uint32_t m = __ballot_sync(0xffffffffu, in);
+    if (m) {
+      if (in) wq[cnt + __popc(m & ((1u << lane) - 1u))] = (uint64_t)u;
+      cnt += __popc(m);
+      if (cnt >= 32) {
+        __syncwarp();
+        cnt -= 32;
+        hll_update(sregs, wq[cnt + lane]);
+        __syncwarp();
+      }
+    }
+  };
+  auto one_tail = [&](U u) {             // any subset of lanes
+    bad = bad || u == empty_of<U>();
+    const uint32_t q = part_id<U>(u, kShift, kPreFan - 1);
+    atomicAdd(s_hist + q, 1u);
+    if (q < sel) hll_update(sregs, (uint64_t)u);
+  };
+  const int64_t pairs = n / 2, stride = (int64_t)gridDim.x * kProfThreads;
+  int64_t p = (int64_t)blockIdx.x * kProfThreads + tid;
+  // warp-uniform bound: the whole warp's last pair of the trip is inside the columns
+  for (; p - lane + 31 + 3 * stride < pairs; p += 4 * stride) {
+    U a[4][2];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) load_u2<KK>(k, 2 * (p + j * stride), a[j]);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { one(a[j][0]); one(a[j][1]); }
+  }
+  for (; p < pairs; p += stride) {
+    U a[2];
+    load_u2<KK>(k, 2 * p, a);
+    one_tail(a[0]); one_tail(a[1]);
+  }
+  if ((n & 1) && blockIdx.x == 0 && tid == 0) one_tail(load_u<KK>(k, n - 1));
+  __syncwarp();
+  if (lane < cnt) hll_update(sregs, wq[lane]);
+  if (bad) atomicOr(&out->oor, 1u);
+  __syncthreads();
+  for (int i = tid; i < kHllM; i += kProfThreads) { const uint32_t r = sregs[i]; if (r) atomicMax(&out->regs[i], r); }
+  for (int i = tid; i < kPreFan; i += kProfThreads) { const uint32_t c = s_hist[i]; if (c) atomicAdd(&out->part_hist[i], c); }
+}
+
 template <int DT>
 int launch_profile_dt(Runtime* rt, const void* keys, int64_t n, int which, int with_hll, cudaStream_t s) {
   const int64_t nvec = n / Elem<DT>::kPerVec;
@@ -424,6 +498,27 @@ int launch_fused_hll(Runtime* rt, const KeyDesc& key, int64_t n, cudaStream_t s)
   return EIGER_OK;
 }
 
+int launch_fused_part_hist_hll(Runtime* rt, const KeyDesc& key, int key_kind, int64_t n, uint32_t sel, cudaStream_t s) {
+  if (key_kind != KK_GEN && key_kind != KK_GEN32) return EIGER_ERR_ARG;
+  profile_reset_kernel<<<16, 1024, 0, s>>>(rt->prof, 1);
+  count_launch();
+  const int64_t want = (n / 2 + (int64_t)kProfThreads * 4 - 1) / ((int64_t)kProfThreads * 4);
+  const int blocks = (int)std::max<int64_t>(1, std::min<int64_t>(want, 2LL * rt->sm_count));
+  const int smem = (kHllM + kPreFan) * 4 + (kProfThreads / 32) * 64 * 8;
+  if (key_kind == KK_GEN32) {
+    auto kern = fused_part_hist_hll_kernel<KK_GEN32>;
+    EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    kern<<<blocks, kProfThreads, smem, s>>>(key, n, sel, rt->prof);
+  } else {
+    auto kern = fused_part_hist_hll_kernel<KK_GEN>;
+    EIGER_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    kern<<<blocks, kProfThreads, smem, s>>>(key, n, sel, rt->prof);
+  }
+  count_launch();
+  EIGER_CUDA(cudaGetLastError());
+  return EIGER_OK;
+}
+
 int launch_part_hist_hll(Runtime* rt, const void* keys, int dtype, int64_t n, uint64_t base, uint32_t sel, cudaStream_t s) {
   if (dtype != EIGER_I32 && dtype != EIGER_I64) return EIGER_ERR_ARG;
   profile_reset_kernel<<<16, 1024, 0, s>>>(rt->prof, 1);
@@ -448,13 +543,13 @@ int launch_part_hist_hll(Runtime* rt, const void* keys, int dtype, int64_t n, ui
 }
 
 int launch_profile_sample(Runtime* rt, const void* keys, int dtype, int64_t n, int64_t samples, int which, int with_hll,
-                          bool reset, cudaStream_t s) {
+                          bool reset, cudaStream_t s, bool last) {
   if (reset) {
     profile_reset_kernel<<<16, 1024, 0, s>>>(rt->prof, 1);
     count_launch();
   }
   if (n > 0 && samples > 0) {
-    profile_sample_kernel<<<(unsigned)((samples + 255) / 256), 256, 0, s>>>(keys, dtype, n, samples, rt->prof, which, with_hll);
+    profile_sample_kernel<<<(unsigned)((samples + 255) / 256), 256, 0, s>>>(keys, dtype, n, samples, rt->prof, which, with_hll, last ? 1 : 0);
     count_launch();
   }
   EIGER_CUDA(cudaGetLastError());

@@ -578,6 +578,41 @@ def test_multi_key_fused_sketch():
     assert [s.ndv_est for s in st] == [8.0, 8.0, 8.0]
 
 
+def test_multi_key_slice_sketch_single_profile_pass(monkeypatch):
+    # EIGER_AUTO, several key columns, enough groups for PARTITION: one pass fuses the columns with the sample's
+    # ranges, takes the level-1 histogram and sketches a slice of the fused keys
+    def sparse_mk(**kw):
+        ds = datagen.config_mk(n=SPEC_N, **kw)
+        ds.keys[0] = ds.keys[0] * 1000                                   # a fused domain too wide for a direct array
+        return ds
+    ds = sparse_mk(nk=4, digit_bits=5)                                    # 2^20 groups, fused domain below 2^32
+    res = _auto_matches(ds, eiger.PARTITION)
+    assert res.info["partition_prehist"] == 1 and res.info["partition_key_bytes"] == 4
+    assert abs(res.info["ndv_est"] / ds.ndv - 1.0) < 0.25                 # slice estimate incl. its head room
+    ds = datagen.config_mk(n=SPEC_N, nk=3, digit_bits=7, dtypes=[torch.int64, torch.int32, torch.int64])
+    ds.keys[0] = ds.keys[0] * 3_000_000_007                              # 64-bit fused keys
+    res = _auto_matches(ds, eiger.PARTITION)
+    assert res.info["partition_prehist"] == 1 and res.info["partition_key_bytes"] == 8
+    # a row outside the sample's ranges flags the pass: the full profile runs after all, same groups
+    ds = sparse_mk(nk=4, digit_bits=5)
+    ds.keys[2][SPEC_N // 3 + 1] = (1 << 20) + 5000                        # the column's values are 2^20 .. 2^20 + 31
+    res = _auto_matches(ds, eiger.PARTITION)
+    assert res.info["partition_prehist"] == 0
+    # few groups scattered over a large fused domain: the product of the columns' sample NDVs sends the sample's
+    # plan to PARTITION, the slice sketch of the fused key says 2000 and the selector takes the shared-memory table
+    g = torch.Generator().manual_seed(21)
+    ids = torch.randint(0, 2000, (SPEC_N,), generator=g, dtype=torch.int64)
+    cols = [(datagen.fmix64(ids) >> 44).to(torch.int32), datagen.fmix64(ids + 77) >> 34, (datagen.fmix64(ids + 999) >> 53).to(torch.int32)]
+    v = torch.randint(0, 1 << 31, (SPEC_N,), generator=g, dtype=torch.int64)
+    ds = datagen.Dataset("mk-sparse", SPEC_N, cols, [v], [(eiger.SUM, 0), (eiger.COUNT, 0)])
+    res = _auto_matches(ds, eiger.SMEM)
+    assert res.n_groups == 2000 and res.info["ndv_est"] < 6000
+    # switched off: the round-1 sequence of passes, same groups
+    set_tunable(monkeypatch, "EIGER_SLICE_FUSED", 0)
+    res = _auto_matches(sparse_mk(nk=4, digit_bits=5), eiger.PARTITION)
+    assert res.info["partition_prehist"] == 0
+
+
 @pytest.mark.parametrize("n", [0, 1, 3, 1025, 4097])
 def test_multi_key_tiny_and_ragged(n):
     g = torch.Generator().manual_seed(40 + n)
