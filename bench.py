@@ -348,12 +348,13 @@ def main(argv=None):
         dist.destroy_process_group()
 
 
-CURVE_POINTS = [f"C5:{lg}:{lay}" for lay in ("dense", "scattered") for lg in (4, 8, 12, 13, 14, 15, 16, 20, 24, 28)] + ["C3", "C4"]
+CURVE_POINTS = [f"C5:{lg}:{lay}" for lay in ("dense", "scattered") for lg in (4, 8, 12, 13, 14, 15, 16, 20, 24, 28)] + ["C3", "C4", "MK:4:2", "MK:4:6"]
 
 
 def ndv_curve(args, eiger, torch, dev, peak):
     """The metric is "rows/s and input GB/s vs NDV": EIGER_AUTO (statistics gathered inside the timed
-    call) at every C5 point (both layouts, 2^13..2^15 included), C3 and C4, each with the per-kernel
+    call) at every C5 point (both layouts, 2^13..2^15 included), C3, C4 and two multi-key points (4 x int32 key
+    columns, 2^8 and 2^24 groups), each with the per-kernel
     device times of a second, instrumented region.  --curve-forced adds the forced variants with the
     statistics supplied (profile excluded), the reading of "within 10 % of the best single variant"."""
     out = []
@@ -385,7 +386,7 @@ def ndv_curve(args, eiger, torch, dev, peak):
             if args.curve_forced:
                 st = eiger.profile_keys(ds.keys)
                 lg = (ds.ndv or 1).bit_length() - 1
-                dense = not ds.meta.get("scattered", False) and name.startswith("C5")
+                dense = (not ds.meta.get("scattered", False) and name.startswith("C5")) or (name.startswith("MK") and lg <= 20)
                 forced = {}
                 for vname, v in VARIANTS.items():
                     if v == 0 or (v == 1 and not dense) or (v == 2 and lg > 16) or (v == 3 and lg > 20):
