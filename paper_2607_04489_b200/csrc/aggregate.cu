@@ -407,7 +407,7 @@ int launch_fb(const AggLaunch& L, cudaStream_t s) {
 template <int KK>
 int launch_sig(const AggLaunch& L, cudaStream_t s) {
   switch (L.sig) {
-    case SIG_GENERIC: return launch_fb<KK, SIG_GENERIC>(L, s);
+    case SIG_GENERIC: case SIG_G1: return launch_fb<KK, SIG_GENERIC>(L, s);      // (SIG_G1 has its own kernels in hashagg.cuh only)
     case SIG_SC: return launch_fb<KK, SIG_SC>(L, s);
     case SIG_A4I: return launch_fb<KK, SIG_A4I>(L, s);
     case SIG_A4F: return launch_fb<KK, SIG_A4F>(L, s);

@@ -96,6 +96,7 @@ struct Tunables {
   double fused_sketch_min_range;      // multi-column keys: sketch the fused key when the ranges multiply to more than this
   int part_full_table;                // EIGER_PARTITION reserves the full-size global table when partitions may be cut (round-1 behaviour)
   int split_max;                      // direct-index array split over up to this many CTAs (splitagg.cu); 0 = off
+  int sig_g1;                         // plans of <= 4 accumulators over <= 1 value column take the light generic hash kernels (SIG_G1)
   int slice_fused;                    // the slice-sketch pass also for several key columns (fused key)
   int miss_queue;                     // EIGER_GLOBAL queues the front's misses per warp (hashagg.cuh)
   int global_spill;                   // EIGER_GLOBAL: the front's misses go to a spill buffer that is partitioned and aggregated afterwards
@@ -143,6 +144,7 @@ struct Tunables {
     pack_stride = (int)env("EIGER_PACK_STRIDE", 1);
     split_max = (int)env("EIGER_SPLIT_MAX", 4);        // measured (C5 dense, ms): C = 2 / 4 / 8 / 16 -> 1.26 / 1.86 / 3.11 / 5.15 against 2.8-3.3 for global RED
     slice_fused = (int)env("EIGER_SLICE_FUSED", 1);
+    sig_g1 = (int)env("EIGER_SIG_G1", 1);
     miss_queue = (int)env("EIGER_MISS_QUEUE", 0);     // measured on C3: 5.25 ms with the queues (and a 32 KB smaller front) against 4.84 ms without
     global_spill = (int)env("EIGER_GLOBAL_SPILL", 0);  // measured on C3: 7.8 ms with the spill buffer against 5.5 ms without
     spill_frac = env("EIGER_SPILL_FRAC", 0.5);
@@ -208,10 +210,11 @@ inline bool Sig_static_or_small(const AggPlan& p, int na) { const int sg = detec
 
 int detect_sig(const AggPlan& p, int n_user) {
   auto is = [&](int j, int op, int col, int f) { return p.op[j] == op && (op == EIGER_COUNT || (p.col[j] == col && p.f64[j] == f)); };
-  if (p.n_acc != n_user) return SIG_GENERIC;
+  const int fallback = (p.n_vals <= 1 && p.n_acc <= 4 && tun().sig_g1) ? SIG_G1 : SIG_GENERIC;
+  if (p.n_acc != n_user) return fallback;
   bool any32 = false;
   for (int c = 0; c < p.n_vals; ++c) any32 = any32 || p.vw[c] == 4;
-  if (any32) return (n_user == 2 && p.n_vals == 1 && is(0, EIGER_SUM, 0, 0) && is(1, EIGER_COUNT, 0, 0)) ? SIG_SC32 : SIG_GENERIC;
+  if (any32) return (n_user == 2 && p.n_vals == 1 && is(0, EIGER_SUM, 0, 0) && is(1, EIGER_COUNT, 0, 0)) ? SIG_SC32 : fallback;
   if (n_user == 2 && is(0, EIGER_SUM, 0, 0) && is(1, EIGER_COUNT, 0, 0)) return SIG_SC;
   if (n_user == 4 && is(1, EIGER_COUNT, 0, 0)) {
     if (is(0, EIGER_SUM, 0, 0) && is(2, EIGER_MIN, 0, 0) && is(3, EIGER_MAX, 0, 0)) return SIG_A4I;
@@ -219,7 +222,7 @@ int detect_sig(const AggPlan& p, int n_user) {
   }
   if (n_user == 5 && p.n_vals == 4 && is(0, EIGER_SUM, 0, 0) && is(1, EIGER_SUM, 1, 0) && is(2, EIGER_SUM, 2, 0) &&
       is(3, EIGER_SUM, 3, 0) && is(4, EIGER_COUNT, 0, 0)) return SIG_S4C;
-  return SIG_GENERIC;
+  return fallback;
 }
 
 // Step A4: choose the variant and size everything (readings R8-R10).

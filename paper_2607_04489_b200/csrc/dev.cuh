@@ -47,7 +47,9 @@ enum SigKind : int {
   SIG_A4I = 2,   // SUM, COUNT, MIN, MAX of int64 c0            (C1)
   SIG_A4F = 3,   // SUM, COUNT, MIN, MAX of fp64  c0            (C3)
   SIG_S4C = 4,   // SUM(int64 c0..c3), COUNT                    (C2)
-  SIG_SC32 = 5   // SUM(int32 c0), COUNT: the paper's 4-byte payloads
+  SIG_SC32 = 5,  // SUM(int32 c0), COUNT: the paper's 4-byte payloads
+  SIG_G1 = 6     // any plan of at most 4 accumulators over at most ONE value column, ops read from the plan at run time:
+                 // the generic path with 1 instead of 8 value registers per row in flight (hash kernels only)
 };
 
 struct AggPlan {
@@ -65,6 +67,14 @@ template <int SIG> struct Sig;
 template <> struct Sig<SIG_GENERIC> {
   static constexpr bool kStatic = false;
   static constexpr int kAcc = kMaxAcc, kVals = kMaxVals;
+  __device__ static constexpr int op(int) { return 0; }
+  __device__ static constexpr int col(int) { return 0; }
+  __device__ static constexpr bool f64(int) { return false; }
+  __device__ static constexpr int vwidth(int) { return 8; }
+};
+template <> struct Sig<SIG_G1> {
+  static constexpr bool kStatic = false;
+  static constexpr int kAcc = 4, kVals = 1;
   __device__ static constexpr int op(int) { return 0; }
   __device__ static constexpr int col(int) { return 0; }
   __device__ static constexpr bool f64(int) { return false; }

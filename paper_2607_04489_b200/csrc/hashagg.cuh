@@ -1079,6 +1079,7 @@ int launch_sig_bk(const HashAggLaunch& L, cudaStream_t s) {
     case SIG_A4F: return launch_one<KK, SIG_A4F, BK>(L, s);
     case SIG_S4C: return launch_one<KK, SIG_S4C, BK>(L, s);
     case SIG_SC32: return launch_one<KK, SIG_SC32, BK>(L, s);
+    case SIG_G1: return launch_one<KK, SIG_G1, BK>(L, s);
     default: return EIGER_ERR_ARG;
   }
 }
@@ -1090,6 +1091,7 @@ int launch_sig(const HashAggLaunch& L, cudaStream_t s) {
     if (L.bucket_keys == 2 && L.sig == SIG_SC) return launch_one<KK, SIG_SC, 2>(L, s);
     if (L.bucket_keys == 2 && L.sig == SIG_SC32) return launch_one<KK, SIG_SC32, 2>(L, s);
     if (L.bucket_keys == 2 && L.sig == SIG_GENERIC) return launch_one<KK, SIG_GENERIC, 2>(L, s);
+    if (L.bucket_keys == 2 && L.sig == SIG_G1) return launch_one<KK, SIG_G1, 2>(L, s);
   }
   return launch_sig_bk<KK, 16 / (int)sizeof(U)>(L, s);
 }

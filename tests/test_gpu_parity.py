@@ -214,6 +214,30 @@ def test_generic_signatures():
     run_all_variants(ds)
 
 
+@pytest.mark.parametrize("g1", [1, 0])
+def test_light_generic_signature_one_value_column(monkeypatch, g1):
+    # plans of at most 4 accumulators over one value column: SIG_G1 (hashagg.cuh) or, switched off, the full generic
+    # kernels - every hash variant, 32- and 64-bit keys, fp64 / int64 / int32 values, skewed and uniform keys
+    set_tunable(monkeypatch, "EIGER_SIG_G1", g1)
+    n = 700_003
+    i = torch.arange(n, dtype=torch.int64)
+    k32 = datagen.scatter64(3, datagen.uniform_int(31, 0, i, 0, 2999)).to(torch.int32)
+    vf = datagen.unit_f64(31, 1, i)                     # k 2^-53: the oracle sums it exactly
+    vneg = -vf - 1.0
+    vi = datagen.uniform_int(31, 2, i, -(1 << 30), (1 << 30) - 2) * 4099
+    v32 = datagen.uniform_int(31, 3, i, -(1 << 30), (1 << 30) - 2).to(torch.int32)
+    hash_variants = (eiger.AUTO, eiger.SMEM, eiger.GLOBAL, eiger.PARTITION, eiger.SORT)
+    for keys, vals, aggs in (
+            ([k32], [vf], [(eiger.SUM, 0), (eiger.COUNT, 0)]),
+            ([k32], [vneg], [(eiger.MAX, 0), (eiger.MIN, 0)]),
+            ([k32], [vi], [(eiger.COUNT, 0), (eiger.MAX, 0), (eiger.SUM, 0), (eiger.SUM, 0)]),
+            ([k32], [v32], [(eiger.MIN, 0), (eiger.SUM, 0)]),
+            ([datagen.config3(n=n, D=40_000).keys[0]], [vf], [(eiger.SUM, 0)]),          # int64 keys, Zipf: heavy hitters
+            ([datagen.config3(n=n, D=40_000).keys[0]], [vi], [(eiger.MIN, 0), (eiger.COUNT, 0), (eiger.SUM, 0)])):
+        ds = datagen.Dataset("g1", n, keys, vals, aggs, exact_f64_sum=True)
+        run_all_variants(ds, variants=hash_variants)
+
+
 def test_table_overflow_retry_and_errors():
     ds = to_dev(datagen.config5(n=1 << 20, ndv=1 << 16, scattered=True))
     want = oracle_result(ds)
