@@ -353,7 +353,7 @@ struct Front {
         if (!S::kStatic && j >= n_acc) break;
         const int op = sig_op<SIG>(a.plan, j); const bool f = sig_f64<SIG>(a.plan, j);
         uint64_t* c = cells + mine * NA + j;
-        if (op == EIGER_COUNT) { atomicAdd(reinterpret_cast<unsigned long long*>(c), 1ull); continue; }
+        if (op == EIGER_COUNT) continue;      // the warp's row counter below IS the count (a 64-bit add here is a CAS loop: 28 % of C3's wavefronts)
         const uint64_t part = row_partial(op, f, raw[sig_col<SIG>(a.plan, j)]);
         if (op == EIGER_SUM) atomic_merge(c, op, f, part);
         else {
@@ -383,7 +383,7 @@ struct Front {
       if (!dst) continue;
       for (int j = 0; j < n_acc; ++j) {
         const int op = sig_op<SIG>(a.plan, j); const bool f = sig_f64<SIG>(a.plan, j);
-        atomic_merge(dst + j, op, f, cells[(w * kMaxHot + hx) * NA + j]);
+        atomic_merge(dst + j, op, f, op == EIGER_COUNT ? (uint64_t)rows[w * kMaxHot + hx] : cells[(w * kMaxHot + hx) * NA + j]);
       }
     }
   }
