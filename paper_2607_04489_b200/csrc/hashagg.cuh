@@ -367,16 +367,18 @@ struct Front {
     (void)lane;
     return mine >= 0;
   }
-  __device__ void hot_init(uint64_t* cells, uint32_t* rows, int tid, int T) {
-    for (int i = tid; i < (T >> 5) * kMaxHot * NA; i += T) {
+  // hs = cell sets per warp (the lanes of a warp are spread over them: fewer lanes retry against each other in the
+  // compare-and-swap loops of the 64-bit adds)
+  __device__ void hot_init(uint64_t* cells, uint32_t* rows, int tid, int T, int hs = 1) {
+    for (int i = tid; i < (T >> 5) * hs * kMaxHot * NA; i += T) {
       const int j = i % NA;
       cells[i] = (S::kStatic || j < n_acc) ? acc_identity(sig_op<SIG>(a.plan, j)) : 0ull;
     }
-    for (int i = tid; i < (T >> 5) * kMaxHot; i += T) rows[i] = 0u;
+    for (int i = tid; i < (T >> 5) * hs * kMaxHot; i += T) rows[i] = 0u;
   }
   // every warp's hot cells into the global table
-  __device__ void hot_flush(const uint64_t* cells, const uint32_t* rows, int tid, int T) {
-    for (int i = tid; i < (T >> 5) * a.n_hot; i += T) {
+  __device__ void hot_flush(const uint64_t* cells, const uint32_t* rows, int tid, int T, int hs = 1) {
+    for (int i = tid; i < (T >> 5) * hs * a.n_hot; i += T) {
       const int w = i / a.n_hot, hx = i % a.n_hot;
       if (rows[w * kMaxHot + hx] == 0u) continue;
       uint64_t* dst = back_find_or_insert(a.table, a.cap, a.stride, a.hot[hx], a.call);
@@ -872,10 +874,13 @@ hash_agg_ldg_kernel(const __grid_constant__ HashAggArgs a) {
     constexpr int UNR = !Sig<SIG>::kStatic ? 1 : (NV >= 4 ? 1 : (sizeof(U) == 8 ? 1 : 2));   // 3 spills at the 64-register cap
     F f(a, smem, a.slots);
     if (a.queue_off && !a.spec) f.q_base = smem + a.queue_off + (size_t)(tid >> 5) * 64 * 8 * (1 + NV);
-    __shared__ uint64_t s_hot[(kMaxThreads / 32) * kMaxHot * F::NA];
-    __shared__ uint32_t s_hot_rows[(kMaxThreads / 32) * kMaxHot];
-    uint64_t* my_hot = s_hot + (tid >> 5) * kMaxHot * F::NA;
-    uint32_t* my_hot_rows = s_hot_rows + (tid >> 5) * kMaxHot;
+    // heavy-hitter cells: two sets per warp (lanes 0-15 / 16-31) while that fits next to the 200 KB table
+    constexpr int HS = F::NA <= 4 ? 2 : 1;
+    __shared__ uint64_t s_hot[(kMaxThreads / 32) * HS * kMaxHot * F::NA];
+    __shared__ uint32_t s_hot_rows[(kMaxThreads / 32) * HS * kMaxHot];
+    const int hot_unit = (tid >> 5) * HS + (HS == 2 ? ((tid >> 4) & 1) : 0);
+    uint64_t* my_hot = s_hot + hot_unit * kMaxHot * F::NA;
+    uint32_t* my_hot_rows = s_hot_rows + hot_unit * kMaxHot;
     __shared__ uint32_t s_sp_cursor;
     __shared__ uint32_t s_sp_base[sizeof(U) == 8 ? kSpillChunks : 1];
     if (tid == 0) { s_count = 0; s_abort = 0; s_sp_cursor = 0; }
@@ -884,7 +889,7 @@ hash_agg_ldg_kernel(const __grid_constant__ HashAggArgs a) {
       f.sp_cursor = &s_sp_cursor; f.sp_base = s_sp_base;
     }
     f.init(tid, T);
-    if (a.n_hot) f.hot_init(s_hot, s_hot_rows, tid, T);
+    if (a.n_hot) f.hot_init(s_hot, s_hot_rows, tid, T, HS);
     __syncthreads();
     const int64_t step = 2 * (int64_t)T, tile = step * UNR;
     const int64_t n_tiles = a.n / tile;
@@ -964,7 +969,7 @@ hash_agg_ldg_kernel(const __grid_constant__ HashAggArgs a) {
     }
     f.spill_pad(tid, T);
     f.flush_merge(tid, T);
-    if (a.n_hot) f.hot_flush(s_hot, s_hot_rows, tid, T);
+    if (a.n_hot) f.hot_flush(s_hot, s_hot_rows, tid, T, HS);
   } else {
     // ---- partition mode: work items blockIdx.x, + gridDim.x, ...; an item is a whole partition
     // (this CTA then owns its keys and emits them) or a slice of a hot one (merged through the
