@@ -61,7 +61,7 @@ class _Stats(ctypes.Structure):
 class _CallInfo(ctypes.Structure):
     _fields_ = [("variant", ctypes.c_int32), ("attempts", ctypes.c_int32), ("partition_levels", ctypes.c_int32),
                 ("partition_prehist", ctypes.c_int32), ("partition_key_bytes", ctypes.c_int32), ("sort_passes", ctypes.c_int32),
-                ("ndv_est", ctypes.c_double), ("kernel_launches", ctypes.c_int64), ("spill_rows", ctypes.c_int64)]
+                ("ndv_est", ctypes.c_double), ("kernel_launches", ctypes.c_int64), ("spill_rows", ctypes.c_int64), ("dict_ids", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
     def as_dict(self) -> dict:
         return {name: getattr(self, name) for name, _ in self._fields_}

@@ -31,9 +31,18 @@ struct AggArgs {
   CallDev* call;
   // FRONT_DICT: key -> dense id dictionary built from the key sample (image in global memory)
   const uint2* dict; uint32_t dict_slots, dict_shift;
+  // dict_compact: the large dictionary (up to ~8300 keys; SUM + COUNT plans only).  Shared memory then holds
+  // [SUM planes: 8 x slots][COUNT plane: 4 x slots][dictionary keys: 4 x dict_slots][dictionary ids: 2 x dict_slots],
+  // one replica - 12 instead of 16 bytes per id and 6 instead of 8 per dictionary entry, which is what lets 2^13
+  // keys fit one CTA
+  uint32_t dict_compact;
 };
 
 constexpr uint32_t kDictMul = 0x9E3779B1u;
+// kernel-side front kind of the large dictionary (AggArgs::dict_compact): its own instantiation, so that the small
+// dictionary's kernel carries none of its branches (they cost 3-4 % at 2^8 / 2^12 keys when tested at run time)
+constexpr int FRONT_DICTC = 100;
+template <int FRONT> constexpr bool kIsDict = (FRONT == FRONT_DICT || FRONT == FRONT_DICTC);
 
 template <int KK, int SIG, int FRONT>
 struct AggCtx {
@@ -54,17 +63,30 @@ struct AggCtx {
     const uint32_t rep = args.front_replicas > 1 ? (threadIdx.x >> 5) % args.front_replicas : 0u;
     rep_base = sm + (size_t)rep * args.front_slots * 8 * (uint32_t)n_acc;
     sdict = reinterpret_cast<const uint2*>(sm + (size_t)args.front_replicas * args.front_slots * 8 * (uint32_t)n_acc);
+    skey = reinterpret_cast<const uint32_t*>(sm + (size_t)args.front_slots * 12);
+    sid = reinterpret_cast<const uint16_t*>(skey + args.dict_slots);
   }
+  const uint32_t* skey;          // FRONT_DICT, dict_compact: dictionary keys, then 16-bit ids
+  const uint16_t* sid;
 
   // dense id of rebased key u, ~0u when the dictionary does not hold it (empty entries carry id ~0u)
   __device__ __forceinline__ uint32_t dict_id(uint32_t u) const {
     uint32_t h = (u * kDictMul) >> a.dict_shift, id = ~0u;
     bool done = false;
-    while (!done) {
-      const uint2 e = sdict[h];
-      if (e.x == u) { id = e.y; done = true; }
-      else if (e.x == kEmpty32) done = true;
-      else h = (h + 1u) & (a.dict_slots - 1u);
+    if constexpr (FRONT == FRONT_DICTC) {
+      while (!done) {
+        const uint32_t k = skey[h];
+        if (k == u) { id = sid[h]; done = true; }
+        else if (k == kEmpty32) done = true;
+        else h = (h + 1u) & (a.dict_slots - 1u);
+      }
+    } else {
+      while (!done) {
+        const uint2 e = sdict[h];
+        if (e.x == u) { id = e.y; done = true; }
+        else if (e.x == kEmpty32) done = true;
+        else h = (h + 1u) & (a.dict_slots - 1u);
+      }
     }
     return id;
   }
@@ -75,13 +97,21 @@ struct AggCtx {
       uint64_t* acc = reinterpret_cast<uint64_t*>(smem);
       for (uint32_t c = 0; c < a.front_slots * (uint32_t)n_acc; ++c)
         acc[(size_t)c * T + tid] = acc_identity(sig_op<SIG>(a.plan, (int)(c % (uint32_t)n_acc)));
-    } else if constexpr (FRONT == FRONT_SDIRECT || FRONT == FRONT_DICT) {
+    } else if constexpr (FRONT == FRONT_SDIRECT || kIsDict<FRONT>) {
+      constexpr bool compact = FRONT == FRONT_DICTC;
+      if constexpr (compact) {
+        uint32_t* w = reinterpret_cast<uint32_t*>(smem);
+        for (uint32_t i = tid; i < 3u * a.front_slots; i += T) w[i] = 0u;        // SUM low, SUM high, COUNT
+        uint32_t* k = const_cast<uint32_t*>(skey); uint16_t* d = const_cast<uint16_t*>(sid);
+        for (uint32_t i = tid; i < a.dict_slots; i += T) { const uint2 e = a.dict[i]; k[i] = e.x; d[i] = (uint16_t)e.y; }
+      } else {
       for (uint32_t rep = 0; rep < a.front_replicas; ++rep)
         for (int j = 0; j < n_acc; ++j)
           smem_init_plane(smem + (size_t)rep * a.front_slots * 8 * (uint32_t)n_acc, a.front_slots, j, sig_op<SIG>(a.plan, j), sig_f64<SIG>(a.plan, j), tid, T);
-      if constexpr (FRONT == FRONT_DICT) {
+      if constexpr (kIsDict<FRONT>) {
         uint2* d = const_cast<uint2*>(sdict);
         for (uint32_t i = tid; i < a.dict_slots; i += T) d[i] = a.dict[i];
+      }
       }
     }
     if constexpr (FRONT != FRONT_NONE) __syncthreads();
@@ -98,14 +128,14 @@ struct AggCtx {
   }
 
   __device__ __forceinline__ void row(U u, const uint64_t (&raw)[NV]) {
-    if constexpr (FRONT == FRONT_DICT) {
+    if constexpr (kIsDict<FRONT>) {
       // the dictionary names the keys of the sample: a key it does not hold discards the pass
       const uint32_t id = dict_id((uint32_t)u);
       if (id >= a.front_slots) { if (*reinterpret_cast<volatile uint32_t*>(&a.call->abort) == 0u) atomicOr(&a.call->abort, 1u); return; }
       u = (U)id;
     }
     // speculative run planned from a sample: the range is checked exactly here
-    if (FRONT != FRONT_DICT && a.spec && (uint64_t)u >= a.cap) { if (*reinterpret_cast<volatile uint32_t*>(&a.call->abort) == 0u) atomicOr(&a.call->abort, 1u); return; }
+    if (!kIsDict<FRONT> && a.spec && (uint64_t)u >= a.cap) { if (*reinterpret_cast<volatile uint32_t*>(&a.call->abort) == 0u) atomicOr(&a.call->abort, 1u); return; }
     if constexpr (FRONT == FRONT_PRIV) {
       uint64_t* acc = reinterpret_cast<uint64_t*>(smem) + (size_t)u * (uint32_t)n_acc * blockDim.x + threadIdx.x;
 #pragma unroll
@@ -115,7 +145,7 @@ struct AggCtx {
         uint64_t* c = acc + (size_t)j * blockDim.x;
         *c = combine(op, f, *c, row_partial(op, f, raw[sig_col<SIG>(a.plan, j)]));
       }
-    } else if constexpr (FRONT == FRONT_SDIRECT || FRONT == FRONT_DICT) {
+    } else if constexpr (FRONT == FRONT_SDIRECT || kIsDict<FRONT>) {
       unsigned char* base = rep_base;
 #pragma unroll
       for (int j = 0; j < NA; ++j) {
@@ -133,11 +163,11 @@ struct AggCtx {
   // (ncu: short_scoreboard was 28 % of the stall samples with one row at a time)
   template <int R>
   __device__ __forceinline__ void rows_sc(const U (&uk)[R], const uint64_t (&raw)[R][NV]) {
-    static_assert((SIG == SIG_SC || SIG == SIG_SC32) && (FRONT == FRONT_SDIRECT || FRONT == FRONT_DICT), "SUM + COUNT signature only");
+    static_assert((SIG == SIG_SC || SIG == SIG_SC32) && (FRONT == FRONT_SDIRECT || kIsDict<FRONT>), "SUM + COUNT signature only");
     uint32_t* lo = reinterpret_cast<uint32_t*>(rep_base);
     uint32_t* cnt = reinterpret_cast<uint32_t*>(rep_base + (size_t)8 * a.front_slots);
     U u[R];
-    if constexpr (FRONT == FRONT_DICT) {
+    if constexpr (kIsDict<FRONT>) {
       // all look-ups first (R independent shared-memory loads in flight), then the misses are settled
       bool bad = false;
 #pragma unroll
@@ -147,7 +177,7 @@ struct AggCtx {
 #pragma unroll
       for (int r = 0; r < R; ++r) u[r] = uk[r];
     }
-    if (FRONT != FRONT_DICT && a.spec) {
+    if (!kIsDict<FRONT> && a.spec) {
       // speculative run planned from a sample: one key outside the planned range discards the whole
       // pass anyway, so the trip is skipped as a whole (one branch per R rows, not one per atomic)
       bool bad = false;
@@ -192,14 +222,17 @@ struct AggCtx {
         for (int o = 16; o > 0; o >>= 1) v = combine(op, f, v, __shfl_xor_sync(0xffffffffu, v, o));
         if (lane == 0) back_merge(c / (uint32_t)n_acc, j, v, static_cast<uint64_t*>(a.table) + (uint64_t)(c / (uint32_t)n_acc) * (uint32_t)n_acc);
       }
-    } else if constexpr (FRONT == FRONT_SDIRECT || FRONT == FRONT_DICT) {
+    } else if constexpr (FRONT == FRONT_SDIRECT || kIsDict<FRONT>) {
       // the CTA's replicas are combined first: one global atomic per cell and CTA (with 8 replicas of
       // a 256-slot table the flush of ~900 CTAs otherwise queues millions of atomics on 512 addresses)
       const uint32_t per = a.front_slots * (uint32_t)n_acc;
       for (uint32_t w = tid; w < per; w += T) {
         const uint32_t j = w / a.front_slots, u = w % a.front_slots;
         const int op = sig_op<SIG>(a.plan, (int)j); const bool f = sig_f64<SIG>(a.plan, (int)j);
-        uint64_t v = smem_read(smem, a.front_slots, (int)j, u, op, f);
+        uint64_t v;
+        const bool compact_count = FRONT == FRONT_DICTC && op == EIGER_COUNT;
+        if (compact_count) v = reinterpret_cast<const uint32_t*>(smem + (size_t)8 * a.front_slots)[u];    // 4-byte COUNT plane
+        else v = smem_read(smem, a.front_slots, (int)j, u, op, f);
         for (uint32_t rep = 1; rep < a.front_replicas; ++rep)
           v = combine(op, f, v, smem_read(smem + (size_t)rep * a.front_slots * 8 * (uint32_t)n_acc, a.front_slots, (int)j, u, op, f));
         back_merge(u, (int)j, v, static_cast<uint64_t*>(a.table) + (uint64_t)u * (uint32_t)n_acc);
@@ -246,7 +279,7 @@ aggregate_kernel(const __grid_constant__ AggArgs a) {
         global_val2(a.plan, c, sig_vw<SIG>(a.plan, c), r0 + s * kStep, raw[s][0][c], raw[s][1][c]);
       }
     }
-    if constexpr ((SIG == SIG_SC || SIG == SIG_SC32) && (FRONT == FRONT_SDIRECT || FRONT == FRONT_DICT)) {
+    if constexpr ((SIG == SIG_SC || SIG == SIG_SC32) && (FRONT == FRONT_SDIRECT || kIsDict<FRONT>)) {
       U uu[2 * UNR]; uint64_t rr[2 * UNR][NV];
 #pragma unroll
       for (int s = 0; s < UNR; ++s) { uu[2 * s] = u[s][0]; uu[2 * s + 1] = u[s][1]; rr[2 * s][0] = raw[s][0][0]; rr[2 * s + 1][0] = raw[s][1][0]; }
@@ -383,6 +416,7 @@ int launch_one(const AggLaunch& L, cudaStream_t s) {
   a.front_slots = L.front_slots; a.front_limit = L.front_limit; a.front_replicas = L.front_replicas; a.spec = L.spec;
   a.stride = L.stride; a.table = L.table; a.cap = L.cap; a.call = L.call;
   a.dict = static_cast<const uint2*>(L.dict); a.dict_slots = L.dict_slots; a.dict_shift = L.dict_shift;
+  a.dict_compact = L.dict_compact;
   kern<<<L.blocks, THREADS, L.smem_bytes, s>>>(a);
   count_launch();
   EIGER_CUDA(cudaGetLastError());
@@ -398,6 +432,10 @@ int launch_fb(const AggLaunch& L, cudaStream_t s) {
     case FRONT_SDIRECT: return L.threads == kAggThreadsWide ? launch_one<KK, SIG, FRONT_SDIRECT, kAggThreadsWide>(L, s)
                                                             : launch_one<KK, SIG, FRONT_SDIRECT>(L, s);
     case FRONT_DICT:
+      if constexpr (sizeof(typename KeyTraits<KK>::U) == 4 && (SIG == SIG_SC || SIG == SIG_SC32)) {
+        if (L.dict_compact) return launch_one<KK, SIG, FRONT_DICTC, kAggThreadsWide>(L, s);
+      }
+      if (L.dict_compact) return EIGER_ERR_ARG;
       if constexpr (sizeof(typename KeyTraits<KK>::U) == 4) return launch_one<KK, SIG, FRONT_DICT, kAggThreadsWide>(L, s);
       else return EIGER_ERR_ARG;
     default: return EIGER_ERR_ARG;

@@ -108,6 +108,7 @@ struct Tunables {
   int pack_stride;                    // global hash table slots of 40 / 48 bytes are not padded to 64
   int dict;                           // EIGER_AUTO: scattered keys the sample names completely get a dictionary + direct array (FRONT_DICT)
   double dict_max_keys;               // ... while the sample holds at most this many distinct keys
+  double dict_big_max_keys;           // ... or, for SUM + COUNT plans, this many in the compact layout (dictionary from 4x the sample); 0 = off
   Tunables() {
     auto env = [](const char* k, double dflt) { const char* v = std::getenv(k); return v ? std::atof(v) : dflt; };
     priv_smem = (size_t)env("EIGER_PRIV_KB", 96) << 10;
@@ -153,6 +154,7 @@ struct Tunables {
     split_hash = (int)env("EIGER_SPLIT_HASH", 0);      // the hash flavour loses everywhere (scattered 2^13 / 2^14: 3.1 / 6.4 ms against 2.7 / 3.4)
     split_bytes = (size_t)env("EIGER_SPLIT_KB", 192) << 10;
     part_full_table = (int)env("EIGER_PART_FULL_TABLE", 0);
+    dict_big_max_keys = env("EIGER_DICT_BIG_MAX_KEYS", 8300);
     dict_max_keys = env("EIGER_DICT_MAX_KEYS", 4600);   // measured: scattered 2^12 keys 0.90 ms through the dictionary, 1.25 ms through the hash table
   }
 };
@@ -191,6 +193,7 @@ struct QueryPlan {
   const uint32_t* pre_hist = nullptr;   // PARTITION: level-1 histogram taken with key.base at fan-out kPreFan
   int sort_bits = 0, sort_passes = 0;   // SORT: significant bits of the rebased fused key, 8-bit passes
   uint32_t dict_slots = 0, dict_shift = 0;   // FRONT_DICT: dictionary image entries (power of two)
+  uint32_t dict_compact = 0;                 // FRONT_DICT: the large-dictionary layout (SUM + COUNT plans, up to ~8300 keys)
   int split_lg = 0;                          // FRONT_SPLIT: log2 of the CTAs that share the array
   // GLOBAL with a spill buffer: capacity in rows (0 = none; a multiple of the chunk), chunk = 2^spill_lg rows, and
   // the plan of the partition + per-partition aggregation that follows
@@ -514,7 +517,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
 // the id - the batched accumulate of FRONT_SDIRECT instead of the hash table's find-or-insert.
 // Only for rebased keys of 32 bits; false when the shape does not fit.
 bool make_dict_plan(QueryPlan* q, const eiger_col* keys, int nk, int na, double sample_ndv, const Tunables& T) {
-  if (!T.dict || sample_ndv > T.dict_max_keys) return false;
+  if (!T.dict || sample_ndv > std::max(T.dict_max_keys, T.dict_big_max_keys)) return false;
   int kk;
   if (nk == 1 && keys[0].dtype == EIGER_I32) kk = KK_I32;
   else if (q->key.flags & kKey32) kk = KK_GEN32;
@@ -525,6 +528,23 @@ bool make_dict_plan(QueryPlan* q, const eiger_col* keys, int nk, int na, double 
   if (!has_count) { if (na >= kMaxAcc) return false; p.op[na] = EIGER_COUNT; p.cnt_acc = na; p.n_acc = na + 1; }
   // ids: an eighth more than the sample shows (keys the sample missed abort the pass anyway)
   const uint32_t cap = (uint32_t)(((size_t)(1.125 * sample_ndv) + 64 + 63) / 64 * 64);
+  if (sample_ndv > T.dict_max_keys) {
+    // the large dictionary: 12 bytes per id (SUM 8 + COUNT 4), 6 per dictionary entry (key 4 + id 2), one replica,
+    // 16384 entries (load <= 0.57): 2^13 scattered keys in one CTA's shared memory.  SUM + COUNT plans only.
+    const int sg = detect_sig(p, na);
+    const uint32_t slots = 16384;
+    if ((sg != SIG_SC && sg != SIG_SC32) || p.n_acc != 2 || cap > 65535u || 10 * (size_t)cap > 6 * (size_t)slots ||
+        (size_t)cap * 12 + (size_t)slots * 6 > (220u << 10)) return false;
+    q->back = BACK_DIRECT; q->front = FRONT_DICT; q->key_kind = kk;
+    q->front_slots = cap; q->front_replicas = 1; q->cap = cap; q->stride = 8u * p.n_acc;
+    q->dict_slots = slots; q->dict_shift = 32 - 14; q->dict_compact = 1;
+    q->smem_bytes = (size_t)cap * 12 + (size_t)slots * 6;
+    q->sig = sg;
+    q->table_bytes = align_up((size_t)cap * q->stride, 256);
+    q->part_bytes = align_up((size_t)slots * 8, 256) + align_up((size_t)cap * 4, 256) + 256;
+    q->total_bytes = q->table_bytes + q->part_bytes + 256;
+    return aggregate_supported(kk, q->sig, FRONT_DICT, BACK_DIRECT);
+  }
   const size_t cell = (size_t)cap * 8 * p.n_acc;
   if (cell > (96u << 10)) return false;
   uint32_t slots = 4096;
@@ -678,6 +698,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
   const int checked = stats_in != nullptr;
   auto execute = [&](QueryPlan& q, const eiger_stats* st, int spec, bool* aborted) -> int {
   if (!have_room(q.total_bytes) || !workspace) return EIGER_ERR_WORKSPACE;
+  info->dict_ids = q.front == FRONT_DICT ? (int32_t)q.front_slots : 0;
   info->variant = q.variant; info->ndv_est = q.ndv; info->sort_passes = q.variant == EIGER_SORT ? q.sort_passes : 0;
   const int src_kind = q.key_kind;
   for (int attempt = 0;; ++attempt) {
@@ -721,9 +742,10 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       // workspace after the table: dictionary image, id -> key, id counter
       auto take = [&](size_t bytes) { char* r = pws; pws += align_up(bytes, 256); return r; };
       L.dict = take((size_t)q.dict_slots * 8); L.dict_slots = q.dict_slots; L.dict_shift = q.dict_shift;
+      L.dict_compact = q.dict_compact;
       dict_keys = reinterpret_cast<uint32_t*>(take((size_t)q.cap * 4));
       uint32_t* dict_n = reinterpret_cast<uint32_t*>(take(256));
-      { Timed t(s, 1); rc = launch_dict_build(L, std::min<int64_t>(n, tun().spec_samples), dict_keys, dict_n, s); if (rc) return rc; }
+      { Timed t(s, 1); rc = launch_dict_build(L, std::min<int64_t>(n, tun().spec_samples * (q.dict_compact ? 4 : 1)), dict_keys, dict_n, s); if (rc) return rc; }
     }
     if (q.variant == EIGER_DIRECT || q.front == FRONT_DICT) {
       // persistent grid: as many CTAs as fit, never more than there are tiles

@@ -92,6 +92,7 @@ struct AggLaunch {
   CallDev* call;
   // FRONT_DICT: dictionary image (key, dense id) of dict_slots entries (a power of two), slot = (u * mul) >> dict_shift
   void* dict; uint32_t dict_slots, dict_shift;
+  uint32_t dict_compact;    // FRONT_DICT: the large-dictionary shared-memory layout (aggregate.cu: AggArgs)
   // launch shape
   int threads, blocks;
   size_t smem_bytes;

@@ -287,6 +287,26 @@ def test_auto_speculative_pass(lg, scattered, variant):
     _auto_matches(datagen.config5(n=SPEC_N, ndv=1 << lg, scattered=scattered), variant)
 
 
+@pytest.mark.parametrize("ndv", [5000, 7000, 8192])
+def test_auto_large_dictionary_front(monkeypatch, ndv):
+    # scattered keys beyond the small dictionary (4600) and up to 2^13: the compact dictionary layout (12 bytes per id,
+    # 6 per entry, dictionary built from four times the sample); SUM + COUNT plans only
+    ds = datagen.config5(n=SPEC_N, ndv=ndv, scattered=True)
+    res = _auto_matches(ds, eiger.SMEM)
+    assert res.info["dict_ids"] >= ndv and res.info["attempts"] == 1
+    # a key that occurs once is not in the dictionary: the pass is discarded and the hash table takes over
+    ds.keys[0][SPEC_N // 2 + 5] = 123456789
+    res = _auto_matches(ds)
+    assert res.n_groups == ndv + 1 and res.info["dict_ids"] == 0
+    # other plans keep the hash table
+    ds4 = datagen.Dataset("a4", ds.n, ds.keys, ds.vals, [(eiger.SUM, 0), (eiger.COUNT, 0), (eiger.MIN, 0), (eiger.MAX, 0)])
+    res = _auto_matches(ds4)
+    assert res.info["dict_ids"] == 0
+    set_tunable(monkeypatch, "EIGER_DICT_BIG_MAX_KEYS", 0)
+    res = _auto_matches(datagen.config5(n=SPEC_N, ndv=ndv, scattered=True))
+    assert res.info["dict_ids"] == 0
+
+
 def test_auto_speculation_gives_up_on_an_outlier():
     # 16 dense groups and ONE row far outside the range the sample sees: the speculative direct pass
     # must notice, discard its result and fall back to the full profile; the answer stays exact
