@@ -36,13 +36,21 @@ struct AggArgs {
   // one replica - 12 instead of 16 bytes per id and 6 instead of 8 per dictionary entry, which is what lets 2^13
   // keys fit one CTA
   uint32_t dict_compact;
+  // several passes over the input, each with the dictionary of ONE slice of the keys (slice = the dict_pass_lg hash bits
+  // below the slot bits): rows of other slices are skipped.  dict_pass_lg = 0: a single pass owns every key.
+  uint32_t dict_pass_lg, dict_pass;
 };
 
 constexpr uint32_t kDictMul = 0x9E3779B1u;
 // kernel-side front kind of the large dictionary (AggArgs::dict_compact): its own instantiation, so that the small
 // dictionary's kernel carries none of its branches (they cost 3-4 % at 2^8 / 2^12 keys when tested at run time)
 constexpr int FRONT_DICTC = 100;
-template <int FRONT> constexpr bool kIsDict = (FRONT == FRONT_DICT || FRONT == FRONT_DICTC);
+constexpr int FRONT_DICTP = 101;        // the large dictionary, one of several passes (rows of other key slices are skipped)
+template <int FRONT> constexpr bool kIsDict = (FRONT == FRONT_DICT || FRONT == FRONT_DICTC || FRONT == FRONT_DICTP);
+template <int FRONT> constexpr bool kIsCompact = (FRONT == FRONT_DICTC || FRONT == FRONT_DICTP);
+__host__ __device__ __forceinline__ uint32_t dict_slice(uint32_t u, uint32_t shift, uint32_t lg) {
+  return ((u * kDictMul) >> (shift - lg)) & ((1u << lg) - 1u);
+}
 
 template <int KK, int SIG, int FRONT>
 struct AggCtx {
@@ -73,7 +81,7 @@ struct AggCtx {
   __device__ __forceinline__ uint32_t dict_id(uint32_t u) const {
     uint32_t h = (u * kDictMul) >> a.dict_shift, id = ~0u;
     bool done = false;
-    if constexpr (FRONT == FRONT_DICTC) {
+    if constexpr (kIsCompact<FRONT>) {
       while (!done) {
         const uint32_t k = skey[h];
         if (k == u) { id = sid[h]; done = true; }
@@ -98,7 +106,7 @@ struct AggCtx {
       for (uint32_t c = 0; c < a.front_slots * (uint32_t)n_acc; ++c)
         acc[(size_t)c * T + tid] = acc_identity(sig_op<SIG>(a.plan, (int)(c % (uint32_t)n_acc)));
     } else if constexpr (FRONT == FRONT_SDIRECT || kIsDict<FRONT>) {
-      constexpr bool compact = FRONT == FRONT_DICTC;
+      constexpr bool compact = kIsCompact<FRONT>;
       if constexpr (compact) {
         uint32_t* w = reinterpret_cast<uint32_t*>(smem);
         for (uint32_t i = tid; i < 3u * a.front_slots; i += T) w[i] = 0u;        // SUM low, SUM high, COUNT
@@ -128,6 +136,7 @@ struct AggCtx {
   }
 
   __device__ __forceinline__ void row(U u, const uint64_t (&raw)[NV]) {
+    if constexpr (FRONT == FRONT_DICTP) { if (dict_slice((uint32_t)u, a.dict_shift, a.dict_pass_lg) != a.dict_pass) return; }
     if constexpr (kIsDict<FRONT>) {
       // the dictionary names the keys of the sample: a key it does not hold discards the pass
       const uint32_t id = dict_id((uint32_t)u);
@@ -170,6 +179,28 @@ struct AggCtx {
     if constexpr (kIsDict<FRONT>) {
       // all look-ups first (R independent shared-memory loads in flight), then the misses are settled
       bool bad = false;
+      if constexpr (FRONT == FRONT_DICTP) {
+        // rows of the other slices are left out one by one (a predicate per row, no early exit: most trips hold both kinds)
+        bool own[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) own[r] = dict_slice((uint32_t)uk[r], a.dict_shift, a.dict_pass_lg) == a.dict_pass;
+#pragma unroll
+        for (int r = 0; r < R; ++r) { u[r] = own[r] ? (U)dict_id((uint32_t)uk[r]) : (U)0; bad = bad || (uint32_t)u[r] >= a.front_slots; }
+        if (bad) { if (*reinterpret_cast<volatile uint32_t*>(&a.call->abort) == 0u) atomicOr(&a.call->abort, 1u); return; }
+        uint32_t old[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) if (own[r]) old[r] = atomicAdd(lo + (uint32_t)u[r], (uint32_t)raw[r][0]);
+#pragma unroll
+        for (int r = 0; r < R; ++r) if (own[r]) atomicAdd(cnt + (uint32_t)u[r], 1u);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          if (!own[r]) continue;
+          const uint32_t vl = (uint32_t)raw[r][0];
+          const uint32_t h = (uint32_t)(raw[r][0] >> 32) + ((uint32_t)(old[r] + vl) < vl ? 1u : 0u);
+          if (h) atomicAdd(lo + a.front_slots + (uint32_t)u[r], h);
+        }
+        return;
+      }
 #pragma unroll
       for (int r = 0; r < R; ++r) { u[r] = (U)dict_id((uint32_t)uk[r]); bad = bad || (uint32_t)u[r] >= a.front_slots; }
       if (bad) { if (*reinterpret_cast<volatile uint32_t*>(&a.call->abort) == 0u) atomicOr(&a.call->abort, 1u); return; }
@@ -230,7 +261,7 @@ struct AggCtx {
         const uint32_t j = w / a.front_slots, u = w % a.front_slots;
         const int op = sig_op<SIG>(a.plan, (int)j); const bool f = sig_f64<SIG>(a.plan, (int)j);
         uint64_t v;
-        const bool compact_count = FRONT == FRONT_DICTC && op == EIGER_COUNT;
+        const bool compact_count = kIsCompact<FRONT> && op == EIGER_COUNT;
         if (compact_count) v = reinterpret_cast<const uint32_t*>(smem + (size_t)8 * a.front_slots)[u];    // 4-byte COUNT plane
         else v = smem_read(smem, a.front_slots, (int)j, u, op, f);
         for (uint32_t rep = 1; rep < a.front_replicas; ++rep)
@@ -308,7 +339,7 @@ aggregate_kernel(const __grid_constant__ AggArgs a) {
 // indexes a direct array with the code.  id >= cap (more keys than planned): the pass gives up.
 __global__ void __launch_bounds__(256)
 dict_build_kernel(const __grid_constant__ KeyDesc key, int64_t n, int64_t samples, uint2* __restrict__ img, uint32_t slots, uint32_t shift,
-                  uint32_t cap, uint32_t* __restrict__ dict_keys, uint32_t* __restrict__ dict_n, CallDev* call) {
+                  uint32_t cap, uint32_t* __restrict__ dict_keys, uint32_t* __restrict__ dict_n, CallDev* call, uint32_t pass_lg) {
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= samples) return;
   const int64_t i = (int64_t)(((unsigned __int128)t * (unsigned __int128)n) / (unsigned __int128)samples);
@@ -316,6 +347,9 @@ dict_build_kernel(const __grid_constant__ KeyDesc key, int64_t n, int64_t sample
   if (u64 >= 0xFFFFFFFFull) return;                           // outside the planned ranges: the aggregation pass will notice
   const uint32_t u = (uint32_t)u64;
   uint32_t h = (u * kDictMul) >> shift;
+  // several passes: slice p of the keys has its own image, its own ids 0 .. cap - 1 and its own part of dict_keys
+  const uint32_t p = pass_lg ? dict_slice(u, shift, pass_lg) : 0u;
+  img += (size_t)p * slots; dict_keys += (size_t)p * cap; dict_n += p;
   uint32_t* w = reinterpret_cast<uint32_t*>(img);
   for (uint32_t probes = 0; probes < slots; ++probes) {
     const uint32_t old = atomicCAS(w + 2 * (size_t)h, kEmpty32, u);
@@ -416,7 +450,7 @@ int launch_one(const AggLaunch& L, cudaStream_t s) {
   a.front_slots = L.front_slots; a.front_limit = L.front_limit; a.front_replicas = L.front_replicas; a.spec = L.spec;
   a.stride = L.stride; a.table = L.table; a.cap = L.cap; a.call = L.call;
   a.dict = static_cast<const uint2*>(L.dict); a.dict_slots = L.dict_slots; a.dict_shift = L.dict_shift;
-  a.dict_compact = L.dict_compact;
+  a.dict_compact = L.dict_compact; a.dict_pass_lg = L.dict_pass_lg; a.dict_pass = L.dict_pass;
   kern<<<L.blocks, THREADS, L.smem_bytes, s>>>(a);
   count_launch();
   EIGER_CUDA(cudaGetLastError());
@@ -433,6 +467,7 @@ int launch_fb(const AggLaunch& L, cudaStream_t s) {
                                                             : launch_one<KK, SIG, FRONT_SDIRECT>(L, s);
     case FRONT_DICT:
       if constexpr (sizeof(typename KeyTraits<KK>::U) == 4 && (SIG == SIG_SC || SIG == SIG_SC32)) {
+        if (L.dict_compact && L.dict_pass_lg > 0) return launch_one<KK, SIG, FRONT_DICTP, kAggThreadsWide>(L, s);
         if (L.dict_compact) return launch_one<KK, SIG, FRONT_DICTC, kAggThreadsWide>(L, s);
       }
       if (L.dict_compact) return EIGER_ERR_ARG;
@@ -476,12 +511,13 @@ int launch_aggregate(const AggLaunch& L, cudaStream_t s) {
 }
 
 int launch_dict_build(const AggLaunch& L, int64_t samples, uint32_t* dict_keys, uint32_t* dict_n, cudaStream_t s) {
-  EIGER_CUDA(cudaMemsetAsync(L.dict, 0xFF, (size_t)L.dict_slots * 8, s));
-  EIGER_CUDA(cudaMemsetAsync(dict_n, 0, 4, s));
+  // (L.dict_pass_lg > 0: 2^dict_pass_lg images / id ranges / counters, one per key slice)
+  EIGER_CUDA(cudaMemsetAsync(L.dict, 0xFF, ((size_t)L.dict_slots * 8) << L.dict_pass_lg, s));
+  EIGER_CUDA(cudaMemsetAsync(dict_n, 0, (size_t)4 << L.dict_pass_lg, s));
   KeyDesc k = L.key;
   k.flags &= ~kKey32;      // 64-bit fusion here (one thread per sampled row: speed is irrelevant), the marker stays ~0ull
   dict_build_kernel<<<(unsigned)((samples + 255) / 256), 256, 0, s>>>(k, L.n, samples, static_cast<uint2*>(L.dict), L.dict_slots, L.dict_shift,
-                                                                       L.front_slots, dict_keys, dict_n, L.call);
+                                                                       L.front_slots, dict_keys, dict_n, L.call, L.dict_pass_lg);
   count_launch();
   EIGER_CUDA(cudaGetLastError());
   return EIGER_OK;

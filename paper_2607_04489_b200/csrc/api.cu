@@ -108,6 +108,7 @@ struct Tunables {
   int pack_stride;                    // global hash table slots of 40 / 48 bytes are not padded to 64
   int dict;                           // EIGER_AUTO: scattered keys the sample names completely get a dictionary + direct array (FRONT_DICT)
   double dict_max_keys;               // ... while the sample holds at most this many distinct keys
+  int dict_max_pass_lg;               // ... or 2^this many times that, in as many passes over the input (one key slice each)
   double dict_big_max_keys;           // ... or, for SUM + COUNT plans, this many in the compact layout (dictionary from 4x the sample); 0 = off
   Tunables() {
     auto env = [](const char* k, double dflt) { const char* v = std::getenv(k); return v ? std::atof(v) : dflt; };
@@ -154,7 +155,8 @@ struct Tunables {
     split_hash = (int)env("EIGER_SPLIT_HASH", 0);      // the hash flavour loses everywhere (scattered 2^13 / 2^14: 3.1 / 6.4 ms against 2.7 / 3.4)
     split_bytes = (size_t)env("EIGER_SPLIT_KB", 192) << 10;
     part_full_table = (int)env("EIGER_PART_FULL_TABLE", 0);
-    dict_big_max_keys = env("EIGER_DICT_BIG_MAX_KEYS", 8300);
+    dict_big_max_keys = env("EIGER_DICT_BIG_MAX_KEYS", 8600);
+    dict_max_pass_lg = (int)env("EIGER_DICT_MAX_PASS_LG", 1);   // measured (C5 scattered, ms per call): 2 passes at 2^14 keys 2.78 against 3.54 partitioned; 4 passes at 2^15 4.52 against 3.47
     dict_max_keys = env("EIGER_DICT_MAX_KEYS", 4600);   // measured: scattered 2^12 keys 0.90 ms through the dictionary, 1.25 ms through the hash table
   }
 };
@@ -194,6 +196,7 @@ struct QueryPlan {
   int sort_bits = 0, sort_passes = 0;   // SORT: significant bits of the rebased fused key, 8-bit passes
   uint32_t dict_slots = 0, dict_shift = 0;   // FRONT_DICT: dictionary image entries (power of two)
   uint32_t dict_compact = 0;                 // FRONT_DICT: the large-dictionary layout (SUM + COUNT plans, up to ~8300 keys)
+  uint32_t dict_pass_lg = 0;                 // FRONT_DICT: 2^dict_pass_lg passes, each with the dictionary of one slice of the keys
   int split_lg = 0;                          // FRONT_SPLIT: log2 of the CTAs that share the array
   // GLOBAL with a spill buffer: capacity in rows (0 = none; a multiple of the chunk), chunk = 2^spill_lg rows, and
   // the plan of the partition + per-partition aggregation that follows
@@ -517,7 +520,7 @@ int plan_query(const Runtime* rt, const eiger_col* keys, int nk, int64_t n, cons
 // the id - the batched accumulate of FRONT_SDIRECT instead of the hash table's find-or-insert.
 // Only for rebased keys of 32 bits; false when the shape does not fit.
 bool make_dict_plan(QueryPlan* q, const eiger_col* keys, int nk, int na, double sample_ndv, const Tunables& T) {
-  if (!T.dict || sample_ndv > std::max(T.dict_max_keys, T.dict_big_max_keys)) return false;
+  if (!T.dict || sample_ndv > std::max(T.dict_max_keys, T.dict_big_max_keys * (double)(1 << std::max(0, T.dict_max_pass_lg)))) return false;
   int kk;
   if (nk == 1 && keys[0].dtype == EIGER_I32) kk = KK_I32;
   else if (q->key.flags & kKey32) kk = KK_GEN32;
@@ -527,21 +530,32 @@ bool make_dict_plan(QueryPlan* q, const eiger_col* keys, int nk, int na, double 
   for (int j = 0; j < na; ++j) has_count = has_count || p.op[j] == EIGER_COUNT;
   if (!has_count) { if (na >= kMaxAcc) return false; p.op[na] = EIGER_COUNT; p.cnt_acc = na; p.n_acc = na + 1; }
   // ids: an eighth more than the sample shows (keys the sample missed abort the pass anyway)
-  const uint32_t cap = (uint32_t)(((size_t)(1.125 * sample_ndv) + 64 + 63) / 64 * 64);
+  // more keys than one large dictionary holds: 2 or 4 passes, each with the dictionary of one hash slice of the keys
+  int pass_lg = 0;
+  if (sample_ndv > T.dict_max_keys) {
+    if (T.dict_big_max_keys <= 0) return false;
+    while (pass_lg < T.dict_max_pass_lg && sample_ndv > T.dict_big_max_keys * (double)(1 << pass_lg)) ++pass_lg;
+    if (sample_ndv > T.dict_big_max_keys * (double)(1 << pass_lg)) return false;
+  }
+  // ids (per pass): an eighth more than the estimate, and four standard deviations of a slice's share on top
+  const double per_pass = sample_ndv / (double)(1 << pass_lg);
+  const uint32_t cap = (uint32_t)(((size_t)(1.125 * per_pass + (pass_lg ? 4.0 * std::sqrt(per_pass) : 0.0)) + 64 + 63) / 64 * 64);
   if (sample_ndv > T.dict_max_keys) {
     // the large dictionary: 12 bytes per id (SUM 8 + COUNT 4), 6 per dictionary entry (key 4 + id 2), one replica,
     // 16384 entries (load <= 0.57): 2^13 scattered keys in one CTA's shared memory.  SUM + COUNT plans only.
     const int sg = detect_sig(p, na);
     const uint32_t slots = 16384;
-    if ((sg != SIG_SC && sg != SIG_SC32) || p.n_acc != 2 || cap > 65535u || 10 * (size_t)cap > 6 * (size_t)slots ||
+    if ((sg != SIG_SC && sg != SIG_SC32) || p.n_acc != 2 || cap > 65535u || 100 * (size_t)cap > 63 * (size_t)slots ||
         (size_t)cap * 12 + (size_t)slots * 6 > (220u << 10)) return false;
     q->back = BACK_DIRECT; q->front = FRONT_DICT; q->key_kind = kk;
-    q->front_slots = cap; q->front_replicas = 1; q->cap = cap; q->stride = 8u * p.n_acc;
-    q->dict_slots = slots; q->dict_shift = 32 - 14; q->dict_compact = 1;
+    const size_t P = (size_t)1 << pass_lg;
+    q->front_slots = cap; q->front_replicas = 1; q->cap = (uint64_t)cap * P; q->stride = 8u * p.n_acc;
+    q->dict_slots = slots; q->dict_shift = 32 - 14; q->dict_compact = 1; q->dict_pass_lg = (uint32_t)pass_lg;
     q->smem_bytes = (size_t)cap * 12 + (size_t)slots * 6;
     q->sig = sg;
-    q->table_bytes = align_up((size_t)cap * q->stride, 256);
-    q->part_bytes = align_up((size_t)slots * 8, 256) + align_up((size_t)cap * 4, 256) + 256;
+    q->variant = EIGER_SMEM;                 // (the sample's plan may have said PARTITION: the dictionary passes replace it)
+    q->table_bytes = align_up((size_t)q->cap * q->stride, 256);
+    q->part_bytes = align_up(P * slots * 8, 256) + align_up((size_t)q->cap * 4, 256) + 256;
     q->total_bytes = q->table_bytes + q->part_bytes + 256;
     return aggregate_supported(kk, q->sig, FRONT_DICT, BACK_DIRECT);
   }
@@ -741,11 +755,13 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     if (q.front == FRONT_DICT) {
       // workspace after the table: dictionary image, id -> key, id counter
       auto take = [&](size_t bytes) { char* r = pws; pws += align_up(bytes, 256); return r; };
-      L.dict = take((size_t)q.dict_slots * 8); L.dict_slots = q.dict_slots; L.dict_shift = q.dict_shift;
-      L.dict_compact = q.dict_compact;
+      L.dict = take(((size_t)q.dict_slots * 8) << q.dict_pass_lg); L.dict_slots = q.dict_slots; L.dict_shift = q.dict_shift;
+      L.dict_compact = q.dict_compact; L.dict_pass_lg = q.dict_pass_lg;
       dict_keys = reinterpret_cast<uint32_t*>(take((size_t)q.cap * 4));
       uint32_t* dict_n = reinterpret_cast<uint32_t*>(take(256));
-      { Timed t(s, 1); rc = launch_dict_build(L, std::min<int64_t>(n, tun().spec_samples * (q.dict_compact ? 4 : 1)), dict_keys, dict_n, s); if (rc) return rc; }
+      // the large dictionaries are built from 4x the sample per pass (every key must be in it: 32 samples per key)
+      const int64_t build_rows = std::min<int64_t>(n, tun().spec_samples * (q.dict_compact ? ((int64_t)4 << q.dict_pass_lg) : 1));
+      { Timed t(s, 1); rc = launch_dict_build(L, build_rows, dict_keys, dict_n, s); if (rc) return rc; }
     }
     if (q.variant == EIGER_DIRECT || q.front == FRONT_DICT) {
       // persistent grid: as many CTAs as fit, never more than there are tiles
@@ -767,6 +783,16 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
         const int64_t want = std::min<int64_t>(rt->sm_count / C, (n + 4095) / 4096);
         SL.blocks = (int)std::max<int64_t>(1, want) * C;
         { Timed t(s, 0); rc = launch_split_direct(SL, s); if (rc) return rc; }
+      } else if (q.front == FRONT_DICT && q.dict_pass_lg > 0) {
+        // one pass per key slice: its dictionary image, its part of the id table
+        const char* img0 = static_cast<const char*>(L.dict);
+        for (uint32_t pi = 0; pi < (1u << q.dict_pass_lg); ++pi) {
+          AggLaunch Lp = L;
+          Lp.dict = const_cast<char*>(img0) + (size_t)pi * q.dict_slots * 8;
+          Lp.table = static_cast<char*>(table) + (size_t)pi * q.front_slots * q.stride;
+          Lp.cap = q.front_slots; Lp.dict_pass = pi;
+          { Timed t(s, 0); rc = launch_aggregate(Lp, s); if (rc) return rc; }
+        }
       } else
       { Timed t(s, 0); rc = launch_aggregate(L, s); if (rc) return rc; }
     } else {
@@ -981,8 +1007,20 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       double sndv = local[0].ndv_est;
       for (int k = 1; k < nk; ++k) sndv *= local[k].ndv_est;
       sndv = std::min(sndv, (double)T.spec_samples);
+      // a single column whose sample is far from having seen every key twice: what that many distinct keys among s
+      // samples mean for UNIFORM keys (the inversion also used below); the large dictionaries are built from a larger
+      // sample, and a key they still lack only costs the discarded pass
+      if (nk == 1 && sndv > T.dict_max_keys) {
+        const double smp = (double)std::min<int64_t>(n, T.spec_samples), r = std::min(sndv / smp, 0.98);
+        if (r > 0.05) {
+          double lo = 0.02, hi = 50.0;
+          for (int it = 0; it < 60; ++it) { const double x = 0.5 * (lo + hi); if ((1.0 - std::exp(-x)) / x > r) lo = x; else hi = x; }
+          sndv = std::max(sndv, smp / (0.5 * (lo + hi)));
+        }
+      }
       if (T.spec && T.dict && !skewed && plan_query(rt, keys, nk, n, vals, nv, aggs, na, local, EIGER_AUTO, &qd, skewed) == EIGER_OK &&
-          qd.variant == EIGER_SMEM && make_dict_plan(&qd, keys, nk, na, sndv, T) && have_room(qd.total_bytes)) {
+          (qd.variant == EIGER_SMEM || (qd.variant == EIGER_PARTITION && nk == 1 && sndv > T.dict_max_keys)) &&
+          make_dict_plan(&qd, keys, nk, na, sndv, T) && have_room(qd.total_bytes)) {
         bool aborted = false;
         rc = execute(qd, local, 1, &aborted);
         if (std::getenv("EIGER_DEBUG")) std::fprintf(stderr, "[eiger] dictionary pass (%u ids, %u dictionary slots, %u replicas): rc %d aborted %d\n", qd.front_slots, qd.dict_slots, qd.front_replicas, rc, (int)aborted);

@@ -287,6 +287,20 @@ def test_auto_speculative_pass(lg, scattered, variant):
     _auto_matches(datagen.config5(n=SPEC_N, ndv=1 << lg, scattered=scattered), variant)
 
 
+@pytest.mark.parametrize("ndv,passes", [(12000, 2), (1 << 14, 2)])
+def test_auto_dictionary_passes(monkeypatch, ndv, passes):
+    # more scattered keys than one large dictionary holds: two passes, each with the dictionary of one hash slice
+    ds = datagen.config5(n=SPEC_N, ndv=ndv, scattered=True)
+    res = _auto_matches(ds, eiger.SMEM)
+    assert res.info["dict_ids"] * passes >= ndv and res.info["dict_ids"] <= 10112 and res.info["attempts"] == 1
+    ds.keys[0][SPEC_N // 2 + 5] = 123456789                 # a key no dictionary holds: discarded, partition takes over
+    res = _auto_matches(ds, eiger.PARTITION)
+    assert res.n_groups == ndv + 1
+    set_tunable(monkeypatch, "EIGER_DICT_MAX_PASS_LG", 0)
+    res = _auto_matches(datagen.config5(n=SPEC_N, ndv=ndv, scattered=True), eiger.PARTITION)
+    assert res.info["dict_ids"] == 0
+
+
 @pytest.mark.parametrize("ndv", [5000, 7000, 8192])
 def test_auto_large_dictionary_front(monkeypatch, ndv):
     # scattered keys beyond the small dictionary (4600) and up to 2^13: the compact dictionary layout (12 bytes per id,
@@ -453,7 +467,7 @@ def test_two_level_partition(small_partition_tables):
 
 
 # ---- EIGER_AUTO sizes PARTITION from a hash-space slice sketch ---------
-@pytest.mark.parametrize("cfg,lg", [("c5", 14), ("c5", 18), ("c5", 22), ("c4", 21)])
+@pytest.mark.parametrize("cfg,lg", [("c5", 15), ("c5", 18), ("c5", 22), ("c4", 21)])      # (2^14 int32 keys now take two dictionary passes)
 def test_auto_slice_sketch(cfg, lg):
     # the sample settles PARTITION; one keys-only pass gives the level-1 histogram, exact min/max
     # and the NDV from the sketch of a slice of the partitions.  The estimate is checked against
