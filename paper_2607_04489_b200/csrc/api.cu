@@ -752,6 +752,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     { Timed t(s, 3); rc = launch_table_init(L, s); if (rc) return rc; }
 
     uint32_t* dict_keys = nullptr;
+    uint32_t* dict_counts = nullptr;
     if (q.front == FRONT_DICT) {
       // workspace after the table: dictionary image, id -> key, id counter
       auto take = [&](size_t bytes) { char* r = pws; pws += align_up(bytes, 256); return r; };
@@ -759,6 +760,7 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       L.dict_compact = q.dict_compact; L.dict_pass_lg = q.dict_pass_lg;
       dict_keys = reinterpret_cast<uint32_t*>(take((size_t)q.cap * 4));
       uint32_t* dict_n = reinterpret_cast<uint32_t*>(take(256));
+      dict_counts = dict_n;
       // the large dictionaries are built from 4x the sample per pass (every key must be in it: 32 samples per key)
       const int64_t build_rows = std::min<int64_t>(n, tun().spec_samples * (q.dict_compact ? ((int64_t)4 << q.dict_pass_lg) : 1));
       { Timed t(s, 1); rc = launch_dict_build(L, build_rows, dict_keys, dict_n, s); if (rc) return rc; }
@@ -924,6 +926,12 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
     EIGER_CUDA(cudaMemcpyAsync(hb, rt->call, sizeof(Back), cudaMemcpyDeviceToHost, s));
     EIGER_CUDA(cudaStreamSynchronize(s));
     resolve_timing();
+    if (dict_counts && std::getenv("EIGER_DEBUG")) {
+      uint32_t dn[4] = {0, 0, 0, 0};
+      cudaMemcpy(dn, dict_counts, sizeof(uint32_t) << q.dict_pass_lg, cudaMemcpyDeviceToHost);
+      std::fprintf(stderr, "[eiger] dictionary: abort %u overflow %u groups %llu, ids per slice %u %u %u %u of %u\n", hb->abort, hb->overflow,
+                   (unsigned long long)hb->n_groups, dn[0], dn[1], dn[2], dn[3], q.front_slots);
+    }
     if (spec && (hb->abort || hb->overflow)) { *aborted = true; return EIGER_OK; }
     if (hb->abort) return EIGER_ERR_STATS;
     if (hb->overflow) {
