@@ -46,7 +46,8 @@ constexpr uint32_t kDictMul = 0x9E3779B1u;
 // dictionary's kernel carries none of its branches (they cost 3-4 % at 2^8 / 2^12 keys when tested at run time)
 constexpr int FRONT_DICTC = 100;
 constexpr int FRONT_DICTP = 101;        // the large dictionary, one of several passes (rows of other key slices are skipped)
-template <int FRONT> constexpr bool kIsDict = (FRONT == FRONT_DICT || FRONT == FRONT_DICTC || FRONT == FRONT_DICTP);
+constexpr int FRONT_DICTG = 102;        // the small dictionary searched two entries at a time (one replica, thousands of keys)
+template <int FRONT> constexpr bool kIsDict = (FRONT == FRONT_DICT || FRONT == FRONT_DICTC || FRONT == FRONT_DICTP || FRONT == FRONT_DICTG);
 template <int FRONT> constexpr bool kIsCompact = (FRONT == FRONT_DICTC || FRONT == FRONT_DICTP);
 __host__ __device__ __forceinline__ uint32_t dict_slice(uint32_t u, uint32_t shift, uint32_t lg) {
   return ((u * kDictMul) >> (shift - lg)) & ((1u << lg) - 1u);
@@ -92,6 +93,17 @@ struct AggCtx {
         if (pos >= 0) { id = sid[h + (uint32_t)pos]; done = true; }
         else if (k.x == kEmpty32 || k.y == kEmpty32 || k.z == kEmpty32 || k.w == kEmpty32) done = true;
         else h = (h + 4u) & (a.dict_slots - 1u);
+      }
+    } else if constexpr (FRONT == FRONT_DICTG) {
+      // (key, id) entries, two per LDS.128: pays from a few thousand keys (2^12: aggregate 0.78 -> 0.72 ms), costs at
+      // 2^4 / 2^8 keys (0.48 -> 0.57, 0.55 -> 0.65 ms), where the one-entry loop below almost never iterates
+      h &= ~1u;
+      while (!done) {
+        const uint4 e = *reinterpret_cast<const uint4*>(sdict + h);
+        if (e.x == u) { id = e.y; done = true; }
+        else if (e.z == u) { id = e.w; done = true; }
+        else if (e.x == kEmpty32 || e.z == kEmpty32) done = true;
+        else h = (h + 2u) & (a.dict_slots - 1u);
       }
     } else {
       while (!done) {
@@ -474,6 +486,7 @@ int launch_fb(const AggLaunch& L, cudaStream_t s) {
       if constexpr (sizeof(typename KeyTraits<KK>::U) == 4 && (SIG == SIG_SC || SIG == SIG_SC32)) {
         if (L.dict_compact && L.dict_pass_lg > 0) return launch_one<KK, SIG, FRONT_DICTP, kAggThreadsWide>(L, s);
         if (L.dict_compact) return launch_one<KK, SIG, FRONT_DICTC, kAggThreadsWide>(L, s);
+        if (L.dict_group == 2) return launch_one<KK, SIG, FRONT_DICTG, kAggThreadsWide>(L, s);
       }
       if (L.dict_compact) return EIGER_ERR_ARG;
       if constexpr (sizeof(typename KeyTraits<KK>::U) == 4) return launch_one<KK, SIG, FRONT_DICT, kAggThreadsWide>(L, s);
@@ -522,7 +535,7 @@ int launch_dict_build(const AggLaunch& L, int64_t samples, uint32_t* dict_keys, 
   KeyDesc k = L.key;
   k.flags &= ~kKey32;      // 64-bit fusion here (one thread per sampled row: speed is irrelevant), the marker stays ~0ull
   dict_build_kernel<<<(unsigned)((samples + 255) / 256), 256, 0, s>>>(k, L.n, samples, static_cast<uint2*>(L.dict), L.dict_slots, L.dict_shift,
-                                                                       L.front_slots, dict_keys, dict_n, L.call, L.dict_pass_lg, L.dict_compact ? 4u : 1u);
+                                                                       L.front_slots, dict_keys, dict_n, L.call, L.dict_pass_lg, L.dict_compact ? 4u : (L.dict_group == 2 ? 2u : 1u));
   count_launch();
   EIGER_CUDA(cudaGetLastError());
   return EIGER_OK;

@@ -108,6 +108,7 @@ struct Tunables {
   int pack_stride;                    // global hash table slots of 40 / 48 bytes are not padded to 64
   int dict;                           // EIGER_AUTO: scattered keys the sample names completely get a dictionary + direct array (FRONT_DICT)
   double dict_max_keys;               // ... while the sample holds at most this many distinct keys
+  int dict_pairs;                     // small dictionaries with one replica are searched two entries at a time
   int dict_max_pass_lg;               // ... or 2^this many times that, in as many passes over the input (one key slice each)
   double dict_big_max_keys;           // ... or, for SUM + COUNT plans, this many in the compact layout (dictionary from 4x the sample); 0 = off
   Tunables() {
@@ -156,6 +157,7 @@ struct Tunables {
     split_bytes = (size_t)env("EIGER_SPLIT_KB", 192) << 10;
     part_full_table = (int)env("EIGER_PART_FULL_TABLE", 0);
     dict_big_max_keys = env("EIGER_DICT_BIG_MAX_KEYS", 8600);
+    dict_pairs = (int)env("EIGER_DICT_PAIRS", 1);
     dict_max_pass_lg = (int)env("EIGER_DICT_MAX_PASS_LG", 1);   // measured (C5 scattered, ms per call): 2 passes at 2^14 keys 2.78 against 3.54 partitioned; 4 passes at 2^15 4.52 against 3.47
     dict_max_keys = env("EIGER_DICT_MAX_KEYS", 4600);   // measured: scattered 2^12 keys 0.90 ms through the dictionary, 1.25 ms through the hash table
   }
@@ -758,6 +760,10 @@ int run_groupby(Runtime* rt, const eiger_col* keys, int nk, int64_t n, const eig
       auto take = [&](size_t bytes) { char* r = pws; pws += align_up(bytes, 256); return r; };
       L.dict = take(((size_t)q.dict_slots * 8) << q.dict_pass_lg); L.dict_slots = q.dict_slots; L.dict_shift = q.dict_shift;
       L.dict_compact = q.dict_compact; L.dict_pass_lg = q.dict_pass_lg;
+      // small dictionaries at a load of 0.25 and more are placed and searched in pairs of entries (measured, 2^28 rows: 4096
+      // keys 0.78 -> 0.72 ms; at 2048 keys / load 0.14 the pairs cost 6 %, at 2^4 / 2^8 keys 20 %)
+      L.dict_group = (!q.dict_compact && q.front_replicas == 1 && 4 * (uint64_t)q.front_slots >= q.dict_slots &&
+                      (q.sig == SIG_SC || q.sig == SIG_SC32) && tun().dict_pairs) ? 2u : 1u;
       dict_keys = reinterpret_cast<uint32_t*>(take((size_t)q.cap * 4));
       uint32_t* dict_n = reinterpret_cast<uint32_t*>(take(256));
       dict_counts = dict_n;

@@ -93,6 +93,7 @@ struct AggLaunch {
   // FRONT_DICT: dictionary image (key, dense id) of dict_slots entries (a power of two), slot = (u * mul) >> dict_shift
   void* dict; uint32_t dict_slots, dict_shift;
   uint32_t dict_compact;    // FRONT_DICT: the large-dictionary shared-memory layout (aggregate.cu: AggArgs)
+  uint32_t dict_group;      // FRONT_DICT, small layout: 2 = entries are placed and searched in pairs (SUM + COUNT plans, one replica)
   uint32_t dict_pass_lg, dict_pass;   // FRONT_DICT, several passes: this launch aggregates key slice dict_pass of 2^dict_pass_lg
   // launch shape
   int threads, blocks;
