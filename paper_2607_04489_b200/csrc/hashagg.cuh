@@ -303,7 +303,9 @@ struct Front {
     int h0, h1;
     if constexpr (sizeof(U) == 8) {
       // measured: the branch-free first look pays for 64-bit keys (C3 -3 %, C4 -3.5 %) and costs
-      // 4-8 % for 32-bit keys, whose kernel is bound by shared-memory wavefronts, not issue slots
+      // 4-8 % for 32-bit keys in whole-input mode and 10-20 % in partition mode (measured again at the end of round 2:
+      // C5 2^16 / 2^20 / 2^24 aggregate 1.12 / 1.30 / 1.48 -> 1.23 / 1.54 / 1.77 ms), although ncu shows that kernel at 84 %
+      // of its issue slots: the four compares and selects per row cost more than the loop they bypass
       h0 = match_home(q0, u0, b0, ok0); h1 = match_home(q1, u1, b1, ok1);
       if ((ok0 && h0 < 0) || (ok1 && h1 < 0)) {
 #pragma unroll 1
