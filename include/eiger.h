@@ -72,7 +72,7 @@ typedef struct {
   double ndv_est;               /* the NDV estimate the tables were sized with (after clamping to min(n, range)) */
   int64_t kernel_launches;      /* kernels this call launched                                                     */
   int64_t spill_rows;           /* EIGER_GLOBAL: rows (padding included) that went through the spill buffer; else 0 */
-  int32_t dict_ids;             /* EIGER_SMEM through the dictionary front: ids the dictionary was planned for; else 0 */
+  int32_t dict_ids;             /* EIGER_SMEM through the dictionary front: ids each dictionary (one per pass) was planned for; else 0 */
   int32_t reserved;
 } eiger_call_info;
 
